@@ -1,0 +1,183 @@
+"""ctypes front-end of the fp64 CPU oracle (oracle/sph_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  It imports nothing from the
+CUDA package.  Argument marshalling only -- all arithmetic is in sph_oracle.c.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import numpy as np
+
+from .build import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build())
+        _lib.orc_w.restype = C.c_double
+        _lib.orc_w.argtypes = [C.c_double, C.c_double, C.c_int]
+        _lib.orc_gfac.restype = C.c_double
+        _lib.orc_gfac.argtypes = [C.c_double, C.c_double, C.c_int]
+        _lib.orc_kfac.restype = C.c_double
+        _lib.orc_kfac.argtypes = [C.c_double, C.c_double, C.c_int]
+        _lib.orc_neighbors.restype = C.c_int64
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def _d(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None else None
+
+
+def _dom(domain):
+    per = np.ascontiguousarray(list(domain.periodic)[:3] + [0] * (3 - len(domain.periodic)), dtype=np.int32)
+    lo = _d(list(domain.lo)[:3] + [0.0] * (3 - len(domain.lo)))
+    hi = _d(list(domain.hi)[:3] + [0.0] * (3 - len(domain.hi)))
+    # the C ABI carries lo/hi as binary32
+    lo = lo.astype(np.float32).astype(np.float64)
+    hi = hi.astype(np.float32).astype(np.float64)
+    return int(domain.dim), per, lo, hi
+
+
+def _par(params):
+    # the C ABI carries the scalars as binary32
+    vals = np.asarray(params.as_list(), dtype=np.float32).astype(np.float64)
+    return _d(list(vals) + [float(params.pressure_form)])
+
+
+def _par_raw(values, form=0):
+    """parameters given directly as 10 doubles (for finite differences in the scalars)"""
+    return _d(list(values) + [float(form)])
+
+
+def w(r, H, dim):
+    return lib().orc_w(float(r), float(H), int(dim))
+
+
+def gfac(r, H, dim):
+    return lib().orc_gfac(float(r), float(H), int(dim))
+
+
+def kfac(r, H, dim):
+    return lib().orc_kfac(float(r), float(H), int(dim))
+
+
+def num_threads():
+    return int(lib().orc_num_threads())
+
+
+def wrap32(domain, x):
+    dim, per, lo, hi = _dom(domain)
+    x = _d(x)
+    n = x.shape[0]
+    xw = np.empty_like(x)
+    bad = C.c_int64(0)
+    lib().orc_wrap32(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(x), _p(xw), C.byref(bad))
+    return xw, int(bad.value)
+
+
+def neighbors(domain, x, h, search_scale=1.0, method=0, prewrapped=False):
+    """CSR neighbour lists (row_ptr int64 [n+1], col_idx int32 [nnz], rows ascending, self included)
+    of the binary32 positions ``x``.  method 0 = brute force, 1 = oracle grid."""
+    dim, per, lo, hi = _dom(domain)
+    if prewrapped:
+        xw = _d(x)
+    else:
+        xw, _ = wrap32(domain, np.asarray(x, dtype=np.float32))
+    h = _d(np.asarray(h, dtype=np.float32))
+    n = xw.shape[0]
+    row_ptr = np.zeros(n + 1, dtype=np.int64)
+    args = [C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(xw), _p(h), C.c_double(float(np.float32(search_scale))),
+            C.c_int(method), _p(row_ptr)]
+    nnz = lib().orc_neighbors(*args, None)
+    if nnz < 0:
+        raise MemoryError("oracle neighbour search")
+    col = np.empty(max(int(nnz), 1), dtype=np.int32)
+    lib().orc_neighbors(*args, _p(col))
+    return row_ptr, col[:nnz]
+
+
+def density(domain, x, h, m, row_ptr, col_idx):
+    dim, per, lo, hi = _dom(domain)
+    x, h, m = _d(x), _d(h), _d(m)
+    n = x.shape[0]
+    rho = np.empty(n, dtype=np.float64)
+    lib().orc_density(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(x), _p(h), _p(m),
+                      _p(np.ascontiguousarray(row_ptr, np.int64)), _p(np.ascontiguousarray(col_idx, np.int32)), _p(rho))
+    return rho
+
+
+def rhs(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, rows=None, with_scales=False, par_raw=None):
+    dim, per, lo, hi = _dom(domain)
+    par = _par(params) if par_raw is None else par_raw
+    x, v, rho, m, h = _d(x), _d(v), _d(rho), _d(m), _d(h)
+    kind = np.ascontiguousarray(kind, dtype=np.uint8)
+    n = x.shape[0]
+    drho = np.zeros(n)
+    acc = np.zeros((n, dim))
+    sd = np.zeros(n) if with_scales else None
+    sa = np.zeros(n) if with_scales else None
+    rp = np.ascontiguousarray(row_ptr, np.int64)
+    ci = np.ascontiguousarray(col_idx, np.int32)
+    rows_a = None if rows is None else np.ascontiguousarray(rows, np.int64)
+    lib().orc_rhs(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(par), _p(x), _p(v), _p(rho), _p(m), _p(h),
+                  _p(kind), _p(rp), _p(ci), _p(rows_a), C.c_int64(0 if rows is None else len(rows_a)),
+                  _p(drho), _p(acc), _p(sd), _p(sa))
+    if with_scales:
+        return drho, acc, sd, sa
+    return drho, acc
+
+
+def rhs_vjp(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, drho_bar, acc_bar, rows=None, par_raw=None):
+    dim, per, lo, hi = _dom(domain)
+    par = _par(params) if par_raw is None else par_raw
+    x, v, rho, m, h = _d(x), _d(v), _d(rho), _d(m), _d(h)
+    lam, mu = _d(drho_bar), _d(acc_bar)
+    kind = np.ascontiguousarray(kind, dtype=np.uint8)
+    n = x.shape[0]
+    xb = np.zeros((n, dim))
+    vb = np.zeros((n, dim))
+    rb = np.zeros(n)
+    pb = np.zeros(10)
+    rp = np.ascontiguousarray(row_ptr, np.int64)
+    ci = np.ascontiguousarray(col_idx, np.int32)
+    rows_a = None if rows is None else np.ascontiguousarray(rows, np.int64)
+    lib().orc_rhs_vjp(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(par), _p(x), _p(v), _p(rho), _p(m), _p(h),
+                      _p(kind), _p(rp), _p(ci), _p(lam), _p(mu), _p(rows_a), C.c_int64(0 if rows is None else len(rows_a)),
+                      _p(xb), _p(vb), _p(rb), _p(pb))
+    return xb, vb, rb, pb
+
+
+def rk4_step(domain, params, dt, x, v, rho, m, h, kind, method=0, par_raw=None):
+    dim, per, lo, hi = _dom(domain)
+    par = _par(params) if par_raw is None else par_raw
+    x, v, rho = _d(x).copy(), _d(v).copy(), _d(rho).copy()
+    m, h = _d(m), _d(h)
+    kind = np.ascontiguousarray(kind, dtype=np.uint8)
+    n = x.shape[0]
+    lib().orc_rk4_step(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(par), C.c_double(dt),
+                       _p(x), _p(v), _p(rho), _p(m), _p(h), _p(kind), C.c_int(method))
+    return x, v, rho
+
+
+def rk4_step_vjp(domain, params, dt, x0, v0, rho0, m, h, kind, x_bar, v_bar, rho_bar, params_bar=None, method=0,
+                 par_raw=None):
+    dim, per, lo, hi = _dom(domain)
+    par = _par(params) if par_raw is None else par_raw
+    x0, v0, rho0, m, h = _d(x0), _d(v0), _d(rho0), _d(m), _d(h)
+    xb, vb, rb = _d(x_bar).copy(), _d(v_bar).copy(), _d(rho_bar).copy()
+    pb = np.zeros(10) if params_bar is None else _d(params_bar).copy()
+    kind = np.ascontiguousarray(kind, dtype=np.uint8)
+    n = x0.shape[0]
+    lib().orc_rk4_step_vjp(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(par), C.c_double(dt),
+                           _p(x0), _p(v0), _p(rho0), _p(m), _p(h), _p(kind), C.c_int(method),
+                           _p(xb), _p(vb), _p(rb), _p(pb))
+    return xb, vb, rb, pb

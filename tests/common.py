@@ -1,0 +1,31 @@
+"""Shared helpers for the tests: golden-file reader and the error metric of SURVEY.md 8c-9."""
+import os
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def golden(fname):
+    out = {}
+    with open(os.path.join(HERE, "golden", fname)) as f:
+        for line in f:
+            line = line.split("#", 1)[0].strip()
+            if not line:
+                continue
+            k, val = line.split()[:2]
+            out[k] = float(val)
+    return out
+
+
+def max_norm_err(y, yref, scale=None, floor_frac=1e-3):
+    """err = max_i |y_i - yref_i|_inf / max(max_i |yref_i|_inf, floor_frac * max_i scale_i).
+    On lattice configs the exact drho/dt is 0 and a has zero crossings, so an element-wise relative error
+    is undefined; ``scale`` is the oracle's per-row sum of |pair terms|."""
+    y = np.asarray(y, dtype=np.float64)
+    yref = np.asarray(yref, dtype=np.float64)
+    den = np.max(np.abs(yref)) if yref.size else 0.0
+    if scale is not None and np.size(scale):
+        den = max(den, floor_frac * float(np.max(scale)))
+    if den == 0.0:
+        den = 1.0
+    return float(np.max(np.abs(y - yref)) / den) if y.size else 0.0
