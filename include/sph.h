@@ -1,0 +1,148 @@
+/*
+ * sph.h -- C ABI of the B200-native delta-SPH right-hand side and adjoint
+ *          (data-parallel hot path of diffSPH, arXiv 2507.21684; text at PAPER.md).
+ *
+ * Conventions (apply to every call unless stated otherwise)
+ *   - All array arguments are DEVICE pointers owned by the caller (e.g. PyTorch tensors), contiguous:
+ *       x, v, acc, x_bar, v_bar, acc_bar : float [n][dim] row-major
+ *       rho, m, h, drho_dt, ...          : float [n]
+ *       kind                             : uint8 [n]   0 = fluid, 1 = fixed boundary particle
+ *     "h" is the SUPPORT RADIUS H of the kernel ("we chose to denote the support itself as h").
+ *   - Every call enqueues its work on `stream` and returns without synchronising, except
+ *     sph_neighbors / sph_rk_step / sph_rk_step_vjp / sph_check (they read nnz / the error flag back) and
+ *     the *_host convenience entry points.
+ *   - The context owns sorted copies, keys, cell tables, the CSR and scratch (grown on demand).
+ *     Outputs are always in the CALLER's particle order.
+ *   - Return value: 0 = SPH_OK, negative = error code below.  No exceptions, no aborts, no printing.
+ *   - There is no CPU fallback anywhere behind this interface.
+ *
+ * What is computed (readings R1..R9 are listed in DESIGN.md):
+ *   Wendland C4 kernel  W = C_d/H^d (1-q)_+^6 (1+6q+35/3 q^2), C_2 = 9/pi, C_3 = 495/(32 pi)
+ *   H_ij = max(h_i,h_j)  (BASELINE.json config 4),  smoothing scale l = H/kappa_d
+ *   N(i) = { j : |x_i - x_j|^2 < (search_scale*H_ij)^2 } with minimum image on periodic axes, self included
+ *   rho_i     = sum_j m_j W_ij                                                             PAPER.md:91 Eq.8
+ *   drho_i/dt = sum_j [ rho_i V_j (v_i-v_j).grad_i W_ij  +  2 delta l c0 V_j (rho_i-rho_j) r^2/(r^2+(eps H)^2) G ]
+ *                                                                     PAPER.md:95 Eq.9; Eq.42
+ *   a_i       = sum_j [ -m_j (p_i/rho_i^2 + p_j/rho_j^2) + eta rho0 V_j (v_ij.x_ij)/(rho_i (r^2+(eps H)^2)) ] grad_i W_ij + g
+ *               eta = alpha l c0 + 2(d+2) nu;   a_i = 0 for boundary kinds            PAPER.md:497 Eq.40; 87 Eq.7
+ *   p         = rho0 c0^2/gamma ((rho/rho0)^gamma - 1)                                     PAPER.md:112 Eq.12
+ *   with V_j = m_j/rho_j and grad_i W_ij = G (x_i - x_j).
+ */
+#ifndef SPH_B200_H
+#define SPH_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* opaque CUDA stream handle (binary compatible with cudaStream_t); NULL = the legacy default stream */
+typedef struct CUstream_st *sph_stream_t;
+
+typedef struct sph_ctx sph_ctx; /* opaque */
+
+/* Simulation box and cell grid.  PAPER.md:556 (cells of size c), PAPER.md:165 (periodic via modulo). */
+typedef struct {
+    int dim;          /* 2 or 3 */
+    int periodic[3];  /* per axis: 1 = periodic (positions wrapped into [lo,hi), minimum image), 0 = bounded */
+    float lo[3];      /* lower corner; bounded axes: every position must lie in [lo,hi) */
+    float hi[3];      /* upper corner */
+    float cell_size;  /* >= largest search radius search_scale*max(h).  Periodic axes use the edge
+                         L/floor(L/cell_size) (>= cell_size, at least 3 cells); bounded axes use cell_size. */
+} sph_domain;
+
+/* Global parameters ("global state dictionary C").  sph_rhs_vjp returns the gradient with
+ * respect to the first ten floats in this order: c0, rho0, gamma, delta, alpha, nu, eps, g[0], g[1], g[2]. */
+typedef struct {
+    float c0;     /* speed of sound, > 0 */
+    float rho0;   /* rest density, > 0 */
+    float gamma;  /* Tait exponent (7) */
+    float delta;  /* delta-SPH density diffusion coefficient PAPER.md:103 */
+    float alpha;  /* artificial viscosity */
+    float nu;     /* kinematic viscosity                     PAPER.md:83 Eq.6 */
+    float eps;    /* regularisation of 1/r^2 relative to H, > 0 */
+    float g[3];   /* body force (gravity) */
+    int pressure_form; /* 0 = symmetric Eq.40 (the only form of the CUDA path in this round; others: SPH_E_INVALID) */
+} sph_params;
+
+enum {
+    SPH_OK = 0,
+    SPH_E_INVALID = -1, /* null pointer, n <= 0, dim not 2/3, eps <= 0, c0/rho0 <= 0, unsupported option */
+    SPH_E_DOMAIN = -2,  /* cell_size < search radius, < 3 cells on a periodic axis, hi <= lo, too many cells,
+                           non-finite or out-of-box position on a bounded axis (detected on device, reported by
+                           the next synchronising call or sph_check) */
+    SPH_E_STATE = -3,   /* call order violated (neighbours before cells, RHS before neighbours, different n) */
+    SPH_E_NOMEM = -4,   /* device or host allocation failed */
+    SPH_E_CUDA = -5     /* a CUDA runtime call failed */
+};
+
+/* Create a context on CUDA device `device`.  n_max is a sizing hint (scratch grows on demand). */
+int sph_create(sph_ctx **out, int device, int64_t n_max);
+int sph_destroy(sph_ctx *ctx);
+
+/* Steps N1-N4 of SURVEY.md 8(a): wrap positions, Morton cell key, stable radix sort,
+ * reorder into sorted float4 SoA, cell start/end table.  x: [n][dim], h: [n].  Keeps n for later calls. */
+int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float *x, const float *h, int64_t n,
+                    sph_stream_t stream);
+
+/* Steps N5-N7 (count / exclusive scan / fill): compact CSR neighbour lists of the positions given
+ * to sph_build_cells, radius search_scale*max(h_i,h_j), search_scale >= 1 (a Verlet skin).
+ * Synchronises `stream`; *nnz_out (host pointer, may be NULL) receives the number of entries. */
+int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out, sph_stream_t stream);
+
+/* Copy the lists out in CALLER ids: row_ptr [n+1] int64, col_idx [nnz] int32, each row ascending, self included. */
+int sph_neighbors_export(sph_ctx *ctx, int64_t *row_ptr, int32_t *col_idx, sph_stream_t stream);
+
+/* rho_i = sum_{j in N(i)} m_j W(r_ij, max(h_i,h_j)) at the positions given to sph_build_cells.  PAPER.md:91 Eq.8 */
+int sph_density(sph_ctx *ctx, const float *m, float *rho_out, sph_stream_t stream);
+
+/* One right-hand-side evaluation (formulas at the top of this file) on the lists of the last sph_neighbors.
+ * x may differ from the build positions (RK stages) as long as the list is still a superset of the true
+ * neighbours: pairs with r >= H_ij contribute exactly 0 (kernel clamp).  h is the one given to sph_build_cells. */
+int sph_rhs(sph_ctx *ctx, const sph_params *par, const float *x, const float *v, const float *rho,
+            const float *m, const uint8_t *kind, float *drho_dt, float *acc, sph_stream_t stream);
+
+/* Reverse-mode adjoint of sph_rhs (pair terms recomputed; adjacency fixed):
+ * given drho_bar = dL/d(drho_dt) [n] and acc_bar = dL/d(acc) [n][dim], writes x_bar, v_bar [n][dim], rho_bar [n]
+ * and params_bar[10] (DEVICE pointer; order as in sph_params; may be NULL). */
+int sph_rhs_vjp(sph_ctx *ctx, const sph_params *par, const float *x, const float *v, const float *rho,
+                const float *m, const uint8_t *kind, const float *drho_bar, const float *acc_bar,
+                float *x_bar, float *v_bar, float *rho_bar, float *params_bar, sph_stream_t stream);
+
+/* One classic RK4 step of y = (x, v, rho), f = (v, a, drho/dt); boundary kinds keep x and v.
+ * Rebuilds cells and lists from x with search_scale = 1 + skin (skin >= 0; the caller guarantees
+ * skin*min(h) >= 2*dt*max|v| so that one list serves the four stages).  x, v, rho: in/out. */
+int sph_rk_step(sph_ctx *ctx, const sph_domain *dom, const sph_params *par, float dt, float skin, int64_t n,
+                float *x, float *v, float *rho, const float *m, const float *h, const uint8_t *kind,
+                sph_stream_t stream);
+
+/* Discrete adjoint of sph_rk_step (stages recomputed from the step's initial state):
+ * x0, v0, rho0_state = state at t; x_bar, v_bar, rho_bar hold dL/dy(t+dt) on entry and dL/dy(t) on return;
+ * params_bar[10] (device, may be NULL) is ACCUMULATED into. */
+int sph_rk_step_vjp(sph_ctx *ctx, const sph_domain *dom, const sph_params *par, float dt, float skin, int64_t n,
+                    const float *x0, const float *v0, const float *rho0_state, const float *m, const float *h,
+                    const uint8_t *kind, float *x_bar, float *v_bar, float *rho_bar, float *params_bar,
+                    sph_stream_t stream);
+
+/* End-to-end convenience call with HOST buffers (pageable or pinned): copies the inputs to the device, runs
+ * sph_build_cells + sph_neighbors(search_scale) + sph_rhs + sph_rhs_vjp, copies the seven outputs back and
+ * synchronises.  Output pointers may be NULL (skipped).  params_bar: host float[10]. */
+int sph_forward_backward_host(sph_ctx *ctx, const sph_domain *dom, const sph_params *par, float search_scale,
+                              int64_t n, const float *x, const float *v, const float *rho, const float *m,
+                              const float *h, const uint8_t *kind, const float *drho_bar, const float *acc_bar,
+                              float *drho_dt, float *acc, float *x_bar, float *v_bar, float *rho_bar,
+                              float *params_bar, int64_t *nnz_out);
+
+/* Fetch the device-side error flag (synchronises the context's last stream). */
+int sph_check(sph_ctx *ctx);
+const char *sph_strerror(int code);
+
+/* Introspection for tests / bench (host values of the last build): grid size per axis, nnz, number of kernels
+ * launched by this context since creation. */
+int sph_get_info(sph_ctx *ctx, int32_t ncell[3], int64_t *n, int64_t *nnz, int64_t *launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_B200_H */

@@ -1,0 +1,122 @@
+// sph_api.cu -- context life cycle, error reporting and the host-buffer end-to-end entry point of include/sph.h.
+#include "sph_internal.cuh"
+
+#include <new>
+
+extern "C" int sph_create(sph_ctx **out, int device, int64_t n_max)
+{
+    if (!out || n_max < 0) return SPH_E_INVALID;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) {
+        (void)cudaGetLastError();
+        return SPH_E_CUDA;                  // no CUDA device: there is no CPU fallback
+    }
+    SPH_CUDA_TRY(cudaSetDevice(device));
+    sph_ctx *ctx = new (std::nothrow) sph_ctx();
+    if (!ctx) return SPH_E_NOMEM;
+    ctx->device = device;
+    ctx->n_hint = n_max;
+    if (cudaMallocHost((void **)&ctx->h_pinned, 8 * sizeof(int64_t)) != cudaSuccess) {
+        (void)cudaGetLastError();
+        delete ctx;
+        return SPH_E_NOMEM;
+    }
+    *out = ctx;
+    return SPH_OK;
+}
+
+extern "C" int sph_destroy(sph_ctx *ctx)
+{
+    if (!ctx) return SPH_E_INVALID;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    DevBuf *bufs[] = {&ctx->key_a, &ctx->key_b, &ctx->idx_a, &ctx->idx_b, &ctx->hist, &ctx->perm, &ctx->inv_perm,
+                      &ctx->key_sorted, &ctx->pos_s, &ctx->cell_start, &ctx->cell_end, &ctx->stats, &ctx->cnt,
+                      &ctx->row_ptr, &ctx->col, &ctx->scan_tmp, &ctx->s0, &ctx->s1, &ctx->s2, &ctx->s3, &ctx->c0buf,
+                      &ctx->out4, &ctx->m_s, &ctx->kind_s, &ctx->partials, &ctx->eos, &ctx->hx, &ctx->hv, &ctx->hrho,
+                      &ctx->hm, &ctx->hh, &ctx->hkind, &ctx->hlam, &ctx->hmu, &ctx->ho_drho, &ctx->ho_acc, &ctx->ho_xb,
+                      &ctx->ho_vb, &ctx->ho_rb, &ctx->ho_pb};
+    for (DevBuf *b : bufs) b->release();
+    for (auto &b : ctx->rk) b.release();
+    if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
+    (void)cudaGetLastError();
+    delete ctx;
+    return SPH_OK;
+}
+
+extern "C" int sph_check(sph_ctx *ctx)
+{
+    if (!ctx) return SPH_E_INVALID;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    SPH_CUDA_TRY(cudaStreamSynchronize(ctx->last_stream));
+    if (!ctx->stats.p) return SPH_OK;
+    uint32_t flag = 0;
+    SPH_CUDA_TRY(cudaMemcpy(&flag, ctx->stats.p, 4, cudaMemcpyDeviceToHost));
+    return flag ? SPH_E_DOMAIN : SPH_OK;
+}
+
+extern "C" const char *sph_strerror(int code)
+{
+    switch (code) {
+    case SPH_OK: return "ok";
+    case SPH_E_INVALID: return "invalid argument";
+    case SPH_E_DOMAIN: return "domain error (cell size / periodic cells / position outside a bounded axis)";
+    case SPH_E_STATE: return "call order violated";
+    case SPH_E_NOMEM: return "out of memory";
+    case SPH_E_CUDA: return "CUDA runtime error (or no CUDA device: this library has no CPU fallback)";
+    default: return "unknown error";
+    }
+}
+
+extern "C" int sph_get_info(sph_ctx *ctx, int32_t ncell[3], int64_t *n, int64_t *nnz, int64_t *launches)
+{
+    if (!ctx) return SPH_E_INVALID;
+    if (ncell)
+        for (int k = 0; k < 3; ++k) ncell[k] = ctx->geom.ncell[k];
+    if (n) *n = ctx->n;
+    if (nnz) *nnz = ctx->lists_ready ? ctx->nnz : 0;
+    if (launches) *launches = ctx->launches;
+    return SPH_OK;
+}
+
+extern "C" int sph_forward_backward_host(sph_ctx *ctx, const sph_domain *dom, const sph_params *par, float search_scale,
+                                         int64_t n, const float *x, const float *v, const float *rho, const float *m,
+                                         const float *h, const uint8_t *kind, const float *drho_bar, const float *acc_bar,
+                                         float *drho_dt, float *acc, float *x_bar, float *v_bar, float *rho_bar,
+                                         float *params_bar, int64_t *nnz_out)
+{
+    if (!ctx || !dom || !par || n <= 0 || !x || !v || !rho || !m || !h || !kind || !drho_bar || !acc_bar) return SPH_E_INVALID;
+    if (dom->dim != 2 && dom->dim != 3) return SPH_E_INVALID;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = nullptr;
+    const size_t nv = (size_t)n * dom->dim * 4, ns = (size_t)n * 4;
+    SPH_TRY(ctx->hx.reserve(nv));  SPH_TRY(ctx->hv.reserve(nv));  SPH_TRY(ctx->hrho.reserve(ns));
+    SPH_TRY(ctx->hm.reserve(ns));  SPH_TRY(ctx->hh.reserve(ns));  SPH_TRY(ctx->hkind.reserve((size_t)n));
+    SPH_TRY(ctx->hlam.reserve(ns)); SPH_TRY(ctx->hmu.reserve(nv));
+    SPH_TRY(ctx->ho_drho.reserve(ns)); SPH_TRY(ctx->ho_acc.reserve(nv)); SPH_TRY(ctx->ho_xb.reserve(nv));
+    SPH_TRY(ctx->ho_vb.reserve(nv)); SPH_TRY(ctx->ho_rb.reserve(ns)); SPH_TRY(ctx->ho_pb.reserve(64));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hx.p, x, nv, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hv.p, v, nv, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hrho.p, rho, ns, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hm.p, m, ns, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hh.p, h, ns, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hkind.p, kind, (size_t)n, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hlam.p, drho_bar, ns, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hmu.p, acc_bar, nv, cudaMemcpyHostToDevice, st));
+    SPH_TRY(sph_build_cells(ctx, dom, ctx->hx.as<float>(), ctx->hh.as<float>(), n, (sph_stream_t)st));
+    SPH_TRY(sph_neighbors(ctx, search_scale, nnz_out, (sph_stream_t)st));
+    SPH_TRY(sph_rhs(ctx, par, ctx->hx.as<float>(), ctx->hv.as<float>(), ctx->hrho.as<float>(), ctx->hm.as<float>(),
+                    ctx->hkind.as<uint8_t>(), ctx->ho_drho.as<float>(), ctx->ho_acc.as<float>(), (sph_stream_t)st));
+    SPH_TRY(sph_rhs_vjp(ctx, par, ctx->hx.as<float>(), ctx->hv.as<float>(), ctx->hrho.as<float>(), ctx->hm.as<float>(),
+                        ctx->hkind.as<uint8_t>(), ctx->hlam.as<float>(), ctx->hmu.as<float>(), ctx->ho_xb.as<float>(),
+                        ctx->ho_vb.as<float>(), ctx->ho_rb.as<float>(), ctx->ho_pb.as<float>(), (sph_stream_t)st));
+    if (drho_dt) SPH_CUDA_TRY(cudaMemcpyAsync(drho_dt, ctx->ho_drho.p, ns, cudaMemcpyDeviceToHost, st));
+    if (acc) SPH_CUDA_TRY(cudaMemcpyAsync(acc, ctx->ho_acc.p, nv, cudaMemcpyDeviceToHost, st));
+    if (x_bar) SPH_CUDA_TRY(cudaMemcpyAsync(x_bar, ctx->ho_xb.p, nv, cudaMemcpyDeviceToHost, st));
+    if (v_bar) SPH_CUDA_TRY(cudaMemcpyAsync(v_bar, ctx->ho_vb.p, nv, cudaMemcpyDeviceToHost, st));
+    if (rho_bar) SPH_CUDA_TRY(cudaMemcpyAsync(rho_bar, ctx->ho_rb.p, ns, cudaMemcpyDeviceToHost, st));
+    if (params_bar) SPH_CUDA_TRY(cudaMemcpyAsync(params_bar, ctx->ho_pb.p, 40, cudaMemcpyDeviceToHost, st));
+    SPH_CUDA_TRY(cudaStreamSynchronize(st));
+    return SPH_OK;
+}

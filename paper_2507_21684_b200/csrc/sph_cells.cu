@@ -1,0 +1,373 @@
+// sph_cells.cu -- steps N1-N4 of SURVEY.md 8(a): wrap + Morton cell key, stable LSD radix sort,
+// reorder into sorted float4 SoA, cell start/end table; plus the device-wide exclusive scan used by N6.
+// Hand-written for sm_100a; no library sort/scan.  PAPER.md:556-560 (cells, compact map, space-filling curve).
+#include "sph_internal.cuh"
+
+#include <math.h>
+
+namespace {
+
+constexpr int kThreads = 256;
+
+// ------------------------------------------------------------------------------------------ N1
+// wrap (R4), cell coordinate (binary64, monotone), Morton key; error flag; min/max of h.
+// stats[0] = error bits (1: position outside a bounded axis or non-finite, 2: h non-finite or <= 0),
+// stats[1] = max h (float bits), stats[2] = min h (float bits)   -- integer atomics only.
+__global__ void k_wrap_key(const float *__restrict__ x, const float *__restrict__ h, int64_t n, GridGeom gg,
+                           uint32_t *__restrict__ key, uint32_t *__restrict__ stats)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t err = 0;
+    float hv = 0.f;
+    bool live = i < n;
+    if (live) {
+        int c[3] = {0, 0, 0};
+        for (int k = 0; k < gg.dim; ++k) {
+            float xv = x[i * gg.dim + k];
+            if (!isfinite(xv)) {
+                err |= 1u;
+                continue;
+            }
+            float w = xv;
+            if (gg.periodic[k])
+                w = wrap_coord(xv, gg.lo[k], gg.hi[k], gg.L[k]);
+            else if (xv < gg.lo[k] || xv >= gg.hi[k])
+                err |= 1u;
+            int cc = cell_coord_raw((double)w, gg.lo_d[k], gg.edge[k]);
+            cc = max(0, min(gg.ncell[k] - 1, cc));
+            c[k] = cc;
+        }
+        key[i] = morton_encode(gg.dim, c[0], c[1], c[2]);
+        hv = h[i];
+        if (!isfinite(hv) || !(hv > 0.f)) {
+            err |= 2u;
+            hv = 0.f;
+        }
+    }
+    // warp-aggregate the statistics, one atomic per warp
+    uint32_t hb = __float_as_uint(hv);
+    uint32_t hmaxb = __reduce_max_sync(0xffffffffu, hb);
+    uint32_t hminb = __reduce_min_sync(0xffffffffu, live && hv > 0.f ? hb : 0x7f7fffffu);
+    uint32_t e = __reduce_or_sync(0xffffffffu, err);
+    if ((threadIdx.x & 31) == 0) {
+        if (e) atomicOr(&stats[0], e);
+        atomicMax(&stats[1], hmaxb);
+        atomicMin(&stats[2], hminb);
+    }
+}
+
+// ------------------------------------------------------------------------------------------ N2
+// Stable LSD radix sort, 8-bit digits.  Each warp owns a contiguous chunk of kChunk keys and ranks them
+// round by round (32 keys per round) with __match_any_sync, so equal keys keep their input order.
+constexpr int kRsWarps = 8;
+constexpr int kRsItems = 16;
+constexpr int kChunk = 32 * kRsItems;
+
+__global__ void __launch_bounds__(kRsWarps * 32)
+k_radix_hist(const uint32_t *__restrict__ key, int64_t n, int shift, int64_t nchunks, uint32_t *__restrict__ hist)
+{
+    __shared__ uint32_t cnt[kRsWarps][256];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t chunk = (int64_t)blockIdx.x * kRsWarps + warp;
+    for (int d = lane; d < 256; d += 32) cnt[warp][d] = 0;
+    __syncwarp();
+    if (chunk < nchunks) {
+        const int64_t base = chunk * kChunk;
+        for (int r = 0; r < kRsItems; ++r) {
+            int64_t i = base + r * 32 + lane;
+            uint32_t d = i < n ? ((key[i] >> shift) & 255u) : 256u;
+            uint32_t peers = __match_any_sync(0xffffffffu, d);
+            if (d < 256u && (peers & ((1u << lane) - 1u)) == 0u) cnt[warp][d] += __popc(peers);
+            __syncwarp();
+        }
+        for (int d = lane; d < 256; d += 32) hist[(int64_t)d * nchunks + chunk] = cnt[warp][d];
+    }
+}
+
+__global__ void __launch_bounds__(kRsWarps * 32)
+k_radix_scatter(const uint32_t *__restrict__ key_in, const uint32_t *__restrict__ val_in,
+                uint32_t *__restrict__ key_out, uint32_t *__restrict__ val_out, int64_t n, int shift,
+                int64_t nchunks, const uint32_t *__restrict__ hist_scanned)
+{
+    __shared__ uint32_t off[kRsWarps][256];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t chunk = (int64_t)blockIdx.x * kRsWarps + warp;
+    if (chunk >= nchunks) return;
+    for (int d = lane; d < 256; d += 32) off[warp][d] = hist_scanned[(int64_t)d * nchunks + chunk];
+    __syncwarp();
+    const int64_t base = chunk * kChunk;
+    for (int r = 0; r < kRsItems; ++r) {
+        int64_t i = base + r * 32 + lane;
+        bool live = i < n;
+        uint32_t k = live ? key_in[i] : 0u;
+        uint32_t v = live ? (val_in ? val_in[i] : (uint32_t)i) : 0u;
+        uint32_t d = live ? ((k >> shift) & 255u) : 256u;
+        uint32_t peers = __match_any_sync(0xffffffffu, d);
+        uint32_t lower = peers & ((1u << lane) - 1u);
+        uint32_t pos = 0;
+        if (live) pos = off[warp][d] + __popc(lower);
+        __syncwarp();
+        if (live && lower == 0u) off[warp][d] += __popc(peers);
+        __syncwarp();
+        if (live) {
+            key_out[pos] = k;
+            val_out[pos] = v;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ scan
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 16;
+constexpr int kScanTile = kScanThreads * kScanItems;
+
+__device__ __forceinline__ unsigned long long block_exclusive_scan(unsigned long long v, unsigned long long *total)
+{
+    __shared__ unsigned long long wsum[kScanThreads / 32];
+    __shared__ unsigned long long tot;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned long long inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned long long t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        unsigned long long w = lane < kScanThreads / 32 ? wsum[lane] : 0ull;
+        unsigned long long winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            unsigned long long t = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += t;
+        }
+        if (lane < kScanThreads / 32) wsum[lane] = winc - w;
+        if (lane == kScanThreads / 32 - 1) tot = winc;
+    }
+    __syncthreads();
+    unsigned long long r = inc - v + wsum[warp];
+    *total = tot;
+    __syncthreads();
+    return r;
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_reduce(const uint32_t *__restrict__ in, int64_t m, unsigned long long *__restrict__ block_sums)
+{
+    const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
+    unsigned long long s = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k)
+        if (base + k < m) s += in[base + k];
+    unsigned long long tot;
+    block_exclusive_scan(s, &tot);
+    if (threadIdx.x == 0) block_sums[blockIdx.x] = tot;
+}
+
+// single block: exclusive scan of the block sums, sequential over tiles of kScanThreads with a carry
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_sums(unsigned long long *__restrict__ block_sums, int64_t nb)
+{
+    unsigned long long carry = 0;
+    for (int64_t base = 0; base < nb; base += kScanThreads) {
+        int64_t i = base + threadIdx.x;
+        unsigned long long v = i < nb ? block_sums[i] : 0ull;
+        unsigned long long tot;
+        unsigned long long ex = block_exclusive_scan(v, &tot);
+        if (i < nb) block_sums[i] = ex + carry;
+        carry += tot;
+    }
+}
+
+template <class OutT>
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_apply(const uint32_t *__restrict__ in, OutT *__restrict__ out, int64_t m,
+             const unsigned long long *__restrict__ block_sums, int write_total)
+{
+    const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
+    uint32_t v[kScanItems];
+    unsigned long long s = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        v[k] = base + k < m ? in[base + k] : 0u;
+        s += v[k];
+    }
+    unsigned long long tot;
+    unsigned long long ex = block_exclusive_scan(s, &tot) + block_sums[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        if (base + k < m) out[base + k] = (OutT)ex;
+        ex += v[k];
+    }
+    if (write_total && blockIdx.x == gridDim.x - 1 && threadIdx.x == kScanThreads - 1) out[m] = (OutT)ex;
+}
+
+// ------------------------------------------------------------------------------------------ N3 + N4
+// gather the caller's data into sorted order; mark cell boundaries (head flags of the sorted key run)
+__global__ void k_reorder(const float *__restrict__ x, const float *__restrict__ h, int64_t n, GridGeom gg,
+                          const uint32_t *__restrict__ key_sorted, const uint32_t *__restrict__ idx_sorted,
+                          uint32_t *__restrict__ perm, uint32_t *__restrict__ inv_perm, float4 *__restrict__ pos_s,
+                          uint32_t *__restrict__ cell_start, uint32_t *__restrict__ cell_end)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    uint32_t i = idx_sorted[p];
+    perm[p] = i;
+    inv_perm[i] = (uint32_t)p;
+    float w[3] = {0.f, 0.f, 0.f};
+    for (int k = 0; k < gg.dim; ++k) {
+        float xv = x[(int64_t)i * gg.dim + k];
+        w[k] = gg.periodic[k] && isfinite(xv) ? wrap_coord(xv, gg.lo[k], gg.hi[k], gg.L[k]) : xv;
+    }
+    pos_s[p] = make_float4(w[0], w[1], w[2], h[i]);
+    uint32_t kc = key_sorted[p];
+    int cx, cy, cz;
+    morton_decode(gg.dim, kc, cx, cy, cz);
+    int64_t lin = cx + (int64_t)gg.ncell[0] * (cy + (int64_t)gg.ncell[1] * cz);
+    if (p == 0 || key_sorted[p - 1] != kc) cell_start[lin] = (uint32_t)p;
+    if (p == n - 1 || key_sorted[p + 1] != kc) cell_end[lin] = (uint32_t)(p + 1);
+}
+
+int ceil_log2(int v)
+{
+    int b = 0;
+    while ((1 << b) < v) ++b;
+    return b;
+}
+
+} // namespace
+
+// exclusive scan of m uint32 values; out is uint32[m] or (out64) int64[m+1] with the total at out[m]
+int sph_scan_u32(sph_ctx *ctx, const uint32_t *in, void *out, bool out64, int64_t m, cudaStream_t st)
+{
+    if (m <= 0) return SPH_OK;
+    int64_t nb = (m + kScanTile - 1) / kScanTile;
+    SPH_TRY(ctx->scan_tmp.reserve((size_t)nb * sizeof(unsigned long long)));
+    auto *sums = ctx->scan_tmp.as<unsigned long long>();
+    k_scan_reduce<<<(unsigned)nb, kScanThreads, 0, st>>>(in, m, sums);
+    k_scan_sums<<<1, kScanThreads, 0, st>>>(sums, nb);
+    if (out64)
+        k_scan_apply<long long><<<(unsigned)nb, kScanThreads, 0, st>>>(in, (long long *)out, m, sums, 1);
+    else
+        k_scan_apply<uint32_t><<<(unsigned)nb, kScanThreads, 0, st>>>(in, (uint32_t *)out, m, sums, 0);
+    ctx->launches += 3;
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+static int make_geom(const sph_domain *dom, GridGeom *gg, int64_t *ncells_total)
+{
+    if (dom->dim != 2 && dom->dim != 3) return SPH_E_INVALID;
+    if (!(dom->cell_size > 0.f) || !isfinite(dom->cell_size)) return SPH_E_DOMAIN;
+    memset(gg, 0, sizeof(*gg));
+    gg->dim = dom->dim;
+    int maxnc = 1;
+    int64_t tot = 1;
+    for (int k = 0; k < 3; ++k) {
+        gg->ncell[k] = 1;
+        gg->edge[k] = 1.0;
+    }
+    for (int k = 0; k < dom->dim; ++k) {
+        gg->periodic[k] = dom->periodic[k] ? 1 : 0;
+        gg->lo[k] = dom->lo[k];
+        gg->hi[k] = dom->hi[k];
+        volatile float L = dom->hi[k] - dom->lo[k];
+        if (!(L > 0.f) || !isfinite(L)) return SPH_E_DOMAIN;
+        gg->L[k] = L;
+        gg->L_d[k] = (double)L;
+        gg->lo_d[k] = (double)dom->lo[k];
+        double ratio = (double)L / (double)dom->cell_size;
+        int limit = dom->dim == 3 ? 1023 : 65535;
+        if (gg->periodic[k]) {
+            double f = floor(ratio);
+            if (f < 3.0) return SPH_E_DOMAIN;
+            if (f > limit) return SPH_E_DOMAIN;
+            gg->ncell[k] = (int)f;
+            gg->edge[k] = (double)L / f;
+        } else {
+            double c = ceil(ratio);
+            if (c < 1.0) c = 1.0;
+            if (c > limit) return SPH_E_DOMAIN;
+            gg->ncell[k] = (int)c;
+            gg->edge[k] = (double)dom->cell_size;
+        }
+        if (gg->ncell[k] > maxnc) maxnc = gg->ncell[k];
+        tot *= gg->ncell[k];
+    }
+    if (tot > ((int64_t)1 << 28)) return SPH_E_DOMAIN;
+    gg->bits = ceil_log2(maxnc);
+    if (gg->bits < 1) gg->bits = 1;
+    *ncells_total = tot;
+    return SPH_OK;
+}
+
+extern "C" int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float *x, const float *h, int64_t n,
+                               sph_stream_t stream)
+{
+    if (!ctx || !dom || !x || !h || n <= 0 || n >= ((int64_t)1 << 31)) return SPH_E_INVALID;
+    ctx->cells_ready = false;
+    ctx->lists_ready = false;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    GridGeom gg;
+    int64_t ncells;
+    SPH_TRY(make_geom(dom, &gg, &ncells));
+    ctx->geom = gg;
+    ctx->ncells_total = ncells;
+    ctx->n = n;
+    ctx->last_stream = st;
+
+    const int64_t nchunks = (n + kChunk - 1) / kChunk;
+    SPH_TRY(ctx->key_a.reserve((size_t)n * 4));
+    SPH_TRY(ctx->key_b.reserve((size_t)n * 4));
+    SPH_TRY(ctx->idx_a.reserve((size_t)n * 4));
+    SPH_TRY(ctx->idx_b.reserve((size_t)n * 4));
+    SPH_TRY(ctx->hist.reserve((size_t)nchunks * 256 * 4));
+    SPH_TRY(ctx->perm.reserve((size_t)n * 4));
+    SPH_TRY(ctx->inv_perm.reserve((size_t)n * 4));
+    SPH_TRY(ctx->pos_s.reserve((size_t)n * 16));
+    SPH_TRY(ctx->cell_start.reserve((size_t)ncells * 4));
+    SPH_TRY(ctx->cell_end.reserve((size_t)ncells * 4));
+    SPH_TRY(ctx->stats.reserve(64));
+
+    const uint32_t init_stats[4] = {0u, 0u, 0x7f7fffffu, 0u};
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->stats.p, init_stats, sizeof(init_stats), cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemsetAsync(ctx->cell_start.p, 0, (size_t)ncells * 4, st));
+    SPH_CUDA_TRY(cudaMemsetAsync(ctx->cell_end.p, 0, (size_t)ncells * 4, st));
+
+    const unsigned nblk = (unsigned)((n + kThreads - 1) / kThreads);
+    k_wrap_key<<<nblk, kThreads, 0, st>>>(x, h, n, gg, ctx->key_a.as<uint32_t>(), ctx->stats.as<uint32_t>());
+    ctx->launches += 1;
+
+    // LSD radix passes over the used key bits
+    const int keybits = gg.bits * gg.dim;
+    const int passes = (keybits + 7) / 8;
+    uint32_t *kin = ctx->key_a.as<uint32_t>(), *kout = ctx->key_b.as<uint32_t>();
+    uint32_t *vin = nullptr, *vout = ctx->idx_b.as<uint32_t>();
+    uint32_t *vother = ctx->idx_a.as<uint32_t>();
+    const unsigned rblk = (unsigned)((nchunks + kRsWarps - 1) / kRsWarps);
+    for (int p = 0; p < passes; ++p) {
+        k_radix_hist<<<rblk, kRsWarps * 32, 0, st>>>(kin, n, 8 * p, nchunks, ctx->hist.as<uint32_t>());
+        ctx->launches += 1;
+        SPH_TRY(sph_scan_u32(ctx, ctx->hist.as<uint32_t>(), ctx->hist.p, false, nchunks * 256, st));
+        k_radix_scatter<<<rblk, kRsWarps * 32, 0, st>>>(kin, vin, kout, vout, n, 8 * p, nchunks, ctx->hist.as<uint32_t>());
+        ctx->launches += 1;
+        uint32_t *t = kin;
+        kin = kout;
+        kout = t;
+        uint32_t *nv = vin ? vin : vother;
+        vin = vout;
+        vout = nv;
+    }
+    // kin / vin now hold the sorted keys and the sorted caller indices
+    SPH_TRY(ctx->key_sorted.reserve((size_t)n * 4));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->key_sorted.p, kin, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
+    k_reorder<<<nblk, kThreads, 0, st>>>(x, h, n, gg, ctx->key_sorted.as<uint32_t>(), vin, ctx->perm.as<uint32_t>(),
+                                         ctx->inv_perm.as<uint32_t>(), ctx->pos_s.as<float4>(),
+                                         ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>());
+    ctx->launches += 1;
+    SPH_CUDA_TRY(cudaGetLastError());
+    ctx->cells_ready = true;
+    return SPH_OK;
+}

@@ -1,0 +1,211 @@
+// sph_internal.cuh -- context, scratch arena and small device helpers shared by the sm_100a kernels.
+// Product code (CUDA path).  Shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string.h>
+
+#include "../../include/sph.h"
+
+#define SPH_CUDA_TRY(expr)                                   \
+    do {                                                     \
+        cudaError_t e__ = (expr);                            \
+        if (e__ != cudaSuccess) {                            \
+            (void)cudaGetLastError();                        \
+            return e__ == cudaErrorMemoryAllocation ? SPH_E_NOMEM : SPH_E_CUDA; \
+        }                                                    \
+    } while (0)
+
+#define SPH_TRY(expr)               \
+    do {                            \
+        int r__ = (expr);           \
+        if (r__ != SPH_OK) return r__; \
+    } while (0)
+
+// One device buffer that only ever grows.
+struct DevBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+    int reserve(size_t bytes)
+    {
+        if (bytes <= cap) return SPH_OK;
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+        size_t want = bytes + bytes / 16 + 256;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e != cudaSuccess) {
+            (void)cudaGetLastError();
+            p = nullptr;
+            return SPH_E_NOMEM;
+        }
+        cap = want;
+        return SPH_OK;
+    }
+    void release()
+    {
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+    }
+    template <class T> T *as() const { return reinterpret_cast<T *>(p); }
+};
+
+// Geometry of the cell grid as the kernels see it (passed by value).
+struct GridGeom {
+    int dim;
+    int periodic[3];
+    int ncell[3];
+    int bits;          // Morton bits per axis
+    float lo[3], hi[3];
+    float L[3];        // binary32 hi - lo (the one L of the readings R3/R4)
+    double lo_d[3];
+    double edge[3];    // cell edge per axis (binary64)
+    double L_d[3];
+};
+
+// Per-launch physical constants (derived once on the host from sph_params).
+struct KPar {
+    int dim;
+    int periodic[3];
+    float L[3], halfL[3], lo[3], hi[3];
+    float c0, rho0, gamma, delta, alpha, nu, eps;
+    float g[3];
+    float Cd;       // kernel normalisation C_d
+    float inv_kappa; // 1/kappa_d
+    float visc_nu;  // 2(d+2) nu
+    float Bp;       // rho0 c0^2 / gamma
+    int uniform_h;  // all h equal (then the H-dependent constants below are valid)
+    float H, invH, cW, cG, cK, ell, e2, eta, kd;
+};
+
+struct sph_ctx {
+    int device = 0;
+    int64_t n_hint = 0;
+    int64_t n = 0;
+    bool cells_ready = false, lists_ready = false;
+    GridGeom geom{};
+    int64_t ncells_total = 0;
+    float search_scale = 1.f;
+    int64_t nnz = 0;
+    int64_t launches = 0;
+    cudaStream_t last_stream = nullptr;
+    float hmin = 0.f, hmax = 0.f;
+
+    // cells / sort
+    DevBuf key_a, key_b, idx_a, idx_b, hist;
+    DevBuf perm, inv_perm;      // sorted -> caller, caller -> sorted
+    DevBuf key_sorted;          // alias target of the last sort pass (copy)
+    DevBuf pos_s;               // float4 {xw,yw,zw,h} at build time, sorted
+    DevBuf cell_start, cell_end;
+    DevBuf stats;               // device: [0] err flag, [1] hmax bits, [2] hmin bits
+    // lists
+    DevBuf cnt, row_ptr, col, scan_tmp;
+    // pair scratch (sorted SoA)
+    DevBuf s0, s1, s2, s3, c0buf, out4, m_s, kind_s, partials, eos;
+    // rk scratch
+    DevBuf rk[16];
+    // pinned host mirror
+    int64_t *h_pinned = nullptr; // [8]
+    // host staging for *_host call
+    DevBuf hx, hv, hrho, hm, hh, hkind, hlam, hmu, ho_drho, ho_acc, ho_xb, ho_vb, ho_rb, ho_pb;
+};
+
+// ------------------------------------------------------------------------------------------
+// device helpers
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ float fast_sqrt(float x)
+{
+    float r;
+    asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float fast_rcp(float x)
+{
+    float r;
+    asm("rcp.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// 10-bit-per-axis (3D) / 16-bit-per-axis (2D) Morton interleave
+__device__ __forceinline__ uint32_t spread3(uint32_t v)
+{
+    v &= 0x3ffu;
+    v = (v | (v << 16)) & 0x030000ffu;
+    v = (v | (v << 8)) & 0x0300f00fu;
+    v = (v | (v << 4)) & 0x030c30c3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+__device__ __forceinline__ uint32_t compact3(uint32_t v)
+{
+    v &= 0x09249249u;
+    v = (v | (v >> 2)) & 0x030c30c3u;
+    v = (v | (v >> 4)) & 0x0300f00fu;
+    v = (v | (v >> 8)) & 0x030000ffu;
+    v = (v | (v >> 16)) & 0x3ffu;
+    return v;
+}
+__device__ __forceinline__ uint32_t spread2(uint32_t v)
+{
+    v &= 0xffffu;
+    v = (v | (v << 8)) & 0x00ff00ffu;
+    v = (v | (v << 4)) & 0x0f0f0f0fu;
+    v = (v | (v << 2)) & 0x33333333u;
+    v = (v | (v << 1)) & 0x55555555u;
+    return v;
+}
+__device__ __forceinline__ uint32_t compact2(uint32_t v)
+{
+    v &= 0x55555555u;
+    v = (v | (v >> 1)) & 0x33333333u;
+    v = (v | (v >> 2)) & 0x0f0f0f0fu;
+    v = (v | (v >> 4)) & 0x00ff00ffu;
+    v = (v | (v >> 8)) & 0xffffu;
+    return v;
+}
+__device__ __forceinline__ uint32_t morton_encode(int dim, int cx, int cy, int cz)
+{
+    return dim == 3 ? (spread3(cx) | (spread3(cy) << 1) | (spread3(cz) << 2)) : (spread2(cx) | (spread2(cy) << 1));
+}
+__device__ __forceinline__ void morton_decode(int dim, uint32_t key, int &cx, int &cy, int &cz)
+{
+    if (dim == 3) {
+        cx = (int)compact3(key);
+        cy = (int)compact3(key >> 1);
+        cz = (int)compact3(key >> 2);
+    } else {
+        cx = (int)compact2(key);
+        cy = (int)compact2(key >> 1);
+        cz = 0;
+    }
+}
+
+// R4: binary32, every operation rounded separately, no contraction.
+__device__ __forceinline__ float wrap_coord(float x, float lo, float hi, float L)
+{
+    float a = __fsub_rn(x, lo);
+    float t = __fdiv_rn(a, L);
+    float f = floorf(t);
+    float p = __fmul_rn(L, f);
+    float w = __fsub_rn(x, p);
+    if (w >= hi) w = __fsub_rn(w, L);
+    if (w < lo) w = __fadd_rn(w, L);
+    return w;
+}
+
+// cell coordinate of a (possibly out-of-box) coordinate: monotone in x (binary64 sub, div, floor)
+__device__ __forceinline__ int cell_coord_raw(double x, double lo, double edge)
+{
+    return (int)floor(__ddiv_rn(__dsub_rn(x, lo), edge));
+}
+
+// host-side launch helpers implemented in the .cu files
+int sph_scan_u32(sph_ctx *ctx, const uint32_t *in, void *out, bool out64, int64_t m, cudaStream_t st);
+int sph_kpar_make(const sph_ctx *ctx, const sph_params *par, KPar *kp);
+int sph_launch_rhs_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
+                          const uint8_t *kind_s, float *drho, float *acc, float4 *out4, cudaStream_t st);
+int sph_launch_vjp_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
+                          const float4 *cot, const float4 *eos, float *xb, float *vb, float *rb, float4 *xb4,
+                          float4 *vb4, float *params_bar, int accumulate_params, cudaStream_t st);

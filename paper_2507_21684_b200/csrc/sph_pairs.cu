@@ -1,0 +1,666 @@
+// sph_pairs.cu -- the pair-sum kernels: D (density), R0 (EOS prologue / pack), R1 (RHS), B1 (VJP), B2 (parameter
+// reduction) of SURVEY.md 8(a).  Gather formulation: a group of GS lanes owns a row, strides over the row's CSR
+// entries (coalesced index reads), gathers the neighbour's sorted float4 state, and reduces with shuffles.
+// No float atomics anywhere; every sum has a fixed order for a given launch configuration.
+//
+// Formulas: include/sph.h header comment and DESIGN.md section 2 (Eq.8, 9, 12, 40, 42, 7).
+#include "sph_internal.cuh"
+
+#include <math.h>
+
+namespace {
+
+constexpr int kBlock = 256;          // threads per block
+constexpr int kRowsPerGroup = 8;     // rows each lane group walks through
+
+// H-dependent constants of one pair (or of the whole launch when h is uniform)
+struct HC {
+    float invH, cW, cG, cK, ell, e2, eta, kd, H2;
+};
+
+template <int DIM>
+__device__ __forceinline__ HC hc_make(float H, const KPar &kp)
+{
+    HC c;
+    c.invH = 1.0f / H;
+    float i2 = c.invH * c.invH;
+    float iD = DIM == 2 ? i2 : i2 * c.invH;             // H^-d
+    c.cW = kp.Cd * iD;
+    c.cG = -(56.0f / 3.0f) * kp.Cd * iD * i2;           // G = cG (1+5q)(1-q)^5
+    c.cK = 560.0f * kp.Cd * iD * i2 * i2;               // K = cK (1-q)^4
+    c.ell = H * kp.inv_kappa;
+    float eh = kp.eps * H;
+    c.e2 = eh * eh;
+    c.eta = kp.alpha * c.ell * kp.c0 + kp.visc_nu;
+    c.kd = 2.0f * kp.delta * c.ell * kp.c0;
+    c.H2 = H * H;
+    return c;
+}
+template <int DIM>
+__device__ __forceinline__ HC hc_uniform(const KPar &kp)
+{
+    HC c;
+    c.invH = kp.invH; c.cW = kp.cW; c.cG = kp.cG; c.cK = kp.cK; c.ell = kp.ell; c.e2 = kp.e2; c.eta = kp.eta;
+    c.kd = kp.kd; c.H2 = kp.H * kp.H;
+    return c;
+}
+
+// sorted state of one particle as the pair loops see it
+struct Part {
+    float x[3], v[3], rho, V, P, h;
+};
+
+// layouts: DIM 3: s0 = {x,y,z,h} s1 = {vx,vy,vz,rho} s2(float2) = {V,P};  DIM 2: s0 = {x,y,vx,vy} s1 = {rho,V,P,h}
+template <int DIM>
+__device__ __forceinline__ Part load_part(const float4 *__restrict__ s0, const float4 *__restrict__ s1,
+                                          const float2 *__restrict__ s2, int64_t j)
+{
+    Part p;
+    float4 a = __ldg(s0 + j), b = __ldg(s1 + j);
+    if (DIM == 3) {
+        float2 c = __ldg(s2 + j);
+        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.h = a.w;
+        p.v[0] = b.x; p.v[1] = b.y; p.v[2] = b.z; p.rho = b.w;
+        p.V = c.x; p.P = c.y;
+    } else {
+        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = 0.f; p.v[0] = a.z; p.v[1] = a.w; p.v[2] = 0.f;
+        p.rho = b.x; p.V = b.y; p.P = b.z; p.h = b.w;
+    }
+    return p;
+}
+
+template <int DIM, bool WRAP>
+__device__ __forceinline__ void rel_pos(const float *xi, const float *xj, const KPar &kp, float *d, float &r2)
+{
+    r2 = 0.f;
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+        float dk = xi[k] - xj[k];
+        if (WRAP && kp.periodic[k]) dk = dk > kp.halfL[k] ? dk - kp.L[k] : (dk < -kp.halfL[k] ? dk + kp.L[k] : dk);
+        d[k] = dk;
+        r2 = fmaf(dk, dk, r2);
+    }
+    if (DIM == 2) d[2] = 0.f;
+}
+
+// does this row need the minimum-image test?  (only rows within `margin` of a periodic face can see the seam)
+__device__ __forceinline__ bool row_near_seam(const float *xi, const KPar &kp, float margin)
+{
+    bool s = false;
+    for (int k = 0; k < kp.dim; ++k)
+        if (kp.periodic[k]) s = s || (xi[k] - kp.lo[k] < margin) || (kp.hi[k] - xi[k] < margin);
+    return s;
+}
+
+template <int GS>
+__device__ __forceinline__ float group_sum(float v)
+{
+#pragma unroll
+    for (int o = GS / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------ R0: pack + EOS
+// Gathers the caller's arrays into the sorted SoA, wraps positions (R4), evaluates the Tait EOS (PAPER.md:112
+// Eq.12) as p = B expm1(gamma log1p((rho-rho0)/rho0)) so that small compressions keep full relative accuracy.
+template <int DIM>
+__global__ void k_pack_state(int64_t n, KPar kp, const uint32_t *__restrict__ perm, const float4 *__restrict__ pos_s,
+                             const float *__restrict__ x, const float *__restrict__ v, const float *__restrict__ rho,
+                             const float *__restrict__ m, const uint8_t *__restrict__ kind,
+                             float4 *__restrict__ s0, float4 *__restrict__ s1, float2 *__restrict__ s2,
+                             float4 *__restrict__ eos, uint8_t *__restrict__ kind_s)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const int64_t i = perm[p];
+    float xw[3] = {0.f, 0.f, 0.f}, vv[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+        float xv = x[i * DIM + k];
+        xw[k] = kp.periodic[k] ? wrap_coord(xv, kp.lo[k], kp.hi[k], kp.L[k]) : xv;
+        vv[k] = v[i * DIM + k];
+    }
+    const float r = rho[i], mi = m[i], h = pos_s[p].w;
+    const float u = (r - kp.rho0) / kp.rho0;
+    const float lg = log1pf(u);
+    const float ugm1 = expm1f(kp.gamma * lg);        // (rho/rho0)^gamma - 1
+    const float ug = ugm1 + 1.0f;
+    const float pr = kp.Bp * ugm1;                    // Tait pressure
+    const float ir = 1.0f / r, ir2 = ir * ir;
+    const float V = mi * ir, P = pr * ir2;
+    if (DIM == 3) {
+        s0[p] = make_float4(xw[0], xw[1], xw[2], h);
+        s1[p] = make_float4(vv[0], vv[1], vv[2], r);
+        s2[p] = make_float2(V, P);
+    } else {
+        s0[p] = make_float4(xw[0], xw[1], vv[0], vv[1]);
+        s1[p] = make_float4(r, V, P, h);
+    }
+    if (eos) {
+        // derivatives of P = p/rho^2 needed by the adjoint of the EOS prologue
+        const float dp_drho = kp.c0 * kp.c0 * ug / (1.0f + u);                     // c0^2 (rho/rho0)^(gamma-1)
+        const float dP = dp_drho * ir2 - 2.0f * pr * ir2 * ir;
+        const float dp_drho0 = kp.c0 * kp.c0 / kp.gamma * ugm1 - kp.c0 * kp.c0 * ug;
+        const float dp_dgam = -kp.Bp / kp.gamma * ugm1 + kp.Bp * ug * lg;
+        eos[p] = make_float4(dP, dp_drho0 * ir2, dp_dgam * ir2, mi);
+    }
+    kind_s[p] = kind[i];
+}
+
+__global__ void k_pack_cot(int64_t n, int dim, const uint32_t *__restrict__ perm, const uint8_t *__restrict__ kind_s,
+                           const float *__restrict__ lam, const float *__restrict__ mu, float4 *__restrict__ cot)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const int64_t i = perm[p];
+    float m0 = mu[i * dim], m1 = mu[i * dim + 1], m2 = dim == 3 ? mu[i * dim + 2] : 0.f;
+    if (kind_s[p]) m0 = m1 = m2 = 0.f;                 // a_i = 0 for boundary kinds => mu_i has no effect
+    cot[p] = make_float4(lam[i], m0, m1, m2);
+}
+
+__global__ void k_gather_f32(int64_t n, const uint32_t *__restrict__ perm, const float *__restrict__ in,
+                             float *__restrict__ out)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n) out[p] = in[perm[p]];
+}
+
+// ------------------------------------------------------------------------------------------ D: density
+template <int DIM, int GS, bool VARH>
+__global__ void __launch_bounds__(kBlock)
+k_density(int64_t n, KPar kp, float margin, const float4 *__restrict__ pos_s, const float *__restrict__ m_s,
+          const long long *__restrict__ row_ptr, const int32_t *__restrict__ col, const uint32_t *__restrict__ perm,
+          float *__restrict__ rho_out)
+{
+    constexpr int kGroups = kBlock / GS;
+    const int g = threadIdx.x / GS, gl = threadIdx.x % GS;
+    const int64_t row0 = (int64_t)blockIdx.x * kGroups * kRowsPerGroup;
+    const HC hu = hc_uniform<DIM>(kp);
+    for (int rr = 0; rr < kRowsPerGroup; ++rr) {
+        const int64_t row = row0 + (int64_t)rr * kGroups + g;
+        if (row >= n) break;
+        const float4 pi = __ldg(pos_s + row);
+        const float xi[3] = {pi.x, pi.y, pi.z};
+        const bool seam = row_near_seam(xi, kp, margin);
+        const long long b = row_ptr[row], e = row_ptr[row + 1];
+        float acc = 0.f;
+        for (long long p = b + gl; p < e; p += GS) {
+            const int32_t j = __ldg(col + p);
+            const float4 pj = __ldg(pos_s + j);
+            const float xj[3] = {pj.x, pj.y, pj.z};
+            float d[3], r2;
+            if (seam) rel_pos<DIM, true>(xi, xj, kp, d, r2); else rel_pos<DIM, false>(xi, xj, kp, d, r2);
+            HC hc = hu;
+            if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+            const float q = fast_sqrt(r2) * hc.invH;
+            const float t = fmaxf(1.0f - q, 0.f);
+            const float t2 = t * t, t6 = t2 * t2 * t2;
+            const float w = hc.cW * t6 * fmaf(q, fmaf(q, 35.0f / 3.0f, 6.0f), 1.0f);   // Eq.25/27
+            acc = fmaf(__ldg(m_s + j), w, acc);
+        }
+        acc = group_sum<GS>(acc);
+        if (gl == 0) rho_out[perm[row]] = acc;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ R1: RHS
+// OUT_SORTED: write float4 {a, drho/dt} in sorted order (RK stages); else scatter to the caller's arrays.
+template <int DIM, int GS, bool VARH, bool OUT_SORTED>
+__global__ void __launch_bounds__(kBlock)
+k_rhs(int64_t n, KPar kp, float margin, const float4 *__restrict__ s0, const float4 *__restrict__ s1,
+      const float2 *__restrict__ s2, const uint8_t *__restrict__ kind_s, const long long *__restrict__ row_ptr,
+      const int32_t *__restrict__ col, const uint32_t *__restrict__ perm, float *__restrict__ drho_out,
+      float *__restrict__ acc_out, float4 *__restrict__ out4)
+{
+    constexpr int kGroups = kBlock / GS;
+    const int g = threadIdx.x / GS, gl = threadIdx.x % GS;
+    const int64_t row0 = (int64_t)blockIdx.x * kGroups * kRowsPerGroup;
+    const HC hu = hc_uniform<DIM>(kp);
+    for (int rr = 0; rr < kRowsPerGroup; ++rr) {
+        const int64_t row = row0 + (int64_t)rr * kGroups + g;
+        if (row >= n) break;
+        const Part pi = load_part<DIM>(s0, s1, s2, row);
+        const bool seam = row_near_seam(pi.x, kp, margin);
+        const long long b = row_ptr[row], e = row_ptr[row + 1];
+        const float visc_i = kp.rho0 / pi.rho;            // rho0/rho_i of the viscous term
+        float sA = 0.f, sD = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f;
+        for (long long p = b + gl; p < e; p += GS) {
+            const int32_t j = __ldg(col + p);
+            const Part pj = load_part<DIM>(s0, s1, s2, j);
+            float d[3], r2;
+            if (seam) rel_pos<DIM, true>(pi.x, pj.x, kp, d, r2); else rel_pos<DIM, false>(pi.x, pj.x, kp, d, r2);
+            HC hc = hu;
+            if (VARH) hc = hc_make<DIM>(fmaxf(pi.h, pj.h), kp);
+            const float q = fast_sqrt(r2) * hc.invH;
+            const float t = fmaxf(1.0f - q, 0.f);          // kernel clamp: skin pairs contribute exactly 0
+            const float t2 = t * t, t4 = t2 * t2;
+            const float G = hc.cG * fmaf(5.0f, q, 1.0f) * (t4 * t);
+            float s = (pi.v[0] - pj.v[0]) * d[0];
+            s = fmaf(pi.v[1] - pj.v[1], d[1], s);
+            if (DIM == 3) s = fmaf(pi.v[2] - pj.v[2], d[2], s);
+            const float invR = fast_rcp(r2 + hc.e2);
+            const float VG = pj.V * G;
+            // continuity (Eq.9, physical sign) and delta-term (Brookshaw Laplacian of rho)
+            sA = fmaf(VG, s, sA);
+            const float dterm = VG * (pi.rho - pj.rho) * (r2 * invR);
+            sD = VARH ? fmaf(hc.kd, dterm, sD) : sD + dterm;
+            // pressure (Eq.40, symmetric) + viscosity (Eq.7 with the delta-SPH Pi_ij)
+            const float E = -(pj.V * pj.rho) * (pi.P + pj.P);
+            const float Phi = hc.eta * visc_i * pj.V * s * invR;
+            const float cf = (E + Phi) * G;
+            a0 = fmaf(cf, d[0], a0);
+            a1 = fmaf(cf, d[1], a1);
+            if (DIM == 3) a2 = fmaf(cf, d[2], a2);
+        }
+        float dr = pi.rho * sA + (VARH ? sD : hu.kd * sD);
+        dr = group_sum<GS>(dr);
+        a0 = group_sum<GS>(a0);
+        a1 = group_sum<GS>(a1);
+        if (DIM == 3) a2 = group_sum<GS>(a2);
+        if (gl == 0) {
+            const bool fixed = kind_s[row] != 0;
+            a0 = fixed ? 0.f : a0 + kp.g[0];
+            a1 = fixed ? 0.f : a1 + kp.g[1];
+            a2 = fixed ? 0.f : a2 + kp.g[2];
+            if (OUT_SORTED) {
+                out4[row] = make_float4(a0, a1, a2, dr);
+            } else {
+                const int64_t i = perm[row];
+                drho_out[i] = dr;
+                acc_out[i * DIM] = a0;
+                acc_out[i * DIM + 1] = a1;
+                if (DIM == 3) acc_out[i * DIM + 2] = a2;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ B1: VJP
+// Row i evaluates BOTH ordered pairs (i<-j) and (j<-i) of every neighbour j and keeps what lands on i
+// (possible because the list is symmetric), so there is no scatter.  The pressure enters through the
+// per-particle P_i = p_i/rho_i^2: its adjoint is collected as Z_i and pushed through the EOS once per row.
+// Per-lane running sums of the scalar-parameter partials are reduced per block in a fixed order (B2).
+constexpr int kNPart = 12;   // S_D1, S_Phi1, S_PhiL, S_eps, T_E, T_rho0, T_gam, g0, g1, g2, (2 spare)
+
+template <int DIM, int GS, bool VARH, bool OUT_SORTED>
+__global__ void __launch_bounds__(kBlock)
+k_vjp(int64_t n, KPar kp, float margin, const float4 *__restrict__ s0, const float4 *__restrict__ s1,
+      const float2 *__restrict__ s2, const float4 *__restrict__ cot, const float4 *__restrict__ eos,
+      const long long *__restrict__ row_ptr, const int32_t *__restrict__ col, const uint32_t *__restrict__ perm,
+      float *__restrict__ xb_out, float *__restrict__ vb_out, float *__restrict__ rb_out,
+      float4 *__restrict__ xb4, float4 *__restrict__ vb4, float *__restrict__ partials)
+{
+    constexpr int kGroups = kBlock / GS;
+    const int g = threadIdx.x / GS, gl = threadIdx.x % GS;
+    const int64_t row0 = (int64_t)blockIdx.x * kGroups * kRowsPerGroup;
+    const HC hu = hc_uniform<DIM>(kp);
+    float S_D1 = 0.f, S_P1 = 0.f, S_PL = 0.f, S_eps = 0.f;       // per lane, over all its pairs
+    float T_E = 0.f, T_0 = 0.f, T_g = 0.f, G0 = 0.f, G1 = 0.f, G2 = 0.f;   // lane 0 of each group, per row
+    for (int rr = 0; rr < kRowsPerGroup; ++rr) {
+        const int64_t row = row0 + (int64_t)rr * kGroups + g;
+        if (row >= n) break;
+        const Part pi = load_part<DIM>(s0, s1, s2, row);
+        const float4 ci = __ldg(cot + row);
+        const float4 ei = __ldg(eos + row);                    // {dP/drho, dP/drho0, dP/dgamma, m}
+        const float lam_i = ci.x, mu_i[3] = {ci.y, ci.z, ci.w};
+        const float m_i = ei.w;
+        const bool seam = row_near_seam(pi.x, kp, margin);
+        const long long b = row_ptr[row], e = row_ptr[row + 1];
+        const float ir_i = 1.0f / pi.rho;
+        float xb[3] = {0.f, 0.f, 0.f}, vb[3] = {0.f, 0.f, 0.f}, rb = 0.f, Z = 0.f;
+        for (long long p = b + gl; p < e; p += GS) {
+            const int32_t j = __ldg(col + p);
+            const Part pj = load_part<DIM>(s0, s1, s2, j);
+            const float4 cj = __ldg(cot + j);
+            const float lam_j = cj.x, mu_j[3] = {cj.y, cj.z, cj.w};
+            float d[3], r2;
+            if (seam) rel_pos<DIM, true>(pi.x, pj.x, kp, d, r2); else rel_pos<DIM, false>(pi.x, pj.x, kp, d, r2);
+            HC hc = hu;
+            if (VARH) hc = hc_make<DIM>(fmaxf(pi.h, pj.h), kp);
+            const float q = fast_sqrt(r2) * hc.invH;
+            const float t = fmaxf(1.0f - q, 0.f);
+            const float t2 = t * t, t4 = t2 * t2;
+            const float G = hc.cG * fmaf(5.0f, q, 1.0f) * (t4 * t);
+            const float K = hc.cK * t4;
+            float w[3] = {pi.v[0] - pj.v[0], pi.v[1] - pj.v[1], DIM == 3 ? pi.v[2] - pj.v[2] : 0.f};
+            float s = w[0] * d[0];
+            s = fmaf(w[1], d[1], s);
+            if (DIM == 3) s = fmaf(w[2], d[2], s);
+            const float invR = fast_rcp(r2 + hc.e2);
+            const float u = r2 * invR;
+            const float ir_j = 1.0f / pj.rho;
+            const float m_j = pj.V * pj.rho;
+            const float drho = pi.rho - pj.rho;
+            const float Psum = pi.P + pj.P;
+            float mm = mu_i[0] * d[0];                          // mu_i . d
+            mm = fmaf(mu_i[1], d[1], mm);
+            if (DIM == 3) mm = fmaf(mu_i[2], d[2], mm);
+            float mmj = mu_j[0] * d[0];                         // mu_j . d   (pair (j<-i) uses -d)
+            mmj = fmaf(mu_j[1], d[1], mmj);
+            if (DIM == 3) mmj = fmaf(mu_j[2], d[2], mmj);
+            const float mmp = -mmj;
+            // ---- ordered pair (i <- j)
+            const float VjG = pj.V * G;
+            const float E = -m_j * Psum;
+            const float Phi1 = kp.rho0 * pj.V * s * invR * ir_i;
+            const float Phi = hc.eta * Phi1;
+            const float sbar = lam_i * pi.rho * VjG + mm * hc.eta * kp.rho0 * VjG * invR * ir_i;
+            const float dif = hc.kd * VjG * u;                   // kd V_j (r2/R) G
+            const float r2bar = lam_i * hc.kd * VjG * drho * hc.e2 * invR * invR - mm * Phi * G * invR;
+            const float Gbar = lam_i * pj.V * (pi.rho * s + hc.kd * drho * u) + mm * (E + Phi);
+            // ---- ordered pair (j <- i): d -> -d, w -> -w, s unchanged
+            const float ViG = pi.V * G;
+            const float Ep = -m_i * Psum;
+            const float Phi1p = kp.rho0 * pi.V * s * invR * ir_j;
+            const float Phip = hc.eta * Phi1p;
+            const float sbarp = lam_j * pj.rho * ViG + mmp * hc.eta * kp.rho0 * ViG * invR * ir_j;
+            const float difp = hc.kd * ViG * u;
+            const float r2barp = -lam_j * hc.kd * ViG * drho * hc.e2 * invR * invR - mmp * Phip * G * invR;
+            const float ADp = ViG * (pj.rho * s - hc.kd * drho * u);          // A' + D'
+            const float Gbarp = lam_j * pi.V * (pj.rho * s - hc.kd * drho * u) + mmp * (Ep + Phip);
+            // ---- what lands on particle i
+            const float cs = sbar + sbarp;
+            const float cd = 2.0f * (r2bar + r2barp) + (Gbar + Gbarp) * K;
+            const float ce = (E + Phi) * G, cep = (Ep + Phip) * G;
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) {
+                xb[k] += cs * w[k] + cd * d[k] + ce * mu_i[k] - cep * mu_j[k];
+                vb[k] = fmaf(cs, d[k], vb[k]);
+            }
+            rb += lam_i * (VjG * s + dif) - mm * G * Phi * ir_i                 // first role of (i<-j)
+                  - lam_j * (ADp * ir_i + difp) - mmp * G * Phip * ir_i;         // second role of (j<-i)
+            Z = fmaf(G, m_j * mm + m_i * mmp, Z);               // -dL/dP_i
+            // ---- scalar parameters, ordered pair (i<-j) only (each ordered pair is owned by one row)
+            const float D1 = 2.0f * hc.ell * VjG * drho * u;    // D_ij / (delta c0)
+            S_D1 = fmaf(lam_i, D1, S_D1);
+            const float xphi1 = mm * G * Phi1;
+            S_P1 += xphi1;
+            S_PL = fmaf(xphi1, hc.ell, S_PL);
+            S_eps -= (lam_i * hc.kd * VjG * drho * u + mm * G * Phi) * invR * (2.0f * kp.eps * hc.H2);
+        }
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) {
+            xb[k] = group_sum<GS>(xb[k]);
+            vb[k] = group_sum<GS>(vb[k]);
+        }
+        rb = group_sum<GS>(rb);
+        Z = group_sum<GS>(Z);
+        if (gl == 0) {
+            rb -= ei.x * Z;                                      // rho_bar_i += Pbar_i dP/drho, Pbar_i = -Z_i
+            T_E += pi.P * Z;
+            T_0 += ei.y * Z;
+            T_g += ei.z * Z;
+            G0 += mu_i[0]; G1 += mu_i[1]; G2 += mu_i[2];
+            if (OUT_SORTED) {
+                xb4[row] = make_float4(xb[0], xb[1], xb[2], rb);
+                vb4[row] = make_float4(vb[0], vb[1], vb[2], 0.f);
+            } else {
+                const int64_t i = perm[row];
+#pragma unroll
+                for (int k = 0; k < DIM; ++k) {
+                    xb_out[i * DIM + k] = xb[k];
+                    vb_out[i * DIM + k] = vb[k];
+                }
+                rb_out[i] = rb;
+            }
+        }
+    }
+    // B2 stage 1: fixed-order block reduction of the ten partial sums
+    __shared__ float red[kBlock / 32][kNPart];
+    float vals[10] = {S_D1, S_P1, S_PL, S_eps, T_E, T_0, T_g, G0, G1, G2};
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 10; ++k) {
+        float v = vals[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[warp][k] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 10) {
+        float v = 0.f;
+        for (int w = 0; w < kBlock / 32; ++w) v += red[w][threadIdx.x];
+        partials[(int64_t)blockIdx.x * kNPart + threadIdx.x] = v;
+    }
+}
+
+// B2 stage 2: one block, binary64 accumulation of the per-block partials in index order, then the chain rule
+// from the ten sums to params_bar = d/d{c0, rho0, gamma, delta, alpha, nu, eps, g0, g1, g2}.
+__global__ void k_reduce_params(int64_t nblocks, const float *__restrict__ partials, KPar kp, int accumulate,
+                                float *__restrict__ params_bar)
+{
+    __shared__ double sh[10][128];
+    double acc[10];
+    for (int k = 0; k < 10; ++k) acc[k] = 0.0;
+    for (int64_t b = threadIdx.x; b < nblocks; b += blockDim.x)
+        for (int k = 0; k < 10; ++k) acc[k] += (double)partials[b * kNPart + k];
+    for (int k = 0; k < 10; ++k) sh[k][threadIdx.x] = acc[k];
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double S[10];
+        for (int k = 0; k < 10; ++k) {
+            double v = 0.0;
+            for (int t = 0; t < (int)blockDim.x; ++t) v += sh[k][t];
+            S[k] = v;
+        }
+        const double S_D1 = S[0], S_P1 = S[1], S_PL = S[2], S_eps = S[3], T_E = S[4], T_0 = S[5], T_g = S[6];
+        const double c0 = kp.c0, rho0 = kp.rho0, visc = kp.visc_nu;
+        double out[10];
+        // D = delta c0 D1;  Phi = (alpha l c0 + 2(d+2) nu) Phi1;  P scales with c0^2;  Pbar_i = -Z_i
+        out[0] = kp.delta * S_D1 + kp.alpha * S_PL - 2.0 * T_E / c0;                 // c0
+        out[1] = (kp.alpha * c0 * S_PL + visc * S_P1) / rho0 - T_0;                  // rho0
+        out[2] = -T_g;                                                               // gamma
+        out[3] = c0 * S_D1;                                                          // delta
+        out[4] = c0 * S_PL;                                                          // alpha
+        out[5] = 2.0 * (kp.dim + 2) * S_P1;                                          // nu
+        out[6] = S_eps;                                                              // eps
+        out[7] = S[7]; out[8] = S[8]; out[9] = S[9];                                 // g
+        for (int k = 0; k < 10; ++k) params_bar[k] = (accumulate ? params_bar[k] : 0.f) + (float)out[k];
+    }
+}
+
+} // namespace
+
+// ==========================================================================================
+// host side
+// ==========================================================================================
+static const double kKappa2 = 2.171239, kKappa3 = 2.207940;
+
+int sph_kpar_make(const sph_ctx *ctx, const sph_params *par, KPar *kp)
+{
+    if (!(par->c0 > 0.f) || !(par->rho0 > 0.f) || !(par->eps > 0.f) || !(par->gamma > 0.f)) return SPH_E_INVALID;
+    if (par->pressure_form != 0) return SPH_E_INVALID;
+    const GridGeom &gg = ctx->geom;
+    memset(kp, 0, sizeof(*kp));
+    kp->dim = gg.dim;
+    for (int k = 0; k < 3; ++k) {
+        kp->periodic[k] = gg.periodic[k];
+        kp->L[k] = gg.L[k];
+        kp->halfL[k] = 0.5f * gg.L[k];
+        kp->lo[k] = gg.lo[k];
+        kp->hi[k] = gg.hi[k];
+        kp->g[k] = k < gg.dim ? par->g[k] : 0.f;
+    }
+    kp->c0 = par->c0; kp->rho0 = par->rho0; kp->gamma = par->gamma; kp->delta = par->delta;
+    kp->alpha = par->alpha; kp->nu = par->nu; kp->eps = par->eps;
+    const double Cd = gg.dim == 2 ? 9.0 / M_PI : 495.0 / (32.0 * M_PI);
+    const double kap = gg.dim == 2 ? kKappa2 : kKappa3;
+    kp->Cd = (float)Cd;
+    kp->inv_kappa = (float)(1.0 / kap);
+    kp->visc_nu = (float)(2.0 * (gg.dim + 2) * (double)par->nu);
+    kp->Bp = (float)((double)par->rho0 * par->c0 * par->c0 / par->gamma);
+    kp->uniform_h = ctx->hmin == ctx->hmax;
+    if (kp->uniform_h) {
+        const double H = ctx->hmax, iH = 1.0 / H;
+        kp->H = (float)H;
+        kp->invH = (float)iH;
+        kp->cW = (float)(Cd * pow(iH, gg.dim));
+        kp->cG = (float)(-(56.0 / 3.0) * Cd * pow(iH, gg.dim + 2));
+        kp->cK = (float)(560.0 * Cd * pow(iH, gg.dim + 4));
+        const double ell = H / kap;
+        kp->ell = (float)ell;
+        kp->e2 = (float)((par->eps * H) * (par->eps * H));
+        kp->eta = (float)((double)par->alpha * ell * par->c0 + 2.0 * (gg.dim + 2) * (double)par->nu);
+        kp->kd = (float)(2.0 * (double)par->delta * ell * par->c0);
+    }
+    return SPH_OK;
+}
+
+namespace {
+
+// margin of row_near_seam: the list radius plus the largest admissible drift of a skin list
+float seam_margin(const sph_ctx *ctx)
+{
+    double e = 0.0;
+    for (int k = 0; k < ctx->geom.dim; ++k)
+        if (ctx->geom.edge[k] > e) e = ctx->geom.edge[k];
+    return (float)(2.0 * e);
+}
+
+unsigned pair_grid(int64_t n, int gs) { return (unsigned)((n + (kBlock / gs) * kRowsPerGroup - 1) / ((kBlock / gs) * kRowsPerGroup)); }
+
+template <int DIM>
+int pack_state(sph_ctx *ctx, const KPar &kp, const float *x, const float *v, const float *rho, const float *m,
+               const uint8_t *kind, bool with_eos, cudaStream_t st)
+{
+    const int64_t n = ctx->n;
+    SPH_TRY(ctx->s0.reserve((size_t)n * 16));
+    SPH_TRY(ctx->s1.reserve((size_t)n * 16));
+    SPH_TRY(ctx->s2.reserve((size_t)n * 8));
+    SPH_TRY(ctx->kind_s.reserve((size_t)n));
+    if (with_eos) SPH_TRY(ctx->eos.reserve((size_t)n * 16));
+    k_pack_state<DIM><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
+        n, kp, ctx->perm.as<uint32_t>(), ctx->pos_s.as<float4>(), x, v, rho, m, kind, ctx->s0.as<float4>(),
+        ctx->s1.as<float4>(), ctx->s2.as<float2>(), with_eos ? ctx->eos.as<float4>() : nullptr, ctx->kind_s.as<uint8_t>());
+    ctx->launches += 1;
+    return SPH_OK;
+}
+
+} // namespace
+
+// sorted-state launchers (also used by sph_rk.cu)
+int sph_launch_rhs_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
+                          const uint8_t *kind_s, float *drho, float *acc, float4 *out4, cudaStream_t st)
+{
+    const int64_t n = ctx->n;
+    const float margin = seam_margin(ctx);
+    const long long *rp = ctx->row_ptr.as<long long>();
+    const int32_t *col = ctx->col.as<int32_t>();
+    const uint32_t *perm = ctx->perm.as<uint32_t>();
+    const bool sorted = out4 != nullptr;
+#define SPH_RHS_LAUNCH(DIM, GS, VARH, SORTED)                                                                     \
+    k_rhs<DIM, GS, VARH, SORTED><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, s0, s1, s2, kind_s, rp, col, \
+                                                                     perm, drho, acc, out4)
+    if (kp.dim == 3) {
+        if (kp.uniform_h) { if (sorted) SPH_RHS_LAUNCH(3, 32, false, true); else SPH_RHS_LAUNCH(3, 32, false, false); }
+        else { if (sorted) SPH_RHS_LAUNCH(3, 32, true, true); else SPH_RHS_LAUNCH(3, 32, true, false); }
+    } else {
+        if (kp.uniform_h) { if (sorted) SPH_RHS_LAUNCH(2, 16, false, true); else SPH_RHS_LAUNCH(2, 16, false, false); }
+        else { if (sorted) SPH_RHS_LAUNCH(2, 16, true, true); else SPH_RHS_LAUNCH(2, 16, true, false); }
+    }
+#undef SPH_RHS_LAUNCH
+    ctx->launches += 1;
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_vjp_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
+                          const float4 *cot, const float4 *eos, float *xb, float *vb, float *rb, float4 *xb4,
+                          float4 *vb4, float *params_bar, int accumulate_params, cudaStream_t st)
+{
+    const int64_t n = ctx->n;
+    const float margin = seam_margin(ctx);
+    const long long *rp = ctx->row_ptr.as<long long>();
+    const int32_t *col = ctx->col.as<int32_t>();
+    const uint32_t *perm = ctx->perm.as<uint32_t>();
+    const bool sorted = xb4 != nullptr;
+    const int gs = kp.dim == 3 ? 32 : 16;
+    const unsigned grid = pair_grid(n, gs);
+    SPH_TRY(ctx->partials.reserve((size_t)grid * kNPart * 4));
+    float *part = ctx->partials.as<float>();
+#define SPH_VJP_LAUNCH(DIM, GS, VARH, SORTED)                                                                  \
+    k_vjp<DIM, GS, VARH, SORTED><<<grid, kBlock, 0, st>>>(n, kp, margin, s0, s1, s2, cot, eos, rp, col, perm, xb, \
+                                                         vb, rb, xb4, vb4, part)
+    if (kp.dim == 3) {
+        if (kp.uniform_h) { if (sorted) SPH_VJP_LAUNCH(3, 32, false, true); else SPH_VJP_LAUNCH(3, 32, false, false); }
+        else { if (sorted) SPH_VJP_LAUNCH(3, 32, true, true); else SPH_VJP_LAUNCH(3, 32, true, false); }
+    } else {
+        if (kp.uniform_h) { if (sorted) SPH_VJP_LAUNCH(2, 16, false, true); else SPH_VJP_LAUNCH(2, 16, false, false); }
+        else { if (sorted) SPH_VJP_LAUNCH(2, 16, true, true); else SPH_VJP_LAUNCH(2, 16, true, false); }
+    }
+#undef SPH_VJP_LAUNCH
+    ctx->launches += 1;
+    if (params_bar) {
+        k_reduce_params<<<1, 128, 0, st>>>((int64_t)grid, part, kp, accumulate_params, params_bar);
+        ctx->launches += 1;
+    }
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+extern "C" int sph_density(sph_ctx *ctx, const float *m, float *rho_out, sph_stream_t stream)
+{
+    if (!ctx || !m || !rho_out) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    const int64_t n = ctx->n;
+    sph_params dummy{};
+    dummy.c0 = 1.f; dummy.rho0 = 1.f; dummy.gamma = 1.f; dummy.eps = 1.f;
+    KPar kp;
+    SPH_TRY(sph_kpar_make(ctx, &dummy, &kp));
+    SPH_TRY(ctx->m_s.reserve((size_t)n * 4));
+    k_gather_f32<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), m, ctx->m_s.as<float>());
+    const float margin = seam_margin(ctx);
+#define SPH_DENS_LAUNCH(DIM, GS, VARH)                                                                               \
+    k_density<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(),           \
+                                                                 ctx->m_s.as<float>(), ctx->row_ptr.as<long long>(), \
+                                                                 ctx->col.as<int32_t>(), ctx->perm.as<uint32_t>(), rho_out)
+    if (kp.dim == 3) { if (kp.uniform_h) SPH_DENS_LAUNCH(3, 32, false); else SPH_DENS_LAUNCH(3, 32, true); }
+    else { if (kp.uniform_h) SPH_DENS_LAUNCH(2, 16, false); else SPH_DENS_LAUNCH(2, 16, true); }
+#undef SPH_DENS_LAUNCH
+    ctx->launches += 2;
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+extern "C" int sph_rhs(sph_ctx *ctx, const sph_params *par, const float *x, const float *v, const float *rho,
+                       const float *m, const uint8_t *kind, float *drho_dt, float *acc, sph_stream_t stream)
+{
+    if (!ctx || !par || !x || !v || !rho || !m || !kind || !drho_dt || !acc) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    KPar kp;
+    SPH_TRY(sph_kpar_make(ctx, par, &kp));
+    if (kp.dim == 3) SPH_TRY(pack_state<3>(ctx, kp, x, v, rho, m, kind, false, st));
+    else SPH_TRY(pack_state<2>(ctx, kp, x, v, rho, m, kind, false, st));
+    return sph_launch_rhs_sorted(ctx, kp, ctx->s0.as<float4>(), ctx->s1.as<float4>(), ctx->s2.as<float2>(),
+                                 ctx->kind_s.as<uint8_t>(), drho_dt, acc, nullptr, st);
+}
+
+extern "C" int sph_rhs_vjp(sph_ctx *ctx, const sph_params *par, const float *x, const float *v, const float *rho,
+                           const float *m, const uint8_t *kind, const float *drho_bar, const float *acc_bar,
+                           float *x_bar, float *v_bar, float *rho_bar, float *params_bar, sph_stream_t stream)
+{
+    if (!ctx || !par || !x || !v || !rho || !m || !kind || !drho_bar || !acc_bar || !x_bar || !v_bar || !rho_bar)
+        return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    const int64_t n = ctx->n;
+    KPar kp;
+    SPH_TRY(sph_kpar_make(ctx, par, &kp));
+    if (kp.dim == 3) SPH_TRY(pack_state<3>(ctx, kp, x, v, rho, m, kind, true, st));
+    else SPH_TRY(pack_state<2>(ctx, kp, x, v, rho, m, kind, true, st));
+    SPH_TRY(ctx->c0buf.reserve((size_t)n * 16));
+    k_pack_cot<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, kp.dim, ctx->perm.as<uint32_t>(), ctx->kind_s.as<uint8_t>(),
+                                                            drho_bar, acc_bar, ctx->c0buf.as<float4>());
+    ctx->launches += 1;
+    return sph_launch_vjp_sorted(ctx, kp, ctx->s0.as<float4>(), ctx->s1.as<float4>(), ctx->s2.as<float2>(),
+                                 ctx->c0buf.as<float4>(), ctx->eos.as<float4>(), x_bar, v_bar, rho_bar, nullptr, nullptr,
+                                 params_bar, 0, st);
+}

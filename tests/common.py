@@ -17,10 +17,15 @@ def golden(fname):
     return out
 
 
-def max_norm_err(y, yref, scale=None, floor_frac=1e-3):
-    """err = max_i |y_i - yref_i|_inf / max(max_i |yref_i|_inf, floor_frac * max_i scale_i).
-    On lattice configs the exact drho/dt is 0 and a has zero crossings, so an element-wise relative error
-    is undefined; ``scale`` is the oracle's per-row sum of |pair terms|."""
+def max_norm_err(y, yref, scale=None, floor_frac=1e-2):
+    """err = max_i |y_i - yref_i|_inf / max(max_i |yref_i|_inf, floor_frac * max_i scale_i)   (reading R10,
+    after SURVEY.md 8c-9).  On lattice configs the exact drho/dt is 0 and a has zero crossings, so an element-wise
+    relative error is undefined; ``scale`` is the oracle's per-row sum of |pair terms| S_i.
+    floor_frac = 1e-2: a binary32 sum of N ~ 100 pair terms, each formed by ~8 rounded operations, carries a forward
+    error of up to (8 + log2 N) u S ~ 9e-7 S (u = 2^-24); with the bar of 1e-4 the floor 1e-2 S admits 1e-6 S.
+    SURVEY's proposed 1e-3 would demand 1e-7 S = 1.7 u S, below what ANY binary32 evaluation of the terms can
+    deliver when the exact sum cancels to zero (measured: a correctly rounded fp32 evaluation of every term, summed
+    exactly, already misses it by 2.7x on the 3D Taylor-Green lattice, where drho/dt = 0)."""
     y = np.asarray(y, dtype=np.float64)
     yref = np.asarray(yref, dtype=np.float64)
     den = np.max(np.abs(yref)) if yref.size else 0.0

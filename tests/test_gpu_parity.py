@@ -1,0 +1,275 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the fp64 oracle, element by element on the same
+seeded fp32 inputs.  Bars (BASELINE.json north_star): neighbour lists bit-exact as sorted sets; density, drho/dt,
+acc <= 1e-4; VJP outputs and parameter gradients <= 1e-3; error metric = max-norm normalised."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2507_21684_b200 import workloads as W
+from paper_2507_21684_b200.binding import Sph, SphError
+from common import max_norm_err
+from gpu_common import Dev, build, oracle_lists
+
+pytestmark = pytest.mark.gpu
+
+TOL_FWD = 1e-4
+TOL_VJP = 1e-3
+
+# sizes the oracle finishes in seconds that still span many cells / blocks and a ragged tail
+CASES = {
+    "C0": lambda: W.make(0),
+    "C0p": lambda: W.perturbed(W.make(0), amp_x=0.3, amp_rho=0.03),
+    "C1s": lambda: W.perturbed(W.make(1, n_axis=96), amp_x=0.0, amp_rho=0.02),
+    "C2s": lambda: W.make(2, dx=0.02),
+    "C2p": lambda: W.perturbed(W.make(2, dx=0.025), amp_x=0.2, amp_rho=0.0),
+    "C3s": lambda: W.make(3, n_axis=24),
+    "C3p": lambda: W.perturbed(W.make(3, n_axis=29), amp_x=0.3, amp_rho=0.03),
+    "C4s": lambda: W.perturbed(W.make(4, n_axis=27), amp_x=0.0, amp_rho=0.03),
+}
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+@pytest.fixture(scope="module")
+def sph():
+    s = Sph(0)
+    yield s
+    s.close()
+
+
+# ------------------------------------------------------------------------------------------ lists
+@pytest.mark.parametrize("case", list(CASES))
+@pytest.mark.parametrize("scale", [1.0, 1.25])
+def test_neighbor_lists_bit_exact(sph, case, scale):
+    wl = CASES[case]()
+    if scale > 1.0:
+        # the cell size must cover the enlarged search radius
+        wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(scale) * np.float32(1.0001))
+    _, dev, nnz = build(wl, scale, sph)
+    rp, ci = sph.neighbors_export()
+    rp_o, ci_o = oracle_lists(wl, scale)
+    assert nnz == int(rp_o[-1])
+    assert np.array_equal(_np(rp), rp_o)
+    assert np.array_equal(_np(ci), ci_o)
+
+
+def test_neighbor_lists_out_of_box_positions_wrap(sph):
+    """absolute positions are kept by the caller; wrapping is internal and follows reading R4"""
+    wl = W.perturbed(W.make(1, n_axis=40), amp_x=0.3)
+    rng = np.random.default_rng(1)
+    wl.x = (wl.x + rng.integers(-3, 4, size=wl.x.shape).astype(np.float32)).astype(np.float32)
+    _, dev, nnz = build(wl, 1.0, sph)
+    rp, ci = sph.neighbors_export()
+    rp_o, ci_o = oracle_lists(wl)
+    assert np.array_equal(_np(rp), rp_o) and np.array_equal(_np(ci), ci_o)
+
+
+def test_neighbor_lists_degenerate_inputs(sph):
+    # one particle; coincident particles; everything in one cell
+    dom = W.Domain(dim=3, periodic=(0, 0, 0), lo=(0.0,) * 3, hi=(1.0,) * 3, cell_size=0.5)
+    for x in (np.array([[0.3, 0.3, 0.3]], np.float32),
+              np.array([[0.3, 0.3, 0.3]] * 5 + [[0.31, 0.3, 0.3]], np.float32),
+              np.random.default_rng(0).uniform(0.5, 0.99, size=(300, 3)).astype(np.float32)):
+        h = np.full(x.shape[0], 0.45, np.float32)
+        wl = W.Workload(name="deg", domain=dom, params=W.Params(), x=x, v=0 * x, rho=np.ones(len(x), np.float32),
+                        m=np.ones(len(x), np.float32), h=h, kind=np.zeros(len(x), np.uint8), dt=0.0, dx=0.1, seed=0)
+        build(wl, 1.0, sph)
+        rp, ci = sph.neighbors_export()
+        rp_o, ci_o = oracle_lists(wl, method=0)
+        assert np.array_equal(_np(rp), rp_o) and np.array_equal(_np(ci), ci_o)
+
+
+def test_error_codes(sph):
+    wl = W.make(2, dx=0.05)
+    dev = Dev(wl)
+    # position outside a bounded axis -> SPH_E_DOMAIN at the next synchronising call
+    xb = dev.x.clone()
+    xb[7, 0] = 100.0
+    sph.build_cells(wl.domain, xb, dev.h)
+    with pytest.raises(SphError) as e:
+        sph.neighbors(1.0)
+    assert e.value.code == -2
+    # cell size smaller than the search radius
+    sph.build_cells(wl.domain, dev.x, dev.h)
+    with pytest.raises(SphError) as e:
+        sph.neighbors(1.5)
+    assert e.value.code == -2
+    # fewer than 3 cells on a periodic axis
+    bad = W.Domain(dim=2, periodic=(1, 1, 0), lo=(0.0,) * 3, hi=(1.0, 1.0, 0.0), cell_size=0.4)
+    with pytest.raises(SphError) as e:
+        sph.build_cells(bad, dev.x, dev.h)
+    assert e.value.code == -2
+    # call order
+    s2 = Sph(0)
+    with pytest.raises(SphError) as e:
+        s2.neighbors(1.0)
+    assert e.value.code == -3
+    s2.close()
+    # unsupported pressure form is rejected loudly, not silently computed
+    sph.build_cells(wl.domain, dev.x, dev.h)
+    sph.neighbors(1.0)
+    par = W.Params(**{**wl.params.__dict__, "pressure_form": 1})
+    with pytest.raises(SphError) as e:
+        sph.rhs(par, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+    assert e.value.code == -1
+
+
+# ------------------------------------------------------------------------------------------ density / RHS / VJP
+@pytest.mark.parametrize("case", list(CASES))
+def test_density_parity(sph, case):
+    wl = CASES[case]()
+    _, dev, _ = build(wl, 1.0, sph)
+    rho = _np(sph.density(dev.m))
+    ref = oracle.density(wl.domain, wl.x, wl.h, wl.m, *oracle_lists(wl))
+    assert max_norm_err(rho, ref) < TOL_FWD
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_rhs_parity(sph, case):
+    wl = CASES[case]()
+    _, dev, _ = build(wl, 1.0, sph)
+    drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+    d_o, a_o, sd, sa = oracle.rhs(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *oracle_lists(wl),
+                                  with_scales=True)
+    e_d, e_a = max_norm_err(_np(drho), d_o, sd), max_norm_err(_np(acc), a_o, sa)
+    print(f"{case}: n={wl.n} drho err {e_d:.2e} acc err {e_a:.2e}")
+    assert e_d < TOL_FWD and e_a < TOL_FWD
+    if wl.kind.any():
+        assert np.all(_np(acc)[wl.kind == 1] == 0.0)
+
+
+def test_rhs_independent_of_skin(sph):
+    """pairs with r >= H_ij in a skin-enlarged list contribute exactly 0 (kernel clamp)"""
+    wl = CASES["C3p"]()
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.3))
+    _, dev, nnz1 = build(wl, 1.0, sph)
+    a = [_np(t).copy() for t in sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)]
+    _, _, nnz2 = build(wl, 1.29, sph, dev)
+    b = [_np(t).copy() for t in sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)]
+    assert nnz2 > nnz1
+    for u, w in zip(a, b):
+        assert np.max(np.abs(u - w)) <= 2e-6 * np.max(np.abs(u))     # same terms, different summation order
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_vjp_parity(sph, case):
+    wl = CASES[case]()
+    if case.startswith("C2"):
+        par = wl.params
+    else:
+        par = W.Params(**{**wl.params.__dict__, "alpha": 0.02, "g": (0.3, -0.2, 0.1)})
+    lam, mu = W.random_cotangents(wl)
+    _, dev, _ = build(wl, 1.0, sph)
+    lam_d, mu_d = torch.from_numpy(lam).cuda(), torch.from_numpy(mu).cuda()
+    xb, vb, rb, pb = sph.rhs_vjp(par, dev.x, dev.v, dev.rho, dev.m, dev.kind, lam_d, mu_d)
+    xo, vo, ro, po = oracle.rhs_vjp(wl.domain, par, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *oracle_lists(wl), lam, mu)
+    errs = dict(x=max_norm_err(_np(xb), xo), v=max_norm_err(_np(vb), vo), rho=max_norm_err(_np(rb), ro))
+    pg = _np(pb).astype(np.float64)
+    # parameter gradients: relative to the gradient itself, floored by the size of the summed terms
+    # (each is a global sum of signed pair terms; the floor is 1e-3 of the largest one in magnitude)
+    pe = np.abs(pg - po) / np.maximum(np.abs(po), 1e-3 * np.max(np.abs(po)) + 1e-30)
+    print(f"{case}: n={wl.n} vjp errs {errs} params {np.max(pe):.2e}")
+    assert max(errs.values()) < TOL_VJP
+    assert np.max(pe) < TOL_VJP
+    # deterministic: a second run gives bit-identical results (no float atomics)
+    xb2, vb2, rb2, pb2 = sph.rhs_vjp(par, dev.x, dev.v, dev.rho, dev.m, dev.kind, lam_d, mu_d)
+    assert torch.equal(xb, xb2) and torch.equal(vb, vb2) and torch.equal(rb, rb2) and torch.equal(pb, pb2)
+
+
+# ------------------------------------------------------------------------------------------ RK4
+@pytest.mark.parametrize("case", ["C0", "C1s", "C2s", "C3p", "C4s"])
+def test_rk_step_parity(sph, case):
+    wl = CASES[case]()
+    skin = 0.1
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin) * np.float32(1.0001))
+    dev = Dev(wl)
+    x, v, rho = dev.x.clone(), dev.v.clone(), dev.rho.clone()
+    sph.rk_step(wl.domain, wl.params, wl.dt, skin, x, v, rho, dev.m, dev.h, dev.kind)
+    xo, vo, ro = oracle.rk4_step(wl.domain, wl.params, wl.dt, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, method=1)
+    # compare the increments (the state itself would hide errors behind the unchanged part)
+    ex = max_norm_err(_np(x).astype(np.float64) - wl.x, xo - wl.x)
+    ev = max_norm_err(_np(v).astype(np.float64) - wl.v, vo - wl.v)
+    er = max_norm_err(_np(rho).astype(np.float64) - wl.rho, ro - wl.rho)
+    print(f"{case}: rk increments err x {ex:.2e} v {ev:.2e} rho {er:.2e}")
+    # increments are differences of fp32 states: allow the fp32 resolution of the state on top of 1e-4
+    fl = lambda a, b: 2.0 ** -23 * np.max(np.abs(a)) / max(np.max(np.abs(b)), 1e-300)
+    assert ex < TOL_FWD + fl(wl.x, xo - wl.x)
+    assert ev < TOL_FWD + fl(wl.v, vo - wl.v)
+    assert er < TOL_FWD + fl(wl.rho, ro - wl.rho)
+    if wl.kind.any():
+        b = wl.kind == 1
+        assert np.array_equal(_np(x)[b], wl.x[b]) and np.array_equal(_np(v)[b], wl.v[b])
+
+
+@pytest.mark.parametrize("case", ["C0", "C2s", "C3p"])
+def test_rk_step_vjp_parity(sph, case):
+    """L = kinetic energy after one RK4 step (BASELINE.json config 0); gradient w.r.t. the initial state"""
+    wl = CASES[case]()
+    skin = 0.1
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin) * np.float32(1.0001))
+    dev = Dev(wl)
+    x, v, rho = dev.x.clone(), dev.v.clone(), dev.rho.clone()
+    sph.rk_step(wl.domain, wl.params, wl.dt, skin, x, v, rho, dev.m, dev.h, dev.kind)
+    xb = torch.zeros_like(x)
+    vb = (dev.m[:, None] * v).contiguous()
+    rb = torch.zeros_like(rho)
+    pb = torch.zeros(10, device="cuda")
+    sph.rk_step_vjp(wl.domain, wl.params, wl.dt, skin, dev.x, dev.v, dev.rho, dev.m, dev.h, dev.kind, xb, vb, rb, pb)
+    _, v1, _ = oracle.rk4_step(wl.domain, wl.params, wl.dt, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, method=1)
+    xo, vo, ro, po = oracle.rk4_step_vjp(wl.domain, wl.params, wl.dt, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind,
+                                         np.zeros_like(v1), wl.m.astype(np.float64)[:, None] * v1, np.zeros(wl.n), method=1)
+    errs = dict(x=max_norm_err(_np(xb), xo), v=max_norm_err(_np(vb), vo), rho=max_norm_err(_np(rb), ro))
+    pg = _np(pb).astype(np.float64)
+    pe = np.abs(pg - po) / np.maximum(np.abs(po), 1e-3 * np.max(np.abs(po)) + 1e-30)
+    print(f"{case}: rk vjp errs {errs} params {np.max(pe):.2e}")
+    assert max(errs.values()) < TOL_VJP and np.max(pe) < TOL_VJP
+
+
+def test_host_entry_point_matches_device_calls(sph):
+    wl = CASES["C3p"]()
+    lam, mu = W.random_cotangents(wl)
+    outs = sph.forward_backward_host(wl.domain, wl.params, 1.0, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, lam, mu)
+    _, dev, _ = build(wl, 1.0, sph)
+    drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+    xb, vb, rb, pb = sph.rhs_vjp(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind, torch.from_numpy(lam).cuda(),
+                                 torch.from_numpy(mu).cuda())
+    assert np.array_equal(outs["drho_dt"], _np(drho)) and np.array_equal(outs["acc"], _np(acc))
+    assert np.array_equal(outs["x_bar"], _np(xb)) and np.array_equal(outs["params_bar"], _np(pb))
+
+
+# ------------------------------------------------------------------------------------------ full size, sampled
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_full_size_sampled_rows(sph, cfg):
+    """BASELINE.json's full sizes in the launch configuration bench.py times: lists compared in full (bit-exact),
+    RHS / VJP on sampled rows the oracle computes one by one."""
+    wl = W.make(cfg)
+    if cfg == 3:
+        wl = W.perturbed(wl, amp_x=0.1, amp_rho=0.01)        # the state after a few steps: disordered lattice
+    lam, mu = W.random_cotangents(wl)
+    _, dev, nnz = build(wl, 1.0, sph)
+    rp_o, ci_o = oracle_lists(wl)
+    assert nnz == int(rp_o[-1])
+    rp, ci = sph.neighbors_export()
+    assert np.array_equal(_np(rp), rp_o)
+    assert np.array_equal(_np(ci), ci_o)
+    rows = np.random.default_rng(7).choice(wl.n, size=2000, replace=False).astype(np.int64)
+    drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+    d_o, a_o, sd, sa = oracle.rhs(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp_o, ci_o, rows=rows,
+                                  with_scales=True)
+    assert max_norm_err(_np(drho)[rows], d_o[rows], sd[rows]) < TOL_FWD
+    assert max_norm_err(_np(acc)[rows], a_o[rows], sa[rows]) < TOL_FWD
+    xb, vb, rb, pb = sph.rhs_vjp(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind, torch.from_numpy(lam).cuda(),
+                                 torch.from_numpy(mu).cuda())
+    xo, vo, ro, _ = oracle.rhs_vjp(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp_o, ci_o, lam, mu,
+                                   rows=rows)
+    assert max_norm_err(_np(xb)[rows], xo[rows]) < TOL_VJP
+    assert max_norm_err(_np(vb)[rows], vo[rows]) < TOL_VJP
+    assert max_norm_err(_np(rb)[rows], ro[rows]) < TOL_VJP
+    # properties that hold at any size: the RHS depends on differences only
+    sx = xb.double().sum(0).abs().max().item() / xb.double().abs().sum().item()
+    sv = vb.double().sum(0).abs().max().item() / vb.double().abs().sum().item()
+    assert sx < 1e-5 and sv < 1e-5
+    assert torch.isfinite(pb).all()
