@@ -1,0 +1,399 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the delta-SPH hot path on B200 (BASELINE.json config 3 by default).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+One "step" is one pass of the whole hot path (every SURVEY.md 8(a) row) over the current particle state:
+
+    sph_build_cells + sph_neighbors(1.0)      N1-N7  rebuild, exact radius, grid of cell size H
+    sph_density                               D
+    sph_rhs                                   R0, R1
+    sph_rhs_vjp (lambda, mu ~ N(0,1))         R0, B1, B2
+    sph_rk_step(dt, skin)                     N1-N7 again on the skin grid, 4 x (R0, R1), T  -> advances the state
+
+`value` = pair interactions per second, a pair interaction being one CSR entry processed by one pair pass
+(SURVEY.md 8(d)): per step  3 * nnz(exact list) + 4 * nnz(skin list), summed over all ranks, divided by the
+max-over-ranks device time.  The north-star figure "ms per forward+backward RHS step" is reported beside it as
+`ms_fwd_bwd` (sph_rhs + sph_rhs_vjp only) with `pairs_per_s_fwd_bwd` = 2 nnz / that time.
+
+N > 1: the path does not shard in this round ("replicas only"): every rank runs an
+independent replica of the workload (different seed), no data-path collective; weak scaling.
+
+--impl reference: the fp64 CPU oracle (oracle/), as it stands, on the host cores, on a bounded sample of rows.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "pair_interactions_per_s"
+UNIT = "pair-interactions/s"
+SKIN = 0.06          # Verlet skin of the RK4 list: skin*H >= 2*dt*max|v| = 0.05 H for dt = 0.25 H/c0, |v| <= c0/10
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
+
+
+def make_workload(config, seed_shift, n_axis=None):
+    from paper_2507_21684_b200 import workloads as W
+    wl = W.make(config, n_axis=n_axis) if config != 2 else W.make(config)
+    if seed_shift:
+        # replicas: same recipe, different random cotangents / jitter stream
+        wl.seed += 7919 * seed_shift
+    return wl
+
+
+def rk_domain(wl):
+    """grid for sph_rk_step: cell_size >= (1+skin) * max h"""
+    from paper_2507_21684_b200 import workloads as W
+    d = wl.domain
+    cs = float(np.float32(np.float32(wl.h.max()) * np.float32(1.0 + SKIN) * np.float32(1.0001)))
+    return W.Domain(dim=d.dim, periodic=d.periodic, lo=d.lo, hi=d.hi, cell_size=max(cs, float(d.cell_size)))
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)"""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", str(gpu_index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [t.strip() for t in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2])); pw.append(float(c[3]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if c[5 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            # under load = samples whose power is above the idle floor; fall back to all samples
+            thr = 0.5 * max(pw)
+            load = [s for s, p in zip(sm, pw) if p >= thr] or sm
+            out = {"sm_mhz": float(np.median(load)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                   "samples": len(sm), "power_w_max": float(max(pw))}
+        return out
+
+
+# --------------------------------------------------------------------------------------------------------------
+# algorithmic bytes per launch of the pair kernels
+def algorithmic_bytes(cls, n, nnz, dim):
+    state = 40 if dim == 3 else 32                   # sorted SoA s0,s1(,s2) read once per row
+    if cls == "rhs":
+        return 4 * nnz + 8 * (n + 1) + n * (state + 1 + 16)              # + kind + {a, drho/dt}
+    if cls == "vjp":
+        return 4 * nnz + 8 * (n + 1) + n * (state + 16 + 16 + 32)        # + cotangents + EOS derivs + {xbar,rhobar},{vbar}
+    if cls == "density":
+        return 4 * nnz + 8 * (n + 1) + n * (16 + 4 + 4 + 4)              # pos, m, perm, rho
+    if cls in ("count", "fill"):
+        return (4 * nnz if cls == "fill" else 0) + n * (16 + 4) + 8 * n  # pos + cnt/row_ptr (+ col written)
+    return None
+
+
+def cpu_sample(wl, budget_s=12.0, seed=3):
+    """The oracle, as it stands, on a bounded sample: forward RHS + VJP of `rows` sampled rows of the workload (lists
+    from the oracle's own grid search over all particles, timed separately)."""
+    import oracle
+    from paper_2507_21684_b200 import workloads as W
+    lam, mu = W.random_cotangents(wl)
+    t0 = time.perf_counter()
+    rp, ci = oracle.neighbors(wl.domain, wl.x, wl.h, method=1)
+    t_lists = time.perf_counter() - t0
+    rng = np.random.default_rng(seed)
+
+    def run(nrows):
+        rows = np.sort(rng.choice(wl.n, size=min(nrows, wl.n), replace=False)).astype(np.int64)
+        t0 = time.perf_counter()
+        oracle.rhs(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp, ci, rows=rows)
+        oracle.rhs_vjp(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp, ci, lam, mu, rows=rows)
+        dt = time.perf_counter() - t0
+        pairs = 2 * int((rp[rows + 1] - rp[rows]).sum())
+        return pairs, dt, len(rows)
+
+    pairs, dt, nr = run(20000)                       # calibration
+    want = int(min(wl.n, max(20000, 20000 * budget_s / max(dt, 1e-3))))
+    pairs, dt, nr = run(want)
+    return {"value": pairs / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"oracle.rhs + oracle.rhs_vjp (fp64, OpenMP) on {nr} sampled rows of {wl.name} "
+                      f"({pairs} pair interactions in {dt:.2f} s); oracle grid neighbour search over all "
+                      f"{wl.n} particles took {t_lists:.2f} s and is not in the figure"}, (rp, ci)
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle on the host cores; rank 0 only."""
+    if rank != 0:
+        return
+    import oracle
+    from paper_2507_21684_b200 import workloads as W
+    wl = make_workload(args.config, 0, args.n_axis)
+    lam, mu = W.random_cotangents(wl)
+    rp, ci = oracle.neighbors(wl.domain, wl.x, wl.h, method=1)
+    rng = np.random.default_rng(11)
+    nrows = args.ref_rows
+
+    def step():
+        rows = np.sort(rng.choice(wl.n, size=min(nrows, wl.n), replace=False)).astype(np.int64)
+        oracle.rhs(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp, ci, rows=rows)
+        oracle.rhs_vjp(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp, ci, lam, mu, rows=rows)
+        return 2 * int((rp[rows + 1] - rp[rows]).sum())
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    pairs = 0
+    for _ in range(args.steps):
+        pairs += step()
+    dt = time.perf_counter() - t0
+    val = pairs / dt
+    sample = (f"per step: oracle.rhs + oracle.rhs_vjp (fp64, OpenMP) on {min(nrows, wl.n)} sampled rows of {wl.name}; "
+              f"lists prebuilt by the oracle grid search")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "n_particles": wl.n, "dim": wl.dim},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (3 = 3D 128^3, the metric's)")
+    ap.add_argument("--n-axis", type=int, default=None, help="shrink the lattice (debugging only; invalid as a result)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
+    ap.add_argument("--ref-rows", type=int, default=100000)
+    ap.add_argument("--cpu-budget", type=float, default=12.0)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = max(args.warmup, 0)            # the driver passes W; W >= 3 is the rule for reported numbers
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2507_21684_b200 import workloads as W
+    from paper_2507_21684_b200.binding import Sph
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the SPH library has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    wl = make_workload(args.config, rank, args.n_axis)
+    dom, dom_rk, par = wl.domain, rk_domain(wl), wl.params
+    lam_h, mu_h = W.random_cotangents(wl)
+    n, dim = wl.n, wl.dim
+    t = lambda a: torch.from_numpy(a).to(dev)
+    x, v, rho, m, h, kind = t(wl.x), t(wl.v), t(wl.rho), t(wl.m), t(wl.h), t(wl.kind)
+    lam, mu = t(lam_h), t(mu_h)
+    dens = torch.empty_like(rho); drho = torch.empty_like(rho); acc = torch.empty_like(v)
+    vjp_out = (torch.empty_like(x), torch.empty_like(v), torch.empty_like(rho), torch.empty(10, dtype=torch.float32, device=dev))
+    sph = Sph(local_rank, n)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    phases = ("rebuild", "density", "fwd", "bwd", "rk4")
+    marks = []                                       # per timed step: 6 events
+    counts = {"nnz": 0, "nnz_rk": 0}
+
+    def step(timed):
+        e = [ev() for _ in range(6)] if timed else None
+        if timed: e[0].record()
+        sph.build_cells(dom, x, h)
+        nnz = sph.neighbors(1.0)
+        if timed: e[1].record()
+        sph.density(m, dens)
+        if timed: e[2].record()
+        sph.rhs(par, x, v, rho, m, kind, drho, acc)
+        if timed: e[3].record()
+        sph.rhs_vjp(par, x, v, rho, m, kind, lam, mu, vjp_out)
+        if timed: e[4].record()
+        sph.rk_step(dom_rk, par, wl.dt, SKIN, x, v, rho, m, h, kind)
+        if timed: e[5].record()
+        nnz_rk = sph.info()["nnz"]
+        if timed:
+            marks.append(e)
+            counts["nnz"] += nnz
+            counts["nnz_rk"] += nnz_rk
+        return nnz, nnz_rk
+
+    for _ in range(args.warmup):
+        step(False)
+    sph.check()
+    sph.profile_read()                               # clear accumulators
+    launches0 = sph.info()["launches"]
+    sph.profile_enable(True)
+    barrier()
+    clocks = ClockSampler(local_rank) if rank == 0 else None
+    t_start, t_stop = ev(), ev()
+    t_start.record()
+    for _ in range(args.steps):
+        nnz_last, nnz_rk_last = step(True)
+    t_stop.record()
+    barrier()
+    clk = clocks.stop() if clocks else None
+    sph.profile_enable(False)
+    ms_total = t_start.elapsed_time(t_stop)
+    prof = sph.profile_read()
+    launches = sph.info()["launches"] - launches0
+    sph.check()
+    assert torch.isfinite(vjp_out[0]).all() and torch.isfinite(x).all(), "non-finite state after the timed steps"
+
+    pairs_rank = 3 * counts["nnz"] + 4 * counts["nnz_rk"]
+    ph_ms = {p: float(np.mean([mk[i].elapsed_time(mk[i + 1]) for mk in marks])) for i, p in enumerate(phases)}
+    fb_ms = ph_ms["fwd"] + ph_ms["bwd"]
+    nnz_mean = counts["nnz"] / args.steps
+
+    tt = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    pp = torch.tensor([float(pairs_rank)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        dist.all_reduce(pp, op=dist.ReduceOp.SUM)
+    ms_max, pairs_all = float(tt.item()), float(pp.item())
+    value = pairs_all / (ms_max * 1e-3)
+
+    # ---- e2e: the same step through sph_step_host with pinned host buffers, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        hx, hv, hr = pin(wl.x.copy()), pin(wl.v.copy()), pin(wl.rho.copy())
+        hm, hh, hk, hl, hmu = pin(wl.m), pin(wl.h), pin(wl.kind), pin(lam_h), pin(mu_h)
+        outs = {"density": pin(np.empty(n, np.float32)), "drho_dt": pin(np.empty(n, np.float32)),
+                "acc": pin(np.empty((n, dim), np.float32)), "x_bar": pin(np.empty((n, dim), np.float32)),
+                "v_bar": pin(np.empty((n, dim), np.float32)), "rho_bar": pin(np.empty(n, np.float32)),
+                "params_bar": pin(np.empty(10, np.float32))}
+        h2d = sum(a.numel() * a.element_size() for a in (hx, hv, hr, hm, hh, hk, hl, hmu))
+        d2h = sum(a.numel() * a.element_size() for a in outs.values()) + sum(a.numel() * a.element_size() for a in (hx, hv, hr))
+        ke = max(3, min(args.steps, 10))
+        for _ in range(2):
+            sph.step_host(dom, dom_rk, par, wl.dt, SKIN, hx, hv, hr, hm, hh, hk, hl, hmu, outs)
+        barrier()
+        pairs_e = 0
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            a, b = sph.step_host(dom, dom_rk, par, wl.dt, SKIN, hx, hv, hr, hm, hh, hk, hl, hmu, outs)
+            pairs_e += 3 * a + 4 * b
+        torch.cuda.synchronize()
+        dt_e = time.perf_counter() - t0
+        te = torch.tensor([dt_e], dtype=torch.float64, device=dev)
+        pe = torch.tensor([float(pairs_e)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+            dist.all_reduce(pe, op=dist.ReduceOp.SUM)
+        assert np.isfinite(outs["params_bar"].numpy()).all()
+        e2e = {"value": float(pe.item()) / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "steps": ke, "ms_per_step": 1e3 * float(te.item()) / ke,
+               "call": "sph_step_host (pinned host buffers; H2D + whole step + D2H inside the timed region)"}
+
+    if rank == 0:
+        hbm, hbm_src, sm_max = peaks()
+        kern = {}
+        tot_k = sum(ms for ms, _ in prof.values()) or 1.0
+        for name, (ms, cnt) in prof.items():
+            if cnt:
+                kern[name] = {"ms_per_step": ms / args.steps, "launches_per_step": cnt / args.steps,
+                              "share": ms / tot_k}
+        # dominant kernel among the classes with a stated byte model
+        cand = [c for c in ("rhs", "vjp", "density", "count", "fill") if c in kern]
+        dom_cls = max(cand, key=lambda c: kern[c]["ms_per_step"])
+        nnz_for = {"rhs": (counts["nnz"] + 4 * counts["nnz_rk"]) / (5.0 * args.steps), "vjp": nnz_mean, "density": nnz_mean,
+                   "count": (counts["nnz"] + counts["nnz_rk"]) / (2.0 * args.steps),
+                   "fill": (counts["nnz"] + counts["nnz_rk"]) / (2.0 * args.steps)}
+        roof = {}
+        for c in cand:
+            ms_launch = prof[c][0] / max(prof[c][1] / (2 if c == "density" else 1), 1)
+            by = algorithmic_bytes(c, n, nnz_for[c], dim)
+            roof[c] = {"bound": "hbm", "achieved": by / (ms_launch * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                       "frac": by / (ms_launch * 1e-3) / 1e9 / hbm, "traffic": None, "kernel": c,
+                       "ms_per_launch": ms_launch, "algorithmic_bytes_per_launch": int(by), "peak_source": hbm_src}
+        fb_bytes = algorithmic_bytes("rhs", n, nnz_mean, dim) + algorithmic_bytes("vjp", n, nnz_mean, dim)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": wl.name, "n_particles": n, "dim": dim, "nnz_exact_list": int(nnz_last),
+                       "nnz_skin_list": int(nnz_rk_last), "skin": SKIN, "replicas": world,
+                       "step": "build_cells+neighbors, density, rhs, rhs_vjp, rk_step(rebuild + 4 rhs)",
+                       "l2": "inputs larger than L2: every pair pass streams the 0.8-1.0 GB CSR (L2 = 126 MB)"},
+            "ms_fwd_bwd": fb_ms, "pairs_per_s_fwd_bwd": 2.0 * nnz_mean / (fb_ms * 1e-3),
+            "hbm_frac_fwd_bwd": fb_bytes / (fb_ms * 1e-3) / 1e9 / hbm,
+            "hbm_frac_fwd_bwd_of_8TBs": fb_bytes / (fb_ms * 1e-3) / 1e9 / 8000.0,
+            "phase_ms": ph_ms, "kernels": kern,
+            "roofline": roof[dom_cls], "roofline_all": roof,
+            "gpu_launches": int(launches), "clocks": clk,
+        }
+        if e2e:
+            line["e2e"] = e2e
+        if world == 1 and not args.no_cpu:
+            wl0 = make_workload(args.config, 0, args.n_axis)
+            line["cpu_baseline"], _ = cpu_sample(wl0, args.cpu_budget)
+        print(json.dumps(line))
+    sph.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -134,6 +134,16 @@ int sph_forward_backward_host(sph_ctx *ctx, const sph_domain *dom, const sph_par
                               float *drho_dt, float *acc, float *x_bar, float *v_bar, float *rho_bar,
                               float *params_bar, int64_t *nnz_out);
 
+/* End-to-end call of ONE WHOLE STEP of the hot path with HOST buffers (all SURVEY.md 8(a) rows): copies the state and
+ * the cotangents to the device, then sph_build_cells + sph_neighbors(1) + sph_density + sph_rhs + sph_rhs_vjp on the
+ * grid of `dom`, then sph_rk_step(dt, skin) on the grid of `dom_rk` (cell_size >= (1+skin) max h), copies every result
+ * back and synchronises.  x, v, rho are advanced IN PLACE (host); the other outputs may be NULL (skipped).
+ * nnz_out[2] (host): entries of the two lists (exact radius; skin radius). */
+int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_domain *dom_rk, const sph_params *par, float dt,
+                  float skin, int64_t n, float *x, float *v, float *rho, const float *m, const float *h,
+                  const uint8_t *kind, const float *drho_bar, const float *acc_bar, float *density, float *drho_dt,
+                  float *acc, float *x_bar, float *v_bar, float *rho_bar, float *params_bar, int64_t *nnz_out);
+
 /* Fetch the device-side error flag (synchronises the context's last stream). */
 int sph_check(sph_ctx *ctx);
 const char *sph_strerror(int code);
@@ -141,6 +151,29 @@ const char *sph_strerror(int code);
 /* Introspection for tests / bench (host values of the last build): grid size per axis, nnz, number of kernels
  * launched by this context since creation. */
 int sph_get_info(sph_ctx *ctx, int32_t ncell[3], int64_t *n, int64_t *nnz, int64_t *launches);
+
+/* Per-kernel-class device timing for the roofline report (bench.py): when enabled, every launch (group) of a class
+ * is bracketed by two CUDA events on the launching stream.  sph_profile_read synchronises the device, adds the
+ * resolved durations to ms_sum[SPH_K_NCLASS] (milliseconds) and the launch counts to launches[SPH_K_NCLASS]
+ * (both host arrays, may be NULL), then clears the accumulators.  Classes follow SURVEY.md 8(a). */
+enum {
+    SPH_K_KEY = 0,   /* N1 wrap + cell key */
+    SPH_K_SORT,      /* N2 radix passes (histogram, scan, scatter) */
+    SPH_K_REORDER,   /* N3 + N4 sorted SoA, cell ranges */
+    SPH_K_COUNT,     /* N5 */
+    SPH_K_SCAN,      /* N6 */
+    SPH_K_FILL,      /* N7 */
+    SPH_K_EXPORT,    /* lists in caller ids */
+    SPH_K_DENSITY,   /* D */
+    SPH_K_PACK,      /* R0 gather into sorted SoA + EOS prologue, cotangent pack */
+    SPH_K_RHS,       /* R1 pair loop */
+    SPH_K_VJP,       /* B1 pair loop */
+    SPH_K_REDUCE,    /* B2 */
+    SPH_K_RK,        /* T stage updates (axpy) and adjoint bookkeeping */
+    SPH_K_NCLASS
+};
+int sph_profile_enable(sph_ctx *ctx, int on);
+int sph_profile_read(sph_ctx *ctx, double *ms_sum, int64_t *launches);
 
 #ifdef __cplusplus
 }

@@ -16,8 +16,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsph_b200.so")
 
 EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph_neighbors_export", "sph_density",
-           "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_check",
-           "sph_strerror", "sph_get_info")
+           "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
+           "sph_check", "sph_strerror", "sph_get_info", "sph_profile_enable", "sph_profile_read")
+
+# kernel classes of sph_profile_read (enum SPH_K_* in include/sph.h)
+KERNEL_CLASSES = ("key", "sort", "reorder", "count", "scan", "fill", "export", "density", "pack", "rhs", "vjp",
+                  "reduce", "rk")
 
 
 class SphDomain(C.Structure):
@@ -62,6 +66,10 @@ def load_library(path: str = LIB_PATH):
     lib.sph_rk_step_vjp.argtypes = [vp, C.POINTER(SphDomain), C.POINTER(SphParams), f32, f32, i64] + [vp] * 10 + [vp]
     lib.sph_forward_backward_host.argtypes = [vp, C.POINTER(SphDomain), C.POINTER(SphParams), f32, i64] + [vp] * 14 + \
                                              [C.POINTER(i64)]
+    lib.sph_step_host.argtypes = [vp, C.POINTER(SphDomain), C.POINTER(SphDomain), C.POINTER(SphParams), f32, f32, i64] + \
+                                 [vp] * 15 + [C.POINTER(i64)]
+    lib.sph_profile_enable.argtypes = [vp, C.c_int]
+    lib.sph_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
     lib.sph_check.argtypes = [vp]
     lib.sph_strerror.argtypes = [C.c_int]
     lib.sph_strerror.restype = C.c_char_p
@@ -226,6 +234,40 @@ class Sph:
             hp(outs["rho_bar"]), hp(outs["params_bar"]), C.byref(nnz)))
         self.n, self.dim, self.nnz = n, dim, int(nnz.value)
         return outs
+
+    def step_host(self, domain, domain_rk, params, dt, skin, x, v, rho, m, h, kind, drho_bar, acc_bar, outs):
+        """One whole step of the hot path on HOST arrays (pinned torch CPU tensors or numpy); x, v, rho are advanced in
+        place; ``outs`` maps density, drho_dt, acc, x_bar, v_bar, rho_bar, params_bar to host arrays (or None)."""
+        d, drk, p = make_domain(domain), make_domain(domain_rk), make_params(params)
+        n = int(x.shape[0])
+
+        def hp(a):
+            if a is None:
+                return None
+            if isinstance(a, torch.Tensor):
+                assert not a.is_cuda and a.is_contiguous()
+                return C.c_void_p(a.data_ptr())
+            assert a.flags["C_CONTIGUOUS"]
+            return a.ctypes.data_as(C.c_void_p)
+
+        nnz = (C.c_int64 * 2)()
+        self._chk(self.lib.sph_step_host(
+            self._ctx, C.byref(d), C.byref(drk), C.byref(p), float(dt), float(skin), n, hp(x), hp(v), hp(rho), hp(m),
+            hp(h), hp(kind), hp(drho_bar), hp(acc_bar), hp(outs.get("density")), hp(outs.get("drho_dt")),
+            hp(outs.get("acc")), hp(outs.get("x_bar")), hp(outs.get("v_bar")), hp(outs.get("rho_bar")),
+            hp(outs.get("params_bar")), C.cast(nnz, C.POINTER(C.c_int64))))
+        self.n, self.dim = n, int(domain.dim)
+        return int(nnz[0]), int(nnz[1])
+
+    def profile_enable(self, on=True):
+        self._chk(self.lib.sph_profile_enable(self._ctx, 1 if on else 0))
+
+    def profile_read(self):
+        """{class: (ms_sum, launches)} since the last read (synchronises the device)"""
+        k = len(KERNEL_CLASSES)
+        ms, cnt = (C.c_double * k)(), (C.c_int64 * k)()
+        self._chk(self.lib.sph_profile_read(self._ctx, C.cast(ms, C.POINTER(C.c_double)), C.cast(cnt, C.POINTER(C.c_int64))))
+        return {name: (float(ms[i]), int(cnt[i])) for i, name in enumerate(KERNEL_CLASSES)}
 
     def check(self):
         self._chk(self.lib.sph_check(self._ctx))

@@ -36,10 +36,15 @@ extern "C" int sph_destroy(sph_ctx *ctx)
                       &ctx->row_ptr, &ctx->col, &ctx->scan_tmp, &ctx->s0, &ctx->s1, &ctx->s2, &ctx->s3, &ctx->c0buf,
                       &ctx->out4, &ctx->m_s, &ctx->kind_s, &ctx->partials, &ctx->eos, &ctx->hx, &ctx->hv, &ctx->hrho,
                       &ctx->hm, &ctx->hh, &ctx->hkind, &ctx->hlam, &ctx->hmu, &ctx->ho_drho, &ctx->ho_acc, &ctx->ho_xb,
-                      &ctx->ho_vb, &ctx->ho_rb, &ctx->ho_pb};
+                      &ctx->ho_vb, &ctx->ho_rb, &ctx->ho_pb, &ctx->ho_dens};
     for (DevBuf *b : bufs) b->release();
     for (auto &b : ctx->rk) b.release();
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
+    for (const ProfRec &r : ctx->prof.live) {
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    for (cudaEvent_t e : ctx->prof.pool) cudaEventDestroy(e);
     (void)cudaGetLastError();
     delete ctx;
     return SPH_OK;
@@ -118,5 +123,92 @@ extern "C" int sph_forward_backward_host(sph_ctx *ctx, const sph_domain *dom, co
     if (rho_bar) SPH_CUDA_TRY(cudaMemcpyAsync(rho_bar, ctx->ho_rb.p, ns, cudaMemcpyDeviceToHost, st));
     if (params_bar) SPH_CUDA_TRY(cudaMemcpyAsync(params_bar, ctx->ho_pb.p, 40, cudaMemcpyDeviceToHost, st));
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
+    return SPH_OK;
+}
+
+extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_domain *dom_rk, const sph_params *par,
+                             float dt, float skin, int64_t n, float *x, float *v, float *rho, const float *m,
+                             const float *h, const uint8_t *kind, const float *drho_bar, const float *acc_bar,
+                             float *density, float *drho_dt, float *acc, float *x_bar, float *v_bar, float *rho_bar,
+                             float *params_bar, int64_t *nnz_out)
+{
+    if (!ctx || !dom || !dom_rk || !par || n <= 0 || !x || !v || !rho || !m || !h || !kind || !drho_bar || !acc_bar)
+        return SPH_E_INVALID;
+    if ((dom->dim != 2 && dom->dim != 3) || dom_rk->dim != dom->dim) return SPH_E_INVALID;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = nullptr;
+    sph_stream_t ss = (sph_stream_t)st;
+    const size_t nv = (size_t)n * dom->dim * 4, ns = (size_t)n * 4;
+    SPH_TRY(ctx->hx.reserve(nv));  SPH_TRY(ctx->hv.reserve(nv));  SPH_TRY(ctx->hrho.reserve(ns));
+    SPH_TRY(ctx->hm.reserve(ns));  SPH_TRY(ctx->hh.reserve(ns));  SPH_TRY(ctx->hkind.reserve((size_t)n));
+    SPH_TRY(ctx->hlam.reserve(ns)); SPH_TRY(ctx->hmu.reserve(nv));
+    SPH_TRY(ctx->ho_drho.reserve(ns)); SPH_TRY(ctx->ho_acc.reserve(nv)); SPH_TRY(ctx->ho_xb.reserve(nv));
+    SPH_TRY(ctx->ho_vb.reserve(nv)); SPH_TRY(ctx->ho_rb.reserve(ns)); SPH_TRY(ctx->ho_pb.reserve(64));
+    SPH_TRY(ctx->ho_dens.reserve(ns));
+    float *dx = ctx->hx.as<float>(), *dv = ctx->hv.as<float>(), *dr = ctx->hrho.as<float>(), *dm = ctx->hm.as<float>();
+    float *dh = ctx->hh.as<float>();
+    uint8_t *dk = ctx->hkind.as<uint8_t>();
+    SPH_CUDA_TRY(cudaMemcpyAsync(dx, x, nv, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(dv, v, nv, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(dr, rho, ns, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(dm, m, ns, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(dh, h, ns, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(dk, kind, (size_t)n, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hlam.p, drho_bar, ns, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hmu.p, acc_bar, nv, cudaMemcpyHostToDevice, st));
+    int64_t nnz0 = 0;
+    SPH_TRY(sph_build_cells(ctx, dom, dx, dh, n, ss));
+    SPH_TRY(sph_neighbors(ctx, 1.0f, &nnz0, ss));
+    SPH_TRY(sph_density(ctx, dm, ctx->ho_dens.as<float>(), ss));
+    SPH_TRY(sph_rhs(ctx, par, dx, dv, dr, dm, dk, ctx->ho_drho.as<float>(), ctx->ho_acc.as<float>(), ss));
+    SPH_TRY(sph_rhs_vjp(ctx, par, dx, dv, dr, dm, dk, ctx->hlam.as<float>(), ctx->hmu.as<float>(), ctx->ho_xb.as<float>(),
+                        ctx->ho_vb.as<float>(), ctx->ho_rb.as<float>(), ctx->ho_pb.as<float>(), ss));
+    if (density) SPH_CUDA_TRY(cudaMemcpyAsync(density, ctx->ho_dens.p, ns, cudaMemcpyDeviceToHost, st));
+    if (drho_dt) SPH_CUDA_TRY(cudaMemcpyAsync(drho_dt, ctx->ho_drho.p, ns, cudaMemcpyDeviceToHost, st));
+    if (acc) SPH_CUDA_TRY(cudaMemcpyAsync(acc, ctx->ho_acc.p, nv, cudaMemcpyDeviceToHost, st));
+    if (x_bar) SPH_CUDA_TRY(cudaMemcpyAsync(x_bar, ctx->ho_xb.p, nv, cudaMemcpyDeviceToHost, st));
+    if (v_bar) SPH_CUDA_TRY(cudaMemcpyAsync(v_bar, ctx->ho_vb.p, nv, cudaMemcpyDeviceToHost, st));
+    if (rho_bar) SPH_CUDA_TRY(cudaMemcpyAsync(rho_bar, ctx->ho_rb.p, ns, cudaMemcpyDeviceToHost, st));
+    if (params_bar) SPH_CUDA_TRY(cudaMemcpyAsync(params_bar, ctx->ho_pb.p, 40, cudaMemcpyDeviceToHost, st));
+    SPH_TRY(sph_rk_step(ctx, dom_rk, par, dt, skin, n, dx, dv, dr, dm, dh, dk, ss));
+    if (nnz_out) {
+        nnz_out[0] = nnz0;
+        nnz_out[1] = ctx->nnz;
+    }
+    SPH_CUDA_TRY(cudaMemcpyAsync(x, dx, nv, cudaMemcpyDeviceToHost, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(v, dv, nv, cudaMemcpyDeviceToHost, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(rho, dr, ns, cudaMemcpyDeviceToHost, st));
+    SPH_CUDA_TRY(cudaStreamSynchronize(st));
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------------------------------ profiling
+extern "C" int sph_profile_enable(sph_ctx *ctx, int on)
+{
+    if (!ctx) return SPH_E_INVALID;
+    ctx->prof.on = on != 0;
+    return SPH_OK;
+}
+
+extern "C" int sph_profile_read(sph_ctx *ctx, double *ms_sum, int64_t *launches)
+{
+    if (!ctx) return SPH_E_INVALID;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    SPH_CUDA_TRY(cudaDeviceSynchronize());
+    Profiler &pf = ctx->prof;
+    for (const ProfRec &r : pf.live) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) pf.ms[r.cls] += (double)ms;
+        else (void)cudaGetLastError();
+        pf.pool.push_back(r.a);
+        pf.pool.push_back(r.b);
+    }
+    pf.live.clear();
+    for (int k = 0; k < SPH_K_NCLASS; ++k) {
+        if (ms_sum) ms_sum[k] = pf.ms[k];
+        if (launches) launches[k] = pf.count[k];
+        pf.ms[k] = 0.0;
+        pf.count[k] = 0;
+    }
     return SPH_OK;
 }

@@ -251,7 +251,7 @@ int sph_scan_u32(sph_ctx *ctx, const uint32_t *in, void *out, bool out64, int64_
         k_scan_apply<long long><<<(unsigned)nb, kScanThreads, 0, st>>>(in, (long long *)out, m, sums, 1);
     else
         k_scan_apply<uint32_t><<<(unsigned)nb, kScanThreads, 0, st>>>(in, (uint32_t *)out, m, sums, 0);
-    ctx->launches += 3;
+    // three launches; counted by the caller's KScope
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
@@ -337,8 +337,10 @@ extern "C" int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float 
     SPH_CUDA_TRY(cudaMemsetAsync(ctx->cell_end.p, 0, (size_t)ncells * 4, st));
 
     const unsigned nblk = (unsigned)((n + kThreads - 1) / kThreads);
-    k_wrap_key<<<nblk, kThreads, 0, st>>>(x, h, n, gg, ctx->key_a.as<uint32_t>(), ctx->stats.as<uint32_t>());
-    ctx->launches += 1;
+    {
+        KScope ks(ctx, SPH_K_KEY, 1, st);
+        k_wrap_key<<<nblk, kThreads, 0, st>>>(x, h, n, gg, ctx->key_a.as<uint32_t>(), ctx->stats.as<uint32_t>());
+    }
 
     // LSD radix passes over the used key bits
     const int keybits = gg.bits * gg.dim;
@@ -348,11 +350,10 @@ extern "C" int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float 
     uint32_t *vother = ctx->idx_a.as<uint32_t>();
     const unsigned rblk = (unsigned)((nchunks + kRsWarps - 1) / kRsWarps);
     for (int p = 0; p < passes; ++p) {
+        KScope ks(ctx, SPH_K_SORT, 5, st);
         k_radix_hist<<<rblk, kRsWarps * 32, 0, st>>>(kin, n, 8 * p, nchunks, ctx->hist.as<uint32_t>());
-        ctx->launches += 1;
         SPH_TRY(sph_scan_u32(ctx, ctx->hist.as<uint32_t>(), ctx->hist.p, false, nchunks * 256, st));
         k_radix_scatter<<<rblk, kRsWarps * 32, 0, st>>>(kin, vin, kout, vout, n, 8 * p, nchunks, ctx->hist.as<uint32_t>());
-        ctx->launches += 1;
         uint32_t *t = kin;
         kin = kout;
         kout = t;
@@ -362,11 +363,13 @@ extern "C" int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float 
     }
     // kin / vin now hold the sorted keys and the sorted caller indices
     SPH_TRY(ctx->key_sorted.reserve((size_t)n * 4));
-    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->key_sorted.p, kin, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
-    k_reorder<<<nblk, kThreads, 0, st>>>(x, h, n, gg, ctx->key_sorted.as<uint32_t>(), vin, ctx->perm.as<uint32_t>(),
-                                         ctx->inv_perm.as<uint32_t>(), ctx->pos_s.as<float4>(),
-                                         ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>());
-    ctx->launches += 1;
+    {
+        KScope ks(ctx, SPH_K_REORDER, 1, st);
+        SPH_CUDA_TRY(cudaMemcpyAsync(ctx->key_sorted.p, kin, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
+        k_reorder<<<nblk, kThreads, 0, st>>>(x, h, n, gg, ctx->key_sorted.as<uint32_t>(), vin, ctx->perm.as<uint32_t>(),
+                                             ctx->inv_perm.as<uint32_t>(), ctx->pos_s.as<float4>(),
+                                             ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>());
+    }
     SPH_CUDA_TRY(cudaGetLastError());
     ctx->cells_ready = true;
     return SPH_OK;

@@ -6,6 +6,8 @@
 #include <stdint.h>
 #include <string.h>
 
+#include <vector>
+
 #include "../../include/sph.h"
 
 #define SPH_CUDA_TRY(expr)                                   \
@@ -80,8 +82,34 @@ struct KPar {
     float H, invH, cW, cG, cK, ell, e2, eta, kd;
 };
 
+// Optional per-kernel-class device timing (sph_profile_enable / sph_profile_read): a pair of CUDA events on the
+// launching stream around every launch (or group of launches) of a class, resolved when read.
+struct ProfRec {
+    cudaEvent_t a, b;
+    int cls;
+};
+struct Profiler {
+    bool on = false;
+    std::vector<ProfRec> live;                                  // recorded, not yet resolved
+    std::vector<cudaEvent_t> pool;                              // free events
+    double ms[SPH_K_NCLASS] = {0};
+    int64_t count[SPH_K_NCLASS] = {0};
+    cudaEvent_t get()
+    {
+        if (!pool.empty()) {
+            cudaEvent_t e = pool.back();
+            pool.pop_back();
+            return e;
+        }
+        cudaEvent_t e = nullptr;
+        cudaEventCreate(&e);
+        return e;
+    }
+};
+
 struct sph_ctx {
     int device = 0;
+    Profiler prof;
     int64_t n_hint = 0;
     int64_t n = 0;
     bool cells_ready = false, lists_ready = false;
@@ -109,7 +137,33 @@ struct sph_ctx {
     // pinned host mirror
     int64_t *h_pinned = nullptr; // [8]
     // host staging for *_host call
-    DevBuf hx, hv, hrho, hm, hh, hkind, hlam, hmu, ho_drho, ho_acc, ho_xb, ho_vb, ho_rb, ho_pb;
+    DevBuf hx, hv, hrho, hm, hh, hkind, hlam, hmu, ho_drho, ho_acc, ho_xb, ho_vb, ho_rb, ho_pb, ho_dens;
+};
+
+// Counts `nlaunch` kernel launches of class `cls` and, when profiling is on, brackets them with events on `st`.
+struct KScope {
+    sph_ctx *ctx;
+    cudaStream_t st;
+    ProfRec rec{};
+    bool timed;
+    KScope(sph_ctx *c, int cls, int nlaunch, cudaStream_t s) : ctx(c), st(s), timed(c->prof.on)
+    {
+        ctx->launches += nlaunch;
+        ctx->prof.count[cls] += nlaunch;
+        if (timed) {
+            rec.a = ctx->prof.get();
+            rec.b = ctx->prof.get();
+            rec.cls = cls;
+            cudaEventRecord(rec.a, st);
+        }
+    }
+    ~KScope()
+    {
+        if (timed) {
+            cudaEventRecord(rec.b, st);
+            ctx->prof.live.push_back(rec);
+        }
+    }
 };
 
 // ------------------------------------------------------------------------------------------

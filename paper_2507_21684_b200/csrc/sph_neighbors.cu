@@ -189,20 +189,27 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
     SPH_TRY(ctx->cnt.reserve((size_t)n * 4));
     SPH_TRY(ctx->row_ptr.reserve((size_t)(n + 1) * 8));
     const unsigned nblk = (unsigned)((n + kWarpsPerBlock - 1) / kWarpsPerBlock);
-    k_neighbors<false><<<nblk, kWarpsPerBlock * 32, 0, st>>>(n, gg, sp, ctx->pos_s.as<float4>(),
-                                                            ctx->key_sorted.as<uint32_t>(), ctx->cell_start.as<uint32_t>(),
-                                                            ctx->cell_end.as<uint32_t>(), ctx->cnt.as<uint32_t>(), nullptr, nullptr);
-    ctx->launches += 1;
-    SPH_TRY(sph_scan_u32(ctx, ctx->cnt.as<uint32_t>(), ctx->row_ptr.p, true, n, st));
+    {
+        KScope ks(ctx, SPH_K_COUNT, 1, st);
+        k_neighbors<false><<<nblk, kWarpsPerBlock * 32, 0, st>>>(n, gg, sp, ctx->pos_s.as<float4>(),
+                                                                ctx->key_sorted.as<uint32_t>(), ctx->cell_start.as<uint32_t>(),
+                                                                ctx->cell_end.as<uint32_t>(), ctx->cnt.as<uint32_t>(), nullptr, nullptr);
+    }
+    {
+        KScope ks(ctx, SPH_K_SCAN, 3, st);
+        SPH_TRY(sph_scan_u32(ctx, ctx->cnt.as<uint32_t>(), ctx->row_ptr.p, true, n, st));
+    }
     SPH_CUDA_TRY(cudaMemcpyAsync(ctx->h_pinned + 4, ctx->row_ptr.as<long long>() + n, 8, cudaMemcpyDeviceToHost, st));
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
     const int64_t nnz = ctx->h_pinned[4];
     SPH_TRY(ctx->col.reserve((size_t)(nnz > 0 ? nnz : 1) * 4));
-    k_neighbors<true><<<nblk, kWarpsPerBlock * 32, 0, st>>>(n, gg, sp, ctx->pos_s.as<float4>(),
-                                                           ctx->key_sorted.as<uint32_t>(), ctx->cell_start.as<uint32_t>(),
-                                                           ctx->cell_end.as<uint32_t>(), nullptr, ctx->row_ptr.as<long long>(),
-                                                           ctx->col.as<int32_t>());
-    ctx->launches += 1;
+    {
+        KScope ks(ctx, SPH_K_FILL, 1, st);
+        k_neighbors<true><<<nblk, kWarpsPerBlock * 32, 0, st>>>(n, gg, sp, ctx->pos_s.as<float4>(),
+                                                               ctx->key_sorted.as<uint32_t>(), ctx->cell_start.as<uint32_t>(),
+                                                               ctx->cell_end.as<uint32_t>(), nullptr, ctx->row_ptr.as<long long>(),
+                                                               ctx->col.as<int32_t>());
+    }
     SPH_CUDA_TRY(cudaGetLastError());
     ctx->nnz = nnz;
     ctx->search_scale = search_scale;
@@ -221,13 +228,12 @@ extern "C" int sph_neighbors_export(sph_ctx *ctx, int64_t *row_ptr, int32_t *col
     const int64_t n = ctx->n;
     SPH_TRY(ctx->s3.reserve((size_t)n * 4));
     uint32_t *cnt_c = ctx->s3.as<uint32_t>();
+    KScope ks(ctx, SPH_K_EXPORT, 5, st);
     k_export_counts<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, ctx->inv_perm.as<uint32_t>(), ctx->cnt.as<uint32_t>(), cnt_c);
-    ctx->launches += 1;
     SPH_TRY(sph_scan_u32(ctx, cnt_c, row_ptr, true, n, st));
     k_export_rows<<<(unsigned)((n + kWarpsPerBlock - 1) / kWarpsPerBlock), kWarpsPerBlock * 32, 0, st>>>(
         n, ctx->inv_perm.as<uint32_t>(), ctx->perm.as<uint32_t>(), ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>(),
         (const long long *)row_ptr, col_idx);
-    ctx->launches += 1;
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

@@ -529,10 +529,10 @@ int pack_state(sph_ctx *ctx, const KPar &kp, const float *x, const float *v, con
     SPH_TRY(ctx->s2.reserve((size_t)n * 8));
     SPH_TRY(ctx->kind_s.reserve((size_t)n));
     if (with_eos) SPH_TRY(ctx->eos.reserve((size_t)n * 16));
+    KScope ks(ctx, SPH_K_PACK, 1, st);
     k_pack_state<DIM><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
         n, kp, ctx->perm.as<uint32_t>(), ctx->pos_s.as<float4>(), x, v, rho, m, kind, ctx->s0.as<float4>(),
         ctx->s1.as<float4>(), ctx->s2.as<float2>(), with_eos ? ctx->eos.as<float4>() : nullptr, ctx->kind_s.as<uint8_t>());
-    ctx->launches += 1;
     return SPH_OK;
 }
 
@@ -548,6 +548,7 @@ int sph_launch_rhs_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
     const int32_t *col = ctx->col.as<int32_t>();
     const uint32_t *perm = ctx->perm.as<uint32_t>();
     const bool sorted = out4 != nullptr;
+    KScope ks(ctx, SPH_K_RHS, 1, st);
 #define SPH_RHS_LAUNCH(DIM, GS, VARH, SORTED)                                                                     \
     k_rhs<DIM, GS, VARH, SORTED><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, s0, s1, s2, kind_s, rp, col, \
                                                                      perm, drho, acc, out4)
@@ -559,7 +560,6 @@ int sph_launch_rhs_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
         else { if (sorted) SPH_RHS_LAUNCH(2, 16, true, true); else SPH_RHS_LAUNCH(2, 16, true, false); }
     }
 #undef SPH_RHS_LAUNCH
-    ctx->launches += 1;
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
@@ -578,6 +578,8 @@ int sph_launch_vjp_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
     const unsigned grid = pair_grid(n, gs);
     SPH_TRY(ctx->partials.reserve((size_t)grid * kNPart * 4));
     float *part = ctx->partials.as<float>();
+    {
+    KScope ks(ctx, SPH_K_VJP, 1, st);
 #define SPH_VJP_LAUNCH(DIM, GS, VARH, SORTED)                                                                  \
     k_vjp<DIM, GS, VARH, SORTED><<<grid, kBlock, 0, st>>>(n, kp, margin, s0, s1, s2, cot, eos, rp, col, perm, xb, \
                                                          vb, rb, xb4, vb4, part)
@@ -589,10 +591,10 @@ int sph_launch_vjp_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
         else { if (sorted) SPH_VJP_LAUNCH(2, 16, true, true); else SPH_VJP_LAUNCH(2, 16, true, false); }
     }
 #undef SPH_VJP_LAUNCH
-    ctx->launches += 1;
+    }
     if (params_bar) {
+        KScope ks(ctx, SPH_K_REDUCE, 1, st);
         k_reduce_params<<<1, 128, 0, st>>>((int64_t)grid, part, kp, accumulate_params, params_bar);
-        ctx->launches += 1;
     }
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
@@ -611,6 +613,7 @@ extern "C" int sph_density(sph_ctx *ctx, const float *m, float *rho_out, sph_str
     KPar kp;
     SPH_TRY(sph_kpar_make(ctx, &dummy, &kp));
     SPH_TRY(ctx->m_s.reserve((size_t)n * 4));
+    KScope ks(ctx, SPH_K_DENSITY, 2, st);
     k_gather_f32<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), m, ctx->m_s.as<float>());
     const float margin = seam_margin(ctx);
 #define SPH_DENS_LAUNCH(DIM, GS, VARH)                                                                               \
@@ -620,7 +623,6 @@ extern "C" int sph_density(sph_ctx *ctx, const float *m, float *rho_out, sph_str
     if (kp.dim == 3) { if (kp.uniform_h) SPH_DENS_LAUNCH(3, 32, false); else SPH_DENS_LAUNCH(3, 32, true); }
     else { if (kp.uniform_h) SPH_DENS_LAUNCH(2, 16, false); else SPH_DENS_LAUNCH(2, 16, true); }
 #undef SPH_DENS_LAUNCH
-    ctx->launches += 2;
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
@@ -657,9 +659,11 @@ extern "C" int sph_rhs_vjp(sph_ctx *ctx, const sph_params *par, const float *x, 
     if (kp.dim == 3) SPH_TRY(pack_state<3>(ctx, kp, x, v, rho, m, kind, true, st));
     else SPH_TRY(pack_state<2>(ctx, kp, x, v, rho, m, kind, true, st));
     SPH_TRY(ctx->c0buf.reserve((size_t)n * 16));
-    k_pack_cot<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, kp.dim, ctx->perm.as<uint32_t>(), ctx->kind_s.as<uint8_t>(),
-                                                            drho_bar, acc_bar, ctx->c0buf.as<float4>());
-    ctx->launches += 1;
+    {
+        KScope ks(ctx, SPH_K_PACK, 1, st);
+        k_pack_cot<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, kp.dim, ctx->perm.as<uint32_t>(), ctx->kind_s.as<uint8_t>(),
+                                                                drho_bar, acc_bar, ctx->c0buf.as<float4>());
+    }
     return sph_launch_vjp_sorted(ctx, kp, ctx->s0.as<float4>(), ctx->s1.as<float4>(), ctx->s2.as<float2>(),
                                  ctx->c0buf.as<float4>(), ctx->eos.as<float4>(), x_bar, v_bar, rho_bar, nullptr, nullptr,
                                  params_bar, 0, st);

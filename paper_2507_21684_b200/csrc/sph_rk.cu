@@ -238,28 +238,32 @@ extern "C" int sph_rk_step(sph_ctx *ctx, const sph_domain *dom, const sph_params
     uint8_t *kind_s = ctx->kind_s.as<uint8_t>();
     float *m_s = ctx->m_s.as<float>();
 
+    {
+    KScope ks(ctx, SPH_K_RK, 1, st);
     if (kp.dim == 3)
         k_rk_base<3><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), v, rho, m, kind, b0, b1, m_s, kind_s, sb);
     else
         k_rk_base<2><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), v, rho, m, kind, b0, b1, m_s, kind_s, sb);
-    ctx->launches += 1;
+    }
     const float c[4] = {0.f, 0.5f, 0.5f, 1.f};
     const float b[4] = {1.f / 6.f, 1.f / 3.f, 1.f / 3.f, 1.f / 6.f};
     for (int s = 0; s < 4; ++s) {
         if (s > 0) {
+            KScope ks(ctx, SPH_K_RK, 1, st);
             if (kp.dim == 3)
                 k_rk_stage<3><<<nb(n), 256, 0, st>>>(n, kp, c[s] * dt, b[s - 1], s == 1, b0, b1, m_s, kind_s, k4, sb, sb, accx, accv);
             else
                 k_rk_stage<2><<<nb(n), 256, 0, st>>>(n, kp, c[s] * dt, b[s - 1], s == 1, b0, b1, m_s, kind_s, k4, sb, sb, accx, accv);
-            ctx->launches += 1;
         }
         SPH_TRY(sph_launch_rhs_sorted(ctx, kp, sb.s0, sb.s1, sb.s2, kind_s, nullptr, nullptr, k4, st));
     }
+    {
+    KScope ks(ctx, SPH_K_RK, 1, st);
     if (kp.dim == 3)
         k_rk_final<3><<<nb(n), 256, 0, st>>>(n, dt, b[3], perm, kind_s, k4, sb, accx, accv, x, v, rho);
     else
         k_rk_final<2><<<nb(n), 256, 0, st>>>(n, dt, b[3], perm, kind_s, k4, sb, accx, accv, x, v, rho);
-    ctx->launches += 1;
+    }
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
@@ -307,34 +311,47 @@ extern "C" int sph_rk_step_vjp(sph_ctx *ctx, const sph_domain *dom, const sph_pa
     const float b[4] = {1.f / 6.f, 1.f / 3.f, 1.f / 3.f, 1.f / 6.f};
 
     // forward sweep: recompute and keep the four stage states
+    {
+    KScope ks(ctx, SPH_K_RK, 1, st);
     if (kp.dim == 3)
         k_rk_base<3><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), v0, rho0_state, m, kind, b0, b1, m_s, kind_s, S[0]);
     else
         k_rk_base<2><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), v0, rho0_state, m, kind, b0, b1, m_s, kind_s, S[0]);
-    ctx->launches += 1;
+    }
     for (int s = 1; s < 4; ++s) {
         SPH_TRY(sph_launch_rhs_sorted(ctx, kp, S[s - 1].s0, S[s - 1].s1, S[s - 1].s2, kind_s, nullptr, nullptr, k4, st));
+        {
+        KScope ks(ctx, SPH_K_RK, 1, st);
         if (kp.dim == 3)
             k_rk_stage<3><<<nb(n), 256, 0, st>>>(n, kp, c[s] * dt, b[s - 1], s == 1, b0, b1, m_s, kind_s, k4, S[s - 1], S[s], accx, accv);
         else
             k_rk_stage<2><<<nb(n), 256, 0, st>>>(n, kp, c[s] * dt, b[s - 1], s == 1, b0, b1, m_s, kind_s, k4, S[s - 1], S[s], accx, accv);
-        ctx->launches += 1;
+        }
     }
     // reverse sweep
+    {
+    KScope ks(ctx, SPH_K_RK, 1, st);
     if (kp.dim == 3) k_adj_gather<3><<<nb(n), 256, 0, st>>>(n, perm, x_bar, v_bar, rho_bar, yx, yv);
     else k_adj_gather<2><<<nb(n), 256, 0, st>>>(n, perm, x_bar, v_bar, rho_bar, yx, yv);
-    ctx->launches += 1;
+    }
     for (int s = 3; s >= 0; --s) {
         const float adt = s == 3 ? 0.f : c[s + 1] * dt;      // a_{s+1,s} = c_{s+1} in the classic tableau
-        k_adj_cot<<<nb(n), 256, 0, st>>>(n, b[s] * dt, adt, kind_s, yx, yv, Yx, Yv, cot, kbx);
+        {
+            KScope ks(ctx, SPH_K_RK, 1, st);
+            k_adj_cot<<<nb(n), 256, 0, st>>>(n, b[s] * dt, adt, kind_s, yx, yv, Yx, Yv, cot, kbx);
+        }
         SPH_TRY(sph_launch_vjp_sorted(ctx, kp, S[s].s0, S[s].s1, S[s].s2, cot, S[s].eos, nullptr, nullptr, nullptr, Yx, Yv,
                                       params_bar, 1, st));
-        k_adj_fix<<<nb(n), 256, 0, st>>>(n, s == 3, kbx, Yx, Yv, sumx, sumv);
-        ctx->launches += 2;
+        {
+            KScope ks(ctx, SPH_K_RK, 1, st);
+            k_adj_fix<<<nb(n), 256, 0, st>>>(n, s == 3, kbx, Yx, Yv, sumx, sumv);
+        }
     }
+    {
+    KScope ks(ctx, SPH_K_RK, 1, st);
     if (kp.dim == 3) k_adj_final<3><<<nb(n), 256, 0, st>>>(n, perm, sumx, sumv, x_bar, v_bar, rho_bar);
     else k_adj_final<2><<<nb(n), 256, 0, st>>>(n, perm, sumx, sumv, x_bar, v_bar, rho_bar);
-    ctx->launches += 1;
+    }
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
