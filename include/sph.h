@@ -172,6 +172,11 @@ enum {
     SPH_K_RK,        /* T stage updates (axpy) and adjoint bookkeeping */
     SPH_K_NCLASS
 };
+/* Tuning knobs (results do not depend on them beyond summation order). */
+enum {
+    SPH_OPT_PAIR_GROUP = 1 /* lanes that share one row in the pair kernels: 4, 8, 16, 32; 0 = default */
+};
+int sph_set_option(sph_ctx *ctx, int key, int value);
 int sph_profile_enable(sph_ctx *ctx, int on);
 int sph_profile_read(sph_ctx *ctx, double *ms_sum, int64_t *launches);
 

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(HERE, "libsph_b200.so")
 
 EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph_neighbors_export", "sph_density",
            "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
-           "sph_check", "sph_strerror", "sph_get_info", "sph_profile_enable", "sph_profile_read")
+           "sph_check", "sph_strerror", "sph_get_info", "sph_profile_enable", "sph_profile_read", "sph_set_option")
 
 # kernel classes of sph_profile_read (enum SPH_K_* in include/sph.h)
 KERNEL_CLASSES = ("key", "sort", "reorder", "count", "scan", "fill", "export", "density", "pack", "rhs", "vjp",
@@ -69,6 +69,7 @@ def load_library(path: str = LIB_PATH):
     lib.sph_step_host.argtypes = [vp, C.POINTER(SphDomain), C.POINTER(SphDomain), C.POINTER(SphParams), f32, f32, i64] + \
                                  [vp] * 15 + [C.POINTER(i64)]
     lib.sph_profile_enable.argtypes = [vp, C.c_int]
+    lib.sph_set_option.argtypes = [vp, C.c_int, C.c_int]
     lib.sph_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
     lib.sph_check.argtypes = [vp]
     lib.sph_strerror.argtypes = [C.c_int]
@@ -258,6 +259,9 @@ class Sph:
             hp(outs.get("params_bar")), C.cast(nnz, C.POINTER(C.c_int64))))
         self.n, self.dim = n, int(domain.dim)
         return int(nnz[0]), int(nnz[1])
+
+    def set_option(self, key, value):
+        self._chk(self.lib.sph_set_option(self._ctx, int(key), int(value)))
 
     def profile_enable(self, on=True):
         self._chk(self.lib.sph_profile_enable(self._ctx, 1 if on else 0))

@@ -212,3 +212,16 @@ extern "C" int sph_profile_read(sph_ctx *ctx, double *ms_sum, int64_t *launches)
     }
     return SPH_OK;
 }
+
+extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
+{
+    if (!ctx) return SPH_E_INVALID;
+    switch (key) {
+    case SPH_OPT_PAIR_GROUP:
+        if (value != 0 && value != 4 && value != 8 && value != 16 && value != 32) return SPH_E_INVALID;
+        ctx->opt_group = value;
+        return SPH_OK;
+    default:
+        return SPH_E_INVALID;
+    }
+}

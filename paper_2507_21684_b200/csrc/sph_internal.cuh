@@ -110,6 +110,7 @@ struct Profiler {
 struct sph_ctx {
     int device = 0;
     Profiler prof;
+    int opt_group = 0;          // lanes per row in the pair kernels (0 = default)
     int64_t n_hint = 0;
     int64_t n = 0;
     bool cells_ready = false, lists_ready = false;

@@ -46,82 +46,237 @@ __device__ __forceinline__ bool pred_exact(const float4 &a, const float4 &b, flo
     return r2 < Hs2;
 }
 
-// fp32 decision when it is safe (|r2 - Hs^2| outside the rounding band), binary64 sequence otherwise
-__device__ __forceinline__ bool pred(const float4 &a, const float4 &b, const SearchPar &sp, const GridGeom &gg,
-                                     bool seam)
-{
-    float Hs = __fmul_rn(sp.scale, fmaxf(a.w, b.w));
-    float d0 = a.x - b.x, d1 = a.y - b.y, d2 = gg.dim == 3 ? a.z - b.z : 0.f;
-    if (seam) {
-        if (gg.periodic[0]) d0 = d0 > 0.5f * gg.L[0] ? d0 - gg.L[0] : (d0 < -0.5f * gg.L[0] ? d0 + gg.L[0] : d0);
-        if (gg.periodic[1]) d1 = d1 > 0.5f * gg.L[1] ? d1 - gg.L[1] : (d1 < -0.5f * gg.L[1] ? d1 + gg.L[1] : d1);
-        if (gg.dim == 3 && gg.periodic[2])
-            d2 = d2 > 0.5f * gg.L[2] ? d2 - gg.L[2] : (d2 < -0.5f * gg.L[2] ? d2 + gg.L[2] : d2);
-    }
-    float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
-    float Hs2 = Hs * Hs;
-    float tol = sp.band * (Hs2 + (seam ? Hs * sp.Lmax : 0.f));
-    float diff = r2 - Hs2;
-    if (fabsf(diff) > tol) return diff < 0.f;
-    return pred_exact(a, b, Hs, gg);
-}
+// ---------------------------------------------------------------------------------------- tile search
+// One CTA owns a block of B^d cells.  It stages the particles of the (B+2)^d halo cells into shared memory
+// (contiguous runs of the cell-sorted array; positions pre-shifted by +-L across a periodic seam, so the inner
+// loop needs no minimum image), then one warp per target row scans the 3^(d-1) x-runs of 3 adjacent cells that
+// make up the row's 3^d neighbour cells: 32 candidates per iteration from shared memory, ballot compaction.
+// The halo is processed in chunks of `cap` candidates, so any cell occupancy works; a block whose halo fits one
+// chunk (the normal case) keeps all row state in registers.
+struct TilePar {
+    int B;             // block edge in cells
+    int nb[3];         // blocks per axis
+    int cap;           // candidates per shared-memory chunk
+    int slow[3];       // periodic axis with fewer than B+2 cells: halo = all cells, minimum image in the loop
+};
 
-template <bool FILL>
+constexpr int kMaxHalo = 64;     // (B+2)^d <= 64: B = 2 in 3D, B <= 6 in 2D
+
+template <int DIM, bool FILL>
 __global__ void __launch_bounds__(kWarpsPerBlock * 32)
-k_neighbors(int64_t n, GridGeom gg, SearchPar sp, const float4 *__restrict__ pos_s,
-            const uint32_t *__restrict__ key_sorted, const uint32_t *__restrict__ cell_start,
-            const uint32_t *__restrict__ cell_end, uint32_t *__restrict__ cnt,
-            const long long *__restrict__ row_ptr, int32_t *__restrict__ col)
+k_neighbors_tile(int64_t n, GridGeom gg, SearchPar sp, TilePar tp, const float4 *__restrict__ pos_s,
+                 const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
+                 uint32_t *__restrict__ cnt, uint32_t *__restrict__ cursor, const long long *__restrict__ row_ptr,
+                 int32_t *__restrict__ col)
 {
-    const int lane = threadIdx.x & 31;
-    const int64_t row = (int64_t)blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
-    if (row >= n) return;
-    const float4 pi = pos_s[row];
-    const float xi[3] = {pi.x, pi.y, pi.z};
-    int clo[3] = {0, 0, 0}, chi[3] = {0, 0, 0};
-    bool seam = false;
-    for (int k = 0; k < gg.dim; ++k) {
-        // candidate interval [x - R, x + R]; the cell map is monotone, so every j with |d_k| < Hs lies in it
-        int a = cell_coord_raw(__dsub_rn((double)xi[k], sp.R), gg.lo_d[k], gg.edge[k]);
-        int b = cell_coord_raw(__dadd_rn((double)xi[k], sp.R), gg.lo_d[k], gg.edge[k]);
-        if (gg.periodic[k]) {
-            if (b - a + 1 > gg.ncell[k]) b = a + gg.ncell[k] - 1;   // never visit a cell twice
-            if (a < 0 || b >= gg.ncell[k]) seam = true;
-        } else {
-            a = max(a, 0);
-            b = min(b, gg.ncell[k] - 1);
-        }
-        clo[k] = a;
-        chi[k] = b;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float4 *cand = reinterpret_cast<float4 *>(smem_raw);
+    uint32_t *gidx = reinterpret_cast<uint32_t *>(smem_raw + (size_t)tp.cap * sizeof(float4));
+    __shared__ uint32_t h_off[kMaxHalo + 1];      // halo-linear offset of each halo cell
+    __shared__ uint32_t h_start[kMaxHalo];        // first sorted index of each halo cell
+    __shared__ uint32_t t_off[kMaxHalo + 1];      // target-row offsets (targets are halo cells too)
+    __shared__ int t_cell[kMaxHalo];              // halo cell id of each target cell
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int bc[3] = {0, 0, 0};
+    {
+        int b = blockIdx.x;
+        bc[0] = b % tp.nb[0];
+        b /= tp.nb[0];
+        bc[1] = b % tp.nb[1];
+        bc[2] = b / tp.nb[1];
     }
-    uint32_t off = 0;
-    const long long base = FILL ? row_ptr[row] : 0;
-    for (int cz = clo[2]; cz <= chi[2]; ++cz) {
-        int wz = cz;
-        if (gg.dim == 3 && gg.periodic[2]) wz = cz < 0 ? cz + gg.ncell[2] : (cz >= gg.ncell[2] ? cz - gg.ncell[2] : cz);
-        for (int cy = clo[1]; cy <= chi[1]; ++cy) {
-            int wy = cy;
-            if (gg.periodic[1]) wy = cy < 0 ? cy + gg.ncell[1] : (cy >= gg.ncell[1] ? cy - gg.ncell[1] : cy);
-            for (int cx = clo[0]; cx <= chi[0]; ++cx) {
-                int wx = cx;
-                if (gg.periodic[0]) wx = cx < 0 ? cx + gg.ncell[0] : (cx >= gg.ncell[0] ? cx - gg.ncell[0] : cx);
-                const int64_t lin = wx + (int64_t)gg.ncell[0] * (wy + (int64_t)gg.ncell[1] * wz);
-                const uint32_t s = cell_start[lin], e = cell_end[lin];
-                for (uint32_t b0 = s; b0 < e; b0 += 32) {
-                    const uint32_t j = b0 + lane;
-                    bool hit = false;
-                    if (j < e) {
-                        const float4 pj = pos_s[j];
-                        hit = pred(pi, pj, sp, gg, seam);
+    // halo extent per axis: hs = first (unwrapped) cell coordinate, ext = number of cells, tlo = slot of the first target
+    int hs[3] = {0, 0, 0}, ext[3] = {1, 1, 1}, tlo[3] = {0, 0, 0}, tn[3] = {1, 1, 1};
+    bool seam = false;
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+        const int c0 = bc[k] * tp.B;
+        tn[k] = min(tp.B, gg.ncell[k] - c0);
+        if (gg.periodic[k]) {
+            if (tp.slow[k]) {
+                hs[k] = 0;
+                ext[k] = gg.ncell[k];
+                seam = true;
+            } else {
+                hs[k] = c0 - 1;
+                ext[k] = tn[k] + 2;
+                if (hs[k] < 0 || hs[k] + ext[k] > gg.ncell[k]) seam = true;
+            }
+        } else {
+            hs[k] = max(c0 - 1, 0);
+            ext[k] = min(c0 + tn[k], gg.ncell[k] - 1) - hs[k] + 1;
+        }
+        tlo[k] = c0 - hs[k];
+    }
+    const int nh = ext[0] * ext[1] * ext[2];
+    const int nt = tn[0] * tn[1] * tn[2];
+
+    // ---- halo tables (warp 0: two cells per lane, warp scan)
+    if (warp == 0) {
+        uint32_t c2[2], s2[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int hc = lane * 2 + u;
+            c2[u] = 0;
+            s2[u] = 0;
+            if (hc < nh) {
+                int sl[3] = {hc % ext[0], (hc / ext[0]) % ext[1], hc / (ext[0] * ext[1])};
+                int64_t lin = 0;
+#pragma unroll
+                for (int k = DIM - 1; k >= 0; --k) {
+                    int c = hs[k] + sl[k];
+                    if (gg.periodic[k]) c = c < 0 ? c + gg.ncell[k] : (c >= gg.ncell[k] ? c - gg.ncell[k] : c);
+                    lin = lin * gg.ncell[k] + c;
+                }
+                s2[u] = cell_start[lin];
+                c2[u] = cell_end[lin] - s2[u];
+                h_start[hc] = s2[u];
+            }
+        }
+        uint32_t tot = c2[0] + c2[1], inc = tot;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        const uint32_t ex = inc - tot;
+        if (lane * 2 < nh) h_off[lane * 2] = ex;
+        if (lane * 2 + 1 < nh) h_off[lane * 2 + 1] = ex + c2[0];
+        if (lane == 31) h_off[nh] = inc;
+    }
+    __syncthreads();
+    if (warp == 1) {
+        // target cells in (z,y,x) order = ascending halo cell id; rows per target cell
+        uint32_t c2[2] = {0, 0};
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int tc = lane * 2 + u;
+            if (tc < nt) {
+                int sl[3] = {tc % tn[0], (tc / tn[0]) % tn[1], tc / (tn[0] * tn[1])};
+                const int hc = (tlo[0] + sl[0]) + ext[0] * ((tlo[1] + sl[1]) + ext[1] * (tlo[2] + sl[2]));
+                t_cell[tc] = hc;
+                c2[u] = h_off[hc + 1] - h_off[hc];
+            }
+        }
+        uint32_t tot = c2[0] + c2[1], inc = tot;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        const uint32_t ex = inc - tot;
+        if (lane * 2 < nt) t_off[lane * 2] = ex;
+        if (lane * 2 + 1 < nt) t_off[lane * 2 + 1] = ex + c2[0];
+        if (lane == 31) t_off[nt] = inc;
+    }
+    __syncthreads();
+    const uint32_t M = h_off[nh], T = t_off[nt];
+    if (T == 0) return;
+    const bool single = M <= (uint32_t)tp.cap;
+    const float tol_rel = sp.band;
+
+    for (uint32_t c0 = 0; c0 < M; c0 += (uint32_t)tp.cap) {
+        const uint32_t c1 = min(M, c0 + (uint32_t)tp.cap);
+        if (c0 > 0) __syncthreads();
+        // ---- stage the chunk [c0, c1) of the halo-linear candidate sequence
+        for (int hc = warp; hc < nh; hc += kWarpsPerBlock) {
+            const uint32_t o0 = h_off[hc], o1 = h_off[hc + 1];
+            if (o1 <= c0 || o0 >= c1) continue;
+            float sh[3] = {0.f, 0.f, 0.f};
+            {
+                int sl[3] = {hc % ext[0], (hc / ext[0]) % ext[1], hc / (ext[0] * ext[1])};
+#pragma unroll
+                for (int k = 0; k < DIM; ++k)
+                    if (gg.periodic[k] && !tp.slow[k]) {
+                        const int c = hs[k] + sl[k];
+                        sh[k] = c < 0 ? -gg.L[k] : (c >= gg.ncell[k] ? gg.L[k] : 0.f);
                     }
-                    const uint32_t m = __ballot_sync(0xffffffffu, hit);
-                    if (FILL && hit) col[base + off + __popc(m & ((1u << lane) - 1u))] = (int32_t)j;
-                    off += __popc(m);
+            }
+            const uint32_t gs = h_start[hc];
+            for (uint32_t q = max(o0, c0) + lane; q < min(o1, c1); q += 32) {
+                const uint32_t g = gs + (q - o0);
+                float4 pj = pos_s[g];
+                pj.x += sh[0];
+                pj.y += sh[1];
+                if (DIM == 3) pj.z += sh[2];
+                cand[q - c0] = pj;
+                gidx[q - c0] = g;
+            }
+        }
+        __syncthreads();
+        // ---- rows: one warp per target row
+        for (uint32_t t = warp; t < T; t += kWarpsPerBlock) {
+            int tc = 0;
+            while (t >= t_off[tc + 1]) ++tc;
+            const int hc_i = t_cell[tc];
+            const uint32_t row = h_start[hc_i] + (t - t_off[tc]);
+            const float4 pi = pos_s[row];
+            int sl[3] = {hc_i % ext[0], (hc_i / ext[0]) % ext[1], hc_i / (ext[0] * ext[1])};
+            uint32_t off = 0;
+            if (!single && c0 > 0) off = FILL ? cursor[row] : cnt[row];
+            const long long base = FILL ? row_ptr[row] : 0;
+            // neighbour cells of the row: dz, dy in {-1,0,1}; along x either one merged run or cell by cell
+            const int zlo = DIM == 3 ? -1 : 0, zhi = DIM == 3 ? 1 : 0;
+            for (int dz = zlo; dz <= zhi; ++dz) {
+                int sz = sl[2] + dz;
+                if (DIM == 3) {
+                    if (tp.slow[2]) sz = sz < 0 ? sz + ext[2] : (sz >= ext[2] ? sz - ext[2] : sz);
+                    else if (sz < 0 || sz >= ext[2]) continue;
+                }
+                for (int dy = -1; dy <= 1; ++dy) {
+                    int sy = sl[1] + dy;
+                    if (tp.slow[1]) sy = sy < 0 ? sy + ext[1] : (sy >= ext[1] ? sy - ext[1] : sy);
+                    else if (sy < 0 || sy >= ext[1]) continue;
+                    const int rowbase = ext[0] * (sy + ext[1] * sz);
+                    const int nrun = tp.slow[0] ? 3 : 1;
+                    for (int rr = 0; rr < nrun; ++rr) {
+                        int xa, xb;                       // first / last halo slot along x of this run
+                        if (tp.slow[0]) {
+                            int sx = sl[0] + rr - 1;
+                            sx = sx < 0 ? sx + ext[0] : (sx >= ext[0] ? sx - ext[0] : sx);
+                            xa = xb = sx;
+                        } else {
+                            xa = max(sl[0] - 1, 0);
+                            xb = min(sl[0] + 1, ext[0] - 1);
+                        }
+                        uint32_t q0 = max(h_off[rowbase + xa], c0), q1 = min(h_off[rowbase + xb + 1], c1);
+                        for (uint32_t qb = q0; qb < q1; qb += 32) {
+                            const uint32_t q = qb + lane;
+                            bool hit = false;
+                            uint32_t g = 0;
+                            if (q < q1) {
+                                const float4 pj = cand[q - c0];
+                                const float Hs = __fmul_rn(sp.scale, fmaxf(pi.w, pj.w));
+                                float d0 = pi.x - pj.x, d1 = pi.y - pj.y, d2 = DIM == 3 ? pi.z - pj.z : 0.f;
+                                if (tp.slow[0]) d0 = d0 > 0.5f * gg.L[0] ? d0 - gg.L[0] : (d0 < -0.5f * gg.L[0] ? d0 + gg.L[0] : d0);
+                                if (tp.slow[1]) d1 = d1 > 0.5f * gg.L[1] ? d1 - gg.L[1] : (d1 < -0.5f * gg.L[1] ? d1 + gg.L[1] : d1);
+                                if (DIM == 3 && tp.slow[2])
+                                    d2 = d2 > 0.5f * gg.L[2] ? d2 - gg.L[2] : (d2 < -0.5f * gg.L[2] ? d2 + gg.L[2] : d2);
+                                const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
+                                const float Hs2 = Hs * Hs;
+                                const float tol = tol_rel * (seam ? fmaf(Hs, sp.Lmax, Hs2) : Hs2);
+                                const float diff = r2 - Hs2;
+                                hit = diff < 0.f;
+                                g = gidx[q - c0];
+                                if (fabsf(diff) <= tol) hit = pred_exact(pi, pos_s[g], Hs, gg);   // R3, binary64
+                            }
+                            const uint32_t m = __ballot_sync(0xffffffffu, hit);
+                            if (FILL && hit) col[base + off + __popc(m & ((1u << lane) - 1u))] = (int32_t)g;
+                            off += __popc(m);
+                        }
+                    }
+                }
+            }
+            if (lane == 0) {
+                if (FILL) {
+                    if (!single) cursor[row] = off;
+                } else {
+                    cnt[row] = off;
                 }
             }
         }
     }
-    if (!FILL && lane == 0) cnt[row] = off;
 }
 
 // ---------------------------------------------------------------------------------------- export
@@ -188,12 +343,45 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
 
     SPH_TRY(ctx->cnt.reserve((size_t)n * 4));
     SPH_TRY(ctx->row_ptr.reserve((size_t)(n + 1) * 8));
-    const unsigned nblk = (unsigned)((n + kWarpsPerBlock - 1) / kWarpsPerBlock);
+    // tile geometry: block edge B and chunk capacity from the mean cell occupancy (any occupancy is handled
+    // by chunking; this only picks the fast configuration)
+    TilePar tp;
+    memset(&tp, 0, sizeof(tp));
+    const double mean_occ = (double)n / (double)ctx->ncells_total;
+    const int cap_max = 8192;                                       // 160 KB of shared memory
+    if (gg.dim == 3) tp.B = 64.0 * mean_occ * 1.25 <= cap_max ? 2 : 1;
+    else tp.B = 36.0 * mean_occ * 1.25 <= cap_max ? 4 : (16.0 * mean_occ * 1.25 <= cap_max ? 2 : 1);
+    double halo_cells = 1.0;
+    int64_t nblocks = 1;
+    for (int k = 0; k < 3; ++k) {
+        tp.nb[k] = 1;
+        if (k < gg.dim) {
+            tp.nb[k] = (gg.ncell[k] + tp.B - 1) / tp.B;
+            tp.slow[k] = gg.periodic[k] && gg.ncell[k] < tp.B + 2;
+            halo_cells *= tp.slow[k] ? gg.ncell[k] : tp.B + 2;
+        }
+        nblocks *= tp.nb[k];
+    }
+    {
+        double want = halo_cells * mean_occ * 1.25 + 64.0;
+        int cap = (int)((want + 255.0) / 256.0) * 256;
+        tp.cap = cap < 1024 ? 1024 : (cap > cap_max ? cap_max : cap);
+    }
+    const size_t smem = (size_t)tp.cap * (sizeof(float4) + sizeof(uint32_t));
+    SPH_TRY(ctx->s3.reserve((size_t)n * 4));                        // cursor of the multi-chunk fill path
+    uint32_t *cursor = ctx->s3.as<uint32_t>();
+#define SPH_NB_LAUNCH(DIM, FILL, CNT, RP, COL)                                                                        \
+    do {                                                                                                              \
+        SPH_CUDA_TRY(cudaFuncSetAttribute(k_neighbors_tile<DIM, FILL>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+                                          (int)smem));                                                                \
+        k_neighbors_tile<DIM, FILL><<<(unsigned)nblocks, kWarpsPerBlock * 32, smem, st>>>(                            \
+            n, gg, sp, tp, ctx->pos_s.as<float4>(), ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), CNT, \
+            cursor, RP, COL);                                                                                         \
+    } while (0)
     {
         KScope ks(ctx, SPH_K_COUNT, 1, st);
-        k_neighbors<false><<<nblk, kWarpsPerBlock * 32, 0, st>>>(n, gg, sp, ctx->pos_s.as<float4>(),
-                                                                ctx->key_sorted.as<uint32_t>(), ctx->cell_start.as<uint32_t>(),
-                                                                ctx->cell_end.as<uint32_t>(), ctx->cnt.as<uint32_t>(), nullptr, nullptr);
+        if (gg.dim == 3) SPH_NB_LAUNCH(3, false, ctx->cnt.as<uint32_t>(), nullptr, nullptr);
+        else SPH_NB_LAUNCH(2, false, ctx->cnt.as<uint32_t>(), nullptr, nullptr);
     }
     {
         KScope ks(ctx, SPH_K_SCAN, 3, st);
@@ -205,11 +393,10 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
     SPH_TRY(ctx->col.reserve((size_t)(nnz > 0 ? nnz : 1) * 4));
     {
         KScope ks(ctx, SPH_K_FILL, 1, st);
-        k_neighbors<true><<<nblk, kWarpsPerBlock * 32, 0, st>>>(n, gg, sp, ctx->pos_s.as<float4>(),
-                                                               ctx->key_sorted.as<uint32_t>(), ctx->cell_start.as<uint32_t>(),
-                                                               ctx->cell_end.as<uint32_t>(), nullptr, ctx->row_ptr.as<long long>(),
-                                                               ctx->col.as<int32_t>());
+        if (gg.dim == 3) SPH_NB_LAUNCH(3, true, nullptr, ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>());
+        else SPH_NB_LAUNCH(2, true, nullptr, ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>());
     }
+#undef SPH_NB_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     ctx->nnz = nnz;
     ctx->search_scale = search_scale;

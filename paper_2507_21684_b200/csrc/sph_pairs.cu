@@ -552,13 +552,22 @@ int sph_launch_rhs_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
 #define SPH_RHS_LAUNCH(DIM, GS, VARH, SORTED)                                                                     \
     k_rhs<DIM, GS, VARH, SORTED><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, s0, s1, s2, kind_s, rp, col, \
                                                                      perm, drho, acc, out4)
-    if (kp.dim == 3) {
-        if (kp.uniform_h) { if (sorted) SPH_RHS_LAUNCH(3, 32, false, true); else SPH_RHS_LAUNCH(3, 32, false, false); }
-        else { if (sorted) SPH_RHS_LAUNCH(3, 32, true, true); else SPH_RHS_LAUNCH(3, 32, true, false); }
-    } else {
-        if (kp.uniform_h) { if (sorted) SPH_RHS_LAUNCH(2, 16, false, true); else SPH_RHS_LAUNCH(2, 16, false, false); }
-        else { if (sorted) SPH_RHS_LAUNCH(2, 16, true, true); else SPH_RHS_LAUNCH(2, 16, true, false); }
+#define SPH_RHS_GS(GS)                                                                                              \
+    if (kp.dim == 3) {                                                                                              \
+        if (kp.uniform_h) { if (sorted) SPH_RHS_LAUNCH(3, GS, false, true); else SPH_RHS_LAUNCH(3, GS, false, false); } \
+        else { if (sorted) SPH_RHS_LAUNCH(3, GS, true, true); else SPH_RHS_LAUNCH(3, GS, true, false); }                \
+    } else {                                                                                                        \
+        if (kp.uniform_h) { if (sorted) SPH_RHS_LAUNCH(2, GS, false, true); else SPH_RHS_LAUNCH(2, GS, false, false); } \
+        else { if (sorted) SPH_RHS_LAUNCH(2, GS, true, true); else SPH_RHS_LAUNCH(2, GS, true, false); }                \
     }
+    const int gs_ = ctx->opt_group ? ctx->opt_group : (kp.dim == 3 ? 32 : 16);
+    switch (gs_) {
+    case 4: SPH_RHS_GS(4) break;
+    case 8: SPH_RHS_GS(8) break;
+    case 16: SPH_RHS_GS(16) break;
+    default: SPH_RHS_GS(32) break;
+    }
+#undef SPH_RHS_GS
 #undef SPH_RHS_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
@@ -574,7 +583,7 @@ int sph_launch_vjp_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
     const int32_t *col = ctx->col.as<int32_t>();
     const uint32_t *perm = ctx->perm.as<uint32_t>();
     const bool sorted = xb4 != nullptr;
-    const int gs = kp.dim == 3 ? 32 : 16;
+    const int gs = ctx->opt_group ? ctx->opt_group : (kp.dim == 3 ? 32 : 16);
     const unsigned grid = pair_grid(n, gs);
     SPH_TRY(ctx->partials.reserve((size_t)grid * kNPart * 4));
     float *part = ctx->partials.as<float>();
@@ -583,13 +592,21 @@ int sph_launch_vjp_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
 #define SPH_VJP_LAUNCH(DIM, GS, VARH, SORTED)                                                                  \
     k_vjp<DIM, GS, VARH, SORTED><<<grid, kBlock, 0, st>>>(n, kp, margin, s0, s1, s2, cot, eos, rp, col, perm, xb, \
                                                          vb, rb, xb4, vb4, part)
-    if (kp.dim == 3) {
-        if (kp.uniform_h) { if (sorted) SPH_VJP_LAUNCH(3, 32, false, true); else SPH_VJP_LAUNCH(3, 32, false, false); }
-        else { if (sorted) SPH_VJP_LAUNCH(3, 32, true, true); else SPH_VJP_LAUNCH(3, 32, true, false); }
-    } else {
-        if (kp.uniform_h) { if (sorted) SPH_VJP_LAUNCH(2, 16, false, true); else SPH_VJP_LAUNCH(2, 16, false, false); }
-        else { if (sorted) SPH_VJP_LAUNCH(2, 16, true, true); else SPH_VJP_LAUNCH(2, 16, true, false); }
+#define SPH_VJP_GS(GS)                                                                                              \
+    if (kp.dim == 3) {                                                                                              \
+        if (kp.uniform_h) { if (sorted) SPH_VJP_LAUNCH(3, GS, false, true); else SPH_VJP_LAUNCH(3, GS, false, false); } \
+        else { if (sorted) SPH_VJP_LAUNCH(3, GS, true, true); else SPH_VJP_LAUNCH(3, GS, true, false); }                \
+    } else {                                                                                                        \
+        if (kp.uniform_h) { if (sorted) SPH_VJP_LAUNCH(2, GS, false, true); else SPH_VJP_LAUNCH(2, GS, false, false); } \
+        else { if (sorted) SPH_VJP_LAUNCH(2, GS, true, true); else SPH_VJP_LAUNCH(2, GS, true, false); }                \
     }
+    switch (gs) {
+    case 4: SPH_VJP_GS(4) break;
+    case 8: SPH_VJP_GS(8) break;
+    case 16: SPH_VJP_GS(16) break;
+    default: SPH_VJP_GS(32) break;
+    }
+#undef SPH_VJP_GS
 #undef SPH_VJP_LAUNCH
     }
     if (params_bar) {
