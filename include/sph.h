@@ -152,6 +152,11 @@ const char *sph_strerror(int code);
  * launched by this context since creation. */
 int sph_get_info(sph_ctx *ctx, int32_t ncell[3], int64_t *n, int64_t *nnz, int64_t *launches);
 
+/* Layout of the lists built by the last sph_neighbors: *mode = 1 generic (32-bit sorted ids) or 2 tile-local (16-bit
+ * indices into the halo of a block of tile_edge^dim cells); halo_max / rows_max = largest halo population / row count
+ * of a block (0 for the generic layout).  Any pointer may be NULL. */
+int sph_get_layout(sph_ctx *ctx, int32_t *mode, int32_t *tile_edge, int64_t *halo_max, int64_t *rows_max);
+
 /* Per-kernel-class device timing for the roofline report (bench.py): when enabled, every launch (group) of a class
  * is bracketed by two CUDA events on the launching stream.  sph_profile_read synchronises the device, adds the
  * resolved durations to ms_sum[SPH_K_NCLASS] (milliseconds) and the launch counts to launches[SPH_K_NCLASS]
@@ -174,7 +179,12 @@ enum {
 };
 /* Tuning knobs (results do not depend on them beyond summation order). */
 enum {
-    SPH_OPT_PAIR_GROUP = 1 /* lanes that share one row in the pair kernels: 4, 8, 16, 32; 0 = default */
+    SPH_OPT_PAIR_GROUP = 1, /* lanes that share one row in the pair kernels: 4, 8, 16, 32; 0 = default */
+    SPH_OPT_LIST_MODE = 2,  /* internal list layout chosen by the next sph_neighbors: 0 = automatic; 1 = generic
+                               (32-bit sorted ids, neighbour state gathered through L1/L2, any cell occupancy);
+                               2 = tile-local (16-bit indices into the halo of a block of cells, neighbour state staged
+                               in shared memory).  2 falls back to 1 when a halo does not fit shared memory. */
+    SPH_OPT_TILE_EDGE = 3   /* edge of the cell blocks of the tile-local layout: 1, 2, 4 cells; 0 = automatic */
 };
 int sph_set_option(sph_ctx *ctx, int key, int value);
 int sph_profile_enable(sph_ctx *ctx, int on);

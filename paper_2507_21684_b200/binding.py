@@ -17,7 +17,12 @@ LIB_PATH = os.path.join(HERE, "libsph_b200.so")
 
 EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph_neighbors_export", "sph_density",
            "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
-           "sph_check", "sph_strerror", "sph_get_info", "sph_profile_enable", "sph_profile_read", "sph_set_option")
+           "sph_check", "sph_strerror", "sph_get_info", "sph_get_layout", "sph_profile_enable", "sph_profile_read",
+           "sph_set_option")
+
+# keys of sph_set_option (enum SPH_OPT_* in include/sph.h)
+OPT_PAIR_GROUP, OPT_LIST_MODE, OPT_TILE_EDGE = 1, 2, 3
+LIST_AUTO, LIST_GENERIC, LIST_TILE = 0, 1, 2
 
 # kernel classes of sph_profile_read (enum SPH_K_* in include/sph.h)
 KERNEL_CLASSES = ("key", "sort", "reorder", "count", "scan", "fill", "export", "density", "pack", "rhs", "vjp",
@@ -75,6 +80,7 @@ def load_library(path: str = LIB_PATH):
     lib.sph_strerror.argtypes = [C.c_int]
     lib.sph_strerror.restype = C.c_char_p
     lib.sph_get_info.argtypes = [vp, C.POINTER(C.c_int32 * 3), C.POINTER(i64), C.POINTER(i64), C.POINTER(i64)]
+    lib.sph_get_layout.argtypes = [vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(i64), C.POINTER(i64)]
     for name in EXPORTS:
         if name != "sph_strerror":
             getattr(lib, name).restype = C.c_int
@@ -275,6 +281,12 @@ class Sph:
 
     def check(self):
         self._chk(self.lib.sph_check(self._ctx))
+
+    def layout(self):
+        """layout of the lists of the last neighbors(): mode 1 generic / 2 tile-local, tile edge, largest halo / rows"""
+        mode, edge, hm, rm = C.c_int32(0), C.c_int32(0), C.c_int64(0), C.c_int64(0)
+        self._chk(self.lib.sph_get_layout(self._ctx, C.byref(mode), C.byref(edge), C.byref(hm), C.byref(rm)))
+        return dict(mode=int(mode.value), tile_edge=int(edge.value), halo_max=int(hm.value), rows_max=int(rm.value))
 
     def info(self):
         nc = (C.c_int32 * 3)()

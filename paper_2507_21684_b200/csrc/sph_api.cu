@@ -17,7 +17,7 @@ extern "C" int sph_create(sph_ctx **out, int device, int64_t n_max)
     if (!ctx) return SPH_E_NOMEM;
     ctx->device = device;
     ctx->n_hint = n_max;
-    if (cudaMallocHost((void **)&ctx->h_pinned, 8 * sizeof(int64_t)) != cudaSuccess) {
+    if (cudaMallocHost((void **)&ctx->h_pinned, 16 * sizeof(int64_t)) != cudaSuccess) {
         (void)cudaGetLastError();
         delete ctx;
         return SPH_E_NOMEM;
@@ -33,7 +33,7 @@ extern "C" int sph_destroy(sph_ctx *ctx)
     cudaDeviceSynchronize();
     DevBuf *bufs[] = {&ctx->key_a, &ctx->key_b, &ctx->idx_a, &ctx->idx_b, &ctx->hist, &ctx->perm, &ctx->inv_perm,
                       &ctx->key_sorted, &ctx->pos_s, &ctx->cell_start, &ctx->cell_end, &ctx->stats, &ctx->cnt,
-                      &ctx->row_ptr, &ctx->col, &ctx->scan_tmp, &ctx->s0, &ctx->s1, &ctx->s2, &ctx->s3, &ctx->c0buf,
+                      &ctx->row_ptr, &ctx->col, &ctx->col16, &ctx->scan_tmp, &ctx->s0, &ctx->s1, &ctx->s2, &ctx->s3, &ctx->c0buf,
                       &ctx->out4, &ctx->m_s, &ctx->kind_s, &ctx->partials, &ctx->eos, &ctx->hx, &ctx->hv, &ctx->hrho,
                       &ctx->hm, &ctx->hh, &ctx->hkind, &ctx->hlam, &ctx->hmu, &ctx->ho_drho, &ctx->ho_acc, &ctx->ho_xb,
                       &ctx->ho_vb, &ctx->ho_rb, &ctx->ho_pb, &ctx->ho_dens};
@@ -82,6 +82,17 @@ extern "C" int sph_get_info(sph_ctx *ctx, int32_t ncell[3], int64_t *n, int64_t 
     if (n) *n = ctx->n;
     if (nnz) *nnz = ctx->lists_ready ? ctx->nnz : 0;
     if (launches) *launches = ctx->launches;
+    return SPH_OK;
+}
+
+extern "C" int sph_get_layout(sph_ctx *ctx, int32_t *mode, int32_t *tile_edge, int64_t *halo_max, int64_t *rows_max)
+{
+    if (!ctx) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    if (mode) *mode = ctx->tile_mode ? 2 : 1;
+    if (tile_edge) *tile_edge = ctx->tile_mode ? ctx->tg.B : 0;
+    if (halo_max) *halo_max = ctx->tile_mode ? (int64_t)ctx->tile_Mmax : 0;
+    if (rows_max) *rows_max = ctx->tile_mode ? (int64_t)ctx->tile_Tmax : 0;
     return SPH_OK;
 }
 
@@ -220,6 +231,14 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
     case SPH_OPT_PAIR_GROUP:
         if (value != 0 && value != 4 && value != 8 && value != 16 && value != 32) return SPH_E_INVALID;
         ctx->opt_group = value;
+        return SPH_OK;
+    case SPH_OPT_LIST_MODE:
+        if (value < 0 || value > 2) return SPH_E_INVALID;
+        ctx->opt_list_mode = value;
+        return SPH_OK;
+    case SPH_OPT_TILE_EDGE:
+        if (value != 0 && value != 1 && value != 2 && value != 4) return SPH_E_INVALID;
+        ctx->opt_tile_edge = value;
         return SPH_OK;
     default:
         return SPH_E_INVALID;

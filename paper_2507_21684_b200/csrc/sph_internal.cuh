@@ -67,6 +67,17 @@ struct GridGeom {
     double L_d[3];
 };
 
+// Cell-block decomposition (sph_tiles.cuh); passed by value.
+struct TileGeom {
+    int dim;
+    int B;             // block edge in cells: 1, 2 or 4
+    int nb[3];         // blocks per axis
+    int ntiles;
+    int ncell[3];
+    int periodic[3];
+    float L[3];
+};
+
 // Per-launch physical constants (derived once on the host from sph_params).
 struct KPar {
     int dim;
@@ -111,6 +122,11 @@ struct sph_ctx {
     int device = 0;
     Profiler prof;
     int opt_group = 0;          // lanes per row in the pair kernels (0 = default)
+    int opt_list_mode = 0;      // 0 auto, 1 force the generic (global-id) lists, 2 force tile-local lists
+    int opt_tile_edge = 0;      // 0 auto, else force the tile edge B (1, 2, 4)
+    bool tile_mode = false;     // lists of the last sph_neighbors are tile-local (col16)
+    TileGeom tg{};
+    uint32_t tile_Mmax = 0, tile_Tmax = 0;   // largest halo / row count of a tile
     int64_t n_hint = 0;
     int64_t n = 0;
     bool cells_ready = false, lists_ready = false;
@@ -130,13 +146,14 @@ struct sph_ctx {
     DevBuf cell_start, cell_end;
     DevBuf stats;               // device: [0] err flag, [1] hmax bits, [2] hmin bits
     // lists
-    DevBuf cnt, row_ptr, col, scan_tmp;
+    DevBuf cnt, row_ptr, col, col16, scan_tmp;
+    bool col_valid = false;     // ctx->col holds the global-id lists of the current build
     // pair scratch (sorted SoA)
     DevBuf s0, s1, s2, s3, c0buf, out4, m_s, kind_s, partials, eos;
     // rk scratch
     DevBuf rk[16];
     // pinned host mirror
-    int64_t *h_pinned = nullptr; // [8]
+    int64_t *h_pinned = nullptr; // [16]
     // host staging for *_host call
     DevBuf hx, hv, hrho, hm, hh, hkind, hlam, hmu, ho_drho, ho_acc, ho_xb, ho_vb, ho_rb, ho_pb, ho_dens;
 };
@@ -257,6 +274,13 @@ __device__ __forceinline__ int cell_coord_raw(double x, double lo, double edge)
 }
 
 // host-side launch helpers implemented in the .cu files
+int sph_tile_expand_col(sph_ctx *ctx, cudaStream_t st);   // tile-local lists -> 32-bit sorted ids in ctx->col
+int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, float *rho_out, cudaStream_t st);
+int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
+                        const uint8_t *kind_s, float *drho, float *acc, float4 *out4, cudaStream_t st);
+int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
+                        const float4 *cot, const float4 *eos, float *xb, float *vb, float *rb, float4 *xb4, float4 *vb4,
+                        float *partials, cudaStream_t st);
 int sph_scan_u32(sph_ctx *ctx, const uint32_t *in, void *out, bool out64, int64_t m, cudaStream_t st);
 int sph_kpar_make(const sph_ctx *ctx, const sph_params *par, KPar *kp);
 int sph_launch_rhs_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,

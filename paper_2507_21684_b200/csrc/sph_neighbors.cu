@@ -4,47 +4,14 @@
 // time, a ballot compacts the hits, so every row is written coalesced and in a fixed order
 // (cells in z,y,x order, ascending sorted index inside a cell) -- deterministic, no atomics.
 #include "sph_internal.cuh"
+#include "sph_tiles.cuh"
+#include "sph_search.cuh"
 
 #include <math.h>
 
 namespace {
 
 constexpr int kWarpsPerBlock = 8;
-
-struct SearchPar {
-    float scale;     // search_scale (binary32)
-    double R;        // scale*hmax*(1+2^-20): half width of the candidate interval per axis
-    float band;      // relative half width of the fp32 "too close to call" band
-    float Lmax;      // largest periodic box length (0 if none)
-};
-
-// R3: the predicate r2 < Hs^2 in binary64 on the wrapped binary32 positions, fixed op order.
-__device__ __forceinline__ bool pred_exact(const float4 &a, const float4 &b, float Hs, const GridGeom &gg)
-{
-    double d0 = __dsub_rn((double)a.x, (double)b.x);
-    double d1 = __dsub_rn((double)a.y, (double)b.y);
-    double d2 = gg.dim == 3 ? __dsub_rn((double)a.z, (double)b.z) : 0.0;
-    if (gg.periodic[0]) {
-        double L = gg.L_d[0];
-        if (d0 > 0.5 * L) d0 = __dsub_rn(d0, L);
-        else if (d0 < -0.5 * L) d0 = __dadd_rn(d0, L);
-    }
-    if (gg.periodic[1]) {
-        double L = gg.L_d[1];
-        if (d1 > 0.5 * L) d1 = __dsub_rn(d1, L);
-        else if (d1 < -0.5 * L) d1 = __dadd_rn(d1, L);
-    }
-    if (gg.dim == 3 && gg.periodic[2]) {
-        double L = gg.L_d[2];
-        if (d2 > 0.5 * L) d2 = __dsub_rn(d2, L);
-        else if (d2 < -0.5 * L) d2 = __dadd_rn(d2, L);
-    }
-    double r2 = __dmul_rn(d0, d0);
-    r2 = __fma_rn(d1, d1, r2);
-    if (gg.dim == 3) r2 = __fma_rn(d2, d2, r2);
-    double Hs2 = __dmul_rn((double)Hs, (double)Hs);
-    return r2 < Hs2;
-}
 
 // ---------------------------------------------------------------------------------------- tile search
 // One CTA owns a block of B^d cells.  It stages the particles of the (B+2)^d halo cells into shared memory
@@ -319,10 +286,16 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
     const int64_t n = ctx->n;
     const GridGeom &gg = ctx->geom;
 
+    // candidate cell-block decompositions: their largest halo decides whether the tile-local layout fits
+    int cand[3], ncand = 0;
+    if (ctx->opt_list_mode != 1) ncand = sph_tile_candidates(ctx, cand);
+    if (ncand) SPH_TRY(sph_tile_stats_launch(ctx, cand, ncand, st));
     // the statistics of sph_build_cells (error flag, max/min h) are needed on the host to size the search
-    uint32_t *hs = reinterpret_cast<uint32_t *>(ctx->h_pinned);
-    SPH_CUDA_TRY(cudaMemcpyAsync(hs, ctx->stats.p, 16, cudaMemcpyDeviceToHost, st));
+    uint32_t hs[10];
+    uint32_t *hpin = reinterpret_cast<uint32_t *>(ctx->h_pinned + 8);
+    SPH_CUDA_TRY(cudaMemcpyAsync(hpin, ctx->stats.p, 40, cudaMemcpyDeviceToHost, st));
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
+    memcpy(hs, hpin, 40);
     if (hs[0] != 0u) return SPH_E_DOMAIN;
     float hmax, hmin;
     memcpy(&hmax, &hs[1], 4);
@@ -340,6 +313,18 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
     sp.Lmax = 0.f;
     for (int k = 0; k < gg.dim; ++k)
         if (gg.periodic[k] && gg.L[k] > sp.Lmax) sp.Lmax = gg.L[k];
+    sp.Hs_u = Rs;                                   // = (float)(scale*h) when h is uniform
+
+    ctx->tile_mode = false;
+    ctx->col_valid = false;
+    for (int k = 0; k < ncand; ++k) {
+        const uint32_t Mmax = hs[4 + 2 * k], Tmax = hs[5 + 2 * k];
+        if (!sph_tile_fits(gg.dim, Mmax)) continue;
+        SPH_TRY(sph_neighbors_tile_run(ctx, sp, cand[k], Mmax, Tmax, st, nnz_out));
+        ctx->search_scale = search_scale;
+        ctx->lists_ready = true;
+        return SPH_OK;
+    }
 
     SPH_TRY(ctx->cnt.reserve((size_t)n * 4));
     SPH_TRY(ctx->row_ptr.reserve((size_t)(n + 1) * 8));
@@ -399,6 +384,7 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
 #undef SPH_NB_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     ctx->nnz = nnz;
+    ctx->col_valid = true;
     ctx->search_scale = search_scale;
     ctx->lists_ready = true;
     if (nnz_out) *nnz_out = nnz;
@@ -413,6 +399,7 @@ extern "C" int sph_neighbors_export(sph_ctx *ctx, int64_t *row_ptr, int32_t *col
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
     const int64_t n = ctx->n;
+    SPH_TRY(sph_tile_expand_col(ctx, st));
     SPH_TRY(ctx->s3.reserve((size_t)n * 4));
     uint32_t *cnt_c = ctx->s3.as<uint32_t>();
     KScope ks(ctx, SPH_K_EXPORT, 5, st);

@@ -1,0 +1,407 @@
+// sph_neighbors_tile.cu -- steps N5/N7 of SURVEY.md 8(a) on the cell-block decomposition of sph_tiles.cuh:
+// count and fill of TILE-LOCAL compact lists (uint16 halo-linear indices), PAPER.md:558 (adjacent-cell query),
+// PAPER.md:163 (pair list), PAPER.md:167 (radius max{h_i,h_j}).
+//
+// One CTA per tile.  The halo positions are staged in shared memory once.  A warp takes 32 rows OF ONE CELL, one
+// row per lane: all lanes walk the same candidate sequence, so every candidate is ONE broadcast shared-memory load
+// and ~11 instructions for 32 row-candidate tests (the first path of this round spent 110 per 32).  Hits go to a
+// per-warp shared-memory image of the warp's contiguous col16 segment (rows of a cell are contiguous in the
+// sorted order, so their list segments are too), which is then flushed coalesced.  Deterministic: fixed candidate
+// order (cells in z,y,x order, ascending sorted index inside a cell), no atomics.
+#include "sph_internal.cuh"
+#include "sph_tiles.cuh"
+#include "sph_search.cuh"
+
+#include <math.h>
+
+namespace {
+
+constexpr int kNbWarps = 8;
+constexpr int kNbBlk = 8;        // candidates per unrolled block
+
+struct RowCtx {
+    float4 pi;         // own position (+h)
+    float Hs2, tol;    // uniform h: thresholds of the fp32 test
+    uint32_t n;        // hits so far
+    uint32_t cap;      // FILL: length of the row (from the count pass)
+};
+
+// One candidate.  EXACT: resolve the "too close to call" band with the binary64 predicate (reading R3).
+template <int DIM, bool VARH, bool EXACT>
+__device__ __forceinline__ bool nb_test(const RowCtx &rc, const float4 &pj, const SearchPar &sp, bool seam, uint32_t q,
+                                        const TileTab &tt, const float4 *__restrict__ pos_s, const GridGeom &gg,
+                                        bool &unsure)
+{
+    const float d0 = rc.pi.x - pj.x, d1 = rc.pi.y - pj.y, d2 = DIM == 3 ? rc.pi.z - pj.z : 0.f;
+    const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
+    float Hs2 = rc.Hs2, tol = rc.tol, Hs = sp.Hs_u;
+    if (VARH) {
+        Hs = __fmul_rn(sp.scale, fmaxf(rc.pi.w, pj.w));
+        Hs2 = Hs * Hs;
+        tol = sp.band * (seam ? fmaf(Hs, sp.Lmax, Hs2) : Hs2);
+    }
+    const float diff = r2 - Hs2;
+    bool hit = diff < 0.f;
+    const bool band = fabsf(diff) <= tol;
+    if (EXACT) {
+        if (band) hit = pred_exact(rc.pi, pos_s[tile_q_to_sorted(tt, q)], Hs, gg);
+    } else {
+        unsure = unsure || band;
+    }
+    return hit;
+}
+
+// `dst`: FILL only -- where this lane's hits go (shared-memory image or global col16), indexed by rc.n
+template <int DIM, bool FILL, bool VARH, bool EXACT, class DstT>
+__device__ __forceinline__ void nb_block(RowCtx &rc, const float4 *__restrict__ cand, uint32_t q, int nq,
+                                         const SearchPar &sp, bool seam, const TileTab &tt,
+                                         const float4 *__restrict__ pos_s, const GridGeom &gg, DstT dst, bool &unsure)
+{
+#pragma unroll
+    for (int u = 0; u < kNbBlk; ++u) {
+        if (u < nq) {
+            const float4 pj = cand[q + u];
+            const bool hit = nb_test<DIM, VARH, EXACT>(rc, pj, sp, seam, q + u, tt, pos_s, gg, unsure);
+            if (FILL) {
+                // rc.n < rc.cap: the speculative fp32 pass of a block that is then redone exactly may see more
+                // hits than the row has; it must not write into the next row's segment
+                if (hit && rc.n < rc.cap) dst[rc.n] = (uint16_t)(q + u);
+            }
+            rc.n += hit ? 1u : 0u;
+        }
+    }
+}
+
+template <int DIM, bool FILL, bool VARH, class DstT>
+__device__ __forceinline__ void nb_rows(RowCtx &rc, const float4 *__restrict__ cand, const int sl[3], const SearchPar &sp,
+                                        bool seam, const TileTab &tt, const float4 *__restrict__ pos_s,
+                                        const GridGeom &gg, DstT dst)
+{
+    const int zlo = DIM == 3 ? -1 : 0, zhi = DIM == 3 ? 1 : 0;
+    for (int dz = zlo; dz <= zhi; ++dz) {
+        const int sz = sl[2] + dz;
+        if (DIM == 3 && (sz < 0 || sz >= tt.ext[2])) continue;
+        for (int dy = -1; dy <= 1; ++dy) {
+            const int sy = sl[1] + dy;
+            if (sy < 0 || sy >= tt.ext[1]) continue;
+            const int rowbase = tt.ext[0] * (sy + tt.ext[1] * sz);
+            const int xa = max(sl[0] - 1, 0), xb = min(sl[0] + 1, tt.ext[0] - 1);
+            const uint32_t q0 = tt.h_off[rowbase + xa], q1 = tt.h_off[rowbase + xb + 1];
+            for (uint32_t q = q0; q < q1; q += kNbBlk) {
+                const int nq = min((uint32_t)kNbBlk, q1 - q);
+                const uint32_t n0 = rc.n;
+                bool unsure = false;
+                if (nq == kNbBlk) nb_block<DIM, FILL, VARH, false>(rc, cand, q, kNbBlk, sp, seam, tt, pos_s, gg, dst, unsure);
+                else nb_block<DIM, FILL, VARH, false>(rc, cand, q, nq, sp, seam, tt, pos_s, gg, dst, unsure);
+                if (unsure) {                      // rare (except on exact lattices): redo the block exactly
+                    rc.n = n0;
+                    bool dummy = false;
+                    nb_block<DIM, FILL, VARH, true>(rc, cand, q, nq, sp, seam, tt, pos_s, gg, dst, dummy);
+                }
+            }
+        }
+    }
+}
+
+template <int DIM, bool FILL, bool VARH>
+__global__ void __launch_bounds__(kNbWarps * 32)
+k_nb_tile(TileGeom tg, GridGeom gg, SearchPar sp, int mcap, int wcap, const float4 *__restrict__ pos_s,
+          const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end, uint32_t *__restrict__ cnt,
+          const long long *__restrict__ row_ptr, uint16_t *__restrict__ col16)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float4 *cand = reinterpret_cast<float4 *>(smem_raw);
+    __shared__ TileTab tt;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (tt.T == 0) return;
+    bool seam = false;
+#pragma unroll
+    for (int k = 0; k < DIM; ++k)
+        if (tg.periodic[k] && (tt.hs[k] < 0 || tt.hs[k] + tt.ext[k] > tg.ncell[k])) seam = true;
+
+    // ---- stage the halo positions (shifted across periodic seams)
+    for (int hc = warp; hc < tt.nh; hc += kNbWarps) {
+        const uint32_t o0 = tt.h_off[hc], o1 = tt.h_off[hc + 1];
+        if (o1 == o0) continue;
+        float sh[3];
+        tile_cell_shift<DIM>(tg, tt, hc, sh);
+        const uint32_t gs = tt.h_start[hc];
+        for (uint32_t q = o0 + lane; q < o1; q += 32) {
+            float4 pj = pos_s[gs + (q - o0)];
+            pj.x += sh[0];
+            pj.y += sh[1];
+            if (DIM == 3) pj.z += sh[2];
+            cand[q] = pj;
+        }
+    }
+    __syncthreads();
+
+    uint16_t *wbuf = reinterpret_cast<uint16_t *>(smem_raw + (size_t)mcap * sizeof(float4)) + (size_t)warp * wcap;
+    // ---- work items: (target cell, chunk of 32 rows), dealt round-robin to the warps
+    int item = 0;
+    for (int tc = 0; tc < tt.nt; ++tc) {
+        const uint32_t nrow = tt.t_off[tc + 1] - tt.t_off[tc];
+        const int hc_i = tt.t_cell[tc];
+        for (uint32_t c0 = 0; c0 < nrow; c0 += 32, ++item) {
+            if (item % kNbWarps != warp) continue;
+            const int sl[3] = {hc_i % tt.ext[0], (hc_i / tt.ext[0]) % tt.ext[1], hc_i / (tt.ext[0] * tt.ext[1])};
+            const uint32_t nact = min(32u, nrow - c0);
+            const bool active = (uint32_t)lane < nact;
+            const uint32_t local = c0 + (active ? lane : 0);
+            const uint32_t row = tt.h_start[hc_i] + local;
+            RowCtx rc;
+            rc.pi = cand[tt.h_off[hc_i] + local];          // target cells are never shifted
+            rc.Hs2 = sp.Hs_u * sp.Hs_u;
+            rc.tol = sp.band * (seam ? fmaf(sp.Hs_u, sp.Lmax, rc.Hs2) : rc.Hs2);
+            rc.n = 0;
+            rc.cap = 0;
+            if (!FILL) {
+                nb_rows<DIM, false, VARH>(rc, cand, sl, sp, seam, tt, pos_s, gg, (uint16_t *)nullptr);
+                if (active) cnt[row] = rc.n;
+            } else {
+                const uint32_t row_first = tt.h_start[hc_i] + c0;
+                const long long seg0 = row_ptr[row_first], seg1 = row_ptr[row_first + nact];
+                const long long mine = row_ptr[row];
+                rc.cap = (uint32_t)(row_ptr[row + 1] - mine);
+                const uint32_t total = (uint32_t)(seg1 - seg0);
+                if (total <= (uint32_t)wcap) {
+                    // inactive lanes duplicate lane 0 and write the same values to the same places
+                    nb_rows<DIM, true, VARH>(rc, cand, sl, sp, seam, tt, pos_s, gg, wbuf + (uint32_t)(mine - seg0));
+                    __syncwarp();
+                    uint16_t *out = col16 + seg0;
+                    for (uint32_t k = lane; k < total; k += 32) out[k] = wbuf[k];
+                    __syncwarp();
+                } else {
+                    nb_rows<DIM, true, VARH>(rc, cand, sl, sp, seam, tt, pos_s, gg, col16 + mine);
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------- tile statistics
+// largest halo population and largest row count over all tiles of a candidate decomposition (one thread per tile)
+template <int DIM>
+__global__ void k_tile_stats(TileGeom tg, const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
+                             uint32_t *__restrict__ out /* [2]: Mmax, Tmax */)
+{
+    const int tile = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t M = 0, T = 0;
+    if (tile < tg.ntiles) {
+        int b = tile, bc[3] = {0, 0, 0};
+        bc[0] = b % tg.nb[0];
+        b /= tg.nb[0];
+        bc[1] = b % tg.nb[1];
+        bc[2] = b / tg.nb[1];
+        int lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0}, t0[3] = {0, 0, 0}, t1[3] = {0, 0, 0};   // inclusive ranges (unwrapped)
+#pragma unroll
+        for (int k = 0; k < DIM; ++k) {
+            const int c0 = bc[k] * tg.B, tn = min(tg.B, tg.ncell[k] - c0);
+            t0[k] = c0;
+            t1[k] = c0 + tn - 1;
+            lo[k] = tg.periodic[k] ? c0 - 1 : max(c0 - 1, 0);
+            hi[k] = tg.periodic[k] ? c0 + tn : min(c0 + tn, tg.ncell[k] - 1);
+        }
+        for (int cz = lo[2]; cz <= hi[2]; ++cz)
+            for (int cy = lo[1]; cy <= hi[1]; ++cy)
+                for (int cx = lo[0]; cx <= hi[0]; ++cx) {
+                    int c[3] = {cx, cy, cz};
+                    bool tgt = true;
+                    int64_t lin = 0;
+#pragma unroll
+                    for (int k = DIM - 1; k >= 0; --k) {
+                        tgt = tgt && c[k] >= t0[k] && c[k] <= t1[k];
+                        int w = c[k];
+                        if (tg.periodic[k]) w = w < 0 ? w + tg.ncell[k] : (w >= tg.ncell[k] ? w - tg.ncell[k] : w);
+                        lin = lin * tg.ncell[k] + w;
+                    }
+                    const uint32_t cc = cell_end[lin] - cell_start[lin];
+                    M += cc;
+                    if (tgt) T += cc;
+                }
+    }
+    M = __reduce_max_sync(0xffffffffu, M);
+    T = __reduce_max_sync(0xffffffffu, T);
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(&out[0], M);
+        atomicMax(&out[1], T);
+    }
+}
+
+// ---------------------------------------------------------------------------------------- col16 -> sorted ids
+// (export and the generic pair kernels only) one CTA per tile; rows of a tile are contiguous
+template <int DIM>
+__global__ void __launch_bounds__(256)
+k_expand_col16(TileGeom tg, const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
+               const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16, int32_t *__restrict__ col)
+{
+    __shared__ TileTab tt;
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (tt.T == 0) return;
+    const long long b = row_ptr[tt.row0], e = row_ptr[tt.row0 + tt.T];
+    for (long long p = b + threadIdx.x; p < e; p += blockDim.x) col[p] = (int32_t)tile_q_to_sorted(tt, col16[p]);
+}
+
+} // namespace
+
+// ==========================================================================================
+// host side
+// ==========================================================================================
+static TileGeom make_tile_geom(const GridGeom &gg, int B)
+{
+    TileGeom tg;
+    memset(&tg, 0, sizeof(tg));
+    tg.dim = gg.dim;
+    tg.B = B;
+    tg.ntiles = 1;
+    for (int k = 0; k < 3; ++k) {
+        tg.nb[k] = 1;
+        tg.ncell[k] = gg.ncell[k];
+        tg.periodic[k] = gg.periodic[k];
+        tg.L[k] = gg.L[k];
+        if (k < gg.dim) tg.nb[k] = (gg.ncell[k] + B - 1) / B;
+        tg.ntiles *= tg.nb[k];
+    }
+    return tg;
+}
+
+static bool tile_geom_ok(const GridGeom &gg, int B)
+{
+    int halo = 1, tgt = 1;
+    for (int k = 0; k < gg.dim; ++k) {
+        if (gg.periodic[k] && gg.ncell[k] < B + 2) return false;   // the halo would wrap onto itself
+        halo *= B + 2;
+        tgt *= B;
+    }
+    return halo <= kTileMaxHalo && tgt <= kTileMaxTgt;
+}
+
+// candidate tile edges of a dimension, best first
+int sph_tile_candidates(const sph_ctx *ctx, int out[3])
+{
+    const GridGeom &gg = ctx->geom;
+    int n = 0;
+    const int pref3[2] = {2, 1}, pref2[3] = {4, 2, 1};
+    const int *pref = gg.dim == 3 ? pref3 : pref2;
+    const int np = gg.dim == 3 ? 2 : 3;
+    for (int i = 0; i < np; ++i) {
+        if (ctx->opt_tile_edge && pref[i] != ctx->opt_tile_edge) continue;
+        if (tile_geom_ok(gg, pref[i])) out[n++] = pref[i];
+    }
+    return n;
+}
+
+// enqueue the statistics of every candidate decomposition into stats[4 + 2k], stats[5 + 2k]
+int sph_tile_stats_launch(sph_ctx *ctx, const int *cand, int ncand, cudaStream_t st)
+{
+    uint32_t *stats = ctx->stats.as<uint32_t>();
+    SPH_CUDA_TRY(cudaMemsetAsync(stats + 4, 0, 6 * sizeof(uint32_t), st));
+    for (int k = 0; k < ncand; ++k) {
+        const TileGeom tg = make_tile_geom(ctx->geom, cand[k]);
+        KScope ks(ctx, SPH_K_COUNT, 1, st);
+        const unsigned nb = (unsigned)((tg.ntiles + 127) / 128);
+        if (tg.dim == 3) k_tile_stats<3><<<nb, 128, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), stats + 4 + 2 * k);
+        else k_tile_stats<2><<<nb, 128, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), stats + 4 + 2 * k);
+    }
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+// shared-memory budget of the pair kernels decides which halo sizes the tile layout accepts
+size_t sph_tile_state_bytes(int dim) { return dim == 3 ? 56 : 48; }   // VJP: state + cotangents per halo particle
+static const size_t kTileSmemBudget = 200 * 1024;
+
+bool sph_tile_fits(int dim, uint32_t Mmax)
+{
+    return Mmax > 0 && Mmax <= 65535u && (size_t)(Mmax + 8) * sph_tile_state_bytes(dim) + (size_t)(Mmax + 8) * 4 <= kTileSmemBudget;
+}
+
+// count / scan / fill of the tile-local lists with tile edge B.  Synchronises `st` once (nnz readback).
+int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mmax, uint32_t Tmax, cudaStream_t st,
+                           int64_t *nnz_out)
+{
+    const int64_t n = ctx->n;
+    const GridGeom &gg = ctx->geom;
+    const TileGeom tg = make_tile_geom(gg, B);
+    const bool varh = ctx->hmin != ctx->hmax;
+    const int mcap = (int)((Mmax + 7u) & ~7u);
+    SPH_TRY(ctx->cnt.reserve((size_t)n * 4));
+    SPH_TRY(ctx->row_ptr.reserve((size_t)(n + 1) * 8));
+    const float4 *pos = ctx->pos_s.as<float4>();
+    const uint32_t *cs = ctx->cell_start.as<uint32_t>(), *ce = ctx->cell_end.as<uint32_t>();
+#define SPH_NBT_LAUNCH(DIM, FILL, VARH, SMEM, WCAP, CNT, RP, COL)                                                      \
+    do {                                                                                                               \
+        SPH_CUDA_TRY(cudaFuncSetAttribute(k_nb_tile<DIM, FILL, VARH>, cudaFuncAttributeMaxDynamicSharedMemorySize,     \
+                                          (int)(SMEM)));                                                               \
+        k_nb_tile<DIM, FILL, VARH><<<(unsigned)tg.ntiles, kNbWarps * 32, (SMEM), st>>>(tg, gg, sp, mcap, (WCAP), pos,  \
+                                                                                      cs, ce, CNT, RP, COL);           \
+    } while (0)
+#define SPH_NBT_DISPATCH(FILL, SMEM, WCAP, CNT, RP, COL)                                                               \
+    do {                                                                                                               \
+        if (gg.dim == 3) { if (varh) SPH_NBT_LAUNCH(3, FILL, true, SMEM, WCAP, CNT, RP, COL);                          \
+                           else SPH_NBT_LAUNCH(3, FILL, false, SMEM, WCAP, CNT, RP, COL); }                            \
+        else { if (varh) SPH_NBT_LAUNCH(2, FILL, true, SMEM, WCAP, CNT, RP, COL);                                      \
+               else SPH_NBT_LAUNCH(2, FILL, false, SMEM, WCAP, CNT, RP, COL); }                                        \
+    } while (0)
+    {
+        KScope ks(ctx, SPH_K_COUNT, 1, st);
+        const size_t smem = (size_t)mcap * sizeof(float4);
+        SPH_NBT_DISPATCH(false, smem, 0, ctx->cnt.as<uint32_t>(), nullptr, nullptr);
+    }
+    {
+        KScope ks(ctx, SPH_K_SCAN, 3, st);
+        SPH_TRY(sph_scan_u32(ctx, ctx->cnt.as<uint32_t>(), ctx->row_ptr.p, true, n, st));
+    }
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->h_pinned + 4, ctx->row_ptr.as<long long>() + n, 8, cudaMemcpyDeviceToHost, st));
+    SPH_CUDA_TRY(cudaStreamSynchronize(st));
+    const int64_t nnz = ctx->h_pinned[4];
+    SPH_TRY(ctx->col16.reserve((size_t)(nnz > 0 ? nnz : 1) * 2 + 64));
+    {
+        // per-warp staging capacity: 32 rows of the mean length with head room; the halo positions come first
+        const double mean = (double)nnz / (double)n;
+        int wcap = (int)(32.0 * mean * 1.35) + 64;
+        wcap = (wcap + 63) & ~63;
+        if (wcap < 512) wcap = 512;
+        const size_t budget = 100 * 1024;                      // two CTAs per SM
+        const size_t pos_bytes = (size_t)mcap * sizeof(float4);
+        if (pos_bytes + (size_t)kNbWarps * wcap * 2 > budget) {
+            const size_t room = pos_bytes < budget ? budget - pos_bytes : 0;
+            int w2 = (int)(room / (kNbWarps * 2)) & ~63;
+            if (w2 < 512) w2 = 512;
+            if (w2 < wcap) wcap = w2;
+        }
+        KScope ks(ctx, SPH_K_FILL, 1, st);
+        const size_t smem = pos_bytes + (size_t)kNbWarps * wcap * 2;
+        SPH_NBT_DISPATCH(true, smem, wcap, nullptr, ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>());
+    }
+#undef SPH_NBT_DISPATCH
+#undef SPH_NBT_LAUNCH
+    SPH_CUDA_TRY(cudaGetLastError());
+    ctx->tg = tg;
+    ctx->tile_mode = true;
+    ctx->tile_Mmax = Mmax;
+    ctx->tile_Tmax = Tmax;
+    ctx->col_valid = false;
+    ctx->nnz = nnz;
+    if (nnz_out) *nnz_out = nnz;
+    return SPH_OK;
+}
+
+// materialise the 32-bit sorted-id lists from the tile-local ones (export; generic pair kernels)
+int sph_tile_expand_col(sph_ctx *ctx, cudaStream_t st)
+{
+    if (!ctx->tile_mode || ctx->col_valid) return SPH_OK;
+    SPH_TRY(ctx->col.reserve((size_t)(ctx->nnz > 0 ? ctx->nnz : 1) * 4));
+    KScope ks(ctx, SPH_K_EXPORT, 1, st);
+    const TileGeom &tg = ctx->tg;
+    if (tg.dim == 3)
+        k_expand_col16<3><<<(unsigned)tg.ntiles, 256, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),
+                                                              ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->col.as<int32_t>());
+    else
+        k_expand_col16<2><<<(unsigned)tg.ntiles, 256, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),
+                                                              ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->col.as<int32_t>());
+    SPH_CUDA_TRY(cudaGetLastError());
+    ctx->col_valid = true;
+    return SPH_OK;
+}

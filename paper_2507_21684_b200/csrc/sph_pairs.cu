@@ -5,6 +5,7 @@
 //
 // Formulas: include/sph.h header comment and DESIGN.md section 2 (Eq.8, 9, 12, 40, 42, 7).
 #include "sph_internal.cuh"
+#include "sph_pair_math.cuh"
 
 #include <math.h>
 
@@ -12,38 +13,6 @@ namespace {
 
 constexpr int kBlock = 256;          // threads per block
 constexpr int kRowsPerGroup = 8;     // rows each lane group walks through
-
-// H-dependent constants of one pair (or of the whole launch when h is uniform)
-struct HC {
-    float invH, cW, cG, cK, ell, e2, eta, kd, H2;
-};
-
-template <int DIM>
-__device__ __forceinline__ HC hc_make(float H, const KPar &kp)
-{
-    HC c;
-    c.invH = 1.0f / H;
-    float i2 = c.invH * c.invH;
-    float iD = DIM == 2 ? i2 : i2 * c.invH;             // H^-d
-    c.cW = kp.Cd * iD;
-    c.cG = -(56.0f / 3.0f) * kp.Cd * iD * i2;           // G = cG (1+5q)(1-q)^5
-    c.cK = 560.0f * kp.Cd * iD * i2 * i2;               // K = cK (1-q)^4
-    c.ell = H * kp.inv_kappa;
-    float eh = kp.eps * H;
-    c.e2 = eh * eh;
-    c.eta = kp.alpha * c.ell * kp.c0 + kp.visc_nu;
-    c.kd = 2.0f * kp.delta * c.ell * kp.c0;
-    c.H2 = H * H;
-    return c;
-}
-template <int DIM>
-__device__ __forceinline__ HC hc_uniform(const KPar &kp)
-{
-    HC c;
-    c.invH = kp.invH; c.cW = kp.cW; c.cG = kp.cG; c.cK = kp.cK; c.ell = kp.ell; c.e2 = kp.e2; c.eta = kp.eta;
-    c.kd = kp.kd; c.H2 = kp.H * kp.H;
-    return c;
-}
 
 // sorted state of one particle as the pair loops see it
 struct Part {
@@ -113,14 +82,23 @@ __global__ void k_pack_state(int64_t n, KPar kp, const uint32_t *__restrict__ pe
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n) return;
     const int64_t i = perm[p];
+    const float4 pb = pos_s[p];                           // wrapped build position, h
+    const float xb[3] = {pb.x, pb.y, pb.z};
     float xw[3] = {0.f, 0.f, 0.f}, vv[3] = {0.f, 0.f, 0.f};
 #pragma unroll
     for (int k = 0; k < DIM; ++k) {
         float xv = x[i * DIM + k];
-        xw[k] = kp.periodic[k] ? wrap_coord(xv, kp.lo[k], kp.hi[k], kp.L[k]) : xv;
+        if (kp.periodic[k]) {
+            // the periodic image next to the build position: a particle that drifted across a face since the
+            // build stays in the frame of its build cell (the tile kernels shift whole halo cells, not pairs)
+            xv = wrap_coord(xv, kp.lo[k], kp.hi[k], kp.L[k]);
+            const float dd = xv - xb[k];
+            xv = dd > kp.halfL[k] ? xv - kp.L[k] : (dd < -kp.halfL[k] ? xv + kp.L[k] : xv);
+        }
+        xw[k] = xv;
         vv[k] = v[i * DIM + k];
     }
-    const float r = rho[i], mi = m[i], h = pos_s[p].w;
+    const float r = rho[i], mi = m[i], h = pb.w;
     const float u = (r - kp.rho0) / kp.rho0;
     const float lg = log1pf(u);
     const float ugm1 = expm1f(kp.gamma * lg);        // (rho/rho0)^gamma - 1
@@ -549,6 +527,7 @@ int sph_launch_rhs_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
     const uint32_t *perm = ctx->perm.as<uint32_t>();
     const bool sorted = out4 != nullptr;
     KScope ks(ctx, SPH_K_RHS, 1, st);
+    if (ctx->tile_mode) return sph_launch_rhs_tile(ctx, kp, s0, s1, s2, kind_s, drho, acc, out4, st);
 #define SPH_RHS_LAUNCH(DIM, GS, VARH, SORTED)                                                                     \
     k_rhs<DIM, GS, VARH, SORTED><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, s0, s1, s2, kind_s, rp, col, \
                                                                      perm, drho, acc, out4)
@@ -584,10 +563,13 @@ int sph_launch_vjp_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
     const uint32_t *perm = ctx->perm.as<uint32_t>();
     const bool sorted = xb4 != nullptr;
     const int gs = ctx->opt_group ? ctx->opt_group : (kp.dim == 3 ? 32 : 16);
-    const unsigned grid = pair_grid(n, gs);
+    const unsigned grid = ctx->tile_mode ? (unsigned)ctx->tg.ntiles : pair_grid(n, gs);
     SPH_TRY(ctx->partials.reserve((size_t)grid * kNPart * 4));
     float *part = ctx->partials.as<float>();
-    {
+    if (ctx->tile_mode) {
+        KScope ks(ctx, SPH_K_VJP, 1, st);
+        SPH_TRY(sph_launch_vjp_tile(ctx, kp, s0, s1, s2, cot, eos, xb, vb, rb, xb4, vb4, part, st));
+    } else {
     KScope ks(ctx, SPH_K_VJP, 1, st);
 #define SPH_VJP_LAUNCH(DIM, GS, VARH, SORTED)                                                                  \
     k_vjp<DIM, GS, VARH, SORTED><<<grid, kBlock, 0, st>>>(n, kp, margin, s0, s1, s2, cot, eos, rp, col, perm, xb, \
@@ -632,6 +614,7 @@ extern "C" int sph_density(sph_ctx *ctx, const float *m, float *rho_out, sph_str
     SPH_TRY(ctx->m_s.reserve((size_t)n * 4));
     KScope ks(ctx, SPH_K_DENSITY, 2, st);
     k_gather_f32<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), m, ctx->m_s.as<float>());
+    if (ctx->tile_mode) return sph_launch_density_tile(ctx, kp, ctx->m_s.as<float>(), rho_out, st);
     const float margin = seam_margin(ctx);
 #define SPH_DENS_LAUNCH(DIM, GS, VARH)                                                                               \
     k_density<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(),           \

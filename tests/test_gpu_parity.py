@@ -7,7 +7,7 @@ import torch
 
 import oracle
 from paper_2507_21684_b200 import workloads as W
-from paper_2507_21684_b200.binding import Sph, SphError
+from paper_2507_21684_b200.binding import Sph, SphError, OPT_LIST_MODE, OPT_TILE_EDGE, LIST_GENERIC
 from common import max_norm_err
 from gpu_common import Dev, build, oracle_lists
 
@@ -33,11 +33,31 @@ def _np(t):
     return t.detach().cpu().numpy()
 
 
-@pytest.fixture(scope="module")
-def sph():
+# every test runs on both list layouts of the library (include/sph.h, SPH_OPT_LIST_MODE): "tile" = automatic choice
+# (tile-local 16-bit lists + shared-memory halo kernels wherever a halo fits), "generic" = 32-bit lists + global
+# gathers, "tile_b1" = tile-local lists on single-cell blocks
+@pytest.fixture(scope="module", params=["tile", "generic", "tile_b1"])
+def sph(request):
     s = Sph(0)
+    s.layout_name = request.param
+    if request.param == "generic":
+        s.set_option(OPT_LIST_MODE, LIST_GENERIC)
+    elif request.param == "tile_b1":
+        s.set_option(OPT_TILE_EDGE, 1)
     yield s
     s.close()
+
+
+def test_layout_is_the_requested_one(sph):
+    for case in ("C0p", "C2s", "C3p", "C4s"):
+        build(CASES[case](), 1.0, sph)
+        lay = sph.layout()
+        if sph.layout_name == "generic":
+            assert lay["mode"] == 1
+        else:
+            assert lay["mode"] == 2 and lay["halo_max"] > 0
+            if sph.layout_name == "tile_b1":
+                assert lay["tile_edge"] == 1
 
 
 # ------------------------------------------------------------------------------------------ lists
@@ -245,6 +265,8 @@ def test_host_entry_point_matches_device_calls(sph):
 def test_full_size_sampled_rows(sph, cfg):
     """BASELINE.json's full sizes in the launch configuration bench.py times: lists compared in full (bit-exact),
     RHS / VJP on sampled rows the oracle computes one by one."""
+    if sph.layout_name == "tile_b1":
+        pytest.skip("full sizes run on the automatic and the generic layout")
     wl = W.make(cfg)
     if cfg == 3:
         wl = W.perturbed(wl, amp_x=0.1, amp_rho=0.01)        # the state after a few steps: disordered lattice
