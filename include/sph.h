@@ -184,7 +184,8 @@ enum {
                                (32-bit sorted ids, neighbour state gathered through L1/L2, any cell occupancy);
                                2 = tile-local (16-bit indices into the halo of a block of cells, neighbour state staged
                                in shared memory).  2 falls back to 1 when a halo does not fit shared memory. */
-    SPH_OPT_TILE_EDGE = 3   /* edge of the cell blocks of the tile-local layout: 1, 2, 4 cells; 0 = automatic */
+    SPH_OPT_TILE_EDGE = 3,  /* edge of the cell blocks of the tile-local layout: 1, 2, 4 cells; 0 = automatic */
+    SPH_OPT_PAIR_WARPS = 4  /* warps per CTA of the tile pair kernels: 4, 8, 16; 0 = automatic */
 };
 int sph_set_option(sph_ctx *ctx, int key, int value);
 int sph_profile_enable(sph_ctx *ctx, int on);

@@ -236,6 +236,10 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
         if (value < 0 || value > 2) return SPH_E_INVALID;
         ctx->opt_list_mode = value;
         return SPH_OK;
+    case SPH_OPT_PAIR_WARPS:
+        if (value != 0 && value != 4 && value != 8 && value != 16) return SPH_E_INVALID;
+        ctx->opt_warps = value;
+        return SPH_OK;
     case SPH_OPT_TILE_EDGE:
         if (value != 0 && value != 1 && value != 2 && value != 4) return SPH_E_INVALID;
         ctx->opt_tile_edge = value;

@@ -122,6 +122,7 @@ struct sph_ctx {
     int device = 0;
     Profiler prof;
     int opt_group = 0;          // lanes per row in the pair kernels (0 = default)
+    int opt_warps = 0;          // warps per CTA of the tile pair kernels (0 = automatic: 8, or 16 when one CTA fits an SM)
     int opt_list_mode = 0;      // 0 auto, 1 force the generic (global-id) lists, 2 force tile-local lists
     int opt_tile_edge = 0;      // 0 auto, else force the tile edge B (1, 2, 4)
     bool tile_mode = false;     // lists of the last sph_neighbors are tile-local (col16)
@@ -190,13 +191,13 @@ struct KScope {
 __device__ __forceinline__ float fast_sqrt(float x)
 {
     float r;
-    asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));   // one MUFU.SQRT (no denormal fix-up code)
     return r;
 }
 __device__ __forceinline__ float fast_rcp(float x)
 {
     float r;
-    asm("rcp.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));    // one MUFU.RCP
     return r;
 }
 

@@ -4,7 +4,10 @@
 //
 // One CTA per tile.  The halo positions are staged in shared memory once.  A warp takes 32 rows OF ONE CELL, one
 // row per lane: all lanes walk the same candidate sequence, so every candidate is ONE broadcast shared-memory load
-// and ~11 instructions for 32 row-candidate tests (the first path of this round spent 110 per 32).  Hits go to a
+// and 9 instructions for 32 row-candidate tests (the first path of this round spent 110 per 32): the verdict is the
+// sign bit of r2 - Hs2, funnel-shifted into a per-lane 32-candidate mask; the binary64 predicate of reading R3 runs
+// only for blocks whose closest call falls inside the fp32 uncertainty band.  Count = popc of the masks; fill
+// expands the masks into a
 // per-warp shared-memory image of the warp's contiguous col16 segment (rows of a cell are contiguous in the
 // sorted order, so their list segments are too), which is then flushed coalesced.  Deterministic: fixed candidate
 // order (cells in z,y,x order, ascending sorted index inside a cell), no atomics.
@@ -17,20 +20,40 @@
 namespace {
 
 constexpr int kNbWarps = 8;
-constexpr int kNbBlk = 8;        // candidates per unrolled block
 
 struct RowCtx {
     float4 pi;         // own position (+h)
     float Hs2, tol;    // uniform h: thresholds of the fp32 test
     uint32_t n;        // hits so far
-    uint32_t cap;      // FILL: length of the row (from the count pass)
 };
 
-// One candidate.  EXACT: resolve the "too close to call" band with the binary64 predicate (reading R3).
-template <int DIM, bool VARH, bool EXACT>
-__device__ __forceinline__ bool nb_test(const RowCtx &rc, const float4 &pj, const SearchPar &sp, bool seam, uint32_t q,
-                                        const TileTab &tt, const float4 *__restrict__ pos_s, const GridGeom &gg,
-                                        bool &unsure)
+// fp32 test of one candidate: shifts the verdict (sign of r2 - Hs2) into the mask and tracks how close to the
+// threshold the block came.  9 instructions per candidate when h is uniform.
+template <int DIM, bool VARH>
+__device__ __forceinline__ void nb_test(const RowCtx &rc, const float4 &pj, const SearchPar &sp, bool seam, uint32_t &m,
+                                        float &amin)
+{
+    const float d0 = rc.pi.x - pj.x, d1 = rc.pi.y - pj.y, d2 = DIM == 3 ? rc.pi.z - pj.z : 0.f;
+    const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
+    if (VARH) {
+        const float Hs = __fmul_rn(sp.scale, fmaxf(rc.pi.w, pj.w));
+        const float Hs2 = Hs * Hs;
+        const float tol = sp.band * (seam ? fmaf(Hs, sp.Lmax, Hs2) : Hs2);
+        const float diff = r2 - Hs2;
+        m = __funnelshift_l(__float_as_uint(diff), m, 1);       // m = (m << 1) | (diff < 0)
+        amin = fminf(amin, fabsf(diff) - tol);
+    } else {
+        const float diff = r2 - rc.Hs2;
+        m = __funnelshift_l(__float_as_uint(diff), m, 1);
+        amin = fminf(amin, fabsf(diff));
+    }
+}
+
+// the same test with the "too close to call" band resolved by the binary64 predicate (reading R3)
+template <int DIM, bool VARH>
+__device__ __forceinline__ bool nb_test_exact(const RowCtx &rc, const float4 &pj, const SearchPar &sp, bool seam,
+                                              uint32_t q, const TileTab &tt, const float4 *__restrict__ pos_s,
+                                              const GridGeom &gg)
 {
     const float d0 = rc.pi.x - pj.x, d1 = rc.pi.y - pj.y, d2 = DIM == 3 ? rc.pi.z - pj.z : 0.f;
     const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
@@ -42,36 +65,34 @@ __device__ __forceinline__ bool nb_test(const RowCtx &rc, const float4 &pj, cons
     }
     const float diff = r2 - Hs2;
     bool hit = diff < 0.f;
-    const bool band = fabsf(diff) <= tol;
-    if (EXACT) {
-        if (band) hit = pred_exact(rc.pi, pos_s[tile_q_to_sorted(tt, q)], Hs, gg);
-    } else {
-        unsure = unsure || band;
-    }
+    if (fabsf(diff) <= tol) hit = pred_exact(rc.pi, pos_s[tile_q_to_sorted(tt, q)], Hs, gg);
     return hit;
 }
 
-// `dst`: FILL only -- where this lane's hits go (shared-memory image or global col16), indexed by rc.n
-template <int DIM, bool FILL, bool VARH, bool EXACT, class DstT>
-__device__ __forceinline__ void nb_block(RowCtx &rc, const float4 *__restrict__ cand, uint32_t q, int nq,
-                                         const SearchPar &sp, bool seam, const TileTab &tt,
-                                         const float4 *__restrict__ pos_s, const GridGeom &gg, DstT dst, bool &unsure)
+// Hit mask of the nq <= 32 candidates q .. q+nq-1 for this lane's row: candidate u at bit nq-1-u.
+template <int DIM, bool VARH, bool FULL>
+__device__ __forceinline__ uint32_t nb_mask(const RowCtx &rc, const float4 *__restrict__ cand, uint32_t q, int nq,
+                                            const SearchPar &sp, bool seam, const TileTab &tt,
+                                            const float4 *__restrict__ pos_s, const GridGeom &gg)
 {
+    uint32_t m = 0;
+    float amin = 3.0e38f;
+    if (FULL) {
 #pragma unroll
-    for (int u = 0; u < kNbBlk; ++u) {
-        if (u < nq) {
-            const float4 pj = cand[q + u];
-            const bool hit = nb_test<DIM, VARH, EXACT>(rc, pj, sp, seam, q + u, tt, pos_s, gg, unsure);
-            if (FILL) {
-                // rc.n < rc.cap: the speculative fp32 pass of a block that is then redone exactly may see more
-                // hits than the row has; it must not write into the next row's segment
-                if (hit && rc.n < rc.cap) dst[rc.n] = (uint16_t)(q + u);
-            }
-            rc.n += hit ? 1u : 0u;
-        }
+        for (int u = 0; u < 32; ++u) nb_test<DIM, VARH>(rc, cand[q + u], sp, seam, m, amin);
+    } else {
+#pragma unroll 4
+        for (int u = 0; u < nq; ++u) nb_test<DIM, VARH>(rc, cand[q + u], sp, seam, m, amin);
     }
+    if (amin <= (VARH ? 0.f : rc.tol)) {              // rare (except on exact lattices): redo the block exactly
+        m = 0;
+        for (int u = 0; u < nq; ++u)
+            m = (m << 1) | (nb_test_exact<DIM, VARH>(rc, cand[q + u], sp, seam, q + u, tt, pos_s, gg) ? 1u : 0u);
+    }
+    return m;
 }
 
+// `dst`: FILL only -- where this lane's hits go (shared-memory image or global col16), indexed by rc.n
 template <int DIM, bool FILL, bool VARH, class DstT>
 __device__ __forceinline__ void nb_rows(RowCtx &rc, const float4 *__restrict__ cand, const int sl[3], const SearchPar &sp,
                                         bool seam, const TileTab &tt, const float4 *__restrict__ pos_s,
@@ -87,16 +108,19 @@ __device__ __forceinline__ void nb_rows(RowCtx &rc, const float4 *__restrict__ c
             const int rowbase = tt.ext[0] * (sy + tt.ext[1] * sz);
             const int xa = max(sl[0] - 1, 0), xb = min(sl[0] + 1, tt.ext[0] - 1);
             const uint32_t q0 = tt.h_off[rowbase + xa], q1 = tt.h_off[rowbase + xb + 1];
-            for (uint32_t q = q0; q < q1; q += kNbBlk) {
-                const int nq = min((uint32_t)kNbBlk, q1 - q);
-                const uint32_t n0 = rc.n;
-                bool unsure = false;
-                if (nq == kNbBlk) nb_block<DIM, FILL, VARH, false>(rc, cand, q, kNbBlk, sp, seam, tt, pos_s, gg, dst, unsure);
-                else nb_block<DIM, FILL, VARH, false>(rc, cand, q, nq, sp, seam, tt, pos_s, gg, dst, unsure);
-                if (unsure) {                      // rare (except on exact lattices): redo the block exactly
-                    rc.n = n0;
-                    bool dummy = false;
-                    nb_block<DIM, FILL, VARH, true>(rc, cand, q, nq, sp, seam, tt, pos_s, gg, dst, dummy);
+            for (uint32_t q = q0; q < q1; q += 32) {
+                const int nq = min(32u, q1 - q);
+                uint32_t m = nq == 32 ? nb_mask<DIM, VARH, true>(rc, cand, q, 32, sp, seam, tt, pos_s, gg)
+                                      : nb_mask<DIM, VARH, false>(rc, cand, q, nq, sp, seam, tt, pos_s, gg);
+                if (FILL) {
+                    const uint32_t qtop = q + (uint32_t)nq - 1u;      // candidate of bit 0
+                    while (m) {                                         // ascending candidate order = descending bits
+                        const int hb = 31 - __clz(m);
+                        m ^= 1u << hb;
+                        dst[rc.n++] = (uint16_t)(qtop - (uint32_t)hb);
+                    }
+                } else {
+                    rc.n += __popc(m);
                 }
             }
         }
@@ -155,7 +179,6 @@ k_nb_tile(TileGeom tg, GridGeom gg, SearchPar sp, int mcap, int wcap, const floa
             rc.Hs2 = sp.Hs_u * sp.Hs_u;
             rc.tol = sp.band * (seam ? fmaf(sp.Hs_u, sp.Lmax, rc.Hs2) : rc.Hs2);
             rc.n = 0;
-            rc.cap = 0;
             if (!FILL) {
                 nb_rows<DIM, false, VARH>(rc, cand, sl, sp, seam, tt, pos_s, gg, (uint16_t *)nullptr);
                 if (active) cnt[row] = rc.n;
@@ -163,7 +186,6 @@ k_nb_tile(TileGeom tg, GridGeom gg, SearchPar sp, int mcap, int wcap, const floa
                 const uint32_t row_first = tt.h_start[hc_i] + c0;
                 const long long seg0 = row_ptr[row_first], seg1 = row_ptr[row_first + nact];
                 const long long mine = row_ptr[row];
-                rc.cap = (uint32_t)(row_ptr[row + 1] - mine);
                 const uint32_t total = (uint32_t)(seg1 - seg0);
                 if (total <= (uint32_t)wcap) {
                     // inactive lanes duplicate lane 0 and write the same values to the same places

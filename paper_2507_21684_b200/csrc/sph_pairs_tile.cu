@@ -2,9 +2,10 @@
 // decomposition of sph_tiles.cuh.  One CTA per tile:
 //   1. the sorted state of the tile's halo ((B+2)^d cells, each a contiguous run of the sorted SoA) is staged in
 //      shared memory, positions shifted by -+L across periodic seams (no minimum image in the inner loop);
-//   2. GS lanes share a row, stride over the row's uint16 halo indices (2 B per pair from HBM, coalesced) and gather
-//      the neighbour state with LDS.128 from shared memory (~10 wavefronts per 32 pairs instead of ~32 L1 wavefronts
-//      of the global-gather kernels, profiles/r01_b);
+//   2. GS lanes share a row.  The uint16 halo indices of the rows a warp works on next (2 B per pair, the only
+//      per-pair HBM traffic) are prefetched one pass ahead into a per-warp shared-memory ring with cp.async, so the
+//      inner loop contains no global load: LDS.U16 index -> LDS.128 gathers of the neighbour state
+//      (~10 shared-memory wavefronts per 32 pairs instead of ~32 L1 wavefronts of global gathers, profiles/r01_b);
 //   3. shuffle reduction inside the lane group, one writer per row.  No float atomics; fixed summation order.
 // Formulas: include/sph.h header comment and DESIGN.md section 2 (Eq.8, 9, 12, 40, 42, 7).
 #include "sph_internal.cuh"
@@ -15,8 +16,7 @@
 
 namespace {
 
-constexpr int kPtWarps = 8;
-constexpr int kPtBlock = kPtWarps * 32;
+constexpr int kPtMaxWarps = 16;
 
 template <int GS>
 __device__ __forceinline__ float group_sum(float v)
@@ -31,8 +31,8 @@ template <int DIM, bool SHIFT>
 __device__ __forceinline__ void stage4(const TileGeom &tg, const TileTab &tt, const float4 *__restrict__ src,
                                        float4 *__restrict__ dst)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int hc = warp; hc < tt.nh; hc += kPtWarps) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    for (int hc = warp; hc < tt.nh; hc += nwarps) {
         const uint32_t o0 = tt.h_off[hc], o1 = tt.h_off[hc + 1];
         if (o1 == o0) continue;
         float sh[3] = {0.f, 0.f, 0.f};
@@ -52,66 +52,84 @@ __device__ __forceinline__ void stage4(const TileGeom &tg, const TileTab &tt, co
 template <class T>
 __device__ __forceinline__ void stage_plain(const TileTab &tt, const T *__restrict__ src, T *__restrict__ dst)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int hc = warp; hc < tt.nh; hc += kPtWarps) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    for (int hc = warp; hc < tt.nh; hc += nwarps) {
         const uint32_t o0 = tt.h_off[hc], o1 = tt.h_off[hc + 1];
         const T *s = src + tt.h_start[hc];
         for (uint32_t q = lane; q < o1 - o0; q += 32) dst[o0 + q] = s[q];
     }
 }
-// tile-relative row offsets: rp[r] = row_ptr[row0 + r] - row_ptr[row0], r = 0..T
-__device__ __forceinline__ void stage_rowptr(const TileTab &tt, const long long *__restrict__ row_ptr, uint32_t *rp)
+// tile-relative row offsets rp[r] = row_ptr[row0 + r] - row_ptr[row0], r = 0..T, and the halo index of every row
+__device__ __forceinline__ void stage_rows(const TileTab &tt, const long long *__restrict__ row_ptr, uint32_t *rp,
+                                           uint16_t *selfq)
 {
     const long long base = row_ptr[tt.row0];
-    for (uint32_t r = threadIdx.x; r <= tt.T; r += kPtBlock) rp[r] = (uint32_t)(row_ptr[tt.row0 + r] - base);
+    for (uint32_t r = threadIdx.x; r <= tt.T; r += blockDim.x) rp[r] = (uint32_t)(row_ptr[tt.row0 + r] - base);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    for (int tc = warp; tc < tt.nt; tc += nwarps) {
+        const int hc = tt.t_cell[tc];
+        const uint32_t o0 = tt.h_off[hc], cnt = tt.h_off[hc + 1] - o0;
+        const uint32_t rbase = tt.h_start[hc] - tt.row0;
+        for (uint32_t l = lane; l < cnt; l += 32) selfq[rbase + l] = (uint16_t)(o0 + l);
+    }
 }
 
-// ------------------------------------------------------------------------------------------ D: density
-// smem: A = {x,y,z,h}[mcap], M = m[mcap], rp[mcap+1]
-template <int DIM, int GS, bool VARH>
-__global__ void __launch_bounds__(kPtBlock)
-k_density_tile(TileGeom tg, KPar kp, int mcap, const float4 *__restrict__ pos_s, const float *__restrict__ m_s,
-               const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
-               const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16,
-               const uint32_t *__restrict__ perm, float *__restrict__ rho_out)
+// ------------------------------------------------------------------------------------------ index ring
+__device__ __forceinline__ void cp_async16(uint32_t smem_addr, const void *gptr)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4 *A = reinterpret_cast<float4 *>(smem_raw);
-    float *Ms = reinterpret_cast<float *>(smem_raw + (size_t)mcap * 16);
-    uint32_t *rp = reinterpret_cast<uint32_t *>(smem_raw + (size_t)mcap * 20);
-    __shared__ TileTab tt;
-    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
-    if (tt.T == 0) return;
-    stage4<DIM, true>(tg, tt, pos_s, A);
-    stage_plain<float>(tt, m_s, Ms);
-    stage_rowptr(tt, row_ptr, rp);
-    __syncthreads();
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// Drives the rows of a tile through `body(r, live, b, e, idx)`: row r of the tile (clamped to T-1; `live` false for
+// the padding groups of the last pass), its tile-relative entry range [b,e), and a pointer such that idx[k] is the
+// halo index of entry k.  A warp works on RPW = 32/GS consecutive rows per pass; the contiguous index segment of
+// its NEXT pass is copied into the other half of its ring (16-byte cp.async chunks) before the current pass is
+// processed.  A segment that does not fit the ring is read from global memory directly (correct, slower).
+template <int GS, class Body>
+__device__ __forceinline__ void tile_row_passes(const TileTab &tt, const uint32_t *rp, uint16_t *ring, int rb,
+                                                const uint16_t *__restrict__ col16, long long tilebase, Body body)
+{
     constexpr int RPW = 32 / GS;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane / GS, gl = lane % GS;
-    const uint16_t *cp = col16 + row_ptr[tt.row0];
-    const HC hu = hc_uniform<DIM>(kp);
-    for (uint32_t r0 = warp * RPW; r0 < tt.T; r0 += kPtWarps * RPW) {
-        const uint32_t r = min(r0 + g, tt.T - 1);
-        const float4 pi = pos_s[tt.row0 + r];
-        const uint32_t b = rp[r], e = rp[r + 1];
-        float acc = 0.f;
-#pragma unroll 4
-        for (uint32_t k = b + gl; k < e; k += GS) {
-            const uint32_t j = cp[k];
-            const float4 pj = A[j];
-            const float d0 = pi.x - pj.x, d1 = pi.y - pj.y, d2 = DIM == 3 ? pi.z - pj.z : 0.f;
-            const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
-            HC hc = hu;
-            if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
-            const float q = fast_sqrt(r2) * hc.invH;
-            const float t = fmaxf(1.0f - q, 0.f);
-            const float t2 = t * t, t6 = t2 * t2 * t2;
-            const float w = hc.cW * t6 * fmaf(q, fmaf(q, 35.0f / 3.0f, 6.0f), 1.0f);   // Eq.25/27
-            acc = fmaf(Ms[j], w, acc);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int g = lane / GS;
+    const uint32_t T = tt.T;
+    const uint32_t step = nwarps * RPW;
+    uint16_t *myring = ring + (size_t)warp * 2 * rb;
+    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(myring);
+
+    auto issue = [&](uint32_t r0, int buf) {
+        if (r0 < T) {
+            const long long a = tilebase + rp[r0], e = tilebase + rp[min(r0 + RPW, T)];
+            const long long a0 = a & ~7ll;
+            const uint32_t nchunk = (uint32_t)((e - a0 + 7) >> 3);
+            if (nchunk * 8 <= (uint32_t)rb)
+                for (uint32_t c = lane; c < nchunk; c += 32)
+                    cp_async16(ring_s + (uint32_t)(buf * rb + c * 8) * 2, col16 + a0 + c * 8);
         }
-        acc = group_sum<GS>(acc);
-        if (gl == 0 && r0 + g < tt.T) rho_out[perm[tt.row0 + r]] = acc;
+        cp_async_commit();
+    };
+    int buf = 0;
+    issue(warp * RPW, 0);
+    for (uint32_t r0 = warp * RPW; r0 < T; r0 += step, buf ^= 1) {
+        issue(r0 + step, buf ^ 1);
+        cp_async_wait<1>();
+        __syncwarp();
+        const uint32_t r = min(r0 + g, T - 1);
+        const bool live = r0 + g < T;
+        const uint32_t b = rp[r], e = rp[r + 1];
+        const uint32_t s = rp[r0];
+        const long long a = tilebase + s, e_seg = tilebase + rp[min(r0 + RPW, T)];
+        const long long a0 = a & ~7ll;
+        if ((uint32_t)((e_seg - a0 + 7) >> 3) * 8 <= (uint32_t)rb)
+            body(r, live, b, e, (const uint16_t *)(myring + buf * rb + (uint32_t)(a - a0)) - s);
+        else
+            body(r, live, b, e, col16 + tilebase);
+        __syncwarp();
     }
+    cp_async_wait<0>();
 }
 
 // sorted state of one particle as the pair loops see it
@@ -136,114 +154,165 @@ __device__ __forceinline__ Part load_part(const float4 *s0, const float4 *s1, co
     return p;
 }
 
-// shared-memory carve-up of the pair kernels: A, B (float4[mcap]), C (float2[mcap], 3D only), [cot float4[mcap]], rp
+// shared-memory carve-up: A, B (float4[mcap]), [cot float4[mcap]], C (float2[mcap], 3D only), rp[tcap+1],
+// selfq[tcap], index ring [nwarps][2][rb]
+struct TileSizes {
+    int mcap, tcap, rb;
+};
 template <int DIM>
 struct SmemMap {
     float4 *A, *B, *cot;
     float2 *C;
     uint32_t *rp;
-    __device__ SmemMap(unsigned char *base, int mcap, bool with_cot)
+    uint16_t *selfq, *ring;
+    __device__ SmemMap(unsigned char *base, const TileSizes &ts, bool with_cot)
     {
         size_t o = 0;
-        A = reinterpret_cast<float4 *>(base + o); o += (size_t)mcap * 16;
-        B = reinterpret_cast<float4 *>(base + o); o += (size_t)mcap * 16;
-        cot = reinterpret_cast<float4 *>(base + o); if (with_cot) o += (size_t)mcap * 16;
-        C = reinterpret_cast<float2 *>(base + o); if (DIM == 3) o += (size_t)mcap * 8;
-        rp = reinterpret_cast<uint32_t *>(base + o);
+        A = reinterpret_cast<float4 *>(base + o); o += (size_t)ts.mcap * 16;
+        B = reinterpret_cast<float4 *>(base + o); o += (size_t)ts.mcap * 16;
+        cot = reinterpret_cast<float4 *>(base + o); if (with_cot) o += (size_t)ts.mcap * 16;
+        C = reinterpret_cast<float2 *>(base + o); if (DIM == 3) o += (size_t)ts.mcap * 8;
+        rp = reinterpret_cast<uint32_t *>(base + o); o += (size_t)(ts.tcap + 4) * 4;
+        selfq = reinterpret_cast<uint16_t *>(base + o); o += (size_t)ts.tcap * 2;
+        o = (o + 15) & ~(size_t)15;
+        ring = reinterpret_cast<uint16_t *>(base + o);
     }
 };
+
+// ------------------------------------------------------------------------------------------ D: density
+// smem: A = {x,y,z,h}[mcap], Ms = m[mcap] (in the B slot), rp, selfq, ring
+template <int DIM, int GS, bool VARH>
+__global__ void __launch_bounds__(kPtMaxWarps * 32)
+k_density_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ pos_s, const float *__restrict__ m_s,
+               const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
+               const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16,
+               const uint32_t *__restrict__ perm, float *__restrict__ rho_out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const SmemMap<DIM> sm(smem_raw, ts, false);
+    float *Ms = reinterpret_cast<float *>(sm.B);
+    __shared__ TileTab tt;
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (tt.T == 0) return;
+    stage4<DIM, true>(tg, tt, pos_s, sm.A);
+    stage_plain<float>(tt, m_s, Ms);
+    stage_rows(tt, row_ptr, sm.rp, sm.selfq);
+    __syncthreads();
+    const int gl = (threadIdx.x & 31) % GS;
+    const HC hu = hc_uniform<DIM>(kp);
+    const float4 *A = sm.A;
+    const uint16_t *selfq = sm.selfq;
+    const uint32_t row0 = tt.row0;
+    tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
+        [&](uint32_t r, bool live, uint32_t b, uint32_t e, const uint16_t *idx) {
+            const float4 pi = A[selfq[r]];
+            float acc = 0.f;
+#pragma unroll 4
+            for (uint32_t k = b + gl; k < e; k += GS) {
+                const uint32_t j = idx[k];
+                const float4 pj = A[j];
+                const float d0 = pi.x - pj.x, d1 = pi.y - pj.y, d2 = DIM == 3 ? pi.z - pj.z : 0.f;
+                const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
+                HC hc = hu;
+                if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+                const float q = fast_sqrt(r2) * hc.invH;
+                const float t = fmaxf(1.0f - q, 0.f);
+                const float t2 = t * t, t6 = t2 * t2 * t2;
+                const float w = hc.cW * t6 * fmaf(q, fmaf(q, 35.0f / 3.0f, 6.0f), 1.0f);   // Eq.25/27
+                acc = fmaf(Ms[j], w, acc);
+            }
+            acc = group_sum<GS>(acc);
+            if (gl == 0 && live) rho_out[perm[row0 + r]] = acc;
+        });
+}
 
 // ------------------------------------------------------------------------------------------ R1: RHS
 // OUT_SORTED: write float4 {a, drho/dt} in sorted order (RK stages); else scatter to the caller's arrays.
 template <int DIM, int GS, bool VARH, bool OUT_SORTED>
-__global__ void __launch_bounds__(kPtBlock)
-k_rhs_tile(TileGeom tg, KPar kp, int mcap, const float4 *__restrict__ s0, const float4 *__restrict__ s1,
+__global__ void __launch_bounds__(kPtMaxWarps * 32)
+k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, const float4 *__restrict__ s1,
            const float2 *__restrict__ s2, const uint8_t *__restrict__ kind_s, const uint32_t *__restrict__ cell_start,
            const uint32_t *__restrict__ cell_end, const long long *__restrict__ row_ptr,
            const uint16_t *__restrict__ col16, const uint32_t *__restrict__ perm, float *__restrict__ drho_out,
            float *__restrict__ acc_out, float4 *__restrict__ out4)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const SmemMap<DIM> sm(smem_raw, mcap, false);
+    const SmemMap<DIM> sm(smem_raw, ts, false);
     __shared__ TileTab tt;
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
     if (tt.T == 0) return;
-    if (DIM == 3) {
-        stage4<DIM, true>(tg, tt, s0, sm.A);
-        stage_plain<float4>(tt, s1, sm.B);
-        stage_plain<float2>(tt, s2, sm.C);
-    } else {
-        stage4<DIM, true>(tg, tt, s0, sm.A);
-        stage_plain<float4>(tt, s1, sm.B);
-    }
-    stage_rowptr(tt, row_ptr, sm.rp);
+    stage4<DIM, true>(tg, tt, s0, sm.A);
+    stage_plain<float4>(tt, s1, sm.B);
+    if (DIM == 3) stage_plain<float2>(tt, s2, sm.C);
+    stage_rows(tt, row_ptr, sm.rp, sm.selfq);
     __syncthreads();
-    constexpr int RPW = 32 / GS;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane / GS, gl = lane % GS;
-    const uint16_t *cp = col16 + row_ptr[tt.row0];
+    const int gl = (threadIdx.x & 31) % GS;
     const HC hu = hc_uniform<DIM>(kp);
     const float rho0 = kp.rho0;
-    for (uint32_t r0 = warp * RPW; r0 < tt.T; r0 += kPtWarps * RPW) {
-        const uint32_t r = min(r0 + g, tt.T - 1);
-        const uint32_t row = tt.row0 + r;
-        const Part pi = load_part<DIM>(s0, s1, s2, row);
-        const uint32_t b = sm.rp[r], e = sm.rp[r + 1];
-        const float visc_i = rho0 / pi.rho;               // rho0/rho_i of the viscous term
-        const float ev_u = hu.eta * visc_i;
-        float sA = 0.f, sD = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f;
+    const float4 *A = sm.A, *B = sm.B;
+    const float2 *C = sm.C;
+    const uint16_t *selfq = sm.selfq;
+    const uint32_t row0 = tt.row0;
+    tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
+        [&](uint32_t r, bool live, uint32_t b, uint32_t e, const uint16_t *idx) {
+            const Part pi = load_part<DIM>(A, B, C, selfq[r]);
+            const float visc_i = rho0 / pi.rho;               // rho0/rho_i of the viscous term
+            const float ev_u = hu.eta * visc_i;
+            float sA = 0.f, sD = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f;
 #pragma unroll 2
-        for (uint32_t k = b + gl; k < e; k += GS) {
-            const uint32_t j = cp[k];
-            const Part pj = load_part<DIM>(sm.A, sm.B, sm.C, j);
-            const float d0 = pi.x[0] - pj.x[0], d1 = pi.x[1] - pj.x[1], d2 = DIM == 3 ? pi.x[2] - pj.x[2] : 0.f;
-            const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
-            HC hc = hu;
-            float ev = ev_u;
-            if (VARH) {
-                hc = hc_make<DIM>(fmaxf(pi.h, pj.h), kp);
-                ev = hc.eta * visc_i;
+            for (uint32_t k = b + gl; k < e; k += GS) {
+                const uint32_t j = idx[k];
+                const Part pj = load_part<DIM>(A, B, C, j);
+                const float d0 = pi.x[0] - pj.x[0], d1 = pi.x[1] - pj.x[1], d2 = DIM == 3 ? pi.x[2] - pj.x[2] : 0.f;
+                const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
+                HC hc = hu;
+                float ev = ev_u;
+                if (VARH) {
+                    hc = hc_make<DIM>(fmaxf(pi.h, pj.h), kp);
+                    ev = hc.eta * visc_i;
+                }
+                const float rr = fast_sqrt(r2);
+                const float t = fmaxf(fmaf(-hc.invH, rr, 1.0f), 0.f);   // (1-q)+ : skin pairs contribute exactly 0
+                const float t2 = t * t, t4 = t2 * t2;
+                const float G = hc.cG * fmaf(5.0f * hc.invH, rr, 1.0f) * (t4 * t);
+                float s = (pi.v[0] - pj.v[0]) * d0;
+                s = fmaf(pi.v[1] - pj.v[1], d1, s);
+                if (DIM == 3) s = fmaf(pi.v[2] - pj.v[2], d2, s);
+                const float invR = fast_rcp(r2 + hc.e2);
+                const float VG = pj.V * G;
+                // continuity (Eq.9, physical sign) and delta-term (Brookshaw Laplacian of rho)
+                sA = fmaf(VG, s, sA);
+                const float dterm = VG * (pi.rho - pj.rho) * (r2 * invR);
+                sD = VARH ? fmaf(hc.kd, dterm, sD) : sD + dterm;
+                // pressure (Eq.40, symmetric) + viscosity (Eq.7 with the delta-SPH Pi_ij)
+                const float E = -(pj.V * pj.rho) * (pi.P + pj.P);
+                const float cf = fmaf(ev * pj.V * s, invR, E) * G;
+                a0 = fmaf(cf, d0, a0);
+                a1 = fmaf(cf, d1, a1);
+                if (DIM == 3) a2 = fmaf(cf, d2, a2);
             }
-            const float rr = fast_sqrt(r2);
-            const float t = fmaxf(fmaf(-hc.invH, rr, 1.0f), 0.f);   // (1-q)+ : skin pairs contribute exactly 0
-            const float t2 = t * t, t4 = t2 * t2;
-            const float G = hc.cG * fmaf(5.0f * hc.invH, rr, 1.0f) * (t4 * t);
-            float s = (pi.v[0] - pj.v[0]) * d0;
-            s = fmaf(pi.v[1] - pj.v[1], d1, s);
-            if (DIM == 3) s = fmaf(pi.v[2] - pj.v[2], d2, s);
-            const float invR = fast_rcp(r2 + hc.e2);
-            const float VG = pj.V * G;
-            // continuity (Eq.9, physical sign) and delta-term (Brookshaw Laplacian of rho)
-            sA = fmaf(VG, s, sA);
-            const float dterm = VG * (pi.rho - pj.rho) * (r2 * invR);
-            sD = VARH ? fmaf(hc.kd, dterm, sD) : sD + dterm;
-            // pressure (Eq.40, symmetric) + viscosity (Eq.7 with the delta-SPH Pi_ij)
-            const float E = -(pj.V * pj.rho) * (pi.P + pj.P);
-            const float cf = fmaf(ev * pj.V * s, invR, E) * G;
-            a0 = fmaf(cf, d0, a0);
-            a1 = fmaf(cf, d1, a1);
-            if (DIM == 3) a2 = fmaf(cf, d2, a2);
-        }
-        float dr = pi.rho * sA + (VARH ? sD : hu.kd * sD);
-        dr = group_sum<GS>(dr);
-        a0 = group_sum<GS>(a0);
-        a1 = group_sum<GS>(a1);
-        if (DIM == 3) a2 = group_sum<GS>(a2);
-        if (gl == 0 && r0 + g < tt.T) {
-            const bool fixed = kind_s[row] != 0;
-            a0 = fixed ? 0.f : a0 + kp.g[0];
-            a1 = fixed ? 0.f : a1 + kp.g[1];
-            a2 = fixed ? 0.f : a2 + kp.g[2];
-            if (OUT_SORTED) {
-                out4[row] = make_float4(a0, a1, a2, dr);
-            } else {
-                const int64_t i = perm[row];
-                drho_out[i] = dr;
-                acc_out[i * DIM] = a0;
-                acc_out[i * DIM + 1] = a1;
-                if (DIM == 3) acc_out[i * DIM + 2] = a2;
+            float dr = pi.rho * sA + (VARH ? sD : hu.kd * sD);
+            dr = group_sum<GS>(dr);
+            a0 = group_sum<GS>(a0);
+            a1 = group_sum<GS>(a1);
+            if (DIM == 3) a2 = group_sum<GS>(a2);
+            if (gl == 0 && live) {
+                const uint32_t row = row0 + r;
+                const bool fixed = kind_s[row] != 0;
+                a0 = fixed ? 0.f : a0 + kp.g[0];
+                a1 = fixed ? 0.f : a1 + kp.g[1];
+                a2 = fixed ? 0.f : a2 + kp.g[2];
+                if (OUT_SORTED) {
+                    out4[row] = make_float4(a0, a1, a2, dr);
+                } else {
+                    const int64_t i = perm[row];
+                    drho_out[i] = dr;
+                    acc_out[i * DIM] = a0;
+                    acc_out[i * DIM + 1] = a1;
+                    if (DIM == 3) acc_out[i * DIM + 2] = a2;
+                }
             }
-        }
-    }
+        });
 }
 
 // ------------------------------------------------------------------------------------------ B1: VJP
@@ -254,8 +323,8 @@ k_rhs_tile(TileGeom tg, KPar kp, int mcap, const float4 *__restrict__ s0, const 
 constexpr int kNPartT = 12;   // must match kNPart of sph_pairs.cu (k_reduce_params)
 
 template <int DIM, int GS, bool VARH, bool OUT_SORTED>
-__global__ void __launch_bounds__(kPtBlock)
-k_vjp_tile(TileGeom tg, KPar kp, int mcap, const float4 *__restrict__ s0, const float4 *__restrict__ s1,
+__global__ void __launch_bounds__(kPtMaxWarps * 32)
+k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, const float4 *__restrict__ s1,
            const float2 *__restrict__ s2, const float4 *__restrict__ cot, const float4 *__restrict__ eos,
            const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
            const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16, const uint32_t *__restrict__ perm,
@@ -263,9 +332,9 @@ k_vjp_tile(TileGeom tg, KPar kp, int mcap, const float4 *__restrict__ s0, const 
            float4 *__restrict__ vb4, float *__restrict__ partials)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const SmemMap<DIM> sm(smem_raw, mcap, true);
+    const SmemMap<DIM> sm(smem_raw, ts, true);
     __shared__ TileTab tt;
-    __shared__ float red[kPtWarps][kNPartT];
+    __shared__ float red[kPtMaxWarps][kNPartT];
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
     if (tt.T == 0) {
         if (threadIdx.x < kNPartT) partials[(int64_t)blockIdx.x * kNPartT + threadIdx.x] = 0.f;
@@ -275,124 +344,126 @@ k_vjp_tile(TileGeom tg, KPar kp, int mcap, const float4 *__restrict__ s0, const 
     stage_plain<float4>(tt, s1, sm.B);
     if (DIM == 3) stage_plain<float2>(tt, s2, sm.C);
     stage_plain<float4>(tt, cot, sm.cot);
-    stage_rowptr(tt, row_ptr, sm.rp);
+    stage_rows(tt, row_ptr, sm.rp, sm.selfq);
     __syncthreads();
-    constexpr int RPW = 32 / GS;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane / GS, gl = lane % GS;
-    const uint16_t *cp = col16 + row_ptr[tt.row0];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gl = lane % GS;
     const HC hu = hc_uniform<DIM>(kp);
     const float rho0 = kp.rho0;
+    const float4 *A = sm.A, *B = sm.B, *Ct = sm.cot;
+    const float2 *C = sm.C;
+    const uint16_t *selfq = sm.selfq;
+    const uint32_t row0 = tt.row0;
     float S_D1 = 0.f, S_P1 = 0.f, S_PL = 0.f, S_eps = 0.f;                 // per lane, over all its pairs
     float T_E = 0.f, T_0 = 0.f, T_g = 0.f, G0 = 0.f, G1 = 0.f, G2 = 0.f;   // lane 0 of each group, per row
-    for (uint32_t r0 = warp * RPW; r0 < tt.T; r0 += kPtWarps * RPW) {
-        const bool live = r0 + g < tt.T;
-        const uint32_t r = min(r0 + g, tt.T - 1);
-        const uint32_t row = tt.row0 + r;
-        const Part pi = load_part<DIM>(s0, s1, s2, row);
-        const float4 ci = cot[row];
-        const float4 ei = eos[row];                                // {dP/drho, dP/drho0, dP/dgamma, m}
-        const float lam_i = ci.x, mu_i[3] = {ci.y, ci.z, ci.w};
-        const float m_i = ei.w;
-        const uint32_t b = sm.rp[r], e = live ? sm.rp[r + 1] : b;  // dead groups run no pairs (partials stay clean)
-        const float ir_i = 1.0f / pi.rho;
-        float xb[3] = {0.f, 0.f, 0.f}, vb[3] = {0.f, 0.f, 0.f}, rb = 0.f, Z = 0.f;
-        for (uint32_t k = b + gl; k < e; k += GS) {
-            const uint32_t j = cp[k];
-            const Part pj = load_part<DIM>(sm.A, sm.B, sm.C, j);
-            const float4 cj = sm.cot[j];
-            const float lam_j = cj.x, mu_j[3] = {cj.y, cj.z, cj.w};
-            const float d[3] = {pi.x[0] - pj.x[0], pi.x[1] - pj.x[1], DIM == 3 ? pi.x[2] - pj.x[2] : 0.f};
-            const float r2 = fmaf(d[2], d[2], fmaf(d[1], d[1], d[0] * d[0]));
-            HC hc = hu;
-            if (VARH) hc = hc_make<DIM>(fmaxf(pi.h, pj.h), kp);
-            const float rr = fast_sqrt(r2);
-            const float t = fmaxf(fmaf(-hc.invH, rr, 1.0f), 0.f);
-            const float t2 = t * t, t4 = t2 * t2;
-            const float G = hc.cG * fmaf(5.0f * hc.invH, rr, 1.0f) * (t4 * t);
-            const float K = hc.cK * t4;
-            const float w[3] = {pi.v[0] - pj.v[0], pi.v[1] - pj.v[1], DIM == 3 ? pi.v[2] - pj.v[2] : 0.f};
-            float s = w[0] * d[0];
-            s = fmaf(w[1], d[1], s);
-            if (DIM == 3) s = fmaf(w[2], d[2], s);
-            const float invR = fast_rcp(r2 + hc.e2);
-            const float u = r2 * invR;
-            const float ir_j = 1.0f / pj.rho;
-            const float m_j = pj.V * pj.rho;
-            const float drho = pi.rho - pj.rho;
-            const float Psum = pi.P + pj.P;
-            float mm = mu_i[0] * d[0];                          // mu_i . d
-            mm = fmaf(mu_i[1], d[1], mm);
-            if (DIM == 3) mm = fmaf(mu_i[2], d[2], mm);
-            float mmj = mu_j[0] * d[0];                         // mu_j . d   (pair (j<-i) uses -d)
-            mmj = fmaf(mu_j[1], d[1], mmj);
-            if (DIM == 3) mmj = fmaf(mu_j[2], d[2], mmj);
-            const float mmp = -mmj;
-            // ---- ordered pair (i <- j)
-            const float VjG = pj.V * G;
-            const float E = -m_j * Psum;
-            const float Phi1 = rho0 * pj.V * s * invR * ir_i;
-            const float Phi = hc.eta * Phi1;
-            const float sbar = lam_i * pi.rho * VjG + mm * hc.eta * rho0 * VjG * invR * ir_i;
-            const float dif = hc.kd * VjG * u;                   // kd V_j (r2/R) G
-            const float r2bar = lam_i * hc.kd * VjG * drho * hc.e2 * invR * invR - mm * Phi * G * invR;
-            const float Gbar = lam_i * pj.V * (pi.rho * s + hc.kd * drho * u) + mm * (E + Phi);
-            // ---- ordered pair (j <- i): d -> -d, w -> -w, s unchanged
-            const float ViG = pi.V * G;
-            const float Ep = -m_i * Psum;
-            const float Phi1p = rho0 * pi.V * s * invR * ir_j;
-            const float Phip = hc.eta * Phi1p;
-            const float sbarp = lam_j * pj.rho * ViG + mmp * hc.eta * rho0 * ViG * invR * ir_j;
-            const float difp = hc.kd * ViG * u;
-            const float r2barp = -lam_j * hc.kd * ViG * drho * hc.e2 * invR * invR - mmp * Phip * G * invR;
-            const float ADp = ViG * (pj.rho * s - hc.kd * drho * u);          // A' + D'
-            const float Gbarp = lam_j * pi.V * (pj.rho * s - hc.kd * drho * u) + mmp * (Ep + Phip);
-            // ---- what lands on particle i
-            const float cs = sbar + sbarp;
-            const float cd = 2.0f * (r2bar + r2barp) + (Gbar + Gbarp) * K;
-            const float ce = (E + Phi) * G, cep = (Ep + Phip) * G;
-#pragma unroll
-            for (int kk = 0; kk < DIM; ++kk) {
-                xb[kk] += cs * w[kk] + cd * d[kk] + ce * mu_i[kk] - cep * mu_j[kk];
-                vb[kk] = fmaf(cs, d[kk], vb[kk]);
-            }
-            rb += lam_i * (VjG * s + dif) - mm * G * Phi * ir_i                 // first role of (i<-j)
-                  - lam_j * (ADp * ir_i + difp) - mmp * G * Phip * ir_i;         // second role of (j<-i)
-            Z = fmaf(G, m_j * mm + m_i * mmp, Z);               // -dL/dP_i
-            // ---- scalar parameters, ordered pair (i<-j) only (each ordered pair is owned by one row)
-            const float D1 = 2.0f * hc.ell * VjG * drho * u;    // D_ij / (delta c0)
-            S_D1 = fmaf(lam_i, D1, S_D1);
-            const float xphi1 = mm * G * Phi1;
-            S_P1 += xphi1;
-            S_PL = fmaf(xphi1, hc.ell, S_PL);
-            S_eps -= (lam_i * hc.kd * VjG * drho * u + mm * G * Phi) * invR * (2.0f * kp.eps * hc.H2);
-        }
-#pragma unroll
-        for (int kk = 0; kk < DIM; ++kk) {
-            xb[kk] = group_sum<GS>(xb[kk]);
-            vb[kk] = group_sum<GS>(vb[kk]);
-        }
-        rb = group_sum<GS>(rb);
-        Z = group_sum<GS>(Z);
-        if (gl == 0 && live) {
-            rb -= ei.x * Z;                                      // rho_bar_i += Pbar_i dP/drho, Pbar_i = -Z_i
-            T_E += pi.P * Z;
-            T_0 += ei.y * Z;
-            T_g += ei.z * Z;
-            G0 += mu_i[0]; G1 += mu_i[1]; G2 += mu_i[2];
-            if (OUT_SORTED) {
-                xb4[row] = make_float4(xb[0], xb[1], xb[2], rb);
-                vb4[row] = make_float4(vb[0], vb[1], vb[2], 0.f);
-            } else {
-                const int64_t i = perm[row];
+    tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
+        [&](uint32_t r, bool live, uint32_t b, uint32_t e_in, const uint16_t *idx) {
+            const uint32_t qi = selfq[r];
+            const Part pi = load_part<DIM>(A, B, C, qi);
+            const float4 ci = Ct[qi];
+            const float lam_i = ci.x, mu_i[3] = {ci.y, ci.z, ci.w};
+            const float m_i = pi.V * pi.rho;
+            const uint32_t e = live ? e_in : b;                    // padding groups run no pairs (partials stay clean)
+            const float ir_i = 1.0f / pi.rho;
+            float xb[3] = {0.f, 0.f, 0.f}, vb[3] = {0.f, 0.f, 0.f}, rb = 0.f, Z = 0.f;
+            for (uint32_t k = b + gl; k < e; k += GS) {
+                const uint32_t j = idx[k];
+                const Part pj = load_part<DIM>(A, B, C, j);
+                const float4 cj = Ct[j];
+                const float lam_j = cj.x, mu_j[3] = {cj.y, cj.z, cj.w};
+                const float d[3] = {pi.x[0] - pj.x[0], pi.x[1] - pj.x[1], DIM == 3 ? pi.x[2] - pj.x[2] : 0.f};
+                const float r2 = fmaf(d[2], d[2], fmaf(d[1], d[1], d[0] * d[0]));
+                HC hc = hu;
+                if (VARH) hc = hc_make<DIM>(fmaxf(pi.h, pj.h), kp);
+                const float rr = fast_sqrt(r2);
+                const float t = fmaxf(fmaf(-hc.invH, rr, 1.0f), 0.f);
+                const float t2 = t * t, t4 = t2 * t2;
+                const float G = hc.cG * fmaf(5.0f * hc.invH, rr, 1.0f) * (t4 * t);
+                const float K = hc.cK * t4;
+                const float w[3] = {pi.v[0] - pj.v[0], pi.v[1] - pj.v[1], DIM == 3 ? pi.v[2] - pj.v[2] : 0.f};
+                float s = w[0] * d[0];
+                s = fmaf(w[1], d[1], s);
+                if (DIM == 3) s = fmaf(w[2], d[2], s);
+                const float invR = fast_rcp(r2 + hc.e2);
+                const float u = r2 * invR;
+                const float ir_j = fast_rcp(pj.rho);
+                const float m_j = pj.V * pj.rho;
+                const float drho = pi.rho - pj.rho;
+                const float Psum = pi.P + pj.P;
+                float mm = mu_i[0] * d[0];                          // mu_i . d
+                mm = fmaf(mu_i[1], d[1], mm);
+                if (DIM == 3) mm = fmaf(mu_i[2], d[2], mm);
+                float mmj = mu_j[0] * d[0];                         // mu_j . d   (pair (j<-i) uses -d)
+                mmj = fmaf(mu_j[1], d[1], mmj);
+                if (DIM == 3) mmj = fmaf(mu_j[2], d[2], mmj);
+                const float mmp = -mmj;
+                // ---- ordered pair (i <- j)
+                const float VjG = pj.V * G;
+                const float E = -m_j * Psum;
+                const float Phi1 = rho0 * pj.V * s * invR * ir_i;
+                const float Phi = hc.eta * Phi1;
+                const float sbar = lam_i * pi.rho * VjG + mm * hc.eta * rho0 * VjG * invR * ir_i;
+                const float dif = hc.kd * VjG * u;                   // kd V_j (r2/R) G
+                const float r2bar = lam_i * hc.kd * VjG * drho * hc.e2 * invR * invR - mm * Phi * G * invR;
+                const float Gbar = lam_i * pj.V * (pi.rho * s + hc.kd * drho * u) + mm * (E + Phi);
+                // ---- ordered pair (j <- i): d -> -d, w -> -w, s unchanged
+                const float ViG = pi.V * G;
+                const float Ep = -m_i * Psum;
+                const float Phi1p = rho0 * pi.V * s * invR * ir_j;
+                const float Phip = hc.eta * Phi1p;
+                const float sbarp = lam_j * pj.rho * ViG + mmp * hc.eta * rho0 * ViG * invR * ir_j;
+                const float difp = hc.kd * ViG * u;
+                const float r2barp = -lam_j * hc.kd * ViG * drho * hc.e2 * invR * invR - mmp * Phip * G * invR;
+                const float ADp = ViG * (pj.rho * s - hc.kd * drho * u);          // A' + D'
+                const float Gbarp = lam_j * pi.V * (pj.rho * s - hc.kd * drho * u) + mmp * (Ep + Phip);
+                // ---- what lands on particle i
+                const float cs = sbar + sbarp;
+                const float cd = 2.0f * (r2bar + r2barp) + (Gbar + Gbarp) * K;
+                const float ce = (E + Phi) * G, cep = (Ep + Phip) * G;
 #pragma unroll
                 for (int kk = 0; kk < DIM; ++kk) {
-                    xb_out[i * DIM + kk] = xb[kk];
-                    vb_out[i * DIM + kk] = vb[kk];
+                    xb[kk] += cs * w[kk] + cd * d[kk] + ce * mu_i[kk] - cep * mu_j[kk];
+                    vb[kk] = fmaf(cs, d[kk], vb[kk]);
                 }
-                rb_out[i] = rb;
+                rb += lam_i * (VjG * s + dif) - mm * G * Phi * ir_i                 // first role of (i<-j)
+                      - lam_j * (ADp * ir_i + difp) - mmp * G * Phip * ir_i;         // second role of (j<-i)
+                Z = fmaf(G, m_j * mm + m_i * mmp, Z);               // -dL/dP_i
+                // ---- scalar parameters, ordered pair (i<-j) only (each ordered pair is owned by one row)
+                const float D1 = 2.0f * hc.ell * VjG * drho * u;    // D_ij / (delta c0)
+                S_D1 = fmaf(lam_i, D1, S_D1);
+                const float xphi1 = mm * G * Phi1;
+                S_P1 += xphi1;
+                S_PL = fmaf(xphi1, hc.ell, S_PL);
+                S_eps -= (lam_i * hc.kd * VjG * drho * u + mm * G * Phi) * invR * (2.0f * kp.eps * hc.H2);
             }
-        }
-    }
+#pragma unroll
+            for (int kk = 0; kk < DIM; ++kk) {
+                xb[kk] = group_sum<GS>(xb[kk]);
+                vb[kk] = group_sum<GS>(vb[kk]);
+            }
+            rb = group_sum<GS>(rb);
+            Z = group_sum<GS>(Z);
+            if (gl == 0 && live) {
+                const uint32_t row = row0 + r;
+                const float4 ei = eos[row];                          // {dP/drho, dP/drho0, dP/dgamma, m}
+                rb -= ei.x * Z;                                      // rho_bar_i += Pbar_i dP/drho, Pbar_i = -Z_i
+                T_E += pi.P * Z;
+                T_0 += ei.y * Z;
+                T_g += ei.z * Z;
+                G0 += mu_i[0]; G1 += mu_i[1]; G2 += mu_i[2];
+                if (OUT_SORTED) {
+                    xb4[row] = make_float4(xb[0], xb[1], xb[2], rb);
+                    vb4[row] = make_float4(vb[0], vb[1], vb[2], 0.f);
+                } else {
+                    const int64_t i = perm[row];
+#pragma unroll
+                    for (int kk = 0; kk < DIM; ++kk) {
+                        xb_out[i * DIM + kk] = xb[kk];
+                        vb_out[i * DIM + kk] = vb[kk];
+                    }
+                    rb_out[i] = rb;
+                }
+            }
+        });
     // B2 stage 1: fixed-order CTA reduction of the ten partial sums
     float vals[10] = {S_D1, S_P1, S_PL, S_eps, T_E, T_0, T_g, G0, G1, G2};
 #pragma unroll
@@ -406,7 +477,7 @@ k_vjp_tile(TileGeom tg, KPar kp, int mcap, const float4 *__restrict__ s0, const 
     if (threadIdx.x < kNPartT) {
         float v = 0.f;
         if (threadIdx.x < 10)
-            for (int w = 0; w < kPtWarps; ++w) v += red[w][threadIdx.x];
+            for (int w = 0; w < nwarps; ++w) v += red[w][threadIdx.x];
         partials[(int64_t)blockIdx.x * kNPartT + threadIdx.x] = v;
     }
 }
@@ -416,12 +487,34 @@ k_vjp_tile(TileGeom tg, KPar kp, int mcap, const float4 *__restrict__ s0, const 
 // ==========================================================================================
 // host side
 // ==========================================================================================
-static int tile_mcap(const sph_ctx *ctx) { return (int)((ctx->tile_Mmax + 7u) & ~7u); }
-static size_t tile_rp_bytes(const sph_ctx *ctx) { return ((size_t)ctx->tile_Tmax + 8) * 4; }
 static int tile_group(const sph_ctx *ctx)
 {
     const int g = ctx->opt_group ? ctx->opt_group : 8;
     return g == 4 ? 8 : g;
+}
+
+// threads per CTA, shared-memory carve-up and size for a pair kernel with `state_bytes` per halo particle
+static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, int *threads, TileSizes *ts, size_t *smem)
+{
+    ts->mcap = (int)((ctx->tile_Mmax + 7u) & ~7u);
+    ts->tcap = (int)((ctx->tile_Tmax + 7u) & ~7u);
+    const double mean = ctx->n > 0 ? (double)ctx->nnz / (double)ctx->n : 1.0;
+    int rb = (int)((32 / gs) * mean * 1.5) + 24;
+    rb = (rb + 7) & ~7;
+    if (rb < 64) rb = 64;
+    ts->rb = rb;
+    const size_t fixed = (size_t)ts->mcap * state_bytes + (size_t)(ts->tcap + 4) * 4 + (size_t)ts->tcap * 2 + 16;
+    const size_t sm_total = 233472, per_cta = 2560, cta_max = 232448 - 2048;
+    auto need = [&](int warps) { return fixed + (size_t)warps * 2 * rb * 2; };
+    int warps = 8;
+    if (ctx->opt_warps) warps = ctx->opt_warps;
+    else if (sm_total / (need(8) + per_cta) < 2) warps = 16;      // one CTA per SM: make it a big one
+    while (warps > 1 && need(warps) > cta_max) warps >>= 1;
+    if (need(warps) > cta_max) {                                   // last resort: a minimal ring (rows fall back to global reads)
+        ts->rb = 8;
+    }
+    *threads = warps * 32;
+    *smem = fixed + (size_t)warps * 2 * ts->rb * 2;
 }
 
 #define SPH_TILE_SMEM_ATTR(KERNEL, SMEM) \
@@ -430,13 +523,16 @@ static int tile_group(const sph_ctx *ctx)
 int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, float *rho_out, cudaStream_t st)
 {
     const TileGeom &tg = ctx->tg;
-    const int mcap = tile_mcap(ctx);
-    const size_t smem = (size_t)mcap * 20 + tile_rp_bytes(ctx);
+    const int gs = tile_group(ctx);
+    int threads;
+    TileSizes ts;
+    size_t smem;
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, &threads, &ts, &smem);   // same carve-up as the RHS kernel (SmemMap)
 #define SPH_DT_LAUNCH(DIM, GS, VARH)                                                                                  \
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_density_tile<DIM, GS, VARH>), smem);                                                    \
-        k_density_tile<DIM, GS, VARH><<<(unsigned)tg.ntiles, kPtBlock, smem, st>>>(                                   \
-            tg, kp, mcap, ctx->pos_s.as<float4>(), m_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), \
+        k_density_tile<DIM, GS, VARH><<<(unsigned)tg.ntiles, threads, smem, st>>>(                                    \
+            tg, kp, ts, ctx->pos_s.as<float4>(), m_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),   \
             ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), rho_out);              \
     } while (0)
 #define SPH_DT_GS(GS)                                                                                     \
@@ -444,7 +540,7 @@ int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, floa
         if (kp.dim == 3) { if (kp.uniform_h) SPH_DT_LAUNCH(3, GS, false); else SPH_DT_LAUNCH(3, GS, true); } \
         else { if (kp.uniform_h) SPH_DT_LAUNCH(2, GS, false); else SPH_DT_LAUNCH(2, GS, true); }             \
     } while (0)
-    switch (tile_group(ctx)) {
+    switch (gs) {
     case 16: SPH_DT_GS(16); break;
     case 32: SPH_DT_GS(32); break;
     default: SPH_DT_GS(8); break;
@@ -459,14 +555,17 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
                         const uint8_t *kind_s, float *drho, float *acc, float4 *out4, cudaStream_t st)
 {
     const TileGeom &tg = ctx->tg;
-    const int mcap = tile_mcap(ctx);
-    const size_t smem = (size_t)mcap * (kp.dim == 3 ? 40 : 32) + tile_rp_bytes(ctx);
+    const int gs = tile_group(ctx);
+    int threads;
+    TileSizes ts;
+    size_t smem;
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, &threads, &ts, &smem);
     const bool sorted = out4 != nullptr;
 #define SPH_RT_LAUNCH(DIM, GS, VARH, SORTED)                                                                         \
     do {                                                                                                             \
         SPH_TILE_SMEM_ATTR((k_rhs_tile<DIM, GS, VARH, SORTED>), smem);                                               \
-        k_rhs_tile<DIM, GS, VARH, SORTED><<<(unsigned)tg.ntiles, kPtBlock, smem, st>>>(                              \
-            tg, kp, mcap, s0, s1, s2, kind_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),          \
+        k_rhs_tile<DIM, GS, VARH, SORTED><<<(unsigned)tg.ntiles, threads, smem, st>>>(                               \
+            tg, kp, ts, s0, s1, s2, kind_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),            \
             ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), drho, acc, out4);     \
     } while (0)
 #define SPH_RT_GS(GS)                                                                                                   \
@@ -479,7 +578,7 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
             else { if (sorted) SPH_RT_LAUNCH(2, GS, true, true); else SPH_RT_LAUNCH(2, GS, true, false); }                \
         }                                                                                                               \
     } while (0)
-    switch (tile_group(ctx)) {
+    switch (gs) {
     case 16: SPH_RT_GS(16); break;
     case 32: SPH_RT_GS(32); break;
     default: SPH_RT_GS(8); break;
@@ -490,20 +589,22 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
     return SPH_OK;
 }
 
-// returns the number of partials records (= CTAs) through *nrec
 int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
                         const float4 *cot, const float4 *eos, float *xb, float *vb, float *rb, float4 *xb4, float4 *vb4,
                         float *partials, cudaStream_t st)
 {
     const TileGeom &tg = ctx->tg;
-    const int mcap = tile_mcap(ctx);
-    const size_t smem = (size_t)mcap * (kp.dim == 3 ? 56 : 48) + tile_rp_bytes(ctx);
+    const int gs = tile_group(ctx);
+    int threads;
+    TileSizes ts;
+    size_t smem;
+    tile_launch_cfg(ctx, kp.dim == 3 ? 56 : 48, gs, &threads, &ts, &smem);
     const bool sorted = xb4 != nullptr;
 #define SPH_VT_LAUNCH(DIM, GS, VARH, SORTED)                                                                          \
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_vjp_tile<DIM, GS, VARH, SORTED>), smem);                                                \
-        k_vjp_tile<DIM, GS, VARH, SORTED><<<(unsigned)tg.ntiles, kPtBlock, smem, st>>>(                               \
-            tg, kp, mcap, s0, s1, s2, cot, eos, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),         \
+        k_vjp_tile<DIM, GS, VARH, SORTED><<<(unsigned)tg.ntiles, threads, smem, st>>>(                                \
+            tg, kp, ts, s0, s1, s2, cot, eos, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),           \
             ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), xb, vb, rb, xb4, vb4,  \
             partials);                                                                                                \
     } while (0)
@@ -517,7 +618,7 @@ int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
             else { if (sorted) SPH_VT_LAUNCH(2, GS, true, true); else SPH_VT_LAUNCH(2, GS, true, false); }                \
         }                                                                                                               \
     } while (0)
-    switch (tile_group(ctx)) {
+    switch (gs) {
     case 16: SPH_VT_GS(16); break;
     case 32: SPH_VT_GS(32); break;
     default: SPH_VT_GS(8); break;
