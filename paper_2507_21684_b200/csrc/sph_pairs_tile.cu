@@ -26,38 +26,67 @@ __device__ __forceinline__ float group_sum(float v)
     return v;
 }
 
-// stage one float4 array of the halo; SHIFT: add the periodic shift to .x/.y(/.z)
-template <int DIM, bool SHIFT>
-__device__ __forceinline__ void stage4(const TileGeom &tg, const TileTab &tt, const float4 *__restrict__ src,
-                                       float4 *__restrict__ dst)
+// ------------------------------------------------------------------------------------------ staging
+__device__ __forceinline__ void cp_async16(uint32_t smem_addr, const void *gptr)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void cp_async8(uint32_t smem_addr, const void *gptr)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void cp_async4(uint32_t smem_addr, const void *gptr)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// Copies the halo of the tile (every halo cell is one contiguous run of the sorted arrays) into shared memory with
+// cp.async: no registers, every copy of the CTA in flight at once.  Null sources are skipped (compile time).
+__device__ __forceinline__ void stage_halo(const TileTab &tt, const float4 *__restrict__ g0, float4 *d0,
+                                           const float4 *__restrict__ g1, float4 *d1, const float4 *__restrict__ g2,
+                                           float4 *d2, const float2 *__restrict__ gc, float2 *dc,
+                                           const float *__restrict__ gf, float *df)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const uint32_t a0 = smem_u32(d0), a1 = smem_u32(d1), a2 = smem_u32(d2), ac = smem_u32(dc), af = smem_u32(df);
     for (int hc = warp; hc < tt.nh; hc += nwarps) {
-        const uint32_t o0 = tt.h_off[hc], o1 = tt.h_off[hc + 1];
-        if (o1 == o0) continue;
-        float sh[3] = {0.f, 0.f, 0.f};
-        if (SHIFT) tile_cell_shift<DIM>(tg, tt, hc, sh);
-        const float4 *s = src + tt.h_start[hc];
-        for (uint32_t q = lane; q < o1 - o0; q += 32) {
-            float4 v = s[q];
-            if (SHIFT) {
-                v.x += sh[0];
-                v.y += sh[1];
-                if (DIM == 3) v.z += sh[2];
-            }
-            dst[o0 + q] = v;
+        const uint32_t o0 = tt.h_off[hc], cnt = tt.h_off[hc + 1] - o0, gs = tt.h_start[hc];
+        for (uint32_t l = lane; l < cnt; l += 32) {
+            const uint32_t q = o0 + l;
+            const size_t g = (size_t)gs + l;
+            if (g0) cp_async16(a0 + q * 16, g0 + g);
+            if (g1) cp_async16(a1 + q * 16, g1 + g);
+            if (g2) cp_async16(a2 + q * 16, g2 + g);
+            if (gc) cp_async8(ac + q * 8, gc + g);
+            if (gf) cp_async4(af + q * 4, gf + g);
         }
     }
+    cp_async_commit();
 }
-template <class T>
-__device__ __forceinline__ void stage_plain(const TileTab &tt, const T *__restrict__ src, T *__restrict__ dst)
+// after the copies have landed (wait + __syncthreads): add the periodic shift to the positions of the halo cells
+// that lie across a face.  Contains a __syncthreads on seam tiles (uniform per CTA).
+template <int DIM>
+__device__ __forceinline__ void stage_shift(const TileTab &tt, float4 *d0)
 {
+    if (!tt.seam) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     for (int hc = warp; hc < tt.nh; hc += nwarps) {
-        const uint32_t o0 = tt.h_off[hc], o1 = tt.h_off[hc + 1];
-        const T *s = src + tt.h_start[hc];
-        for (uint32_t q = lane; q < o1 - o0; q += 32) dst[o0 + q] = s[q];
+        const float sx = tt.h_shift[0][hc], sy = tt.h_shift[1][hc], sz = DIM == 3 ? tt.h_shift[2][hc] : 0.f;
+        if (sx == 0.f && sy == 0.f && sz == 0.f) continue;
+        const uint32_t o0 = tt.h_off[hc], cnt = tt.h_off[hc + 1] - o0;
+        for (uint32_t l = lane; l < cnt; l += 32) {
+            float4 v = d0[o0 + l];
+            v.x += sx;
+            v.y += sy;
+            if (DIM == 3) v.z += sz;
+            d0[o0 + l] = v;
+        }
     }
+    __syncthreads();
 }
 // tile-relative row offsets rp[r] = row_ptr[row0 + r] - row_ptr[row0], r = 0..T, and the halo index of every row
 __device__ __forceinline__ void stage_rows(const TileTab &tt, const long long *__restrict__ row_ptr, uint32_t *rp,
@@ -75,14 +104,6 @@ __device__ __forceinline__ void stage_rows(const TileTab &tt, const long long *_
 }
 
 // ------------------------------------------------------------------------------------------ index ring
-__device__ __forceinline__ void cp_async16(uint32_t smem_addr, const void *gptr)
-{
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr), "l"(gptr) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
 // Drives the rows of a tile through `body(r, live, b, e, idx)`: row r of the tile (clamped to T-1; `live` false for
 // the padding groups of the last pass), its tile-relative entry range [b,e), and a pointer such that idx[k] is the
 // halo index of entry k.  A warp works on RPW = 32/GS consecutive rows per pass; the contiguous index segment of
@@ -194,10 +215,11 @@ k_density_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ po
     __shared__ TileTab tt;
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
     if (tt.T == 0) return;
-    stage4<DIM, true>(tg, tt, pos_s, sm.A);
-    stage_plain<float>(tt, m_s, Ms);
+    stage_halo(tt, pos_s, sm.A, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, m_s, Ms);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
+    cp_async_wait<0>();
     __syncthreads();
+    stage_shift<DIM>(tt, sm.A);
     const int gl = (threadIdx.x & 31) % GS;
     const HC hu = hc_uniform<DIM>(kp);
     const float4 *A = sm.A;
@@ -241,11 +263,11 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
     __shared__ TileTab tt;
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
     if (tt.T == 0) return;
-    stage4<DIM, true>(tg, tt, s0, sm.A);
-    stage_plain<float4>(tt, s1, sm.B);
-    if (DIM == 3) stage_plain<float2>(tt, s2, sm.C);
+    stage_halo(tt, s0, sm.A, s1, sm.B, nullptr, nullptr, DIM == 3 ? s2 : nullptr, sm.C, nullptr, nullptr);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
+    cp_async_wait<0>();
     __syncthreads();
+    stage_shift<DIM>(tt, sm.A);
     const int gl = (threadIdx.x & 31) % GS;
     const HC hu = hc_uniform<DIM>(kp);
     const float rho0 = kp.rho0;
@@ -340,12 +362,11 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
         if (threadIdx.x < kNPartT) partials[(int64_t)blockIdx.x * kNPartT + threadIdx.x] = 0.f;
         return;
     }
-    stage4<DIM, true>(tg, tt, s0, sm.A);
-    stage_plain<float4>(tt, s1, sm.B);
-    if (DIM == 3) stage_plain<float2>(tt, s2, sm.C);
-    stage_plain<float4>(tt, cot, sm.cot);
+    stage_halo(tt, s0, sm.A, s1, sm.B, cot, sm.cot, DIM == 3 ? s2 : nullptr, sm.C, nullptr, nullptr);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
+    cp_async_wait<0>();
     __syncthreads();
+    stage_shift<DIM>(tt, sm.A);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gl = lane % GS;
     const HC hu = hc_uniform<DIM>(kp);
     const float rho0 = kp.rho0;
@@ -487,9 +508,10 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
 // ==========================================================================================
 // host side
 // ==========================================================================================
-static int tile_group(const sph_ctx *ctx)
+// lanes per row: measured on C3 (profiles/r01_c): RHS/density 16, VJP 8 (its row epilogue is heavier); 2D rows are short
+static int tile_group(const sph_ctx *ctx, bool vjp)
 {
-    const int g = ctx->opt_group ? ctx->opt_group : 8;
+    const int g = ctx->opt_group ? ctx->opt_group : (ctx->geom.dim == 3 && !vjp ? 16 : 8);
     return g == 4 ? 8 : g;
 }
 
@@ -506,9 +528,9 @@ static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, int *th
     const size_t fixed = (size_t)ts->mcap * state_bytes + (size_t)(ts->tcap + 4) * 4 + (size_t)ts->tcap * 2 + 16;
     const size_t sm_total = 233472, per_cta = 2560, cta_max = 232448 - 2048;
     auto need = [&](int warps) { return fixed + (size_t)warps * 2 * rb * 2; };
-    int warps = 8;
+    int warps = 16;                                                // measured: 16 warps beat 8 at one and at two CTAs per SM
     if (ctx->opt_warps) warps = ctx->opt_warps;
-    else if (sm_total / (need(8) + per_cta) < 2) warps = 16;      // one CTA per SM: make it a big one
+    (void)sm_total; (void)per_cta;
     while (warps > 1 && need(warps) > cta_max) warps >>= 1;
     if (need(warps) > cta_max) {                                   // last resort: a minimal ring (rows fall back to global reads)
         ts->rb = 8;
@@ -523,7 +545,7 @@ static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, int *th
 int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, float *rho_out, cudaStream_t st)
 {
     const TileGeom &tg = ctx->tg;
-    const int gs = tile_group(ctx);
+    const int gs = tile_group(ctx, false);
     int threads;
     TileSizes ts;
     size_t smem;
@@ -555,7 +577,7 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
                         const uint8_t *kind_s, float *drho, float *acc, float4 *out4, cudaStream_t st)
 {
     const TileGeom &tg = ctx->tg;
-    const int gs = tile_group(ctx);
+    const int gs = tile_group(ctx, false);
     int threads;
     TileSizes ts;
     size_t smem;
@@ -594,7 +616,7 @@ int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
                         float *partials, cudaStream_t st)
 {
     const TileGeom &tg = ctx->tg;
-    const int gs = tile_group(ctx);
+    const int gs = tile_group(ctx, true);
     int threads;
     TileSizes ts;
     size_t smem;

@@ -25,7 +25,9 @@ struct TileTab {                       // one per CTA, in shared memory
     int t_cell[kTileMaxTgt];           // halo slot of each target cell
     int ext[3], hs[3], tlo[3], tn[3];  // halo extent, first (unwrapped) halo cell coordinate, slot of the first target, targets
     int nh, nt;
+    int seam;                          // some halo cell lies across a periodic face (h_shift != 0)
     uint32_t row0, T, M;               // first sorted row of the tile, rows, halo particles
+    float h_shift[3][kTileMaxHalo];    // shift (0, -L or +L per axis) that moves a halo cell next to the tile
 };
 
 // Computes the tables of tile `tile`.  Must be called by every thread of the CTA (contains __syncthreads); needs
@@ -63,6 +65,11 @@ __device__ __forceinline__ void tile_setup(const TileGeom &tg, int tile, const u
         }
         tt.nh = nh;
         tt.nt = nt;
+        int seam = 0;
+#pragma unroll
+        for (int k = 0; k < DIM; ++k)
+            if (tg.periodic[k] && (tt.hs[k] < 0 || tt.hs[k] + tt.ext[k] > tg.ncell[k])) seam = 1;
+        tt.seam = seam;
     }
     __syncthreads();
     const int nh = tt.nh, nt = tt.nt;
@@ -85,6 +92,15 @@ __device__ __forceinline__ void tile_setup(const TileGeom &tg, int tile, const u
                 s2[u] = cell_start[lin];
                 c2[u] = cell_end[lin] - s2[u];
                 tt.h_start[hc] = s2[u];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    float sh = 0.f;
+                    if (k < DIM && tg.periodic[k]) {
+                        const int c = tt.hs[k] + sl[k];
+                        sh = c < 0 ? -tg.L[k] : (c >= tg.ncell[k] ? tg.L[k] : 0.f);
+                    }
+                    tt.h_shift[k][hc] = sh;
+                }
             }
         }
         uint32_t tot = c2[0] + c2[1], inc = tot;
@@ -133,14 +149,9 @@ __device__ __forceinline__ void tile_setup(const TileGeom &tg, int tile, const u
 template <int DIM>
 __device__ __forceinline__ void tile_cell_shift(const TileGeom &tg, const TileTab &tt, int hc, float sh[3])
 {
-    const int sl[3] = {hc % tt.ext[0], (hc / tt.ext[0]) % tt.ext[1], hc / (tt.ext[0] * tt.ext[1])};
-    sh[0] = sh[1] = sh[2] = 0.f;
-#pragma unroll
-    for (int k = 0; k < DIM; ++k)
-        if (tg.periodic[k]) {
-            const int c = tt.hs[k] + sl[k];
-            sh[k] = c < 0 ? -tg.L[k] : (c >= tg.ncell[k] ? tg.L[k] : 0.f);
-        }
+    sh[0] = tt.h_shift[0][hc];
+    sh[1] = tt.h_shift[1][hc];
+    sh[2] = DIM == 3 ? tt.h_shift[2][hc] : 0.f;
 }
 
 // sorted index of the particle with halo-linear index q (binary search over the <= 64 halo cells)
