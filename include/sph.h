@@ -185,7 +185,9 @@ enum {
                                2 = tile-local (16-bit indices into the halo of a block of cells, neighbour state staged
                                in shared memory).  2 falls back to 1 when a halo does not fit shared memory. */
     SPH_OPT_TILE_EDGE = 3,  /* edge of the cell blocks of the tile-local layout: 1, 2, 4 cells; 0 = automatic */
-    SPH_OPT_PAIR_WARPS = 4  /* warps per CTA of the tile pair kernels: 4, 8, 16; 0 = automatic */
+    SPH_OPT_PAIR_WARPS = 4, /* warps per CTA of the tile pair kernels: 4, 8, 16; 0 = automatic */
+    SPH_OPT_FILL_MASKS = 5  /* 1 (default): the fill of the tile-local lists expands the hit masks saved by the count pass;
+                               0: it repeats the distance tests (no mask buffer) */
 };
 int sph_set_option(sph_ctx *ctx, int key, int value);
 int sph_profile_enable(sph_ctx *ctx, int on);

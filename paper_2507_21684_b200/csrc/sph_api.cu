@@ -33,7 +33,7 @@ extern "C" int sph_destroy(sph_ctx *ctx)
     cudaDeviceSynchronize();
     DevBuf *bufs[] = {&ctx->key_a, &ctx->key_b, &ctx->idx_a, &ctx->idx_b, &ctx->hist, &ctx->perm, &ctx->inv_perm,
                       &ctx->key_sorted, &ctx->pos_s, &ctx->cell_start, &ctx->cell_end, &ctx->stats, &ctx->cnt,
-                      &ctx->row_ptr, &ctx->col, &ctx->col16, &ctx->scan_tmp, &ctx->s0, &ctx->s1, &ctx->s2, &ctx->s3, &ctx->c0buf,
+                      &ctx->row_ptr, &ctx->col, &ctx->col16, &ctx->scan_tmp, &ctx->maskbuf, &ctx->tile_words, &ctx->tile_mask_base, &ctx->s0, &ctx->s1, &ctx->s2, &ctx->s3, &ctx->c0buf,
                       &ctx->out4, &ctx->m_s, &ctx->kind_s, &ctx->partials, &ctx->eos, &ctx->hx, &ctx->hv, &ctx->hrho,
                       &ctx->hm, &ctx->hh, &ctx->hkind, &ctx->hlam, &ctx->hmu, &ctx->ho_drho, &ctx->ho_acc, &ctx->ho_xb,
                       &ctx->ho_vb, &ctx->ho_rb, &ctx->ho_pb, &ctx->ho_dens};
@@ -239,6 +239,9 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
     case SPH_OPT_PAIR_WARPS:
         if (value != 0 && value != 4 && value != 8 && value != 16) return SPH_E_INVALID;
         ctx->opt_warps = value;
+        return SPH_OK;
+    case SPH_OPT_FILL_MASKS:
+        ctx->opt_fill_masks = value != 0;
         return SPH_OK;
     case SPH_OPT_TILE_EDGE:
         if (value != 0 && value != 1 && value != 2 && value != 4) return SPH_E_INVALID;

@@ -124,6 +124,7 @@ struct sph_ctx {
     int opt_group = 0;          // lanes per row in the pair kernels (0 = default)
     int opt_warps = 0;          // warps per CTA of the tile pair kernels (0 = automatic: 8, or 16 when one CTA fits an SM)
     int opt_list_mode = 0;      // 0 auto, 1 force the generic (global-id) lists, 2 force tile-local lists
+    int opt_fill_masks = 1;     // the fill expands the hit masks saved by the count pass (0: repeats the tests)
     int opt_tile_edge = 0;      // 0 auto, else force the tile edge B (1, 2, 4)
     bool tile_mode = false;     // lists of the last sph_neighbors are tile-local (col16)
     TileGeom tg{};
@@ -148,6 +149,7 @@ struct sph_ctx {
     DevBuf stats;               // device: [0] err flag, [1] hmax bits, [2] hmin bits
     // lists
     DevBuf cnt, row_ptr, col, col16, scan_tmp;
+    DevBuf maskbuf, tile_words, tile_mask_base;   // hit masks of the count pass, per-tile mask offsets
     bool col_valid = false;     // ctx->col holds the global-id lists of the current build
     // pair scratch (sorted SoA)
     DevBuf s0, s1, s2, s3, c0buf, out4, m_s, kind_s, partials, eos;

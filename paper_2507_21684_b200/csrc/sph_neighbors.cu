@@ -291,11 +291,11 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
     if (ctx->opt_list_mode != 1) ncand = sph_tile_candidates(ctx, cand);
     if (ncand) SPH_TRY(sph_tile_stats_launch(ctx, cand, ncand, st));
     // the statistics of sph_build_cells (error flag, max/min h) are needed on the host to size the search
-    uint32_t hs[10];
+    uint32_t hs[11];
     uint32_t *hpin = reinterpret_cast<uint32_t *>(ctx->h_pinned + 8);
-    SPH_CUDA_TRY(cudaMemcpyAsync(hpin, ctx->stats.p, 40, cudaMemcpyDeviceToHost, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(hpin, ctx->stats.p, 44, cudaMemcpyDeviceToHost, st));
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
-    memcpy(hs, hpin, 40);
+    memcpy(hs, hpin, 44);
     if (hs[0] != 0u) return SPH_E_DOMAIN;
     float hmax, hmin;
     memcpy(&hmax, &hs[1], 4);
@@ -320,7 +320,7 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
     for (int k = 0; k < ncand; ++k) {
         const uint32_t Mmax = hs[4 + 2 * k], Tmax = hs[5 + 2 * k];
         if (!sph_tile_fits(gg.dim, Mmax)) continue;
-        SPH_TRY(sph_neighbors_tile_run(ctx, sp, cand[k], Mmax, Tmax, st, nnz_out));
+        SPH_TRY(sph_neighbors_tile_run(ctx, sp, cand[k], Mmax, Tmax, hs[10], st, nnz_out));
         ctx->search_scale = search_scale;
         ctx->lists_ready = true;
         return SPH_OK;

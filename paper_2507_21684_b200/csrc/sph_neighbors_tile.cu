@@ -20,6 +20,7 @@
 namespace {
 
 constexpr int kNbWarps = 8;
+constexpr uint32_t kWqCap = 96;    // mask words per row handled by the fast expansion
 
 struct RowCtx {
     float4 pi;         // own position (+h)
@@ -93,10 +94,31 @@ __device__ __forceinline__ uint32_t nb_mask(const RowCtx &rc, const float4 *__re
 }
 
 // `dst`: FILL only -- where this lane's hits go (shared-memory image or global col16), indexed by rc.n
+// mask words per row of the cell at halo slot sl: one per 32 candidates of each of its 3^(d-1) x-runs
+template <int DIM>
+__device__ __forceinline__ uint32_t cell_words(const TileTab &tt, const int sl[3])
+{
+    uint32_t w = 0;
+    const int zlo = DIM == 3 ? -1 : 0, zhi = DIM == 3 ? 1 : 0;
+    for (int dz = zlo; dz <= zhi; ++dz) {
+        const int sz = sl[2] + dz;
+        if (DIM == 3 && (sz < 0 || sz >= tt.ext[2])) continue;
+        for (int dy = -1; dy <= 1; ++dy) {
+            const int sy = sl[1] + dy;
+            if (sy < 0 || sy >= tt.ext[1]) continue;
+            const int rowbase = tt.ext[0] * (sy + tt.ext[1] * sz);
+            const int xa = max(sl[0] - 1, 0), xb = min(sl[0] + 1, tt.ext[0] - 1);
+            w += (tt.h_off[rowbase + xb + 1] - tt.h_off[rowbase + xa] + 31u) >> 5;
+        }
+    }
+    return w;
+}
+
+// `maskp` (count pass, may be null): this lane's column of the item's mask block; word w of the row at maskp[32 w]
 template <int DIM, bool FILL, bool VARH, class DstT>
 __device__ __forceinline__ void nb_rows(RowCtx &rc, const float4 *__restrict__ cand, const int sl[3], const SearchPar &sp,
                                         bool seam, const TileTab &tt, const float4 *__restrict__ pos_s,
-                                        const GridGeom &gg, DstT dst)
+                                        const GridGeom &gg, DstT dst, uint32_t *__restrict__ maskp = nullptr)
 {
     const int zlo = DIM == 3 ? -1 : 0, zhi = DIM == 3 ? 1 : 0;
     for (int dz = zlo; dz <= zhi; ++dz) {
@@ -121,6 +143,10 @@ __device__ __forceinline__ void nb_rows(RowCtx &rc, const float4 *__restrict__ c
                     }
                 } else {
                     rc.n += __popc(m);
+                    if (maskp) {
+                        *maskp = m;
+                        maskp += 32;
+                    }
                 }
             }
         }
@@ -131,7 +157,8 @@ template <int DIM, bool FILL, bool VARH>
 __global__ void __launch_bounds__(kNbWarps * 32)
 k_nb_tile(TileGeom tg, GridGeom gg, SearchPar sp, int mcap, int wcap, const float4 *__restrict__ pos_s,
           const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end, uint32_t *__restrict__ cnt,
-          const long long *__restrict__ row_ptr, uint16_t *__restrict__ col16)
+          const long long *__restrict__ row_ptr, uint16_t *__restrict__ col16, uint32_t *__restrict__ maskbuf,
+          const long long *__restrict__ tile_mask_base)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4 *cand = reinterpret_cast<float4 *>(smem_raw);
@@ -164,12 +191,14 @@ k_nb_tile(TileGeom tg, GridGeom gg, SearchPar sp, int mcap, int wcap, const floa
     uint16_t *wbuf = reinterpret_cast<uint16_t *>(smem_raw + (size_t)mcap * sizeof(float4)) + (size_t)warp * wcap;
     // ---- work items: (target cell, chunk of 32 rows), dealt round-robin to the warps
     int item = 0;
+    long long mask_off = maskbuf ? tile_mask_base[blockIdx.x] : 0;   // start of the next item's mask block
     for (int tc = 0; tc < tt.nt; ++tc) {
         const uint32_t nrow = tt.t_off[tc + 1] - tt.t_off[tc];
         const int hc_i = tt.t_cell[tc];
-        for (uint32_t c0 = 0; c0 < nrow; c0 += 32, ++item) {
+        const int sl[3] = {hc_i % tt.ext[0], (hc_i / tt.ext[0]) % tt.ext[1], hc_i / (tt.ext[0] * tt.ext[1])};
+        const uint32_t item_words = (!FILL && maskbuf && nrow) ? 32u * cell_words<DIM>(tt, sl) : 0u;
+        for (uint32_t c0 = 0; c0 < nrow; c0 += 32, ++item, mask_off += item_words) {
             if (item % kNbWarps != warp) continue;
-            const int sl[3] = {hc_i % tt.ext[0], (hc_i / tt.ext[0]) % tt.ext[1], hc_i / (tt.ext[0] * tt.ext[1])};
             const uint32_t nact = min(32u, nrow - c0);
             const bool active = (uint32_t)lane < nact;
             const uint32_t local = c0 + (active ? lane : 0);
@@ -180,7 +209,8 @@ k_nb_tile(TileGeom tg, GridGeom gg, SearchPar sp, int mcap, int wcap, const floa
             rc.tol = sp.band * (seam ? fmaf(sp.Hs_u, sp.Lmax, rc.Hs2) : rc.Hs2);
             rc.n = 0;
             if (!FILL) {
-                nb_rows<DIM, false, VARH>(rc, cand, sl, sp, seam, tt, pos_s, gg, (uint16_t *)nullptr);
+                nb_rows<DIM, false, VARH>(rc, cand, sl, sp, seam, tt, pos_s, gg, (uint16_t *)nullptr,
+                                          maskbuf ? maskbuf + mask_off + lane : nullptr);
                 if (active) cnt[row] = rc.n;
             } else {
                 const uint32_t row_first = tt.h_start[hc_i] + c0;
@@ -202,14 +232,158 @@ k_nb_tile(TileGeom tg, GridGeom gg, SearchPar sp, int mcap, int wcap, const floa
     }
 }
 
+// ---------------------------------------------------------------------------------------- masks -> lists
+// mask words of every tile (same item enumeration as k_nb_tile): words[tile] = sum over items of 32 * cell_words
+template <int DIM>
+__global__ void __launch_bounds__(64)
+k_tile_words(TileGeom tg, const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
+             uint32_t *__restrict__ words)
+{
+    __shared__ TileTab tt;
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (threadIdx.x >= 32) return;
+    uint32_t w = 0;
+    const int tc = threadIdx.x;
+    if (tc < tt.nt) {
+        const uint32_t nrow = tt.t_off[tc + 1] - tt.t_off[tc];
+        const int hc_i = tt.t_cell[tc];
+        const int sl[3] = {hc_i % tt.ext[0], (hc_i / tt.ext[0]) % tt.ext[1], hc_i / (tt.ext[0] * tt.ext[1])};
+        if (nrow) w = ((nrow + 31u) >> 5) * 32u * cell_words<DIM>(tt, sl);
+    }
+    w = __reduce_add_sync(0xffffffffu, w);
+    if (threadIdx.x == 0) words[blockIdx.x] = w;
+}
+
+// N7 from the hit masks of the count pass: no distance test is repeated.  Same work items as k_nb_tile (32 rows of one
+// cell per warp, one row per lane); every lane expands its own mask words in candidate order into the warp's
+// shared-memory image of its contiguous col16 segment, which is flushed coalesced.
+template <int DIM>
+__global__ void __launch_bounds__(kNbWarps * 32)
+k_nb_expand(TileGeom tg, int wcap, int wbcap, const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
+            const long long *__restrict__ row_ptr, uint16_t *__restrict__ col16, const uint32_t *__restrict__ maskbuf,
+            const long long *__restrict__ tile_mask_base)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ TileTab tt;
+    __shared__ uint16_t wqtab[kNbWarps][kWqCap];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (tt.T == 0) return;
+    const int nwarps = blockDim.x >> 5;
+    // per warp: image of its col16 segment (wcap entries) and the mask block of its item (wbcap words x 32 lanes)
+    uint16_t *wbuf = reinterpret_cast<uint16_t *>(smem_raw) + (size_t)warp * wcap;
+    uint32_t *mblk = reinterpret_cast<uint32_t *>(smem_raw + (size_t)nwarps * wcap * 2) + (size_t)warp * wbcap * 32;
+    int item = 0;
+    long long mask_off = tile_mask_base[blockIdx.x];
+    for (int tc = 0; tc < tt.nt; ++tc) {
+        const uint32_t nrow = tt.t_off[tc + 1] - tt.t_off[tc];
+        const int hc_i = tt.t_cell[tc];
+        const int sl[3] = {hc_i % tt.ext[0], (hc_i / tt.ext[0]) % tt.ext[1], hc_i / (tt.ext[0] * tt.ext[1])};
+        const uint32_t item_words = nrow ? 32u * cell_words<DIM>(tt, sl) : 0u;
+        for (uint32_t c0 = 0; c0 < nrow; c0 += 32, ++item, mask_off += item_words) {
+            if (item % nwarps != warp) continue;
+            const uint32_t nact = min(32u, nrow - c0);
+            const bool active = (uint32_t)lane < nact;
+            const uint32_t row_first = tt.h_start[hc_i] + c0;
+            const uint32_t row = row_first + (active ? lane : 0);
+            const long long seg0 = row_ptr[row_first], seg1 = row_ptr[row_first + nact];
+            const long long mine = row_ptr[row];
+            const uint32_t total = (uint32_t)(seg1 - seg0);
+            const bool staged = total <= (uint32_t)wcap;
+            // inactive lanes duplicate lane 0: same masks, same values to the same places
+            const uint32_t *mp = maskbuf + mask_off + (active ? lane : 0);
+            uint16_t *dst_s = wbuf + (uint32_t)(mine - seg0);
+            uint16_t *dst_g = col16 + mine;
+            // candidate of bit 0 of every mask word of this cell's rows
+            uint16_t *wq = wqtab[warp];
+            uint32_t W = 0;
+            {
+                const int zlo = DIM == 3 ? -1 : 0, zhi = DIM == 3 ? 1 : 0;
+                for (int dz = zlo; dz <= zhi; ++dz) {
+                    const int sz = sl[2] + dz;
+                    if (DIM == 3 && (sz < 0 || sz >= tt.ext[2])) continue;
+                    for (int dy = -1; dy <= 1; ++dy) {
+                        const int sy = sl[1] + dy;
+                        if (sy < 0 || sy >= tt.ext[1]) continue;
+                        const int rowbase = tt.ext[0] * (sy + tt.ext[1] * sz);
+                        const int xa = max(sl[0] - 1, 0), xb = min(sl[0] + 1, tt.ext[0] - 1);
+                        const uint32_t q0 = tt.h_off[rowbase + xa], q1 = tt.h_off[rowbase + xb + 1];
+                        const uint32_t nb = (q1 - q0 + 31u) >> 5;
+                        for (uint32_t bb = lane; bb < nb; bb += 32)
+                            if (W + bb < kWqCap) wq[W + bb] = (uint16_t)(min(q0 + 32u * bb + 32u, q1) - 1u);
+                        W += nb;
+                    }
+                }
+            }
+            uint32_t n = 0;
+            if (W <= kWqCap && W <= (uint32_t)wbcap) {
+                // the item's mask block into shared memory (coalesced), then every lane walks its own column at its
+                // own pace (no per-word reconvergence): ~hits + words iterations instead of sum over words of the
+                // largest popcount of the warp
+                {
+                    const uint32_t *src = maskbuf + mask_off + lane;
+                    for (uint32_t w = 0; w < W; ++w) mblk[w * 32 + lane] = src[w * 32];
+                }
+                __syncwarp();
+                const uint32_t *mcol = mblk + (active ? lane : 0);
+                uint32_t w = 0, m = 0, qtop = 0;
+                for (;;) {
+                    while (m == 0 && w < W) {
+                        m = mcol[w * 32];
+                        qtop = wq[w];
+                        ++w;
+                    }
+                    if (m == 0) break;
+                    const int hb = 31 - __clz(m);                       // ascending candidates = descending bits
+                    m ^= 1u << hb;
+                    const uint16_t v = (uint16_t)(qtop - (uint32_t)hb);
+                    if (staged) dst_s[n] = v; else dst_g[n] = v;
+                    ++n;
+                }
+            } else {
+                __syncwarp();
+                const int zlo = DIM == 3 ? -1 : 0, zhi = DIM == 3 ? 1 : 0;
+                for (int dz = zlo; dz <= zhi; ++dz) {
+                    const int sz = sl[2] + dz;
+                    if (DIM == 3 && (sz < 0 || sz >= tt.ext[2])) continue;
+                    for (int dy = -1; dy <= 1; ++dy) {
+                        const int sy = sl[1] + dy;
+                        if (sy < 0 || sy >= tt.ext[1]) continue;
+                        const int rowbase = tt.ext[0] * (sy + tt.ext[1] * sz);
+                        const int xa = max(sl[0] - 1, 0), xb = min(sl[0] + 1, tt.ext[0] - 1);
+                        const uint32_t q0 = tt.h_off[rowbase + xa], q1 = tt.h_off[rowbase + xb + 1];
+                        for (uint32_t q = q0; q < q1; q += 32, mp += 32) {
+                            const uint32_t qtop = min(q + 32u, q1) - 1u;       // candidate of bit 0
+                            uint32_t m = *mp;
+                            while (m) {
+                                const int hb = 31 - __clz(m);
+                                m ^= 1u << hb;
+                                const uint16_t v = (uint16_t)(qtop - (uint32_t)hb);
+                                if (staged) dst_s[n] = v; else dst_g[n] = v;
+                                ++n;
+                            }
+                        }
+                    }
+                }
+            }
+            if (staged) {
+                __syncwarp();
+                uint16_t *out = col16 + seg0;
+                for (uint32_t k = lane; k < total; k += 32) out[k] = wbuf[k];
+                __syncwarp();
+            }
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------- tile statistics
 // largest halo population and largest row count over all tiles of a candidate decomposition (one thread per tile)
 template <int DIM>
 __global__ void k_tile_stats(TileGeom tg, const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
-                             uint32_t *__restrict__ out /* [2]: Mmax, Tmax */)
+                             uint32_t *__restrict__ out /* [2]: Mmax, Tmax */, uint32_t *__restrict__ occ_out)
 {
     const int tile = blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t M = 0, T = 0;
+    uint32_t M = 0, T = 0, occ = 0;
     if (tile < tg.ntiles) {
         int b = tile, bc[3] = {0, 0, 0};
         bc[0] = b % tg.nb[0];
@@ -241,13 +415,16 @@ __global__ void k_tile_stats(TileGeom tg, const uint32_t *__restrict__ cell_star
                     const uint32_t cc = cell_end[lin] - cell_start[lin];
                     M += cc;
                     if (tgt) T += cc;
+                    occ = max(occ, cc);
                 }
     }
     M = __reduce_max_sync(0xffffffffu, M);
     T = __reduce_max_sync(0xffffffffu, T);
+    occ = __reduce_max_sync(0xffffffffu, occ);
     if ((threadIdx.x & 31) == 0) {
         atomicMax(&out[0], M);
         atomicMax(&out[1], T);
+        atomicMax(occ_out, occ);                     // largest cell occupancy
     }
 }
 
@@ -318,13 +495,13 @@ int sph_tile_candidates(const sph_ctx *ctx, int out[3])
 int sph_tile_stats_launch(sph_ctx *ctx, const int *cand, int ncand, cudaStream_t st)
 {
     uint32_t *stats = ctx->stats.as<uint32_t>();
-    SPH_CUDA_TRY(cudaMemsetAsync(stats + 4, 0, 6 * sizeof(uint32_t), st));
+    SPH_CUDA_TRY(cudaMemsetAsync(stats + 4, 0, 7 * sizeof(uint32_t), st));
     for (int k = 0; k < ncand; ++k) {
         const TileGeom tg = make_tile_geom(ctx->geom, cand[k]);
         KScope ks(ctx, SPH_K_COUNT, 1, st);
         const unsigned nb = (unsigned)((tg.ntiles + 127) / 128);
-        if (tg.dim == 3) k_tile_stats<3><<<nb, 128, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), stats + 4 + 2 * k);
-        else k_tile_stats<2><<<nb, 128, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), stats + 4 + 2 * k);
+        if (tg.dim == 3) k_tile_stats<3><<<nb, 128, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), stats + 4 + 2 * k, stats + 10);
+        else k_tile_stats<2><<<nb, 128, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), stats + 4 + 2 * k, stats + 10);
     }
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
@@ -340,8 +517,8 @@ bool sph_tile_fits(int dim, uint32_t Mmax)
 }
 
 // count / scan / fill of the tile-local lists with tile edge B.  Synchronises `st` once (nnz readback).
-int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mmax, uint32_t Tmax, cudaStream_t st,
-                           int64_t *nnz_out)
+int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mmax, uint32_t Tmax, uint32_t occmax,
+                           cudaStream_t st, int64_t *nnz_out)
 {
     const int64_t n = ctx->n;
     const GridGeom &gg = ctx->geom;
@@ -352,12 +529,32 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
     SPH_TRY(ctx->row_ptr.reserve((size_t)(n + 1) * 8));
     const float4 *pos = ctx->pos_s.as<float4>();
     const uint32_t *cs = ctx->cell_start.as<uint32_t>(), *ce = ctx->cell_end.as<uint32_t>();
+    // hit masks of the count pass (so that the fill repeats no distance test): upper bound of the mask words from
+    // the largest cell occupancy -- no extra readback.  Beyond 6 GB the fill recomputes the tests instead.
+    uint32_t *maskbuf = nullptr;
+    long long *mask_base = nullptr;
+    {
+        int nr = gg.dim == 3 ? 9 : 3;
+        const double wmax = (double)nr * (double)((3u * occmax + 31u) / 32u);
+        const double bound = ((double)n + 32.0 * (double)ctx->ncells_total) * wmax;
+        if (ctx->opt_fill_masks && bound * 4.0 <= 6.0e9) {
+            SPH_TRY(ctx->maskbuf.reserve((size_t)bound * 4 + 256));
+            SPH_TRY(ctx->tile_words.reserve((size_t)tg.ntiles * 4));
+            SPH_TRY(ctx->tile_mask_base.reserve((size_t)(tg.ntiles + 1) * 8));
+            maskbuf = ctx->maskbuf.as<uint32_t>();
+            mask_base = ctx->tile_mask_base.as<long long>();
+            KScope ks(ctx, SPH_K_COUNT, 4, st);
+            if (gg.dim == 3) k_tile_words<3><<<(unsigned)tg.ntiles, 64, 0, st>>>(tg, cs, ce, ctx->tile_words.as<uint32_t>());
+            else k_tile_words<2><<<(unsigned)tg.ntiles, 64, 0, st>>>(tg, cs, ce, ctx->tile_words.as<uint32_t>());
+            SPH_TRY(sph_scan_u32(ctx, ctx->tile_words.as<uint32_t>(), mask_base, true, tg.ntiles, st));
+        }
+    }
 #define SPH_NBT_LAUNCH(DIM, FILL, VARH, SMEM, WCAP, CNT, RP, COL)                                                      \
     do {                                                                                                               \
         SPH_CUDA_TRY(cudaFuncSetAttribute(k_nb_tile<DIM, FILL, VARH>, cudaFuncAttributeMaxDynamicSharedMemorySize,     \
                                           (int)(SMEM)));                                                               \
-        k_nb_tile<DIM, FILL, VARH><<<(unsigned)tg.ntiles, kNbWarps * 32, (SMEM), st>>>(tg, gg, sp, mcap, (WCAP), pos,  \
-                                                                                      cs, ce, CNT, RP, COL);           \
+        k_nb_tile<DIM, FILL, VARH><<<(unsigned)tg.ntiles, kNbWarps * 32, (SMEM), st>>>(                                \
+            tg, gg, sp, mcap, (WCAP), pos, cs, ce, CNT, RP, COL, (FILL) ? nullptr : maskbuf, mask_base);               \
     } while (0)
 #define SPH_NBT_DISPATCH(FILL, SMEM, WCAP, CNT, RP, COL)                                                               \
     do {                                                                                                               \
@@ -394,8 +591,28 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
             if (w2 < wcap) wcap = w2;
         }
         KScope ks(ctx, SPH_K_FILL, 1, st);
+        if (maskbuf) {
+            int wc = (int)(32.0 * mean * 1.2) + 64;
+            wc = (wc + 63) & ~63;
+            if (wc < 512) wc = 512;
+            if (wc > 12288) wc = 12288;
+            int wb = (gg.dim == 3 ? 9 : 3) * (int)((3u * occmax + 31u) / 32u);      // most mask words a row can have
+            if (wb > 64) wb = 64;
+            const int ew = 4;                                                       // warps per CTA
+            const size_t smem = (size_t)ew * ((size_t)wc * 2 + (size_t)wb * 128);
+            if (gg.dim == 3) {
+                SPH_CUDA_TRY(cudaFuncSetAttribute(k_nb_expand<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                k_nb_expand<3><<<(unsigned)tg.ntiles, ew * 32, smem, st>>>(tg, wc, wb, cs, ce, ctx->row_ptr.as<long long>(),
+                                                                               ctx->col16.as<uint16_t>(), maskbuf, mask_base);
+            } else {
+                SPH_CUDA_TRY(cudaFuncSetAttribute(k_nb_expand<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                k_nb_expand<2><<<(unsigned)tg.ntiles, ew * 32, smem, st>>>(tg, wc, wb, cs, ce, ctx->row_ptr.as<long long>(),
+                                                                               ctx->col16.as<uint16_t>(), maskbuf, mask_base);
+            }
+        } else {
         const size_t smem = pos_bytes + (size_t)kNbWarps * wcap * 2;
         SPH_NBT_DISPATCH(true, smem, wcap, nullptr, ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>());
+        }
     }
 #undef SPH_NBT_DISPATCH
 #undef SPH_NBT_LAUNCH

@@ -7,7 +7,7 @@ import torch
 
 import oracle
 from paper_2507_21684_b200 import workloads as W
-from paper_2507_21684_b200.binding import Sph, SphError, OPT_LIST_MODE, OPT_TILE_EDGE, LIST_GENERIC
+from paper_2507_21684_b200.binding import Sph, SphError, OPT_LIST_MODE, OPT_TILE_EDGE, OPT_FILL_MASKS, LIST_GENERIC
 from common import max_norm_err
 from gpu_common import Dev, build, oracle_lists
 
@@ -44,6 +44,7 @@ def sph(request):
         s.set_option(OPT_LIST_MODE, LIST_GENERIC)
     elif request.param == "tile_b1":
         s.set_option(OPT_TILE_EDGE, 1)
+        s.set_option(OPT_FILL_MASKS, 0)          # this variant also covers the fill that repeats the distance tests
     yield s
     s.close()
 
