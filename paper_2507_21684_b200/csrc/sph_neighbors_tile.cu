@@ -325,20 +325,48 @@ k_nb_expand(TileGeom tg, int wcap, int wbcap, const uint32_t *__restrict__ cell_
                     for (uint32_t w = 0; w < W; ++w) mblk[w * 32 + lane] = src[w * 32];
                 }
                 __syncwarp();
-                const uint32_t *mcol = mblk + (active ? lane : 0);
-                uint32_t w = 0, m = 0, qtop = 0;
-                for (;;) {
-                    while (m == 0 && w < W) {
-                        m = mcol[w * 32];
-                        qtop = wq[w];
-                        ++w;
+                // one flat loop, byte addresses kept in registers: an iteration either fetches the lane's next mask
+                // word or emits one hit
+                uint32_t maddr = (uint32_t)__cvta_generic_to_shared(mblk + (active ? lane : 0));
+                uint32_t waddr = (uint32_t)__cvta_generic_to_shared(wq);
+                const uint32_t mend = maddr + W * 128u;
+                uint32_t m = 0, qtop = 0;
+                if (staged) {
+                    uint32_t daddr = (uint32_t)__cvta_generic_to_shared(dst_s);
+                    // the warp vote ends the loop for all lanes together and keeps them converged: without it the
+                    // lanes split into independently scheduled fragments and the instruction count triples
+                    for (;;) {
+                        const bool empty = m == 0;
+                        const bool more = maddr != mend;
+                        if (empty) {
+                            if (more) {
+                                asm volatile("ld.shared.u32 %0, [%1];" : "=r"(m) : "r"(maddr));
+                                asm volatile("ld.shared.u16 %0, [%1];" : "=r"(qtop) : "r"(waddr));
+                                maddr += 128u;
+                                waddr += 2u;
+                            }
+                        } else {
+                            const uint32_t hb = 31u - (uint32_t)__clz(m);      // ascending candidates = descending bits
+                            m ^= 1u << hb;
+                            asm volatile("st.shared.u16 [%0], %1;" ::"r"(daddr), "r"(qtop - hb) : "memory");
+                            daddr += 2u;
+                        }
+                        if (__all_sync(0xffffffffu, empty && !more)) break;
                     }
-                    if (m == 0) break;
-                    const int hb = 31 - __clz(m);                       // ascending candidates = descending bits
-                    m ^= 1u << hb;
-                    const uint16_t v = (uint16_t)(qtop - (uint32_t)hb);
-                    if (staged) dst_s[n] = v; else dst_g[n] = v;
-                    ++n;
+                } else {
+                    for (;;) {
+                        if (m == 0) {
+                            if (maddr == mend) break;
+                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(m) : "r"(maddr));
+                            asm volatile("ld.shared.u16 %0, [%1];" : "=r"(qtop) : "r"(waddr));
+                            maddr += 128u;
+                            waddr += 2u;
+                        } else {
+                            const uint32_t hb = 31u - (uint32_t)__clz(m);
+                            m ^= 1u << hb;
+                            dst_g[n++] = (uint16_t)(qtop - hb);
+                        }
+                    }
                 }
             } else {
                 __syncwarp();
