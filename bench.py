@@ -121,18 +121,34 @@ class ClockSampler:
 
 
 # --------------------------------------------------------------------------------------------------------------
-# algorithmic bytes per launch of the pair kernels
-def algorithmic_bytes(cls, n, nnz, dim):
+# algorithmic bytes / flops per launch
+FLOP_PER_PAIR = {"rhs": 60.0, "vjp": 170.0, "density": 25.0}     # FMA = 2 flop, MUFU = 1
+FP32_LANES_PER_SM, N_SM = 128, 148                               # B200_PROFILING.md / B300_MICROARCH.md unit counts
+
+
+def algorithmic_bytes(cls, n, nnz, dim, idx_bytes):
+    """HBM bytes one launch has to move: the index stream (2 B per entry in the tile-local layout, 4 B in the generic
+    one), row_ptr, the per-particle state read once and the outputs written once.  Neighbour state is served from
+    shared memory / L2 and is not HBM traffic."""
     state = 40 if dim == 3 else 32                   # sorted SoA s0,s1(,s2) read once per row
     if cls == "rhs":
-        return 4 * nnz + 8 * (n + 1) + n * (state + 1 + 16)              # + kind + {a, drho/dt}
+        return idx_bytes * nnz + 8 * (n + 1) + n * (state + 1 + 16)              # + kind + {a, drho/dt}
     if cls == "vjp":
-        return 4 * nnz + 8 * (n + 1) + n * (state + 16 + 16 + 32)        # + cotangents + EOS derivs + {xbar,rhobar},{vbar}
+        return idx_bytes * nnz + 8 * (n + 1) + n * (state + 16 + 16 + 32)        # + cotangents + EOS derivs + {xbar,rhobar},{vbar}
     if cls == "density":
-        return 4 * nnz + 8 * (n + 1) + n * (16 + 4 + 4 + 4)              # pos, m, perm, rho
+        return idx_bytes * nnz + 8 * (n + 1) + n * (16 + 4 + 4 + 4)              # pos, m, perm, rho
     if cls in ("count", "fill"):
-        return (4 * nnz if cls == "fill" else 0) + n * (16 + 4) + 8 * n  # pos + cnt/row_ptr (+ col written)
+        return (idx_bytes * nnz if cls == "fill" else 0) + n * (16 + 4) + 8 * n  # pos + cnt/row_ptr (+ lists written)
     return None
+
+
+def measured_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture"""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p))
+    except Exception:
+        return {}
 
 
 def cpu_sample(wl, budget_s=12.0, seed=3):
@@ -282,6 +298,8 @@ def main():
     for _ in range(args.warmup):
         step(False)
     sph.check()
+    layout = sph.layout()
+    idx_bytes = 2 if layout["mode"] == 2 else 4
     sph.profile_read()                               # clear accumulators
     launches0 = sph.info()["launches"]
     sph.profile_enable(True)
@@ -362,21 +380,42 @@ def main():
                    "count": (counts["nnz"] + counts["nnz_rk"]) / (2.0 * args.steps),
                    "fill": (counts["nnz"] + counts["nnz_rk"]) / (2.0 * args.steps)}
         roof = {}
+        traffic = measured_traffic()
+        fp32_peak = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12       # TFLOP/s, FMA = 2 flop
         for c in cand:
             ms_launch = prof[c][0] / max(prof[c][1] / (2 if c == "density" else 1), 1)
-            by = algorithmic_bytes(c, n, nnz_for[c], dim)
-            roof[c] = {"bound": "hbm", "achieved": by / (ms_launch * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
-                       "frac": by / (ms_launch * 1e-3) / 1e9 / hbm, "traffic": None, "kernel": c,
-                       "ms_per_launch": ms_launch, "algorithmic_bytes_per_launch": int(by), "peak_source": hbm_src}
-        fb_bytes = algorithmic_bytes("rhs", n, nnz_mean, dim) + algorithmic_bytes("vjp", n, nnz_mean, dim)
+            if c == "count":                         # the class also holds the tiny tile-statistics launches
+                ms_launch = prof[c][0] / (2.0 * args.steps)
+            by = algorithmic_bytes(c, n, nnz_for[c], dim, idx_bytes)
+            tr = traffic.get(c)
+            hbm_view = {"bound": "hbm", "achieved": by / (ms_launch * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                        "frac": by / (ms_launch * 1e-3) / 1e9 / hbm, "traffic": tr, "kernel": c,
+                        "ms_per_launch": ms_launch, "algorithmic_bytes_per_launch": int(by), "peak_source": hbm_src}
+            if c in FLOP_PER_PAIR:
+                # the pair kernels are bound by FP32 issue / shared-memory gathers, not by HBM (profiles/): their
+                # roofline is the plain-ALU one; the HBM view north_star asks for is kept beside it
+                fl = FLOP_PER_PAIR[c] * nnz_for[c]
+                ach = fl / (ms_launch * 1e-3) / 1e12
+                roof[c] = {"bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s", "frac": ach / fp32_peak,
+                           "traffic": tr, "kernel": c, "ms_per_launch": ms_launch,
+                           "algorithmic_flop_per_launch": fl, "flop_per_pair": FLOP_PER_PAIR[c],
+                           "peak_source": f"{N_SM} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max:.0f} MHz "
+                                          "(unit counts of the guides, clocks.max.sm of MEASURED_PEAKS.json)",
+                           "hbm": hbm_view}
+            else:
+                roof[c] = hbm_view
+        fb_bytes = algorithmic_bytes("rhs", n, nnz_mean, dim, idx_bytes) + algorithmic_bytes("vjp", n, nnz_mean, dim, idx_bytes)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl.name, "n_particles": n, "dim": dim, "nnz_exact_list": int(nnz_last),
                        "nnz_skin_list": int(nnz_rk_last), "skin": SKIN, "replicas": world,
+                       "list_layout": {1: "generic int32 ids", 2: "tile-local uint16"}[layout["mode"]],
+                       "tile_edge_cells": layout["tile_edge"], "tile_halo_max": layout["halo_max"],
                        "step": "build_cells+neighbors, density, rhs, rhs_vjp, rk_step(rebuild + 4 rhs)",
-                       "l2": "inputs larger than L2: every pair pass streams the 0.8-1.0 GB CSR (L2 = 126 MB)"},
+                       "l2": "inputs larger than L2: every pair pass streams its 0.45-0.55 GB list (2 B per entry) and the "
+                             "rebuild writes it; per step > 4 GB of list traffic against L2 = 126 MB"},
             "ms_fwd_bwd": fb_ms, "pairs_per_s_fwd_bwd": 2.0 * nnz_mean / (fb_ms * 1e-3),
             "hbm_frac_fwd_bwd": fb_bytes / (fb_ms * 1e-3) / 1e9 / hbm,
             "hbm_frac_fwd_bwd_of_8TBs": fb_bytes / (fb_ms * 1e-3) / 1e9 / 8000.0,
