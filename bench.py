@@ -151,6 +151,21 @@ def measured_traffic():
         return {}
 
 
+def reduce_over_ranks(ms_local, units_local, device="cpu"):
+    """Timing contract for N > 1 (replicas only): the job's time is the MAX over ranks of the
+    device time, the job's work the SUM over ranks of the units processed.  Returns (ms_max, units_sum); a plain
+    pass-through when torch.distributed is not initialised.  The only collectives of the bench."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms_local), float(units_local)
+    tt = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    pp = torch.tensor([float(units_local)], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    dist.all_reduce(pp, op=dist.ReduceOp.SUM)
+    return float(tt.item()), float(pp.item())
+
+
 def cpu_sample(wl, budget_s=12.0, seed=3):
     """The oracle, as it stands, on a bounded sample: forward RHS + VJP of `rows` sampled rows of the workload (lists
     from the oracle's own grid search over all particles, timed separately)."""
@@ -324,12 +339,7 @@ def main():
     fb_ms = ph_ms["fwd"] + ph_ms["bwd"]
     nnz_mean = counts["nnz"] / args.steps
 
-    tt = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    pp = torch.tensor([float(pairs_rank)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        dist.all_reduce(pp, op=dist.ReduceOp.SUM)
-    ms_max, pairs_all = float(tt.item()), float(pp.item())
+    ms_max, pairs_all = reduce_over_ranks(ms_total, pairs_rank, dev)
     value = pairs_all / (ms_max * 1e-3)
 
     # ---- e2e: the same step through sph_step_host with pinned host buffers, copies inside the timed region
@@ -355,14 +365,10 @@ def main():
             pairs_e += 3 * a + 4 * b
         torch.cuda.synchronize()
         dt_e = time.perf_counter() - t0
-        te = torch.tensor([dt_e], dtype=torch.float64, device=dev)
-        pe = torch.tensor([float(pairs_e)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-            dist.all_reduce(pe, op=dist.ReduceOp.SUM)
+        te_max, pe_sum = reduce_over_ranks(dt_e, pairs_e, dev)
         assert np.isfinite(outs["params_bar"].numpy()).all()
-        e2e = {"value": float(pe.item()) / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "steps": ke, "ms_per_step": 1e3 * float(te.item()) / ke,
+        e2e = {"value": pe_sum / te_max, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "steps": ke, "ms_per_step": 1e3 * te_max / ke,
                "call": "sph_step_host (pinned host buffers; H2D + whole step + D2H inside the timed region)"}
 
     if rank == 0:
