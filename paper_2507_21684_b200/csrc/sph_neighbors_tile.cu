@@ -333,25 +333,32 @@ k_nb_expand(TileGeom tg, int wcap, int wbcap, const uint32_t *__restrict__ cell_
                 uint32_t m = 0, qtop = 0;
                 if (staged) {
                     uint32_t daddr = (uint32_t)__cvta_generic_to_shared(dst_s);
-                    // the warp vote ends the loop for all lanes together and keeps them converged: without it the
-                    // lanes split into independently scheduled fragments and the instruction count triples
+                    // One predicated instruction block per iteration (no divergent branch: with branches the lanes
+                    // split into independently scheduled fragments and the instruction count triples): a lane whose
+                    // word is empty fetches its next word, any other lane emits its highest set bit (ascending
+                    // candidates = descending bits).  The warp vote ends the loop for all lanes together.
                     for (;;) {
-                        const bool empty = m == 0;
-                        const bool more = maddr != mend;
-                        if (empty) {
-                            if (more) {
-                                asm volatile("ld.shared.u32 %0, [%1];" : "=r"(m) : "r"(maddr));
-                                asm volatile("ld.shared.u16 %0, [%1];" : "=r"(qtop) : "r"(waddr));
-                                maddr += 128u;
-                                waddr += 2u;
-                            }
-                        } else {
-                            const uint32_t hb = 31u - (uint32_t)__clz(m);      // ascending candidates = descending bits
-                            m ^= 1u << hb;
-                            asm volatile("st.shared.u16 [%0], %1;" ::"r"(daddr), "r"(qtop - hb) : "memory");
-                            daddr += 2u;
-                        }
-                        if (__all_sync(0xffffffffu, empty && !more)) break;
+                        asm volatile(
+                            "{\n"
+                            ".reg .pred pe, pf;\n"
+                            ".reg .u32 hb, v, bit;\n"
+                            "setp.eq.u32 pe, %0, 0;\n"
+                            "setp.ne.and.u32 pf, %2, %5, pe;\n"
+                            "@!pe bfind.u32 hb, %0;\n"
+                            "@!pe sub.u32 v, %1, hb;\n"
+                            "@!pe st.shared.u16 [%3], v;\n"
+                            "@!pe add.u32 %3, %3, 2;\n"
+                            "@!pe shl.b32 bit, 1, hb;\n"
+                            "@!pe xor.b32 %0, %0, bit;\n"
+                            "@pf ld.shared.u32 %0, [%2];\n"
+                            "@pf ld.shared.u16 %1, [%4];\n"
+                            "@pf add.u32 %2, %2, 128;\n"
+                            "@pf add.u32 %4, %4, 2;\n"
+                            "}\n"
+                            : "+r"(m), "+r"(qtop), "+r"(maddr), "+r"(daddr), "+r"(waddr)
+                            : "r"(mend)
+                            : "memory");
+                        if (__all_sync(0xffffffffu, m == 0 && maddr == mend)) break;
                     }
                 } else {
                     for (;;) {

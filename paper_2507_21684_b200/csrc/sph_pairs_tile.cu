@@ -526,11 +526,13 @@ static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, int *th
     if (rb < 64) rb = 64;
     ts->rb = rb;
     const size_t fixed = (size_t)ts->mcap * state_bytes + (size_t)(ts->tcap + 4) * 4 + (size_t)ts->tcap * 2 + 16;
-    const size_t sm_total = 233472, per_cta = 2560, cta_max = 232448 - 2048;
+    const size_t sm_total = 233472, per_cta = 4096, cta_max = 232448 - 3072;
     auto need = [&](int warps) { return fixed + (size_t)warps * 2 * rb * 2; };
-    int warps = 16;                                                // measured: 16 warps beat 8 at one and at two CTAs per SM
+    // measured (C3): two co-resident CTAs beat one (their staging and epilogue phases overlap), and at equal
+    // residency 16 warps beat 8: the largest CTA of which two fit an SM, else one 16-warp CTA
+    int warps = 16;
     if (ctx->opt_warps) warps = ctx->opt_warps;
-    (void)sm_total; (void)per_cta;
+    else if (sm_total / (need(16) + per_cta) < 2 && sm_total / (need(8) + per_cta) >= 2) warps = 8;
     while (warps > 1 && need(warps) > cta_max) warps >>= 1;
     if (need(warps) > cta_max) {                                   // last resort: a minimal ring (rows fall back to global reads)
         ts->rb = 8;
