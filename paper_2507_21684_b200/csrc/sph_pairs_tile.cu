@@ -382,7 +382,7 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
             const Part pi = load_part<DIM>(A, B, C, qi);
             const float4 ci = Ct[qi];
             const float lam_i = ci.x, mu_i[3] = {ci.y, ci.z, ci.w};
-            const float m_i = pi.V * pi.rho;
+            const float m_i = pi.V * pi.rho, Vi = pi.V, Li = lam_i * pi.rho;
             const uint32_t e = live ? e_in : b;                    // padding groups run no pairs (partials stay clean)
             const float ir_i = 1.0f / pi.rho;
             float xb[3] = {0.f, 0.f, 0.f}, vb[3] = {0.f, 0.f, 0.f}, rb = 0.f, Z = 0.f;
@@ -413,48 +413,57 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                 float mm = mu_i[0] * d[0];                          // mu_i . d
                 mm = fmaf(mu_i[1], d[1], mm);
                 if (DIM == 3) mm = fmaf(mu_i[2], d[2], mm);
-                float mmj = mu_j[0] * d[0];                         // mu_j . d   (pair (j<-i) uses -d)
+                float mmj = mu_j[0] * d[0];                         // mu_j . d   (pair (j<-i) uses -d: mmp = -mmj)
                 mmj = fmaf(mu_j[1], d[1], mmj);
                 if (DIM == 3) mmj = fmaf(mu_j[2], d[2], mmj);
-                const float mmp = -mmj;
-                // ---- ordered pair (i <- j)
-                const float VjG = pj.V * G;
-                const float E = -m_j * Psum;
-                const float Phi1 = rho0 * pj.V * s * invR * ir_i;
-                const float Phi = hc.eta * Phi1;
-                const float sbar = lam_i * pi.rho * VjG + mm * hc.eta * rho0 * VjG * invR * ir_i;
-                const float dif = hc.kd * VjG * u;                   // kd V_j (r2/R) G
-                const float r2bar = lam_i * hc.kd * VjG * drho * hc.e2 * invR * invR - mm * Phi * G * invR;
-                const float Gbar = lam_i * pj.V * (pi.rho * s + hc.kd * drho * u) + mm * (E + Phi);
-                // ---- ordered pair (j <- i): d -> -d, w -> -w, s unchanged
-                const float ViG = pi.V * G;
-                const float Ep = -m_i * Psum;
-                const float Phi1p = rho0 * pi.V * s * invR * ir_j;
-                const float Phip = hc.eta * Phi1p;
-                const float sbarp = lam_j * pj.rho * ViG + mmp * hc.eta * rho0 * ViG * invR * ir_j;
-                const float difp = hc.kd * ViG * u;
-                const float r2barp = -lam_j * hc.kd * ViG * drho * hc.e2 * invR * invR - mmp * Phip * G * invR;
-                const float ADp = ViG * (pj.rho * s - hc.kd * drho * u);          // A' + D'
-                const float Gbarp = lam_j * pi.V * (pj.rho * s - hc.kd * drho * u) + mmp * (Ep + Phip);
-                // ---- what lands on particle i
-                const float cs = sbar + sbarp;
-                const float cd = 2.0f * (r2bar + r2barp) + (Gbar + Gbarp) * K;
-                const float ce = (E + Phi) * G, cep = (Ep + Phip) * G;
+                // The two ordered pairs (i<-j) and (j<-i) of SURVEY.md 8(c-7), with their common factors pulled out
+                // (G, eta rho0 G / R, kd drho / R); primes mark the (j<-i) quantities, which use -d, -w and the roles
+                // of i and j swapped.
+                const float p = pj.V * ir_i, pp = Vi * ir_j;        // V_j/rho_i, V_i/rho_j
+                const float ri = rho0 * invR;
+                const float t0 = ri * s;
+                const float Phi1 = t0 * p, Phi1p = t0 * pp;         // Phi/eta, Phi'/eta
+                const float Phi = hc.eta * Phi1, Phip = hc.eta * Phi1p;
+                const float zz = fmaf(m_j, mm, -(m_i * mmj));       // m_j mm + m_i mm'      (-dL/dP share of the pair)
+                const float q2 = fmaf(mm, Phi, -(mmj * Phip));      // mm Phi + mm' Phi'
+                const float Lj = lam_j * pj.rho;
+                const float aV = lam_i * pj.V, bV = lam_j * Vi;
+                const float q1 = aV - bV;
+                const float du = drho * u;
+                const float kr = hc.kd * drho * invR;
+                const float D = kr * r2;                            // kd drho r2/R        (delta-term / (V G))
+                const float Dp = kr * (hc.e2 * invR);               // kd drho e2/R^2      (its r2 derivative)
+                const float gG = hc.eta * ri * G;
+                const float LL = fmaf(pj.V, Li, Vi * Lj);           // lam_i rho_i V_j + lam_j rho_j V_i
+                const float mp = fmaf(mm, p, -(mmj * pp));
+                const float cs = fmaf(G, LL, gG * mp);              // sbar + sbar'
+                const float X1 = fmaf(Dp, q1, -(invR * q2));        // (r2bar + r2bar') / G
+                const float X2 = fmaf(s, LL, fmaf(D, q1, fmaf(-Psum, zz, q2)));   // Gbar + Gbar'
+                const float cd = fmaf(G + G, X1, K * X2);
+                const float ce = G * fmaf(-m_j, Psum, Phi), cep = G * fmaf(-m_i, Psum, Phip);   // (E+Phi) G, (E'+Phi') G
 #pragma unroll
                 for (int kk = 0; kk < DIM; ++kk) {
-                    xb[kk] += cs * w[kk] + cd * d[kk] + ce * mu_i[kk] - cep * mu_j[kk];
+                    xb[kk] = fmaf(cs, w[kk], fmaf(cd, d[kk], fmaf(ce, mu_i[kk], fmaf(-cep, mu_j[kk], xb[kk]))));
                     vb[kk] = fmaf(cs, d[kk], vb[kk]);
                 }
-                rb += lam_i * (VjG * s + dif) - mm * G * Phi * ir_i                 // first role of (i<-j)
-                      - lam_j * (ADp * ir_i + difp) - mmp * G * Phip * ir_i;         // second role of (j<-i)
-                Z = fmaf(G, m_j * mm + m_i * mmp, Z);               // -dL/dP_i
-                // ---- scalar parameters, ordered pair (i<-j) only (each ordered pair is owned by one row)
-                const float D1 = 2.0f * hc.ell * VjG * drho * u;    // D_ij / (delta c0)
-                S_D1 = fmaf(lam_i, D1, S_D1);
+                const float kdu = hc.kd * u;
+                const float y2 = fmaf(fmaf(pj.rho, s, -D), ir_i, kdu);
+                rb = fmaf(G, fmaf(aV, s + kdu, -fmaf(bV, y2, ir_i * q2)), rb);
+                Z = fmaf(G, zz, Z);                                 // -dL/dP_i
+                // ---- scalar parameters, ordered pair (i<-j) only (each ordered pair is owned by one row); the
+                // H-dependent factors (2 ell, ell, H^2) are applied after the loops when h is uniform
+                const float Gdu = G * du;
                 const float xphi1 = mm * G * Phi1;
+                const float se = invR * G * fmaf(aV, D, mm * Phi);
                 S_P1 += xphi1;
-                S_PL = fmaf(xphi1, hc.ell, S_PL);
-                S_eps -= (lam_i * hc.kd * VjG * drho * u + mm * G * Phi) * invR * (2.0f * kp.eps * hc.H2);
+                if (VARH) {
+                    S_D1 = fmaf(aV * Gdu, 2.0f * hc.ell, S_D1);
+                    S_PL = fmaf(xphi1, hc.ell, S_PL);
+                    S_eps = fmaf(se, hc.H2, S_eps);
+                } else {
+                    S_D1 = fmaf(aV, Gdu, S_D1);
+                    S_eps += se;
+                }
             }
 #pragma unroll
             for (int kk = 0; kk < DIM; ++kk) {
@@ -485,6 +494,14 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                 }
             }
         });
+    // S_D1 = sum lam_i D_ij/(delta c0), S_PL = sum ell xphi1, S_eps = d/d eps: factors left out of the loop
+    if (!VARH) {
+        S_D1 *= 2.0f * hu.ell;
+        S_PL = hu.ell * S_P1;
+        S_eps *= -2.0f * kp.eps * hu.H2;
+    } else {
+        S_eps *= -2.0f * kp.eps;
+    }
     // B2 stage 1: fixed-order CTA reduction of the ten partial sums
     float vals[10] = {S_D1, S_P1, S_PL, S_eps, T_E, T_0, T_g, G0, G1, G2};
 #pragma unroll
