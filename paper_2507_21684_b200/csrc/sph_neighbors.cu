@@ -325,6 +325,19 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
         ctx->lists_ready = true;
         return SPH_OK;
     }
+    // no halo fits the pair kernels: the tile SEARCH (positions only) may still fit; its lists are translated to
+    // sorted ids and the generic pair kernels run on them
+    if (ctx->opt_list_mode == 0)
+        for (int k = ncand - 1; k >= 0; --k) {
+            const uint32_t Mmax = hs[4 + 2 * k], Tmax = hs[5 + 2 * k];
+            if (!sph_tile_search_fits(Mmax)) continue;
+            SPH_TRY(sph_neighbors_tile_run(ctx, sp, cand[k], Mmax, Tmax, hs[10], st, nnz_out));
+            SPH_TRY(sph_tile_expand_col(ctx, st));
+            ctx->tile_mode = false;
+            ctx->search_scale = search_scale;
+            ctx->lists_ready = true;
+            return SPH_OK;
+        }
 
     SPH_TRY(ctx->cnt.reserve((size_t)n * 4));
     SPH_TRY(ctx->row_ptr.reserve((size_t)(n + 1) * 8));

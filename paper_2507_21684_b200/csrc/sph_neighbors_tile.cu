@@ -546,6 +546,13 @@ int sph_tile_stats_launch(sph_ctx *ctx, const int *cand, int ncand, cudaStream_t
 size_t sph_tile_state_bytes(int dim) { return dim == 3 ? 56 : 48; }   // VJP: state + cotangents per halo particle
 static const size_t kTileSmemBudget = 200 * 1024;
 
+// the tile SEARCH only stages positions (16 B per halo particle): it fits far larger halos than the pair kernels.
+// Its lists are then translated to sorted ids for the generic pair kernels (BASELINE config 4: 134 particles per cell).
+bool sph_tile_search_fits(uint32_t Mmax)
+{
+    return Mmax > 0 && Mmax <= 65535u && (size_t)(Mmax + 8) * 16 + 8 * 2 * 4096 <= kTileSmemBudget;
+}
+
 bool sph_tile_fits(int dim, uint32_t Mmax)
 {
     return Mmax > 0 && Mmax <= 65535u && (size_t)(Mmax + 8) * sph_tile_state_bytes(dim) + (size_t)(Mmax + 8) * 4 <= kTileSmemBudget;
@@ -565,14 +572,14 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
     const float4 *pos = ctx->pos_s.as<float4>();
     const uint32_t *cs = ctx->cell_start.as<uint32_t>(), *ce = ctx->cell_end.as<uint32_t>();
     // hit masks of the count pass (so that the fill repeats no distance test): upper bound of the mask words from
-    // the largest cell occupancy -- no extra readback.  Beyond 6 GB the fill recomputes the tests instead.
+    // the largest cell occupancy -- no extra readback.  Beyond 24 GB the fill recomputes the tests instead.
     uint32_t *maskbuf = nullptr;
     long long *mask_base = nullptr;
     {
         int nr = gg.dim == 3 ? 9 : 3;
         const double wmax = (double)nr * (double)((3u * occmax + 31u) / 32u);
         const double bound = ((double)n + 32.0 * (double)ctx->ncells_total) * wmax;
-        if (ctx->opt_fill_masks && bound * 4.0 <= 6.0e9) {
+        if (ctx->opt_fill_masks && bound * 4.0 <= 24.0e9) {
             SPH_TRY(ctx->maskbuf.reserve((size_t)bound * 4 + 256));
             SPH_TRY(ctx->tile_words.reserve((size_t)tg.ntiles * 4));
             SPH_TRY(ctx->tile_mask_base.reserve((size_t)(tg.ntiles + 1) * 8));
@@ -617,8 +624,8 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
         int wcap = (int)(32.0 * mean * 1.35) + 64;
         wcap = (wcap + 63) & ~63;
         if (wcap < 512) wcap = 512;
-        const size_t budget = 100 * 1024;                      // two CTAs per SM
         const size_t pos_bytes = (size_t)mcap * sizeof(float4);
+        const size_t budget = pos_bytes > 48 * 1024 ? 200 * 1024 : 100 * 1024;   // two CTAs per SM when the halo is small
         if (pos_bytes + (size_t)kNbWarps * wcap * 2 > budget) {
             const size_t room = pos_bytes < budget ? budget - pos_bytes : 0;
             int w2 = (int)(room / (kNbWarps * 2)) & ~63;

@@ -278,8 +278,9 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
     tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
         [&](uint32_t r, bool live, uint32_t b, uint32_t e, const uint16_t *idx) {
             const Part pi = load_part<DIM>(A, B, C, selfq[r]);
-            const float visc_i = rho0 / pi.rho;               // rho0/rho_i of the viscous term
+            const float visc_i = rho0 * fast_rcp(pi.rho);     // rho0/rho_i of the viscous term
             const float ev_u = hu.eta * visc_i;
+            const bool fixed = kind_s[row0 + r] != 0;         // loaded before the pair loop: its latency is hidden
             float sA = 0.f, sD = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f;
 #pragma unroll 2
             for (uint32_t k = b + gl; k < e; k += GS) {
@@ -320,7 +321,6 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
             if (DIM == 3) a2 = group_sum<GS>(a2);
             if (gl == 0 && live) {
                 const uint32_t row = row0 + r;
-                const bool fixed = kind_s[row] != 0;
                 a0 = fixed ? 0.f : a0 + kp.g[0];
                 a1 = fixed ? 0.f : a1 + kp.g[1];
                 a2 = fixed ? 0.f : a2 + kp.g[2];

@@ -45,5 +45,6 @@ static __device__ __forceinline__ bool pred_exact(const float4 &a, const float4 
 int sph_tile_candidates(const sph_ctx *ctx, int out[3]);
 int sph_tile_stats_launch(sph_ctx *ctx, const int *cand, int ncand, cudaStream_t st);
 bool sph_tile_fits(int dim, uint32_t Mmax);
+bool sph_tile_search_fits(uint32_t Mmax);
 int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mmax, uint32_t Tmax, uint32_t occmax,
                            cudaStream_t st, int64_t *nnz_out);

@@ -296,3 +296,29 @@ def test_full_size_sampled_rows(sph, cfg):
     sv = vb.double().sum(0).abs().max().item() / vb.double().abs().sum().item()
     assert sx < 1e-5 and sv < 1e-5
     assert torch.isfinite(pb).all()
+
+
+def test_tile_search_with_generic_lists_when_a_halo_exceeds_the_pair_budget(sph):
+    """dense cells (~300 particles each, the regime of BASELINE config 4): the halo of even a one-cell block does not
+    fit the shared-memory budget of the pair kernels, so the tile search runs alone and hands 32-bit lists to the
+    generic pair kernels; lists stay bit-exact, sums within tolerance"""
+    if sph.layout_name != "tile":
+        pytest.skip("automatic layout only")
+    rng = np.random.default_rng(5)
+    n = 8000
+    x = rng.uniform(0.0, 1.0, size=(n, 3)).astype(np.float32)
+    h = np.full(n, 0.3, np.float32)
+    dom = W.Domain(dim=3, periodic=(1, 1, 1), lo=(0.0,) * 3, hi=(1.0,) * 3, cell_size=0.3)
+    par = W.make(3, n_axis=8).params
+    wl = W.Workload(name="dense", domain=dom, params=par, x=x, v=rng.normal(0, 0.1, size=(n, 3)).astype(np.float32),
+                    rho=(1.0 + 0.02 * rng.normal(size=n)).astype(np.float32), m=np.full(n, 1.0 / n, np.float32), h=h,
+                    kind=np.zeros(n, np.uint8), dt=0.0, dx=0.05, seed=0)
+    _, dev, nnz = build(wl, 1.0, sph)
+    lay = sph.layout()
+    assert lay["mode"] == 1                       # generic lists ...
+    rp, ci = sph.neighbors_export()
+    rp_o, ci_o = oracle_lists(wl)
+    assert nnz == int(rp_o[-1]) and np.array_equal(_np(rp), rp_o) and np.array_equal(_np(ci), ci_o)
+    drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+    d_o, a_o, sd, sa = oracle.rhs(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp_o, ci_o, with_scales=True)
+    assert max_norm_err(_np(drho), d_o, sd) < TOL_FWD and max_norm_err(_np(acc), a_o, sa) < TOL_FWD
