@@ -538,7 +538,7 @@ static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, int *th
     ts->mcap = (int)((ctx->tile_Mmax + 7u) & ~7u);
     ts->tcap = (int)((ctx->tile_Tmax + 7u) & ~7u);
     const double mean = ctx->n > 0 ? (double)ctx->nnz / (double)ctx->n : 1.0;
-    int rb = (int)((32 / gs) * mean * 1.5) + 24;
+    int rb = (int)((32 / gs) * mean * 1.25) + 24;
     rb = (rb + 7) & ~7;
     if (rb < 64) rb = 64;
     ts->rb = rb;
