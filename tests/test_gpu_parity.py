@@ -322,3 +322,39 @@ def test_tile_search_with_generic_lists_when_a_halo_exceeds_the_pair_budget(sph)
     drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)
     d_o, a_o, sd, sa = oracle.rhs(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp_o, ci_o, with_scales=True)
     assert max_norm_err(_np(drho), d_o, sd) < TOL_FWD and max_norm_err(_np(acc), a_o, sa) < TOL_FWD
+
+
+def test_gradient_through_several_rk_steps(sph):
+    """BASELINE.json config 1 in miniature: several RK4 steps forward (the states are kept by the caller), then the
+    gradient of the final kinetic energy with respect to the initial state back through all steps, one
+    sph_rk_step_vjp per step in reverse; the oracle does the same chain in fp64"""
+    wl = W.perturbed(W.make(1, n_axis=40), amp_x=0.0, amp_rho=0.01)
+    skin, nsteps = 0.1, 3
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin) * np.float32(1.0001))
+    dev = Dev(wl)
+    states = [(dev.x.clone(), dev.v.clone(), dev.rho.clone())]
+    for _ in range(nsteps):
+        x, v, rho = (t.clone() for t in states[-1])
+        sph.rk_step(wl.domain, wl.params, wl.dt, skin, x, v, rho, dev.m, dev.h, dev.kind)
+        states.append((x, v, rho))
+    xb = torch.zeros_like(dev.x)
+    vb = (dev.m[:, None] * states[-1][1]).contiguous()
+    rb = torch.zeros_like(dev.rho)
+    pb = torch.zeros(10, device="cuda")
+    for k in range(nsteps - 1, -1, -1):
+        x0, v0, r0 = states[k]
+        sph.rk_step_vjp(wl.domain, wl.params, wl.dt, skin, x0, v0, r0, dev.m, dev.h, dev.kind, xb, vb, rb, pb)
+    # oracle chain
+    so = [(wl.x.astype(np.float64), wl.v.astype(np.float64), wl.rho.astype(np.float64))]
+    for _ in range(nsteps):
+        so.append(oracle.rk4_step(wl.domain, wl.params, wl.dt, *so[-1], wl.m, wl.h, wl.kind, method=1))
+    xo, vo, ro = np.zeros_like(so[-1][0]), wl.m.astype(np.float64)[:, None] * so[-1][1], np.zeros(wl.n)
+    po = np.zeros(10)
+    for k in range(nsteps - 1, -1, -1):
+        xo, vo, ro, pk = oracle.rk4_step_vjp(wl.domain, wl.params, wl.dt, *so[k], wl.m, wl.h, wl.kind, xo, vo, ro, method=1)
+        po = po + pk
+    errs = dict(x=max_norm_err(_np(xb), xo), v=max_norm_err(_np(vb), vo), rho=max_norm_err(_np(rb), ro))
+    pg = _np(pb).astype(np.float64)
+    pe = np.abs(pg - po) / np.maximum(np.abs(po), 1e-3 * np.max(np.abs(po)) + 1e-30)
+    print(f"{nsteps} steps: vjp errs {errs} params {np.max(pe):.2e}")
+    assert max(errs.values()) < TOL_VJP and np.max(pe) < TOL_VJP
