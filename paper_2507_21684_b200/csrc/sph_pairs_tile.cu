@@ -533,7 +533,8 @@ static int tile_group(const sph_ctx *ctx, bool vjp)
 }
 
 // threads per CTA, shared-memory carve-up and size for a pair kernel with `state_bytes` per halo particle
-static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, int *threads, TileSizes *ts, size_t *smem)
+static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, size_t static_smem, int *threads, TileSizes *ts,
+                            size_t *smem)
 {
     ts->mcap = (int)((ctx->tile_Mmax + 7u) & ~7u);
     ts->tcap = (int)((ctx->tile_Tmax + 7u) & ~7u);
@@ -543,7 +544,7 @@ static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, int *th
     if (rb < 64) rb = 64;
     ts->rb = rb;
     const size_t fixed = (size_t)ts->mcap * state_bytes + (size_t)(ts->tcap + 4) * 4 + (size_t)ts->tcap * 2 + 16;
-    const size_t sm_total = 233472, per_cta = 4096, cta_max = 232448 - 3072;
+    const size_t sm_total = 233472, per_cta = 1024 + static_smem, cta_max = 232448 - static_smem;   // B200: 228 KB per SM, 227 KB per CTA
     auto need = [&](int warps) { return fixed + (size_t)warps * 2 * rb * 2; };
     // measured (C3): two co-resident CTAs beat one (their staging and epilogue phases overlap), and at equal
     // residency 16 warps beat 8: the largest CTA of which two fit an SM, else one 16-warp CTA
@@ -568,7 +569,7 @@ int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, floa
     int threads;
     TileSizes ts;
     size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, &threads, &ts, &smem);   // same carve-up as the RHS kernel (SmemMap)
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);   // same carve-up as the RHS kernel (SmemMap)
 #define SPH_DT_LAUNCH(DIM, GS, VARH)                                                                                  \
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_density_tile<DIM, GS, VARH>), smem);                                                    \
@@ -600,7 +601,7 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
     int threads;
     TileSizes ts;
     size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, &threads, &ts, &smem);
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);
     const bool sorted = out4 != nullptr;
 #define SPH_RT_LAUNCH(DIM, GS, VARH, SORTED)                                                                         \
     do {                                                                                                             \
@@ -639,7 +640,7 @@ int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
     int threads;
     TileSizes ts;
     size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 56 : 48, gs, &threads, &ts, &smem);
+    tile_launch_cfg(ctx, kp.dim == 3 ? 56 : 48, gs, sizeof(TileTab) + kPtMaxWarps * kNPartT * 4, &threads, &ts, &smem);
     const bool sorted = xb4 != nullptr;
 #define SPH_VT_LAUNCH(DIM, GS, VARH, SORTED)                                                                          \
     do {                                                                                                              \
