@@ -2,15 +2,17 @@
 // count and fill of TILE-LOCAL compact lists (uint16 halo-linear indices), PAPER.md:558 (adjacent-cell query),
 // PAPER.md:163 (pair list), PAPER.md:167 (radius max{h_i,h_j}).
 //
-// One CTA per tile.  The halo positions are staged in shared memory once.  A warp takes 32 rows OF ONE CELL, one
-// row per lane: all lanes walk the same candidate sequence, so every candidate is ONE broadcast shared-memory load
-// and 9 instructions for 32 row-candidate tests (the first path of this round spent 110 per 32): the verdict is the
-// sign bit of r2 - Hs2, funnel-shifted into a per-lane 32-candidate mask; the binary64 predicate of reading R3 runs
-// only for blocks whose closest call falls inside the fp32 uncertainty band.  Count = popc of the masks; fill
-// expands the masks into a
-// per-warp shared-memory image of the warp's contiguous col16 segment (rows of a cell are contiguous in the
-// sorted order, so their list segments are too), which is then flushed coalesced.  Deterministic: fixed candidate
-// order (cells in z,y,x order, ascending sorted index inside a cell), no atomics.
+// Count (k_nb_tile<FILL=0>): one CTA per tile.  The halo positions are staged in shared memory once.  A warp takes 32
+// rows OF ONE CELL, one row per lane: all lanes walk the same candidate sequence, so every candidate is ONE broadcast
+// shared-memory load and 8-9 instructions for 32 row-candidate tests (the first path of this round spent 110 per 32):
+// the verdict is the sign bit of r2 - Hs2, funnel-shifted into a per-lane 32-candidate mask; the binary64 predicate of
+// reading R3 runs only for blocks whose closest call falls inside the fp32 uncertainty band.  The count of a row is the
+// popcount of its masks; the masks are kept (coalesced, [item][word][lane]).
+// Fill (k_nb_expand): no distance is computed twice.  Same work items; a lane expands the masks of its row in candidate
+// order (cells in z,y,x order, ascending sorted index inside a cell) into a per-warp shared-memory image of the warp's
+// contiguous col16 segment (rows of a cell are contiguous in the sorted order, so their list segments are too), which
+// is then flushed coalesced.  k_nb_tile<FILL=1> is the variant that repeats the tests (no mask buffer).
+// Deterministic: fixed candidate order, no atomics.
 #include "sph_internal.cuh"
 #include "sph_tiles.cuh"
 #include "sph_search.cuh"
@@ -93,7 +95,6 @@ __device__ __forceinline__ uint32_t nb_mask(const RowCtx &rc, const float4 *__re
     return m;
 }
 
-// `dst`: FILL only -- where this lane's hits go (shared-memory image or global col16), indexed by rc.n
 // mask words per row of the cell at halo slot sl: one per 32 candidates of each of its 3^(d-1) x-runs
 template <int DIM>
 __device__ __forceinline__ uint32_t cell_words(const TileTab &tt, const int sl[3])
@@ -114,6 +115,7 @@ __device__ __forceinline__ uint32_t cell_words(const TileTab &tt, const int sl[3
     return w;
 }
 
+// `dst`: FILL only -- where this lane's hits go (shared-memory image or global col16), indexed by rc.n
 // `maskp` (count pass, may be null): this lane's column of the item's mask block; word w of the row at maskp[32 w]
 template <int DIM, bool FILL, bool VARH, class DstT>
 __device__ __forceinline__ void nb_rows(RowCtx &rc, const float4 *__restrict__ cand, const int sl[3], const SearchPar &sp,
