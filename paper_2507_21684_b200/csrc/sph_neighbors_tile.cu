@@ -296,6 +296,16 @@ k_nb_expand(TileGeom tg, int wcap, int wbcap, const uint32_t *__restrict__ cell_
             const uint32_t *mp = maskbuf + mask_off + (active ? lane : 0);
             uint16_t *dst_s = wbuf + (uint32_t)(mine - seg0);
             uint16_t *dst_g = col16 + mine;
+            // the item's mask block into shared memory with cp.async (all W x 128 B in flight at once, overlapped
+            // with the table build below; a plain load/store loop exposes the global latency once per word)
+            const uint32_t Wi = item_words >> 5;
+            if (Wi <= kWqCap && Wi <= (uint32_t)wbcap) {
+                const uint32_t *src = maskbuf + mask_off + lane;
+                const uint32_t dsts = (uint32_t)__cvta_generic_to_shared(mblk + lane);
+                for (uint32_t w = 0; w < Wi; ++w)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dsts + w * 128u), "l"(src + w * 32) : "memory");
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
             // candidate of bit 0 of every mask word of this cell's rows
             uint16_t *wq = wqtab[warp];
             uint32_t W = 0;
@@ -322,10 +332,7 @@ k_nb_expand(TileGeom tg, int wcap, int wbcap, const uint32_t *__restrict__ cell_
                 // the item's mask block into shared memory (coalesced), then every lane walks its own column at its
                 // own pace (no per-word reconvergence): ~hits + words iterations instead of sum over words of the
                 // largest popcount of the warp
-                {
-                    const uint32_t *src = maskbuf + mask_off + lane;
-                    for (uint32_t w = 0; w < W; ++w) mblk[w * 32 + lane] = src[w * 32];
-                }
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
                 __syncwarp();
                 // one flat loop, byte addresses kept in registers: an iteration either fetches the lane's next mask
                 // word or emits one hit
