@@ -358,3 +358,27 @@ def test_gradient_through_several_rk_steps(sph):
     pe = np.abs(pg - po) / np.maximum(np.abs(po), 1e-3 * np.max(np.abs(po)) + 1e-30)
     print(f"{nsteps} steps: vjp errs {errs} params {np.max(pe):.2e}")
     assert max(errs.values()) < TOL_VJP and np.max(pe) < TOL_VJP
+
+
+def test_rhs_at_drifted_and_periodically_shifted_positions(sph):
+    """lists built at x with a skin; sph_rhs called at x' = x + drift (some particles cross a periodic face) and at
+    x' + k L (other periodic images): both must match the oracle evaluated at x' with its own exact lists"""
+    wl = W.perturbed(W.make(3, n_axis=24), amp_x=0.3, amp_rho=0.02)
+    skin = 0.1
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin) * np.float32(1.0001))
+    _, dev, _ = build(wl, 1.0 + skin, sph)
+    rng = np.random.default_rng(9)
+    H = float(wl.h.max())
+    drift = rng.uniform(-0.02 * H, 0.02 * H, size=wl.x.shape).astype(np.float32)
+    x1 = (wl.x + drift).astype(np.float32)                        # not wrapped: may leave the box
+    x2 = (x1 + rng.integers(-2, 3, size=wl.x.shape).astype(np.float32)).astype(np.float32)
+    import copy
+    wl1 = copy.copy(wl)
+    wl1.x = x1
+    rp_o, ci_o = oracle_lists(wl1)
+    d_o, a_o, sd, sa = oracle.rhs(wl.domain, wl.params, x1, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp_o, ci_o, with_scales=True)
+    for xx in (x1, x2):
+        drho, acc = sph.rhs(wl.params, torch.from_numpy(xx).cuda(), dev.v, dev.rho, dev.m, dev.kind)
+        # x2 = x1 + k is rounded to fp32 again: allow that rounding of the positions (1 ulp of 2 against dx/24)
+        tol = TOL_FWD if xx is x1 else 3e-4
+        assert max_norm_err(_np(drho), d_o, sd) < tol and max_norm_err(_np(acc), a_o, sa) < tol
