@@ -115,6 +115,19 @@ def density(domain, x, h, m, row_ptr, col_idx):
     return rho
 
 
+def density_vjp(domain, x, h, m, row_ptr, col_idx, rho_bar):
+    """(x_bar, m_bar) = J^T rho_bar of density() with the adjacency held fixed (Eq.21)"""
+    dim, per, lo, hi = _dom(domain)
+    x, h, m, rb = _d(x), _d(h), _d(m), _d(rho_bar)
+    n = x.shape[0]
+    xb = np.empty((n, dim), dtype=np.float64)
+    mb = np.empty(n, dtype=np.float64)
+    lib().orc_density_vjp(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(x), _p(h), _p(m),
+                          _p(np.ascontiguousarray(row_ptr, np.int64)), _p(np.ascontiguousarray(col_idx, np.int32)),
+                          _p(rb), _p(xb), _p(mb))
+    return xb, mb
+
+
 def rhs(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, rows=None, with_scales=False, par_raw=None):
     dim, per, lo, hi = _dom(domain)
     par = _par(params) if par_raw is None else par_raw

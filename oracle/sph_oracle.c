@@ -17,6 +17,8 @@
  *   orc_neighbors               : lattice counts 45 (2D,H=4dx) / 93 (3D,H=3dx), symmetry, brute vs grid,
  *                                 pure-Python brute force on tiny inputs
  *   orc_density                 : interior lattice 1.000415750 / 1.002898240, Riemann-sum argument
+ *   orc_density_vjp             : central finite differences of orc_density (x and m), sum x_bar = 0, two-particle
+ *                                 closed form, zero on a lattice with uniform rho_bar
  *   orc_rhs                     : momentum conservation, Galilean / rigid rotation invariance, uniform
  *                                 compression, Brookshaw Laplacian of |x|^2, hydrostatic column, viscous symbol
  *   orc_rhs_vjp                 : central finite differences of orc_rhs (x, v, rho, all 10 scalars),
@@ -320,6 +322,47 @@ void orc_density(int64_t n, int dim, const int *periodic, const double *lo, cons
             acc += m[j] * orc_w(r, H, dim);
         }
         rho_out[i] = acc;
+    }
+    free(xw);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * NEXT-1  Adjoint of the summation density: the paper's own backward benchmark differentiates the
+ *      summation density w.r.t. the particle positions, and the density-matching loss of PAPER.md:353
+ *      Eq.21 needs the same product.  Given rho_bar_i = dL/d rho_i, reverse mode of the loop of orc_density, term
+ *      by term, adjacency fixed, h not differentiated:
+ *          rho_i = sum_j m_j W(|x_i - x_j|, H_ij)
+ *          d rho_i = sum_j [ W_ij dm_j + m_j G_ij d_ij . (dx_i - dx_j) ],   grad_i W_ij = G_ij d_ij  (Eq.29)
+ *      =>  x_bar_i += rho_bar_i m_j G_ij d_ij,   x_bar_j -= rho_bar_i m_j G_ij d_ij,   m_bar_j += rho_bar_i W_ij.
+ *      Plain scatter, sequential (no threads): this is test infrastructure, obviously correct beats fast.
+ * ------------------------------------------------------------------------------------------ */
+void orc_density_vjp(int64_t n, int dim, const int *periodic, const double *lo, const double *hi,
+                     const double *x, const double *h, const double *m,
+                     const int64_t *row_ptr, const int32_t *col_idx, const double *rho_bar,
+                     double *x_bar, double *m_bar)
+{
+    double L[3];
+    box_len(dim, lo, hi, L);
+    double *xw = (double *)malloc((size_t)n * dim * sizeof(double));
+    wrap64(n, dim, periodic, lo, hi, x, xw);
+    for (int64_t i = 0; i < n * dim; ++i) x_bar[i] = 0.0;
+    for (int64_t i = 0; i < n; ++i) m_bar[i] = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
+            int64_t j = col_idx[p];
+            double d[3] = {0, 0, 0};
+            for (int k = 0; k < dim; ++k) d[k] = xw[i * dim + k] - xw[j * dim + k];
+            min_image(d, dim, periodic, L);
+            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            double H = h[i] > h[j] ? h[i] : h[j];
+            double G = orc_gfac(r, H, dim);
+            m_bar[j] += rho_bar[i] * orc_w(r, H, dim);
+            for (int k = 0; k < dim; ++k) {
+                double c = rho_bar[i] * m[j] * G * d[k];
+                x_bar[i * dim + k] += c;
+                x_bar[j * dim + k] -= c;
+            }
+        }
     }
     free(xw);
 }

@@ -186,6 +186,57 @@ def test_density_single_particle_and_two_particles():
     assert abs(rho[1] - (3.0 * oracle.w(0, H, 3) + 2.0 * oracle.w(r, H, 3))) < 1e-12
 
 
+# ------------------------------------------------------------------------------------------ density adjoint (NEXT-1)
+@pytest.mark.parametrize("cfg,kw", [(1, dict(n_axis=20)), (3, dict(n_axis=9)), (4, dict(n_axis=9)), (2, dict(dx=0.08))])
+def test_density_vjp_matches_central_differences_of_density(cfg, kw):
+    """the backward benchmark differentiates the summation density w.r.t. positions; adjacency fixed"""
+    wl = W.perturbed(W.make(cfg, **kw), amp_x=0.3, amp_rho=0.0)
+    rp, ci = oracle.neighbors(wl.domain, wl.x, wl.h)
+    rng = np.random.default_rng(42)
+    rb = rng.normal(size=wl.n)
+    x, m = wl.x.astype(np.float64), wl.m.astype(np.float64)
+    xb, mb = oracle.density_vjp(wl.domain, x, wl.h, m, rp, ci, rb)
+    L = lambda xx, mm: float(np.dot(rb, oracle.density(wl.domain, xx, wl.h, mm, rp, ci)))
+    zx, zm = rng.normal(size=x.shape), rng.normal(size=m.shape) * float(m.mean())
+    eps = 1e-6 * float(wl.h.min())
+    fd_x = (L(x + eps * zx, m) - L(x - eps * zx, m)) / (2 * eps)
+    fd_m = (L(x, m + 1e-3 * zm) - L(x, m - 1e-3 * zm)) / 2e-3          # linear in m: exact up to round-off
+    an_x, an_m = float(np.sum(xb * zx)), float(np.dot(mb, zm))
+    assert abs(fd_x - an_x) <= 1e-6 * max(abs(an_x), np.sum(np.abs(xb * zx)) * 1e-3)
+    assert abs(fd_m - an_m) <= 1e-9 * max(abs(an_m), np.sum(np.abs(mb * zm)))
+    # single components as well (a transposed or mis-signed operand would survive a random direction by luck only)
+    for i, k in ((0, 0), (wl.n // 2, wl.dim - 1)):
+        e = np.zeros_like(x)
+        e[i, k] = 1.0
+        fd = (L(x + eps * e, m) - L(x - eps * e, m)) / (2 * eps)
+        assert abs(fd - xb[i, k]) <= 1e-6 * max(abs(xb[i, k]), np.max(np.abs(xb)) * 1e-3)
+    # the density depends on position differences only
+    assert np.max(np.abs(xb.sum(0))) <= 1e-12 * np.sum(np.abs(xb))
+
+
+def test_density_vjp_two_particle_closed_form_and_lattice_symmetry():
+    dom = W.Domain(dim=3, periodic=(0, 0, 0), lo=(0.0,) * 3, hi=(1.0,) * 3, cell_size=0.5)
+    x = np.array([[0.5, 0.5, 0.5], [0.6, 0.52, 0.47]], dtype=np.float32)
+    h = np.array([0.3, 0.4], dtype=np.float32)
+    m = np.array([2.0, 3.0])
+    rb = np.array([0.7, -1.3])
+    rp, ci = oracle.neighbors(dom, x, h)
+    xb, mb = oracle.density_vjp(dom, x, h, m, rp, ci, rb)
+    d = x[0].astype(np.float64) - x[1].astype(np.float64)
+    r, H = float(np.linalg.norm(d)), float(np.float32(0.4))
+    G = oracle.gfac(r, H, 3)
+    want = (rb[0] * m[1] + rb[1] * m[0]) * G * d                  # both densities see the pair; grad_i W_ij = G d_ij
+    assert np.max(np.abs(xb[0] - want)) < 1e-12 * np.max(np.abs(want)) and np.max(np.abs(xb[1] + want)) < 1e-12 * np.max(np.abs(want))
+    assert abs(mb[0] - (rb[0] * oracle.w(0.0, float(np.float32(0.3)), 3) + rb[1] * oracle.w(r, H, 3))) < 1e-12
+    assert abs(mb[1] - (rb[1] * oracle.w(0.0, H, 3) + rb[0] * oracle.w(r, H, 3))) < 1e-12
+    # uniform cotangent on a periodic lattice: every pair contribution is cancelled by its mirror image
+    wl = W.make(0)
+    rp, ci = oracle.neighbors(wl.domain, wl.x, wl.h)
+    xb, _ = oracle.density_vjp(wl.domain, wl.x, wl.h, wl.m, rp, ci, np.ones(wl.n))
+    S = float(np.abs(oracle.gfac(0.03, float(wl.h[0]), 2)) * wl.m[0] * 0.03 * 45)
+    assert np.max(np.abs(xb)) < 1e-9 * S
+
+
 # ------------------------------------------------------------------------------------------ RHS
 def _lists(wl, method=1):
     return oracle.neighbors(wl.domain, wl.x, wl.h, method=method)
