@@ -342,6 +342,23 @@ def main():
     ms_max, pairs_all = reduce_over_ranks(ms_total, pairs_rank, dev)
     value = pairs_all / (ms_max * 1e-3)
 
+    # ---- NEXT-1 row, outside the timed step: adjoint of the summation density (the paper's
+    # own backward benchmark) on the exact-radius list of the current state
+    sph.build_cells(dom, x, h)
+    nnz_x = sph.neighbors(1.0)
+    rb_dev = lam                                          # any cotangent: reuse lambda ~ N(0,1)
+    xb_dev, mb_dev = torch.empty_like(x), torch.empty_like(rho)
+    sph.density_vjp(m, rb_dev, xb_dev, mb_dev)
+    e0, e1 = ev(), ev()
+    e0.record()
+    for _ in range(5):
+        sph.density_vjp(m, rb_dev, xb_dev, mb_dev)
+    e1.record()
+    torch.cuda.synchronize()
+    dvjp_ms = e0.elapsed_time(e1) / 5.0
+    extras = {"density_vjp": {"ms": dvjp_ms, "pair_interactions_per_s": nnz_x / (dvjp_ms * 1e-3), "nnz": int(nnz_x),
+                              "note": "sph_density_vjp (x_bar and m_bar), not part of the timed step"}}
+
     # ---- e2e: the same step through sph_step_host with pinned host buffers, copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -427,7 +444,7 @@ def main():
             "hbm_frac_fwd_bwd_of_8TBs": fb_bytes / (fb_ms * 1e-3) / 1e9 / 8000.0,
             "phase_ms": ph_ms, "kernels": kern,
             "roofline": roof[dom_cls], "roofline_all": roof,
-            "gpu_launches": int(launches), "clocks": clk,
+            "gpu_launches": int(launches), "clocks": clk, "next_rows": extras,
         }
         if e2e:
             line["e2e"] = e2e

@@ -97,6 +97,14 @@ int sph_neighbors_export(sph_ctx *ctx, int64_t *row_ptr, int32_t *col_idx, sph_s
 /* rho_i = sum_{j in N(i)} m_j W(r_ij, max(h_i,h_j)) at the positions given to sph_build_cells.  PAPER.md:91 Eq.8 */
 int sph_density(sph_ctx *ctx, const float *m, float *rho_out, sph_stream_t stream);
 
+/* Reverse-mode adjoint of sph_density (the paper's backward benchmark differentiates the
+ * summation density w.r.t. the positions; density-matching loss PAPER.md:353 Eq.21): given
+ * rho_bar = dL/d rho [n], writes x_bar [n][dim] = sum_j (rho_bar_i m_j + rho_bar_j m_i) G_ij (x_i - x_j) and, if
+ * m_bar is not NULL, m_bar [n] = sum_j rho_bar_j W_ij, at the positions given to sph_build_cells, adjacency fixed
+ * (PAPER.md:161), h not differentiated.  Gather form over the symmetric lists: no atomics. */
+int sph_density_vjp(sph_ctx *ctx, const float *m, const float *rho_bar, float *x_bar, float *m_bar,
+                    sph_stream_t stream);
+
 /* One right-hand-side evaluation (formulas at the top of this file) on the lists of the last sph_neighbors.
  * x may differ from the build positions (RK stages) as long as the list is still a superset of the true
  * neighbours: pairs with r >= H_ij contribute exactly 0 (kernel clamp).  h is the one given to sph_build_cells. */

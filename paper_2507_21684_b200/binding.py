@@ -16,6 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsph_b200.so")
 
 EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph_neighbors_export", "sph_density",
+           "sph_density_vjp",
            "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
            "sph_check", "sph_strerror", "sph_get_info", "sph_get_layout", "sph_profile_enable", "sph_profile_read",
            "sph_set_option")
@@ -65,6 +66,7 @@ def load_library(path: str = LIB_PATH):
     lib.sph_neighbors.argtypes = [vp, f32, C.POINTER(i64), vp]
     lib.sph_neighbors_export.argtypes = [vp, vp, vp, vp]
     lib.sph_density.argtypes = [vp, vp, vp, vp]
+    lib.sph_density_vjp.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.sph_rhs.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 7 + [vp]
     lib.sph_rhs_vjp.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 11 + [vp]
     lib.sph_rk_step.argtypes = [vp, C.POINTER(SphDomain), C.POINTER(SphParams), f32, f32, i64] + [vp] * 6 + [vp]
@@ -178,6 +180,17 @@ class Sph:
         out = torch.empty_like(m) if out is None else out
         self._chk(self.lib.sph_density(self._ctx, _ptr(m), _ptr(out), _stream()))
         return out
+
+    def density_vjp(self, m, rho_bar, x_bar=None, m_bar=None, want_m_bar=True):
+        """(x_bar, m_bar) = J^T rho_bar of density() at the build positions"""
+        import torch
+        m, rho_bar = _f32(m, (self.n,)), _f32(rho_bar, (self.n,))
+        x_bar = torch.empty((self.n, self.dim), dtype=torch.float32, device=m.device) if x_bar is None else _f32(x_bar, (self.n, self.dim))
+        if m_bar is None and want_m_bar:
+            m_bar = torch.empty(self.n, dtype=torch.float32, device=m.device)
+        self._chk(self.lib.sph_density_vjp(self._ctx, _ptr(m), _ptr(rho_bar), _ptr(x_bar),
+                                           _ptr(m_bar) if m_bar is not None else None, _stream()))
+        return x_bar, m_bar
 
     def rhs(self, params, x, v, rho, m, kind, drho_dt=None, acc=None):
         p = make_params(params)

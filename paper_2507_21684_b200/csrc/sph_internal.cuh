@@ -279,6 +279,8 @@ __device__ __forceinline__ int cell_coord_raw(double x, double lo, double edge)
 // host-side launch helpers implemented in the .cu files
 int sph_tile_expand_col(sph_ctx *ctx, cudaStream_t st);   // tile-local lists -> 32-bit sorted ids in ctx->col
 int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, float *rho_out, cudaStream_t st);
+int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s, float *x_bar, float *m_bar,
+                                cudaStream_t st);
 int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
                         const uint8_t *kind_s, float *drho, float *acc, float4 *out4, cudaStream_t st);
 int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,

@@ -181,6 +181,71 @@ k_density(int64_t n, KPar kp, float margin, const float4 *__restrict__ pos_s, co
     }
 }
 
+// ------------------------------------------------------------------------------------------ D^T: density adjoint
+// x_bar_i = sum_j (rb_i m_j + rb_j m_i) G_ij d_ij,  m_bar_i = sum_j rb_j W_ij   (include/sph.h sph_density_vjp)
+__global__ void k_gather_f32x2(int64_t n, const uint32_t *__restrict__ perm, const float *__restrict__ a,
+                               const float *__restrict__ b, float2 *__restrict__ out)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n) {
+        const int64_t i = perm[p];
+        out[p] = make_float2(a[i], b[i]);
+    }
+}
+
+template <int DIM, int GS, bool VARH>
+__global__ void __launch_bounds__(kBlock)
+k_density_vjp(int64_t n, KPar kp, float margin, const float4 *__restrict__ pos_s, const float2 *__restrict__ mr_s,
+              const long long *__restrict__ row_ptr, const int32_t *__restrict__ col, const uint32_t *__restrict__ perm,
+              float *__restrict__ xb_out, float *__restrict__ mb_out)
+{
+    constexpr int kGroups = kBlock / GS;
+    const int g = threadIdx.x / GS, gl = threadIdx.x % GS;
+    const int64_t row0 = (int64_t)blockIdx.x * kGroups * kRowsPerGroup;
+    const HC hu = hc_uniform<DIM>(kp);
+    for (int rr = 0; rr < kRowsPerGroup; ++rr) {
+        const int64_t row = row0 + (int64_t)rr * kGroups + g;
+        if (row >= n) break;
+        const float4 pi = __ldg(pos_s + row);
+        const float2 ai = __ldg(mr_s + row);                  // {m_i, rho_bar_i}
+        const float xi[3] = {pi.x, pi.y, pi.z};
+        const bool seam = row_near_seam(xi, kp, margin);
+        const long long b = row_ptr[row], e = row_ptr[row + 1];
+        float x0 = 0.f, x1 = 0.f, x2 = 0.f, mb = 0.f;
+        for (long long p = b + gl; p < e; p += GS) {
+            const int32_t j = __ldg(col + p);
+            const float4 pj = __ldg(pos_s + j);
+            const float2 aj = __ldg(mr_s + j);
+            const float xj[3] = {pj.x, pj.y, pj.z};
+            float d[3], r2;
+            if (seam) rel_pos<DIM, true>(xi, xj, kp, d, r2); else rel_pos<DIM, false>(xi, xj, kp, d, r2);
+            HC hc = hu;
+            if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+            const float q = fast_sqrt(r2) * hc.invH;
+            const float t = fmaxf(1.0f - q, 0.f);
+            const float t2 = t * t, t4 = t2 * t2;
+            const float G = hc.cG * fmaf(5.0f, q, 1.0f) * (t4 * t);                               // Eq.29
+            const float w = hc.cW * (t4 * t2) * fmaf(q, fmaf(q, 35.0f / 3.0f, 6.0f), 1.0f);       // Eq.25/27
+            const float c = fmaf(ai.y, aj.x, aj.y * ai.x) * G;
+            x0 = fmaf(c, d[0], x0);
+            x1 = fmaf(c, d[1], x1);
+            if (DIM == 3) x2 = fmaf(c, d[2], x2);
+            mb = fmaf(aj.y, w, mb);
+        }
+        x0 = group_sum<GS>(x0);
+        x1 = group_sum<GS>(x1);
+        if (DIM == 3) x2 = group_sum<GS>(x2);
+        mb = group_sum<GS>(mb);
+        if (gl == 0) {
+            const int64_t i = perm[row];
+            xb_out[i * DIM] = x0;
+            xb_out[i * DIM + 1] = x1;
+            if (DIM == 3) xb_out[i * DIM + 2] = x2;
+            if (mb_out) mb_out[i] = mb;
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------ R1: RHS
 // OUT_SORTED: write float4 {a, drho/dt} in sorted order (RK stages); else scatter to the caller's arrays.
 template <int DIM, int GS, bool VARH, bool OUT_SORTED>
@@ -623,6 +688,36 @@ extern "C" int sph_density(sph_ctx *ctx, const float *m, float *rho_out, sph_str
     if (kp.dim == 3) { if (kp.uniform_h) SPH_DENS_LAUNCH(3, 32, false); else SPH_DENS_LAUNCH(3, 32, true); }
     else { if (kp.uniform_h) SPH_DENS_LAUNCH(2, 16, false); else SPH_DENS_LAUNCH(2, 16, true); }
 #undef SPH_DENS_LAUNCH
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+extern "C" int sph_density_vjp(sph_ctx *ctx, const float *m, const float *rho_bar, float *x_bar, float *m_bar,
+                               sph_stream_t stream)
+{
+    if (!ctx || !m || !rho_bar || !x_bar) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    const int64_t n = ctx->n;
+    sph_params dummy{};
+    dummy.c0 = 1.f; dummy.rho0 = 1.f; dummy.gamma = 1.f; dummy.eps = 1.f;
+    KPar kp;
+    SPH_TRY(sph_kpar_make(ctx, &dummy, &kp));
+    SPH_TRY(ctx->s2.reserve((size_t)n * 8));
+    float2 *mr_s = ctx->s2.as<float2>();
+    KScope ks(ctx, SPH_K_DENSITY, 2, st);
+    k_gather_f32x2<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), m, rho_bar, mr_s);
+    if (ctx->tile_mode) return sph_launch_density_vjp_tile(ctx, kp, mr_s, x_bar, m_bar, st);
+    const float margin = seam_margin(ctx);
+#define SPH_DVJP_LAUNCH(DIM, GS, VARH)                                                                                 \
+    k_density_vjp<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), mr_s,    \
+                                                                     ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>(), \
+                                                                     ctx->perm.as<uint32_t>(), x_bar, m_bar)
+    if (kp.dim == 3) { if (kp.uniform_h) SPH_DVJP_LAUNCH(3, 32, false); else SPH_DVJP_LAUNCH(3, 32, true); }
+    else { if (kp.uniform_h) SPH_DVJP_LAUNCH(2, 16, false); else SPH_DVJP_LAUNCH(2, 16, true); }
+#undef SPH_DVJP_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

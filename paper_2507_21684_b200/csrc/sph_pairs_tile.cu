@@ -248,6 +248,72 @@ k_density_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ po
         });
 }
 
+// ------------------------------------------------------------------------------------------ D^T: density adjoint
+// x_bar_i = sum_j (rb_i m_j + rb_j m_i) G_ij d_ij,  m_bar_i = sum_j rb_j W_ij   (include/sph.h sph_density_vjp;
+// PAPER.md:242, 353 Eq.21).  smem: A = {x,y,z,h}[mcap], MR = {m, rho_bar}[mcap] (in the B slot), rp, selfq, ring
+template <int DIM, int GS, bool VARH>
+__global__ void __launch_bounds__(kPtMaxWarps * 32)
+k_density_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ pos_s, const float2 *__restrict__ mr_s,
+                   const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
+                   const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16,
+                   const uint32_t *__restrict__ perm, float *__restrict__ xb_out, float *__restrict__ mb_out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const SmemMap<DIM> sm(smem_raw, ts, false);
+    float2 *MR = reinterpret_cast<float2 *>(sm.B);
+    __shared__ TileTab tt;
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (tt.T == 0) return;
+    stage_halo(tt, pos_s, sm.A, nullptr, nullptr, nullptr, nullptr, mr_s, MR, nullptr, nullptr);
+    stage_rows(tt, row_ptr, sm.rp, sm.selfq);
+    cp_async_wait<0>();
+    __syncthreads();
+    stage_shift<DIM>(tt, sm.A);
+    const int gl = (threadIdx.x & 31) % GS;
+    const HC hu = hc_uniform<DIM>(kp);
+    const float4 *A = sm.A;
+    const uint16_t *selfq = sm.selfq;
+    const uint32_t row0 = tt.row0;
+    tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
+        [&](uint32_t r, bool live, uint32_t b, uint32_t e, const uint16_t *idx) {
+            const uint32_t qi = selfq[r];
+            const float4 pi = A[qi];
+            const float2 ai = MR[qi];                          // {m_i, rho_bar_i}
+            float x0 = 0.f, x1 = 0.f, x2 = 0.f, mb = 0.f;
+#pragma unroll 2
+            for (uint32_t k = b + gl; k < e; k += GS) {
+                const uint32_t j = idx[k];
+                const float4 pj = A[j];
+                const float2 aj = MR[j];
+                const float d0 = pi.x - pj.x, d1 = pi.y - pj.y, d2 = DIM == 3 ? pi.z - pj.z : 0.f;
+                const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
+                HC hc = hu;
+                if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+                const float q = fast_sqrt(r2) * hc.invH;
+                const float t = fmaxf(1.0f - q, 0.f);
+                const float t2 = t * t, t4 = t2 * t2;
+                const float G = hc.cG * fmaf(5.0f, q, 1.0f) * (t4 * t);                             // Eq.29
+                const float w = hc.cW * (t4 * t2) * fmaf(q, fmaf(q, 35.0f / 3.0f, 6.0f), 1.0f);     // Eq.25/27
+                const float c = fmaf(ai.y, aj.x, aj.y * ai.x) * G;
+                x0 = fmaf(c, d0, x0);
+                x1 = fmaf(c, d1, x1);
+                if (DIM == 3) x2 = fmaf(c, d2, x2);
+                mb = fmaf(aj.y, w, mb);
+            }
+            x0 = group_sum<GS>(x0);
+            x1 = group_sum<GS>(x1);
+            if (DIM == 3) x2 = group_sum<GS>(x2);
+            mb = group_sum<GS>(mb);
+            if (gl == 0 && live) {
+                const int64_t i = perm[row0 + r];
+                xb_out[i * DIM] = x0;
+                xb_out[i * DIM + 1] = x1;
+                if (DIM == 3) xb_out[i * DIM + 2] = x2;
+                if (mb_out) mb_out[i] = mb;
+            }
+        });
+}
+
 // ------------------------------------------------------------------------------------------ R1: RHS
 // OUT_SORTED: write float4 {a, drho/dt} in sorted order (RK stages); else scatter to the caller's arrays.
 template <int DIM, int GS, bool VARH, bool OUT_SORTED>
@@ -589,6 +655,38 @@ int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, floa
     }
 #undef SPH_DT_GS
 #undef SPH_DT_LAUNCH
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s, float *x_bar, float *m_bar,
+                                cudaStream_t st)
+{
+    const TileGeom &tg = ctx->tg;
+    const int gs = tile_group(ctx, false);
+    int threads;
+    TileSizes ts;
+    size_t smem;
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);   // carve-up of SmemMap
+#define SPH_DVT_LAUNCH(DIM, GS, VARH)                                                                                 \
+    do {                                                                                                              \
+        SPH_TILE_SMEM_ATTR((k_density_vjp_tile<DIM, GS, VARH>), smem);                                                \
+        k_density_vjp_tile<DIM, GS, VARH><<<(unsigned)tg.ntiles, threads, smem, st>>>(                                \
+            tg, kp, ts, ctx->pos_s.as<float4>(), mr_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),  \
+            ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), x_bar, m_bar);         \
+    } while (0)
+#define SPH_DVT_GS(GS)                                                                                      \
+    do {                                                                                                    \
+        if (kp.dim == 3) { if (kp.uniform_h) SPH_DVT_LAUNCH(3, GS, false); else SPH_DVT_LAUNCH(3, GS, true); } \
+        else { if (kp.uniform_h) SPH_DVT_LAUNCH(2, GS, false); else SPH_DVT_LAUNCH(2, GS, true); }             \
+    } while (0)
+    switch (gs) {
+    case 16: SPH_DVT_GS(16); break;
+    case 32: SPH_DVT_GS(32); break;
+    default: SPH_DVT_GS(8); break;
+    }
+#undef SPH_DVT_GS
+#undef SPH_DVT_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

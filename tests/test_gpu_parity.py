@@ -149,6 +149,21 @@ def test_density_parity(sph, case):
 
 
 @pytest.mark.parametrize("case", list(CASES))
+def test_density_vjp_parity(sph, case):
+    """adjoint of the summation density w.r.t. positions and masses (Eq.21)"""
+    wl = CASES[case]()
+    _, dev, _ = build(wl, 1.0, sph)
+    rb = np.random.default_rng(wl.seed + 77).normal(size=wl.n).astype(np.float32)
+    xb, mb = sph.density_vjp(dev.m, torch.from_numpy(rb).cuda())
+    xo, mo = oracle.density_vjp(wl.domain, wl.x, wl.h, wl.m, *oracle_lists(wl), rb)
+    ex, em = max_norm_err(_np(xb), xo), max_norm_err(_np(mb), mo)
+    print(f"{case}: density vjp err x {ex:.2e} m {em:.2e}")
+    assert ex < TOL_VJP and em < TOL_VJP
+    xb2, _ = sph.density_vjp(dev.m, torch.from_numpy(rb).cuda(), want_m_bar=False)      # m_bar is optional
+    assert torch.equal(xb, xb2)
+
+
+@pytest.mark.parametrize("case", list(CASES))
 def test_rhs_parity(sph, case):
     wl = CASES[case]()
     _, dev, _ = build(wl, 1.0, sph)
