@@ -397,3 +397,54 @@ def test_rhs_at_drifted_and_periodically_shifted_positions(sph):
         # x2 = x1 + k is rounded to fp32 again: allow that rounding of the positions (1 ulp of 2 against dx/24)
         tol = TOL_FWD if xx is x1 else 3e-4
         assert max_norm_err(_np(drho), d_o, sd) < tol and max_norm_err(_np(acc), a_o, sa) < tol
+
+
+def test_color_field_loss_gradient_by_chaining_density_and_density_vjp(sph):
+    """The naive particle-shifting loss of the paper, Eq.23: L = 1/n sum_i (1 - sum_j m_j/rho_j W_ij)^2
+    with rho the summation density, on n = 32^2 equal-mass particles sampled uniformly at random in [-1,1]^2
+    (a synthetic stand-in drawn here from a seed).  The colour field is a summation density with the
+    "masses" m_j/rho_j, so its position gradient is a chain of the built calls:
+        rho = D(x; m), m' = m/rho, c = D(x; m'), L = mean((1-c)^2)
+        c_bar = -2 (1-c)/n, (x1, m'_bar) = D^T(x; m', c_bar), rho_bar = -m'_bar m/rho^2, (x2, .) = D^T(x; m, rho_bar)
+    compared with the same chain in the fp64 oracle; one descent step must lower the loss."""
+    rng = np.random.default_rng(2024)
+    n_axis = 32
+    n = n_axis * n_axis
+    dx = 2.0 / n_axis
+    x = rng.uniform(-1.0, 1.0, size=(n, 2)).astype(np.float32)
+    h = np.full(n, 4.0 * dx, np.float32)
+    m = np.full(n, dx * dx, np.float32)
+    dom = W.Domain(dim=2, periodic=(1, 1, 0), lo=(-1.0, -1.0, 0.0), hi=(1.0, 1.0, 0.0), cell_size=float(4.0 * dx))
+    wl = W.Workload(name="shift", domain=dom, params=W.make(0).params, x=x, v=0 * x, rho=np.ones(n, np.float32), m=m, h=h,
+                    kind=np.zeros(n, np.uint8), dt=0.0, dx=dx, seed=0)
+
+    def gpu_loss_and_grad(xh):
+        wl.x = xh
+        _, dev, _ = build(wl, 1.0, sph)
+        rho = sph.density(dev.m)
+        mp = dev.m / rho
+        c = sph.density(mp)
+        L = float(((1.0 - c.double()) ** 2).mean())
+        c_bar = (-2.0 * (1.0 - c) / n).contiguous()
+        x1, mp_bar = sph.density_vjp(mp, c_bar)
+        rho_bar = (-mp_bar * dev.m / (rho * rho)).contiguous()
+        x2, _ = sph.density_vjp(dev.m, rho_bar, want_m_bar=False)
+        return L, _np(x1 + x2)
+
+    L0, g = gpu_loss_and_grad(x)
+    lists = oracle_lists(wl)
+    x64, m64 = x.astype(np.float64), m.astype(np.float64)
+    rho_o = oracle.density(dom, x64, h, m64, *lists)
+    mp_o = m64 / rho_o
+    c_o = oracle.density(dom, x64, h, mp_o, *lists)
+    L_o = float(np.mean((1.0 - c_o) ** 2))
+    x1_o, mpb_o = oracle.density_vjp(dom, x64, h, mp_o, *lists, -2.0 * (1.0 - c_o) / n)
+    x2_o, _ = oracle.density_vjp(dom, x64, h, m64, *lists, -mpb_o * m64 / rho_o ** 2)
+    g_o = x1_o + x2_o
+    assert abs(L0 - L_o) <= 1e-4 * L_o
+    assert max_norm_err(g, g_o) < TOL_VJP
+    # a small step against the gradient lowers the loss (step sized to move particles by at most 0.05 dx)
+    step = 0.05 * dx / float(np.max(np.abs(g)))
+    L1, _ = gpu_loss_and_grad((x - step * g).astype(np.float32))
+    print(f"colour-field loss {L0:.5e} -> {L1:.5e}, gradient err {max_norm_err(g, g_o):.2e}")
+    assert L1 < L0
