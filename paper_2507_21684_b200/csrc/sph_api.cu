@@ -40,6 +40,9 @@ extern "C" int sph_destroy(sph_ctx *ctx)
     for (DevBuf *b : bufs) b->release();
     for (auto &b : ctx->rk) b.release();
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    if (ctx->ev_in) cudaEventDestroy(ctx->ev_in);
+    if (ctx->ev_out) cudaEventDestroy(ctx->ev_out);
     for (const ProfRec &r : ctx->prof.live) {
         cudaEventDestroy(r.a);
         cudaEventDestroy(r.b);
@@ -159,28 +162,41 @@ extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_doma
     float *dx = ctx->hx.as<float>(), *dv = ctx->hv.as<float>(), *dr = ctx->hrho.as<float>(), *dm = ctx->hm.as<float>();
     float *dh = ctx->hh.as<float>();
     uint8_t *dk = ctx->hkind.as<uint8_t>();
+    // Copies off the critical path run on a second (non-blocking) stream: the cotangents and v, rho, m, kind arrive while
+    // the cells and lists are built from x and h; the seven results of the first half leave while sph_rk_step runs.
+    if (!ctx->copy_stream) {
+        SPH_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        SPH_CUDA_TRY(cudaEventCreateWithFlags(&ctx->ev_in, cudaEventDisableTiming));
+        SPH_CUDA_TRY(cudaEventCreateWithFlags(&ctx->ev_out, cudaEventDisableTiming));
+    }
+    cudaStream_t cs = ctx->copy_stream;
+    SPH_CUDA_TRY(cudaStreamSynchronize(st));                      // the staging buffers of the previous call are free
     SPH_CUDA_TRY(cudaMemcpyAsync(dx, x, nv, cudaMemcpyHostToDevice, st));
-    SPH_CUDA_TRY(cudaMemcpyAsync(dv, v, nv, cudaMemcpyHostToDevice, st));
-    SPH_CUDA_TRY(cudaMemcpyAsync(dr, rho, ns, cudaMemcpyHostToDevice, st));
-    SPH_CUDA_TRY(cudaMemcpyAsync(dm, m, ns, cudaMemcpyHostToDevice, st));
     SPH_CUDA_TRY(cudaMemcpyAsync(dh, h, ns, cudaMemcpyHostToDevice, st));
-    SPH_CUDA_TRY(cudaMemcpyAsync(dk, kind, (size_t)n, cudaMemcpyHostToDevice, st));
-    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hlam.p, drho_bar, ns, cudaMemcpyHostToDevice, st));
-    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hmu.p, acc_bar, nv, cudaMemcpyHostToDevice, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(dm, m, ns, cudaMemcpyHostToDevice, cs));
+    SPH_CUDA_TRY(cudaMemcpyAsync(dv, v, nv, cudaMemcpyHostToDevice, cs));
+    SPH_CUDA_TRY(cudaMemcpyAsync(dr, rho, ns, cudaMemcpyHostToDevice, cs));
+    SPH_CUDA_TRY(cudaMemcpyAsync(dk, kind, (size_t)n, cudaMemcpyHostToDevice, cs));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hlam.p, drho_bar, ns, cudaMemcpyHostToDevice, cs));
+    SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hmu.p, acc_bar, nv, cudaMemcpyHostToDevice, cs));
+    SPH_CUDA_TRY(cudaEventRecord(ctx->ev_in, cs));
     int64_t nnz0 = 0;
     SPH_TRY(sph_build_cells(ctx, dom, dx, dh, n, ss));
     SPH_TRY(sph_neighbors(ctx, 1.0f, &nnz0, ss));
+    SPH_CUDA_TRY(cudaStreamWaitEvent(st, ctx->ev_in, 0));
     SPH_TRY(sph_density(ctx, dm, ctx->ho_dens.as<float>(), ss));
     SPH_TRY(sph_rhs(ctx, par, dx, dv, dr, dm, dk, ctx->ho_drho.as<float>(), ctx->ho_acc.as<float>(), ss));
     SPH_TRY(sph_rhs_vjp(ctx, par, dx, dv, dr, dm, dk, ctx->hlam.as<float>(), ctx->hmu.as<float>(), ctx->ho_xb.as<float>(),
                         ctx->ho_vb.as<float>(), ctx->ho_rb.as<float>(), ctx->ho_pb.as<float>(), ss));
-    if (density) SPH_CUDA_TRY(cudaMemcpyAsync(density, ctx->ho_dens.p, ns, cudaMemcpyDeviceToHost, st));
-    if (drho_dt) SPH_CUDA_TRY(cudaMemcpyAsync(drho_dt, ctx->ho_drho.p, ns, cudaMemcpyDeviceToHost, st));
-    if (acc) SPH_CUDA_TRY(cudaMemcpyAsync(acc, ctx->ho_acc.p, nv, cudaMemcpyDeviceToHost, st));
-    if (x_bar) SPH_CUDA_TRY(cudaMemcpyAsync(x_bar, ctx->ho_xb.p, nv, cudaMemcpyDeviceToHost, st));
-    if (v_bar) SPH_CUDA_TRY(cudaMemcpyAsync(v_bar, ctx->ho_vb.p, nv, cudaMemcpyDeviceToHost, st));
-    if (rho_bar) SPH_CUDA_TRY(cudaMemcpyAsync(rho_bar, ctx->ho_rb.p, ns, cudaMemcpyDeviceToHost, st));
-    if (params_bar) SPH_CUDA_TRY(cudaMemcpyAsync(params_bar, ctx->ho_pb.p, 40, cudaMemcpyDeviceToHost, st));
+    SPH_CUDA_TRY(cudaEventRecord(ctx->ev_out, st));
+    SPH_CUDA_TRY(cudaStreamWaitEvent(cs, ctx->ev_out, 0));
+    if (density) SPH_CUDA_TRY(cudaMemcpyAsync(density, ctx->ho_dens.p, ns, cudaMemcpyDeviceToHost, cs));
+    if (drho_dt) SPH_CUDA_TRY(cudaMemcpyAsync(drho_dt, ctx->ho_drho.p, ns, cudaMemcpyDeviceToHost, cs));
+    if (acc) SPH_CUDA_TRY(cudaMemcpyAsync(acc, ctx->ho_acc.p, nv, cudaMemcpyDeviceToHost, cs));
+    if (x_bar) SPH_CUDA_TRY(cudaMemcpyAsync(x_bar, ctx->ho_xb.p, nv, cudaMemcpyDeviceToHost, cs));
+    if (v_bar) SPH_CUDA_TRY(cudaMemcpyAsync(v_bar, ctx->ho_vb.p, nv, cudaMemcpyDeviceToHost, cs));
+    if (rho_bar) SPH_CUDA_TRY(cudaMemcpyAsync(rho_bar, ctx->ho_rb.p, ns, cudaMemcpyDeviceToHost, cs));
+    if (params_bar) SPH_CUDA_TRY(cudaMemcpyAsync(params_bar, ctx->ho_pb.p, 40, cudaMemcpyDeviceToHost, cs));
     SPH_TRY(sph_rk_step(ctx, dom_rk, par, dt, skin, n, dx, dv, dr, dm, dh, dk, ss));
     if (nnz_out) {
         nnz_out[0] = nnz0;
@@ -190,6 +206,7 @@ extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_doma
     SPH_CUDA_TRY(cudaMemcpyAsync(v, dv, nv, cudaMemcpyDeviceToHost, st));
     SPH_CUDA_TRY(cudaMemcpyAsync(rho, dr, ns, cudaMemcpyDeviceToHost, st));
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
+    SPH_CUDA_TRY(cudaStreamSynchronize(cs));
     return SPH_OK;
 }
 

@@ -157,6 +157,9 @@ struct sph_ctx {
     DevBuf rk[16];
     // pinned host mirror
     int64_t *h_pinned = nullptr; // [16]
+    // sph_step_host: copies that are not on the critical path run on their own stream
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_in = nullptr, ev_out = nullptr;
     // host staging for *_host call
     DevBuf hx, hv, hrho, hm, hh, hkind, hlam, hmu, ho_drho, ho_acc, ho_xb, ho_vb, ho_rb, ho_pb, ho_dens;
 };

@@ -448,3 +448,33 @@ def test_color_field_loss_gradient_by_chaining_density_and_density_vjp(sph):
     L1, _ = gpu_loss_and_grad((x - step * g).astype(np.float32))
     print(f"colour-field loss {L0:.5e} -> {L1:.5e}, gradient err {max_norm_err(g, g_o):.2e}")
     assert L1 < L0
+
+
+def test_step_host_matches_the_device_calls(sph):
+    """sph_step_host (the e2e leg of bench.py; its copies overlap the compute on a second stream) returns exactly what
+    the same sequence of device calls returns"""
+    import bench
+    wl = CASES["C3p"]()
+    lam, mu = W.random_cotangents(wl)
+    dom_rk = bench.rk_domain(wl)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    hx, hv, hr = pin(wl.x.copy()), pin(wl.v.copy()), pin(wl.rho.copy())
+    outs = {"density": pin(np.empty(wl.n, np.float32)), "drho_dt": pin(np.empty(wl.n, np.float32)),
+            "acc": pin(np.empty((wl.n, 3), np.float32)), "x_bar": pin(np.empty((wl.n, 3), np.float32)),
+            "v_bar": pin(np.empty((wl.n, 3), np.float32)), "rho_bar": pin(np.empty(wl.n, np.float32)),
+            "params_bar": pin(np.empty(10, np.float32))}
+    for _ in range(2):                                    # twice: the second call reuses the staging buffers
+        hx.copy_(torch.from_numpy(wl.x)); hv.copy_(torch.from_numpy(wl.v)); hr.copy_(torch.from_numpy(wl.rho))
+        sph.step_host(wl.domain, dom_rk, wl.params, wl.dt, bench.SKIN, hx, hv, hr, pin(wl.m), pin(wl.h), pin(wl.kind),
+                      pin(lam), pin(mu), outs)
+    _, dev, _ = build(wl, 1.0, sph)
+    dens = sph.density(dev.m)
+    drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+    xb, vb, rb, pb = sph.rhs_vjp(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind, torch.from_numpy(lam).cuda(),
+                                 torch.from_numpy(mu).cuda())
+    x, v, rho = dev.x.clone(), dev.v.clone(), dev.rho.clone()
+    sph.rk_step(dom_rk, wl.params, wl.dt, bench.SKIN, x, v, rho, dev.m, dev.h, dev.kind)
+    for name, t in (("density", dens), ("drho_dt", drho), ("acc", acc), ("x_bar", xb), ("v_bar", vb), ("rho_bar", rb),
+                    ("params_bar", pb)):
+        assert np.array_equal(outs[name].numpy(), _np(t)), name
+    assert np.array_equal(hx.numpy(), _np(x)) and np.array_equal(hv.numpy(), _np(v)) and np.array_equal(hr.numpy(), _np(rho))
