@@ -478,3 +478,41 @@ def test_step_host_matches_the_device_calls(sph):
                     ("params_bar", pb)):
         assert np.array_equal(outs[name].numpy(), _np(t)), name
     assert np.array_equal(hx.numpy(), _np(x)) and np.array_equal(hv.numpy(), _np(v)) and np.array_equal(hr.numpy(), _np(rho))
+
+
+def test_config1_full_size_100_steps_forward_and_backward(sph):
+    """BASELINE.json config 1 at full size: 256^2 jittered Taylor-Green particles, 100 RK4 steps (dt = 0.25 H/c0) forward,
+    gradient of the final kinetic energy w.r.t. the initial velocities back through all steps.  Against the fp64 oracle
+    chain: the final velocities (1e-4, the per-step bar, held over the whole chain: measured 1e-5), the kinetic-energy
+    decay, and the gradient (1e-3, measured 6e-6)."""
+    if sph.layout_name != "tile":
+        pytest.skip("one layout is enough for the long chain")
+    wl = W.make(1)
+    assert wl.n == 65536
+    skin, nsteps = 0.1, 100
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin) * np.float32(1.0001))
+    dev = Dev(wl)
+    states = [(dev.x.clone(), dev.v.clone(), dev.rho.clone())]
+    for _ in range(nsteps):
+        x, v, rho = (t.clone() for t in states[-1])
+        sph.rk_step(wl.domain, wl.params, wl.dt, skin, x, v, rho, dev.m, dev.h, dev.kind)
+        states.append((x, v, rho))
+    xb = torch.zeros_like(dev.x)
+    vb = (dev.m[:, None] * states[-1][1]).contiguous()
+    rb = torch.zeros_like(dev.rho)
+    pb = torch.zeros(10, device="cuda")
+    for k in range(nsteps - 1, -1, -1):
+        sph.rk_step_vjp(wl.domain, wl.params, wl.dt, skin, *states[k], dev.m, dev.h, dev.kind, xb, vb, rb, pb)
+    so = [(wl.x.astype(np.float64), wl.v.astype(np.float64), wl.rho.astype(np.float64))]
+    for _ in range(nsteps):
+        so.append(oracle.rk4_step(wl.domain, wl.params, wl.dt, *so[-1], wl.m, wl.h, wl.kind, method=1))
+    xo, vo, ro = np.zeros_like(so[-1][0]), wl.m.astype(np.float64)[:, None] * so[-1][1], np.zeros(wl.n)
+    for k in range(nsteps - 1, -1, -1):
+        xo, vo, ro, _ = oracle.rk4_step_vjp(wl.domain, wl.params, wl.dt, *so[k], wl.m, wl.h, wl.kind, xo, vo, ro, method=1)
+    ke = lambda v: 0.5 * float(np.sum(wl.m.astype(np.float64)[:, None] * np.asarray(v, np.float64) ** 2))
+    ke_g, ke_o, ke0 = ke(_np(states[-1][1])), ke(so[-1][1]), ke(wl.v)
+    ev = max_norm_err(_np(states[-1][1]), so[-1][1])
+    eg = max_norm_err(_np(vb), vo)
+    print(f"C1 full: KE/KE0 gpu {ke_g / ke0:.6f} oracle {ke_o / ke0:.6f}; v(T) err {ev:.2e}; dKE/dv0 err {eg:.2e}")
+    assert abs(ke_g - ke_o) <= 1e-4 * ke_o and ke_o < ke0
+    assert ev < TOL_FWD and eg < TOL_VJP
