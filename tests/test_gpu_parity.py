@@ -516,3 +516,38 @@ def test_config1_full_size_100_steps_forward_and_backward(sph):
     print(f"C1 full: KE/KE0 gpu {ke_g / ke0:.6f} oracle {ke_o / ke0:.6f}; v(T) err {ev:.2e}; dKE/dv0 err {eg:.2e}")
     assert abs(ke_g - ke_o) <= 1e-4 * ke_o and ke_o < ke0
     assert ev < TOL_FWD and eg < TOL_VJP
+
+
+def test_config4_full_size_lists_and_sampled_rows(sph):
+    """BASELINE.json config 4 at full size (256^3 = 16.8 M particles, log-normal h, cell edge = max h, ~134 particles per
+    cell, 2.3e9 list entries) in the configuration bench.py --config 4 times (tile search + generic pair kernels): the
+    lists in full, bit-exact against the oracle's grid search; RHS and VJP on sampled rows."""
+    if sph.layout_name != "tile":
+        pytest.skip("one layout at this size")
+    wl = W.make(4)
+    assert wl.n == 256 ** 3
+    lam, mu = W.random_cotangents(wl)
+    _, dev, nnz = build(wl, 1.0, sph)
+    rp_o, ci_o = oracle_lists(wl)
+    assert nnz == int(rp_o[-1])
+    rp, ci = sph.neighbors_export()
+    assert np.array_equal(_np(rp), rp_o)
+    ci_h = _np(ci)
+    del ci
+    torch.cuda.empty_cache()
+    assert np.array_equal(ci_h, ci_o)
+    del ci_h
+    rows = np.random.default_rng(11).choice(wl.n, size=2000, replace=False).astype(np.int64)
+    drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+    d_o, a_o, sd, sa = oracle.rhs(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp_o, ci_o, rows=rows,
+                                  with_scales=True)
+    assert max_norm_err(_np(drho)[rows], d_o[rows], sd[rows]) < TOL_FWD
+    assert max_norm_err(_np(acc)[rows], a_o[rows], sa[rows]) < TOL_FWD
+    xb, vb, rb, pb = sph.rhs_vjp(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind, torch.from_numpy(lam).cuda(),
+                                 torch.from_numpy(mu).cuda())
+    xo, vo, ro, _ = oracle.rhs_vjp(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp_o, ci_o, lam, mu,
+                                   rows=rows)
+    assert max_norm_err(_np(xb)[rows], xo[rows]) < TOL_VJP
+    assert max_norm_err(_np(vb)[rows], vo[rows]) < TOL_VJP
+    assert max_norm_err(_np(rb)[rows], ro[rows]) < TOL_VJP
+    assert torch.isfinite(pb).all()
