@@ -115,6 +115,15 @@ def density(domain, x, h, m, row_ptr, col_idx):
     return rho
 
 
+def max_displacement(domain, x, x_build):
+    """largest minimum-image displacement of a particle since the positions of the neighbour query"""
+    dim, per, lo, hi = _dom(domain)
+    x, xb = _d(x), _d(x_build)
+    f = lib().orc_max_displacement
+    f.restype = C.c_double
+    return float(f(C.c_int64(x.shape[0]), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(x), _p(xb)))
+
+
 def density_vjp(domain, x, h, m, row_ptr, col_idx, rho_bar):
     """(x_bar, m_bar) = J^T rho_bar of density() with the adjacency held fixed (Eq.21)"""
     dim, per, lo, hi = _dom(domain)

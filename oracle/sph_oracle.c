@@ -17,6 +17,7 @@
  *   orc_neighbors               : lattice counts 45 (2D,H=4dx) / 93 (3D,H=3dx), symmetry, brute vs grid,
  *                                 pure-Python brute force on tiny inputs
  *   orc_density                 : interior lattice 1.000415750 / 1.002898240, Riemann-sum argument
+ *   orc_max_displacement        : hand cases (known shift, shift by the box length, crossing a periodic face)
  *   orc_density_vjp             : central finite differences of orc_density (x and m), sum x_bar = 0, two-particle
  *                                 closed form, zero on a lattice with uniform rho_bar
  *   orc_rhs                     : momentum conservation, Galilean / rigid rotation invariance, uniform
@@ -295,6 +296,35 @@ int64_t orc_neighbors(int64_t n, int dim, const int *periodic, const double *lo,
         nnz = row_ptr[n];
     free(cnt);
     return nnz;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * NEXT-3a  Verlet-list validity: "the neighbor list needs to be updated if any particle
+ *      moves more than half of the skin-width, where it is important to compute this update with respect to the
+ *      positions used during the original neighborhood query".  Returns D = max_i |x_i - xb_i| with the minimum image
+ *      on periodic axes ("tracking of total particle motion is significantly simplified for periodic BCs when using
+ *      the minimum image convention").  The decision itself, 2 D <= skin width, is one comparison made by the caller.
+ * ------------------------------------------------------------------------------------------ */
+double orc_max_displacement(int64_t n, int dim, const int *periodic, const double *lo, const double *hi,
+                            const double *x, const double *x_build)
+{
+    double L[3];
+    box_len(dim, lo, hi, L);
+    double *xw = (double *)malloc((size_t)n * dim * sizeof(double));
+    double *bw = (double *)malloc((size_t)n * dim * sizeof(double));
+    wrap64(n, dim, periodic, lo, hi, x, xw);
+    wrap64(n, dim, periodic, lo, hi, x_build, bw);
+    double D = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        double d[3] = {0, 0, 0};
+        for (int k = 0; k < dim; ++k) d[k] = xw[i * dim + k] - bw[i * dim + k];
+        min_image(d, dim, periodic, L);
+        double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        if (r > D) D = r;
+    }
+    free(xw);
+    free(bw);
+    return D;
 }
 
 /* ------------------------------------------------------------------------------------------

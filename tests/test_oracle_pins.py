@@ -186,6 +186,23 @@ def test_density_single_particle_and_two_particles():
     assert abs(rho[1] - (3.0 * oracle.w(0, H, 3) + 2.0 * oracle.w(r, H, 3))) < 1e-12
 
 
+# ------------------------------------------------------------------------------------------ Verlet validity (NEXT-3a)
+def test_max_displacement_hand_cases():
+    """displacement w.r.t. the positions of the original query, minimum image on periodic axes"""
+    dom = W.Domain(dim=2, periodic=(1, 0, 0), lo=(0.0, 0.0, 0.0), hi=(2.0, 1.0, 0.0), cell_size=0.25)
+    xb = np.array([[0.1, 0.2], [1.9, 0.5], [1.0, 0.9]])
+    x = xb.copy()
+    assert oracle.max_displacement(dom, x, xb) == 0.0
+    x[0] += (0.03, 0.04)                                    # |d| = 0.05
+    assert abs(oracle.max_displacement(dom, x, xb) - 0.05) < 1e-15
+    x[1, 0] += 0.2                                          # crosses the periodic face at x = 2: still 0.2, not 1.8
+    assert abs(oracle.max_displacement(dom, x, xb) - 0.2) < 1e-12
+    x[2, 0] += 2.0                                          # a whole box length along the periodic axis: no motion
+    assert abs(oracle.max_displacement(dom, x, xb) - 0.2) < 1e-12
+    x[2, 1] -= 0.7                                          # bounded axis: plain difference
+    assert abs(oracle.max_displacement(dom, x, xb) - 0.7) < 1e-12
+
+
 # ------------------------------------------------------------------------------------------ density adjoint (NEXT-1)
 @pytest.mark.parametrize("cfg,kw", [(1, dict(n_axis=20)), (3, dict(n_axis=9)), (4, dict(n_axis=9)), (2, dict(dx=0.08))])
 def test_density_vjp_matches_central_differences_of_density(cfg, kw):
