@@ -91,6 +91,15 @@ int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float *x, const f
  * Synchronises `stream`; *nnz_out (host pointer, may be NULL) receives the number of entries. */
 int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out, sph_stream_t stream);
 
+/* Verlet-list validity ("the neighbor list needs to be updated if any particle
+ * moves more than half of the skin-width ... with respect to the positions used during the original neighborhood
+ * query"): D = max_i |x_i - x_build_i| (minimum image on periodic axes) of the positions x [n][dim] against those given
+ * to sph_build_cells.  *valid_out = 1 iff 2 D <= (search_scale - 1 - skin_needed) * min h, i.e. every pair closer than
+ * (1 + skin_needed) * H_ij at x is still in the lists of the last sph_neighbors(search_scale).  valid_out and
+ * max_disp_out are HOST pointers (either may be NULL).  Synchronises `stream`. */
+int sph_lists_valid(sph_ctx *ctx, const float *x, float skin_needed, int32_t *valid_out, float *max_disp_out,
+                    sph_stream_t stream);
+
 /* Copy the lists out in CALLER ids: row_ptr [n+1] int64, col_idx [nnz] int32, each row ascending, self included. */
 int sph_neighbors_export(sph_ctx *ctx, int64_t *row_ptr, int32_t *col_idx, sph_stream_t stream);
 

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsph_b200.so")
 
 EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph_neighbors_export", "sph_density",
-           "sph_density_vjp",
+           "sph_density_vjp", "sph_lists_valid",
            "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
            "sph_check", "sph_strerror", "sph_get_info", "sph_get_layout", "sph_profile_enable", "sph_profile_read",
            "sph_set_option")
@@ -67,6 +67,7 @@ def load_library(path: str = LIB_PATH):
     lib.sph_neighbors_export.argtypes = [vp, vp, vp, vp]
     lib.sph_density.argtypes = [vp, vp, vp, vp]
     lib.sph_density_vjp.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.sph_lists_valid.argtypes = [vp, vp, f32, C.POINTER(C.c_int32), C.POINTER(f32), vp]
     lib.sph_rhs.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 7 + [vp]
     lib.sph_rhs_vjp.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 11 + [vp]
     lib.sph_rk_step.argtypes = [vp, C.POINTER(SphDomain), C.POINTER(SphParams), f32, f32, i64] + [vp] * 6 + [vp]
@@ -174,6 +175,13 @@ class Sph:
         col = torch.empty(max(self.nnz, 1), dtype=torch.int32, device=f"cuda:{self.device}")
         self._chk(self.lib.sph_neighbors_export(self._ctx, _ptr(row_ptr), _ptr(col), _stream()))
         return row_ptr, col[: self.nnz]
+
+    def lists_valid(self, x, skin_needed: float = 0.0):
+        """(valid, max displacement since the build): the Verlet-list test of PAPER.md:568"""
+        _f32(x, (self.n, self.dim))
+        ok, D = C.c_int32(0), C.c_float(0.0)
+        self._chk(self.lib.sph_lists_valid(self._ctx, _ptr(x), float(skin_needed), C.byref(ok), C.byref(D), _stream()))
+        return bool(ok.value), float(D.value)
 
     def density(self, m, out=None):
         _f32(m, (self.n,))

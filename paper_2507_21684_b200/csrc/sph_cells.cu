@@ -232,6 +232,37 @@ __global__ void k_reorder(const float *__restrict__ x, const float *__restrict__
     if (p == n - 1 || key_sorted[p + 1] != kc) cell_end[lin] = (uint32_t)(p + 1);
 }
 
+// ------------------------------------------------------------------------------------------ Verlet validity
+// largest minimum-image displacement since the build; float bits of a non-negative float order like
+// unsigned integers, so the maximum is an integer atomic
+__global__ void k_max_displacement(const float *__restrict__ x, int64_t n, GridGeom gg,
+                                   const uint32_t *__restrict__ inv_perm, const float4 *__restrict__ pos_s,
+                                   uint32_t *__restrict__ out)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    float r = 0.f;
+    if (i < n) {
+        const float4 b = pos_s[inv_perm[i]];
+        const float xb[3] = {b.x, b.y, b.z};
+        float r2 = 0.f;
+        for (int k = 0; k < gg.dim; ++k) {
+            float xv = x[i * gg.dim + k];
+            float d;
+            if (gg.periodic[k]) {
+                d = wrap_coord(xv, gg.lo[k], gg.hi[k], gg.L[k]) - xb[k];
+                d = d > 0.5f * gg.L[k] ? d - gg.L[k] : (d < -0.5f * gg.L[k] ? d + gg.L[k] : d);
+            } else {
+                d = xv - xb[k];
+            }
+            r2 = fmaf(d, d, r2);
+        }
+        r = sqrtf(r2);
+        if (!(r >= 0.f)) r = __uint_as_float(0x7f800000u);        // NaN position: never valid
+    }
+    uint32_t rb = __reduce_max_sync(0xffffffffu, __float_as_uint(r));
+    if ((threadIdx.x & 31) == 0 && rb > *(volatile uint32_t *)out) atomicMax(out, rb);
+}
+
 int ceil_log2(int v)
 {
     int b = 0;
@@ -375,5 +406,35 @@ extern "C" int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float 
     }
     SPH_CUDA_TRY(cudaGetLastError());
     ctx->cells_ready = true;
+    return SPH_OK;
+}
+
+extern "C" int sph_lists_valid(sph_ctx *ctx, const float *x, float skin_needed, int32_t *valid_out, float *max_disp_out,
+                               sph_stream_t stream)
+{
+    if (!ctx || !x || !(skin_needed >= 0.f)) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    const int64_t n = ctx->n;
+    uint32_t *slot = ctx->stats.as<uint32_t>() + 12;
+    SPH_CUDA_TRY(cudaMemsetAsync(slot, 0, 4, st));
+    {
+        KScope ks(ctx, SPH_K_KEY, 1, st);
+        k_max_displacement<<<(unsigned)((n + kThreads - 1) / kThreads), kThreads, 0, st>>>(
+            x, n, ctx->geom, ctx->inv_perm.as<uint32_t>(), ctx->pos_s.as<float4>(), slot);
+    }
+    SPH_CUDA_TRY(cudaGetLastError());
+    uint32_t *hp = reinterpret_cast<uint32_t *>(ctx->h_pinned + 14);
+    SPH_CUDA_TRY(cudaMemcpyAsync(hp, slot, 4, cudaMemcpyDeviceToHost, st));
+    SPH_CUDA_TRY(cudaStreamSynchronize(st));
+    float D;
+    memcpy(&D, hp, 4);
+    if (max_disp_out) *max_disp_out = D;
+    if (valid_out) {
+        const double width = ((double)ctx->search_scale - 1.0 - (double)skin_needed) * (double)ctx->hmin;
+        *valid_out = (2.0 * (double)D <= width) ? 1 : 0;
+    }
     return SPH_OK;
 }

@@ -551,3 +551,38 @@ def test_config4_full_size_lists_and_sampled_rows(sph):
     assert max_norm_err(_np(vb)[rows], vo[rows]) < TOL_VJP
     assert max_norm_err(_np(rb)[rows], ro[rows]) < TOL_VJP
     assert torch.isfinite(pb).all()
+
+
+def test_verlet_list_validity(sph):
+    """PAPER.md:568: the lists stay usable while no particle has moved more than half the skin width since the query;
+    the displacement is the minimum-image one and is measured against the positions of the query"""
+    wl = W.perturbed(W.make(3, n_axis=20), amp_x=0.3, amp_rho=0.02)
+    skin = 0.1
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin) * np.float32(1.0001))
+    _, dev, _ = build(wl, 1.0 + skin, sph)
+    H = float(wl.h.min())
+    ok, D = sph.lists_valid(dev.x)
+    assert ok and D == 0.0
+    rng = np.random.default_rng(3)
+    for frac, want in ((0.45, True), (0.55, False)):
+        u = rng.normal(size=wl.x.shape)
+        u /= np.linalg.norm(u, axis=1, keepdims=True)
+        amp = rng.uniform(0.0, 1.0, size=(wl.n, 1))
+        amp[rng.integers(wl.n)] = 1.0                                    # somebody moves the full distance
+        x1 = (wl.x + frac * skin * H * amp * u).astype(np.float32)
+        x1 = (x1 + rng.integers(-1, 2, size=x1.shape).astype(np.float32)).astype(np.float32)   # other periodic images
+        ok, D = sph.lists_valid(torch.from_numpy(x1).cuda())
+        D_o = oracle.max_displacement(wl.domain, x1, wl.x)
+        assert abs(D - D_o) <= 2e-6 * H + 1e-6 * D_o                   # fp32 positions near 1-2 box lengths
+        assert ok == want and ok == (2.0 * D_o <= skin * H)
+        ok2, _ = sph.lists_valid(torch.from_numpy(x1).cuda(), skin_needed=0.02)
+        assert ok2 == (2.0 * D_o <= (skin - 0.02) * H)
+        if ok:                                                          # valid lists: the RHS at x1 needs no rebuild
+            import copy
+            wl1 = copy.copy(wl)
+            wl1.x = x1
+            rp_o, ci_o = oracle_lists(wl1)
+            d_o, a_o, sd, sa = oracle.rhs(wl.domain, wl.params, x1, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp_o, ci_o,
+                                          with_scales=True)
+            drho, acc = sph.rhs(wl.params, torch.from_numpy(x1).cuda(), dev.v, dev.rho, dev.m, dev.kind)
+            assert max_norm_err(_np(drho), d_o, sd) < 3e-4 and max_norm_err(_np(acc), a_o, sa) < 3e-4
