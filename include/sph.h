@@ -203,8 +203,12 @@ enum {
                                in shared memory).  2 falls back to 1 when a halo does not fit shared memory. */
     SPH_OPT_TILE_EDGE = 3,  /* edge of the cell blocks of the tile-local layout: 1, 2, 4 cells; 0 = automatic */
     SPH_OPT_PAIR_WARPS = 4, /* warps per CTA of the tile pair kernels: 4, 8, 16; 0 = automatic */
-    SPH_OPT_FILL_MASKS = 5  /* 1 (default): the fill of the tile-local lists expands the hit masks saved by the count pass;
+    SPH_OPT_FILL_MASKS = 5, /* 1 (default): the fill of the tile-local lists expands the hit masks saved by the count pass;
                                0: it repeats the distance tests (no mask buffer) */
+    SPH_OPT_RK_EXTRA_SKIN = 6 /* Verlet lists across steps: value/1000 = extra skin e (in units of h).  With
+                               e > 0 sph_rk_step / sph_rk_step_vjp build their lists with search_scale = 1 + skin + e
+                               (the domain's cell_size must cover it) and a later call with the same domain, n and h
+                               REUSES them while sph_lists_valid(x, skin) holds; 0 (default): rebuilt in every call */
 };
 int sph_set_option(sph_ctx *ctx, int key, int value);
 int sph_profile_enable(sph_ctx *ctx, int on);

@@ -348,6 +348,7 @@ extern "C" int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float 
     int64_t ncells;
     SPH_TRY(make_geom(dom, &gg, &ncells));
     ctx->geom = gg;
+    ctx->dom_last = *dom;
     ctx->ncells_total = ncells;
     ctx->n = n;
     ctx->last_stream = st;

@@ -124,6 +124,8 @@ struct sph_ctx {
     int opt_group = 0;          // lanes per row in the pair kernels (0 = default)
     int opt_warps = 0;          // warps per CTA of the tile pair kernels (0 = automatic: 8, or 16 when one CTA fits an SM)
     int opt_list_mode = 0;      // 0 auto, 1 force the generic (global-id) lists, 2 force tile-local lists
+    int opt_rk_extra_permille = 0;   // sph_rk_step: extra list skin (1/1000 of h) that lets later steps reuse the lists
+    sph_domain dom_last{};      // domain of the last sph_build_cells
     int opt_fill_masks = 1;     // the fill expands the hit masks saved by the count pass (0: repeats the tests)
     int opt_tile_edge = 0;      // 0 auto, else force the tile edge B (1, 2, 4)
     bool tile_mode = false;     // lists of the last sph_neighbors are tile-local (col16)

@@ -55,7 +55,8 @@ __device__ __forceinline__ void store_stage(const StageBufs &sb, int64_t p, cons
 // base state in sorted order: b0 = {xw,yw,zw,h}, b1 = {vx,vy,vz,rho}, m_s, kind_s; also writes stage 1 (= base)
 template <int DIM>
 __global__ void k_rk_base(int64_t n, KPar kp, const uint32_t *__restrict__ perm, const float4 *__restrict__ pos_s,
-                          const float *__restrict__ v, const float *__restrict__ rho, const float *__restrict__ m,
+                          const float *__restrict__ x, const float *__restrict__ v, const float *__restrict__ rho,
+                          const float *__restrict__ m,
                           const uint8_t *__restrict__ kind, float4 *__restrict__ b0, float4 *__restrict__ b1,
                           float *__restrict__ m_s, uint8_t *__restrict__ kind_s, StageBufs sb)
 {
@@ -63,11 +64,23 @@ __global__ void k_rk_base(int64_t n, KPar kp, const uint32_t *__restrict__ perm,
     if (p >= n) return;
     const int64_t i = perm[p];
     const float4 ps = pos_s[p];                              // wrapped build positions (R4) + h
-    float X[3] = {ps.x, ps.y, ps.z}, Vv[3] = {0.f, 0.f, 0.f};
+    // current position: the periodic image next to the build position (identical to it when the lists were built
+    // from x in this call; differs when Verlet lists are reused across steps)
+    const float xb[3] = {ps.x, ps.y, ps.z};
+    float X[3] = {0.f, 0.f, 0.f}, Vv[3] = {0.f, 0.f, 0.f};
 #pragma unroll
-    for (int k = 0; k < DIM; ++k) Vv[k] = v[i * DIM + k];
+    for (int k = 0; k < DIM; ++k) {
+        float xv = x[i * DIM + k];
+        if (kp.periodic[k]) {
+            xv = wrap_coord(xv, kp.lo[k], kp.hi[k], kp.L[k]);
+            const float dd = xv - xb[k];
+            xv = dd > kp.halfL[k] ? xv - kp.L[k] : (dd < -kp.halfL[k] ? xv + kp.L[k] : xv);
+        }
+        X[k] = xv;
+        Vv[k] = v[i * DIM + k];
+    }
     const float r = rho[i], mi = m[i];
-    b0[p] = ps;
+    b0[p] = make_float4(X[0], X[1], X[2], ps.w);
     b1[p] = make_float4(Vv[0], Vv[1], Vv[2], r);
     m_s[p] = mi;
     kind_s[p] = kind[i];
@@ -204,10 +217,20 @@ __global__ void k_adj_final(int64_t n, const uint32_t *__restrict__ perm, const 
 
 inline unsigned nb(int64_t n) { return (unsigned)((n + 255) / 256); }
 
+// Lists for one step.  Default: cells and lists from x with search_scale = 1 + skin.  With SPH_OPT_RK_EXTRA_SKIN the lists
+// carry an extra skin and are kept across steps while no particle has moved more than half of what is left of it
+// (the caller keeps the domain, n and h unchanged).
 int rebuild(sph_ctx *ctx, const sph_domain *dom, float skin, const float *x, const float *h, int64_t n, cudaStream_t st)
 {
+    const float extra = 0.001f * (float)ctx->opt_rk_extra_permille;
+    if (extra > 0.f && ctx->lists_ready && ctx->n == n && memcmp(&ctx->dom_last, dom, sizeof(*dom)) == 0 &&
+        ctx->search_scale >= 1.0f + skin) {
+        int32_t ok = 0;
+        SPH_TRY(sph_lists_valid(ctx, x, skin, &ok, nullptr, (sph_stream_t)st));
+        if (ok) return SPH_OK;
+    }
     SPH_TRY(sph_build_cells(ctx, dom, x, h, n, (sph_stream_t)st));
-    return sph_neighbors(ctx, 1.0f + skin, nullptr, (sph_stream_t)st);
+    return sph_neighbors(ctx, 1.0f + skin + extra, nullptr, (sph_stream_t)st);
 }
 
 } // namespace
@@ -241,9 +264,9 @@ extern "C" int sph_rk_step(sph_ctx *ctx, const sph_domain *dom, const sph_params
     {
     KScope ks(ctx, SPH_K_RK, 1, st);
     if (kp.dim == 3)
-        k_rk_base<3><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), v, rho, m, kind, b0, b1, m_s, kind_s, sb);
+        k_rk_base<3><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x, v, rho, m, kind, b0, b1, m_s, kind_s, sb);
     else
-        k_rk_base<2><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), v, rho, m, kind, b0, b1, m_s, kind_s, sb);
+        k_rk_base<2><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x, v, rho, m, kind, b0, b1, m_s, kind_s, sb);
     }
     const float c[4] = {0.f, 0.5f, 0.5f, 1.f};
     const float b[4] = {1.f / 6.f, 1.f / 3.f, 1.f / 3.f, 1.f / 6.f};
@@ -314,9 +337,9 @@ extern "C" int sph_rk_step_vjp(sph_ctx *ctx, const sph_domain *dom, const sph_pa
     {
     KScope ks(ctx, SPH_K_RK, 1, st);
     if (kp.dim == 3)
-        k_rk_base<3><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), v0, rho0_state, m, kind, b0, b1, m_s, kind_s, S[0]);
+        k_rk_base<3><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x0, v0, rho0_state, m, kind, b0, b1, m_s, kind_s, S[0]);
     else
-        k_rk_base<2><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), v0, rho0_state, m, kind, b0, b1, m_s, kind_s, S[0]);
+        k_rk_base<2><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x0, v0, rho0_state, m, kind, b0, b1, m_s, kind_s, S[0]);
     }
     for (int s = 1; s < 4; ++s) {
         SPH_TRY(sph_launch_rhs_sorted(ctx, kp, S[s - 1].s0, S[s - 1].s1, S[s - 1].s2, kind_s, nullptr, nullptr, k4, st));

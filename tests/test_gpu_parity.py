@@ -586,3 +586,43 @@ def test_verlet_list_validity(sph):
                                           with_scales=True)
             drho, acc = sph.rhs(wl.params, torch.from_numpy(x1).cuda(), dev.v, dev.rho, dev.m, dev.kind)
             assert max_norm_err(_np(drho), d_o, sd) < 3e-4 and max_norm_err(_np(acc), a_o, sa) < 3e-4
+
+
+def test_rk_steps_with_verlet_lists_reused_across_steps(sph):
+    """SPH_OPT_RK_EXTRA_SKIN: lists built once with an extra skin serve several RK4 steps; the trajectory
+    and the gradient through it stay within the per-step bars of the fp64 oracle (which rebuilds exact lists at every
+    stage), and most steps run without a neighbour search"""
+    from paper_2507_21684_b200.binding import OPT_RK_EXTRA_SKIN
+    wl = W.perturbed(W.make(3, n_axis=24), amp_x=0.2, amp_rho=0.02)
+    skin, extra, nsteps = 0.06, 0.30, 8
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin + extra) * np.float32(1.0001))
+    dev = Dev(wl)
+    sph.set_option(OPT_RK_EXTRA_SKIN, int(round(1000 * extra)))
+    try:
+        sph.profile_read()
+        states = [(dev.x.clone(), dev.v.clone(), dev.rho.clone())]
+        for _ in range(nsteps):
+            x, v, rho = (t.clone() for t in states[-1])
+            sph.rk_step(wl.domain, wl.params, wl.dt, skin, x, v, rho, dev.m, dev.h, dev.kind)
+            states.append((x, v, rho))
+        fills = sph.profile_read()["fill"][1]
+        xb = torch.zeros_like(dev.x)
+        vb = (dev.m[:, None] * states[-1][1]).contiguous()
+        rb = torch.zeros_like(dev.rho)
+        pb = torch.zeros(10, device="cuda")
+        for k in range(nsteps - 1, -1, -1):
+            sph.rk_step_vjp(wl.domain, wl.params, wl.dt, skin, *states[k], dev.m, dev.h, dev.kind, xb, vb, rb, pb)
+    finally:
+        sph.set_option(OPT_RK_EXTRA_SKIN, 0)
+    assert 1 <= fills < nsteps                              # at least one reuse (TGV: |v| dt = 0.006 H per step)
+    so = [(wl.x.astype(np.float64), wl.v.astype(np.float64), wl.rho.astype(np.float64))]
+    for _ in range(nsteps):
+        so.append(oracle.rk4_step(wl.domain, wl.params, wl.dt, *so[-1], wl.m, wl.h, wl.kind, method=1))
+    xo, vo, ro = np.zeros_like(so[-1][0]), wl.m.astype(np.float64)[:, None] * so[-1][1], np.zeros(wl.n)
+    for k in range(nsteps - 1, -1, -1):
+        xo, vo, ro, _ = oracle.rk4_step_vjp(wl.domain, wl.params, wl.dt, *so[k], wl.m, wl.h, wl.kind, xo, vo, ro, method=1)
+    ev = max_norm_err(_np(states[-1][1]).astype(np.float64) - wl.v, so[-1][1] - wl.v)
+    er = max_norm_err(_np(states[-1][2]).astype(np.float64) - wl.rho, so[-1][2] - wl.rho)
+    eg = max_norm_err(_np(vb), vo)
+    print(f"verlet reuse: {fills} list builds in {nsteps} steps; increments err v {ev:.2e} rho {er:.2e}; gradient err {eg:.2e}")
+    assert ev < 2e-4 and er < 2e-4 and eg < TOL_VJP
