@@ -617,7 +617,7 @@ static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, size_t 
     int warps = 16;
     if (ctx->opt_warps) warps = ctx->opt_warps;
     else if (sm_total / (need(16) + per_cta) < 2 && sm_total / (need(8) + per_cta) >= 2) warps = 8;
-    while (warps > 1 && need(warps) > cta_max) warps >>= 1;
+    while (warps > 2 && need(warps) > cta_max) warps >>= 1;           // tile_setup needs two warps
     if (need(warps) > cta_max) {                                   // last resort: a minimal ring (rows fall back to global reads)
         ts->rb = 8;
     }
