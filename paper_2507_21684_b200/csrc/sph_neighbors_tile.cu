@@ -239,7 +239,7 @@ k_nb_tile(TileGeom tg, GridGeom gg, SearchPar sp, int mcap, int wcap, const floa
 template <int DIM>
 __global__ void __launch_bounds__(64)
 k_tile_words(TileGeom tg, const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
-             uint32_t *__restrict__ words)
+             uint32_t *__restrict__ words, uint32_t *__restrict__ wmax_out)
 {
     __shared__ TileTab tt;
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
@@ -250,7 +250,15 @@ k_tile_words(TileGeom tg, const uint32_t *__restrict__ cell_start, const uint32_
         const uint32_t nrow = tt.t_off[tc + 1] - tt.t_off[tc];
         const int hc_i = tt.t_cell[tc];
         const int sl[3] = {hc_i % tt.ext[0], (hc_i / tt.ext[0]) % tt.ext[1], hc_i / (tt.ext[0] * tt.ext[1])};
-        if (nrow) w = ((nrow + 31u) >> 5) * 32u * cell_words<DIM>(tt, sl);
+        uint32_t cw = 0;
+        if (nrow) {
+            cw = cell_words<DIM>(tt, sl);
+            w = ((nrow + 31u) >> 5) * 32u * cw;
+        }
+        cw = __reduce_max_sync(0xffffffffu, cw);
+        if (threadIdx.x == 0 && cw > *(volatile uint32_t *)wmax_out) atomicMax(wmax_out, cw);
+    } else {
+        (void)__reduce_max_sync(0xffffffffu, 0u);
     }
     w = __reduce_add_sync(0xffffffffu, w);
     if (threadIdx.x == 0) words[blockIdx.x] = w;
@@ -595,8 +603,10 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
             maskbuf = ctx->maskbuf.as<uint32_t>();
             mask_base = ctx->tile_mask_base.as<long long>();
             KScope ks(ctx, SPH_K_COUNT, 4, st);
-            if (gg.dim == 3) k_tile_words<3><<<(unsigned)tg.ntiles, 64, 0, st>>>(tg, cs, ce, ctx->tile_words.as<uint32_t>());
-            else k_tile_words<2><<<(unsigned)tg.ntiles, 64, 0, st>>>(tg, cs, ce, ctx->tile_words.as<uint32_t>());
+            uint32_t *wmax_dev = ctx->stats.as<uint32_t>() + 11;       // largest number of mask words of a row
+            SPH_CUDA_TRY(cudaMemsetAsync(wmax_dev, 0, 4, st));
+            if (gg.dim == 3) k_tile_words<3><<<(unsigned)tg.ntiles, 64, 0, st>>>(tg, cs, ce, ctx->tile_words.as<uint32_t>(), wmax_dev);
+            else k_tile_words<2><<<(unsigned)tg.ntiles, 64, 0, st>>>(tg, cs, ce, ctx->tile_words.as<uint32_t>(), wmax_dev);
             SPH_TRY(sph_scan_u32(ctx, ctx->tile_words.as<uint32_t>(), mask_base, true, tg.ntiles, st));
         }
     }
@@ -624,8 +634,11 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
         SPH_TRY(sph_scan_u32(ctx, ctx->cnt.as<uint32_t>(), ctx->row_ptr.p, true, n, st));
     }
     SPH_CUDA_TRY(cudaMemcpyAsync(ctx->h_pinned + 4, ctx->row_ptr.as<long long>() + n, 8, cudaMemcpyDeviceToHost, st));
+    if (maskbuf) SPH_CUDA_TRY(cudaMemcpyAsync(ctx->h_pinned + 5, ctx->stats.as<uint32_t>() + 11, 4, cudaMemcpyDeviceToHost, st));
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
     const int64_t nnz = ctx->h_pinned[4];
+    uint32_t wmax_rows = 0;
+    if (maskbuf) memcpy(&wmax_rows, ctx->h_pinned + 5, 4);
     SPH_TRY(ctx->col16.reserve((size_t)(nnz > 0 ? nnz : 1) * 2 + 64));
     {
         // per-warp staging capacity: 32 rows of the mean length with head room; the halo positions come first
@@ -647,8 +660,9 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
             wc = (wc + 63) & ~63;
             if (wc < 512) wc = 512;
             if (wc > 12288) wc = 12288;
-            int wb = (gg.dim == 3 ? 9 : 3) * (int)((3u * occmax + 31u) / 32u);      // most mask words a row can have
-            if (wb > 64) wb = 64;
+            int wb = (int)wmax_rows;                            // most mask words any row has (k_tile_words)
+            if (wb < 1) wb = 1;
+            if (wb > 64) wb = 64;                               // rows beyond take the word-synchronous expansion
             const int ew = 4;                                                       // warps per CTA
             const size_t smem = (size_t)ew * ((size_t)wc * 2 + (size_t)wb * 128);
             if (gg.dim == 3) {
