@@ -124,6 +124,30 @@ def max_displacement(domain, x, x_build):
     return float(f(C.c_int64(x.shape[0]), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(x), _p(xb)))
 
 
+def grad_sum(domain, x, h, a, row_ptr, col_idx):
+    """g_i = sum_j a_j grad_i W_ij (the gradient term of PAPER.md:379 Eq.24 with a = m/rho)"""
+    dim, per, lo, hi = _dom(domain)
+    x, h, a = _d(x), _d(h), _d(a)
+    n = x.shape[0]
+    g = np.empty((n, dim), dtype=np.float64)
+    lib().orc_grad_sum(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(x), _p(h), _p(a),
+                       _p(np.ascontiguousarray(row_ptr, np.int64)), _p(np.ascontiguousarray(col_idx, np.int32)), _p(g))
+    return g
+
+
+def grad_sum_vjp(domain, x, h, a, row_ptr, col_idx, g_bar):
+    """(x_bar, a_bar) = J^T g_bar of grad_sum() with the adjacency held fixed"""
+    dim, per, lo, hi = _dom(domain)
+    x, h, a, gb = _d(x), _d(h), _d(a), _d(g_bar)
+    n = x.shape[0]
+    xb = np.empty((n, dim), dtype=np.float64)
+    ab = np.empty(n, dtype=np.float64)
+    lib().orc_grad_sum_vjp(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(x), _p(h), _p(a),
+                           _p(np.ascontiguousarray(row_ptr, np.int64)), _p(np.ascontiguousarray(col_idx, np.int32)),
+                           _p(gb), _p(xb), _p(ab))
+    return xb, ab
+
+
 def density_vjp(domain, x, h, m, row_ptr, col_idx, rho_bar):
     """(x_bar, m_bar) = J^T rho_bar of density() with the adjacency held fixed (Eq.21)"""
     dim, per, lo, hi = _dom(domain)

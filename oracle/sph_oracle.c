@@ -18,6 +18,9 @@
  *                                 pure-Python brute force on tiny inputs
  *   orc_density                 : interior lattice 1.000415750 / 1.002898240, Riemann-sum argument
  *   orc_max_displacement        : hand cases (known shift, shift by the box length, crossing a periodic face)
+ *   orc_grad_sum(_vjp)          : two-particle closed form, zero on a periodic lattice with uniform weights, equals the
+ *                                 own-position derivative of orc_density for a = m; central finite differences (x, a),
+ *                                 sum x_bar = 0
  *   orc_density_vjp             : central finite differences of orc_density (x and m), sum x_bar = 0, two-particle
  *                                 closed form, zero on a lattice with uniform rho_bar
  *   orc_rhs                     : momentum conservation, Galilean / rigid rotation invariance, uniform
@@ -391,6 +394,73 @@ void orc_density_vjp(int64_t n, int dim, const int *periodic, const double *lo, 
                 double c = rho_bar[i] * m[j] * G * d[k];
                 x_bar[i * dim + k] += c;
                 x_bar[j * dim + k] -= c;
+            }
+        }
+    }
+    free(xw);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * NEXT-1, second half: the gradient term of the particle-shifting loss, Eq.24,
+ *      [ sum_j m_j/rho_j grad_i W_ij ]^2.  The operator is the SPH gradient of the constant field with weights a_j
+ *      (a_j = m_j/rho_j in Eq.24):
+ *          g_i = sum_{j in N(i)} a_j grad_i W_ij = sum_j a_j G_ij d_ij,      d_ij = x_i - x_j   (Eq.29)
+ *      and its reverse mode, term by term, adjacency fixed, with the exact Hessian of the kernel
+ *      d(G d) = G dd + K (d . dd) d   (Eq.16):
+ *          a_bar_j += g_bar_i . (G d),   D = a_j (G g_bar_i + K (d . g_bar_i) d),   x_bar_i += D,   x_bar_j -= D.
+ * ------------------------------------------------------------------------------------------ */
+void orc_grad_sum(int64_t n, int dim, const int *periodic, const double *lo, const double *hi,
+                  const double *x, const double *h, const double *a,
+                  const int64_t *row_ptr, const int32_t *col_idx, double *g_out)
+{
+    double L[3];
+    box_len(dim, lo, hi, L);
+    double *xw = (double *)malloc((size_t)n * dim * sizeof(double));
+    wrap64(n, dim, periodic, lo, hi, x, xw);
+    for (int64_t i = 0; i < n; ++i) {
+        double acc[3] = {0, 0, 0};
+        for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
+            int64_t j = col_idx[p];
+            double d[3] = {0, 0, 0};
+            for (int k = 0; k < dim; ++k) d[k] = xw[i * dim + k] - xw[j * dim + k];
+            min_image(d, dim, periodic, L);
+            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            double H = h[i] > h[j] ? h[i] : h[j];
+            double G = orc_gfac(r, H, dim);
+            for (int k = 0; k < dim; ++k) acc[k] += a[j] * G * d[k];
+        }
+        for (int k = 0; k < dim; ++k) g_out[i * dim + k] = acc[k];
+    }
+    free(xw);
+}
+
+void orc_grad_sum_vjp(int64_t n, int dim, const int *periodic, const double *lo, const double *hi,
+                      const double *x, const double *h, const double *a,
+                      const int64_t *row_ptr, const int32_t *col_idx, const double *g_bar,
+                      double *x_bar, double *a_bar)
+{
+    double L[3];
+    box_len(dim, lo, hi, L);
+    double *xw = (double *)malloc((size_t)n * dim * sizeof(double));
+    wrap64(n, dim, periodic, lo, hi, x, xw);
+    for (int64_t i = 0; i < n * dim; ++i) x_bar[i] = 0.0;
+    for (int64_t i = 0; i < n; ++i) a_bar[i] = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
+            int64_t j = col_idx[p];
+            double d[3] = {0, 0, 0};
+            for (int k = 0; k < dim; ++k) d[k] = xw[i * dim + k] - xw[j * dim + k];
+            min_image(d, dim, periodic, L);
+            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            double H = h[i] > h[j] ? h[i] : h[j];
+            double G = orc_gfac(r, H, dim), K = orc_kfac(r, H, dim);
+            double dg = 0.0;
+            for (int k = 0; k < dim; ++k) dg += d[k] * g_bar[i * dim + k];
+            a_bar[j] += G * dg;
+            for (int k = 0; k < dim; ++k) {
+                double D = a[j] * (G * g_bar[i * dim + k] + K * dg * d[k]);
+                x_bar[i * dim + k] += D;
+                x_bar[j * dim + k] -= D;
             }
         }
     }

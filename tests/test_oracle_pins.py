@@ -254,6 +254,61 @@ def test_density_vjp_two_particle_closed_form_and_lattice_symmetry():
     assert np.max(np.abs(xb)) < 1e-9 * S
 
 
+# ------------------------------------------------------------------------------------------ kernel-gradient sum (NEXT-1, Eq.24)
+def test_grad_sum_closed_forms():
+    """g_i = sum_j a_j grad_i W_ij (Eq.24 with a = m/rho; grad_i W_ij = G d_ij, Eq.29)"""
+    dom = W.Domain(dim=3, periodic=(0, 0, 0), lo=(0.0,) * 3, hi=(1.0,) * 3, cell_size=0.5)
+    x = np.array([[0.5, 0.5, 0.5], [0.6, 0.52, 0.47]], dtype=np.float32)
+    h = np.array([0.3, 0.4], dtype=np.float32)
+    a = np.array([2.0, 3.0])
+    rp, ci = oracle.neighbors(dom, x, h)
+    g = oracle.grad_sum(dom, x, h, a, rp, ci)
+    d = x[0].astype(np.float64) - x[1].astype(np.float64)
+    G = oracle.gfac(float(np.linalg.norm(d)), float(np.float32(0.4)), 3)
+    assert np.max(np.abs(g[0] - a[1] * G * d)) < 1e-13 * abs(G) and np.max(np.abs(g[1] + a[0] * G * d)) < 1e-13 * abs(G)
+    # uniform weights on a periodic lattice: the kernel gradients cancel pairwise (the SPH gradient of a constant)
+    wl = W.make(0)
+    rp, ci = oracle.neighbors(wl.domain, wl.x, wl.h)
+    g = oracle.grad_sum(wl.domain, wl.x, wl.h, np.ones(wl.n), rp, ci)
+    S = abs(oracle.gfac(0.03, float(wl.h[0]), 2)) * 0.03 * 45
+    assert np.max(np.abs(g)) < 1e-9 * S
+    # a = m: g_i is the derivative of rho_i with respect to its OWN position (pinned against differences of density)
+    wl = W.perturbed(W.make(1, n_axis=16), amp_x=0.3)
+    rp, ci = oracle.neighbors(wl.domain, wl.x, wl.h)
+    x64, m64 = wl.x.astype(np.float64), wl.m.astype(np.float64)
+    g = oracle.grad_sum(wl.domain, x64, wl.h, m64, rp, ci)
+    eps = 1e-6 * float(wl.h[0])
+    for i, k in ((3, 0), (100, 1)):
+        e = np.zeros_like(x64)
+        e[i, k] = eps
+        fd = (oracle.density(wl.domain, x64 + e, wl.h, m64, rp, ci)[i] - oracle.density(wl.domain, x64 - e, wl.h, m64, rp, ci)[i]) / (2 * eps)
+        assert abs(fd - g[i, k]) < 1e-6 * np.max(np.abs(g))
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, dict(n_axis=20)), (3, dict(n_axis=9)), (4, dict(n_axis=9)), (2, dict(dx=0.08))])
+def test_grad_sum_vjp_matches_central_differences(cfg, kw):
+    wl = W.perturbed(W.make(cfg, **kw), amp_x=0.3, amp_rho=0.0)
+    rp, ci = oracle.neighbors(wl.domain, wl.x, wl.h)
+    rng = np.random.default_rng(7)
+    gb = rng.normal(size=(wl.n, wl.dim))
+    x, a = wl.x.astype(np.float64), wl.m.astype(np.float64) * (1.0 + 0.1 * rng.normal(size=wl.n))
+    xb, ab = oracle.grad_sum_vjp(wl.domain, x, wl.h, a, rp, ci, gb)
+    L = lambda xx, aa: float(np.sum(gb * oracle.grad_sum(wl.domain, xx, wl.h, aa, rp, ci)))
+    zx, za = rng.normal(size=x.shape), rng.normal(size=a.shape) * float(a.mean())
+    eps = 1e-6 * float(wl.h.min())
+    fd_x = (L(x + eps * zx, a) - L(x - eps * zx, a)) / (2 * eps)
+    fd_a = (L(x, a + 1e-3 * za) - L(x, a - 1e-3 * za)) / 2e-3           # linear in a
+    an_x, an_a = float(np.sum(xb * zx)), float(np.dot(ab, za))
+    assert abs(fd_x - an_x) <= 1e-6 * max(abs(an_x), np.sum(np.abs(xb * zx)) * 1e-3)
+    assert abs(fd_a - an_a) <= 1e-9 * max(abs(an_a), np.sum(np.abs(ab * za)))
+    for i, k in ((0, 0), (wl.n // 2, wl.dim - 1)):
+        e = np.zeros_like(x)
+        e[i, k] = 1.0
+        fd = (L(x + eps * e, a) - L(x - eps * e, a)) / (2 * eps)
+        assert abs(fd - xb[i, k]) <= 1e-6 * max(abs(xb[i, k]), np.max(np.abs(xb)) * 1e-3)
+    assert np.max(np.abs(xb.sum(0))) <= 1e-12 * np.sum(np.abs(xb))
+
+
 # ------------------------------------------------------------------------------------------ RHS
 def _lists(wl, method=1):
     return oracle.neighbors(wl.domain, wl.x, wl.h, method=method)
