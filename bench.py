@@ -358,6 +358,20 @@ def main():
     dvjp_ms = e0.elapsed_time(e1) / 5.0
     extras = {"density_vjp": {"ms": dvjp_ms, "pair_interactions_per_s": nnz_x / (dvjp_ms * 1e-3), "nnz": int(nnz_x),
                               "note": "sph_density_vjp (x_bar and m_bar), not part of the timed step"}}
+    # kernel-gradient sum and its adjoint (gradient term of the shifting loss, Eq.24), a = m/rho
+    a_dev = (m / rho).contiguous()
+    gs_dev, ab_dev = torch.empty_like(x), torch.empty_like(rho)
+    for name, call in (("grad_sum", lambda: sph.grad_sum(a_dev, gs_dev)),
+                       ("grad_sum_vjp", lambda: sph.grad_sum_vjp(a_dev, mu, xb_dev, ab_dev))):
+        call()
+        e0, e1 = ev(), ev()
+        e0.record()
+        for _ in range(5):
+            call()
+        e1.record()
+        torch.cuda.synchronize()
+        ms_x = e0.elapsed_time(e1) / 5.0
+        extras[name] = {"ms": ms_x, "pair_interactions_per_s": nnz_x / (ms_x * 1e-3), "nnz": int(nnz_x)}
 
     # ---- e2e: the same step through sph_step_host with pinned host buffers, copies inside the timed region
     e2e = None

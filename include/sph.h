@@ -114,6 +114,17 @@ int sph_density(sph_ctx *ctx, const float *m, float *rho_out, sph_stream_t strea
 int sph_density_vjp(sph_ctx *ctx, const float *m, const float *rho_bar, float *x_bar, float *m_bar,
                     sph_stream_t stream);
 
+/* Kernel-gradient sum with per-particle weights (the gradient term of the particle-shifting loss,
+ * PAPER.md:379 Eq.24, with a_j = m_j/rho_j): g_i = sum_j a_j grad_i W_ij = sum_j a_j G_ij (x_i - x_j), g_out [n][dim], at
+ * the positions given to sph_build_cells. */
+int sph_grad_sum(sph_ctx *ctx, const float *a, float *g_out, sph_stream_t stream);
+
+/* Reverse-mode adjoint of sph_grad_sum with the exact kernel Hessian G Id + K d d^T: given
+ * g_bar [n][dim], writes x_bar [n][dim] = sum_j [ a_j (G g_bar_i + K (d.g_bar_i) d) - a_i (G g_bar_j + K (d.g_bar_j) d) ]
+ * and, if a_bar is not NULL, a_bar [n] = - sum_j G_ij (x_i - x_j) . g_bar_j.  Adjacency fixed; gather form, no atomics. */
+int sph_grad_sum_vjp(sph_ctx *ctx, const float *a, const float *g_bar, float *x_bar, float *a_bar,
+                     sph_stream_t stream);
+
 /* One right-hand-side evaluation (formulas at the top of this file) on the lists of the last sph_neighbors.
  * x may differ from the build positions (RK stages) as long as the list is still a superset of the true
  * neighbours: pairs with r >= H_ij contribute exactly 0 (kernel clamp).  h is the one given to sph_build_cells. */

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsph_b200.so")
 
 EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph_neighbors_export", "sph_density",
-           "sph_density_vjp", "sph_lists_valid",
+           "sph_density_vjp", "sph_lists_valid", "sph_grad_sum", "sph_grad_sum_vjp",
            "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
            "sph_check", "sph_strerror", "sph_get_info", "sph_get_layout", "sph_profile_enable", "sph_profile_read",
            "sph_set_option")
@@ -67,6 +67,8 @@ def load_library(path: str = LIB_PATH):
     lib.sph_neighbors_export.argtypes = [vp, vp, vp, vp]
     lib.sph_density.argtypes = [vp, vp, vp, vp]
     lib.sph_density_vjp.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.sph_grad_sum.argtypes = [vp, vp, vp, vp]
+    lib.sph_grad_sum_vjp.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.sph_lists_valid.argtypes = [vp, vp, f32, C.POINTER(C.c_int32), C.POINTER(f32), vp]
     lib.sph_rhs.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 7 + [vp]
     lib.sph_rhs_vjp.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 11 + [vp]
@@ -199,6 +201,23 @@ class Sph:
         self._chk(self.lib.sph_density_vjp(self._ctx, _ptr(m), _ptr(rho_bar), _ptr(x_bar),
                                            _ptr(m_bar) if m_bar is not None else None, _stream()))
         return x_bar, m_bar
+
+    def grad_sum(self, a, out=None):
+        """g_i = sum_j a_j grad_i W_ij at the build positions (Eq.24 with a = m/rho)"""
+        a = _f32(a, (self.n,))
+        out = torch.empty((self.n, self.dim), dtype=torch.float32, device=a.device) if out is None else _f32(out, (self.n, self.dim))
+        self._chk(self.lib.sph_grad_sum(self._ctx, _ptr(a), _ptr(out), _stream()))
+        return out
+
+    def grad_sum_vjp(self, a, g_bar, x_bar=None, a_bar=None, want_a_bar=True):
+        """(x_bar, a_bar) = J^T g_bar of grad_sum()"""
+        a, g_bar = _f32(a, (self.n,)), _f32(g_bar, (self.n, self.dim))
+        x_bar = torch.empty((self.n, self.dim), dtype=torch.float32, device=a.device) if x_bar is None else _f32(x_bar, (self.n, self.dim))
+        if a_bar is None and want_a_bar:
+            a_bar = torch.empty(self.n, dtype=torch.float32, device=a.device)
+        self._chk(self.lib.sph_grad_sum_vjp(self._ctx, _ptr(a), _ptr(g_bar), _ptr(x_bar),
+                                            _ptr(a_bar) if a_bar is not None else None, _stream()))
+        return x_bar, a_bar
 
     def rhs(self, params, x, v, rho, m, kind, drho_dt=None, acc=None):
         p = make_params(params)

@@ -286,6 +286,9 @@ int sph_tile_expand_col(sph_ctx *ctx, cudaStream_t st);   // tile-local lists ->
 int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, float *rho_out, cudaStream_t st);
 int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s, float *x_bar, float *m_bar,
                                 cudaStream_t st);
+int sph_launch_grad_sum_tile(sph_ctx *ctx, const KPar &kp, const float *a_s, float *g_out, cudaStream_t st);
+int sph_launch_grad_sum_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *ga_s, float *x_bar, float *a_bar,
+                                 cudaStream_t st);
 int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
                         const uint8_t *kind_s, float *drho, float *acc, float4 *out4, cudaStream_t st);
 int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,

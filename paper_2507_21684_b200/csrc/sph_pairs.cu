@@ -142,6 +142,12 @@ __global__ void k_gather_f32(int64_t n, const uint32_t *__restrict__ perm, const
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p < n) out[p] = in[perm[p]];
 }
+__global__ void k_gather_f32_w(int64_t n, const uint32_t *__restrict__ perm, const float *__restrict__ in,
+                               float4 *__restrict__ out)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n) out[p] = make_float4(0.f, 0.f, 0.f, in[perm[p]]);
+}
 
 // ------------------------------------------------------------------------------------------ D: density
 template <int DIM, int GS, bool VARH>
@@ -242,6 +248,83 @@ k_density_vjp(int64_t n, KPar kp, float margin, const float4 *__restrict__ pos_s
             xb_out[i * DIM + 1] = x1;
             if (DIM == 3) xb_out[i * DIM + 2] = x2;
             if (mb_out) mb_out[i] = mb;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ kernel-gradient sum
+// g_i = sum_j a_j G_ij d_ij and its adjoint (include/sph.h sph_grad_sum / sph_grad_sum_vjp; Eq.24)
+template <int DIM>
+__global__ void k_gather_vec_a(int64_t n, const uint32_t *__restrict__ perm, const float *__restrict__ vec,
+                               const float *__restrict__ a, float4 *__restrict__ out)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n) {
+        const int64_t i = perm[p];
+        out[p] = make_float4(vec[i * DIM], vec[i * DIM + 1], DIM == 3 ? vec[i * DIM + 2] : 0.f, a[i]);
+    }
+}
+
+// VJP = false: GA.w = a (xyz unused), writes g;  VJP = true: GA = {g_bar, a}, writes x_bar and a_bar
+template <int DIM, int GS, bool VARH, bool VJP>
+__global__ void __launch_bounds__(kBlock)
+k_grad_sum(int64_t n, KPar kp, float margin, const float4 *__restrict__ pos_s, const float4 *__restrict__ ga_s,
+           const long long *__restrict__ row_ptr, const int32_t *__restrict__ col, const uint32_t *__restrict__ perm,
+           float *__restrict__ v_out, float *__restrict__ a_out)
+{
+    constexpr int kGroups = kBlock / GS;
+    const int g = threadIdx.x / GS, gl = threadIdx.x % GS;
+    const int64_t row0 = (int64_t)blockIdx.x * kGroups * kRowsPerGroup;
+    const HC hu = hc_uniform<DIM>(kp);
+    for (int rr = 0; rr < kRowsPerGroup; ++rr) {
+        const int64_t row = row0 + (int64_t)rr * kGroups + g;
+        if (row >= n) break;
+        const float4 pi = __ldg(pos_s + row);
+        const float4 gi = __ldg(ga_s + row);
+        const float xi[3] = {pi.x, pi.y, pi.z};
+        const bool seam = row_near_seam(xi, kp, margin);
+        const long long b = row_ptr[row], e = row_ptr[row + 1];
+        float x0 = 0.f, x1 = 0.f, x2 = 0.f, ab = 0.f;
+        for (long long p = b + gl; p < e; p += GS) {
+            const int32_t j = __ldg(col + p);
+            const float4 pj = __ldg(pos_s + j);
+            const float4 gj = __ldg(ga_s + j);
+            const float xj[3] = {pj.x, pj.y, pj.z};
+            float d[3], r2;
+            if (seam) rel_pos<DIM, true>(xi, xj, kp, d, r2); else rel_pos<DIM, false>(xi, xj, kp, d, r2);
+            HC hc = hu;
+            if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+            const float q = fast_sqrt(r2) * hc.invH;
+            const float t = fmaxf(1.0f - q, 0.f);
+            const float t2 = t * t, t4 = t2 * t2;
+            const float G = hc.cG * fmaf(5.0f, q, 1.0f) * (t4 * t);                               // Eq.29
+            if (!VJP) {
+                const float c = gj.w * G;
+                x0 = fmaf(c, d[0], x0);
+                x1 = fmaf(c, d[1], x1);
+                if (DIM == 3) x2 = fmaf(c, d[2], x2);
+            } else {
+                const float K = hc.cK * t4;                                                       // Eq.16
+                const float dgi = fmaf(d[2], gi.z, fmaf(d[1], gi.y, d[0] * gi.x));
+                const float dgj = fmaf(d[2], gj.z, fmaf(d[1], gj.y, d[0] * gj.x));
+                const float cG = G * gj.w, cGp = G * gi.w;                    // a_j G, a_i G
+                const float cd = K * fmaf(gj.w, dgi, -(gi.w * dgj));          // K (a_j d.gb_i - a_i d.gb_j)
+                x0 += fmaf(cG, gi.x, fmaf(-cGp, gj.x, cd * d[0]));
+                x1 += fmaf(cG, gi.y, fmaf(-cGp, gj.y, cd * d[1]));
+                if (DIM == 3) x2 += fmaf(cG, gi.z, fmaf(-cGp, gj.z, cd * d[2]));
+                ab = fmaf(-G, dgj, ab);
+            }
+        }
+        x0 = group_sum<GS>(x0);
+        x1 = group_sum<GS>(x1);
+        if (DIM == 3) x2 = group_sum<GS>(x2);
+        if (VJP) ab = group_sum<GS>(ab);
+        if (gl == 0) {
+            const int64_t i = perm[row];
+            v_out[i * DIM] = x0;
+            v_out[i * DIM + 1] = x1;
+            if (DIM == 3) v_out[i * DIM + 2] = x2;
+            if (VJP && a_out) a_out[i] = ab;
         }
     }
 }
@@ -720,6 +803,69 @@ extern "C" int sph_density_vjp(sph_ctx *ctx, const float *m, const float *rho_ba
 #undef SPH_DVJP_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
+}
+
+static int grad_sum_common(sph_ctx *ctx, const float *a, const float *g_bar, float *v_out, float *a_out, bool vjp,
+                           cudaStream_t st)
+{
+    const int64_t n = ctx->n;
+    sph_params dummy{};
+    dummy.c0 = 1.f; dummy.rho0 = 1.f; dummy.gamma = 1.f; dummy.eps = 1.f;
+    KPar kp;
+    SPH_TRY(sph_kpar_make(ctx, &dummy, &kp));
+    KScope ks(ctx, SPH_K_DENSITY, 2, st);
+    const unsigned nb1 = (unsigned)((n + 255) / 256);
+    if (!vjp && ctx->tile_mode) {
+        SPH_TRY(ctx->m_s.reserve((size_t)n * 4));
+        k_gather_f32<<<nb1, 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), a, ctx->m_s.as<float>());
+        return sph_launch_grad_sum_tile(ctx, kp, ctx->m_s.as<float>(), v_out, st);
+    }
+    SPH_TRY(ctx->c0buf.reserve((size_t)n * 16));
+    float4 *ga = ctx->c0buf.as<float4>();
+    // forward on the generic layout: the weights ride in .w of the same float4 record (xyz unused)
+    const float *vec = vjp ? g_bar : nullptr;
+    if (kp.dim == 3) {
+        if (vec) k_gather_vec_a<3><<<nb1, 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), vec, a, ga);
+        else k_gather_f32_w<<<nb1, 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), a, ga);
+    } else {
+        if (vec) k_gather_vec_a<2><<<nb1, 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), vec, a, ga);
+        else k_gather_f32_w<<<nb1, 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), a, ga);
+    }
+    if (ctx->tile_mode) return sph_launch_grad_sum_vjp_tile(ctx, kp, ga, v_out, a_out, st);
+    const float margin = seam_margin(ctx);
+#define SPH_GS_LAUNCH(DIM, GS, VARH, VJP)                                                                             \
+    k_grad_sum<DIM, GS, VARH, VJP><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), ga,   \
+                                                                       ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>(), \
+                                                                       ctx->perm.as<uint32_t>(), v_out, a_out)
+#define SPH_GS_DIM(DIM, GS)                                                                                  \
+    do {                                                                                                     \
+        if (kp.uniform_h) { if (vjp) SPH_GS_LAUNCH(DIM, GS, false, true); else SPH_GS_LAUNCH(DIM, GS, false, false); } \
+        else { if (vjp) SPH_GS_LAUNCH(DIM, GS, true, true); else SPH_GS_LAUNCH(DIM, GS, true, false); }               \
+    } while (0)
+    if (kp.dim == 3) SPH_GS_DIM(3, 32); else SPH_GS_DIM(2, 16);
+#undef SPH_GS_DIM
+#undef SPH_GS_LAUNCH
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+extern "C" int sph_grad_sum(sph_ctx *ctx, const float *a, float *g_out, sph_stream_t stream)
+{
+    if (!ctx || !a || !g_out) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    ctx->last_stream = (cudaStream_t)stream;
+    return grad_sum_common(ctx, a, nullptr, g_out, nullptr, false, (cudaStream_t)stream);
+}
+
+extern "C" int sph_grad_sum_vjp(sph_ctx *ctx, const float *a, const float *g_bar, float *x_bar, float *a_bar,
+                                sph_stream_t stream)
+{
+    if (!ctx || !a || !g_bar || !x_bar) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    ctx->last_stream = (cudaStream_t)stream;
+    return grad_sum_common(ctx, a, g_bar, x_bar, a_bar, true, (cudaStream_t)stream);
 }
 
 extern "C" int sph_rhs(sph_ctx *ctx, const sph_params *par, const float *x, const float *v, const float *rho,

@@ -314,6 +314,86 @@ k_density_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict_
         });
 }
 
+// ------------------------------------------------------------------------------------------ kernel-gradient sum
+// g_i = sum_j a_j G_ij d_ij (VJP = false; smem A = positions, W = a[mcap] in the B slot) and its adjoint (VJP = true;
+// smem A, GA = {g_bar, a}[mcap] in the B slot): include/sph.h sph_grad_sum / sph_grad_sum_vjp; Eq.24
+template <int DIM, int GS, bool VARH, bool VJP>
+__global__ void __launch_bounds__(kPtMaxWarps * 32)
+k_grad_sum_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ pos_s, const float *__restrict__ a_s,
+                const float4 *__restrict__ ga_s, const uint32_t *__restrict__ cell_start,
+                const uint32_t *__restrict__ cell_end, const long long *__restrict__ row_ptr,
+                const uint16_t *__restrict__ col16, const uint32_t *__restrict__ perm, float *__restrict__ v_out,
+                float *__restrict__ a_out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const SmemMap<DIM> sm(smem_raw, ts, false);
+    float *Ws = reinterpret_cast<float *>(sm.B);
+    const float4 *GA = sm.B;
+    __shared__ TileTab tt;
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (tt.T == 0) return;
+    if (VJP) stage_halo(tt, pos_s, sm.A, ga_s, sm.B, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+    else stage_halo(tt, pos_s, sm.A, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, a_s, Ws);
+    stage_rows(tt, row_ptr, sm.rp, sm.selfq);
+    cp_async_wait<0>();
+    __syncthreads();
+    stage_shift<DIM>(tt, sm.A);
+    const int gl = (threadIdx.x & 31) % GS;
+    const HC hu = hc_uniform<DIM>(kp);
+    const float4 *A = sm.A;
+    const uint16_t *selfq = sm.selfq;
+    const uint32_t row0 = tt.row0;
+    tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
+        [&](uint32_t r, bool live, uint32_t b, uint32_t e, const uint16_t *idx) {
+            const uint32_t qi = selfq[r];
+            const float4 pi = A[qi];
+            float4 gi = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (VJP) gi = GA[qi];
+            float x0 = 0.f, x1 = 0.f, x2 = 0.f, ab = 0.f;
+#pragma unroll 2
+            for (uint32_t k = b + gl; k < e; k += GS) {
+                const uint32_t j = idx[k];
+                const float4 pj = A[j];
+                const float d0 = pi.x - pj.x, d1 = pi.y - pj.y, d2 = DIM == 3 ? pi.z - pj.z : 0.f;
+                const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
+                HC hc = hu;
+                if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+                const float q = fast_sqrt(r2) * hc.invH;
+                const float t = fmaxf(1.0f - q, 0.f);
+                const float t2 = t * t, t4 = t2 * t2;
+                const float G = hc.cG * fmaf(5.0f, q, 1.0f) * (t4 * t);                             // Eq.29
+                if (!VJP) {
+                    const float c = Ws[j] * G;
+                    x0 = fmaf(c, d0, x0);
+                    x1 = fmaf(c, d1, x1);
+                    if (DIM == 3) x2 = fmaf(c, d2, x2);
+                } else {
+                    const float4 gj = GA[j];
+                    const float K = hc.cK * t4;                                                     // Eq.16
+                    const float dgi = fmaf(d2, gi.z, fmaf(d1, gi.y, d0 * gi.x));
+                    const float dgj = fmaf(d2, gj.z, fmaf(d1, gj.y, d0 * gj.x));
+                    const float cG = G * gj.w, cGp = G * gi.w;                  // a_j G, a_i G
+                    const float cd = K * fmaf(gj.w, dgi, -(gi.w * dgj));        // K (a_j d.gb_i - a_i d.gb_j)
+                    x0 += fmaf(cG, gi.x, fmaf(-cGp, gj.x, cd * d0));
+                    x1 += fmaf(cG, gi.y, fmaf(-cGp, gj.y, cd * d1));
+                    if (DIM == 3) x2 += fmaf(cG, gi.z, fmaf(-cGp, gj.z, cd * d2));
+                    ab = fmaf(-G, dgj, ab);
+                }
+            }
+            x0 = group_sum<GS>(x0);
+            x1 = group_sum<GS>(x1);
+            if (DIM == 3) x2 = group_sum<GS>(x2);
+            if (VJP) ab = group_sum<GS>(ab);
+            if (gl == 0 && live) {
+                const int64_t i = perm[row0 + r];
+                v_out[i * DIM] = x0;
+                v_out[i * DIM + 1] = x1;
+                if (DIM == 3) v_out[i * DIM + 2] = x2;
+                if (VJP && a_out) a_out[i] = ab;
+            }
+        });
+}
+
 // ------------------------------------------------------------------------------------------ R1: RHS
 // OUT_SORTED: write float4 {a, drho/dt} in sorted order (RK stages); else scatter to the caller's arrays.
 template <int DIM, int GS, bool VARH, bool OUT_SORTED>
@@ -689,6 +769,55 @@ int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s
 #undef SPH_DVT_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
+}
+
+static int launch_grad_sum_tile(sph_ctx *ctx, const KPar &kp, const float *a_s, const float4 *ga_s, float *v_out,
+                                float *a_out, bool vjp, cudaStream_t st)
+{
+    const TileGeom &tg = ctx->tg;
+    const int gs = tile_group(ctx, false);
+    int threads;
+    TileSizes ts;
+    size_t smem;
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);   // carve-up of SmemMap
+#define SPH_GT_LAUNCH(DIM, GS, VARH, VJP)                                                                             \
+    do {                                                                                                              \
+        SPH_TILE_SMEM_ATTR((k_grad_sum_tile<DIM, GS, VARH, VJP>), smem);                                              \
+        k_grad_sum_tile<DIM, GS, VARH, VJP><<<(unsigned)tg.ntiles, threads, smem, st>>>(                              \
+            tg, kp, ts, ctx->pos_s.as<float4>(), a_s, ga_s, ctx->cell_start.as<uint32_t>(),                           \
+            ctx->cell_end.as<uint32_t>(), ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(),                    \
+            ctx->perm.as<uint32_t>(), v_out, a_out);                                                                  \
+    } while (0)
+#define SPH_GT_GS(GS)                                                                                                 \
+    do {                                                                                                              \
+        if (kp.dim == 3) {                                                                                            \
+            if (kp.uniform_h) { if (vjp) SPH_GT_LAUNCH(3, GS, false, true); else SPH_GT_LAUNCH(3, GS, false, false); } \
+            else { if (vjp) SPH_GT_LAUNCH(3, GS, true, true); else SPH_GT_LAUNCH(3, GS, true, false); }                \
+        } else {                                                                                                      \
+            if (kp.uniform_h) { if (vjp) SPH_GT_LAUNCH(2, GS, false, true); else SPH_GT_LAUNCH(2, GS, false, false); } \
+            else { if (vjp) SPH_GT_LAUNCH(2, GS, true, true); else SPH_GT_LAUNCH(2, GS, true, false); }                \
+        }                                                                                                             \
+    } while (0)
+    switch (gs) {
+    case 16: SPH_GT_GS(16); break;
+    case 32: SPH_GT_GS(32); break;
+    default: SPH_GT_GS(8); break;
+    }
+#undef SPH_GT_GS
+#undef SPH_GT_LAUNCH
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_grad_sum_tile(sph_ctx *ctx, const KPar &kp, const float *a_s, float *g_out, cudaStream_t st)
+{
+    return launch_grad_sum_tile(ctx, kp, a_s, nullptr, g_out, nullptr, false, st);
+}
+
+int sph_launch_grad_sum_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *ga_s, float *x_bar, float *a_bar,
+                                 cudaStream_t st)
+{
+    return launch_grad_sum_tile(ctx, kp, nullptr, ga_s, x_bar, a_bar, true, st);
 }
 
 int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,

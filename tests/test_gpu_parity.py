@@ -164,6 +164,31 @@ def test_density_vjp_parity(sph, case):
 
 
 @pytest.mark.parametrize("case", list(CASES))
+def test_grad_sum_and_its_vjp_parity(sph, case):
+    """g_i = sum_j a_j grad_i W_ij and its adjoint (Eq.24)"""
+    wl = CASES[case]()
+    _, dev, _ = build(wl, 1.0, sph)
+    rng = np.random.default_rng(wl.seed + 5)
+    a = (wl.m / wl.rho * (1.0 + 0.1 * rng.normal(size=wl.n))).astype(np.float32)
+    gb = rng.normal(size=(wl.n, wl.dim)).astype(np.float32)
+    lists = oracle_lists(wl)
+    g = sph.grad_sum(torch.from_numpy(a).cuda())
+    g_o = oracle.grad_sum(wl.domain, wl.x, wl.h, a, *lists)
+    # the exact sum cancels on (near-)lattices: normalise by the size of the summed terms as for drho/dt (R10)
+    S = np.zeros(wl.n)
+    np.add.at(S, np.repeat(np.arange(wl.n), np.diff(lists[0])), 1.0)
+    scale = float(np.max(np.abs(a))) * abs(oracle.gfac(0.5 * float(wl.h.min()), float(wl.h.min()), wl.dim)) * 0.5 * float(wl.h.min())
+    eg = float(np.max(np.abs(_np(g) - g_o)) / max(np.max(np.abs(g_o)), 1e-2 * scale * np.max(S)))
+    xb, ab = sph.grad_sum_vjp(torch.from_numpy(a).cuda(), torch.from_numpy(gb).cuda())
+    xo, ao = oracle.grad_sum_vjp(wl.domain, wl.x, wl.h, a, *lists, gb)
+    ex, ea = max_norm_err(_np(xb), xo), max_norm_err(_np(ab), ao)
+    print(f"{case}: grad_sum err {eg:.2e}; vjp err x {ex:.2e} a {ea:.2e}")
+    assert eg < TOL_FWD and ex < TOL_VJP and ea < TOL_VJP
+    xb2, _ = sph.grad_sum_vjp(torch.from_numpy(a).cuda(), torch.from_numpy(gb).cuda(), want_a_bar=False)
+    assert torch.equal(xb, xb2)
+
+
+@pytest.mark.parametrize("case", list(CASES))
 def test_rhs_parity(sph, case):
     wl = CASES[case]()
     _, dev, _ = build(wl, 1.0, sph)
@@ -443,6 +468,22 @@ def test_color_field_loss_gradient_by_chaining_density_and_density_vjp(sph):
     g_o = x1_o + x2_o
     assert abs(L0 - L_o) <= 1e-4 * L_o
     assert max_norm_err(g, g_o) < TOL_VJP
+    # the full loss of PAPER.md:379 Eq.24 adds 1/n sum_i |sum_j m_j/rho_j grad_i W_ij|^2: the kernel-gradient sum with
+    # a = m/rho, chained the same way (gs = G(x; a), gs_bar = 2 gs/n, (x3, a_bar) = G^T, rho_bar = -a_bar m/rho^2)
+    wl.x = x
+    _, dev, _ = build(wl, 1.0, sph)
+    rho = sph.density(dev.m)
+    a_dev = (dev.m / rho).contiguous()
+    gs = sph.grad_sum(a_dev)
+    L24 = float((gs.double() ** 2).sum() / n)
+    x3, a_bar = sph.grad_sum_vjp(a_dev, (2.0 * gs / n).contiguous())
+    x4, _ = sph.density_vjp(dev.m, (-a_bar * dev.m / (rho * rho)).contiguous(), want_m_bar=False)
+    g24 = _np(x3 + x4)
+    gs_o = oracle.grad_sum(dom, x64, h, mp_o, *lists)
+    x3_o, ab_o = oracle.grad_sum_vjp(dom, x64, h, mp_o, *lists, 2.0 * gs_o / n)
+    x4_o, _ = oracle.density_vjp(dom, x64, h, m64, *lists, -ab_o * m64 / rho_o ** 2)
+    assert abs(L24 - float(np.sum(gs_o ** 2) / n)) <= 1e-4 * float(np.sum(gs_o ** 2) / n)
+    assert max_norm_err(g24, x3_o + x4_o) < TOL_VJP
     # a small step against the gradient lowers the loss (step sized to move particles by at most 0.05 dx)
     step = 0.05 * dx / float(np.max(np.abs(g)))
     L1, _ = gpu_loss_and_grad((x - step * g).astype(np.float32))
