@@ -63,7 +63,8 @@ typedef struct {
     float nu;     /* kinematic viscosity                     PAPER.md:83 Eq.6 */
     float eps;    /* regularisation of 1/r^2 relative to H, > 0 */
     float g[3];   /* body force (gravity) */
-    int pressure_form; /* 0 = symmetric Eq.40 (the only form of the CUDA path in this round; others: SPH_E_INVALID) */
+    int pressure_form; /* 0 = symmetric Eq.40: -m_j (p_i/rho_i^2 + p_j/rho_j^2);  1 = -m_j (p_i + p_j)/(rho_i rho_j), the form
+                          the paper's own WCSPH scheme uses;  others: SPH_E_INVALID */
 } sph_params;
 
 enum {

@@ -89,6 +89,7 @@ struct KPar {
     float inv_kappa; // 1/kappa_d
     float visc_nu;  // 2(d+2) nu
     float Bp;       // rho0 c0^2 / gamma
+    int form;       // pressure form: 0 symmetric Eq.40, 1 (p_i+p_j)/(rho_i rho_j)
     int uniform_h;  // all h equal (then the H-dependent constants below are valid)
     float H, invH, cW, cG, cK, ell, e2, eta, kd;
 };

@@ -371,7 +371,10 @@ k_rhs(int64_t n, KPar kp, float margin, const float4 *__restrict__ s0, const flo
             const float dterm = VG * (pi.rho - pj.rho) * (r2 * invR);
             sD = VARH ? fmaf(hc.kd, dterm, sD) : sD + dterm;
             // pressure (Eq.40, symmetric) + viscosity (Eq.7 with the delta-SPH Pi_ij)
-            const float E = -(pj.V * pj.rho) * (pi.P + pj.P);
+            // pressure pair factor e: P_i + P_j (form 0, Eq.40) or (p_i + p_j)/(rho_i rho_j) (form 1)
+            const float epair = kp.form == 0 ? pi.P + pj.P
+                                             : fmaf(pi.P * pi.rho, fast_rcp(pj.rho), pj.P * pj.rho * (visc_i / kp.rho0));
+            const float E = -(pj.V * pj.rho) * epair;
             const float Phi = hc.eta * visc_i * pj.V * s * invR;
             const float cf = (E + Phi) * G;
             a0 = fmaf(cf, d[0], a0);
@@ -433,7 +436,7 @@ k_vjp(int64_t n, KPar kp, float margin, const float4 *__restrict__ s0, const flo
         const bool seam = row_near_seam(pi.x, kp, margin);
         const long long b = row_ptr[row], e = row_ptr[row + 1];
         const float ir_i = 1.0f / pi.rho;
-        float xb[3] = {0.f, 0.f, 0.f}, vb[3] = {0.f, 0.f, 0.f}, rb = 0.f, Z = 0.f;
+        float xb[3] = {0.f, 0.f, 0.f}, vb[3] = {0.f, 0.f, 0.f}, rb = 0.f, Z = 0.f, Zr = 0.f;
         for (long long p = b + gl; p < e; p += GS) {
             const int32_t j = __ldg(col + p);
             const Part pj = load_part<DIM>(s0, s1, s2, j);
@@ -457,7 +460,9 @@ k_vjp(int64_t n, KPar kp, float margin, const float4 *__restrict__ s0, const flo
             const float ir_j = 1.0f / pj.rho;
             const float m_j = pj.V * pj.rho;
             const float drho = pi.rho - pj.rho;
-            const float Psum = pi.P + pj.P;
+            const float W2 = ir_i * ir_j;
+            // pressure pair factor e (see k_rhs): form 1 = (p_i + p_j)/(rho_i rho_j) with p = P rho^2
+            const float Psum = kp.form == 0 ? pi.P + pj.P : fmaf(pi.P * pi.rho, pi.rho, pj.P * pj.rho * pj.rho) * W2;
             float mm = mu_i[0] * d[0];                          // mu_i . d
             mm = fmaf(mu_i[1], d[1], mm);
             if (DIM == 3) mm = fmaf(mu_i[2], d[2], mm);
@@ -495,7 +500,15 @@ k_vjp(int64_t n, KPar kp, float margin, const float4 *__restrict__ s0, const flo
             }
             rb += lam_i * (VjG * s + dif) - mm * G * Phi * ir_i                 // first role of (i<-j)
                   - lam_j * (ADp * ir_i + difp) - mmp * G * Phip * ir_i;         // second role of (j<-i)
-            Z = fmaf(G, m_j * mm + m_i * mmp, Z);               // -dL/dP_i
+            {
+                const float Gzz = G * (m_j * mm + m_i * mmp);
+                if (kp.form == 0) {
+                    Z = fmaf(Gzz, 1.0f, Z);                         // -dL/dP_i
+                } else {
+                    Z = fmaf(Gzz, W2, Z);                           // -dL/dp_i
+                    Zr = fmaf(Gzz, Psum, Zr);                       // explicit 1/(rho_i rho_j) dependence
+                }
+            }
             // ---- scalar parameters, ordered pair (i<-j) only (each ordered pair is owned by one row)
             const float D1 = 2.0f * hc.ell * VjG * drho * u;    // D_ij / (delta c0)
             S_D1 = fmaf(lam_i, D1, S_D1);
@@ -511,11 +524,21 @@ k_vjp(int64_t n, KPar kp, float margin, const float4 *__restrict__ s0, const flo
         }
         rb = group_sum<GS>(rb);
         Z = group_sum<GS>(Z);
+        Zr = group_sum<GS>(Zr);
         if (gl == 0) {
-            rb -= ei.x * Z;                                      // rho_bar_i += Pbar_i dP/drho, Pbar_i = -Z_i
-            T_E += pi.P * Z;
-            T_0 += ei.y * Z;
-            T_g += ei.z * Z;
+            if (kp.form == 0) {
+                rb -= ei.x * Z;                                  // rho_bar_i += Pbar_i dP/drho, Pbar_i = -Z_i
+                T_E += pi.P * Z;
+                T_0 += ei.y * Z;
+                T_g += ei.z * Z;
+            } else {
+                // form 1: the EOS enters through p = P rho^2: dp/drho = (dP/drho + 2 P/rho) rho^2, dp/dtheta = dP/dtheta rho^2
+                const float r2i = pi.rho * pi.rho;
+                rb += fmaf(-(ei.x + 2.0f * pi.P * ir_i) * r2i, Z, ir_i * Zr);
+                T_E += pi.P * r2i * Z;
+                T_0 += ei.y * r2i * Z;
+                T_g += ei.z * r2i * Z;
+            }
             G0 += mu_i[0]; G1 += mu_i[1]; G2 += mu_i[2];
             if (OUT_SORTED) {
                 xb4[row] = make_float4(xb[0], xb[1], xb[2], rb);
@@ -595,10 +618,11 @@ static const double kKappa2 = 2.171239, kKappa3 = 2.207940;
 int sph_kpar_make(const sph_ctx *ctx, const sph_params *par, KPar *kp)
 {
     if (!(par->c0 > 0.f) || !(par->rho0 > 0.f) || !(par->eps > 0.f) || !(par->gamma > 0.f)) return SPH_E_INVALID;
-    if (par->pressure_form != 0) return SPH_E_INVALID;
+    if (par->pressure_form != 0 && par->pressure_form != 1) return SPH_E_INVALID;
     const GridGeom &gg = ctx->geom;
     memset(kp, 0, sizeof(*kp));
     kp->dim = gg.dim;
+    kp->form = par->pressure_form;
     for (int k = 0; k < 3; ++k) {
         kp->periodic[k] = gg.periodic[k];
         kp->L[k] = gg.L[k];

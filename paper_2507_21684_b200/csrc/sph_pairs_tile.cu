@@ -396,7 +396,8 @@ k_grad_sum_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ p
 
 // ------------------------------------------------------------------------------------------ R1: RHS
 // OUT_SORTED: write float4 {a, drho/dt} in sorted order (RK stages); else scatter to the caller's arrays.
-template <int DIM, int GS, bool VARH, bool OUT_SORTED>
+// F1: pressure form 1, (p_i + p_j)/(rho_i rho_j), instead of the symmetric Eq.40
+template <int DIM, int GS, bool VARH, bool OUT_SORTED, bool F1>
 __global__ void __launch_bounds__(kPtMaxWarps * 32)
 k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, const float4 *__restrict__ s1,
            const float2 *__restrict__ s2, const uint8_t *__restrict__ kind_s, const uint32_t *__restrict__ cell_start,
@@ -424,8 +425,10 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
     tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
         [&](uint32_t r, bool live, uint32_t b, uint32_t e, const uint16_t *idx) {
             const Part pi = load_part<DIM>(A, B, C, selfq[r]);
-            const float visc_i = rho0 * fast_rcp(pi.rho);     // rho0/rho_i of the viscous term
+            const float ir_i = fast_rcp(pi.rho);
+            const float visc_i = rho0 * ir_i;                 // rho0/rho_i of the viscous term
             const float ev_u = hu.eta * visc_i;
+            const float Pr_i = pi.P * pi.rho;                 // form 1: p_i/rho_i
             const bool fixed = kind_s[row0 + r] != 0;         // loaded before the pair loop: its latency is hidden
             float sA = 0.f, sD = 0.f, a0 = 0.f, a1 = 0.f, a2 = 0.f;
 #pragma unroll 2
@@ -454,7 +457,8 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                 const float dterm = VG * (pi.rho - pj.rho) * (r2 * invR);
                 sD = VARH ? fmaf(hc.kd, dterm, sD) : sD + dterm;
                 // pressure (Eq.40, symmetric) + viscosity (Eq.7 with the delta-SPH Pi_ij)
-                const float E = -(pj.V * pj.rho) * (pi.P + pj.P);
+                // E = -m_j e,  e = P_i + P_j (Eq.40)  or  (p_i + p_j)/(rho_i rho_j) = (p_i/rho_i + p_j/rho_i)/rho_j
+                const float E = F1 ? -pj.V * fmaf(pj.P * pj.rho * pj.rho, ir_i, Pr_i) : -(pj.V * pj.rho) * (pi.P + pj.P);
                 const float cf = fmaf(ev * pj.V * s, invR, E) * G;
                 a0 = fmaf(cf, d0, a0);
                 a1 = fmaf(cf, d1, a1);
@@ -490,7 +494,7 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
 // are reduced per CTA in a fixed order (B2 stage 1); one CTA = one tile = one partials record.
 constexpr int kNPartT = 12;   // must match kNPart of sph_pairs.cu (k_reduce_params)
 
-template <int DIM, int GS, bool VARH, bool OUT_SORTED>
+template <int DIM, int GS, bool VARH, bool OUT_SORTED, bool F1>
 __global__ void __launch_bounds__(kPtMaxWarps * 32)
 k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, const float4 *__restrict__ s1,
            const float2 *__restrict__ s2, const float4 *__restrict__ cot, const float4 *__restrict__ eos,
@@ -531,7 +535,8 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
             const float m_i = pi.V * pi.rho, Vi = pi.V, Li = lam_i * pi.rho;
             const uint32_t e = live ? e_in : b;                    // padding groups run no pairs (partials stay clean)
             const float ir_i = 1.0f / pi.rho;
-            float xb[3] = {0.f, 0.f, 0.f}, vb[3] = {0.f, 0.f, 0.f}, rb = 0.f, Z = 0.f;
+            const float p_i = pi.P * pi.rho * pi.rho;             // form 1: the pressure itself
+            float xb[3] = {0.f, 0.f, 0.f}, vb[3] = {0.f, 0.f, 0.f}, rb = 0.f, Z = 0.f, Zr = 0.f;
             for (uint32_t k = b + gl; k < e; k += GS) {
                 const uint32_t j = idx[k];
                 const Part pj = load_part<DIM>(A, B, C, j);
@@ -555,7 +560,9 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                 const float ir_j = fast_rcp(pj.rho);
                 const float m_j = pj.V * pj.rho;
                 const float drho = pi.rho - pj.rho;
-                const float Psum = pi.P + pj.P;
+                // pressure pair factor e: E = -m_j e, E' = -m_i e;  e = P_i + P_j (Eq.40) or (p_i + p_j)/(rho_i rho_j)
+                const float W2 = ir_i * ir_j;
+                const float Psum = F1 ? fmaf(pj.P * pj.rho, pj.rho, p_i) * W2 : pi.P + pj.P;
                 float mm = mu_i[0] * d[0];                          // mu_i . d
                 mm = fmaf(mu_i[1], d[1], mm);
                 if (DIM == 3) mm = fmaf(mu_i[2], d[2], mm);
@@ -595,7 +602,13 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                 const float kdu = hc.kd * u;
                 const float y2 = fmaf(fmaf(pj.rho, s, -D), ir_i, kdu);
                 rb = fmaf(G, fmaf(aV, s + kdu, -fmaf(bV, y2, ir_i * q2)), rb);
-                Z = fmaf(G, zz, Z);                                 // -dL/dP_i
+                if (F1) {
+                    const float Gzz = G * zz;
+                    Z = fmaf(Gzz, W2, Z);                           // -dL/dp_i
+                    Zr = fmaf(Gzz, Psum, Zr);                       // explicit 1/(rho_i rho_j) dependence of e
+                } else {
+                    Z = fmaf(G, zz, Z);                             // -dL/dP_i
+                }
                 // ---- scalar parameters, ordered pair (i<-j) only (each ordered pair is owned by one row); the
                 // H-dependent factors (2 ell, ell, H^2) are applied after the loops when h is uniform
                 const float Gdu = G * du;
@@ -618,13 +631,23 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
             }
             rb = group_sum<GS>(rb);
             Z = group_sum<GS>(Z);
+            if (F1) Zr = group_sum<GS>(Zr);
             if (gl == 0 && live) {
                 const uint32_t row = row0 + r;
                 const float4 ei = eos[row];                          // {dP/drho, dP/drho0, dP/dgamma, m}
-                rb -= ei.x * Z;                                      // rho_bar_i += Pbar_i dP/drho, Pbar_i = -Z_i
-                T_E += pi.P * Z;
-                T_0 += ei.y * Z;
-                T_g += ei.z * Z;
+                if (F1) {
+                    // the EOS enters through p = P rho^2: dp/drho = (dP/drho + 2 P/rho) rho^2, dp/dtheta = dP/dtheta rho^2
+                    const float r2i = pi.rho * pi.rho;
+                    rb += fmaf(-(ei.x + 2.0f * pi.P * ir_i) * r2i, Z, ir_i * Zr);
+                    T_E += p_i * Z;
+                    T_0 += ei.y * r2i * Z;
+                    T_g += ei.z * r2i * Z;
+                } else {
+                    rb -= ei.x * Z;                                  // rho_bar_i += Pbar_i dP/drho, Pbar_i = -Z_i
+                    T_E += pi.P * Z;
+                    T_0 += ei.y * Z;
+                    T_g += ei.z * Z;
+                }
                 G0 += mu_i[0]; G1 += mu_i[1]; G2 += mu_i[2];
                 if (OUT_SORTED) {
                     xb4[row] = make_float4(xb[0], xb[1], xb[2], rb);
@@ -830,12 +853,16 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
     size_t smem;
     tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);
     const bool sorted = out4 != nullptr;
-#define SPH_RT_LAUNCH(DIM, GS, VARH, SORTED)                                                                         \
+#define SPH_RT_LAUNCH1(DIM, GS, VARH, SORTED, F1)                                                                    \
     do {                                                                                                             \
-        SPH_TILE_SMEM_ATTR((k_rhs_tile<DIM, GS, VARH, SORTED>), smem);                                               \
-        k_rhs_tile<DIM, GS, VARH, SORTED><<<(unsigned)tg.ntiles, threads, smem, st>>>(                               \
+        SPH_TILE_SMEM_ATTR((k_rhs_tile<DIM, GS, VARH, SORTED, F1>), smem);                                           \
+        k_rhs_tile<DIM, GS, VARH, SORTED, F1><<<(unsigned)tg.ntiles, threads, smem, st>>>(                           \
             tg, kp, ts, s0, s1, s2, kind_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),            \
             ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), drho, acc, out4);     \
+    } while (0)
+#define SPH_RT_LAUNCH(DIM, GS, VARH, SORTED)                                                                         \
+    do {                                                                                                             \
+        if (kp.form == 0) SPH_RT_LAUNCH1(DIM, GS, VARH, SORTED, false); else SPH_RT_LAUNCH1(DIM, GS, VARH, SORTED, true); \
     } while (0)
 #define SPH_RT_GS(GS)                                                                                                   \
     do {                                                                                                                \
@@ -854,6 +881,7 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
     }
 #undef SPH_RT_GS
 #undef SPH_RT_LAUNCH
+#undef SPH_RT_LAUNCH1
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
@@ -869,13 +897,17 @@ int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
     size_t smem;
     tile_launch_cfg(ctx, kp.dim == 3 ? 56 : 48, gs, sizeof(TileTab) + kPtMaxWarps * kNPartT * 4, &threads, &ts, &smem);
     const bool sorted = xb4 != nullptr;
-#define SPH_VT_LAUNCH(DIM, GS, VARH, SORTED)                                                                          \
+#define SPH_VT_LAUNCH1(DIM, GS, VARH, SORTED, F1)                                                                     \
     do {                                                                                                              \
-        SPH_TILE_SMEM_ATTR((k_vjp_tile<DIM, GS, VARH, SORTED>), smem);                                                \
-        k_vjp_tile<DIM, GS, VARH, SORTED><<<(unsigned)tg.ntiles, threads, smem, st>>>(                                \
+        SPH_TILE_SMEM_ATTR((k_vjp_tile<DIM, GS, VARH, SORTED, F1>), smem);                                            \
+        k_vjp_tile<DIM, GS, VARH, SORTED, F1><<<(unsigned)tg.ntiles, threads, smem, st>>>(                            \
             tg, kp, ts, s0, s1, s2, cot, eos, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),           \
             ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), xb, vb, rb, xb4, vb4,  \
             partials);                                                                                                \
+    } while (0)
+#define SPH_VT_LAUNCH(DIM, GS, VARH, SORTED)                                                                          \
+    do {                                                                                                              \
+        if (kp.form == 0) SPH_VT_LAUNCH1(DIM, GS, VARH, SORTED, false); else SPH_VT_LAUNCH1(DIM, GS, VARH, SORTED, true); \
     } while (0)
 #define SPH_VT_GS(GS)                                                                                                   \
     do {                                                                                                                \
@@ -894,6 +926,7 @@ int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
     }
 #undef SPH_VT_GS
 #undef SPH_VT_LAUNCH
+#undef SPH_VT_LAUNCH1
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

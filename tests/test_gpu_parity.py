@@ -132,7 +132,7 @@ def test_error_codes(sph):
     # unsupported pressure form is rejected loudly, not silently computed
     sph.build_cells(wl.domain, dev.x, dev.h)
     sph.neighbors(1.0)
-    par = W.Params(**{**wl.params.__dict__, "pressure_form": 1})
+    par = W.Params(**{**wl.params.__dict__, "pressure_form": 2})
     with pytest.raises(SphError) as e:
         sph.rhs(par, dev.x, dev.v, dev.rho, dev.m, dev.kind)
     assert e.value.code == -1
@@ -200,6 +200,41 @@ def test_rhs_parity(sph, case):
     assert e_d < TOL_FWD and e_a < TOL_FWD
     if wl.kind.any():
         assert np.all(_np(acc)[wl.kind == 1] == 0.0)
+
+
+@pytest.mark.parametrize("case", ["C0p", "C2p", "C3p", "C4s"])
+def test_pressure_form_1_rhs_vjp_and_rk_parity(sph, case):
+    """pressure_form = 1: -m_j (p_i + p_j)/(rho_i rho_j), the form of the paper's own WCSPH scheme (reading
+    R8): RHS, VJP (the EOS then enters through p and through the explicit 1/(rho_i rho_j)) and one RK4 step"""
+    wl = CASES[case]()
+    base = wl.params.__dict__
+    par = W.Params(**{**base, "pressure_form": 1, **({} if case.startswith("C2") else {"alpha": 0.02, "g": (0.3, -0.2, 0.1)})})
+    lam, mu = W.random_cotangents(wl)
+    _, dev, _ = build(wl, 1.0, sph)
+    lists = oracle_lists(wl)
+    drho, acc = sph.rhs(par, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+    d_o, a_o, sd, sa = oracle.rhs(wl.domain, par, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *lists, with_scales=True)
+    assert max_norm_err(_np(drho), d_o, sd) < TOL_FWD and max_norm_err(_np(acc), a_o, sa) < TOL_FWD
+    # the two forms differ (otherwise this test would prove nothing)
+    _, a0 = oracle.rhs(wl.domain, W.Params(**{**par.__dict__, "pressure_form": 0}), wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *lists)
+    if case != "C2p":                            # (hydrostatic densities without noise: the forms nearly coincide)
+        assert np.max(np.abs(a0 - a_o)) > 1e-3 * np.max(np.abs(a_o))
+    xb, vb, rb, pb = sph.rhs_vjp(par, dev.x, dev.v, dev.rho, dev.m, dev.kind, torch.from_numpy(lam).cuda(),
+                                 torch.from_numpy(mu).cuda())
+    xo, vo, ro, po = oracle.rhs_vjp(wl.domain, par, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *lists, lam, mu)
+    errs = dict(x=max_norm_err(_np(xb), xo), v=max_norm_err(_np(vb), vo), rho=max_norm_err(_np(rb), ro))
+    pg = _np(pb).astype(np.float64)
+    pe = np.abs(pg - po) / np.maximum(np.abs(po), 1e-3 * np.max(np.abs(po)) + 1e-30)
+    print(f"{case} form 1: vjp errs {errs} params {np.max(pe):.2e}")
+    assert max(errs.values()) < TOL_VJP and np.max(pe) < TOL_VJP
+    skin = 0.1
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin) * np.float32(1.0001))
+    x, v, rho = dev.x.clone(), dev.v.clone(), dev.rho.clone()
+    sph.rk_step(wl.domain, par, wl.dt, skin, x, v, rho, dev.m, dev.h, dev.kind)
+    xo2, vo2, ro2 = oracle.rk4_step(wl.domain, par, wl.dt, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, method=1)
+    fl = lambda a, b: 2.0 ** -23 * np.max(np.abs(a)) / max(np.max(np.abs(b)), 1e-300)
+    assert max_norm_err(_np(v).astype(np.float64) - wl.v, vo2 - wl.v) < TOL_FWD + fl(wl.v, vo2 - wl.v)
+    assert max_norm_err(_np(rho).astype(np.float64) - wl.rho, ro2 - wl.rho) < TOL_FWD + fl(wl.rho, ro2 - wl.rho)
 
 
 def test_rhs_independent_of_skin(sph):
