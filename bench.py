@@ -188,9 +188,12 @@ def cpu_sample(wl, budget_s=12.0, seed=3):
 
     pairs, dt, nr = run(20000)                       # calibration
     want = int(min(wl.n, max(20000, 20000 * budget_s / max(dt, 1e-3))))
-    pairs, dt, nr = run(want)
+    pairs, dt, nr, passes = 0, 0.0, 0, 0
+    while dt < 0.8 * budget_s and passes < 16:       # a sample capped by the workload size is repeated
+        p1, d1, nr = run(want)
+        pairs, dt, passes = pairs + p1, dt + d1, passes + 1
     return {"value": pairs / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"oracle.rhs + oracle.rhs_vjp (fp64, OpenMP) on {nr} sampled rows of {wl.name} "
+            "sample": f"oracle.rhs + oracle.rhs_vjp (fp64, OpenMP) on {passes} x {nr} sampled rows of {wl.name} "
                       f"({pairs} pair interactions in {dt:.2f} s); oracle grid neighbour search over all "
                       f"{wl.n} particles took {t_lists:.2f} s and is not in the figure"}, (rp, ci)
 
