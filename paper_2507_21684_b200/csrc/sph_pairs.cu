@@ -61,11 +61,14 @@ __device__ __forceinline__ bool row_near_seam(const float *xi, const KPar &kp, f
     return s;
 }
 
+// Sum over the GS lanes that share a row.  The shuffles name only the lanes of the group: groups of one warp leave
+// the row loop at different times (row >= n in the last block), so a full-warp mask would be undefined there.
 template <int GS>
 __device__ __forceinline__ float group_sum(float v)
 {
+    const uint32_t gmask = (0xffffffffu >> (32 - GS)) << ((threadIdx.x & 31u) & ~(uint32_t)(GS - 1));
 #pragma unroll
-    for (int o = GS / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    for (int o = GS / 2; o > 0; o >>= 1) v += __shfl_xor_sync(gmask, v, o);
     return v;
 }
 

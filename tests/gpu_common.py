@@ -3,6 +3,7 @@ import numpy as np
 import torch
 
 import oracle
+from paper_2507_21684_b200 import workloads as W
 from paper_2507_21684_b200.binding import Sph
 
 
@@ -27,3 +28,42 @@ def build(wl, scale=1.0, sph=None, dev=None):
 
 def oracle_lists(wl, scale=1.0, method=1):
     return oracle.neighbors(wl.domain, wl.x, wl.h, search_scale=scale, method=method)
+
+
+def fuzz_workload(seed, scale=None, dt_cfl=0.0):
+    """seeded random small problem: dimension, periodicity per axis, box aspect, clustered positions (some cells empty),
+    uniform or log-normal h, cell size with or without slack, search scale (drawn unless `scale` is given).  dt =
+    dt_cfl * min(h) / c0.  Returns (workload, search_scale)."""
+    rng = np.random.default_rng(1234 + seed)
+    dim = int(rng.integers(2, 4))
+    per = tuple(int(rng.integers(0, 2)) for _ in range(dim)) + (0,) * (3 - dim)
+    Lbox = rng.uniform(0.6, 1.6, size=dim)
+    lo = rng.uniform(-1.0, 1.0, size=dim)
+    n = int(rng.integers(300, 3000))
+    hbar = float(rng.uniform(0.08, 0.16)) * float(Lbox.min())
+    varh = bool(rng.integers(0, 2))
+    h = (hbar * np.exp(rng.normal(0, 0.1, size=n)) if varh else np.full(n, hbar)).astype(np.float32)
+    # clustered positions: a mixture of a uniform background and a few blobs, so that some cells are empty
+    x = rng.uniform(0.0, 1.0, size=(n, dim))
+    nb = n // 2
+    centres = rng.uniform(0.2, 0.8, size=(3, dim))
+    x[:nb] = centres[rng.integers(0, 3, size=nb)] + rng.normal(0, 0.07, size=(nb, dim))
+    x = np.clip(x, 1e-4, 1.0 - 1e-4) * Lbox + lo
+    drawn = float(rng.choice([1.0, 1.15]))
+    scale = drawn if scale is None else float(scale)
+    cell = float(np.float32(h.max()) * np.float32(scale) * np.float32(rng.choice([1.0001, 1.3])))
+    lo3 = tuple(lo) + (0.0,) * (3 - dim)
+    hi3 = tuple(lo + Lbox) + (0.0,) * (3 - dim)
+    if any(per[k] and Lbox[k] / cell < 3.0 for k in range(dim)):
+        cell = float(min(Lbox[k] for k in range(dim) if per[k]) / 3.0001)
+        h = np.minimum(h, np.float32(cell / scale / 1.0001)).astype(np.float32)
+    dom = W.Domain(dim=dim, periodic=per, lo=lo3, hi=hi3, cell_size=cell)
+    base = W.make(3 if dim == 3 else 0, **(dict(n_axis=8) if dim == 3 else {})).params
+    par = W.Params(**{**base.__dict__, "alpha": 0.02, "g": (0.1, -0.2, 0.05)})
+    wl = W.Workload(name=f"fuzz{seed}", domain=dom, params=par, x=x.astype(np.float32),
+                    v=rng.normal(0, 0.3, size=(n, dim)).astype(np.float32),
+                    rho=(1.0 + 0.03 * rng.normal(size=n)).astype(np.float32),
+                    m=(np.full(n, 1.0 / n) * np.exp(rng.normal(0, 0.05, size=n))).astype(np.float32), h=h,
+                    kind=(rng.uniform(size=n) < 0.05).astype(np.uint8), dt=dt_cfl * float(h.min()) / par.c0, dx=0.05,
+                    seed=seed)
+    return wl, scale

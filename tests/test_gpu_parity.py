@@ -9,7 +9,7 @@ import oracle
 from paper_2507_21684_b200 import workloads as W
 from paper_2507_21684_b200.binding import Sph, SphError, OPT_LIST_MODE, OPT_TILE_EDGE, OPT_FILL_MASKS, LIST_GENERIC
 from common import max_norm_err
-from gpu_common import Dev, build, oracle_lists
+from gpu_common import Dev, build, oracle_lists, fuzz_workload
 
 pytestmark = pytest.mark.gpu
 
@@ -702,3 +702,63 @@ def test_rk_steps_with_verlet_lists_reused_across_steps(sph):
     eg = max_norm_err(_np(vb), vo)
     print(f"verlet reuse: {fills} list builds in {nsteps} steps; increments err v {ev:.2e} rho {er:.2e}; gradient err {eg:.2e}")
     assert ev < 2e-4 and er < 2e-4 and eg < TOL_VJP
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_domains_lists_and_rhs(sph, seed):
+    """seeded random small problems (dimension, periodicity per axis, box aspect, clustered positions with empty cells,
+    uniform or log-normal h, cell size with or without slack, search scale): lists bit-exact against the oracle's brute
+    force, RHS and VJP within tolerance -- exercises partial blocks at domain edges, empty cells, seam tiles in one axis
+    only, and halos of very different sizes"""
+    wl, scale = fuzz_workload(seed)
+    dom, par = wl.domain, wl.params
+    _, dev, nnz = build(wl, scale, sph)
+    rp, ci = sph.neighbors_export()
+    rp_o, ci_o = oracle_lists(wl, scale, method=0)
+    assert nnz == int(rp_o[-1]) and np.array_equal(_np(rp), rp_o) and np.array_equal(_np(ci), ci_o)
+    lam, mu = W.random_cotangents(wl)
+    drho, acc = sph.rhs(par, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+    d_o, a_o, sd, sa = oracle.rhs(dom, par, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp_o, ci_o, with_scales=True)
+    assert max_norm_err(_np(drho), d_o, sd) < TOL_FWD and max_norm_err(_np(acc), a_o, sa) < TOL_FWD
+    xb, vb, rb, pb = sph.rhs_vjp(par, dev.x, dev.v, dev.rho, dev.m, dev.kind, torch.from_numpy(lam).cuda(),
+                                 torch.from_numpy(mu).cuda())
+    xo, vo, ro, po = oracle.rhs_vjp(dom, par, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, rp_o, ci_o, lam, mu)
+    assert max(max_norm_err(_np(xb), xo), max_norm_err(_np(vb), vo), max_norm_err(_np(rb), ro)) < TOL_VJP
+    pe = np.abs(_np(pb).astype(np.float64) - po) / np.maximum(np.abs(po), 1e-3 * np.max(np.abs(po)) + 1e-30)
+    assert np.max(pe) < TOL_VJP
+    dens = sph.density(dev.m)
+    assert max_norm_err(_np(dens), oracle.density(dom, wl.x, wl.h, wl.m, rp_o, ci_o)) < TOL_FWD
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_domains_rk_step_and_its_adjoint(sph, seed):
+    """the same random problems through one RK4 step (skin 0.1) and its discrete adjoint, loss = kinetic energy"""
+    skin = 0.1
+    wl, _ = fuzz_workload(100 + seed, scale=1.0 + skin, dt_cfl=0.05)
+    # bounded axes get a margin so that no particle leaves the box within the step, and dt is limited so that the
+    # (unphysical, far from equilibrium) state changes by a few percent only
+    d = wl.domain
+    pad = [0.0 if d.periodic[k] or k >= d.dim else 0.01 for k in range(3)]
+    wl.domain = W.Domain(dim=d.dim, periodic=d.periodic, lo=tuple(d.lo[k] - pad[k] for k in range(3)),
+                         hi=tuple(d.hi[k] + pad[k] for k in range(3)), cell_size=d.cell_size)
+    d0, a0 = oracle.rhs(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *oracle_lists(wl, 1.0, method=0))
+    wl.dt = float(min(wl.dt, 0.02 / np.abs(d0).max(), 0.05 / np.abs(a0).max()))
+    dev = Dev(wl)
+    x, v, rho = dev.x.clone(), dev.v.clone(), dev.rho.clone()
+    sph.rk_step(wl.domain, wl.params, wl.dt, skin, x, v, rho, dev.m, dev.h, dev.kind)
+    xo, vo, ro = oracle.rk4_step(wl.domain, wl.params, wl.dt, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, method=0)
+    fl = lambda a, b: 2.0 ** -23 * np.max(np.abs(a)) / max(np.max(np.abs(b)), 1e-300)
+    assert max_norm_err(_np(x).astype(np.float64) - wl.x, xo - wl.x) < TOL_FWD + fl(wl.x, xo - wl.x)
+    assert max_norm_err(_np(v).astype(np.float64) - wl.v, vo - wl.v) < TOL_FWD + fl(wl.v, vo - wl.v)
+    assert max_norm_err(_np(rho).astype(np.float64) - wl.rho, ro - wl.rho) < TOL_FWD + fl(wl.rho, ro - wl.rho)
+    xb = torch.zeros_like(x)
+    vb = (dev.m[:, None] * v).contiguous()
+    rb = torch.zeros_like(rho)
+    pb = torch.zeros(10, device="cuda")
+    sph.rk_step_vjp(wl.domain, wl.params, wl.dt, skin, dev.x, dev.v, dev.rho, dev.m, dev.h, dev.kind, xb, vb, rb, pb)
+    gx, gv, gr, gp = oracle.rk4_step_vjp(wl.domain, wl.params, wl.dt, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind,
+                                         np.zeros_like(vo), wl.m.astype(np.float64)[:, None] * vo, np.zeros(wl.n), method=0)
+    errs = dict(x=max_norm_err(_np(xb), gx), v=max_norm_err(_np(vb), gv), rho=max_norm_err(_np(rb), gr))
+    pe = np.abs(_np(pb).astype(np.float64) - gp) / np.maximum(np.abs(gp), 1e-3 * np.max(np.abs(gp)) + 1e-30)
+    print(f"fuzz rk {seed}: errs {errs} params {np.max(pe):.2e}")
+    assert max(errs.values()) < TOL_VJP and np.max(pe) < TOL_VJP
