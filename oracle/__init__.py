@@ -161,6 +161,24 @@ def density_vjp(domain, x, h, m, row_ptr, col_idx, rho_bar):
     return xb, mb
 
 
+def renorm_gradient(domain, x, h, vol, A, row_ptr, col_idx, rcond=1e-4):
+    """Kernel renormalisation (Eq.44, Eq.45): L_i = [sum_j V_j (x_j - x_i) (x) grad_i W_ij]^+ and the
+    corrected gradient <grad A>_i = sum_j V_j (A_j - A_i) L_i grad_i W_ij.  The pseudo-inverse is the Moore-Penrose
+    inverse with eigenvalues below rcond * (largest |eigenvalue|) dropped (numpy.linalg.pinv; the matrix is symmetric
+    because grad W is parallel to x_i - x_j).  Returns (L [n,d,d], grad [n,d], M [n,d,d])."""
+    dim, per, lo, hi = _dom(domain)
+    x, h, vol, A = _d(x), _d(h), _d(vol), _d(A)
+    n = x.shape[0]
+    M = np.empty((n, dim, dim), dtype=np.float64)
+    b = np.empty((n, dim), dtype=np.float64)
+    lib().orc_renorm_moments(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(x), _p(h), _p(vol), _p(A),
+                             _p(np.ascontiguousarray(row_ptr, np.int64)), _p(np.ascontiguousarray(col_idx, np.int32)),
+                             _p(M), _p(b))
+    L = np.linalg.pinv(M, rcond=rcond, hermitian=True)
+    grad = np.einsum("nkl,nl->nk", L, b)
+    return L, grad, M
+
+
 def rhs(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, rows=None, with_scales=False, par_raw=None):
     dim, per, lo, hi = _dom(domain)
     par = _par(params) if par_raw is None else par_raw

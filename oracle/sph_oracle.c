@@ -23,6 +23,9 @@
  *                                 sum x_bar = 0
  *   orc_density_vjp             : central finite differences of orc_density (x and m), sum x_bar = 0, two-particle
  *                                 closed form, zero on a lattice with uniform rho_bar
+ *   orc_renorm_moments (+ numpy pinv in renorm_gradient): linear fields reproduced exactly on disordered / free-surface /
+ *                                 varying-h particles, L M = I, M rebuilt from central differences of orc_w, M ~ I on a
+ *                                 full lattice, x^2 exact on symmetric neighbourhoods, rank-1 line and isolated particle
  *   orc_rhs                     : momentum conservation, Galilean / rigid rotation invariance, uniform
  *                                 compression, Brookshaw Laplacian of |x|^2, hydrostatic column, viscous symbol
  *   orc_rhs_vjp                 : central finite differences of orc_rhs (x, v, rho, all 10 scalars),
@@ -463,6 +466,45 @@ void orc_grad_sum_vjp(int64_t n, int dim, const int *periodic, const double *lo,
                 x_bar[j * dim + k] -= D;
             }
         }
+    }
+    free(xw);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * NEXT-2, first part: kernel renormalisation, Eq.44, Eq.45.  With V_j = m_j/rho_j
+ * passed in as `vol`, and grad_i W_ij = G_ij d_ij, d_ij = x_i - x_j (Eq.29):
+ *      M_i = sum_j V_j (x_j - x_i) (x) grad_i W_ij          the matrix Eq.45 inverts,   L_i = M_i^+
+ *      b_i = sum_j V_j (A_j - A_i) grad_i W_ij               so that Eq.44 reads  <grad A>_i = L_i b_i
+ * This routine only accumulates the two sums (M row-major d x d, b); the pseudo-inverse of Eq.45 ("commonly performed
+ * as a pseudo-inverse") is numpy.linalg.pinv in oracle/__init__.py renorm_gradient().
+ * ------------------------------------------------------------------------------------------ */
+void orc_renorm_moments(int64_t n, int dim, const int *periodic, const double *lo, const double *hi,
+                        const double *x, const double *h, const double *vol, const double *A,
+                        const int64_t *row_ptr, const int32_t *col_idx, double *M_out, double *b_out)
+{
+    double L[3];
+    box_len(dim, lo, hi, L);
+    double *xw = (double *)malloc((size_t)n * dim * sizeof(double));
+    wrap64(n, dim, periodic, lo, hi, x, xw);
+    for (int64_t i = 0; i < n; ++i) {
+        double M[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, b[3] = {0, 0, 0};
+        for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
+            int64_t j = col_idx[p];
+            double d[3] = {0, 0, 0};
+            for (int k = 0; k < dim; ++k) d[k] = xw[i * dim + k] - xw[j * dim + k];
+            min_image(d, dim, periodic, L);
+            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            double H = h[i] > h[j] ? h[i] : h[j];
+            double G = orc_gfac(r, H, dim);
+            for (int k = 0; k < dim; ++k) {
+                double gw = G * d[k];                                   /* component k of grad_i W_ij */
+                for (int l = 0; l < dim; ++l) M[l][k] += vol[j] * (-d[l]) * gw;   /* (x_j - x_i)_l (grad W)_k */
+                b[k] += vol[j] * (A[j] - A[i]) * gw;
+            }
+        }
+        for (int l = 0; l < dim; ++l)
+            for (int k = 0; k < dim; ++k) M_out[(i * dim + l) * dim + k] = M[l][k];
+        for (int k = 0; k < dim; ++k) b_out[i * dim + k] = b[k];
     }
     free(xw);
 }

@@ -30,7 +30,7 @@ def oracle_lists(wl, scale=1.0, method=1):
     return oracle.neighbors(wl.domain, wl.x, wl.h, search_scale=scale, method=method)
 
 
-def fuzz_workload(seed, scale=None, dt_cfl=0.0):
+def fuzz_workload(seed, scale=None, dt_cfl=0.0, tiny=False):
     """seeded random small problem: dimension, periodicity per axis, box aspect, clustered positions (some cells empty),
     uniform or log-normal h, cell size with or without slack, search scale (drawn unless `scale` is given).  dt =
     dt_cfl * min(h) / c0.  Returns (workload, search_scale)."""
@@ -40,6 +40,8 @@ def fuzz_workload(seed, scale=None, dt_cfl=0.0):
     Lbox = rng.uniform(0.6, 1.6, size=dim)
     lo = rng.uniform(-1.0, 1.0, size=dim)
     n = int(rng.integers(300, 3000))
+    if tiny:
+        n = 1 + n % 40
     hbar = float(rng.uniform(0.08, 0.16)) * float(Lbox.min())
     varh = bool(rng.integers(0, 2))
     h = (hbar * np.exp(rng.normal(0, 0.1, size=n)) if varh else np.full(n, hbar)).astype(np.float32)

@@ -709,8 +709,8 @@ def test_random_domains_lists_and_rhs(sph, seed):
     """seeded random small problems (dimension, periodicity per axis, box aspect, clustered positions with empty cells,
     uniform or log-normal h, cell size with or without slack, search scale): lists bit-exact against the oracle's brute
     force, RHS and VJP within tolerance -- exercises partial blocks at domain edges, empty cells, seam tiles in one axis
-    only, and halos of very different sizes"""
-    wl, scale = fuzz_workload(seed)
+    only, and halos of very different sizes; the last seeds have between 1 and 40 particles"""
+    wl, scale = fuzz_workload(seed, tiny=seed >= 12)
     dom, par = wl.domain, wl.params
     _, dev, nnz = build(wl, scale, sph)
     rp, ci = sph.neighbors_export()
@@ -728,6 +728,19 @@ def test_random_domains_lists_and_rhs(sph, seed):
     assert np.max(pe) < TOL_VJP
     dens = sph.density(dev.m)
     assert max_norm_err(_np(dens), oracle.density(dom, wl.x, wl.h, wl.m, rp_o, ci_o)) < TOL_FWD
+    # the NEXT rows on the same lists: density adjoint, kernel-gradient sum and its adjoint
+    rng = np.random.default_rng(seed + 31)
+    rbar = rng.normal(size=wl.n).astype(np.float32)
+    a = (wl.m / wl.rho * (1.0 + 0.1 * rng.normal(size=wl.n))).astype(np.float32)
+    gbar = rng.normal(size=(wl.n, wl.dim)).astype(np.float32)
+    xb, mb = sph.density_vjp(dev.m, torch.from_numpy(rbar).cuda())
+    xo, mo = oracle.density_vjp(dom, wl.x, wl.h, wl.m, rp_o, ci_o, rbar)
+    assert max_norm_err(_np(xb), xo) < TOL_VJP and max_norm_err(_np(mb), mo) < TOL_VJP
+    g = sph.grad_sum(torch.from_numpy(a).cuda())
+    assert max_norm_err(_np(g), oracle.grad_sum(dom, wl.x, wl.h, a, rp_o, ci_o)) < TOL_FWD   # disordered: no cancellation
+    xb, ab = sph.grad_sum_vjp(torch.from_numpy(a).cuda(), torch.from_numpy(gbar).cuda())
+    xo, ao = oracle.grad_sum_vjp(dom, wl.x, wl.h, a, rp_o, ci_o, gbar)
+    assert max_norm_err(_np(xb), xo) < TOL_VJP and max_norm_err(_np(ab), ao) < TOL_VJP
 
 
 @pytest.mark.parametrize("seed", range(8))

@@ -626,3 +626,103 @@ def test_rk4_vjp_against_finite_differences_of_kinetic_energy():
     xb0, vb0, _, _ = oracle.rk4_step_vjp(wl.domain, wl.params, 1e-9, x0, v0, r0, wl.m, wl.h, wl.kind,
                                          np.zeros_like(x0), m[:, None] * v0, np.zeros_like(r0), method=0)
     assert np.max(np.abs(vb0 - m[:, None] * v0)) < 1e-6 * np.max(np.abs(m[:, None] * v0))
+
+
+# ------------------------------------------------------------------------------------------ kernel renormalisation (NEXT-2, Eq.44/45)
+def _renorm_inputs(cfg, kw, amp=0.3, open_box=False):
+    wl = W.perturbed(W.make(cfg, **kw), amp_x=amp, amp_rho=0.03)
+    if open_box:
+        # same particles in an open box: the faces become free surfaces (incomplete support)
+        d = wl.domain
+        wl.domain = W.Domain(dim=d.dim, periodic=(0, 0, 0), lo=d.lo, hi=d.hi, cell_size=d.cell_size)
+    rp, ci = oracle.neighbors(wl.domain, wl.x, wl.h)
+    vol = wl.m.astype(np.float64) / wl.rho.astype(np.float64)
+    return wl, rp, ci, vol
+
+
+@pytest.mark.parametrize("cfg,kw", [(2, dict(dx=0.06)), (4, dict(n_axis=9))])
+def test_renorm_gradient_is_exact_for_linear_fields(cfg, kw):
+    """the point of Eq.44/45: with L_i the corrected gradient of a LINEAR field is exact for any
+    particle arrangement with full-rank neighbourhoods -- free surfaces, walls, disorder, varying h, any weights"""
+    wl, rp, ci, vol = _renorm_inputs(cfg, kw, open_box=True)
+    x = wl.x.astype(np.float64)
+    g = np.array([0.7, -1.3, 0.45])[: wl.dim]
+    A = 2.5 + x @ g
+    L, grad, M = oracle.renorm_gradient(wl.domain, x, wl.h, vol, A, rp, ci, rcond=1e-9)
+    rank_ok = np.linalg.cond(M) < 1e6
+    assert rank_ok.sum() > 0.9 * wl.n
+    assert np.max(np.abs(grad[rank_ok] - g)) < 1e-9
+    # and L M = I there; M is symmetric (grad W is parallel to x_i - x_j)
+    assert np.max(np.abs(np.einsum("nab,nbc->nac", L[rank_ok], M[rank_ok]) - np.eye(wl.dim))) < 1e-8
+    assert np.max(np.abs(M - np.swapaxes(M, 1, 2))) < 1e-14 * np.max(np.abs(M))
+
+
+def test_renorm_matrix_against_differences_of_the_kernel():
+    """M_i (Eq.45 before inversion) rebuilt for a few particles from central differences of W itself (orc_w, pinned by
+    quadrature above) instead of the gradient factor: fixes the sign, the weights V_j and the (x_j - x_i) (x) grad order"""
+    wl, rp, ci, vol = _renorm_inputs(1, dict(n_axis=16))
+    x = wl.x.astype(np.float64)
+    A = np.sin(3.0 * x[:, 0]) + x[:, 1] ** 2
+    _, _, M = oracle.renorm_gradient(wl.domain, x, wl.h, vol, A, rp, ci)
+    Lbox = np.array(wl.domain.hi[:2]) - np.array(wl.domain.lo[:2])
+    eps = 1e-6
+    for i in (0, 57, 200):
+        Mi = np.zeros((2, 2))
+        bi = np.zeros(2)
+        for j in ci[rp[i]:rp[i + 1]]:
+            d = x[i] - x[j]
+            d -= Lbox * np.round(d / Lbox)                         # minimum image (C1 is periodic)
+            H = float(max(wl.h[i], wl.h[j]))
+            gw = np.array([(oracle.w(float(np.linalg.norm(d + e)), H, 2) - oracle.w(float(np.linalg.norm(d - e)), H, 2)) / (2 * eps)
+                           for e in (np.array([eps, 0.0]), np.array([0.0, eps]))])
+            Mi += vol[j] * np.outer(-d, gw)
+            bi += vol[j] * (A[j] - A[i]) * gw
+        assert np.max(np.abs(Mi - M[i])) < 1e-7 * np.max(np.abs(M[i]))
+        L, grad, _ = oracle.renorm_gradient(wl.domain, x, wl.h, vol, A, rp, ci)
+        assert np.max(np.abs(np.linalg.solve(Mi, bi) - grad[i])) < 1e-6 * np.max(np.abs(grad[i]))
+
+
+def test_renorm_matrix_is_near_identity_on_a_full_lattice_and_quadratics_are_exact_there():
+    """continuum limit: -int (x'-x) (x) grad W dV = I (integration by parts), so on a full periodic lattice with V = dx^d
+    M ~ I; and on a point-symmetric neighbourhood the odd moments vanish, so the corrected gradient of x^2 is 2x exactly"""
+    for cfg, kw in ((0, {}), (3, dict(n_axis=12))):
+        wl = W.make(cfg, **kw)
+        rp, ci = oracle.neighbors(wl.domain, wl.x, wl.h)
+        x = wl.x.astype(np.float64)
+        vol = np.full(wl.n, wl.dx ** wl.dim)
+        lo, hi = np.array(wl.domain.lo[: wl.dim]), np.array(wl.domain.hi[: wl.dim])
+        A = x[:, 0] ** 2
+        L, grad, M = oracle.renorm_gradient(wl.domain, x, wl.h, vol, A, rp, ci)
+        assert np.max(np.abs(M - np.eye(wl.dim))) < 2e-2
+        # rows away from the periodic seam (where x^2 jumps)
+        Hmax = float(wl.h.max())
+        inner = np.all((x - lo > Hmax) & (hi - x > Hmax), axis=1)
+        assert inner.sum() > 0
+        want = np.zeros_like(x)
+        want[:, 0] = 2.0 * x[:, 0]
+        assert np.max(np.abs(grad[inner] - want[inner])) < 1e-6      # lattice positions are binary32: symmetric to 6e-8
+
+
+def test_renorm_pseudo_inverse_on_rank_deficient_neighbourhoods():
+    """Eq.45 "performed as a pseudo-inverse": particles on a straight line in 2D have a rank-1 M; the pseudo-inverse gives
+    the gradient ALONG the line exactly and nothing across it; an isolated particle gets L = 0"""
+    dom = W.Domain(dim=2, periodic=(0, 0, 0), lo=(0.0, 0.0, 0.0), hi=(2.0, 2.0, 0.0), cell_size=0.4)
+    tdir = np.array([0.6, 0.8])
+    s = np.array([0.0, 0.11, 0.2, 0.33, 0.41, 0.55])
+    x = np.vstack([np.array([0.5, 0.5]) + np.outer(s, tdir), [[1.8, 0.2]]])
+    n = len(x)
+    h = np.full(n, 0.4, np.float32)
+    rp, ci = oracle.neighbors(dom, x.astype(np.float32), h)
+    x = x.astype(np.float32).astype(np.float64)
+    g = np.array([1.5, -0.5])
+    A = x @ g
+    vol = np.full(n, 0.01)
+    L, grad, M = oracle.renorm_gradient(dom, x, h, vol, A, rp, ci, rcond=1e-4)
+    assert rp[n] - rp[n - 1] == 1 and np.all(L[n - 1] == 0.0) and np.all(grad[n - 1] == 0.0)
+    # direction of the line as stored in binary32 positions
+    t = x[5] - x[0]
+    t /= np.linalg.norm(t)
+    nrm = np.array([-t[1], t[0]])
+    for i in range(6):
+        assert np.max(np.abs(L[i] @ nrm)) < 1e-5 * np.max(np.abs(L[i]))
+        assert abs(grad[i] @ t - g @ t) < 1e-5 and abs(grad[i] @ nrm) < 1e-5
