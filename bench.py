@@ -364,8 +364,11 @@ def main():
     # kernel-gradient sum and its adjoint (gradient term of the shifting loss, Eq.24), a = m/rho
     a_dev = (m / rho).contiguous()
     gs_dev, ab_dev = torch.empty_like(x), torch.empty_like(rho)
+    # kernel renormalisation (Eq.44/45): L_i and the corrected density gradient, V = m/rho
+    L_dev = torch.empty((x.shape[0], x.shape[1], x.shape[1]), dtype=torch.float32, device=x.device)
     for name, call in (("grad_sum", lambda: sph.grad_sum(a_dev, gs_dev)),
-                       ("grad_sum_vjp", lambda: sph.grad_sum_vjp(a_dev, mu, xb_dev, ab_dev))):
+                       ("grad_sum_vjp", lambda: sph.grad_sum_vjp(a_dev, mu, xb_dev, ab_dev)),
+                       ("renorm_gradient", lambda: sph.renorm_gradient(a_dev, rho, 1e-4, L_dev, gs_dev))):
         call()
         e0, e1 = ev(), ev()
         e0.record()

@@ -126,6 +126,19 @@ int sph_grad_sum(sph_ctx *ctx, const float *a, float *g_out, sph_stream_t stream
 int sph_grad_sum_vjp(sph_ctx *ctx, const float *a, const float *g_bar, float *x_bar, float *a_bar,
                      sph_stream_t stream);
 
+/* Kernel renormalisation, Eq.44 and Eq.45, on the lists of the last sph_neighbors and at the build
+ * positions: with V_j = vol[j] (the caller passes m_j/rho_j) and grad_i W_ij = G_ij (x_i - x_j),
+ *     L_i = [ sum_j V_j (x_j - x_i) (x) grad_i W_ij ]^+                 (Eq.45; the matrix is symmetric)
+ *     <grad A>_i = sum_j V_j (A_j - A_i) L_i grad_i W_ij                  (Eq.44)
+ * ^+ is the Moore-Penrose inverse taken by eigen-decomposition: eigenvalues with |lambda| <= rcond * max|lambda| are
+ * dropped ("commonly performed as a pseudo-inverse for numerical stability"), so a particle without
+ * neighbours gets L = 0 and particles on a line / in a plane get the gradient within it.  0 <= rcond < 1.
+ * vol, A: device float[n] in caller order.  L_out: device float[n*d*d], row-major d x d per particle, or NULL;
+ * grad_out: device float[n*d] or NULL (not both NULL).  All buffers stay owned by the caller.  Forward only: the adjoint
+ * of this operation is not part of the library.  Returns SPH_E_INVALID on bad arguments, SPH_E_STATE without lists. */
+int sph_renorm_gradient(sph_ctx *ctx, const float *vol, const float *A, float rcond, float *L_out, float *grad_out,
+                        sph_stream_t stream);
+
 /* One right-hand-side evaluation (formulas at the top of this file) on the lists of the last sph_neighbors.
  * x may differ from the build positions (RK stages) as long as the list is still a superset of the true
  * neighbours: pairs with r >= H_ij contribute exactly 0 (kernel clamp).  h is the one given to sph_build_cells. */

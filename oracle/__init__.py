@@ -179,6 +179,35 @@ def renorm_gradient(domain, x, h, vol, A, row_ptr, col_idx, rcond=1e-4):
     return L, grad, M
 
 
+def renorm_gradient_vjp(domain, x, h, vol, A, row_ptr, col_idx, grad_bar, rcond=1e-4):
+    """(x_bar, vol_bar, A_bar) = J^T grad_bar of the corrected gradient of renorm_gradient(), adjacency fixed.
+    Per particle, with g = L b, L = M^+ (symmetric), P = M L the projector on the range of M:
+        b_bar = L g_bar,   L_bar = g_bar b^T,
+        M_bar = -L L_bar L + (I - P) L_bar L L        (differential of the pseudo-inverse at constant rank,
+              = -b_bar g^T + ((I - P) g_bar) (L g)^T    Golub & Pereyra 1973; the third term of that formula
+                                                         vanishes because b lies in the range of M)
+    then the pair terms by orc_renorm_moments_vjp."""
+    dim, per, lo, hi = _dom(domain)
+    x, h, vol, A, gb = _d(x), _d(h), _d(vol), _d(A), _d(grad_bar)
+    n = x.shape[0]
+    rp = np.ascontiguousarray(row_ptr, np.int64)
+    ci = np.ascontiguousarray(col_idx, np.int32)
+    L, g, M = renorm_gradient(domain, x, h, vol, A, rp, ci, rcond=rcond)
+    bbar = np.einsum("nkl,nl->nk", L, gb)
+    P = np.einsum("nkl,nlm->nkm", M, L)
+    c = gb - np.einsum("nkl,nl->nk", P, gb)
+    u = np.einsum("nkl,nl->nk", L, g)
+    Mbar = -np.einsum("nk,nl->nkl", bbar, g) + np.einsum("nk,nl->nkl", c, u)
+    Mbar = np.ascontiguousarray(Mbar)
+    bbar = np.ascontiguousarray(bbar)
+    xb = np.empty((n, dim), dtype=np.float64)
+    vb = np.empty(n, dtype=np.float64)
+    ab = np.empty(n, dtype=np.float64)
+    lib().orc_renorm_moments_vjp(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(x), _p(h), _p(vol), _p(A),
+                                 _p(rp), _p(ci), _p(Mbar), _p(bbar), _p(xb), _p(vb), _p(ab))
+    return xb, vb, ab
+
+
 def rhs(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, rows=None, with_scales=False, par_raw=None):
     dim, per, lo, hi = _dom(domain)
     par = _par(params) if par_raw is None else par_raw

@@ -26,6 +26,9 @@
  *   orc_renorm_moments (+ numpy pinv in renorm_gradient): linear fields reproduced exactly on disordered / free-surface /
  *                                 varying-h particles, L M = I, M rebuilt from central differences of orc_w, M ~ I on a
  *                                 full lattice, x^2 exact on symmetric neighbourhoods, rank-1 line and isolated particle
+ *   orc_renorm_moments_vjp (+ the pseudo-inverse adjoint in renorm_gradient_vjp): central differences of renorm_gradient
+ *                                 w.r.t. x (random direction, single components), vol and A on 2D/3D/varying-h/wall cases and
+ *                                 on a rank-1 line (constant-rank term), sum x_bar = 0, sum A_bar = 0
  *   orc_rhs                     : momentum conservation, Galilean / rigid rotation invariance, uniform
  *                                 compression, Brookshaw Laplacian of |x|^2, hydrostatic column, viscous symbol
  *   orc_rhs_vjp                 : central finite differences of orc_rhs (x, v, rho, all 10 scalars),
@@ -505,6 +508,58 @@ void orc_renorm_moments(int64_t n, int dim, const int *periodic, const double *l
         for (int l = 0; l < dim; ++l)
             for (int k = 0; k < dim; ++k) M_out[(i * dim + l) * dim + k] = M[l][k];
         for (int k = 0; k < dim; ++k) b_out[i * dim + k] = b[k];
+    }
+    free(xw);
+}
+
+/* Reverse mode of orc_renorm_moments, term by term with the adjacency held fixed ("fully supports
+ * backpropagation through this operation as well").  Given the cotangents Mbar_i (d x d, row-major, of
+ * M_i) and bbar_i (of b_i), and with  d(G d) = G dd + K (d . dd) d  (Eq.16), every ordered pair
+ * (i <- j) of the list contributes, with d = x_i - x_j, dA = A_j - A_i, a = d^T Mbar_i d, be = bbar_i . d:
+ *      M_i term  -V_j G d d^T :   vol_bar_j += -G a ;   F += -V_j [ K a d + G (Mbar_i + Mbar_i^T) d ]
+ *      b_i term   V_j dA G d  :   vol_bar_j += dA G be ; A_bar_j += V_j G be ; A_bar_i -= V_j G be ;
+ *                                 F += V_j dA [ K be d + G bbar_i ]
+ *      x_bar_i += F ,  x_bar_j -= F .
+ * The adjoint of the pseudo-inverse itself is taken in oracle/__init__.py renorm_gradient_vjp(). */
+void orc_renorm_moments_vjp(int64_t n, int dim, const int *periodic, const double *lo, const double *hi,
+                            const double *x, const double *h, const double *vol, const double *A,
+                            const int64_t *row_ptr, const int32_t *col_idx, const double *Mbar, const double *bbar,
+                            double *x_bar, double *vol_bar, double *A_bar)
+{
+    double L[3];
+    box_len(dim, lo, hi, L);
+    double *xw = (double *)malloc((size_t)n * dim * sizeof(double));
+    wrap64(n, dim, periodic, lo, hi, x, xw);
+    for (int64_t i = 0; i < n * dim; ++i) x_bar[i] = 0.0;
+    for (int64_t i = 0; i < n; ++i) vol_bar[i] = A_bar[i] = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        const double *Mb = Mbar + i * dim * dim, *bb = bbar + i * dim;
+        for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
+            int64_t j = col_idx[p];
+            double d[3] = {0, 0, 0};
+            for (int k = 0; k < dim; ++k) d[k] = xw[i * dim + k] - xw[j * dim + k];
+            min_image(d, dim, periodic, L);
+            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            double H = h[i] > h[j] ? h[i] : h[j];
+            double G = orc_gfac(r, H, dim), K = orc_kfac(r, H, dim);
+            double dA = A[j] - A[i];
+            double a = 0.0, be = 0.0, Nd[3] = {0, 0, 0};
+            for (int k = 0; k < dim; ++k) {
+                be += bb[k] * d[k];
+                for (int l = 0; l < dim; ++l) {
+                    a += d[k] * Mb[k * dim + l] * d[l];
+                    Nd[k] += (Mb[k * dim + l] + Mb[l * dim + k]) * d[l];
+                }
+            }
+            vol_bar[j] += -G * a + dA * G * be;
+            A_bar[j] += vol[j] * G * be;
+            A_bar[i] -= vol[j] * G * be;
+            for (int k = 0; k < dim; ++k) {
+                double F = -vol[j] * (K * a * d[k] + G * Nd[k]) + vol[j] * dA * (K * be * d[k] + G * bb[k]);
+                x_bar[i * dim + k] += F;
+                x_bar[j * dim + k] -= F;
+            }
+        }
     }
     free(xw);
 }

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsph_b200.so")
 
 EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph_neighbors_export", "sph_density",
-           "sph_density_vjp", "sph_lists_valid", "sph_grad_sum", "sph_grad_sum_vjp",
+           "sph_density_vjp", "sph_lists_valid", "sph_grad_sum", "sph_grad_sum_vjp", "sph_renorm_gradient",
            "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
            "sph_check", "sph_strerror", "sph_get_info", "sph_get_layout", "sph_profile_enable", "sph_profile_read",
            "sph_set_option")
@@ -69,6 +69,7 @@ def load_library(path: str = LIB_PATH):
     lib.sph_density_vjp.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.sph_grad_sum.argtypes = [vp, vp, vp, vp]
     lib.sph_grad_sum_vjp.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.sph_renorm_gradient.argtypes = [vp, vp, vp, C.c_float, vp, vp, vp]
     lib.sph_lists_valid.argtypes = [vp, vp, f32, C.POINTER(C.c_int32), C.POINTER(f32), vp]
     lib.sph_rhs.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 7 + [vp]
     lib.sph_rhs_vjp.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 11 + [vp]
@@ -218,6 +219,16 @@ class Sph:
         self._chk(self.lib.sph_grad_sum_vjp(self._ctx, _ptr(a), _ptr(g_bar), _ptr(x_bar),
                                             _ptr(a_bar) if a_bar is not None else None, _stream()))
         return x_bar, a_bar
+
+    def renorm_gradient(self, vol, A, rcond=1e-4, L=None, grad=None, want_L=True):
+        """(L [n,d,d], grad [n,d]): renormalisation matrix and corrected gradient of the scalar field A"""
+        vol, A = _f32(vol, (self.n,)), _f32(A, (self.n,))
+        if L is None and want_L:
+            L = torch.empty((self.n, self.dim, self.dim), dtype=torch.float32, device=A.device)
+        grad = torch.empty((self.n, self.dim), dtype=torch.float32, device=A.device) if grad is None else _f32(grad, (self.n, self.dim))
+        self._chk(self.lib.sph_renorm_gradient(self._ctx, _ptr(vol), _ptr(A), C.c_float(rcond),
+                                               _ptr(L) if L is not None else None, _ptr(grad), _stream()))
+        return L, grad
 
     def rhs(self, params, x, v, rho, m, kind, drho_dt=None, acc=None):
         p = make_params(params)

@@ -332,6 +332,166 @@ k_grad_sum(int64_t n, KPar kp, float margin, const float4 *__restrict__ pos_s, c
     }
 }
 
+// ------------------------------------------------------------------------------------------ kernel renormalisation
+// PAPER.md:524-528 Eq.44/45 (include/sph.h sph_renorm_gradient).  The pair pass accumulates the symmetric matrix
+// M_i = sum_j V_j (x_j - x_i) (x) grad_i W_ij = -sum_j V_j G_ij d d^T and b_i = sum_j V_j (A_j - A_i) G_ij d into a
+// sorted-order record of kRenormRec<DIM> float4 per row; k_renorm_solve then takes L_i = M_i^+ and L_i b_i with one
+// thread per particle (the eigen-solve would otherwise serialise on one lane of every row group).
+// record: 3D {xx,xy,xz,yy} {yz,zz,b0,b1} {b2,-,-,-};  2D {xx,xy,yy,b0} {b1,-,-,-}
+template <int DIM, int GS, bool VARH>
+__global__ void __launch_bounds__(kBlock)
+k_renorm(int64_t n, KPar kp, float margin, const float4 *__restrict__ pos_s, const float2 *__restrict__ va_s,
+         const long long *__restrict__ row_ptr, const int32_t *__restrict__ col, float4 *__restrict__ mom)
+{
+    constexpr int kGroups = kBlock / GS;
+    const int g = threadIdx.x / GS, gl = threadIdx.x % GS;
+    const int64_t row0 = (int64_t)blockIdx.x * kGroups * kRowsPerGroup;
+    const HC hu = hc_uniform<DIM>(kp);
+    for (int rr = 0; rr < kRowsPerGroup; ++rr) {
+        const int64_t row = row0 + (int64_t)rr * kGroups + g;
+        if (row >= n) break;
+        const float4 pi = __ldg(pos_s + row);
+        const float Ai = __ldg(va_s + row).y;
+        const float xi[3] = {pi.x, pi.y, pi.z};
+        const bool seam = row_near_seam(xi, kp, margin);
+        const long long b = row_ptr[row], e = row_ptr[row + 1];
+        float mxx = 0.f, mxy = 0.f, mxz = 0.f, myy = 0.f, myz = 0.f, mzz = 0.f, b0 = 0.f, b1 = 0.f, b2 = 0.f;
+        for (long long p = b + gl; p < e; p += GS) {
+            const int32_t j = __ldg(col + p);
+            const float4 pj = __ldg(pos_s + j);
+            const float2 aj = __ldg(va_s + j);                  // {V_j, A_j}
+            const float xj[3] = {pj.x, pj.y, pj.z};
+            float d[3], r2;
+            if (seam) rel_pos<DIM, true>(xi, xj, kp, d, r2); else rel_pos<DIM, false>(xi, xj, kp, d, r2);
+            HC hc = hu;
+            if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+            const float q = fast_sqrt(r2) * hc.invH;
+            const float t = fmaxf(1.0f - q, 0.f);
+            const float t2 = t * t, t4 = t2 * t2;
+            const float G = hc.cG * fmaf(5.0f, q, 1.0f) * (t4 * t);                               // Eq.29
+            const float c = aj.x * G, dA = aj.y - Ai;
+            const float c0 = c * d[0], c1 = c * d[1], c2 = c * d[2];
+            mxx = fmaf(-c0, d[0], mxx);
+            mxy = fmaf(-c0, d[1], mxy);
+            myy = fmaf(-c1, d[1], myy);
+            b0 = fmaf(c0, dA, b0);
+            b1 = fmaf(c1, dA, b1);
+            if (DIM == 3) {
+                mxz = fmaf(-c0, d[2], mxz);
+                myz = fmaf(-c1, d[2], myz);
+                mzz = fmaf(-c2, d[2], mzz);
+                b2 = fmaf(c2, dA, b2);
+            }
+        }
+        mxx = group_sum<GS>(mxx); mxy = group_sum<GS>(mxy); myy = group_sum<GS>(myy);
+        b0 = group_sum<GS>(b0); b1 = group_sum<GS>(b1);
+        if (DIM == 3) {
+            mxz = group_sum<GS>(mxz); myz = group_sum<GS>(myz); mzz = group_sum<GS>(mzz); b2 = group_sum<GS>(b2);
+        }
+        if (gl == 0) {
+            if (DIM == 3) {
+                mom[row * 3] = make_float4(mxx, mxy, mxz, myy);
+                mom[row * 3 + 1] = make_float4(myz, mzz, b0, b1);
+                mom[row * 3 + 2] = make_float4(b2, 0.f, 0.f, 0.f);
+            } else {
+                mom[row * 2] = make_float4(mxx, mxy, myy, b0);
+                mom[row * 2 + 1] = make_float4(b1, 0.f, 0.f, 0.f);
+            }
+        }
+    }
+}
+
+// Moore-Penrose inverse of a symmetric matrix by its eigen-decomposition: eigenvalues with |lambda| <= rcond * max|lambda|
+// are dropped ("pseudo-inverse for numerical stability"; explicit in 2D as in the paper, cyclic Jacobi in 3D)
+__device__ __forceinline__ void jacobi_rotate(float &app, float &aqq, float &apq, float &arp, float &arq,
+                                              float (&V)[3][3], int p, int q)
+{
+    if (fabsf(apq) <= 1e-30f) return;
+    const float theta = (aqq - app) / (2.0f * apq);
+    const float t = copysignf(1.0f, theta) / (fabsf(theta) + sqrtf(fmaf(theta, theta, 1.0f)));
+    const float c = rsqrtf(fmaf(t, t, 1.0f)), s = t * c;
+    app = fmaf(-t, apq, app);
+    aqq = fmaf(t, apq, aqq);
+    apq = 0.f;
+    const float rp = arp, rq = arq;                             // the third row/column r
+    arp = c * rp - s * rq;
+    arq = s * rp + c * rq;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const float vp = V[k][p], vq = V[k][q];
+        V[k][p] = c * vp - s * vq;
+        V[k][q] = s * vp + c * vq;
+    }
+}
+
+template <int DIM>
+__global__ void k_renorm_solve(int64_t n, const float4 *__restrict__ mom, const uint32_t *__restrict__ perm, float rcond,
+                               float *__restrict__ L_out, float *__restrict__ grad_out)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const int64_t i = perm[p];
+    if (DIM == 2) {
+        const float4 r0 = mom[p * 2];
+        const float a = r0.x, b = r0.y, c = r0.z, b0 = r0.w, b1 = mom[p * 2 + 1].x;
+        const float hd = 0.5f * (a - c), rad = sqrtf(fmaf(hd, hd, b * b)), mid = 0.5f * (a + c);
+        const float l0 = mid + rad, l1 = mid - rad;
+        // unit eigenvector of l0: (cos, sin) of half the angle of (a - c, 2b)
+        float cs = 1.f, sn = 0.f;
+        if (rad > 0.f) {
+            const float cx = hd / rad, sx = b / rad;            // cos, sin of the full angle
+            // the larger of the two from the half-angle formula (no cancellation), the other from sin(2p) = 2 sin cos
+            if (cx >= 0.f) {
+                cs = sqrtf(0.5f * (1.0f + cx));
+                sn = sx / (2.0f * cs);
+            } else {
+                sn = copysignf(sqrtf(0.5f * (1.0f - cx)), b);
+                cs = sx / (2.0f * sn);
+            }
+        }
+        const float cut = rcond * fmaxf(fabsf(l0), fabsf(l1));
+        const float i0 = fabsf(l0) > cut ? 1.0f / l0 : 0.f, i1 = fabsf(l1) > cut ? 1.0f / l1 : 0.f;
+        const float Lxx = i0 * cs * cs + i1 * sn * sn, Lxy = (i0 - i1) * cs * sn, Lyy = i0 * sn * sn + i1 * cs * cs;
+        if (L_out) {
+            L_out[i * 4] = Lxx; L_out[i * 4 + 1] = Lxy; L_out[i * 4 + 2] = Lxy; L_out[i * 4 + 3] = Lyy;
+        }
+        if (grad_out) {
+            grad_out[i * 2] = fmaf(Lxx, b0, Lxy * b1);
+            grad_out[i * 2 + 1] = fmaf(Lxy, b0, Lyy * b1);
+        }
+    } else {
+        const float4 r0 = mom[p * 3], r1 = mom[p * 3 + 1];
+        float axx = r0.x, axy = r0.y, axz = r0.z, ayy = r0.w, ayz = r1.x, azz = r1.y;
+        const float bb[3] = {r1.z, r1.w, mom[p * 3 + 2].x};
+        float V[3][3] = {{1.f, 0.f, 0.f}, {0.f, 1.f, 0.f}, {0.f, 0.f, 1.f}};
+#pragma unroll 1
+        for (int sweep = 0; sweep < 6; ++sweep) {
+            jacobi_rotate(axx, ayy, axy, axz, ayz, V, 0, 1);
+            jacobi_rotate(axx, azz, axz, axy, ayz, V, 0, 2);
+            jacobi_rotate(ayy, azz, ayz, axy, axz, V, 1, 2);
+        }
+        const float lam[3] = {axx, ayy, azz};
+        const float cut = rcond * fmaxf(fabsf(lam[0]), fmaxf(fabsf(lam[1]), fabsf(lam[2])));
+        float L[3][3] = {{0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}};
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const float inv = fabsf(lam[k]) > cut ? 1.0f / lam[k] : 0.f;
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) L[r][c] = fmaf(inv * V[r][k], V[c][k], L[r][c]);
+        }
+        if (L_out)
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) L_out[i * 9 + r * 3 + c] = L[r][c];
+        if (grad_out)
+#pragma unroll
+            for (int r = 0; r < 3; ++r) grad_out[i * 3 + r] = fmaf(L[r][0], bb[0], fmaf(L[r][1], bb[1], L[r][2] * bb[2]));
+    }
+}
+
 // ------------------------------------------------------------------------------------------ R1: RHS
 // OUT_SORTED: write float4 {a, drho/dt} in sorted order (RK stages); else scatter to the caller's arrays.
 template <int DIM, int GS, bool VARH, bool OUT_SORTED>
@@ -893,6 +1053,43 @@ extern "C" int sph_grad_sum_vjp(sph_ctx *ctx, const float *a, const float *g_bar
     SPH_CUDA_TRY(cudaSetDevice(ctx->device));
     ctx->last_stream = (cudaStream_t)stream;
     return grad_sum_common(ctx, a, g_bar, x_bar, a_bar, true, (cudaStream_t)stream);
+}
+
+extern "C" int sph_renorm_gradient(sph_ctx *ctx, const float *vol, const float *A, float rcond, float *L_out,
+                                   float *grad_out, sph_stream_t stream)
+{
+    if (!ctx || !vol || !A || (!L_out && !grad_out) || !(rcond >= 0.f) || !(rcond < 1.f)) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    const int64_t n = ctx->n;
+    sph_params dummy{};
+    dummy.c0 = 1.f; dummy.rho0 = 1.f; dummy.gamma = 1.f; dummy.eps = 1.f;
+    KPar kp;
+    SPH_TRY(sph_kpar_make(ctx, &dummy, &kp));
+    SPH_TRY(ctx->s2.reserve((size_t)n * 8));
+    SPH_TRY(ctx->c0buf.reserve((size_t)n * 48));
+    float2 *va_s = ctx->s2.as<float2>();
+    float4 *mom = ctx->c0buf.as<float4>();
+    KScope ks(ctx, SPH_K_DENSITY, 3, st);
+    const unsigned nb1 = (unsigned)((n + 255) / 256);
+    k_gather_f32x2<<<nb1, 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), vol, A, va_s);
+    if (ctx->tile_mode) {
+        SPH_TRY(sph_launch_renorm_tile(ctx, kp, va_s, mom, st));
+    } else {
+        const float margin = seam_margin(ctx);
+#define SPH_RN_LAUNCH(DIM, GS, VARH)                                                                             \
+    k_renorm<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), va_s,  \
+                                                                ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>(), mom)
+        if (kp.dim == 3) { if (kp.uniform_h) SPH_RN_LAUNCH(3, 32, false); else SPH_RN_LAUNCH(3, 32, true); }
+        else { if (kp.uniform_h) SPH_RN_LAUNCH(2, 16, false); else SPH_RN_LAUNCH(2, 16, true); }
+#undef SPH_RN_LAUNCH
+    }
+    if (kp.dim == 3) k_renorm_solve<3><<<nb1, 256, 0, st>>>(n, mom, ctx->perm.as<uint32_t>(), rcond, L_out, grad_out);
+    else k_renorm_solve<2><<<nb1, 256, 0, st>>>(n, mom, ctx->perm.as<uint32_t>(), rcond, L_out, grad_out);
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
 }
 
 extern "C" int sph_rhs(sph_ctx *ctx, const sph_params *par, const float *x, const float *v, const float *rho,

@@ -314,6 +314,84 @@ k_density_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict_
         });
 }
 
+// ------------------------------------------------------------------------------------------ kernel renormalisation
+// moments of PAPER.md:524-528 Eq.44/45: M_i = -sum_j V_j G_ij d d^T (symmetric) and b_i = sum_j V_j (A_j - A_i) G_ij d,
+// written as a sorted-order record (3D: 3 float4, 2D: 2 float4; layout in sph_pairs.cu) for k_renorm_solve.
+// smem: A = {x,y,z,h}[mcap], VA = {V, A}[mcap] (in the B slot), rp, selfq, ring
+template <int DIM, int GS, bool VARH>
+__global__ void __launch_bounds__(kPtMaxWarps * 32)
+k_renorm_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ pos_s, const float2 *__restrict__ va_s,
+              const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
+              const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16, float4 *__restrict__ mom)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const SmemMap<DIM> sm(smem_raw, ts, false);
+    float2 *VA = reinterpret_cast<float2 *>(sm.B);
+    __shared__ TileTab tt;
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (tt.T == 0) return;
+    stage_halo(tt, pos_s, sm.A, nullptr, nullptr, nullptr, nullptr, va_s, VA, nullptr, nullptr);
+    stage_rows(tt, row_ptr, sm.rp, sm.selfq);
+    cp_async_wait<0>();
+    __syncthreads();
+    stage_shift<DIM>(tt, sm.A);
+    const int gl = (threadIdx.x & 31) % GS;
+    const HC hu = hc_uniform<DIM>(kp);
+    const float4 *A = sm.A;
+    const uint16_t *selfq = sm.selfq;
+    const uint32_t row0 = tt.row0;
+    tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
+        [&](uint32_t r, bool live, uint32_t b, uint32_t e, const uint16_t *idx) {
+            const uint32_t qi = selfq[r];
+            const float4 pi = A[qi];
+            const float Ai = VA[qi].y;
+            float mxx = 0.f, mxy = 0.f, mxz = 0.f, myy = 0.f, myz = 0.f, mzz = 0.f, b0 = 0.f, b1 = 0.f, b2 = 0.f;
+#pragma unroll 2
+            for (uint32_t k = b + gl; k < e; k += GS) {
+                const uint32_t j = idx[k];
+                const float4 pj = A[j];
+                const float2 aj = VA[j];                           // {V_j, A_j}
+                const float d0 = pi.x - pj.x, d1 = pi.y - pj.y, d2 = DIM == 3 ? pi.z - pj.z : 0.f;
+                const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
+                HC hc = hu;
+                if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+                const float q = fast_sqrt(r2) * hc.invH;
+                const float t = fmaxf(1.0f - q, 0.f);
+                const float t2 = t * t, t4 = t2 * t2;
+                const float G = hc.cG * fmaf(5.0f, q, 1.0f) * (t4 * t);                             // Eq.29
+                const float c = aj.x * G, dA = aj.y - Ai;
+                const float c0 = c * d0, c1 = c * d1, c2 = c * d2;
+                mxx = fmaf(-c0, d0, mxx);
+                mxy = fmaf(-c0, d1, mxy);
+                myy = fmaf(-c1, d1, myy);
+                b0 = fmaf(c0, dA, b0);
+                b1 = fmaf(c1, dA, b1);
+                if (DIM == 3) {
+                    mxz = fmaf(-c0, d2, mxz);
+                    myz = fmaf(-c1, d2, myz);
+                    mzz = fmaf(-c2, d2, mzz);
+                    b2 = fmaf(c2, dA, b2);
+                }
+            }
+            mxx = group_sum<GS>(mxx); mxy = group_sum<GS>(mxy); myy = group_sum<GS>(myy);
+            b0 = group_sum<GS>(b0); b1 = group_sum<GS>(b1);
+            if (DIM == 3) {
+                mxz = group_sum<GS>(mxz); myz = group_sum<GS>(myz); mzz = group_sum<GS>(mzz); b2 = group_sum<GS>(b2);
+            }
+            if (gl == 0 && live) {
+                const size_t row = (size_t)row0 + r;
+                if (DIM == 3) {
+                    mom[row * 3] = make_float4(mxx, mxy, mxz, myy);
+                    mom[row * 3 + 1] = make_float4(myz, mzz, b0, b1);
+                    mom[row * 3 + 2] = make_float4(b2, 0.f, 0.f, 0.f);
+                } else {
+                    mom[row * 2] = make_float4(mxx, mxy, myy, b0);
+                    mom[row * 2 + 1] = make_float4(b1, 0.f, 0.f, 0.f);
+                }
+            }
+        });
+}
+
 // ------------------------------------------------------------------------------------------ kernel-gradient sum
 // g_i = sum_j a_j G_ij d_ij (VJP = false; smem A = positions, W = a[mcap] in the B slot) and its adjoint (VJP = true;
 // smem A, GA = {g_bar, a}[mcap] in the B slot): include/sph.h sph_grad_sum / sph_grad_sum_vjp; Eq.24
@@ -790,6 +868,37 @@ int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s
     }
 #undef SPH_DVT_GS
 #undef SPH_DVT_LAUNCH
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float2 *va_s, float4 *mom, cudaStream_t st)
+{
+    const TileGeom &tg = ctx->tg;
+    const int gs = tile_group(ctx, false);
+    int threads;
+    TileSizes ts;
+    size_t smem;
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);   // carve-up of SmemMap
+#define SPH_RNT_LAUNCH(DIM, GS, VARH)                                                                                 \
+    do {                                                                                                              \
+        SPH_TILE_SMEM_ATTR((k_renorm_tile<DIM, GS, VARH>), smem);                                                     \
+        k_renorm_tile<DIM, GS, VARH><<<(unsigned)tg.ntiles, threads, smem, st>>>(                                     \
+            tg, kp, ts, ctx->pos_s.as<float4>(), va_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),  \
+            ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), mom);                                            \
+    } while (0)
+#define SPH_RNT_GS(GS)                                                                                      \
+    do {                                                                                                    \
+        if (kp.dim == 3) { if (kp.uniform_h) SPH_RNT_LAUNCH(3, GS, false); else SPH_RNT_LAUNCH(3, GS, true); } \
+        else { if (kp.uniform_h) SPH_RNT_LAUNCH(2, GS, false); else SPH_RNT_LAUNCH(2, GS, true); }             \
+    } while (0)
+    switch (gs) {
+    case 16: SPH_RNT_GS(16); break;
+    case 32: SPH_RNT_GS(32); break;
+    default: SPH_RNT_GS(8); break;
+    }
+#undef SPH_RNT_GS
+#undef SPH_RNT_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

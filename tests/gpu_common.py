@@ -69,3 +69,30 @@ def fuzz_workload(seed, scale=None, dt_cfl=0.0, tiny=False):
                     kind=(rng.uniform(size=n) < 0.05).astype(np.uint8), dt=dt_cfl * float(h.min()) / par.c0, dx=0.05,
                     seed=seed)
     return wl, scale
+
+
+def renorm_errors(L_gpu, grad_gpu, L_o, grad_o, M_o, rcond):
+    """Per-row errors of the renormalisation outputs against the oracle, for the rows where the comparison is meaningful.
+    The pseudo-inverse takes a rank decision (eigenvalue against rcond * largest): rows with an eigenvalue within a
+    factor 3 of the cutoff are left out (fp32 and fp64 may decide differently there; both results are valid).
+    What fp32 bounds is the ABSOLUTE error of the sums M_i, b_i, about 1e-6 of the size a full neighbourhood gives
+    them (as for drho/dt, reading R10: sums are judged against the size of the summed terms).  The inverse turns it
+    into a relative error dL/|L| ~ dM / lambda_min, so a row is measured against its own size times
+        amp_i = max(1, s_i / (50 lambda_min_i)),   s_i = max(lambda_max_i, half the median lambda_max),
+    i.e. the plain bar for rows with condition number <= 50 and a typical M; a row whose few neighbours all sit at the
+    very edge of the support (M_i orders of magnitude below typical, (1-q)^5 cancelling in fp32) is relaxed in
+    proportion.  Returns (err_L, err_grad, rows compared)."""
+    lam = np.abs(np.linalg.eigvalsh(M_o))
+    lmax = np.maximum(lam.max(axis=1), 1e-300)
+    ratio = lam / lmax[:, None]
+    near = np.any((ratio > rcond / 3.0) & (ratio < rcond * 3.0), axis=1)
+    lmin = np.where(ratio > rcond, lam, np.inf).min(axis=1)                # smallest retained eigenvalue
+    s_i = np.maximum(lmax, 0.5 * np.median(lmax))
+    amp = np.maximum(1.0, s_i / (50.0 * lmin))          # rows without a retained eigenvalue (L = 0 exactly): amp = 1
+    ok = ~near
+    sL = np.abs(L_o).reshape(len(L_o), -1).max(axis=1)
+    sL = np.maximum(np.maximum(sL, np.median(sL)), 1e-300)
+    eL = np.abs(L_gpu.astype(np.float64) - L_o).reshape(len(L_o), -1).max(axis=1) / (sL * amp)
+    sg = np.maximum(np.maximum(np.abs(grad_o).max(axis=1), np.median(np.abs(grad_o).max(axis=1))), 1e-300)
+    eg = np.abs(grad_gpu.astype(np.float64) - grad_o).max(axis=1) / (sg * amp)
+    return float(eL[ok].max()), float(eg[ok].max()), int(ok.sum())

@@ -9,7 +9,7 @@ import oracle
 from paper_2507_21684_b200 import workloads as W
 from paper_2507_21684_b200.binding import Sph, SphError, OPT_LIST_MODE, OPT_TILE_EDGE, OPT_FILL_MASKS, LIST_GENERIC
 from common import max_norm_err
-from gpu_common import Dev, build, oracle_lists, fuzz_workload
+from gpu_common import Dev, build, oracle_lists, fuzz_workload, renorm_errors
 
 pytestmark = pytest.mark.gpu
 
@@ -186,6 +186,61 @@ def test_grad_sum_and_its_vjp_parity(sph, case):
     assert eg < TOL_FWD and ex < TOL_VJP and ea < TOL_VJP
     xb2, _ = sph.grad_sum_vjp(torch.from_numpy(a).cuda(), torch.from_numpy(gb).cuda(), want_a_bar=False)
     assert torch.equal(xb, xb2)
+
+
+def _renorm_field(wl):
+    """vol = m/rho and a smooth, periodic, nowhere-constant scalar field on top of the density (the paper's use of Eq.44
+    is the renormalised density gradient of the delta-term)"""
+    lo, hi = np.array(wl.domain.lo[: wl.dim]), np.array(wl.domain.hi[: wl.dim])
+    xi = (wl.x.astype(np.float64) - lo) / (hi - lo)
+    A = wl.rho * (1.0 + 0.2 * np.sin(2 * np.pi * xi[:, 0]) * np.cos(2 * np.pi * xi[:, 1]))
+    return (wl.m / wl.rho).astype(np.float32), A.astype(np.float32)
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_renorm_gradient_parity(sph, case):
+    """renormalisation matrix L_i and corrected gradient (Eq.44/45)"""
+    wl = CASES[case]()
+    _, dev, _ = build(wl, 1.0, sph)
+    vol, A = _renorm_field(wl)
+    rcond = 1e-4
+    L, grad = sph.renorm_gradient(torch.from_numpy(vol).cuda(), torch.from_numpy(A).cuda(), rcond)
+    L_o, g_o, M_o = oracle.renorm_gradient(wl.domain, wl.x, wl.h, vol, A, *oracle_lists(wl), rcond=rcond)
+    eL, eg, rows = renorm_errors(_np(L), _np(grad), L_o, g_o, M_o, rcond)
+    print(f"{case}: renorm err L {eL:.2e} grad {eg:.2e} on {rows}/{wl.n} rows")
+    assert rows > 0.99 * wl.n and eL < TOL_FWD and eg < TOL_FWD
+    # either output is optional, and the result does not depend on which are asked for
+    _, g2 = sph.renorm_gradient(torch.from_numpy(vol).cuda(), torch.from_numpy(A).cuda(), rcond, want_L=False)
+    assert torch.equal(grad, g2)
+
+
+def test_renorm_gradient_rank_deficient_neighbourhoods(sph):
+    """particles on a line in 2D (rank 1), in a plane in 3D (rank 2), and an isolated particle (L = 0)"""
+    rng = np.random.default_rng(5)
+    for dim in (2, 3):
+        dom = W.Domain(dim=dim, periodic=(0, 0, 0), lo=(0.0,) * 3, hi=(2.0, 2.0, 2.0 if dim == 3 else 0.0), cell_size=0.4)
+        if dim == 2:
+            pts = np.array([0.5, 0.5]) + np.outer(np.sort(rng.uniform(0, 0.6, 9)), np.array([0.6, 0.8]))
+            far = [[1.8, 0.2]]
+        else:
+            uv = rng.uniform(0, 0.5, size=(14, 2))
+            pts = np.array([0.5, 0.5, 0.5]) + np.outer(uv[:, 0], [1.0, 0.0, 0.0]) + np.outer(uv[:, 1], [0.0, 0.6, 0.8])
+            far = [[1.8, 0.2, 1.7]]
+        x = np.vstack([pts, far]).astype(np.float32)
+        n = len(x)
+        wl = W.Workload(name="rank", domain=dom, params=W.Params(), x=x, v=0 * x, rho=np.ones(n, np.float32),
+                        m=np.full(n, 0.01, np.float32), h=np.full(n, 0.4, np.float32), kind=np.zeros(n, np.uint8),
+                        dt=0.0, dx=0.1, seed=0)
+        build(wl, 1.0, sph)
+        A = (x.astype(np.float64) @ np.array([1.5, -0.5, 0.8])[:dim]).astype(np.float32)
+        vol = np.full(n, 0.01, np.float32)
+        L, grad = sph.renorm_gradient(torch.from_numpy(vol).cuda(), torch.from_numpy(A).cuda(), 1e-3)
+        L_o, g_o, M_o = oracle.renorm_gradient(dom, x, wl.h, vol, A, *oracle_lists(wl, method=0), rcond=1e-3)
+        assert np.linalg.matrix_rank(M_o[0], tol=1e-6 * np.abs(M_o[0]).max()) == dim - 1
+        assert np.all(_np(L)[n - 1] == 0.0) and np.all(_np(grad)[n - 1] == 0.0)
+        eL, eg, rows = renorm_errors(_np(L), _np(grad), L_o, g_o, M_o, 1e-3)
+        print(f"rank-deficient {dim}D: err L {eL:.2e} grad {eg:.2e} rows {rows}/{n}")
+        assert rows == n and eL < TOL_FWD and eg < TOL_FWD
 
 
 @pytest.mark.parametrize("case", list(CASES))
@@ -741,6 +796,11 @@ def test_random_domains_lists_and_rhs(sph, seed):
     xb, ab = sph.grad_sum_vjp(torch.from_numpy(a).cuda(), torch.from_numpy(gbar).cuda())
     xo, ao = oracle.grad_sum_vjp(dom, wl.x, wl.h, a, rp_o, ci_o, gbar)
     assert max_norm_err(_np(xb), xo) < TOL_VJP and max_norm_err(_np(ab), ao) < TOL_VJP
+    vol, A = _renorm_field(wl)
+    L, grad = sph.renorm_gradient(torch.from_numpy(vol).cuda(), torch.from_numpy(A).cuda(), 1e-4)
+    L_o, g_o, M_o = oracle.renorm_gradient(dom, wl.x, wl.h, vol, A, rp_o, ci_o, rcond=1e-4)
+    eL, eg, rows = renorm_errors(_np(L), _np(grad), L_o, g_o, M_o, 1e-4)
+    assert rows > 0.9 * wl.n and eL < TOL_FWD and eg < TOL_FWD
 
 
 @pytest.mark.parametrize("seed", range(8))

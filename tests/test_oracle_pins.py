@@ -726,3 +726,69 @@ def test_renorm_pseudo_inverse_on_rank_deficient_neighbourhoods():
     for i in range(6):
         assert np.max(np.abs(L[i] @ nrm)) < 1e-5 * np.max(np.abs(L[i]))
         assert abs(grad[i] @ t - g @ t) < 1e-5 and abs(grad[i] @ nrm) < 1e-5
+
+
+def _renorm_vjp_fd(wl, rp, ci, vol, A, gb, rcond, eps_x):
+    """dot products of the oracle's adjoint with random directions against central differences of the forward"""
+    rng = np.random.default_rng(11)
+    x = wl.x.astype(np.float64)
+    xb, vb, ab = oracle.renorm_gradient_vjp(wl.domain, x, wl.h, vol, A, rp, ci, gb, rcond)
+    loss = lambda xx, vv, aa: float(np.sum(gb * oracle.renorm_gradient(wl.domain, xx, wl.h, vv, aa, rp, ci, rcond)[1]))
+    out = {}
+    dx = rng.normal(size=x.shape)
+    out["x"] = ((loss(x + eps_x * dx, vol, A) - loss(x - eps_x * dx, vol, A)) / (2 * eps_x), float(np.sum(xb * dx)))
+    dv = rng.normal(size=wl.n) * vol
+    out["vol"] = ((loss(x, vol + 1e-6 * dv, A) - loss(x, vol - 1e-6 * dv, A)) / 2e-6, float(np.sum(vb * dv)))
+    da = rng.normal(size=wl.n)
+    out["A"] = ((loss(x, vol, A + 1e-6 * da) - loss(x, vol, A - 1e-6 * da)) / 2e-6, float(np.sum(ab * da)))
+    # single components too (a random direction could hide a transposed index)
+    for i, k in ((1, 0), (wl.n // 2, wl.dim - 1)):
+        e = np.zeros_like(x)
+        e[i, k] = eps_x
+        out[f"x[{i},{k}]"] = ((loss(x + e, vol, A) - loss(x - e, vol, A)) / (2 * eps_x), float(xb[i, k]))
+    return out, xb, ab
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, dict(n_axis=16)), (4, dict(n_axis=9)), (2, dict(dx=0.08))])
+def test_renorm_gradient_vjp_matches_central_differences(cfg, kw):
+    """adjoint of Eq.44/45 ("fully supports backpropagation through this operation") w.r.t. positions,
+    volumes and the field, against central differences of renorm_gradient(); translation invariance gives sum x_bar = 0,
+    invariance under A -> A + const gives sum A_bar = 0"""
+    wl, rp, ci, vol = _renorm_inputs(cfg, kw)
+    rng = np.random.default_rng(7)
+    x = wl.x.astype(np.float64)
+    vol = vol * (1 + 0.1 * rng.normal(size=wl.n))
+    A = wl.rho.astype(np.float64) + 0.3 * np.sin(5 * x[:, 0]) * np.cos(3 * x[:, 1])
+    gb = rng.normal(size=(wl.n, wl.dim))
+    out, xb, ab = _renorm_vjp_fd(wl, rp, ci, vol, A, gb, 1e-6, 1e-6 * float(wl.h.min()))
+    scale = max(abs(v[1]) for v in out.values())
+    for name, (fd, an) in out.items():
+        assert abs(fd - an) < 1e-6 * max(abs(an), 1e-3 * scale), (name, fd, an)
+    assert np.max(np.abs(xb.sum(axis=0))) < 1e-12 * np.max(np.abs(xb)) and abs(ab.sum()) < 1e-12 * np.max(np.abs(ab))
+
+
+def test_renorm_gradient_vjp_on_a_rank_deficient_neighbourhood():
+    """particles on a line in 2D: M has rank 1 and the constant-rank differential of the pseudo-inverse carries the extra
+    term (I - P) g_bar (L g)^T; perturbing the particles OFF the line keeps the dropped eigenvalue at O(eps^2), so central
+    differences of the truncated forward see exactly that differential"""
+    dom = W.Domain(dim=2, periodic=(0, 0, 0), lo=(0.0, 0.0, 0.0), hi=(2.0, 2.0, 0.0), cell_size=0.4)
+    s = np.array([0.0, 0.11, 0.2, 0.33, 0.41, 0.55])
+    x = (np.array([0.5, 0.5]) + np.outer(s, [0.6, 0.8])).astype(np.float32)
+    n = len(x)
+    wl = W.Workload(name="line", domain=dom, params=W.Params(), x=x, v=0 * x, rho=np.ones(n, np.float32),
+                    m=np.full(n, 0.01, np.float32), h=np.full(n, 0.4, np.float32), kind=np.zeros(n, np.uint8),
+                    dt=0.0, dx=0.1, seed=0)
+    rp, ci = oracle.neighbors(dom, x, wl.h)
+    rng = np.random.default_rng(2)
+    vol = np.full(n, 0.01) * (1 + 0.1 * rng.normal(size=n))
+    A = rng.normal(size=n)
+    gb = rng.normal(size=(n, 2))
+    out, xb, ab = _renorm_vjp_fd(wl, rp, ci, vol, A, gb, 1e-4, 1e-6)
+    scale = max(abs(v[1]) for v in out.values())
+    for name, (fd, an) in out.items():
+        assert abs(fd - an) < 1e-5 * max(abs(an), 1e-3 * scale), (name, fd, an)
+    # without the extra term the position gradient would be visibly wrong: the term is not negligible here
+    L, g, M = oracle.renorm_gradient(dom, x.astype(np.float64), wl.h, vol, A, rp, ci, rcond=1e-4)
+    P = np.einsum("nkl,nlm->nkm", M, L)
+    c = gb - np.einsum("nkl,nl->nk", P, gb)
+    assert np.max(np.abs(c)) > 0.1
