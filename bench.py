@@ -368,7 +368,8 @@ def main():
     L_dev = torch.empty((x.shape[0], x.shape[1], x.shape[1]), dtype=torch.float32, device=x.device)
     for name, call in (("grad_sum", lambda: sph.grad_sum(a_dev, gs_dev)),
                        ("grad_sum_vjp", lambda: sph.grad_sum_vjp(a_dev, mu, xb_dev, ab_dev)),
-                       ("renorm_gradient", lambda: sph.renorm_gradient(a_dev, rho, 1e-4, L_dev, gs_dev))):
+                       ("renorm_gradient", lambda: sph.renorm_gradient(a_dev, rho, 1e-4, L_dev, gs_dev)),
+                       ("renorm_gradient_vjp", lambda: sph.renorm_gradient_vjp(a_dev, rho, mu, 1e-4, xb_dev, mb_dev, ab_dev))):
         call()
         e0, e1 = ev(), ev()
         e0.record()

@@ -134,10 +134,18 @@ int sph_grad_sum_vjp(sph_ctx *ctx, const float *a, const float *g_bar, float *x_
  * dropped ("commonly performed as a pseudo-inverse for numerical stability"), so a particle without
  * neighbours gets L = 0 and particles on a line / in a plane get the gradient within it.  0 <= rcond < 1.
  * vol, A: device float[n] in caller order.  L_out: device float[n*d*d], row-major d x d per particle, or NULL;
- * grad_out: device float[n*d] or NULL (not both NULL).  All buffers stay owned by the caller.  Forward only: the adjoint
- * of this operation is not part of the library.  Returns SPH_E_INVALID on bad arguments, SPH_E_STATE without lists. */
+ * grad_out: device float[n*d] or NULL (not both NULL).  All buffers stay owned by the caller.  Returns SPH_E_INVALID on bad arguments, SPH_E_STATE without lists. */
 int sph_renorm_gradient(sph_ctx *ctx, const float *vol, const float *A, float rcond, float *L_out, float *grad_out,
                         sph_stream_t stream);
+
+/* Reverse-mode adjoint of the corrected gradient of sph_renorm_gradient ("fully supports backpropagation through this
+ * operation as well"), adjacency held fixed: given grad_bar (device float[n*d], the cotangent
+ * of <grad A>), writes x_bar (float[n*d]), vol_bar (float[n] or NULL) and A_bar (float[n] or NULL).  The moments are
+ * recomputed (nothing is kept between calls); the pseudo-inverse is differentiated at constant rank
+ * (d M^+ = -M^+ dM M^+ + (I - M M^+) dM M^+ M^+ on the range of the data), exact wherever no eigenvalue crosses the cutoff.
+ * Gather form over the symmetric list, no atomics, bit-reproducible.  Same argument rules and errors as the forward. */
+int sph_renorm_gradient_vjp(sph_ctx *ctx, const float *vol, const float *A, float rcond, const float *grad_bar,
+                            float *x_bar, float *vol_bar, float *A_bar, sph_stream_t stream);
 
 /* One right-hand-side evaluation (formulas at the top of this file) on the lists of the last sph_neighbors.
  * x may differ from the build positions (RK stages) as long as the list is still a superset of the true

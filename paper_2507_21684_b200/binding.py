@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsph_b200.so")
 
 EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph_neighbors_export", "sph_density",
-           "sph_density_vjp", "sph_lists_valid", "sph_grad_sum", "sph_grad_sum_vjp", "sph_renorm_gradient",
+           "sph_density_vjp", "sph_lists_valid", "sph_grad_sum", "sph_grad_sum_vjp", "sph_renorm_gradient", "sph_renorm_gradient_vjp",
            "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
            "sph_check", "sph_strerror", "sph_get_info", "sph_get_layout", "sph_profile_enable", "sph_profile_read",
            "sph_set_option")
@@ -70,6 +70,7 @@ def load_library(path: str = LIB_PATH):
     lib.sph_grad_sum.argtypes = [vp, vp, vp, vp]
     lib.sph_grad_sum_vjp.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.sph_renorm_gradient.argtypes = [vp, vp, vp, C.c_float, vp, vp, vp]
+    lib.sph_renorm_gradient_vjp.argtypes = [vp, vp, vp, C.c_float, vp, vp, vp, vp, vp]
     lib.sph_lists_valid.argtypes = [vp, vp, f32, C.POINTER(C.c_int32), C.POINTER(f32), vp]
     lib.sph_rhs.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 7 + [vp]
     lib.sph_rhs_vjp.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 11 + [vp]
@@ -229,6 +230,16 @@ class Sph:
         self._chk(self.lib.sph_renorm_gradient(self._ctx, _ptr(vol), _ptr(A), C.c_float(rcond),
                                                _ptr(L) if L is not None else None, _ptr(grad), _stream()))
         return L, grad
+
+    def renorm_gradient_vjp(self, vol, A, grad_bar, rcond=1e-4, x_bar=None, vol_bar=None, A_bar=None):
+        """(x_bar, vol_bar, A_bar) = J^T grad_bar of the corrected gradient of renorm_gradient()"""
+        vol, A, grad_bar = _f32(vol, (self.n,)), _f32(A, (self.n,)), _f32(grad_bar, (self.n, self.dim))
+        x_bar = torch.empty((self.n, self.dim), dtype=torch.float32, device=A.device) if x_bar is None else _f32(x_bar, (self.n, self.dim))
+        vol_bar = torch.empty(self.n, dtype=torch.float32, device=A.device) if vol_bar is None else _f32(vol_bar, (self.n,))
+        A_bar = torch.empty(self.n, dtype=torch.float32, device=A.device) if A_bar is None else _f32(A_bar, (self.n,))
+        self._chk(self.lib.sph_renorm_gradient_vjp(self._ctx, _ptr(vol), _ptr(A), C.c_float(rcond), _ptr(grad_bar),
+                                                   _ptr(x_bar), _ptr(vol_bar), _ptr(A_bar), _stream()))
+        return x_bar, vol_bar, A_bar
 
     def rhs(self, params, x, v, rho, m, kind, drho_dt=None, acc=None):
         p = make_params(params)

@@ -288,6 +288,8 @@ int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, floa
 int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s, float *x_bar, float *m_bar,
                                 cudaStream_t st);
 int sph_launch_grad_sum_tile(sph_ctx *ctx, const KPar &kp, const float *a_s, float *g_out, cudaStream_t st);
+int sph_launch_renorm_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *rb, const float4 *rc, const float2 *rd,
+                               const float *re, float *x_bar, float *vol_bar, float *A_bar, cudaStream_t st);
 int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float2 *va_s, float4 *mom, cudaStream_t st);
 int sph_launch_grad_sum_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *ga_s, float *x_bar, float *a_bar,
                                  cudaStream_t st);

@@ -36,3 +36,47 @@ static __device__ __forceinline__ HC hc_uniform(const KPar &kp)
     return c;
 }
 
+// ------------------------------------------------------------------------------------------ kernel renormalisation, adjoint
+// per-particle record of the pair pass of sph_renorm_gradient_vjp (written by k_renorm_solve_vjp, sph_pairs.cu)
+struct RenormRec {
+    float V, A, bb[3], N[6];                                   // N = {xx, xy, xz, yy, yz, zz}
+};
+template <int DIM>
+static __device__ __forceinline__ RenormRec renorm_rec(const float4 &b, const float4 &c, const float2 &d, float e)
+{
+    RenormRec r;
+    r.V = b.x; r.A = b.y; r.bb[0] = b.z; r.bb[1] = b.w;
+    if (DIM == 3) {
+        r.bb[2] = c.x; r.N[0] = c.y; r.N[1] = c.z; r.N[2] = c.w; r.N[3] = d.x; r.N[4] = d.y; r.N[5] = e;
+    } else {
+        r.bb[2] = 0.f; r.N[0] = d.x; r.N[1] = d.y; r.N[2] = 0.f; r.N[3] = e; r.N[4] = 0.f; r.N[5] = 0.f;
+    }
+    return r;
+}
+// contributions of neighbour j to row i; d = x_i - x_j
+template <int DIM>
+static __device__ __forceinline__ void renorm_vjp_pair(const RenormRec &ri, const RenormRec &rj, const float (&d)[3], float G,
+                                                float K, float (&xb)[3], float &vb, float &ab)
+{
+    float Nid[3], Njd[3];
+    Nid[0] = fmaf(ri.N[0], d[0], fmaf(ri.N[1], d[1], ri.N[2] * d[2]));
+    Nid[1] = fmaf(ri.N[1], d[0], fmaf(ri.N[3], d[1], ri.N[4] * d[2]));
+    Nid[2] = fmaf(ri.N[2], d[0], fmaf(ri.N[4], d[1], ri.N[5] * d[2]));
+    Njd[0] = fmaf(rj.N[0], d[0], fmaf(rj.N[1], d[1], rj.N[2] * d[2]));
+    Njd[1] = fmaf(rj.N[1], d[0], fmaf(rj.N[3], d[1], rj.N[4] * d[2]));
+    Njd[2] = fmaf(rj.N[2], d[0], fmaf(rj.N[4], d[1], rj.N[5] * d[2]));
+    const float ai = 0.5f * fmaf(d[0], Nid[0], fmaf(d[1], Nid[1], d[2] * Nid[2]));
+    const float aj = 0.5f * fmaf(d[0], Njd[0], fmaf(d[1], Njd[1], d[2] * Njd[2]));
+    const float bi = fmaf(ri.bb[0], d[0], fmaf(ri.bb[1], d[1], ri.bb[2] * d[2]));
+    const float bj = fmaf(rj.bb[0], d[0], fmaf(rj.bb[1], d[1], rj.bb[2] * d[2]));
+    const float dA = rj.A - ri.A;
+    // x_bar: coefficient of d, then the N d and b_bar parts
+    const float cd = K * (rj.V * fmaf(dA, bi, -ai) - ri.V * fmaf(-dA, bj, aj));
+    const float gVj = G * rj.V, gVi = G * ri.V;
+#pragma unroll
+    for (int k = 0; k < DIM; ++k)
+        xb[k] += cd * d[k] - gVj * Nid[k] - gVi * Njd[k] + dA * (gVj * ri.bb[k] + gVi * rj.bb[k]);
+    vb = fmaf(G, fmaf(dA, bj, -aj), vb);
+    ab = fmaf(-G, fmaf(ri.V, bj, rj.V * bi), ab);
+}
+

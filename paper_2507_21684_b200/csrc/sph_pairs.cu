@@ -424,19 +424,19 @@ __device__ __forceinline__ void jacobi_rotate(float &app, float &aqq, float &apq
     }
 }
 
+// L = M^+ and P = projector on the range of M (sum of v v^T over the retained eigenvectors), M symmetric given as
+// {xx, xy, xz, yy, yz, zz} (2D: xz = yz = zz = 0 and only the upper-left 2x2 of L, P is meaningful)
 template <int DIM>
-__global__ void k_renorm_solve(int64_t n, const float4 *__restrict__ mom, const uint32_t *__restrict__ perm, float rcond,
-                               float *__restrict__ L_out, float *__restrict__ grad_out)
+__device__ __forceinline__ void renorm_pinv(const float (&m)[6], float rcond, float (&L)[3][3], float (&P)[3][3])
 {
-    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n) return;
-    const int64_t i = perm[p];
+    float lam[3] = {0.f, 0.f, 0.f};
+    float V[3][3] = {{1.f, 0.f, 0.f}, {0.f, 1.f, 0.f}, {0.f, 0.f, 1.f}};
     if (DIM == 2) {
-        const float4 r0 = mom[p * 2];
-        const float a = r0.x, b = r0.y, c = r0.z, b0 = r0.w, b1 = mom[p * 2 + 1].x;
+        const float a = m[0], b = m[1], c = m[3];
         const float hd = 0.5f * (a - c), rad = sqrtf(fmaf(hd, hd, b * b)), mid = 0.5f * (a + c);
-        const float l0 = mid + rad, l1 = mid - rad;
-        // unit eigenvector of l0: (cos, sin) of half the angle of (a - c, 2b)
+        lam[0] = mid + rad;
+        lam[1] = mid - rad;
+        // unit eigenvector of lam[0]: (cos, sin) of half the angle of (a - c, 2b)
         float cs = 1.f, sn = 0.f;
         if (rad > 0.f) {
             const float cx = hd / rad, sx = b / rad;            // cos, sin of the full angle
@@ -449,46 +449,162 @@ __global__ void k_renorm_solve(int64_t n, const float4 *__restrict__ mom, const 
                 cs = sx / (2.0f * sn);
             }
         }
-        const float cut = rcond * fmaxf(fabsf(l0), fabsf(l1));
-        const float i0 = fabsf(l0) > cut ? 1.0f / l0 : 0.f, i1 = fabsf(l1) > cut ? 1.0f / l1 : 0.f;
-        const float Lxx = i0 * cs * cs + i1 * sn * sn, Lxy = (i0 - i1) * cs * sn, Lyy = i0 * sn * sn + i1 * cs * cs;
-        if (L_out) {
-            L_out[i * 4] = Lxx; L_out[i * 4 + 1] = Lxy; L_out[i * 4 + 2] = Lxy; L_out[i * 4 + 3] = Lyy;
-        }
-        if (grad_out) {
-            grad_out[i * 2] = fmaf(Lxx, b0, Lxy * b1);
-            grad_out[i * 2 + 1] = fmaf(Lxy, b0, Lyy * b1);
-        }
+        V[0][0] = cs; V[1][0] = sn; V[0][1] = -sn; V[1][1] = cs;
     } else {
-        const float4 r0 = mom[p * 3], r1 = mom[p * 3 + 1];
-        float axx = r0.x, axy = r0.y, axz = r0.z, ayy = r0.w, ayz = r1.x, azz = r1.y;
-        const float bb[3] = {r1.z, r1.w, mom[p * 3 + 2].x};
-        float V[3][3] = {{1.f, 0.f, 0.f}, {0.f, 1.f, 0.f}, {0.f, 0.f, 1.f}};
+        float axx = m[0], axy = m[1], axz = m[2], ayy = m[3], ayz = m[4], azz = m[5];
 #pragma unroll 1
         for (int sweep = 0; sweep < 6; ++sweep) {
             jacobi_rotate(axx, ayy, axy, axz, ayz, V, 0, 1);
             jacobi_rotate(axx, azz, axz, axy, ayz, V, 0, 2);
             jacobi_rotate(ayy, azz, ayz, axy, axz, V, 1, 2);
         }
-        const float lam[3] = {axx, ayy, azz};
-        const float cut = rcond * fmaxf(fabsf(lam[0]), fmaxf(fabsf(lam[1]), fabsf(lam[2])));
-        float L[3][3] = {{0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}};
+        lam[0] = axx; lam[1] = ayy; lam[2] = azz;
+    }
+    const float cut = rcond * fmaxf(fabsf(lam[0]), fmaxf(fabsf(lam[1]), fabsf(lam[2])));
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const float inv = fabsf(lam[k]) > cut ? 1.0f / lam[k] : 0.f;
+    for (int r = 0; r < 3; ++r)
 #pragma unroll
-            for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c) L[r][c] = P[r][c] = 0.f;
 #pragma unroll
-                for (int c = 0; c < 3; ++c) L[r][c] = fmaf(inv * V[r][k], V[c][k], L[r][c]);
+    for (int k = 0; k < DIM; ++k) {
+        const bool keep = fabsf(lam[k]) > cut;
+        const float inv = keep ? 1.0f / lam[k] : 0.f, one = keep ? 1.0f : 0.f;
+#pragma unroll
+        for (int r = 0; r < DIM; ++r)
+#pragma unroll
+            for (int c = 0; c < DIM; ++c) {
+                L[r][c] = fmaf(inv * V[r][k], V[c][k], L[r][c]);
+                P[r][c] = fmaf(one * V[r][k], V[c][k], P[r][c]);
+            }
+    }
+}
+
+template <int DIM>
+__device__ __forceinline__ void renorm_load(const float4 *__restrict__ mom, int64_t p, float (&m)[6], float (&b)[3])
+{
+    if (DIM == 2) {
+        const float4 r0 = mom[p * 2];
+        m[0] = r0.x; m[1] = r0.y; m[2] = 0.f; m[3] = r0.z; m[4] = 0.f; m[5] = 0.f;
+        b[0] = r0.w; b[1] = mom[p * 2 + 1].x; b[2] = 0.f;
+    } else {
+        const float4 r0 = mom[p * 3], r1 = mom[p * 3 + 1];
+        m[0] = r0.x; m[1] = r0.y; m[2] = r0.z; m[3] = r0.w; m[4] = r1.x; m[5] = r1.y;
+        b[0] = r1.z; b[1] = r1.w; b[2] = mom[p * 3 + 2].x;
+    }
+}
+
+template <int DIM>
+__global__ void k_renorm_solve(int64_t n, const float4 *__restrict__ mom, const uint32_t *__restrict__ perm, float rcond,
+                               float *__restrict__ L_out, float *__restrict__ grad_out)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const int64_t i = perm[p];
+    float m[6], b[3], L[3][3], P[3][3];
+    renorm_load<DIM>(mom, p, m, b);
+    renorm_pinv<DIM>(m, rcond, L, P);
+    if (L_out)
+#pragma unroll
+        for (int r = 0; r < DIM; ++r)
+#pragma unroll
+            for (int c = 0; c < DIM; ++c) L_out[i * DIM * DIM + r * DIM + c] = L[r][c];
+    if (grad_out)
+#pragma unroll
+        for (int r = 0; r < DIM; ++r) grad_out[i * DIM + r] = fmaf(L[r][0], b[0], fmaf(L[r][1], b[1], L[r][2] * b[2]));
+}
+
+// Adjoint of g = M^+ b per particle (include/sph.h sph_renorm_gradient_vjp): b_bar = L g_bar and, with the differential of
+// the pseudo-inverse at constant rank, M_bar = -b_bar g^T + ((I - P) g_bar) (L g)^T.  Only N = M_bar + M_bar^T enters the
+// pair terms.  Writes the sorted records the pair pass gathers:
+//   rb = {V, A, b_bar0, b_bar1};  3D: rc = {b_bar2, Nxx, Nxy, Nxz}, rd = {Nyy, Nyz}, re = Nzz;  2D: rd = {Nxx, Nxy}, re = Nyy
+template <int DIM>
+__global__ void k_renorm_solve_vjp(int64_t n, const float4 *__restrict__ mom, const float2 *__restrict__ va_s,
+                                   const uint32_t *__restrict__ perm, const float *__restrict__ grad_bar, float rcond,
+                                   float4 *__restrict__ rb, float4 *__restrict__ rc, float2 *__restrict__ rd,
+                                   float *__restrict__ re)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const int64_t i = perm[p];
+    float m[6], b[3], L[3][3], P[3][3];
+    renorm_load<DIM>(mom, p, m, b);
+    renorm_pinv<DIM>(m, rcond, L, P);
+    float gb[3] = {grad_bar[i * DIM], grad_bar[i * DIM + 1], DIM == 3 ? grad_bar[i * DIM + 2] : 0.f};
+    float g[3], bb[3], c[3], u[3];
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        g[r] = fmaf(L[r][0], b[0], fmaf(L[r][1], b[1], L[r][2] * b[2]));
+        bb[r] = fmaf(L[r][0], gb[0], fmaf(L[r][1], gb[1], L[r][2] * gb[2]));
+        c[r] = gb[r] - fmaf(P[r][0], gb[0], fmaf(P[r][1], gb[1], P[r][2] * gb[2]));
+    }
+#pragma unroll
+    for (int r = 0; r < 3; ++r) u[r] = fmaf(L[r][0], g[0], fmaf(L[r][1], g[1], L[r][2] * g[2]));
+    auto N = [&](int r, int s) { return -(bb[r] * g[s] + g[r] * bb[s]) + (c[r] * u[s] + u[r] * c[s]); };
+    const float2 va = va_s[p];
+    rb[p] = make_float4(va.x, va.y, bb[0], bb[1]);
+    if (DIM == 3) {
+        rc[p] = make_float4(bb[2], N(0, 0), N(0, 1), N(0, 2));
+        rd[p] = make_float2(N(1, 1), N(1, 2));
+        re[p] = N(2, 2);
+    } else {
+        rd[p] = make_float2(N(0, 0), N(0, 1));
+        re[p] = N(1, 1);
+    }
+}
+
+// Pair pass of the adjoint, gather form over the symmetric list: row i evaluates the ordered pairs (i <- j) and (j <- i)
+// and keeps what lands on i.  With d = x_i - x_j, dA = A_j - A_i, a_i = d^T M_bar_i d = (d^T N_i d)/2, be_i = b_bar_i . d:
+//   F_ij = V_j [ -K a_i d - G N_i d + dA (K be_i d + G b_bar_i) ],   F_ji = V_i [ K a_j d + G N_j d - dA (K be_j d + G b_bar_j) ]
+//   x_bar_i = sum_j F_ij - F_ji,   vol_bar_i = sum_j G (-a_j + dA be_j),   A_bar_i = -sum_j G (V_i be_j + V_j be_i)
+template <int DIM, int GS, bool VARH>
+__global__ void __launch_bounds__(kBlock)
+k_renorm_vjp(int64_t n, KPar kp, float margin, const float4 *__restrict__ pos_s, const float4 *__restrict__ rb,
+             const float4 *__restrict__ rc, const float2 *__restrict__ rd, const float *__restrict__ re,
+             const long long *__restrict__ row_ptr, const int32_t *__restrict__ col, const uint32_t *__restrict__ perm,
+             float *__restrict__ xb_out, float *__restrict__ vb_out, float *__restrict__ ab_out)
+{
+    constexpr int kGroups = kBlock / GS;
+    const int g = threadIdx.x / GS, gl = threadIdx.x % GS;
+    const int64_t row0 = (int64_t)blockIdx.x * kGroups * kRowsPerGroup;
+    const HC hu = hc_uniform<DIM>(kp);
+    for (int rr = 0; rr < kRowsPerGroup; ++rr) {
+        const int64_t row = row0 + (int64_t)rr * kGroups + g;
+        if (row >= n) break;
+        const float4 pi = __ldg(pos_s + row);
+        const RenormRec ri = renorm_rec<DIM>(__ldg(rb + row), DIM == 3 ? __ldg(rc + row) : make_float4(0.f, 0.f, 0.f, 0.f),
+                                             __ldg(rd + row), __ldg(re + row));
+        const float xi[3] = {pi.x, pi.y, pi.z};
+        const bool seam = row_near_seam(xi, kp, margin);
+        const long long b = row_ptr[row], e = row_ptr[row + 1];
+        float xb[3] = {0.f, 0.f, 0.f}, vb = 0.f, ab = 0.f;
+        for (long long p = b + gl; p < e; p += GS) {
+            const int32_t j = __ldg(col + p);
+            const float4 pj = __ldg(pos_s + j);
+            const RenormRec rj = renorm_rec<DIM>(__ldg(rb + j), DIM == 3 ? __ldg(rc + j) : make_float4(0.f, 0.f, 0.f, 0.f),
+                                                 __ldg(rd + j), __ldg(re + j));
+            const float xj[3] = {pj.x, pj.y, pj.z};
+            float d[3], r2;
+            if (seam) rel_pos<DIM, true>(xi, xj, kp, d, r2); else rel_pos<DIM, false>(xi, xj, kp, d, r2);
+            HC hc = hu;
+            if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+            const float q = fast_sqrt(r2) * hc.invH;
+            const float t = fmaxf(1.0f - q, 0.f);
+            const float t2 = t * t, t4 = t2 * t2;
+            const float G = hc.cG * fmaf(5.0f, q, 1.0f) * (t4 * t);                               // Eq.29
+            const float K = hc.cK * t4;                                                           // Eq.16
+            renorm_vjp_pair<DIM>(ri, rj, d, G, K, xb, vb, ab);
         }
-        if (L_out)
 #pragma unroll
-            for (int r = 0; r < 3; ++r)
+        for (int k = 0; k < DIM; ++k) xb[k] = group_sum<GS>(xb[k]);
+        vb = group_sum<GS>(vb);
+        ab = group_sum<GS>(ab);
+        if (gl == 0) {
+            const int64_t i = perm[row];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) L_out[i * 9 + r * 3 + c] = L[r][c];
-        if (grad_out)
-#pragma unroll
-            for (int r = 0; r < 3; ++r) grad_out[i * 3 + r] = fmaf(L[r][0], bb[0], fmaf(L[r][1], bb[1], L[r][2] * bb[2]));
+            for (int k = 0; k < DIM; ++k) xb_out[i * DIM + k] = xb[k];
+            if (vb_out) vb_out[i] = vb;
+            if (ab_out) ab_out[i] = ab;
+        }
     }
 }
 
@@ -1088,6 +1204,62 @@ extern "C" int sph_renorm_gradient(sph_ctx *ctx, const float *vol, const float *
     }
     if (kp.dim == 3) k_renorm_solve<3><<<nb1, 256, 0, st>>>(n, mom, ctx->perm.as<uint32_t>(), rcond, L_out, grad_out);
     else k_renorm_solve<2><<<nb1, 256, 0, st>>>(n, mom, ctx->perm.as<uint32_t>(), rcond, L_out, grad_out);
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+extern "C" int sph_renorm_gradient_vjp(sph_ctx *ctx, const float *vol, const float *A, float rcond, const float *grad_bar,
+                                       float *x_bar, float *vol_bar, float *A_bar, sph_stream_t stream)
+{
+    if (!ctx || !vol || !A || !grad_bar || !x_bar || !(rcond >= 0.f) || !(rcond < 1.f)) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    const int64_t n = ctx->n;
+    sph_params dummy{};
+    dummy.c0 = 1.f; dummy.rho0 = 1.f; dummy.gamma = 1.f; dummy.eps = 1.f;
+    KPar kp;
+    SPH_TRY(sph_kpar_make(ctx, &dummy, &kp));
+    SPH_TRY(ctx->s2.reserve((size_t)n * 8));
+    SPH_TRY(ctx->c0buf.reserve((size_t)n * 48));
+    SPH_TRY(ctx->s0.reserve((size_t)n * 16));
+    SPH_TRY(ctx->s1.reserve((size_t)n * 16));
+    SPH_TRY(ctx->out4.reserve((size_t)n * 16));
+    SPH_TRY(ctx->m_s.reserve((size_t)n * 4));
+    float2 *va_s = ctx->s2.as<float2>();
+    float4 *mom = ctx->c0buf.as<float4>();
+    float4 *rb = ctx->s0.as<float4>(), *rc = ctx->s1.as<float4>();
+    float2 *rd = ctx->out4.as<float2>();
+    float *re = ctx->m_s.as<float>();
+    KScope ks(ctx, SPH_K_DENSITY, 4, st);
+    const unsigned nb1 = (unsigned)((n + 255) / 256);
+    const float margin = seam_margin(ctx);
+    // forward moments again (nothing is kept between calls), then the per-particle adjoint of g = M^+ b
+    k_gather_f32x2<<<nb1, 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), vol, A, va_s);
+    if (ctx->tile_mode) {
+        SPH_TRY(sph_launch_renorm_tile(ctx, kp, va_s, mom, st));
+    } else {
+#define SPH_RN_LAUNCH(DIM, GS, VARH)                                                                             \
+    k_renorm<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), va_s,  \
+                                                                ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>(), mom)
+        if (kp.dim == 3) { if (kp.uniform_h) SPH_RN_LAUNCH(3, 32, false); else SPH_RN_LAUNCH(3, 32, true); }
+        else { if (kp.uniform_h) SPH_RN_LAUNCH(2, 16, false); else SPH_RN_LAUNCH(2, 16, true); }
+#undef SPH_RN_LAUNCH
+    }
+    if (kp.dim == 3)
+        k_renorm_solve_vjp<3><<<nb1, 256, 0, st>>>(n, mom, va_s, ctx->perm.as<uint32_t>(), grad_bar, rcond, rb, rc, rd, re);
+    else
+        k_renorm_solve_vjp<2><<<nb1, 256, 0, st>>>(n, mom, va_s, ctx->perm.as<uint32_t>(), grad_bar, rcond, rb, rc, rd, re);
+    if (ctx->tile_mode) return sph_launch_renorm_vjp_tile(ctx, kp, rb, rc, rd, re, x_bar, vol_bar, A_bar, st);
+#define SPH_RNV_LAUNCH(DIM, GS, VARH)                                                                                  \
+    k_renorm_vjp<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), rb, rc, rd, \
+                                                                    re, ctx->row_ptr.as<long long>(),                   \
+                                                                    ctx->col.as<int32_t>(), ctx->perm.as<uint32_t>(),   \
+                                                                    x_bar, vol_bar, A_bar)
+    if (kp.dim == 3) { if (kp.uniform_h) SPH_RNV_LAUNCH(3, 16, false); else SPH_RNV_LAUNCH(3, 16, true); }
+    else { if (kp.uniform_h) SPH_RNV_LAUNCH(2, 16, false); else SPH_RNV_LAUNCH(2, 16, true); }
+#undef SPH_RNV_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

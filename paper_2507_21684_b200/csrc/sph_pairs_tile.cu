@@ -392,6 +392,76 @@ k_renorm_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ pos
         });
 }
 
+// pair pass of the adjoint of the renormalised gradient (formulas: sph_pairs.cu k_renorm_vjp, sph_pair_math.cuh).
+// smem (own carve-up, 60 B per halo particle in 3D, 44 B in 2D): A = {x,y,z,h}, RB = {V, A, b_bar0, b_bar1},
+// RC = {b_bar2, Nxx, Nxy, Nxz} (3D only), RD = float2, RE = float; then rp, selfq, ring as in SmemMap
+template <int DIM, int GS, bool VARH>
+__global__ void __launch_bounds__(kPtMaxWarps * 32)
+k_renorm_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ pos_s, const float4 *__restrict__ rb,
+                  const float4 *__restrict__ rc, const float2 *__restrict__ rd, const float *__restrict__ re,
+                  const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
+                  const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16,
+                  const uint32_t *__restrict__ perm, float *__restrict__ xb_out, float *__restrict__ vb_out,
+                  float *__restrict__ ab_out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    size_t o = 0;
+    float4 *A = reinterpret_cast<float4 *>(smem_raw + o); o += (size_t)ts.mcap * 16;
+    float4 *RB = reinterpret_cast<float4 *>(smem_raw + o); o += (size_t)ts.mcap * 16;
+    float4 *RC = reinterpret_cast<float4 *>(smem_raw + o); if (DIM == 3) o += (size_t)ts.mcap * 16;
+    float2 *RD = reinterpret_cast<float2 *>(smem_raw + o); o += (size_t)ts.mcap * 8;
+    float *RE = reinterpret_cast<float *>(smem_raw + o); o += (size_t)ts.mcap * 4;
+    uint32_t *rp = reinterpret_cast<uint32_t *>(smem_raw + o); o += (size_t)(ts.tcap + 4) * 4;
+    uint16_t *selfq = reinterpret_cast<uint16_t *>(smem_raw + o); o += (size_t)ts.tcap * 2;
+    o = (o + 15) & ~(size_t)15;
+    uint16_t *ring = reinterpret_cast<uint16_t *>(smem_raw + o);
+    __shared__ TileTab tt;
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (tt.T == 0) return;
+    stage_halo(tt, pos_s, A, rb, RB, DIM == 3 ? rc : nullptr, RC, rd, RD, re, RE);
+    stage_rows(tt, row_ptr, rp, selfq);
+    cp_async_wait<0>();
+    __syncthreads();
+    stage_shift<DIM>(tt, A);
+    const int gl = (threadIdx.x & 31) % GS;
+    const HC hu = hc_uniform<DIM>(kp);
+    const uint32_t row0 = tt.row0;
+    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    tile_row_passes<GS>(tt, rp, ring, ts.rb, col16, row_ptr[tt.row0],
+        [&](uint32_t r, bool live, uint32_t b, uint32_t e, const uint16_t *idx) {
+            const uint32_t qi = selfq[r];
+            const float4 pi = A[qi];
+            const RenormRec ri = renorm_rec<DIM>(RB[qi], DIM == 3 ? RC[qi] : zero4, RD[qi], RE[qi]);
+            float xb[3] = {0.f, 0.f, 0.f}, vb = 0.f, ab = 0.f;
+            for (uint32_t k = b + gl; k < e; k += GS) {
+                const uint32_t j = idx[k];
+                const float4 pj = A[j];
+                const RenormRec rj = renorm_rec<DIM>(RB[j], DIM == 3 ? RC[j] : zero4, RD[j], RE[j]);
+                const float d[3] = {pi.x - pj.x, pi.y - pj.y, DIM == 3 ? pi.z - pj.z : 0.f};
+                const float r2 = fmaf(d[2], d[2], fmaf(d[1], d[1], d[0] * d[0]));
+                HC hc = hu;
+                if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+                const float q = fast_sqrt(r2) * hc.invH;
+                const float t = fmaxf(1.0f - q, 0.f);
+                const float t2 = t * t, t4 = t2 * t2;
+                const float G = hc.cG * fmaf(5.0f, q, 1.0f) * (t4 * t);                             // Eq.29
+                const float K = hc.cK * t4;                                                         // Eq.16
+                renorm_vjp_pair<DIM>(ri, rj, d, G, K, xb, vb, ab);
+            }
+#pragma unroll
+            for (int k = 0; k < DIM; ++k) xb[k] = group_sum<GS>(xb[k]);
+            vb = group_sum<GS>(vb);
+            ab = group_sum<GS>(ab);
+            if (gl == 0 && live) {
+                const int64_t i = perm[row0 + r];
+#pragma unroll
+                for (int k = 0; k < DIM; ++k) xb_out[i * DIM + k] = xb[k];
+                if (vb_out) vb_out[i] = vb;
+                if (ab_out) ab_out[i] = ab;
+            }
+        });
+}
+
 // ------------------------------------------------------------------------------------------ kernel-gradient sum
 // g_i = sum_j a_j G_ij d_ij (VJP = false; smem A = positions, W = a[mcap] in the B slot) and its adjoint (VJP = true;
 // smem A, GA = {g_bar, a}[mcap] in the B slot): include/sph.h sph_grad_sum / sph_grad_sum_vjp; Eq.24
@@ -899,6 +969,39 @@ int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float2 *va_s, flo
     }
 #undef SPH_RNT_GS
 #undef SPH_RNT_LAUNCH
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_renorm_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *rb, const float4 *rc, const float2 *rd,
+                               const float *re, float *x_bar, float *vol_bar, float *A_bar, cudaStream_t st)
+{
+    const TileGeom &tg = ctx->tg;
+    const int gs = tile_group(ctx, true);
+    int threads;
+    TileSizes ts;
+    size_t smem;
+    tile_launch_cfg(ctx, kp.dim == 3 ? 60 : 44, gs, sizeof(TileTab), &threads, &ts, &smem);   // carve-up of k_renorm_vjp_tile
+#define SPH_RNVT_LAUNCH(DIM, GS, VARH)                                                                                \
+    do {                                                                                                              \
+        SPH_TILE_SMEM_ATTR((k_renorm_vjp_tile<DIM, GS, VARH>), smem);                                                 \
+        k_renorm_vjp_tile<DIM, GS, VARH><<<(unsigned)tg.ntiles, threads, smem, st>>>(                                 \
+            tg, kp, ts, ctx->pos_s.as<float4>(), rb, rc, rd, re, ctx->cell_start.as<uint32_t>(),                      \
+            ctx->cell_end.as<uint32_t>(), ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(),                    \
+            ctx->perm.as<uint32_t>(), x_bar, vol_bar, A_bar);                                                         \
+    } while (0)
+#define SPH_RNVT_GS(GS)                                                                                       \
+    do {                                                                                                      \
+        if (kp.dim == 3) { if (kp.uniform_h) SPH_RNVT_LAUNCH(3, GS, false); else SPH_RNVT_LAUNCH(3, GS, true); } \
+        else { if (kp.uniform_h) SPH_RNVT_LAUNCH(2, GS, false); else SPH_RNVT_LAUNCH(2, GS, true); }             \
+    } while (0)
+    switch (gs) {
+    case 16: SPH_RNVT_GS(16); break;
+    case 32: SPH_RNVT_GS(32); break;
+    default: SPH_RNVT_GS(8); break;
+    }
+#undef SPH_RNVT_GS
+#undef SPH_RNVT_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

@@ -96,3 +96,15 @@ def renorm_errors(L_gpu, grad_gpu, L_o, grad_o, M_o, rcond):
     sg = np.maximum(np.maximum(np.abs(grad_o).max(axis=1), np.median(np.abs(grad_o).max(axis=1))), 1e-300)
     eg = np.abs(grad_gpu.astype(np.float64) - grad_o).max(axis=1) / (sg * amp)
     return float(eL[ok].max()), float(eg[ok].max()), int(ok.sum())
+
+
+def renorm_good_rows(M_o, rcond):
+    """rows on which the renormalisation is well-posed in fp32: no eigenvalue within a factor 3 of the rank cutoff,
+    condition number of the retained part <= 50, and M_i not orders of magnitude below the typical one (see
+    renorm_errors).  The adjoint tests put their cotangent on these rows only."""
+    lam = np.abs(np.linalg.eigvalsh(M_o))
+    lmax = np.maximum(lam.max(axis=1), 1e-300)
+    ratio = lam / lmax[:, None]
+    near = np.any((ratio > rcond / 3.0) & (ratio < rcond * 3.0), axis=1)
+    lmin = np.where(ratio > rcond, lam, np.inf).min(axis=1)
+    return (~near) & (lmax / lmin <= 50.0) & (lmax >= 1e-2 * np.median(lmax))

@@ -9,7 +9,7 @@ import oracle
 from paper_2507_21684_b200 import workloads as W
 from paper_2507_21684_b200.binding import Sph, SphError, OPT_LIST_MODE, OPT_TILE_EDGE, OPT_FILL_MASKS, LIST_GENERIC
 from common import max_norm_err
-from gpu_common import Dev, build, oracle_lists, fuzz_workload, renorm_errors
+from gpu_common import Dev, build, oracle_lists, fuzz_workload, renorm_errors, renorm_good_rows
 
 pytestmark = pytest.mark.gpu
 
@@ -214,6 +214,40 @@ def test_renorm_gradient_parity(sph, case):
     assert torch.equal(grad, g2)
 
 
+def _renorm_vjp_check(sph, wl, lists, vol, A, rcond, seed, all_rows=False):
+    """cotangent on the well-posed rows (renorm_good_rows), adjoint against the oracle"""
+    _, _, M_o = oracle.renorm_gradient(wl.domain, wl.x, wl.h, vol, A, *lists, rcond=rcond)
+    good = np.ones(wl.n, bool) if all_rows else renorm_good_rows(M_o, rcond)
+    gb = (np.random.default_rng(seed).normal(size=(wl.n, wl.dim)) * good[:, None]).astype(np.float32)
+    xb, vb, ab = sph.renorm_gradient_vjp(torch.from_numpy(vol).cuda(), torch.from_numpy(A).cuda(), torch.from_numpy(gb).cuda(), rcond)
+    xo, vo, ao = oracle.renorm_gradient_vjp(wl.domain, wl.x, wl.h, vol, A, *lists, gb, rcond=rcond)
+    # max-norm errors, floored by the size of the summed terms (reading R10): the loss density |g_bar_i| |g_i| is what every
+    # pair term is made of, per unit of ln V (vol_bar), of x / h (x_bar) and of A / spread(A) (A_bar).  Without the floor an
+    # exactly cancelling sum (vol_bar = 0 for a linear field, or for two particles that only see each other) has no scale
+    _, g_o, _ = oracle.renorm_gradient(wl.domain, wl.x, wl.h, vol, A, *lists, rcond=rcond)
+    S = float(np.max(np.linalg.norm(gb, axis=1) * np.linalg.norm(g_o, axis=1))) + 1e-300
+    err = lambda got, ref, floor: float(np.max(np.abs(got - ref)) / max(np.max(np.abs(ref)), floor))
+    v64 = vol.astype(np.float64)
+    return (err(_np(xb), xo, S / float(wl.h.max())), err(_np(vb) * v64, vo * v64, S),
+            err(_np(ab), ao, S / (float(np.ptp(A)) + 1e-300)), int(good.sum()))
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_renorm_gradient_vjp_parity(sph, case):
+    """adjoint of the corrected gradient w.r.t. positions, volumes and the field (include/sph.h)"""
+    wl = CASES[case]()
+    build(wl, 1.0, sph)
+    vol, A = _renorm_field(wl)
+    ex, ev, ea, rows = _renorm_vjp_check(sph, wl, oracle_lists(wl), vol, A, 1e-4, wl.seed + 9)
+    print(f"{case}: renorm vjp err x {ex:.2e} vol {ev:.2e} A {ea:.2e}, cotangent on {rows}/{wl.n} rows")
+    assert rows > 0.9 * wl.n and max(ex, ev, ea) < TOL_VJP
+    # deterministic (no float atomics)
+    gb = torch.from_numpy(np.random.default_rng(1).normal(size=(wl.n, wl.dim)).astype(np.float32)).cuda()
+    r1 = sph.renorm_gradient_vjp(torch.from_numpy(vol).cuda(), torch.from_numpy(A).cuda(), gb, 1e-4)
+    r2 = sph.renorm_gradient_vjp(torch.from_numpy(vol).cuda(), torch.from_numpy(A).cuda(), gb, 1e-4)
+    assert all(torch.equal(a, b) for a, b in zip(r1, r2))
+
+
 def test_renorm_gradient_rank_deficient_neighbourhoods(sph):
     """particles on a line in 2D (rank 1), in a plane in 3D (rank 2), and an isolated particle (L = 0)"""
     rng = np.random.default_rng(5)
@@ -241,6 +275,12 @@ def test_renorm_gradient_rank_deficient_neighbourhoods(sph):
         eL, eg, rows = renorm_errors(_np(L), _np(grad), L_o, g_o, M_o, 1e-3)
         print(f"rank-deficient {dim}D: err L {eL:.2e} grad {eg:.2e} rows {rows}/{n}")
         assert rows == n and eL < TOL_FWD and eg < TOL_FWD
+        # the adjoint on the rank-deficient rows exercises the constant-rank term (I - P) g_bar (L g)^T
+        # (with a non-linear field: for a linear one the gradient does not depend on the volumes, vol_bar = 0 exactly)
+        A2 = rng.normal(size=n).astype(np.float32)
+        ex, ev, ea, _ = _renorm_vjp_check(sph, wl, oracle_lists(wl, method=0), vol, A2, 1e-3, 3, all_rows=True)
+        print(f"rank-deficient {dim}D: vjp err x {ex:.2e} vol {ev:.2e} A {ea:.2e}")
+        assert max(ex, ev, ea) < TOL_VJP
 
 
 @pytest.mark.parametrize("case", list(CASES))
@@ -801,6 +841,8 @@ def test_random_domains_lists_and_rhs(sph, seed):
     L_o, g_o, M_o = oracle.renorm_gradient(dom, wl.x, wl.h, vol, A, rp_o, ci_o, rcond=1e-4)
     eL, eg, rows = renorm_errors(_np(L), _np(grad), L_o, g_o, M_o, 1e-4)
     assert rows > 0.9 * wl.n and eL < TOL_FWD and eg < TOL_FWD
+    ex, ev, ea, _ = _renorm_vjp_check(sph, wl, (rp_o, ci_o), vol, A, 1e-4, seed + 17)
+    assert max(ex, ev, ea) < TOL_VJP
 
 
 @pytest.mark.parametrize("seed", range(8))
