@@ -468,6 +468,53 @@ def test_full_size_sampled_rows(sph, cfg):
     assert torch.isfinite(pb).all()
 
 
+_FULL_NEXT = {}
+
+
+def _full_size_next_oracle():
+    """oracle results of the NEXT rows at C3 (computed once, shared by the list layouts)"""
+    if not _FULL_NEXT:
+        wl = W.perturbed(W.make(3), amp_x=0.1, amp_rho=0.01)
+        lists = oracle_lists(wl)
+        rng = np.random.default_rng(21)
+        rbar = rng.normal(size=wl.n).astype(np.float32)
+        gbar = rng.normal(size=(wl.n, wl.dim)).astype(np.float32)
+        vol, A = _renorm_field(wl)
+        _FULL_NEXT.update(
+            wl=wl, lists=lists, rbar=rbar, gbar=gbar, vol=vol, A=A,
+            dvjp=oracle.density_vjp(wl.domain, wl.x, wl.h, wl.m, *lists, rbar),
+            gs=oracle.grad_sum(wl.domain, wl.x, wl.h, vol, *lists),
+            gsv=oracle.grad_sum_vjp(wl.domain, wl.x, wl.h, vol, *lists, gbar),
+            rn=oracle.renorm_gradient(wl.domain, wl.x, wl.h, vol, A, *lists, rcond=1e-4),
+            rnv=oracle.renorm_gradient_vjp(wl.domain, wl.x, wl.h, vol, A, *lists, gbar, rcond=1e-4))
+    return _FULL_NEXT
+
+
+def test_full_size_next_rows(sph):
+    """the NEXT rows (density adjoint, kernel-gradient sum and adjoint, renormalisation and adjoint) at BASELINE config 3's
+    full size (2 097 152 particles, the state bench.py times), every row against the oracle"""
+    if sph.layout_name == "tile_b1":
+        pytest.skip("full sizes run on the automatic and the generic layout")
+    o = _full_size_next_oracle()
+    wl, cu = o["wl"], lambda a: torch.from_numpy(a).cuda()
+    _, dev, nnz = build(wl, 1.0, sph)
+    assert nnz == int(o["lists"][0][-1])
+    xb, mb = sph.density_vjp(dev.m, cu(o["rbar"]))
+    assert max_norm_err(_np(xb), o["dvjp"][0]) < TOL_VJP and max_norm_err(_np(mb), o["dvjp"][1]) < TOL_VJP
+    g = sph.grad_sum(cu(o["vol"]))
+    assert max_norm_err(_np(g), o["gs"]) < TOL_FWD
+    xb, ab = sph.grad_sum_vjp(cu(o["vol"]), cu(o["gbar"]))
+    assert max_norm_err(_np(xb), o["gsv"][0]) < TOL_VJP and max_norm_err(_np(ab), o["gsv"][1]) < TOL_VJP
+    L, grad = sph.renorm_gradient(cu(o["vol"]), cu(o["A"]), 1e-4)
+    eL, eg, rows = renorm_errors(_np(L), _np(grad), *o["rn"], 1e-4)
+    assert rows == wl.n and eL < TOL_FWD and eg < TOL_FWD
+    xb, vb, ab = sph.renorm_gradient_vjp(cu(o["vol"]), cu(o["A"]), cu(o["gbar"]), 1e-4)
+    xo, vo, ao = o["rnv"]
+    print(f"C3 full size: renorm err L {eL:.2e} grad {eg:.2e}; vjp err x {max_norm_err(_np(xb), xo):.2e} "
+          f"vol {max_norm_err(_np(vb), vo):.2e} A {max_norm_err(_np(ab), ao):.2e}")
+    assert max(max_norm_err(_np(xb), xo), max_norm_err(_np(vb), vo), max_norm_err(_np(ab), ao)) < TOL_VJP
+
+
 def test_tile_search_with_generic_lists_when_a_halo_exceeds_the_pair_budget(sph):
     """dense cells (~300 particles each, the regime of BASELINE config 4): the halo of even a one-cell block does not
     fit the shared-memory budget of the pair kernels, so the tile search runs alone and hands 32-bit lists to the
