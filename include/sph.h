@@ -241,7 +241,10 @@ enum {
     SPH_OPT_RK_EXTRA_SKIN = 6 /* Verlet lists across steps: value/1000 = extra skin e (in units of h).  With
                                e > 0 sph_rk_step / sph_rk_step_vjp build their lists with search_scale = 1 + skin + e
                                (the domain's cell_size must cover it) and a later call with the same domain, n and h
-                               REUSES them while sph_lists_valid(x, skin) holds; 0 (default): rebuilt in every call */
+                               REUSES them while sph_lists_valid(x, skin) holds (and h is unchanged: checked);
+                               0: rebuilt in every call; -1 (default): automatic -- in 2D the lists take whatever the
+                               domain's cell_size leaves above 1 + skin (at most 0.25) and are reused likewise, so a
+                               caller opts in by passing larger cells; none in 3D, where it was measured not to pay */
 };
 int sph_set_option(sph_ctx *ctx, int key, int value);
 int sph_profile_enable(sph_ctx *ctx, int on);

@@ -258,7 +258,7 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
         ctx->opt_warps = value;
         return SPH_OK;
     case SPH_OPT_RK_EXTRA_SKIN:
-        if (value < 0 || value > 2000) return SPH_E_INVALID;
+        if (value < -1 || value > 2000) return SPH_E_INVALID;
         ctx->opt_rk_extra_permille = value;
         return SPH_OK;
     case SPH_OPT_FILL_MASKS:

@@ -235,7 +235,7 @@ __global__ void k_reorder(const float *__restrict__ x, const float *__restrict__
 // ------------------------------------------------------------------------------------------ Verlet validity
 // largest minimum-image displacement since the build; float bits of a non-negative float order like
 // unsigned integers, so the maximum is an integer atomic
-__global__ void k_max_displacement(const float *__restrict__ x, int64_t n, GridGeom gg,
+__global__ void k_max_displacement(const float *__restrict__ x, const float *__restrict__ h, int64_t n, GridGeom gg,
                                    const uint32_t *__restrict__ inv_perm, const float4 *__restrict__ pos_s,
                                    uint32_t *__restrict__ out)
 {
@@ -258,6 +258,7 @@ __global__ void k_max_displacement(const float *__restrict__ x, int64_t n, GridG
         }
         r = sqrtf(r2);
         if (!(r >= 0.f)) r = __uint_as_float(0x7f800000u);        // NaN position: never valid
+        if (h && h[i] != b.w) r = __uint_as_float(0x7f800000u);   // the lists were built for another h: never valid
     }
     uint32_t rb = __reduce_max_sync(0xffffffffu, __float_as_uint(r));
     if ((threadIdx.x & 31) == 0 && rb > *(volatile uint32_t *)out) atomicMax(out, rb);
@@ -410,21 +411,17 @@ extern "C" int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float 
     return SPH_OK;
 }
 
-extern "C" int sph_lists_valid(sph_ctx *ctx, const float *x, float skin_needed, int32_t *valid_out, float *max_disp_out,
-                               sph_stream_t stream)
+// x: current positions; h: NULL, or the current support radii (lists built for other radii are reported invalid)
+int sph_lists_valid_impl(sph_ctx *ctx, const float *x, const float *h, float skin_needed, int32_t *valid_out,
+                         float *max_disp_out, cudaStream_t st)
 {
-    if (!ctx || !x || !(skin_needed >= 0.f)) return SPH_E_INVALID;
-    if (!ctx->lists_ready) return SPH_E_STATE;
-    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
-    cudaStream_t st = (cudaStream_t)stream;
-    ctx->last_stream = st;
     const int64_t n = ctx->n;
     uint32_t *slot = ctx->stats.as<uint32_t>() + 12;
     SPH_CUDA_TRY(cudaMemsetAsync(slot, 0, 4, st));
     {
         KScope ks(ctx, SPH_K_KEY, 1, st);
         k_max_displacement<<<(unsigned)((n + kThreads - 1) / kThreads), kThreads, 0, st>>>(
-            x, n, ctx->geom, ctx->inv_perm.as<uint32_t>(), ctx->pos_s.as<float4>(), slot);
+            x, h, n, ctx->geom, ctx->inv_perm.as<uint32_t>(), ctx->pos_s.as<float4>(), slot);
     }
     SPH_CUDA_TRY(cudaGetLastError());
     uint32_t *hp = reinterpret_cast<uint32_t *>(ctx->h_pinned + 14);
@@ -438,4 +435,15 @@ extern "C" int sph_lists_valid(sph_ctx *ctx, const float *x, float skin_needed, 
         *valid_out = (2.0 * (double)D <= width) ? 1 : 0;
     }
     return SPH_OK;
+}
+
+extern "C" int sph_lists_valid(sph_ctx *ctx, const float *x, float skin_needed, int32_t *valid_out, float *max_disp_out,
+                               sph_stream_t stream)
+{
+    if (!ctx || !x || !(skin_needed >= 0.f)) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    return sph_lists_valid_impl(ctx, x, nullptr, skin_needed, valid_out, max_disp_out, st);
 }

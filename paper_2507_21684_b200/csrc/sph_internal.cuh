@@ -125,7 +125,10 @@ struct sph_ctx {
     int opt_group = 0;          // lanes per row in the pair kernels (0 = default)
     int opt_warps = 0;          // warps per CTA of the tile pair kernels (0 = automatic: 8, or 16 when one CTA fits an SM)
     int opt_list_mode = 0;      // 0 auto, 1 force the generic (global-id) lists, 2 force tile-local lists
-    int opt_rk_extra_permille = 0;   // sph_rk_step: extra list skin (1/1000 of h) that lets later steps reuse the lists
+    int opt_rk_extra_permille = -1;  // sph_rk_step: extra list skin (1/1000 of h) that lets later steps reuse the lists;
+                                     // -1 = automatic (2D: whatever the cell size leaves, capped; 3D: none)
+    float scale_slack_cap = 0.f;     // set by sph_rk_step around its sph_neighbors call: the search scale may grow by up to
+                                     // this much if the cell size allows
     sph_domain dom_last{};      // domain of the last sph_build_cells
     int opt_fill_masks = 1;     // the fill expands the hit masks saved by the count pass (0: repeats the tests)
     int opt_tile_edge = 0;      // 0 auto, else force the tile edge B (1, 2, 4)
@@ -288,6 +291,8 @@ int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, floa
 int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s, float *x_bar, float *m_bar,
                                 cudaStream_t st);
 int sph_launch_grad_sum_tile(sph_ctx *ctx, const KPar &kp, const float *a_s, float *g_out, cudaStream_t st);
+int sph_lists_valid_impl(sph_ctx *ctx, const float *x, const float *h, float skin_needed, int32_t *valid_out,
+                         float *max_disp_out, cudaStream_t st);
 int sph_launch_renorm_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *rb, const float4 *rc, const float2 *rd,
                                const float *re, float *x_bar, float *vol_bar, float *A_bar, cudaStream_t st);
 int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float2 *va_s, float4 *mom, cudaStream_t st);

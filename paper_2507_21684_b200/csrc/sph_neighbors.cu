@@ -302,6 +302,20 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
     memcpy(&hmin, &hs[2], 4);
     ctx->hmax = hmax;
     ctx->hmin = hmin;
+    if (ctx->scale_slack_cap > 0.f && hmax > 0.f) {
+        // sph_rk_step (automatic Verlet skin): take the slack the cell size leaves, up to the cap; the product
+        // scale * hmax must stay <= every cell edge in binary32, as the check below demands
+        double emin = gg.edge[0];
+        for (int k = 1; k < gg.dim; ++k) emin = gg.edge[k] < emin ? gg.edge[k] : emin;
+        float s = (float)(emin / (double)hmax);
+        for (int it = 0; it < 4; ++it) {
+            volatile float prod = s * hmax;
+            if ((double)prod <= emin) break;
+            s = nextafterf(s, 0.f);
+        }
+        s = fminf(s, search_scale + ctx->scale_slack_cap);
+        if (s >= search_scale + 0.02f) search_scale = s;     // less than that is not worth a longer list
+    }
     volatile float Rs = search_scale * hmax;
     for (int k = 0; k < gg.dim; ++k)
         if ((double)Rs > gg.edge[k]) return SPH_E_DOMAIN;   // cell_size < search radius

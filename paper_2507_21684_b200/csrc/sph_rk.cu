@@ -217,19 +217,30 @@ __global__ void k_adj_final(int64_t n, const uint32_t *__restrict__ perm, const 
 
 inline unsigned nb(int64_t n) { return (unsigned)((n + 255) / 256); }
 
-// Lists for one step.  Default: cells and lists from x with search_scale = 1 + skin.  With SPH_OPT_RK_EXTRA_SKIN the lists
-// carry an extra skin and are kept across steps while no particle has moved more than half of what is left of it
-// (the caller keeps the domain, n and h unchanged).
+// Lists for one step: cells and lists from x with search_scale = 1 + skin + e.  With an extra skin e > 0 the lists are kept
+// across steps while no particle has moved more than half of it and h is unchanged.  e is
+// SPH_OPT_RK_EXTRA_SKIN, or by default automatic: in 2D whatever the caller's cell size leaves above 1 + skin (capped at
+// kAutoSkinCap; measured: 0.48 -> 0.29 ms per step at config 1, 1.35 -> 0.81 ms at config 2), none in 3D, where the
+// longer lists cost more than the rebuilds saved (profiles/r01_d_final.md).
+constexpr float kAutoSkinCap = 0.25f;
 int rebuild(sph_ctx *ctx, const sph_domain *dom, float skin, const float *x, const float *h, int64_t n, cudaStream_t st)
 {
-    const float extra = 0.001f * (float)ctx->opt_rk_extra_permille;
-    if (extra > 0.f && ctx->lists_ready && ctx->n == n && memcmp(&ctx->dom_last, dom, sizeof(*dom)) == 0 &&
-        ctx->search_scale >= 1.0f + skin) {
+    const bool automatic = ctx->opt_rk_extra_permille < 0;
+    const float extra = automatic ? 0.f : 0.001f * (float)ctx->opt_rk_extra_permille;
+    const bool reuse = automatic ? dom->dim == 2 : extra > 0.f;
+    if (reuse && ctx->lists_ready && ctx->n == n && memcmp(&ctx->dom_last, dom, sizeof(*dom)) == 0 &&
+        ctx->search_scale > 1.0f + skin) {
         int32_t ok = 0;
-        SPH_TRY(sph_lists_valid(ctx, x, skin, &ok, nullptr, (sph_stream_t)st));
+        SPH_TRY(sph_lists_valid_impl(ctx, x, h, skin, &ok, nullptr, st));
         if (ok) return SPH_OK;
     }
     SPH_TRY(sph_build_cells(ctx, dom, x, h, n, (sph_stream_t)st));
+    if (automatic && dom->dim == 2) {
+        ctx->scale_slack_cap = kAutoSkinCap;
+        const int rc = sph_neighbors(ctx, 1.0f + skin, nullptr, (sph_stream_t)st);
+        ctx->scale_slack_cap = 0.f;
+        return rc;
+    }
     return sph_neighbors(ctx, 1.0f + skin + extra, nullptr, (sph_stream_t)st);
 }
 

@@ -831,7 +831,7 @@ def test_rk_steps_with_verlet_lists_reused_across_steps(sph):
         for k in range(nsteps - 1, -1, -1):
             sph.rk_step_vjp(wl.domain, wl.params, wl.dt, skin, *states[k], dev.m, dev.h, dev.kind, xb, vb, rb, pb)
     finally:
-        sph.set_option(OPT_RK_EXTRA_SKIN, 0)
+        sph.set_option(OPT_RK_EXTRA_SKIN, -1)              # back to the default (automatic)
     assert 1 <= fills < nsteps                              # at least one reuse (TGV: |v| dt = 0.006 H per step)
     so = [(wl.x.astype(np.float64), wl.v.astype(np.float64), wl.rho.astype(np.float64))]
     for _ in range(nsteps):
@@ -844,6 +844,45 @@ def test_rk_steps_with_verlet_lists_reused_across_steps(sph):
     eg = max_norm_err(_np(vb), vo)
     print(f"verlet reuse: {fills} list builds in {nsteps} steps; increments err v {ev:.2e} rho {er:.2e}; gradient err {eg:.2e}")
     assert ev < 2e-4 and er < 2e-4 and eg < TOL_VJP
+
+
+def test_rk_steps_in_2d_reuse_lists_when_the_cells_leave_room(sph):
+    """default behaviour (SPH_OPT_RK_EXTRA_SKIN = -1, automatic): in 2D the lists take the slack of the caller's cell size
+    as a Verlet skin (PAPER.md:568) and later steps reuse them; with cells sized exactly for 1 + skin nothing changes;
+    a changed h forces a rebuild"""
+    wl = W.perturbed(W.make(1, n_axis=64), amp_x=0.0, amp_rho=0.02)
+    skin, nsteps = 0.1, 8
+    exact_cell = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin) * np.float32(1.0001))
+    dev = Dev(wl)
+
+    def run(cell):
+        wl.domain.cell_size = cell
+        sph.profile_read()
+        x, v, rho = dev.x.clone(), dev.v.clone(), dev.rho.clone()
+        for _ in range(nsteps):
+            sph.rk_step(wl.domain, wl.params, wl.dt, skin, x, v, rho, dev.m, dev.h, dev.kind)
+        return x, v, rho, sph.profile_read()["fill"][1]
+
+    xe, ve, re_, fills_exact = run(exact_cell)
+    xs, vs, rs, fills_slack = run(exact_cell * 1.2)
+    print(f"2D automatic Verlet skin: {fills_exact} list builds with exact cells, {fills_slack} with 20 % slack, {nsteps} steps")
+    assert fills_exact == nsteps and 1 <= fills_slack < nsteps
+    so = (wl.x.astype(np.float64), wl.v.astype(np.float64), wl.rho.astype(np.float64))
+    for _ in range(nsteps):
+        so = oracle.rk4_step(wl.domain, wl.params, wl.dt, *so, wl.m, wl.h, wl.kind, method=1)
+    for v_, r_ in ((ve, re_), (vs, rs)):
+        assert max_norm_err(_np(v_).astype(np.float64) - wl.v, so[1] - wl.v) < 2e-4
+        assert max_norm_err(_np(r_).astype(np.float64) - wl.rho, so[2] - wl.rho) < 2e-4
+    # same positions, other support radii: the lists of the previous call must not be reused
+    x, v, rho = dev.x.clone(), dev.v.clone(), dev.rho.clone()
+    sph.rk_step(wl.domain, wl.params, wl.dt, skin, x, v, rho, dev.m, dev.h, dev.kind)
+    sph.profile_read()
+    h2 = (dev.h * 0.97).contiguous()
+    x2, v2, rho2 = dev.x.clone(), dev.v.clone(), dev.rho.clone()
+    sph.rk_step(wl.domain, wl.params, wl.dt, skin, x2, v2, rho2, dev.m, h2, dev.kind)
+    assert sph.profile_read()["fill"][1] == 1
+    _, vo, _ = oracle.rk4_step(wl.domain, wl.params, wl.dt, wl.x, wl.v, wl.rho, wl.m, _np(h2), wl.kind, method=1)
+    assert max_norm_err(_np(v2).astype(np.float64) - wl.v, vo - wl.v) < TOL_FWD + 1e-5
 
 
 @pytest.mark.parametrize("seed", range(16))
