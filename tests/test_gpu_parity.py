@@ -123,6 +123,10 @@ def test_error_codes(sph):
     with pytest.raises(SphError) as e:
         sph.build_cells(bad, dev.x, dev.h)
     assert e.value.code == -2
+    # empty input: rejected (SPH_E_INVALID), nothing is launched
+    with pytest.raises(SphError) as e:
+        sph.build_cells(wl.domain, dev.x[:0].contiguous(), dev.h[:0].contiguous())
+    assert e.value.code == -1
     # call order
     s2 = Sph(0)
     with pytest.raises(SphError) as e:
