@@ -43,6 +43,8 @@ extern "C" int sph_destroy(sph_ctx *ctx)
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->ev_in) cudaEventDestroy(ctx->ev_in);
     if (ctx->ev_out) cudaEventDestroy(ctx->ev_out);
+    for (int c = 0; c < 4; ++c)
+        if (ctx->ev_final[c]) cudaEventDestroy(ctx->ev_final[c]);
     for (const ProfRec &r : ctx->prof.live) {
         cudaEventDestroy(r.a);
         cudaEventDestroy(r.b);
@@ -189,6 +191,9 @@ extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_doma
     SPH_TRY(sph_rhs_vjp(ctx, par, dx, dv, dr, dm, dk, ctx->hlam.as<float>(), ctx->hmu.as<float>(), ctx->ho_xb.as<float>(),
                         ctx->ho_vb.as<float>(), ctx->ho_rb.as<float>(), ctx->ho_pb.as<float>(), ss));
     SPH_CUDA_TRY(cudaEventRecord(ctx->ev_out, st));
+    // the lists of the RK4 step first: their build reads a few words back, and those read-backs must not queue behind
+    // the 100 MB of results in the device-to-host copy engine
+    SPH_TRY(sph_rk_prepare_lists(ctx, dom_rk, skin, dx, dh, n, st));
     SPH_CUDA_TRY(cudaStreamWaitEvent(cs, ctx->ev_out, 0));
     if (density) SPH_CUDA_TRY(cudaMemcpyAsync(density, ctx->ho_dens.p, ns, cudaMemcpyDeviceToHost, cs));
     if (drho_dt) SPH_CUDA_TRY(cudaMemcpyAsync(drho_dt, ctx->ho_drho.p, ns, cudaMemcpyDeviceToHost, cs));
@@ -197,14 +202,28 @@ extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_doma
     if (v_bar) SPH_CUDA_TRY(cudaMemcpyAsync(v_bar, ctx->ho_vb.p, nv, cudaMemcpyDeviceToHost, cs));
     if (rho_bar) SPH_CUDA_TRY(cudaMemcpyAsync(rho_bar, ctx->ho_rb.p, ns, cudaMemcpyDeviceToHost, cs));
     if (params_bar) SPH_CUDA_TRY(cudaMemcpyAsync(params_bar, ctx->ho_pb.p, 40, cudaMemcpyDeviceToHost, cs));
-    SPH_TRY(sph_rk_step(ctx, dom_rk, par, dt, skin, n, dx, dv, dr, dm, dh, dk, ss));
+    // the advanced state leaves in ranges of caller indices, each as soon as its part of the final update is done
+    constexpr int kFinalChunks = 4;
+    for (int c = 0; c < kFinalChunks; ++c)
+        if (!ctx->ev_final[c]) SPH_CUDA_TRY(cudaEventCreateWithFlags(&ctx->ev_final[c], cudaEventDisableTiming));
+    ctx->rk_final_chunks = kFinalChunks;
+    const int rc_rk = sph_rk_step(ctx, dom_rk, par, dt, skin, n, dx, dv, dr, dm, dh, dk, ss);
+    ctx->rk_final_chunks = 1;
+    ctx->rk_lists_prepared = false;
+    SPH_TRY(rc_rk);
     if (nnz_out) {
         nnz_out[0] = nnz0;
         nnz_out[1] = ctx->nnz;
     }
-    SPH_CUDA_TRY(cudaMemcpyAsync(x, dx, nv, cudaMemcpyDeviceToHost, st));
-    SPH_CUDA_TRY(cudaMemcpyAsync(v, dv, nv, cudaMemcpyDeviceToHost, st));
-    SPH_CUDA_TRY(cudaMemcpyAsync(rho, dr, ns, cudaMemcpyDeviceToHost, st));
+    for (int c = 0; c < kFinalChunks; ++c) {
+        const int64_t i0 = n * c / kFinalChunks, i1 = n * (c + 1) / kFinalChunks;
+        SPH_CUDA_TRY(cudaStreamWaitEvent(cs, ctx->ev_final[c], 0));
+        if (i1 <= i0) continue;
+        const size_t ov = (size_t)i0 * dom->dim, cv = (size_t)(i1 - i0) * dom->dim * 4, cs1 = (size_t)(i1 - i0) * 4;
+        SPH_CUDA_TRY(cudaMemcpyAsync(x + ov, dx + ov, cv, cudaMemcpyDeviceToHost, cs));
+        SPH_CUDA_TRY(cudaMemcpyAsync(v + ov, dv + ov, cv, cudaMemcpyDeviceToHost, cs));
+        SPH_CUDA_TRY(cudaMemcpyAsync(rho + i0, dr + i0, cs1, cudaMemcpyDeviceToHost, cs));
+    }
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
     SPH_CUDA_TRY(cudaStreamSynchronize(cs));
     return SPH_OK;

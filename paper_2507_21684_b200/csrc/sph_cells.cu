@@ -343,6 +343,7 @@ extern "C" int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float 
     if (!ctx || !dom || !x || !h || n <= 0 || n >= ((int64_t)1 << 31)) return SPH_E_INVALID;
     ctx->cells_ready = false;
     ctx->lists_ready = false;
+    ctx->rk_lists_prepared = false;
     SPH_CUDA_TRY(cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
     GridGeom gg;

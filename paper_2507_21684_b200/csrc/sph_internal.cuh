@@ -166,6 +166,11 @@ struct sph_ctx {
     // sph_step_host: copies that are not on the critical path run on their own stream
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_in = nullptr, ev_out = nullptr;
+    // sph_step_host: the final update of sph_rk_step runs in `rk_final_chunks` ranges of caller indices, each followed by
+    // an event, so that the device-to-host copy of one range overlaps the update of the next
+    int rk_final_chunks = 1;
+    bool rk_lists_prepared = false;  // sph_step_host has already run sph_rk_prepare_lists for the coming sph_rk_step
+    cudaEvent_t ev_final[4] = {nullptr, nullptr, nullptr, nullptr};
     // host staging for *_host call
     DevBuf hx, hv, hrho, hm, hh, hkind, hlam, hmu, ho_drho, ho_acc, ho_xb, ho_vb, ho_rb, ho_pb, ho_dens;
 };
@@ -291,6 +296,10 @@ int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, floa
 int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s, float *x_bar, float *m_bar,
                                 cudaStream_t st);
 int sph_launch_grad_sum_tile(sph_ctx *ctx, const KPar &kp, const float *a_s, float *g_out, cudaStream_t st);
+// the list build of sph_rk_step on its own (sph_step_host runs it before it queues its result copies: the small
+// read-backs of the build would otherwise wait behind those copies in the device-to-host copy engine)
+int sph_rk_prepare_lists(sph_ctx *ctx, const sph_domain *dom, float skin, const float *x, const float *h, int64_t n,
+                         cudaStream_t st);
 int sph_lists_valid_impl(sph_ctx *ctx, const float *x, const float *h, float skin_needed, int32_t *valid_out,
                          float *max_disp_out, cudaStream_t st);
 int sph_launch_renorm_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *rb, const float4 *rc, const float2 *rd,

@@ -143,6 +143,32 @@ __global__ void k_rk_final(int64_t n, float dt, float blast, const uint32_t *__r
     rho[i] = fmaf(dt, fmaf(blast, k.w, ax.w), rho[i]);
 }
 
+// the same update for the caller indices [i0, i1) (one thread per caller index, gathers through inv_perm)
+template <int DIM>
+__global__ void k_rk_final_range(int64_t i0, int64_t i1, float dt, float blast, const uint32_t *__restrict__ inv_perm,
+                                 const uint8_t *__restrict__ kind_s, const float4 *__restrict__ k4, StageBufs last,
+                                 const float4 *__restrict__ accx, const float4 *__restrict__ accv, float *__restrict__ x,
+                                 float *__restrict__ v, float *__restrict__ rho)
+{
+    const int64_t i = i0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= i1) return;
+    const int64_t p = inv_perm[i];
+    const float4 k = k4[p];
+    float vp[3];
+    if (DIM == 3) { const float4 t = last.s1[p]; vp[0] = t.x; vp[1] = t.y; vp[2] = t.z; }
+    else { const float4 t = last.s0[p]; vp[0] = t.z; vp[1] = t.w; vp[2] = 0.f; }
+    if (kind_s[p]) vp[0] = vp[1] = vp[2] = 0.f;
+    const float4 ax = accx[p], av = accv[p];
+    const float dx[3] = {fmaf(blast, vp[0], ax.x), fmaf(blast, vp[1], ax.y), fmaf(blast, vp[2], ax.z)};
+    const float dv[3] = {fmaf(blast, k.x, av.x), fmaf(blast, k.y, av.y), fmaf(blast, k.z, av.z)};
+#pragma unroll
+    for (int kk = 0; kk < DIM; ++kk) {
+        x[i * DIM + kk] = fmaf(dt, dx[kk], x[i * DIM + kk]);
+        v[i * DIM + kk] = fmaf(dt, dv[kk], v[i * DIM + kk]);
+    }
+    rho[i] = fmaf(dt, fmaf(blast, k.w, ax.w), rho[i]);
+}
+
 // ---- adjoint helpers ---------------------------------------------------------------------------------
 // gather the incoming cotangents ybar(t+dt) into sorted order: yx = {xbar, rhobar}, yv = {vbar, 0}
 template <int DIM>
@@ -246,6 +272,14 @@ int rebuild(sph_ctx *ctx, const sph_domain *dom, float skin, const float *x, con
 
 } // namespace
 
+int sph_rk_prepare_lists(sph_ctx *ctx, const sph_domain *dom, float skin, const float *x, const float *h, int64_t n,
+                         cudaStream_t st)
+{
+    SPH_TRY(rebuild(ctx, dom, skin, x, h, n, st));
+    ctx->rk_lists_prepared = true;
+    return SPH_OK;
+}
+
 extern "C" int sph_rk_step(sph_ctx *ctx, const sph_domain *dom, const sph_params *par, float dt, float skin, int64_t n,
                            float *x, float *v, float *rho, const float *m, const float *h, const uint8_t *kind,
                            sph_stream_t stream)
@@ -254,7 +288,8 @@ extern "C" int sph_rk_step(sph_ctx *ctx, const sph_domain *dom, const sph_params
     if (n <= 0) return SPH_E_INVALID;
     SPH_CUDA_TRY(cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
-    SPH_TRY(rebuild(ctx, dom, skin, x, h, n, st));
+    if (ctx->rk_lists_prepared) ctx->rk_lists_prepared = false;     // built by sph_rk_prepare_lists for this call
+    else SPH_TRY(rebuild(ctx, dom, skin, x, h, n, st));
     KPar kp;
     SPH_TRY(sph_kpar_make(ctx, par, &kp));
     SPH_TRY(ctx->s0.reserve((size_t)n * 16));
@@ -291,7 +326,22 @@ extern "C" int sph_rk_step(sph_ctx *ctx, const sph_domain *dom, const sph_params
         }
         SPH_TRY(sph_launch_rhs_sorted(ctx, kp, sb.s0, sb.s1, sb.s2, kind_s, nullptr, nullptr, k4, st));
     }
-    {
+    if (ctx->rk_final_chunks > 1) {
+        // sph_step_host: ranges of caller indices, an event after each (the caller copies the range out meanwhile)
+        const int C = ctx->rk_final_chunks;
+        const uint32_t *inv_perm = ctx->inv_perm.as<uint32_t>();
+        for (int cI = 0; cI < C; ++cI) {
+            const int64_t i0 = n * cI / C, i1 = n * (cI + 1) / C;
+            if (i1 > i0) {
+                KScope ks(ctx, SPH_K_RK, 1, st);
+                if (kp.dim == 3)
+                    k_rk_final_range<3><<<nb(i1 - i0), 256, 0, st>>>(i0, i1, dt, b[3], inv_perm, kind_s, k4, sb, accx, accv, x, v, rho);
+                else
+                    k_rk_final_range<2><<<nb(i1 - i0), 256, 0, st>>>(i0, i1, dt, b[3], inv_perm, kind_s, k4, sb, accx, accv, x, v, rho);
+            }
+            SPH_CUDA_TRY(cudaEventRecord(ctx->ev_final[cI], st));
+        }
+    } else {
     KScope ks(ctx, SPH_K_RK, 1, st);
     if (kp.dim == 3)
         k_rk_final<3><<<nb(n), 256, 0, st>>>(n, dt, b[3], perm, kind_s, k4, sb, accx, accv, x, v, rho);
