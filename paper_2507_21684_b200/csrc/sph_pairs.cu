@@ -1171,6 +1171,22 @@ extern "C" int sph_grad_sum_vjp(sph_ctx *ctx, const float *a, const float *g_bar
     return grad_sum_common(ctx, a, g_bar, x_bar, a_bar, true, (cudaStream_t)stream);
 }
 
+// moments M_i, b_i of the kernel renormalisation on either list layout (forward, and recomputed by the adjoint)
+static int launch_renorm_moments(sph_ctx *ctx, const KPar &kp, const float2 *va_s, float4 *mom, cudaStream_t st)
+{
+    if (ctx->tile_mode) return sph_launch_renorm_tile(ctx, kp, va_s, mom, st);
+    const int64_t n = ctx->n;
+    const float margin = seam_margin(ctx);
+#define SPH_RN_LAUNCH(DIM, GS, VARH)                                                                             \
+    k_renorm<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), va_s,  \
+                                                                ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>(), mom)
+    if (kp.dim == 3) { if (kp.uniform_h) SPH_RN_LAUNCH(3, 32, false); else SPH_RN_LAUNCH(3, 32, true); }
+    else { if (kp.uniform_h) SPH_RN_LAUNCH(2, 16, false); else SPH_RN_LAUNCH(2, 16, true); }
+#undef SPH_RN_LAUNCH
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
 extern "C" int sph_renorm_gradient(sph_ctx *ctx, const float *vol, const float *A, float rcond, float *L_out,
                                    float *grad_out, sph_stream_t stream)
 {
@@ -1191,17 +1207,7 @@ extern "C" int sph_renorm_gradient(sph_ctx *ctx, const float *vol, const float *
     KScope ks(ctx, SPH_K_DENSITY, 3, st);
     const unsigned nb1 = (unsigned)((n + 255) / 256);
     k_gather_f32x2<<<nb1, 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), vol, A, va_s);
-    if (ctx->tile_mode) {
-        SPH_TRY(sph_launch_renorm_tile(ctx, kp, va_s, mom, st));
-    } else {
-        const float margin = seam_margin(ctx);
-#define SPH_RN_LAUNCH(DIM, GS, VARH)                                                                             \
-    k_renorm<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), va_s,  \
-                                                                ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>(), mom)
-        if (kp.dim == 3) { if (kp.uniform_h) SPH_RN_LAUNCH(3, 32, false); else SPH_RN_LAUNCH(3, 32, true); }
-        else { if (kp.uniform_h) SPH_RN_LAUNCH(2, 16, false); else SPH_RN_LAUNCH(2, 16, true); }
-#undef SPH_RN_LAUNCH
-    }
+    SPH_TRY(launch_renorm_moments(ctx, kp, va_s, mom, st));
     if (kp.dim == 3) k_renorm_solve<3><<<nb1, 256, 0, st>>>(n, mom, ctx->perm.as<uint32_t>(), rcond, L_out, grad_out);
     else k_renorm_solve<2><<<nb1, 256, 0, st>>>(n, mom, ctx->perm.as<uint32_t>(), rcond, L_out, grad_out);
     SPH_CUDA_TRY(cudaGetLastError());
@@ -1237,16 +1243,7 @@ extern "C" int sph_renorm_gradient_vjp(sph_ctx *ctx, const float *vol, const flo
     const float margin = seam_margin(ctx);
     // forward moments again (nothing is kept between calls), then the per-particle adjoint of g = M^+ b
     k_gather_f32x2<<<nb1, 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), vol, A, va_s);
-    if (ctx->tile_mode) {
-        SPH_TRY(sph_launch_renorm_tile(ctx, kp, va_s, mom, st));
-    } else {
-#define SPH_RN_LAUNCH(DIM, GS, VARH)                                                                             \
-    k_renorm<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), va_s,  \
-                                                                ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>(), mom)
-        if (kp.dim == 3) { if (kp.uniform_h) SPH_RN_LAUNCH(3, 32, false); else SPH_RN_LAUNCH(3, 32, true); }
-        else { if (kp.uniform_h) SPH_RN_LAUNCH(2, 16, false); else SPH_RN_LAUNCH(2, 16, true); }
-#undef SPH_RN_LAUNCH
-    }
+    SPH_TRY(launch_renorm_moments(ctx, kp, va_s, mom, st));
     if (kp.dim == 3)
         k_renorm_solve_vjp<3><<<nb1, 256, 0, st>>>(n, mom, va_s, ctx->perm.as<uint32_t>(), grad_bar, rcond, rb, rc, rd, re);
     else
