@@ -283,6 +283,11 @@ k_nb_expand(TileGeom tg, int wcap, int wbcap, const uint32_t *__restrict__ cell_
     // per warp: image of its col16 segment (wcap entries) and the mask block of its item (wbcap words x 32 lanes)
     uint16_t *wbuf = reinterpret_cast<uint16_t *>(smem_raw) + (size_t)warp * wcap;
     uint32_t *mblk = reinterpret_cast<uint32_t *>(smem_raw + (size_t)nwarps * wcap * 2) + (size_t)warp * wbcap * 32;
+    // word table of the warp: the static one, or (rows with more than kWqCap mask words: dense cells, config 4) a
+    // dynamic one of wbcap entries behind the mask blocks
+    const uint32_t wqcap = (uint32_t)wbcap > kWqCap ? (uint32_t)wbcap : kWqCap;
+    uint16_t *wq_dyn = reinterpret_cast<uint16_t *>(smem_raw + (size_t)nwarps * ((size_t)wcap * 2 + (size_t)wbcap * 128)) +
+                       (size_t)warp * wbcap;
     int item = 0;
     long long mask_off = tile_mask_base[blockIdx.x];
     for (int tc = 0; tc < tt.nt; ++tc) {
@@ -307,7 +312,7 @@ k_nb_expand(TileGeom tg, int wcap, int wbcap, const uint32_t *__restrict__ cell_
             // the item's mask block into shared memory with cp.async (all W x 128 B in flight at once, overlapped
             // with the table build below; a plain load/store loop exposes the global latency once per word)
             const uint32_t Wi = item_words >> 5;
-            if (Wi <= kWqCap && Wi <= (uint32_t)wbcap) {
+            if (Wi <= wqcap && Wi <= (uint32_t)wbcap) {
                 const uint32_t *src = maskbuf + mask_off + lane;
                 const uint32_t dsts = (uint32_t)__cvta_generic_to_shared(mblk + lane);
                 for (uint32_t w = 0; w < Wi; ++w)
@@ -315,7 +320,7 @@ k_nb_expand(TileGeom tg, int wcap, int wbcap, const uint32_t *__restrict__ cell_
             }
             asm volatile("cp.async.commit_group;" ::: "memory");
             // candidate of bit 0 of every mask word of this cell's rows
-            uint16_t *wq = wqtab[warp];
+            uint16_t *wq = (uint32_t)wbcap > kWqCap ? wq_dyn : wqtab[warp];
             uint32_t W = 0;
             {
                 const int zlo = DIM == 3 ? -1 : 0, zhi = DIM == 3 ? 1 : 0;
@@ -330,13 +335,13 @@ k_nb_expand(TileGeom tg, int wcap, int wbcap, const uint32_t *__restrict__ cell_
                         const uint32_t q0 = tt.h_off[rowbase + xa], q1 = tt.h_off[rowbase + xb + 1];
                         const uint32_t nb = (q1 - q0 + 31u) >> 5;
                         for (uint32_t bb = lane; bb < nb; bb += 32)
-                            if (W + bb < kWqCap) wq[W + bb] = (uint16_t)(min(q0 + 32u * bb + 32u, q1) - 1u);
+                            if (W + bb < wqcap) wq[W + bb] = (uint16_t)(min(q0 + 32u * bb + 32u, q1) - 1u);
                         W += nb;
                     }
                 }
             }
             uint32_t n = 0;
-            if (W <= kWqCap && W <= (uint32_t)wbcap) {
+            if (W <= wqcap && W <= (uint32_t)wbcap) {
                 // the item's mask block into shared memory (coalesced), then every lane walks its own column at its
                 // own pace (no per-word reconvergence): ~hits + words iterations instead of sum over words of the
                 // largest popcount of the warp
@@ -662,9 +667,12 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
             if (wc > 12288) wc = 12288;
             int wb = (int)wmax_rows;                            // most mask words any row has (k_tile_words)
             if (wb < 1) wb = 1;
-            if (wb > 64) wb = 64;                               // rows beyond take the word-synchronous expansion
-            const int ew = 4;                                                       // warps per CTA
-            const size_t smem = (size_t)ew * ((size_t)wc * 2 + (size_t)wb * 128);
+            // rows with up to 64 mask words (the usual case): 4 warps per CTA, static word table.  Dense cells (config 4:
+            // ~190 words per row): the mask block of an item is up to 28 KB, so 2 warps per CTA keep three CTAs per SM;
+            // rows beyond 224 words take the word-synchronous expansion
+            if (wb > 224) wb = 224;
+            const int ew = wb > 64 ? 2 : 4;                                         // warps per CTA
+            const size_t smem = (size_t)ew * ((size_t)wc * 2 + (size_t)wb * 128 + ((uint32_t)wb > kWqCap ? (size_t)wb * 2 : 0)) + 16;
             if (gg.dim == 3) {
                 SPH_CUDA_TRY(cudaFuncSetAttribute(k_nb_expand<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                 k_nb_expand<3><<<(unsigned)tg.ntiles, ew * 32, smem, st>>>(tg, wc, wb, cs, ce, ctx->row_ptr.as<long long>(),
