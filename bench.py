@@ -39,7 +39,7 @@ if ROOT not in sys.path:
 
 METRIC = "pair_interactions_per_s"
 UNIT = "pair-interactions/s"
-SKIN = 0.06          # Verlet skin of the RK4 list: skin*H >= 2*dt*max|v| = 0.05 H for dt = 0.25 H/c0, |v| <= c0/10
+from paper_2507_21684_b200.workloads import RK_SKIN as SKIN, rk_domain   # noqa: E402  (input generation only)
 
 
 def peaks():
@@ -57,14 +57,6 @@ def make_workload(config, seed_shift, n_axis=None):
         # replicas: same recipe, different random cotangents / jitter stream
         wl.seed += 7919 * seed_shift
     return wl
-
-
-def rk_domain(wl):
-    """grid for sph_rk_step: cell_size >= (1+skin) * max h"""
-    from paper_2507_21684_b200 import workloads as W
-    d = wl.domain
-    cs = float(np.float32(np.float32(wl.h.max()) * np.float32(1.0 + SKIN) * np.float32(1.0001)))
-    return W.Domain(dim=d.dim, periodic=d.periodic, lo=d.lo, hi=d.hi, cell_size=max(cs, float(d.cell_size)))
 
 
 class ClockSampler:

@@ -213,6 +213,16 @@ def make(config: int, n_axis: int | None = None, dx: float | None = None) -> Wor
     raise ValueError("config must be 0..4")
 
 
+RK_SKIN = 0.06      # Verlet skin of the RK4 list: skin*H >= 2*dt*max|v| = 0.05 H for dt = 0.25 H/c0, |v| <= c0/10
+
+
+def rk_domain(wl: Workload, skin: float = RK_SKIN) -> Domain:
+    """grid for sph_rk_step: the same box with cell_size >= (1 + skin) * max h (input generation only)"""
+    d = wl.domain
+    cs = float(np.float32(np.float32(wl.h.max()) * np.float32(1.0 + skin) * np.float32(1.0001)))
+    return Domain(dim=d.dim, periodic=d.periodic, lo=d.lo, hi=d.hi, cell_size=max(cs, float(d.cell_size)))
+
+
 def random_cotangents(wl: Workload, seed_offset: int = 500):
     """lambda = dL/d(drho/dt), mu = dL/d(acc) ~ N(0,1) (C2, C3, C4)."""
     rng = np.random.Generator(np.random.PCG64(wl.seed + seed_offset))

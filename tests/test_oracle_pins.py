@@ -399,8 +399,11 @@ def test_rhs_delta_term_is_brookshaw_laplacian(dim, n_axis, key, exact):
     assert drho_b[c] < 0
 
 
-def test_rhs_hydrostatic_column_balances_gravity():
-    """Pressure-only a_y of a hydrostatic column ~ +g (9.70 for g = 9.81 at H = 4dx)."""
+@pytest.mark.parametrize("form", [0, 1])
+def test_rhs_hydrostatic_column_balances_gravity(form):
+    """Pressure-only a_y of a hydrostatic column ~ +g (9.70 for g = 9.81 at H = 4dx).  Both pressure forms
+    discretise the same -grad p / rho and the density varies by < 1 % over the column, so the survey's value pins the
+    MAGNITUDE of form 1 as well as of form 0 (Eq.40): a stray factor in either fails here."""
     n = 32                      # dyadic spacing: lattice positions are exact in binary32
     dx = 1.0 / n
     wl = W.make(0, n_axis=n)
@@ -408,7 +411,8 @@ def test_rhs_hydrostatic_column_balances_gravity():
     g, c0, gamma, rho0 = 9.81, 40.0, 7.0, 1000.0
     y = wl.x[:, 1].astype(np.float64)
     rho = rho0 * (1.0 + gamma * g * (1.0 - y) / c0 ** 2) ** (1.0 / gamma)
-    par = W.Params(c0=c0, rho0=rho0, gamma=gamma, delta=0.0, alpha=0.0, nu=0.0, eps=0.01, g=(0.0, 0.0, 0.0))
+    par = W.Params(c0=c0, rho0=rho0, gamma=gamma, delta=0.0, alpha=0.0, nu=0.0, eps=0.01, g=(0.0, 0.0, 0.0),
+                   pressure_form=form)
     m = np.full(wl.n, rho0 * dx * dx)
     lists = oracle.neighbors(dom, wl.x, wl.h, method=1)
     _, acc = oracle.rhs(dom, par, wl.x, 0 * wl.v, rho, m, wl.h, wl.kind, *lists)
@@ -427,6 +431,76 @@ def test_rhs_hydrostatic_column_balances_gravity():
     rho_iso = rho0 * (1.0 + g * (1.0 - y) / c0 ** 2)
     _, acc1 = oracle.rhs(dom, par1, wl.x, 0 * wl.v, rho_iso, m, wl.h, wl.kind, *lists)
     assert np.max(np.abs(acc1[interior, 1] - acc[interior, 1])) < 0.05
+
+
+def _wendland_c4_from_the_paper(r, H, dim):
+    """W(r, H) typed from PAPER.md:421-436 (Eq.25, Eq.27 with q = r/H) and the paper's printed constants."""
+    Cd = PAPER["wendland_c4_C2"] if dim == 2 else PAPER["wendland_c4_C3"]
+    q = r / H
+    return Cd / H ** dim * max(1.0 - q, 0.0) ** 6 * (1.0 + 6.0 * q + 35.0 / 3.0 * q * q)
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+@pytest.mark.parametrize("form", [0, 1])
+def test_rhs_two_particle_pressure_closed_form(dim, form):
+    """Two particles with DIFFERENT densities and masses, at rest, no viscosity, no gravity: the acceleration is one pair
+    term, a_i = -m_j e_ij grad_i W_ij with e = p_i/rho_i^2 + p_j/rho_j^2 (form 0, Eq.40) or
+    e = (p_i + p_j)/(rho_i rho_j) (form 1), p from the Tait equation PAPER.md:112 Eq.12.  grad W is taken by
+    central differences of the kernel typed from the paper's Eq.25/27 and printed constants, so nothing of the oracle
+    enters the expected value.  With rho_i != rho_j the two forms (and every symmetric look-alike such as
+    2(p_i+p_j)/(rho_i+rho_j)^2) give different numbers: this pins the magnitude of each form."""
+    H = 0.25
+    dom = W.Domain(dim=dim, periodic=(0, 0, 0), lo=(0.0,) * 3, hi=(1.0,) * dim + (0.0,) * (3 - dim), cell_size=H)
+    xi = np.array([0.40, 0.50, 0.45][:dim])
+    xj = np.array([0.52, 0.44, 0.53][:dim])
+    x = np.stack([xi, xj])
+    rho = np.array([1.07, 1.31])
+    m = np.array([0.011, 0.017])
+    c0, rho0, gamma = 12.0, 1.1, 7.0
+    par = [c0, rho0, gamma, 0.0, 0.0, 0.0, 0.01, 0.0, 0.0, 0.0]
+    h = np.full(2, H)
+    lists = oracle.neighbors(dom, x.astype(np.float32), h, method=0)
+    assert list(np.diff(lists[0])) == [2, 2]
+    _, acc = oracle.rhs(dom, None, x, 0 * x, rho, m, h, np.zeros(2, np.uint8), *lists, par_raw=oracle._par_raw(par, form))
+    p = rho0 * c0 ** 2 / gamma * ((rho / rho0) ** gamma - 1.0)                       # Eq.12
+    e = p[0] / rho[0] ** 2 + p[1] / rho[1] ** 2 if form == 0 else (p[0] + p[1]) / (rho[0] * rho[1])
+    d = xi - xj
+    r = float(np.linalg.norm(d))
+    eps = 1e-6
+    dWdr = (_wendland_c4_from_the_paper(r + eps, H, dim) - _wendland_c4_from_the_paper(r - eps, H, dim)) / (2 * eps)
+    gradW_i = dWdr * d / r                                                           # Eq.29: along x_i - x_j
+    a0 = -m[1] * e * gradW_i
+    a1 = +m[0] * e * gradW_i
+    scale = np.max(np.abs(a0))
+    assert scale > 1e-3
+    assert np.max(np.abs(acc[0] - a0)) < 1e-8 * scale and np.max(np.abs(acc[1] - a1)) < 1e-8 * scale
+    # the two forms differ by far more than the tolerance for these densities
+    other = p[0] / rho[0] ** 2 + p[1] / rho[1] ** 2 if form == 1 else (p[0] + p[1]) / (rho[0] * rho[1])
+    assert abs(other - e) > 1e-3 * abs(e)
+
+
+@pytest.mark.parametrize("cfg,kw,form", [(1, dict(n_axis=24), 0), (1, dict(n_axis=24), 1), (3, dict(n_axis=10), 0),
+                                         (4, dict(n_axis=10), 1)])
+def test_rhs_angular_momentum_conservation_in_a_bounded_domain(cfg, kw, form):
+    """pressure and viscous pair forces are central (along x_i - x_j) and antisymmetric, so in a bounded
+    domain without gravity the total torque sum_i m_i x_i x a_i vanishes to round-off (it does not in a periodic one,
+    where x_i - x_j is the minimum image)."""
+    wl = W.perturbed(W.make(cfg, **kw), amp_x=0.3, amp_rho=0.05)
+    dim = wl.dim
+    dom = W.Domain(dim=dim, periodic=(0, 0, 0), lo=(0.0,) * 3, hi=(1.0,) * dim + (0.0,) * (3 - dim),
+                   cell_size=wl.domain.cell_size)
+    par = W.Params(**{**wl.params.__dict__, "alpha": 0.05, "pressure_form": form, "g": (0.0, 0.0, 0.0)})
+    lists = oracle.neighbors(dom, wl.x, wl.h, method=1)
+    _, acc, _, sa = oracle.rhs(dom, par, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *lists, with_scales=True)
+    x = wl.x.astype(np.float64) - 0.5
+    m = wl.m.astype(np.float64)
+    if dim == 2:
+        torque = np.array([np.sum(m * (x[:, 0] * acc[:, 1] - x[:, 1] * acc[:, 0]))])
+    else:
+        torque = np.sum(m[:, None] * np.cross(x, acc), axis=0)
+    ref = np.sum(m * sa) * 0.5                       # sum of |pair forces| times the lever arm scale
+    assert np.max(np.abs(torque)) < 1e-12 * ref
+    assert np.max(np.abs(acc)) > 0
 
 
 @pytest.mark.parametrize("cfg,n_axis,key", [(0, 32, "viscous_symbol_2d_n32"), (3, 128, "viscous_symbol_3d_n128_H3dx")])
@@ -567,6 +641,11 @@ def test_rk4_taylor_green_decay_short_times():
             assert abs(_ke(wl, v) / ke0 - np.exp(-16 * np.pi ** 2 * lam * nu * wl.dt)) < 2e-5
     r10 = _ke(wl, v) / ke0
     assert abs(r10 - PINS["tgv_c0_ke_ratio_step10"]) < 2e-6
+    v10 = v
+    for step in range(11, 26):
+        x, v, rho = oracle.rk4_step(wl.domain, wl.params, wl.dt, x, v, rho, wl.m, wl.h, wl.kind, method=1)
+    assert abs(_ke(wl, v) / ke0 - PINS["tgv_c0_ke_ratio_step25"]) < 2e-6
+    v = v10
     t = 10 * wl.dt
     assert abs(r10 / np.exp(-16 * np.pi ** 2 * nu * t) - 1.0) < 0.01
     assert abs(np.sqrt(r10) / np.exp(-8 * np.pi ** 2 * nu * t) - 1.0) < 0.01     # north_star's amplitude rate
