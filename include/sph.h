@@ -235,9 +235,15 @@ enum {
                                2 = tile-local (16-bit indices into the halo of a block of cells, neighbour state staged
                                in shared memory).  2 falls back to 1 when a halo does not fit shared memory. */
     SPH_OPT_TILE_EDGE = 3,  /* edge of the cell blocks of the tile-local layout: 1, 2, 4 cells; 0 = automatic */
-    SPH_OPT_PAIR_WARPS = 4, /* warps per CTA of the tile pair kernels: 4, 8, 16; 0 = automatic */
+    SPH_OPT_PAIR_WARPS = 4, /* warps per CTA of the tile pair kernels: 4, 8, 10, 12, 16, 20, 24 (capped by a kernel's launch
+                               bound); 0 = automatic: the most resident warps shared memory and registers admit */
     SPH_OPT_FILL_MASKS = 5, /* 1 (default): the fill of the tile-local lists expands the hit masks saved by the count pass;
                                0: it repeats the distance tests (no mask buffer) */
+    SPH_OPT_UNIFORM_MASS_PATH = 7, /* 1 (default): in 3D with uniform h the tile pair kernels (sph_rhs, sph_rhs_vjp) are
+                               enqueued in two variants -- one that assumes all masses equal and gathers 32 / 48
+                               instead of 40 / 56 bytes per pair, one general -- and a device flag written by this
+                               call's own pack kernel decides which of them runs (no host synchronisation);
+                               0: only the general variant is launched */
     SPH_OPT_RK_EXTRA_SKIN = 6 /* Verlet lists across steps: value/1000 = extra skin e (in units of h).  With
                                e > 0 sph_rk_step / sph_rk_step_vjp build their lists with search_scale = 1 + skin + e
                                (the domain's cell_size must cover it) and a later call with the same domain, n and h

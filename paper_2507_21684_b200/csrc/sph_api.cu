@@ -273,7 +273,8 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
         ctx->opt_list_mode = value;
         return SPH_OK;
     case SPH_OPT_PAIR_WARPS:
-        if (value != 0 && value != 4 && value != 8 && value != 16) return SPH_E_INVALID;
+        if (value != 0 && value != 4 && value != 8 && value != 10 && value != 12 && value != 16 && value != 20 && value != 24)
+            return SPH_E_INVALID;
         ctx->opt_warps = value;
         return SPH_OK;
     case SPH_OPT_RK_EXTRA_SKIN:
@@ -286,6 +287,9 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
     case SPH_OPT_TILE_EDGE:
         if (value != 0 && value != 1 && value != 2 && value != 4) return SPH_E_INVALID;
         ctx->opt_tile_edge = value;
+        return SPH_OK;
+    case SPH_OPT_UNIFORM_MASS_PATH:
+        ctx->opt_no_um = value == 0;
         return SPH_OK;
     default:
         return SPH_E_INVALID;

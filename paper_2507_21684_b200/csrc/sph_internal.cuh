@@ -132,6 +132,7 @@ struct sph_ctx {
     sph_domain dom_last{};      // domain of the last sph_build_cells
     int opt_fill_masks = 1;     // the fill expands the hit masks saved by the count pass (0: repeats the tests)
     int opt_tile_edge = 0;      // 0 auto, else force the tile edge B (1, 2, 4)
+    int opt_no_um = 0;          // 1: never launch the uniform-mass variants of the tile pair kernels (A/B measurements, tests)
     bool tile_mode = false;     // lists of the last sph_neighbors are tile-local (col16)
     TileGeom tg{};
     uint32_t tile_Mmax = 0, tile_Tmax = 0;   // largest halo / row count of a tile
@@ -174,6 +175,11 @@ struct sph_ctx {
     // host staging for *_host call
     DevBuf hx, hv, hrho, hm, hh, hkind, hlam, hmu, ho_drho, ho_acc, ho_xb, ho_vb, ho_rb, ho_pb, ho_dens;
 };
+
+// device flag pair of the uniform-mass fast path: [0] non-zero = all masses of the last pack equal, [1] = that mass
+// (float bits).  Written on the stream by the pack kernels (k_pack_state, k_rk_base), read by the pair kernels: the
+// host never needs to know -- both variants of a pair kernel are launched and the one whose turn it is not returns.
+inline uint32_t *sph_um_flag(const sph_ctx *ctx) { return ctx->stats.as<uint32_t>() + 13; }
 
 // Counts `nlaunch` kernel launches of class `cls` and, when profiling is on, brackets them with events on `st`.
 struct KScope {

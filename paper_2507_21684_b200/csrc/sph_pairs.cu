@@ -19,7 +19,8 @@ struct Part {
     float x[3], v[3], rho, V, P, h;
 };
 
-// layouts: DIM 3: s0 = {x,y,z,h} s1 = {vx,vy,vz,rho} s2(float2) = {V,P};  DIM 2: s0 = {x,y,vx,vy} s1 = {rho,V,P,h}
+// layouts: DIM 3: s0 = {x,y,z,rho} s1 = {vx,vy,vz,P} s2(float2) = {V,h};  DIM 2: s0 = {x,y,vx,vy} s1 = {rho,V,P,h}
+// (3D: everything a pair needs when mass and h are uniform sits in s0, s1 -- the tile kernels then leave s2 out)
 template <int DIM>
 __device__ __forceinline__ Part load_part(const float4 *__restrict__ s0, const float4 *__restrict__ s1,
                                           const float2 *__restrict__ s2, int64_t j)
@@ -28,9 +29,9 @@ __device__ __forceinline__ Part load_part(const float4 *__restrict__ s0, const f
     float4 a = __ldg(s0 + j), b = __ldg(s1 + j);
     if (DIM == 3) {
         float2 c = __ldg(s2 + j);
-        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.h = a.w;
-        p.v[0] = b.x; p.v[1] = b.y; p.v[2] = b.z; p.rho = b.w;
-        p.V = c.x; p.P = c.y;
+        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.rho = a.w;
+        p.v[0] = b.x; p.v[1] = b.y; p.v[2] = b.z; p.P = b.w;
+        p.V = c.x; p.h = c.y;
     } else {
         p.x[0] = a.x; p.x[1] = a.y; p.x[2] = 0.f; p.v[0] = a.z; p.v[1] = a.w; p.v[2] = 0.f;
         p.rho = b.x; p.V = b.y; p.P = b.z; p.h = b.w;
@@ -80,11 +81,14 @@ __global__ void k_pack_state(int64_t n, KPar kp, const uint32_t *__restrict__ pe
                              const float *__restrict__ x, const float *__restrict__ v, const float *__restrict__ rho,
                              const float *__restrict__ m, const uint8_t *__restrict__ kind,
                              float4 *__restrict__ s0, float4 *__restrict__ s1, float2 *__restrict__ s2,
-                             float4 *__restrict__ eos, uint8_t *__restrict__ kind_s)
+                             float4 *__restrict__ eos, uint8_t *__restrict__ kind_s, uint32_t *__restrict__ um)
 {
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n) return;
     const int64_t i = perm[p];
+    // um[0] (preset to non-zero): cleared when the masses are not all equal; um[1] = the common mass (bits of m[0])
+    const float m_first = __ldg(m);
+    if (p == 0) um[1] = __float_as_uint(m_first);
     const float4 pb = pos_s[p];                           // wrapped build position, h
     const float xb[3] = {pb.x, pb.y, pb.z};
     float xw[3] = {0.f, 0.f, 0.f}, vv[3] = {0.f, 0.f, 0.f};
@@ -102,6 +106,7 @@ __global__ void k_pack_state(int64_t n, KPar kp, const uint32_t *__restrict__ pe
         vv[k] = v[i * DIM + k];
     }
     const float r = rho[i], mi = m[i], h = pb.w;
+    if (mi != m_first) um[0] = 0u;
     const float u = (r - kp.rho0) / kp.rho0;
     const float lg = log1pf(u);
     const float ugm1 = expm1f(kp.gamma * lg);        // (rho/rho0)^gamma - 1
@@ -110,9 +115,9 @@ __global__ void k_pack_state(int64_t n, KPar kp, const uint32_t *__restrict__ pe
     const float ir = 1.0f / r, ir2 = ir * ir;
     const float V = mi * ir, P = pr * ir2;
     if (DIM == 3) {
-        s0[p] = make_float4(xw[0], xw[1], xw[2], h);
-        s1[p] = make_float4(vv[0], vv[1], vv[2], r);
-        s2[p] = make_float2(V, P);
+        s0[p] = make_float4(xw[0], xw[1], xw[2], r);
+        s1[p] = make_float4(vv[0], vv[1], vv[2], P);
+        s2[p] = make_float2(V, h);
     } else {
         s0[p] = make_float4(xw[0], xw[1], vv[0], vv[1]);
         s1[p] = make_float4(r, V, P, h);
@@ -959,9 +964,11 @@ int pack_state(sph_ctx *ctx, const KPar &kp, const float *x, const float *v, con
     SPH_TRY(ctx->kind_s.reserve((size_t)n));
     if (with_eos) SPH_TRY(ctx->eos.reserve((size_t)n * 16));
     KScope ks(ctx, SPH_K_PACK, 1, st);
+    SPH_CUDA_TRY(cudaMemsetAsync(sph_um_flag(ctx), 1, 4, st));       // "masses uniform" until a thread finds otherwise
     k_pack_state<DIM><<<(unsigned)((n + 255) / 256), 256, 0, st>>>(
         n, kp, ctx->perm.as<uint32_t>(), ctx->pos_s.as<float4>(), x, v, rho, m, kind, ctx->s0.as<float4>(),
-        ctx->s1.as<float4>(), ctx->s2.as<float2>(), with_eos ? ctx->eos.as<float4>() : nullptr, ctx->kind_s.as<uint8_t>());
+        ctx->s1.as<float4>(), ctx->s2.as<float2>(), with_eos ? ctx->eos.as<float4>() : nullptr, ctx->kind_s.as<uint8_t>(),
+        sph_um_flag(ctx));
     return SPH_OK;
 }
 

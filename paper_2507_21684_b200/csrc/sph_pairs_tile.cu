@@ -16,7 +16,8 @@
 
 namespace {
 
-constexpr int kPtMaxWarps = 16;
+constexpr int kPtMaxWarps = 16;      // launch bound of the light pair kernels (<= 128 registers)
+constexpr int kVjpMaxWarps = 21;     // k_vjp_tile: the bound of 672 threads caps it at 96 registers, so that 20 warps fit one SM
 
 template <int GS>
 __device__ __forceinline__ float group_sum(float v)
@@ -154,20 +155,28 @@ __device__ __forceinline__ void tile_row_passes(const TileTab &tt, const uint32_
 }
 
 // sorted state of one particle as the pair loops see it
-// layouts: DIM 3: s0 = {x,y,z,h} s1 = {vx,vy,vz,rho} s2(float2) = {V,P};  DIM 2: s0 = {x,y,vx,vy} s1 = {rho,V,P,h}
+// layouts: DIM 3: s0 = {x,y,z,rho} s1 = {vx,vy,vz,P} s2(float2) = {V,h};  DIM 2: s0 = {x,y,vx,vy} s1 = {rho,V,P,h}
+// UM (3D, uniform mass m0 and uniform h): s2 is not staged at all -- V = m0/rho costs one MUFU and one multiply against
+// a third gather with its bank conflicts (the shared-memory data pipe is the binding unit, profiles/r01_g)
 struct Part {
     float x[3], v[3], rho, V, P, h;
 };
-template <int DIM>
-__device__ __forceinline__ Part load_part(const float4 *s0, const float4 *s1, const float2 *s2, uint32_t j)
+template <int DIM, bool UM = false>
+__device__ __forceinline__ Part load_part(const float4 *s0, const float4 *s1, const float2 *s2, uint32_t j, float m0 = 0.f,
+                                          float H = 0.f)
 {
     Part p;
     const float4 a = s0[j], b = s1[j];
     if (DIM == 3) {
-        const float2 c = s2[j];
-        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.h = a.w;
-        p.v[0] = b.x; p.v[1] = b.y; p.v[2] = b.z; p.rho = b.w;
-        p.V = c.x; p.P = c.y;
+        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.rho = a.w;
+        p.v[0] = b.x; p.v[1] = b.y; p.v[2] = b.z; p.P = b.w;
+        if (UM) {
+            p.V = m0 * fast_rcp(a.w);
+            p.h = H;
+        } else {
+            const float2 c = s2[j];
+            p.V = c.x; p.h = c.y;
+        }
     } else {
         p.x[0] = a.x; p.x[1] = a.y; p.x[2] = 0.f; p.v[0] = a.z; p.v[1] = a.w; p.v[2] = 0.f;
         p.rho = b.x; p.V = b.y; p.P = b.z; p.h = b.w;
@@ -186,13 +195,13 @@ struct SmemMap {
     float2 *C;
     uint32_t *rp;
     uint16_t *selfq, *ring;
-    __device__ SmemMap(unsigned char *base, const TileSizes &ts, bool with_cot)
+    __device__ SmemMap(unsigned char *base, const TileSizes &ts, bool with_cot, bool with_C = true)
     {
         size_t o = 0;
         A = reinterpret_cast<float4 *>(base + o); o += (size_t)ts.mcap * 16;
         B = reinterpret_cast<float4 *>(base + o); o += (size_t)ts.mcap * 16;
         cot = reinterpret_cast<float4 *>(base + o); if (with_cot) o += (size_t)ts.mcap * 16;
-        C = reinterpret_cast<float2 *>(base + o); if (DIM == 3) o += (size_t)ts.mcap * 8;
+        C = reinterpret_cast<float2 *>(base + o); if (DIM == 3 && with_C) o += (size_t)ts.mcap * 8;
         rp = reinterpret_cast<uint32_t *>(base + o); o += (size_t)(ts.tcap + 4) * 4;
         selfq = reinterpret_cast<uint16_t *>(base + o); o += (size_t)ts.tcap * 2;
         o = (o + 15) & ~(size_t)15;
@@ -545,20 +554,25 @@ k_grad_sum_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ p
 // ------------------------------------------------------------------------------------------ R1: RHS
 // OUT_SORTED: write float4 {a, drho/dt} in sorted order (RK stages); else scatter to the caller's arrays.
 // F1: pressure form 1, (p_i + p_j)/(rho_i rho_j), instead of the symmetric Eq.40
-template <int DIM, int GS, bool VARH, bool OUT_SORTED, bool F1>
+// UM: uniform-mass variant (3D, uniform h).  `um` = sph_um_flag: a launch whose UM does not match the flag returns at
+// once, so the host can enqueue both variants without knowing the masses (um == nullptr: run unconditionally)
+template <int DIM, int GS, bool VARH, bool OUT_SORTED, bool F1, bool UM>
 __global__ void __launch_bounds__(kPtMaxWarps * 32)
 k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, const float4 *__restrict__ s1,
            const float2 *__restrict__ s2, const uint8_t *__restrict__ kind_s, const uint32_t *__restrict__ cell_start,
            const uint32_t *__restrict__ cell_end, const long long *__restrict__ row_ptr,
            const uint16_t *__restrict__ col16, const uint32_t *__restrict__ perm, float *__restrict__ drho_out,
-           float *__restrict__ acc_out, float4 *__restrict__ out4)
+           float *__restrict__ acc_out, float4 *__restrict__ out4, const uint32_t *__restrict__ um)
 {
+    static_assert(!UM || (DIM == 3 && !VARH), "the uniform-mass variant is the 3D, uniform-h one");
+    if (um && (um[0] != 0u) != UM) return;
+    const float m0 = UM ? __uint_as_float(um[1]) : 0.f;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const SmemMap<DIM> sm(smem_raw, ts, false);
+    const SmemMap<DIM> sm(smem_raw, ts, false, !UM);
     __shared__ TileTab tt;
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
     if (tt.T == 0) return;
-    stage_halo(tt, s0, sm.A, s1, sm.B, nullptr, nullptr, DIM == 3 ? s2 : nullptr, sm.C, nullptr, nullptr);
+    stage_halo(tt, s0, sm.A, s1, sm.B, nullptr, nullptr, (DIM == 3 && !UM) ? s2 : nullptr, sm.C, nullptr, nullptr);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
     cp_async_wait<0>();
     __syncthreads();
@@ -572,7 +586,7 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
     const uint32_t row0 = tt.row0;
     tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
         [&](uint32_t r, bool live, uint32_t b, uint32_t e, const uint16_t *idx) {
-            const Part pi = load_part<DIM>(A, B, C, selfq[r]);
+            const Part pi = load_part<DIM, UM>(A, B, C, selfq[r], m0, kp.H);
             const float ir_i = fast_rcp(pi.rho);
             const float visc_i = rho0 * ir_i;                 // rho0/rho_i of the viscous term
             const float ev_u = hu.eta * visc_i;
@@ -582,7 +596,7 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
 #pragma unroll 2
             for (uint32_t k = b + gl; k < e; k += GS) {
                 const uint32_t j = idx[k];
-                const Part pj = load_part<DIM>(A, B, C, j);
+                const Part pj = load_part<DIM, UM>(A, B, C, j, m0, kp.H);
                 const float d0 = pi.x[0] - pj.x[0], d1 = pi.x[1] - pj.x[1], d2 = DIM == 3 ? pi.x[2] - pj.x[2] : 0.f;
                 const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
                 HC hc = hu;
@@ -606,7 +620,8 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                 sD = VARH ? fmaf(hc.kd, dterm, sD) : sD + dterm;
                 // pressure (Eq.40, symmetric) + viscosity (Eq.7 with the delta-SPH Pi_ij)
                 // E = -m_j e,  e = P_i + P_j (Eq.40)  or  (p_i + p_j)/(rho_i rho_j) = (p_i/rho_i + p_j/rho_i)/rho_j
-                const float E = F1 ? -pj.V * fmaf(pj.P * pj.rho * pj.rho, ir_i, Pr_i) : -(pj.V * pj.rho) * (pi.P + pj.P);
+                const float mj = UM ? m0 : pj.V * pj.rho;
+                const float E = F1 ? -pj.V * fmaf(pj.P * pj.rho * pj.rho, ir_i, Pr_i) : -mj * (pi.P + pj.P);
                 const float cf = fmaf(ev * pj.V * s, invR, E) * G;
                 a0 = fmaf(cf, d0, a0);
                 a1 = fmaf(cf, d1, a1);
@@ -642,25 +657,28 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
 // are reduced per CTA in a fixed order (B2 stage 1); one CTA = one tile = one partials record.
 constexpr int kNPartT = 12;   // must match kNPart of sph_pairs.cu (k_reduce_params)
 
-template <int DIM, int GS, bool VARH, bool OUT_SORTED, bool F1>
-__global__ void __launch_bounds__(kPtMaxWarps * 32)
+template <int DIM, int GS, bool VARH, bool OUT_SORTED, bool F1, bool UM>
+__global__ void __launch_bounds__(kVjpMaxWarps * 32)
 k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, const float4 *__restrict__ s1,
            const float2 *__restrict__ s2, const float4 *__restrict__ cot, const float4 *__restrict__ eos,
            const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
            const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16, const uint32_t *__restrict__ perm,
            float *__restrict__ xb_out, float *__restrict__ vb_out, float *__restrict__ rb_out, float4 *__restrict__ xb4,
-           float4 *__restrict__ vb4, float *__restrict__ partials)
+           float4 *__restrict__ vb4, float *__restrict__ partials, const uint32_t *__restrict__ um)
 {
+    static_assert(!UM || (DIM == 3 && !VARH), "the uniform-mass variant is the 3D, uniform-h one");
+    if (um && (um[0] != 0u) != UM) return;          // see k_rhs_tile
+    const float m0 = UM ? __uint_as_float(um[1]) : 0.f;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const SmemMap<DIM> sm(smem_raw, ts, true);
+    const SmemMap<DIM> sm(smem_raw, ts, true, !UM);
     __shared__ TileTab tt;
-    __shared__ float red[kPtMaxWarps][kNPartT];
+    __shared__ float red[kVjpMaxWarps][kNPartT];
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
     if (tt.T == 0) {
         if (threadIdx.x < kNPartT) partials[(int64_t)blockIdx.x * kNPartT + threadIdx.x] = 0.f;
         return;
     }
-    stage_halo(tt, s0, sm.A, s1, sm.B, cot, sm.cot, DIM == 3 ? s2 : nullptr, sm.C, nullptr, nullptr);
+    stage_halo(tt, s0, sm.A, s1, sm.B, cot, sm.cot, (DIM == 3 && !UM) ? s2 : nullptr, sm.C, nullptr, nullptr);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
     cp_async_wait<0>();
     __syncthreads();
@@ -677,17 +695,17 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
     tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
         [&](uint32_t r, bool live, uint32_t b, uint32_t e_in, const uint16_t *idx) {
             const uint32_t qi = selfq[r];
-            const Part pi = load_part<DIM>(A, B, C, qi);
+            const Part pi = load_part<DIM, UM>(A, B, C, qi, m0, kp.H);
             const float4 ci = Ct[qi];
             const float lam_i = ci.x, mu_i[3] = {ci.y, ci.z, ci.w};
-            const float m_i = pi.V * pi.rho, Vi = pi.V, Li = lam_i * pi.rho;
+            const float m_i = UM ? m0 : pi.V * pi.rho, Vi = pi.V, Li = lam_i * pi.rho;
             const uint32_t e = live ? e_in : b;                    // padding groups run no pairs (partials stay clean)
             const float ir_i = 1.0f / pi.rho;
             const float p_i = pi.P * pi.rho * pi.rho;             // form 1: the pressure itself
             float xb[3] = {0.f, 0.f, 0.f}, vb[3] = {0.f, 0.f, 0.f}, rb = 0.f, Z = 0.f, Zr = 0.f;
             for (uint32_t k = b + gl; k < e; k += GS) {
                 const uint32_t j = idx[k];
-                const Part pj = load_part<DIM>(A, B, C, j);
+                Part pj = load_part<DIM, UM>(A, B, C, j, m0, kp.H);
                 const float4 cj = Ct[j];
                 const float lam_j = cj.x, mu_j[3] = {cj.y, cj.z, cj.w};
                 const float d[3] = {pi.x[0] - pj.x[0], pi.x[1] - pj.x[1], DIM == 3 ? pi.x[2] - pj.x[2] : 0.f};
@@ -706,7 +724,8 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                 const float invR = fast_rcp(r2 + hc.e2);
                 const float u = r2 * invR;
                 const float ir_j = fast_rcp(pj.rho);
-                const float m_j = pj.V * pj.rho;
+                const float m_j = UM ? m0 : pj.V * pj.rho;
+                if (UM) pj.V = m0 * ir_j;                           // the same MUFU result load_part used
                 const float drho = pi.rho - pj.rho;
                 // pressure pair factor e: E = -m_j e, E' = -m_i e;  e = P_i + P_j (Eq.40) or (p_i + p_j)/(rho_i rho_j)
                 const float W2 = ir_i * ir_j;
@@ -849,9 +868,13 @@ static int tile_group(const sph_ctx *ctx, bool vjp)
     return g == 4 ? 8 : g;
 }
 
-// threads per CTA, shared-memory carve-up and size for a pair kernel with `state_bytes` per halo particle
-static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, size_t static_smem, int *threads, TileSizes *ts,
-                            size_t *smem)
+// threads per CTA, shared-memory carve-up and size for a pair kernel with `state_bytes` per halo particle, at most
+// `max_warps` warps per CTA (its launch bound) and about `regs` registers per thread.  Picks the (CTAs per SM, warps per
+// CTA) pair with the most resident warps that shared memory (228 KB per SM, 227 KB per CTA, 1 KB reserved per CTA) and
+// the register file (64 K per SM, allocated per warp in units of 256) admit; ties go to more CTAs (measured on C3,
+// profiles/r01_c: two co-resident CTAs beat one of twice the size -- their staging and epilogue phases overlap).
+static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, size_t static_smem, int max_warps, int regs,
+                            int *threads, TileSizes *ts, size_t *smem)
 {
     ts->mcap = (int)((ctx->tile_Mmax + 7u) & ~7u);
     ts->tcap = (int)((ctx->tile_Tmax + 7u) & ~7u);
@@ -861,13 +884,22 @@ static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, size_t 
     if (rb < 64) rb = 64;
     ts->rb = rb;
     const size_t fixed = (size_t)ts->mcap * state_bytes + (size_t)(ts->tcap + 4) * 4 + (size_t)ts->tcap * 2 + 16;
-    const size_t sm_total = 233472, per_cta = 1024 + static_smem, cta_max = 232448 - static_smem;   // B200: 228 KB per SM, 227 KB per CTA
+    const size_t sm_total = 233472, per_cta = 1024 + static_smem, cta_max = 232448 - static_smem;
     auto need = [&](int warps) { return fixed + (size_t)warps * 2 * rb * 2; };
-    // measured (C3): two co-resident CTAs beat one (their staging and epilogue phases overlap), and at equal
-    // residency 16 warps beat 8: the largest CTA of which two fit an SM, else one 16-warp CTA
-    int warps = 16;
-    if (ctx->opt_warps) warps = ctx->opt_warps;
-    else if (sm_total / (need(16) + per_cta) < 2 && sm_total / (need(8) + per_cta) >= 2) warps = 8;
+    const int regs_warp = ((regs + 7) & ~7) * 32;
+    int warps = 0, best = 0;
+    if (ctx->opt_warps) {
+        warps = ctx->opt_warps < max_warps ? ctx->opt_warps : max_warps;
+    } else {
+        const int cand[] = {24, 20, 16, 12, 10, 8, 6, 4};
+        for (int c = 4; c >= 1; --c)
+            for (int w : cand) {
+                if (w > max_warps || need(w) > cta_max) continue;
+                if ((size_t)c * (need(w) + per_cta) > sm_total || (long)c * w * regs_warp > 65536 || c * w > 64) continue;
+                if (c * w > best) { best = c * w; warps = w; }
+            }
+    }
+    if (warps == 0) warps = 2;
     while (warps > 2 && need(warps) > cta_max) warps >>= 1;           // tile_setup needs two warps
     if (need(warps) > cta_max) {                                   // last resort: a minimal ring (rows fall back to global reads)
         ts->rb = 8;
@@ -886,7 +918,7 @@ int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, floa
     int threads;
     TileSizes ts;
     size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);   // same carve-up as the RHS kernel (SmemMap)
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), kPtMaxWarps, 64, &threads, &ts, &smem);   // same carve-up as the RHS kernel (SmemMap)
 #define SPH_DT_LAUNCH(DIM, GS, VARH)                                                                                  \
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_density_tile<DIM, GS, VARH>), smem);                                                    \
@@ -918,7 +950,7 @@ int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s
     int threads;
     TileSizes ts;
     size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);   // carve-up of SmemMap
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), kPtMaxWarps, 64, &threads, &ts, &smem);   // carve-up of SmemMap
 #define SPH_DVT_LAUNCH(DIM, GS, VARH)                                                                                 \
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_density_vjp_tile<DIM, GS, VARH>), smem);                                                \
@@ -949,7 +981,7 @@ int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float2 *va_s, flo
     int threads;
     TileSizes ts;
     size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);   // carve-up of SmemMap
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), kPtMaxWarps, 64, &threads, &ts, &smem);   // carve-up of SmemMap
 #define SPH_RNT_LAUNCH(DIM, GS, VARH)                                                                                 \
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_renorm_tile<DIM, GS, VARH>), smem);                                                     \
@@ -981,7 +1013,7 @@ int sph_launch_renorm_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *rb, c
     int threads;
     TileSizes ts;
     size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 60 : 44, gs, sizeof(TileTab), &threads, &ts, &smem);   // carve-up of k_renorm_vjp_tile
+    tile_launch_cfg(ctx, kp.dim == 3 ? 60 : 44, gs, sizeof(TileTab), kPtMaxWarps, 96, &threads, &ts, &smem);   // carve-up of k_renorm_vjp_tile
 #define SPH_RNVT_LAUNCH(DIM, GS, VARH)                                                                                \
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_renorm_vjp_tile<DIM, GS, VARH>), smem);                                                 \
@@ -1014,7 +1046,7 @@ static int launch_grad_sum_tile(sph_ctx *ctx, const KPar &kp, const float *a_s, 
     int threads;
     TileSizes ts;
     size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);   // carve-up of SmemMap
+    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), kPtMaxWarps, 64, &threads, &ts, &smem);   // carve-up of SmemMap
 #define SPH_GT_LAUNCH(DIM, GS, VARH, VJP)                                                                             \
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_grad_sum_tile<DIM, GS, VARH, VJP>), smem);                                              \
@@ -1055,22 +1087,36 @@ int sph_launch_grad_sum_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *ga_
     return launch_grad_sum_tile(ctx, kp, nullptr, ga_s, x_bar, a_bar, true, st);
 }
 
+// Both pair kernels come in a general variant and (3D, uniform h) a uniform-mass one that gathers 32 / 48 instead of
+// 40 / 56 bytes per pair.  Whether the masses are uniform is known on the device only (sph_um_flag, written by the pack
+// kernel of this call on the same stream), so both variants are enqueued, each with its own shared-memory carve-up, and
+// the one whose turn it is not returns in its first instruction.
 int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
                         const uint8_t *kind_s, float *drho, float *acc, float4 *out4, cudaStream_t st)
 {
     const TileGeom &tg = ctx->tg;
     const int gs = tile_group(ctx, false);
-    int threads;
-    TileSizes ts;
-    size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), &threads, &ts, &smem);
     const bool sorted = out4 != nullptr;
+    const bool dual = kp.dim == 3 && kp.uniform_h && !ctx->opt_no_um;
+    const uint32_t *um = dual ? sph_um_flag(ctx) : nullptr;
+    for (int pass = 0; pass < (dual ? 2 : 1); ++pass) {
+        const bool UMv = dual && pass == 0;
+        int threads;
+        TileSizes ts;
+        size_t smem;
+        tile_launch_cfg(ctx, kp.dim == 3 ? (UMv ? 32 : 40) : 32, gs, sizeof(TileTab), kPtMaxWarps, 64, &threads, &ts, &smem);
+        if (pass == 1) ctx->launches += 1;                     // the second variant is a launch too
+#define SPH_RT_LAUNCH2(DIM, GS, VARH, SORTED, F1, UM)                                                                \
+    do {                                                                                                             \
+        SPH_TILE_SMEM_ATTR((k_rhs_tile<DIM, GS, VARH, SORTED, F1, UM>), smem);                                       \
+        k_rhs_tile<DIM, GS, VARH, SORTED, F1, UM><<<(unsigned)tg.ntiles, threads, smem, st>>>(                       \
+            tg, kp, ts, s0, s1, s2, kind_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),            \
+            ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), drho, acc, out4, um); \
+    } while (0)
 #define SPH_RT_LAUNCH1(DIM, GS, VARH, SORTED, F1)                                                                    \
     do {                                                                                                             \
-        SPH_TILE_SMEM_ATTR((k_rhs_tile<DIM, GS, VARH, SORTED, F1>), smem);                                           \
-        k_rhs_tile<DIM, GS, VARH, SORTED, F1><<<(unsigned)tg.ntiles, threads, smem, st>>>(                           \
-            tg, kp, ts, s0, s1, s2, kind_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),            \
-            ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), drho, acc, out4);     \
+        if (DIM == 3 && !VARH && UMv) SPH_RT_LAUNCH2(3, GS, false, SORTED, F1, true);                                \
+        else SPH_RT_LAUNCH2(DIM, GS, VARH, SORTED, F1, false);                                                       \
     } while (0)
 #define SPH_RT_LAUNCH(DIM, GS, VARH, SORTED)                                                                         \
     do {                                                                                                             \
@@ -1086,14 +1132,16 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
             else { if (sorted) SPH_RT_LAUNCH(2, GS, true, true); else SPH_RT_LAUNCH(2, GS, true, false); }                \
         }                                                                                                               \
     } while (0)
-    switch (gs) {
-    case 16: SPH_RT_GS(16); break;
-    case 32: SPH_RT_GS(32); break;
-    default: SPH_RT_GS(8); break;
-    }
+        switch (gs) {
+        case 16: SPH_RT_GS(16); break;
+        case 32: SPH_RT_GS(32); break;
+        default: SPH_RT_GS(8); break;
+        }
 #undef SPH_RT_GS
 #undef SPH_RT_LAUNCH
 #undef SPH_RT_LAUNCH1
+#undef SPH_RT_LAUNCH2
+    }
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
@@ -1104,18 +1152,29 @@ int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
 {
     const TileGeom &tg = ctx->tg;
     const int gs = tile_group(ctx, true);
-    int threads;
-    TileSizes ts;
-    size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 56 : 48, gs, sizeof(TileTab) + kPtMaxWarps * kNPartT * 4, &threads, &ts, &smem);
     const bool sorted = xb4 != nullptr;
-#define SPH_VT_LAUNCH1(DIM, GS, VARH, SORTED, F1)                                                                     \
+    const bool dual = kp.dim == 3 && kp.uniform_h && !ctx->opt_no_um;
+    const uint32_t *um = dual ? sph_um_flag(ctx) : nullptr;
+    for (int pass = 0; pass < (dual ? 2 : 1); ++pass) {
+        const bool UMv = dual && pass == 0;
+        int threads;
+        TileSizes ts;
+        size_t smem;
+        tile_launch_cfg(ctx, kp.dim == 3 ? (UMv ? 48 : 56) : 48, gs, sizeof(TileTab) + kVjpMaxWarps * kNPartT * 4, kVjpMaxWarps, 80, &threads,
+                        &ts, &smem);
+        if (pass == 1) ctx->launches += 1;
+#define SPH_VT_LAUNCH2(DIM, GS, VARH, SORTED, F1, UM)                                                                 \
     do {                                                                                                              \
-        SPH_TILE_SMEM_ATTR((k_vjp_tile<DIM, GS, VARH, SORTED, F1>), smem);                                            \
-        k_vjp_tile<DIM, GS, VARH, SORTED, F1><<<(unsigned)tg.ntiles, threads, smem, st>>>(                            \
+        SPH_TILE_SMEM_ATTR((k_vjp_tile<DIM, GS, VARH, SORTED, F1, UM>), smem);                                        \
+        k_vjp_tile<DIM, GS, VARH, SORTED, F1, UM><<<(unsigned)tg.ntiles, threads, smem, st>>>(                        \
             tg, kp, ts, s0, s1, s2, cot, eos, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),           \
             ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), xb, vb, rb, xb4, vb4,  \
-            partials);                                                                                                \
+            partials, um);                                                                                            \
+    } while (0)
+#define SPH_VT_LAUNCH1(DIM, GS, VARH, SORTED, F1)                                                                     \
+    do {                                                                                                              \
+        if (DIM == 3 && !VARH && UMv) SPH_VT_LAUNCH2(3, GS, false, SORTED, F1, true);                                 \
+        else SPH_VT_LAUNCH2(DIM, GS, VARH, SORTED, F1, false);                                                        \
     } while (0)
 #define SPH_VT_LAUNCH(DIM, GS, VARH, SORTED)                                                                          \
     do {                                                                                                              \
@@ -1131,14 +1190,16 @@ int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
             else { if (sorted) SPH_VT_LAUNCH(2, GS, true, true); else SPH_VT_LAUNCH(2, GS, true, false); }                \
         }                                                                                                               \
     } while (0)
-    switch (gs) {
-    case 16: SPH_VT_GS(16); break;
-    case 32: SPH_VT_GS(32); break;
-    default: SPH_VT_GS(8); break;
-    }
+        switch (gs) {
+        case 16: SPH_VT_GS(16); break;
+        case 32: SPH_VT_GS(32); break;
+        default: SPH_VT_GS(8); break;
+        }
 #undef SPH_VT_GS
 #undef SPH_VT_LAUNCH
 #undef SPH_VT_LAUNCH1
+#undef SPH_VT_LAUNCH2
+    }
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

@@ -42,9 +42,9 @@ __device__ __forceinline__ void store_stage(const StageBufs &sb, int64_t p, cons
     float4 e;
     eos_eval(kp, r, mi, V, P, sb.eos ? &e : nullptr);
     if (DIM == 3) {
-        sb.s0[p] = make_float4(X[0], X[1], X[2], h);
-        sb.s1[p] = make_float4(Vv[0], Vv[1], Vv[2], r);
-        sb.s2[p] = make_float2(V, P);
+        sb.s0[p] = make_float4(X[0], X[1], X[2], r);
+        sb.s1[p] = make_float4(Vv[0], Vv[1], Vv[2], P);
+        sb.s2[p] = make_float2(V, h);
     } else {
         sb.s0[p] = make_float4(X[0], X[1], Vv[0], Vv[1]);
         sb.s1[p] = make_float4(r, V, P, h);
@@ -58,11 +58,13 @@ __global__ void k_rk_base(int64_t n, KPar kp, const uint32_t *__restrict__ perm,
                           const float *__restrict__ x, const float *__restrict__ v, const float *__restrict__ rho,
                           const float *__restrict__ m,
                           const uint8_t *__restrict__ kind, float4 *__restrict__ b0, float4 *__restrict__ b1,
-                          float *__restrict__ m_s, uint8_t *__restrict__ kind_s, StageBufs sb)
+                          float *__restrict__ m_s, uint8_t *__restrict__ kind_s, StageBufs sb, uint32_t *__restrict__ um)
 {
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n) return;
     const int64_t i = perm[p];
+    const float m_first = __ldg(m);                          // uniform-mass flag pair (sph_um_flag)
+    if (p == 0) um[1] = __float_as_uint(m_first);
     const float4 ps = pos_s[p];                              // wrapped build positions (R4) + h
     // current position: the periodic image next to the build position (identical to it when the lists were built
     // from x in this call; differs when Verlet lists are reused across steps)
@@ -80,6 +82,7 @@ __global__ void k_rk_base(int64_t n, KPar kp, const uint32_t *__restrict__ perm,
         Vv[k] = v[i * DIM + k];
     }
     const float r = rho[i], mi = m[i];
+    if (mi != m_first) um[0] = 0u;
     b0[p] = make_float4(X[0], X[1], X[2], ps.w);
     b1[p] = make_float4(Vv[0], Vv[1], Vv[2], r);
     m_s[p] = mi;
@@ -309,10 +312,11 @@ extern "C" int sph_rk_step(sph_ctx *ctx, const sph_domain *dom, const sph_params
 
     {
     KScope ks(ctx, SPH_K_RK, 1, st);
+    SPH_CUDA_TRY(cudaMemsetAsync(sph_um_flag(ctx), 1, 4, st));
     if (kp.dim == 3)
-        k_rk_base<3><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x, v, rho, m, kind, b0, b1, m_s, kind_s, sb);
+        k_rk_base<3><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x, v, rho, m, kind, b0, b1, m_s, kind_s, sb, sph_um_flag(ctx));
     else
-        k_rk_base<2><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x, v, rho, m, kind, b0, b1, m_s, kind_s, sb);
+        k_rk_base<2><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x, v, rho, m, kind, b0, b1, m_s, kind_s, sb, sph_um_flag(ctx));
     }
     const float c[4] = {0.f, 0.5f, 0.5f, 1.f};
     const float b[4] = {1.f / 6.f, 1.f / 3.f, 1.f / 3.f, 1.f / 6.f};
@@ -397,10 +401,11 @@ extern "C" int sph_rk_step_vjp(sph_ctx *ctx, const sph_domain *dom, const sph_pa
     // forward sweep: recompute and keep the four stage states
     {
     KScope ks(ctx, SPH_K_RK, 1, st);
+    SPH_CUDA_TRY(cudaMemsetAsync(sph_um_flag(ctx), 1, 4, st));
     if (kp.dim == 3)
-        k_rk_base<3><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x0, v0, rho0_state, m, kind, b0, b1, m_s, kind_s, S[0]);
+        k_rk_base<3><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x0, v0, rho0_state, m, kind, b0, b1, m_s, kind_s, S[0], sph_um_flag(ctx));
     else
-        k_rk_base<2><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x0, v0, rho0_state, m, kind, b0, b1, m_s, kind_s, S[0]);
+        k_rk_base<2><<<nb(n), 256, 0, st>>>(n, kp, perm, ctx->pos_s.as<float4>(), x0, v0, rho0_state, m, kind, b0, b1, m_s, kind_s, S[0], sph_um_flag(ctx));
     }
     for (int s = 1; s < 4; ++s) {
         SPH_TRY(sph_launch_rhs_sorted(ctx, kp, S[s - 1].s0, S[s - 1].s1, S[s - 1].s2, kind_s, nullptr, nullptr, k4, st));

@@ -317,6 +317,36 @@ def test_rhs_parity(sph, case):
         assert np.all(_np(acc)[wl.kind == 1] == 0.0)
 
 
+def test_uniform_mass_variant_and_general_variant_agree(sph):
+    """3D, uniform h: sph_rhs / sph_rhs_vjp enqueue a uniform-mass variant of the tile pair kernels and a general one; a
+    device flag set by the pack kernel picks the one that runs (include/sph.h SPH_OPT_UNIFORM_MASS_PATH).  Equal masses:
+    both variants against the oracle.  One particle with a different mass: the flag must flip to the general variant
+    (the uniform-mass one would be wrong by 30 % on that particle's neighbours)."""
+    from paper_2507_21684_b200.binding import OPT_UNIFORM_MASS_PATH
+    wl = CASES["C3p"]()
+    lam, mu = W.random_cotangents(wl)
+    lists = oracle_lists(wl)
+    for variant in ("equal", "one_heavier"):
+        m = wl.m.copy()
+        if variant == "one_heavier":
+            m[wl.n // 2] *= np.float32(1.3)
+        d_o, a_o, sd, sa = oracle.rhs(wl.domain, wl.params, wl.x, wl.v, wl.rho, m, wl.h, wl.kind, *lists, with_scales=True)
+        xo, vo, ro, po = oracle.rhs_vjp(wl.domain, wl.params, wl.x, wl.v, wl.rho, m, wl.h, wl.kind, *lists, lam, mu)
+        for um_path in (1, 0):
+            sph.set_option(OPT_UNIFORM_MASS_PATH, um_path)
+            try:
+                _, dev, _ = build(wl, 1.0, sph)
+                m_dev = torch.from_numpy(m).cuda()
+                drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, m_dev, dev.kind)
+                _check_forward(f"C3p masses {variant}, uniform-mass path {um_path}", _np(drho), _np(acc), d_o, a_o, sd, sa, FLOOR)
+                xb, vb, rb, pb = sph.rhs_vjp(wl.params, dev.x, dev.v, dev.rho, m_dev, dev.kind, torch.from_numpy(lam).cuda(),
+                                             torch.from_numpy(mu).cuda())
+                assert max(max_norm_err(_np(xb), xo), max_norm_err(_np(vb), vo), max_norm_err(_np(rb), ro)) < TOL_VJP
+                assert _params_err(_np(pb), po) < TOL_VJP
+            finally:
+                sph.set_option(OPT_UNIFORM_MASS_PATH, 1)
+
+
 @pytest.mark.parametrize("case", ["C0p", "C2p", "C3p", "C4s"])
 def test_pressure_form_1_rhs_vjp_and_rk_parity(sph, case):
     """pressure_form = 1: -m_j (p_i + p_j)/(rho_i rho_j), the form of the paper's own WCSPH scheme (reading
