@@ -239,6 +239,9 @@ enum {
                                bound); 0 = automatic: the most resident warps shared memory and registers admit */
     SPH_OPT_FILL_MASKS = 5, /* 1 (default): the fill of the tile-local lists expands the hit masks saved by the count pass;
                                0: it repeats the distance tests (no mask buffer) */
+    SPH_OPT_BUILD_FUSED = 8, /* 1 (default): the tile-local lists are built by ONE kernel per build (tests, offsets by a
+                               decoupled look-back over the tiles, fill; the hit masks stay in shared memory);
+                               0: count / scan / fill as three steps with the masks in global memory */
     SPH_OPT_UNIFORM_MASS_PATH = 7, /* 1 (default): in 3D with uniform h the tile pair kernels (sph_rhs, sph_rhs_vjp) are
                                enqueued in two variants -- one that assumes all masses equal and gathers 32 / 48
                                instead of 40 / 56 bytes per pair, one general -- and a device flag written by this

@@ -17,7 +17,7 @@ extern "C" int sph_create(sph_ctx **out, int device, int64_t n_max)
     if (!ctx) return SPH_E_NOMEM;
     ctx->device = device;
     ctx->n_hint = n_max;
-    if (cudaMallocHost((void **)&ctx->h_pinned, 16 * sizeof(int64_t)) != cudaSuccess) {
+    if (cudaMallocHost((void **)&ctx->h_pinned, 64 * sizeof(int64_t)) != cudaSuccess) {
         (void)cudaGetLastError();
         delete ctx;
         return SPH_E_NOMEM;
@@ -33,7 +33,7 @@ extern "C" int sph_destroy(sph_ctx *ctx)
     cudaDeviceSynchronize();
     DevBuf *bufs[] = {&ctx->key_a, &ctx->key_b, &ctx->idx_a, &ctx->idx_b, &ctx->hist, &ctx->perm, &ctx->inv_perm,
                       &ctx->key_sorted, &ctx->pos_s, &ctx->cell_start, &ctx->cell_end, &ctx->stats, &ctx->cnt,
-                      &ctx->row_ptr, &ctx->col, &ctx->col16, &ctx->scan_tmp, &ctx->maskbuf, &ctx->tile_words, &ctx->tile_mask_base, &ctx->s0, &ctx->s1, &ctx->s2, &ctx->s3, &ctx->c0buf,
+                      &ctx->row_ptr, &ctx->col, &ctx->col16, &ctx->scan_tmp, &ctx->maskbuf, &ctx->tile_words, &ctx->tile_mask_base, &ctx->fstats, &ctx->tstate, &ctx->fctl, &ctx->tile_orders[0].buf, &ctx->tile_orders[1].buf, &ctx->tile_orders[2].buf, &ctx->tile_orders[3].buf, &ctx->s0, &ctx->s1, &ctx->s2, &ctx->s3, &ctx->c0buf,
                       &ctx->out4, &ctx->m_s, &ctx->kind_s, &ctx->partials, &ctx->eos, &ctx->hx, &ctx->hv, &ctx->hrho,
                       &ctx->hm, &ctx->hh, &ctx->hkind, &ctx->hlam, &ctx->hmu, &ctx->ho_drho, &ctx->ho_acc, &ctx->ho_xb,
                       &ctx->ho_vb, &ctx->ho_rb, &ctx->ho_pb, &ctx->ho_dens};
@@ -287,6 +287,9 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
     case SPH_OPT_TILE_EDGE:
         if (value != 0 && value != 1 && value != 2 && value != 4) return SPH_E_INVALID;
         ctx->opt_tile_edge = value;
+        return SPH_OK;
+    case SPH_OPT_BUILD_FUSED:
+        ctx->opt_build_fused = value != 0;
         return SPH_OK;
     case SPH_OPT_UNIFORM_MASS_PATH:
         ctx->opt_no_um = value == 0;

@@ -132,6 +132,8 @@ struct sph_ctx {
     sph_domain dom_last{};      // domain of the last sph_build_cells
     int opt_fill_masks = 1;     // the fill expands the hit masks saved by the count pass (0: repeats the tests)
     int opt_tile_edge = 0;      // 0 auto, else force the tile edge B (1, 2, 4)
+    int opt_fused_warps = 0;    // warps per CTA of the one-kernel build (0 = default)
+    int opt_build_fused = 1;    // 1: the tile-local lists are built by the one-kernel build (sph_neighbors_fused.cu) when a tile fits it
     int opt_no_um = 0;          // 1: never launch the uniform-mass variants of the tile pair kernels (A/B measurements, tests)
     bool tile_mode = false;     // lists of the last sph_neighbors are tile-local (col16)
     TileGeom tg{};
@@ -157,6 +159,19 @@ struct sph_ctx {
     // lists
     DevBuf cnt, row_ptr, col, col16, scan_tmp;
     DevBuf maskbuf, tile_words, tile_mask_base;   // hit masks of the count pass, per-tile mask offsets
+    // one-kernel build: cell statistics, look-back states, {ticket, overflow}, tiles in Morton order (cached per grid)
+    DevBuf fstats, tstate, fctl;
+    struct TileOrder {                            // cache slot: the order depends on the grid and on B only
+        DevBuf buf;
+        bool valid = false;
+        int B = 0, dim = 0, nb[3] = {0, 0, 0};
+    } tile_orders[4];
+    int tile_order_next = 0;                      // slot replaced next
+    const uint32_t *tile_order_cur = nullptr;     // order of the current build (device)
+    std::vector<uint32_t> tile_order_host;
+    uint32_t f_ncmax = 0;                         // largest candidate count of a cell (k_cell_stats)
+    unsigned long long f_pairs = 0;               // sum over rows of their candidate counts: upper bound of nnz
+    int64_t n_lists = 0;                          // n of the lists `nnz` belongs to
     bool col_valid = false;     // ctx->col holds the global-id lists of the current build
     // pair scratch (sorted SoA)
     DevBuf s0, s1, s2, s3, c0buf, out4, m_s, kind_s, partials, eos;
@@ -318,6 +333,10 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
 int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
                         const float4 *cot, const float4 *eos, float *xb, float *vb, float *rb, float4 *xb4, float4 *vb4,
                         float *partials, cudaStream_t st);
+struct SearchPar;
+int sph_fused_stats_launch(sph_ctx *ctx, cudaStream_t st);
+int sph_neighbors_fused_run(sph_ctx *ctx, const SearchPar &sp, const TileGeom &tg, uint32_t Mmax, uint32_t Tmax,
+                            uint32_t ncmax, unsigned long long pairs_bound, cudaStream_t st, int64_t *nnz_out);
 int sph_scan_u32(sph_ctx *ctx, const uint32_t *in, void *out, bool out64, int64_t m, cudaStream_t st);
 int sph_kpar_make(const sph_ctx *ctx, const sph_params *par, KPar *kp);
 int sph_launch_rhs_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,

@@ -290,12 +290,23 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
     int cand[3], ncand = 0;
     if (ctx->opt_list_mode != 1) ncand = sph_tile_candidates(ctx, cand);
     if (ncand) SPH_TRY(sph_tile_stats_launch(ctx, cand, ncand, st));
+    const bool fused_stats = ncand && ctx->opt_build_fused;
+    if (fused_stats) {
+        SPH_TRY(sph_fused_stats_launch(ctx, st));
+        SPH_CUDA_TRY(cudaMemcpyAsync(ctx->h_pinned + 16, ctx->fstats.p, 16, cudaMemcpyDeviceToHost, st));
+    }
     // the statistics of sph_build_cells (error flag, max/min h) are needed on the host to size the search
     uint32_t hs[11];
     uint32_t *hpin = reinterpret_cast<uint32_t *>(ctx->h_pinned + 8);
     SPH_CUDA_TRY(cudaMemcpyAsync(hpin, ctx->stats.p, 44, cudaMemcpyDeviceToHost, st));
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
     memcpy(hs, hpin, 44);
+    ctx->f_ncmax = 0;
+    ctx->f_pairs = 0;
+    if (fused_stats) {
+        memcpy(&ctx->f_ncmax, ctx->h_pinned + 16, 4);
+        memcpy(&ctx->f_pairs, ctx->h_pinned + 17, 8);
+    }
     if (hs[0] != 0u) return SPH_E_DOMAIN;
     float hmax, hmin;
     memcpy(&hmax, &hs[1], 4);

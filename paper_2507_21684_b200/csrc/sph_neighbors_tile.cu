@@ -587,6 +587,11 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
     const int64_t n = ctx->n;
     const GridGeom &gg = ctx->geom;
     const TileGeom tg = make_tile_geom(gg, B);
+    if (ctx->opt_build_fused && ctx->f_ncmax) {
+        // the one-kernel build (sph_neighbors_fused.cu); 1 = a tile does not fit its shared-memory carve-up
+        const int rc = sph_neighbors_fused_run(ctx, sp, tg, Mmax, Tmax, ctx->f_ncmax, ctx->f_pairs, st, nnz_out);
+        if (rc != 1) return rc;
+    }
     const bool varh = ctx->hmin != ctx->hmax;
     const int mcap = (int)((Mmax + 7u) & ~7u);
     SPH_TRY(ctx->cnt.reserve((size_t)n * 4));
@@ -696,6 +701,7 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
     ctx->tile_Tmax = Tmax;
     ctx->col_valid = false;
     ctx->nnz = nnz;
+    ctx->n_lists = n;
     if (nnz_out) *nnz_out = nnz;
     return SPH_OK;
 }

@@ -7,7 +7,8 @@ import torch
 
 import oracle
 from paper_2507_21684_b200 import workloads as W
-from paper_2507_21684_b200.binding import Sph, SphError, OPT_LIST_MODE, OPT_TILE_EDGE, OPT_FILL_MASKS, LIST_GENERIC
+from paper_2507_21684_b200.binding import (Sph, SphError, OPT_LIST_MODE, OPT_TILE_EDGE, OPT_FILL_MASKS, OPT_BUILD_FUSED,
+                                           LIST_GENERIC)
 from common import max_norm_err, per_row_err, floor_for, FLOOR, FLOOR_LATTICE
 from gpu_common import Dev, build, oracle_lists, fuzz_workload, renorm_errors, renorm_good_rows
 
@@ -62,6 +63,7 @@ def sph(request):
         s.set_option(OPT_LIST_MODE, LIST_GENERIC)
     elif request.param == "tile_b1":
         s.set_option(OPT_TILE_EDGE, 1)
+        s.set_option(OPT_BUILD_FUSED, 0)
         s.set_option(OPT_FILL_MASKS, 0)          # this variant also covers the fill that repeats the distance tests
     yield s
     s.close()
