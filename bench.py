@@ -238,6 +238,9 @@ def main():
     ap.add_argument("--n-axis", type=int, default=None, help="shrink the lattice (debugging only; invalid as a result)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="sph_set_option before the run (integer keys of include/sph.h, e.g. 9=0: rows in stored order); "
+                         "repeatable.  For A/B measurements: the line records it in config.options")
     ap.add_argument("--ref-rows", type=int, default=100000)
     ap.add_argument("--cpu-budget", type=float, default=12.0)
     args = ap.parse_args()
@@ -279,6 +282,9 @@ def main():
     dens = torch.empty_like(rho); drho = torch.empty_like(rho); acc = torch.empty_like(v)
     vjp_out = (torch.empty_like(x), torch.empty_like(v), torch.empty_like(rho), torch.empty(10, dtype=torch.float32, device=dev))
     sph = Sph(local_rank, n)
+    for kv in args.opt:
+        k_, v_ = kv.split("=")
+        sph.set_option(int(k_), int(v_))
     ev = lambda: torch.cuda.Event(enable_timing=True)
     phases = ("rebuild", "density", "fwd", "bwd", "rk4")
     marks = []                                       # per timed step: 6 events

@@ -1,6 +1,9 @@
 """Build libsph_b200.so (the C-ABI CUDA library, include/sph.h) in-tree with nvcc for sm_100a.
 
-    python -m paper_2507_21684_b200.build [--force] [--verbose]
+    python -m paper_2507_21684_b200.build [--force] [--verbose] [--bounds]
+
+--bounds: debug build with -DSPH_BOUNDS (checked shared-memory indices in the tile kernels, sph_internal.cuh); it
+replaces the library in place, so rebuild with --force afterwards.
 
 nvcc cross-compiles without a GPU.  No --use_fast_math: the neighbour predicate and the position wrap
 are fixed sequences of IEEE operations (readings R3/R4); fast approximations are used
@@ -29,14 +32,16 @@ def _stale():
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
+def build(force: bool = False, verbose: bool = False, bounds: bool = False) -> str:
+    if not force and not bounds and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     flags = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC"]
     if verbose:
         flags = ["-Xptxas", "-v"] + flags
-    objdir = os.path.join(HERE, "_obj")
+    if bounds:
+        flags = flags + ["-DSPH_BOUNDS"]
+    objdir = os.path.join(HERE, "_obj_bounds" if bounds else "_obj")
     os.makedirs(objdir, exist_ok=True)
     srcs = sources()
     objs = [os.path.join(objdir, os.path.basename(f)[:-3] + ".o") for f in srcs]
@@ -59,4 +64,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, bounds="--bounds" in sys.argv))

@@ -223,6 +223,26 @@ struct KScope {
 };
 
 // ------------------------------------------------------------------------------------------
+// Debug build (python -m paper_2507_21684_b200.build --bounds, i.e. -DSPH_BOUNDS): every shared-memory gather index, ring
+// offset and staging offset of the tile kernels is checked; a violation prints its source line and is counted in
+// sph_bounds_count (read with sph_debug_bounds_violations()).  compute-sanitizer is closed on the GPU pool this was
+// developed on; this stands in for memcheck on the hand-carved shared-memory layouts.
+#ifdef SPH_BOUNDS
+#include <stdio.h>
+static __device__ unsigned int sph_bounds_count = 0;   // one per translation unit (no -rdc); summed by sph_api.cu
+#define SPH_ASSERT(cond)                                                                                              \
+    do {                                                                                                              \
+        if (!(cond)) {                                                                                                \
+            if (atomicAdd(&sph_bounds_count, 1u) < 16u)                                                               \
+                printf("SPH_BOUNDS %s:%d block %d thread %d: %s\n", __FILE__, __LINE__, (int)blockIdx.x,              \
+                       (int)threadIdx.x, #cond);                                                                      \
+        }                                                                                                             \
+    } while (0)
+#else
+#define SPH_ASSERT(cond) ((void)0)
+#endif
+
+// ------------------------------------------------------------------------------------------
 // device helpers
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ float fast_sqrt(float x)
