@@ -11,10 +11,15 @@ One "step" is one pass of the whole hot path (every SURVEY.md 8(a) row) over the
     sph_rhs_vjp (lambda, mu ~ N(0,1))         R0, B1, B2
     sph_rk_step(dt, skin)                     N1-N7 again on the skin grid, 4 x (R0, R1), T  -> advances the state
 
-`value` = pair interactions per second, a pair interaction being one CSR entry processed by one pair pass
-(SURVEY.md 8(d)): per step  3 * nnz(exact list) + 4 * nnz(skin list), summed over all ranks, divided by the
-max-over-ranks device time.  The north-star figure "ms per forward+backward RHS step" is reported beside it as
-`ms_fwd_bwd` (sph_rhs + sph_rhs_vjp only) with `pairs_per_s_fwd_bwd` = 2 nnz / that time.
+`value` = pair interactions per second, a pair interaction being one pair with r < H processed by one pair pass
+(self pairs included): per step 7 x nnz(exact list), summed over all ranks, divided by the
+max-over-ranks device time.  The RK list carries a Verlet skin; its entries beyond H contribute exactly 0, are no work
+of the method and are NOT counted (`value_on_list_entries` = 3 nnz(exact) + 4 nnz(skin) is printed beside it).
+The headline loop runs with the library's per-class profiling OFF; `kernels` comes from a second, untimed loop.
+The north-star figure "ms per forward+backward RHS step" and its HBM / FP32 fractions sit inside `roofline`
+(`ms_fwd_bwd`, `hbm_frac_fwd_bwd`, `hbm_frac_fwd_bwd_of_8TBs`, `fp32_frac_fwd_bwd`).  `roofline.traffic` is NOT
+measured in the run: it is the ncu capture named by `roofline.traffic_source` (profiles/traffic.json), printed only
+for the workload and layout it was taken on.  `--opt KEY=VALUE` passes sph_set_option knobs (A/B runs, sweeps).
 
 N > 1: the path does not shard in this round ("replicas only"): every rank runs an
 independent replica of the workload (different seed), no data-path collective; weak scaling.
@@ -129,18 +134,23 @@ def algorithmic_bytes(cls, n, nnz, dim, idx_bytes):
         return idx_bytes * nnz + 8 * (n + 1) + n * (state + 16 + 16 + 32)        # + cotangents + EOS derivs + {xbar,rhobar},{vbar}
     if cls == "density":
         return idx_bytes * nnz + 8 * (n + 1) + n * (16 + 4 + 4 + 4)              # pos, m, perm, rho
-    if cls in ("count", "fill"):
-        return (idx_bytes * nnz if cls == "fill" else 0) + n * (16 + 4) + 8 * n  # pos + cnt/row_ptr (+ lists written)
+    if cls == "fill":                                # the one-kernel list build: positions in, lists + row_ptr + cnt out
+        return idx_bytes * nnz + n * (16 + 8 + 4)
     return None
 
 
-def measured_traffic():
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture"""
+def measured_traffic(workload, layout_mode):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
+    (profiles/traffic.json).  NOT measured in this run: returned with its source, and only for the workload and list
+    layout the captures were taken on."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     try:
-        return json.load(open(p))
+        d = json.load(open(p))
     except Exception:
         return {}
+    if d.get("workload") != workload or d.get("layout") != layout_mode:
+        return {}
+    return {k: v for k, v in d.items() if isinstance(v, dict)}
 
 
 def reduce_over_ranks(ms_local, units_local, device="cpu"):
@@ -185,6 +195,9 @@ def cpu_sample(wl, budget_s=12.0, seed=3):
         p1, d1, nr = run(want)
         pairs, dt, passes = pairs + p1, dt + d1, passes + 1
     return {"value": pairs / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "note": "the parity oracle as it stands (plain fp64 C, OpenMP over rows), NOT a tuned CPU implementation; it runs "
+                    "the two pair passes sph_rhs + sph_rhs_vjp only (no neighbour search, no RK4), so it is a stated "
+                    "baseline for the pair-pass rate and no like-for-like ratio to `value` is claimed",
             "sample": f"oracle.rhs + oracle.rhs_vjp (fp64, OpenMP) on {passes} x {nr} sampled rows of {wl.name} "
                       f"({pairs} pair interactions in {dt:.2f} s); oracle grid neighbour search over all "
                       f"{wl.n} particles took {t_lists:.2f} s and is not in the figure"}, (rp, ci)
@@ -316,9 +329,9 @@ def main():
     sph.check()
     layout = sph.layout()
     idx_bytes = 2 if layout["mode"] == 2 else 4
-    sph.profile_read()                               # clear accumulators
+    # headline loop: class profiling OFF (its ~60 event records per step stay out of the timed region)
+    sph.profile_enable(False)
     launches0 = sph.info()["launches"]
-    sph.profile_enable(True)
     barrier()
     clocks = ClockSampler(local_rank) if rank == 0 else None
     t_start, t_stop = ev(), ev()
@@ -328,19 +341,32 @@ def main():
     t_stop.record()
     barrier()
     clk = clocks.stop() if clocks else None
-    sph.profile_enable(False)
     ms_total = t_start.elapsed_time(t_stop)
-    prof = sph.profile_read()
     launches = sph.info()["launches"] - launches0
     sph.check()
+    # second loop, not part of `value`: per-class device times (sph_profile_enable brackets every launch with events)
+    prof_steps = max(1, min(args.steps, 5))
+    sph.profile_read()                               # clear accumulators
+    sph.profile_enable(True)
+    for _ in range(prof_steps):
+        step(False)
+    torch.cuda.synchronize()
+    sph.profile_enable(False)
+    prof = sph.profile_read()
     assert torch.isfinite(vjp_out[0]).all() and torch.isfinite(x).all(), "non-finite state after the timed steps"
 
-    pairs_rank = 3 * counts["nnz"] + 4 * counts["nnz_rk"]
+    # work of a step.  list_entries: CSR entries the seven pair passes walk (3 on the exact list, 4 on the RK list with
+    # its Verlet skin).  pairs_in_support: pairs with r < H only -- the entries of the skin list beyond H contribute
+    # exactly 0 and are no work of the method; the four RK stages are counted with the exact list's size (the state moves
+    # by < 3 % of H within a step).  `value` is quoted on pairs_in_support.
+    entries_rank = 3 * counts["nnz"] + 4 * counts["nnz_rk"]
+    pairs_rank = 7 * counts["nnz"]
     ph_ms = {p: float(np.mean([mk[i].elapsed_time(mk[i + 1]) for mk in marks])) for i, p in enumerate(phases)}
     fb_ms = ph_ms["fwd"] + ph_ms["bwd"]
     nnz_mean = counts["nnz"] / args.steps
 
     ms_max, pairs_all = reduce_over_ranks(ms_total, pairs_rank, dev)
+    _, entries_all = reduce_over_ranks(ms_total, entries_rank, dev)
     value = pairs_all / (ms_max * 1e-3)
 
     # ---- NEXT-1 row, outside the timed step: adjoint of the summation density (the paper's
@@ -398,7 +424,7 @@ def main():
         t0 = time.perf_counter()
         for _ in range(ke):
             a, b = sph.step_host(dom, dom_rk, par, wl.dt, SKIN, hx, hv, hr, hm, hh, hk, hl, hmu, outs)
-            pairs_e += 3 * a + 4 * b
+            pairs_e += 7 * a                          # pairs in support, as for `value`
         torch.cuda.synchronize()
         dt_e = time.perf_counter() - t0
         te_max, pe_sum = reduce_over_ranks(dt_e, pairs_e, dev)
@@ -413,25 +439,24 @@ def main():
         tot_k = sum(ms for ms, _ in prof.values()) or 1.0
         for name, (ms, cnt) in prof.items():
             if cnt:
-                kern[name] = {"ms_per_step": ms / args.steps, "launches_per_step": cnt / args.steps,
+                kern[name] = {"ms_per_step": ms / prof_steps, "launches_per_step": cnt / prof_steps,
                               "share": ms / tot_k}
         # dominant kernel among the classes with a stated byte model
-        cand = [c for c in ("rhs", "vjp", "density", "count", "fill") if c in kern]
+        cand = [c for c in ("rhs", "vjp", "density", "fill") if c in kern]
         dom_cls = max(cand, key=lambda c: kern[c]["ms_per_step"])
-        nnz_for = {"rhs": (counts["nnz"] + 4 * counts["nnz_rk"]) / (5.0 * args.steps), "vjp": nnz_mean, "density": nnz_mean,
-                   "count": (counts["nnz"] + counts["nnz_rk"]) / (2.0 * args.steps),
-                   "fill": (counts["nnz"] + counts["nnz_rk"]) / (2.0 * args.steps)}
+        # algorithmic work per launch is counted on pairs in support (see above), also for the four RK launches
+        nnz_for = {"rhs": nnz_mean, "vjp": nnz_mean, "density": nnz_mean,
+                   "fill": (counts["nnz"] + counts["nnz_rk"]) / (2.0 * args.steps)}    # entries written per build
         roof = {}
-        traffic = measured_traffic()
+        traffic = measured_traffic(wl.name, layout["mode"])
         fp32_peak = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12       # TFLOP/s, FMA = 2 flop
         for c in cand:
             ms_launch = prof[c][0] / max(prof[c][1] / (2 if c == "density" else 1), 1)
-            if c == "count":                         # the class also holds the tiny tile-statistics launches
-                ms_launch = prof[c][0] / (2.0 * args.steps)
             by = algorithmic_bytes(c, n, nnz_for[c], dim, idx_bytes)
-            tr = traffic.get(c)
+            tr = traffic.get(c, {}).get("bytes")
+            tr_src = traffic.get(c, {}).get("source")
             hbm_view = {"bound": "hbm", "achieved": by / (ms_launch * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
-                        "frac": by / (ms_launch * 1e-3) / 1e9 / hbm, "traffic": tr, "kernel": c,
+                        "frac": by / (ms_launch * 1e-3) / 1e9 / hbm, "traffic": tr, "traffic_source": tr_src, "kernel": c,
                         "ms_per_launch": ms_launch, "algorithmic_bytes_per_launch": int(by), "peak_source": hbm_src}
             if c in FLOP_PER_PAIR:
                 # the pair kernels are bound by FP32 issue / shared-memory gathers, not by HBM (profiles/): their
@@ -439,7 +464,7 @@ def main():
                 fl = FLOP_PER_PAIR[c] * nnz_for[c]
                 ach = fl / (ms_launch * 1e-3) / 1e12
                 roof[c] = {"bound": "alu", "achieved": ach, "peak": fp32_peak, "unit": "TFLOP/s", "frac": ach / fp32_peak,
-                           "traffic": tr, "kernel": c, "ms_per_launch": ms_launch,
+                           "traffic": tr, "traffic_source": tr_src, "kernel": c, "ms_per_launch": ms_launch,
                            "algorithmic_flop_per_launch": fl, "flop_per_pair": FLOP_PER_PAIR[c],
                            "peak_source": f"{N_SM} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max:.0f} MHz "
                                           "(unit counts of the guides, clocks.max.sm of MEASURED_PEAKS.json)",
@@ -447,22 +472,40 @@ def main():
             else:
                 roof[c] = hbm_view
         fb_bytes = algorithmic_bytes("rhs", n, nnz_mean, dim, idx_bytes) + algorithmic_bytes("vjp", n, nnz_mean, dim, idx_bytes)
+        fb_flop = (FLOP_PER_PAIR["rhs"] + FLOP_PER_PAIR["vjp"]) * nnz_mean
+        # BASELINE.json's metric -- ms per forward+backward RHS step at this config and the fraction of the HBM peak --
+        # rides inside `roofline` so that it is part of every parsed record; the FP32 fraction is the binding roof
+        # (with 2-byte indices the arithmetic needs 3.5x the time of the bytes)
+        fwd_bwd = {"ms_fwd_bwd": fb_ms, "pairs_per_s_fwd_bwd": 2.0 * nnz_mean / (fb_ms * 1e-3),
+                   "hbm_frac_fwd_bwd": fb_bytes / (fb_ms * 1e-3) / 1e9 / hbm,
+                   "hbm_frac_fwd_bwd_of_8TBs": fb_bytes / (fb_ms * 1e-3) / 1e9 / 8000.0,
+                   "fp32_frac_fwd_bwd": fb_flop / (fb_ms * 1e-3) / 1e12 / fp32_peak,
+                   "algorithmic_bytes_fwd_bwd": int(fb_bytes), "algorithmic_flop_fwd_bwd": fb_flop}
+        roof_main = dict(roof[dom_cls])
+        roof_main.update(fwd_bwd)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl.name, "n_particles": n, "dim": dim, "nnz_exact_list": int(nnz_last),
                        "nnz_skin_list": int(nnz_rk_last), "skin": SKIN, "replicas": world,
+                       "pairs_in_support_per_step": int(pairs_all / args.steps),
+                       "list_entries_per_step": int(entries_all / args.steps),
+                       "value_counts": "pairs in support (r < H): 7 x nnz of the exact list per step; the RK list's "
+                                       "entries beyond H contribute exactly 0 and are not counted",
+                       "options": list(args.opt),
                        "list_layout": {1: "generic int32 ids", 2: "tile-local uint16"}[layout["mode"]],
                        "tile_edge_cells": layout["tile_edge"], "tile_halo_max": layout["halo_max"],
                        "step": "build_cells+neighbors, density, rhs, rhs_vjp, rk_step(rebuild + 4 rhs)",
                        "l2": "inputs larger than L2: every pair pass streams its 0.45-0.55 GB list (2 B per entry) and the "
                              "rebuild writes it; per step > 4 GB of list traffic against L2 = 126 MB"},
+            "value_on_list_entries": entries_all / (ms_max * 1e-3),
             "ms_fwd_bwd": fb_ms, "pairs_per_s_fwd_bwd": 2.0 * nnz_mean / (fb_ms * 1e-3),
-            "hbm_frac_fwd_bwd": fb_bytes / (fb_ms * 1e-3) / 1e9 / hbm,
-            "hbm_frac_fwd_bwd_of_8TBs": fb_bytes / (fb_ms * 1e-3) / 1e9 / 8000.0,
-            "phase_ms": ph_ms, "kernels": kern,
-            "roofline": roof[dom_cls], "roofline_all": roof,
+            "hbm_frac_fwd_bwd": fwd_bwd["hbm_frac_fwd_bwd"],
+            "hbm_frac_fwd_bwd_of_8TBs": fwd_bwd["hbm_frac_fwd_bwd_of_8TBs"],
+            "phase_ms": ph_ms, "kernels": kern, "kernels_note": f"per-class device times from a second loop of {prof_steps} "
+            "steps with sph_profile_enable(1); the headline loop runs with profiling off",
+            "roofline": roof_main, "roofline_all": roof,
             "gpu_launches": int(launches), "clocks": clk, "next_rows": extras,
         }
         if e2e:
