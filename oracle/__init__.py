@@ -208,7 +208,23 @@ def renorm_gradient_vjp(domain, x, h, vol, A, row_ptr, col_idx, grad_bar, rcond=
     return xb, vb, ab
 
 
-def rhs(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, rows=None, with_scales=False, par_raw=None):
+def _delta_form(params, delta_form):
+    if delta_form is not None:
+        return int(delta_form)
+    return int(getattr(params, "delta_form", 0)) if params is not None else 0
+
+
+def _rcond(params, rcond):
+    if rcond is not None:
+        return float(rcond)
+    return float(getattr(params, "renorm_rcond", 1e-4)) if params is not None else 1e-4
+
+
+def rhs(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, rows=None, with_scales=False, par_raw=None,
+        delta_form=None, rcond=None):
+    """drho/dt and acceleration.  delta_form 1 (params.delta_form or the argument): the delta-term of
+    [43] with the renormalised density gradient -- orc_rhs's Molteni-Colagrossi term plus orc_delta_renorm_term, with
+    <grad rho>^L from renorm_gradient(vol = m/rho, A = rho)."""
     dim, per, lo, hi = _dom(domain)
     par = _par(params) if par_raw is None else par_raw
     x, v, rho, m, h = _d(x), _d(v), _d(rho), _d(m), _d(h)
@@ -216,7 +232,8 @@ def rhs(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, rows=None, with
     n = x.shape[0]
     drho = np.zeros(n)
     acc = np.zeros((n, dim))
-    sd = np.zeros(n) if with_scales else None
+    dform = _delta_form(params, delta_form)
+    sd = np.zeros(n) if (with_scales or dform) else None
     sa = np.zeros(n) if with_scales else None
     rp = np.ascontiguousarray(row_ptr, np.int64)
     ci = np.ascontiguousarray(col_idx, np.int32)
@@ -224,12 +241,22 @@ def rhs(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, rows=None, with
     lib().orc_rhs(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(par), _p(x), _p(v), _p(rho), _p(m), _p(h),
                   _p(kind), _p(rp), _p(ci), _p(rows_a), C.c_int64(0 if rows is None else len(rows_a)),
                   _p(drho), _p(acc), _p(sd), _p(sa))
+    if dform == 1:
+        _, g, _ = renorm_gradient(domain, x, h, m / rho, rho, rp, ci, rcond=_rcond(params, rcond))
+        g = np.ascontiguousarray(g)
+        lib().orc_delta_renorm_term(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(par), _p(x), _p(rho), _p(m),
+                                    _p(h), _p(rp), _p(ci), _p(g), _p(rows_a), C.c_int64(0 if rows is None else len(rows_a)),
+                                    _p(drho), _p(sd))
     if with_scales:
         return drho, acc, sd, sa
     return drho, acc
 
 
-def rhs_vjp(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, drho_bar, acc_bar, rows=None, par_raw=None):
+def rhs_vjp(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, drho_bar, acc_bar, rows=None, par_raw=None,
+            delta_form=None, rcond=None):
+    """(x_bar, v_bar, rho_bar, params_bar) = J^T (drho_bar, acc_bar) of rhs(), adjacency held fixed.  delta_form 1 adds the
+    adjoint of orc_delta_renorm_term: its direct dependences (orc_delta_renorm_term_vjp) and, through the cotangent of
+    the gradient field, the adjoint of the renormalised gradient with vol = m/rho and A = rho (full rows only)."""
     dim, per, lo, hi = _dom(domain)
     par = _par(params) if par_raw is None else par_raw
     x, v, rho, m, h = _d(x), _d(v), _d(rho), _d(m), _d(h)
@@ -246,10 +273,92 @@ def rhs_vjp(domain, params, x, v, rho, m, h, kind, row_ptr, col_idx, drho_bar, a
     lib().orc_rhs_vjp(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(par), _p(x), _p(v), _p(rho), _p(m), _p(h),
                       _p(kind), _p(rp), _p(ci), _p(lam), _p(mu), _p(rows_a), C.c_int64(0 if rows is None else len(rows_a)),
                       _p(xb), _p(vb), _p(rb), _p(pb))
+    if _delta_form(params, delta_form) == 1:
+        if rows is not None:
+            raise ValueError("delta_form 1: the adjoint is computed for all rows")
+        rc = _rcond(params, rcond)
+        vol = m / rho
+        _, g, _ = renorm_gradient(domain, x, h, vol, rho, rp, ci, rcond=rc)
+        g = np.ascontiguousarray(g)
+        gbar = np.zeros((n, dim))
+        lib().orc_delta_renorm_term_vjp(C.c_int64(n), C.c_int(dim), _p(per), _p(lo), _p(hi), _p(par), _p(x), _p(rho),
+                                        _p(m), _p(h), _p(rp), _p(ci), _p(g), _p(lam), _p(xb), _p(rb), _p(gbar), _p(pb))
+        xb2, volb, Ab = renorm_gradient_vjp(domain, x, h, vol, rho, rp, ci, gbar, rcond=rc)
+        xb += xb2
+        rb += Ab - volb * m / (rho * rho)                 # A = rho;  vol = m / rho
     return xb, vb, rb, pb
 
 
+def _wrap64(domain, x):
+    """binary64 wrap of stage positions into the periodic box (same formula as wrap64 in sph_oracle.c)"""
+    dim, per, lo, hi = _dom(domain)
+    xw = _d(x).copy()
+    for k in range(dim):
+        if per[k]:
+            Lk = float(np.float32(hi[k]) - np.float32(lo[k]))       # the one binary32 L of readings R3/R4
+            xw[:, k] = xw[:, k] - Lk * np.floor((xw[:, k] - lo[k]) / Lk)
+            xw[xw[:, k] >= hi[k], k] -= Lk
+            xw[xw[:, k] < lo[k], k] += Lk
+    return xw
+
+
+def _f_eval(domain, params, X, V, R, m, h, kind, method, par_raw):
+    """k = f(Y) with exact neighbours of the stage positions; returns (kx, kv, kr, lists)"""
+    lists = neighbors(domain, _wrap64(domain, X), h, method=method, prewrapped=True)
+    kr, kv = rhs(domain, params, X, V, R, m, h, kind, *lists, par_raw=par_raw)
+    kx = np.where(np.asarray(kind)[:, None] != 0, 0.0, V)
+    return kx, kv, kr, lists
+
+
+def _rk4_step_py(domain, params, dt, x, v, rho, m, h, kind, method, par_raw):
+    """classic RK4 written out in Python on top of rhs() -- used for delta_form 1, whose right-hand side is composed in
+    this module"""
+    c = (0.0, 0.5, 0.5, 1.0)
+    b = (1.0 / 6.0, 1.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0)
+    x, v, rho = _d(x), _d(v), _d(rho)
+    ax, av, ar = np.zeros_like(x), np.zeros_like(v), np.zeros_like(rho)
+    kx = kv = kr = None
+    for s in range(4):
+        X = x if s == 0 else x + c[s] * dt * kx
+        V = v if s == 0 else v + c[s] * dt * kv
+        R = rho if s == 0 else rho + c[s] * dt * kr
+        kx, kv, kr, _ = _f_eval(domain, params, X, V, R, m, h, kind, method, par_raw)
+        ax, av, ar = ax + b[s] * kx, av + b[s] * kv, ar + b[s] * kr
+    return x + dt * ax, v + dt * av, rho + dt * ar
+
+
+def _rk4_step_vjp_py(domain, params, dt, x0, v0, r0, m, h, kind, xb, vb, rb, pb, method, par_raw):
+    """discrete adjoint of _rk4_step_py with recomputed stages"""
+    c = (0.0, 0.5, 0.5, 1.0)
+    b = (1.0 / 6.0, 1.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0)
+    x0, v0, r0 = _d(x0), _d(v0), _d(r0)
+    Y, lists = [], []
+    kx = kv = kr = None
+    for s in range(4):
+        X = x0 if s == 0 else x0 + c[s] * dt * kx
+        V = v0 if s == 0 else v0 + c[s] * dt * kv
+        R = r0 if s == 0 else r0 + c[s] * dt * kr
+        Y.append((X, V, R))
+        kx, kv, kr, l = _f_eval(domain, params, X, V, R, m, h, kind, method, par_raw)
+        lists.append(l)
+    fluid = (np.asarray(kind) == 0)[:, None]
+    Ybx, Ybv, Ybr = np.zeros_like(x0), np.zeros_like(v0), np.zeros_like(r0)
+    sx, sv, sr = np.zeros_like(x0), np.zeros_like(v0), np.zeros_like(r0)
+    for s in (3, 2, 1, 0):
+        a_next = 0.0 if s == 3 else c[s + 1]
+        kbx = b[s] * dt * xb + a_next * dt * Ybx
+        kbv = b[s] * dt * vb + a_next * dt * Ybv
+        kbr = b[s] * dt * rb + a_next * dt * Ybr
+        Ybx, Ybv, Ybr, pk = rhs_vjp(domain, params, *Y[s], m, h, kind, *lists[s], kbr, kbv, par_raw=par_raw)
+        Ybv = Ybv + np.where(fluid, kbx, 0.0)             # dx/dt = v for fluid kinds
+        sx, sv, sr = sx + Ybx, sv + Ybv, sr + Ybr
+        pb = pb + pk
+    return xb + sx, vb + sv, rb + sr, pb
+
+
 def rk4_step(domain, params, dt, x, v, rho, m, h, kind, method=0, par_raw=None):
+    if _delta_form(params, None) == 1:
+        return _rk4_step_py(domain, params, dt, x, v, rho, m, h, kind, method, par_raw)
     dim, per, lo, hi = _dom(domain)
     par = _par(params) if par_raw is None else par_raw
     x, v, rho = _d(x).copy(), _d(v).copy(), _d(rho).copy()
@@ -263,6 +372,10 @@ def rk4_step(domain, params, dt, x, v, rho, m, h, kind, method=0, par_raw=None):
 
 def rk4_step_vjp(domain, params, dt, x0, v0, rho0, m, h, kind, x_bar, v_bar, rho_bar, params_bar=None, method=0,
                  par_raw=None):
+    if _delta_form(params, None) == 1:
+        pb0 = np.zeros(10) if params_bar is None else _d(params_bar).copy()
+        return _rk4_step_vjp_py(domain, params, dt, x0, v0, rho0, m, h, kind, _d(x_bar).copy(), _d(v_bar).copy(),
+                                _d(rho_bar).copy(), pb0, method, par_raw)
     dim, per, lo, hi = _dom(domain)
     par = _par(params) if par_raw is None else par_raw
     x0, v0, rho0, m, h = _d(x0), _d(v0), _d(rho0), _d(m), _d(h)

@@ -962,6 +962,103 @@ void orc_rk4_step_vjp(int64_t n, int dim, const int *periodic, const double *lo,
     free(Ybx); free(Ybv); free(Ybr); free(sx); free(sv); free(sr);
 }
 
+/* ------------------------------------------------------------------------------------------
+ * NEXT-2  delta-SPH diffusion with the renormalised density gradient (PAPER.md:103 cites [43], PAPER.md:85 [51];
+ * the equation is not printed -- DESIGN.md reading R17).  The term of Antuono et al. [43]:
+ *     D_i = delta l c0 sum_j psi_ij . grad_i W_ij V_j ,
+ *     psi_ij = 2 (rho_j - rho_i) (x_j - x_i)/|x_ij|^2  -  [ <grad rho>^L_i + <grad rho>^L_j ] ,
+ * <grad rho>^L the renormalised gradient of PAPER.md:524-528 Eq.44/45.  The first part is the Molteni-Colagrossi
+ * term orc_rhs already adds (delta_form 0, with its (eps H)^2 regularisation); this function adds the second,
+ *     X_ij = - delta l_ij c0 V_j (g_i + g_j) . d G ,   d = x_i - x_j ,  grad_i W_ij = G d ,
+ * with g = <grad rho>^L passed in (the pseudo-inverse L_i is formed by the caller, oracle/__init__.py).
+ * drho_dt is ADDED to; scale_drho (may be NULL) gets sum_j |X_ij| added.
+ * ------------------------------------------------------------------------------------------ */
+void orc_delta_renorm_term(int64_t n, int dim, const int *periodic, const double *lo, const double *hi,
+                           const double *par, const double *x, const double *rho, const double *m, const double *h,
+                           const int64_t *row_ptr, const int32_t *col_idx, const double *grho,
+                           const int64_t *rows, int64_t nrows, double *drho_dt, double *scale_drho)
+{
+    Par P = par_load(par);
+    double L[3];
+    box_len(dim, lo, hi, L);
+    double *xw = (double *)malloc((size_t)n * dim * sizeof(double));
+    wrap64(n, dim, periodic, lo, hi, x, xw);
+    int64_t cnt = rows ? nrows : n;
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t t = 0; t < cnt; ++t) {
+        int64_t i = rows ? rows[t] : t;
+        double dr = 0.0, sd = 0.0;
+        for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
+            int64_t j = col_idx[p];
+            double d[3] = {0, 0, 0};
+            for (int k = 0; k < dim; ++k) d[k] = xw[i * dim + k] - xw[j * dim + k];
+            min_image(d, dim, periodic, L);
+            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            double H = h[i] > h[j] ? h[i] : h[j];
+            if (r >= H) continue;
+            double G = orc_gfac(r, H, dim);
+            double ell = H / kappa(dim);
+            double S = 0.0;
+            for (int k = 0; k < dim; ++k) S += (grho[i * dim + k] + grho[j * dim + k]) * d[k];
+            double X = -P.delta * ell * P.c0 * (m[j] / rho[j]) * S * G;
+            dr += X;
+            sd += fabs(X);
+        }
+        drho_dt[i] += dr;
+        if (scale_drho) scale_drho[i] += sd;
+    }
+    free(xw);
+}
+
+/* Adjoint of the term above for the cotangent lam = dL/d(drho_dt), scatter form over ordered pairs (serial: the
+ * definition).  Direct dependences only: x (through d and G; dG = K d.dd), rho_j (through V_j = m_j/rho_j), delta, c0,
+ * and the gradient field g, whose cotangent g_bar [n][dim] is returned for the caller to push through the adjoint of
+ * the renormalised gradient (orc_renorm_moments_vjp + the pseudo-inverse, oracle/__init__.py).
+ * x_bar, rho_bar, params_bar[10] are ADDED to; g_bar is overwritten. */
+void orc_delta_renorm_term_vjp(int64_t n, int dim, const int *periodic, const double *lo, const double *hi,
+                               const double *par, const double *x, const double *rho, const double *m, const double *h,
+                               const int64_t *row_ptr, const int32_t *col_idx, const double *grho, const double *lam,
+                               double *x_bar, double *rho_bar, double *g_bar, double *params_bar)
+{
+    Par P = par_load(par);
+    double L[3];
+    box_len(dim, lo, hi, L);
+    double *xw = (double *)malloc((size_t)n * dim * sizeof(double));
+    wrap64(n, dim, periodic, lo, hi, x, xw);
+    memset(g_bar, 0, (size_t)n * dim * sizeof(double));
+    for (int64_t i = 0; i < n; ++i) {
+        for (int64_t p = row_ptr[i]; p < row_ptr[i + 1]; ++p) {
+            int64_t j = col_idx[p];
+            double d[3] = {0, 0, 0};
+            for (int k = 0; k < dim; ++k) d[k] = xw[i * dim + k] - xw[j * dim + k];
+            min_image(d, dim, periodic, L);
+            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            double H = h[i] > h[j] ? h[i] : h[j];
+            if (r >= H) continue;
+            double G = orc_gfac(r, H, dim), K = orc_kfac(r, H, dim);
+            double ell = H / kappa(dim);
+            double Vj = m[j] / rho[j];
+            double c = -P.delta * ell * P.c0 * Vj;              /* X = c S G */
+            double S = 0.0;
+            for (int k = 0; k < dim; ++k) S += (grho[i * dim + k] + grho[j * dim + k]) * d[k];
+            double X = c * S * G;
+            for (int k = 0; k < dim; ++k) {
+                /* dX/dd_k = c [ (g_i + g_j)_k G + S K d_k ] */
+                double F = lam[i] * c * ((grho[i * dim + k] + grho[j * dim + k]) * G + S * K * d[k]);
+                x_bar[i * dim + k] += F;
+                x_bar[j * dim + k] -= F;
+                /* dX/dg_i = dX/dg_j = c G d */
+                g_bar[i * dim + k] += lam[i] * c * G * d[k];
+                g_bar[j * dim + k] += lam[i] * c * G * d[k];
+            }
+            rho_bar[j] += -lam[i] * X / rho[j];                 /* V_j = m_j / rho_j */
+            params_bar[3] += lam[i] * X / P.delta;              /* delta */
+            params_bar[0] += lam[i] * X / P.c0;                 /* c0 */
+        }
+    }
+    free(xw);
+}
+
 int orc_num_threads(void)
 {
     int nt = 1;

@@ -42,6 +42,8 @@ class Params:
     eps: float = 0.01
     g: tuple = (0.0, 0.0, 0.0)
     pressure_form: int = 0
+    delta_form: int = 0          # 0 = Molteni-Colagrossi delta-term; 1 = with the renormalised density gradient of [43]
+    renorm_rcond: float = 1e-4   # relative eigenvalue cutoff of the pseudo-inverse L_i, delta_form 1 only
 
     def as_list(self):
         return [self.c0, self.rho0, self.gamma, self.delta, self.alpha, self.nu, self.eps,

@@ -547,6 +547,77 @@ def test_rhs_boundary_kinds():
     assert acc2[near, 0] > acc1[near, 0]
 
 
+# ------------------------------------------------------------------------------------------ delta-term of [43]
+def _open_box_case(dim, n_axis, seed, amp):
+    """disordered particles in an open (bounded) box: the outer layers have truncated neighbourhoods (free surface)"""
+    wl = W.perturbed(W.make(0 if dim == 2 else 3, n_axis=n_axis), amp_x=amp, amp_rho=0.0, seed_offset=seed)
+    dom = W.Domain(dim=dim, periodic=(0, 0, 0), lo=(0.0,) * 3, hi=(1.0,) * dim + (0.0,) * (3 - dim),
+                   cell_size=wl.domain.cell_size)
+    return wl, dom
+
+
+@pytest.mark.parametrize("dim,n_axis", [(2, 20), (3, 10)])
+def test_delta_form_1_vanishes_for_a_linear_density_field_up_to_the_free_surface(dim, n_axis):
+    """The reason [43] exists: with the renormalised gradient <grad rho>^L, which is exact for linear
+    fields on ANY particle configuration, psi_ij = 2(rho_j-rho_i) x_ji/r^2 - (g_i+g_j) vanishes
+    identically for rho = a.x + b, so the diffusion is zero at every particle, free surface included; the
+    Molteni-Colagrossi term (delta_form 0) is zero in the interior of a lattice only."""
+    wl, dom = _open_box_case(dim, n_axis, 3, 0.3)
+    a = np.array([0.7, -0.4, 0.5][:dim])
+    rho = 1.0 + wl.x.astype(np.float64) @ a * 0.05
+    lists = oracle.neighbors(dom, wl.x, wl.h, method=1)
+    par1 = W.Params(**{**wl.params.__dict__, "delta_form": 1, "eps": 1e-9})     # eps -> 0: r^2/R -> 1 in the first part
+    par0 = W.Params(**{**par1.__dict__, "delta_form": 0})
+    d1, _, s1, _ = oracle.rhs(dom, par1, wl.x, 0 * wl.v, rho, wl.m, wl.h, wl.kind, *lists, with_scales=True)
+    d0, _ = oracle.rhs(dom, par0, wl.x, 0 * wl.v, rho, wl.m, wl.h, wl.kind, *lists)
+    H = float(wl.h[0])
+    surface = ~np.all((wl.x > H) & (wl.x < 1 - H), axis=1)
+    assert surface.sum() > 0.3 * wl.n
+    assert np.max(np.abs(d1)) < 1e-9 * np.max(s1)                      # zero everywhere (self pair: r^2/R = 0 exactly)
+    assert np.max(np.abs(d0[surface])) > 1e-2 * np.max(s1)            # ... where form 0 is far from zero
+
+
+@pytest.mark.parametrize("dim,n_axis,klap,kc,exact", [(2, 32, "brookshaw_lap_r2_2d_H4dx", "compression_factor_2d_H4dx", 4.0),
+                                                      (3, 16, "brookshaw_lap_r2_3d_H3dx", "compression_factor_3d_H3dx", 6.0)])
+def test_delta_form_1_on_a_quadratic_field_combines_two_survey_pins(dim, n_axis, klap, kc, exact):
+    """rho = rho0 (1 + beta |x|^2) on an interior lattice, v = 0.  There <grad rho>^L = 2 beta x exactly (odd moments
+    vanish), hence (g_i+g_j).d = 2 (rho_i - rho_j) and the second part of the term is -2 delta l c0 sum V_j (rho_i-rho_j) G
+    = -2 d c beta delta l c0 with c the lattice moment of the uniform-compression pin; the first part is the Brookshaw
+    Laplacian pin.  So drho/dt / (delta l c0 beta) = Lap_pin - 2 d c_pin: both values come from the survey, none from the
+    oracle (SURVEY.md:424-425), and a wrong sign, factor or transposed L in the new term fails this."""
+    wl = W.make(0 if dim == 2 else 3, n_axis=n_axis)
+    dom = W.Domain(dim=dim, periodic=(0, 0, 0), lo=(0.0,) * 3, hi=(1.0,) * dim + (0.0,) * (3 - dim),
+                   cell_size=wl.domain.cell_size)
+    beta = 1e-7
+    xc = wl.x.astype(np.float64) - 0.5
+    rho = 1.0 + beta * np.sum(xc * xc, axis=1)
+    lists = oracle.neighbors(dom, wl.x, wl.h, method=1)
+    par = W.Params(**{**wl.params.__dict__, "delta_form": 1})
+    drho, _ = oracle.rhs(dom, par, wl.x, 0 * wl.v, rho, wl.m, wl.h, wl.kind, *lists)
+    H = float(wl.h[0])
+    kap = PAPER["kernel_scale_2d"] if dim == 2 else PAPER["kernel_scale_3d"]
+    coef = float(np.float32(wl.params.delta)) * (H / kap) * wl.params.c0
+    interior = np.all((wl.x > 2 * H) & (wl.x < 1 - 2 * H), axis=1)      # the gradient of the neighbours must be interior too
+    val = drho[interior] / (coef * beta)
+    want = PINS[klap] - 2.0 * dim * PINS[kc]
+    assert np.max(np.abs(val - want)) < 5e-5
+    assert abs(want) < 0.05 and abs(PINS[klap] - exact) < 0.05          # the two parts cancel to the lattice error
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, dict(n_axis=24)), (4, dict(n_axis=10))])
+def test_delta_form_1_conserves_mass(cfg, kw):
+    """V_i X_ij is antisymmetric in (i, j): sum_i V_i D_i = 0 to round-off for any density field (v = 0)"""
+    wl = W.perturbed(W.make(cfg, **kw), amp_x=0.3, amp_rho=0.05)
+    par = W.Params(**{**wl.params.__dict__, "delta_form": 1})
+    lists = _lists(wl)
+    drho, _, sd, _ = oracle.rhs(wl.domain, par, wl.x, 0 * wl.v, wl.rho, wl.m, wl.h, wl.kind, *lists, with_scales=True)
+    V = wl.m.astype(np.float64) / wl.rho.astype(np.float64)
+    assert abs(np.sum(V * drho)) < 1e-12 * np.sum(V * sd)
+    d0, _ = oracle.rhs(wl.domain, W.Params(**{**par.__dict__, "delta_form": 0}), wl.x, 0 * wl.v, wl.rho, wl.m, wl.h,
+                       wl.kind, *lists)
+    assert np.max(np.abs(drho - d0)) > 1e-2 * np.max(np.abs(d0))       # the new term is not a no-op
+
+
 # ------------------------------------------------------------------------------------------ VJP
 def _objective(dom, par_raw, form, x, v, rho, wl, lists, lam, mu):
     drho, acc = oracle.rhs(dom, None, x, v, rho, wl.m, wl.h, wl.kind, *lists, par_raw=oracle._par_raw(par_raw, form))
@@ -605,6 +676,89 @@ def test_vjp_against_central_differences(cfg, kw, form):
     assert np.max(np.abs(xb2[rows] - xb[rows])) < 1e-10 * np.max(np.abs(xb))
     assert np.max(np.abs(vb2[rows] - vb[rows])) < 1e-10 * np.max(np.abs(vb))
     assert np.max(np.abs(rb2[rows] - rb[rows])) < 1e-10 * np.max(np.abs(rb))
+
+
+@pytest.mark.parametrize("cfg,kw,form", [(1, dict(n_axis=16), 1), (2, dict(dx=0.1), 0), (4, dict(n_axis=8), 0)])
+def test_vjp_delta_form_1_against_central_differences(cfg, kw, form):
+    """delta_form 1: the adjoint includes the path through the renormalised gradient -- L_i depends on the positions
+    and on the volumes m/rho, the gradient on rho itself (PAPER.md:530 'fully supports backpropagation through this
+    operation').  Central differences of the forward in x, v, rho and in delta, c0 (the scalars the new term carries);
+    2D periodic, 2D with walls and a free surface (rank changes excluded by a loose rcond), 3D with varying h."""
+    wl = W.perturbed(W.make(cfg, **kw), amp_x=0.25, amp_rho=0.03)
+    rng = np.random.default_rng(15 + cfg)
+    p0 = np.array(wl.params.as_list(), dtype=np.float32).astype(np.float64)
+    lists = oracle.neighbors(wl.domain, wl.x, wl.h, method=0)
+    lam = rng.normal(size=wl.n)
+    mu = rng.normal(size=(wl.n, wl.dim))
+    x, v, rho = wl.x.astype(np.float64), wl.v.astype(np.float64), wl.rho.astype(np.float64)
+    rc = 1e-6
+
+    def f(X, V, R, P):
+        drho, acc = oracle.rhs(wl.domain, None, X, V, R, wl.m, wl.h, wl.kind, *lists, par_raw=oracle._par_raw(P, form),
+                               delta_form=1, rcond=rc)
+        return float(np.sum(lam * drho) + np.sum(mu * acc))
+
+    xb, vb, rb, pb = oracle.rhs_vjp(wl.domain, None, x, v, rho, wl.m, wl.h, wl.kind, *lists, lam, mu,
+                                    par_raw=oracle._par_raw(p0, form), delta_form=1, rcond=rc)
+    xb0, vb0, rb0, pb0 = oracle.rhs_vjp(wl.domain, None, x, v, rho, wl.m, wl.h, wl.kind, *lists, lam, mu,
+                                        par_raw=oracle._par_raw(p0, form), delta_form=0)
+    assert np.max(np.abs(xb - xb0)) > 1e-3 * np.max(np.abs(xb0)) and np.max(np.abs(rb - rb0)) > 1e-3 * np.max(np.abs(rb0))
+    assert np.max(np.abs(vb - vb0)) <= 1e-12 * np.max(np.abs(vb0))          # the term does not see velocities
+    scale = abs(f(x, v, rho, p0)) + 1.0
+    for name, bar in (("x", xb), ("rho", rb)):
+        for trial in range(3):
+            z = rng.normal(size=bar.shape)
+            e = {"x": 1e-7 * wl.dx / 0.03, "rho": 1e-6 * float(np.mean(rho))}[name]
+            args_p, args_m = ((x + e * z, v, rho), (x - e * z, v, rho)) if name == "x" else ((x, v, rho + e * z), (x, v, rho - e * z))
+            fd = (f(*args_p, p0) - f(*args_m, p0)) / (2 * e)
+            an = float(np.sum(bar * z))
+            assert abs(fd - an) < 5e-6 * max(abs(an), abs(fd)) + 1e-9 * scale / e * 1e-6, (name, fd, an)
+    for k in (0, 3):                                                      # c0, delta
+        e = 1e-6 * max(abs(p0[k]), 1e-2)
+        pp, pm = p0.copy(), p0.copy()
+        pp[k] += e
+        pm[k] -= e
+        fd = (f(x, v, rho, pp) - f(x, v, rho, pm)) / (2 * e)
+        assert abs(fd - pb[k]) < 5e-6 * max(abs(fd), abs(pb[k])) + 1e-7 * scale, (k, fd, pb[k])
+    assert np.max(np.abs(xb.sum(axis=0))) < 1e-9 * np.sum(np.abs(xb))      # differences only
+
+
+def test_rk4_delta_form_1_step_and_adjoint():
+    """RK4 with delta_form 1 (composed in oracle/__init__.py): 4th order under dt halving, and the adjoint of
+    KE(t+dt) against central differences in v0 and rho0"""
+    wl = W.perturbed(W.make(0, n_axis=12), amp_x=0.15, amp_rho=0.02)
+    par = W.Params(**{**wl.params.__dict__, "delta_form": 1})
+    x0, v0, r0 = wl.x.astype(np.float64), wl.v.astype(np.float64), wl.rho.astype(np.float64)
+    m = wl.m.astype(np.float64)
+
+    def run(nsteps, T):
+        x, v, r = x0, v0, r0
+        for _ in range(nsteps):
+            x, v, r = oracle.rk4_step(wl.domain, par, T / nsteps, x, v, r, wl.m, wl.h, wl.kind, method=0)
+        return np.concatenate([x.ravel(), v.ravel(), r.ravel()])
+
+    T = 2 * wl.dt
+    ref = run(16, T)
+    e2, e4 = (np.max(np.abs(run(k, T) - ref)) for k in (2, 4))
+    assert e2 / e4 > 10.0
+    # differs from delta_form 0 (density noise is being diffused differently)
+    _, _, r_f0 = oracle.rk4_step(wl.domain, wl.params, wl.dt, x0, v0, r0, wl.m, wl.h, wl.kind, method=0)
+    _, v1, r_f1 = oracle.rk4_step(wl.domain, par, wl.dt, x0, v0, r0, wl.m, wl.h, wl.kind, method=0)
+    assert np.max(np.abs(r_f1 - r_f0)) > 1e-6
+
+    def ke_after(v, r):
+        _, vv, _ = oracle.rk4_step(wl.domain, par, wl.dt, x0, v, r, wl.m, wl.h, wl.kind, method=0)
+        return 0.5 * float(np.sum(m[:, None] * vv ** 2))
+
+    xb, vb, rb, pb = oracle.rk4_step_vjp(wl.domain, par, wl.dt, x0, v0, r0, wl.m, wl.h, wl.kind, np.zeros_like(x0),
+                                         m[:, None] * v1, np.zeros(wl.n), method=0)
+    rng = np.random.default_rng(2)
+    zv, zr = rng.normal(size=v0.shape), rng.normal(size=wl.n)
+    e = 1e-6
+    fd_v = (ke_after(v0 + e * zv, r0) - ke_after(v0 - e * zv, r0)) / (2 * e)
+    fd_r = (ke_after(v0, r0 + e * zr) - ke_after(v0, r0 - e * zr)) / (2 * e)
+    assert abs(fd_v - np.sum(vb * zv)) < 1e-5 * abs(fd_v) + 1e-9
+    assert abs(fd_r - np.sum(rb * zr)) < 1e-4 * abs(fd_r) + 1e-9
 
 
 def test_vjp_dot_product_identity_and_viscous_self_adjointness():
