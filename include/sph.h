@@ -65,6 +65,15 @@ typedef struct {
     float g[3];   /* body force (gravity) */
     int pressure_form; /* 0 = symmetric Eq.40: -m_j (p_i/rho_i^2 + p_j/rho_j^2);  1 = -m_j (p_i + p_j)/(rho_i rho_j), the form
                           the paper's own WCSPH scheme uses;  others: SPH_E_INVALID */
+    int delta_form;    /* density diffusion (the equation is not printed, R6 / R17):
+                          0 = Molteni-Colagrossi: delta l c0 sum_j 2 (rho_i - rho_j) r^2/(r^2 + (eps H)^2) G V_j;
+                          1 = the delta-SPH term of Antuono et al. [43]: the same minus
+                              delta l c0 sum_j V_j (g_i + g_j).(x_i - x_j) G  with g = <grad rho>^L, the renormalised density
+                              gradient of PAPER.md:524-528 Eq.44/45 (zero diffusion of linear density fields up to the
+                              free surface).  sph_rhs then runs the renormalisation passes first; sph_rhs_vjp
+                              differentiates through L_i.  others: SPH_E_INVALID */
+    float renorm_rcond; /* delta_form 1: eigenvalues of the renormalisation matrix below renorm_rcond * largest are dropped
+                          in the pseudo-inverse; 0 <= renorm_rcond < 1, e.g. 1e-4 */
 } sph_params;
 
 enum {

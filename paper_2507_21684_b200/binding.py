@@ -39,7 +39,7 @@ class SphDomain(C.Structure):
 class SphParams(C.Structure):
     _fields_ = [("c0", C.c_float), ("rho0", C.c_float), ("gamma", C.c_float), ("delta", C.c_float),
                 ("alpha", C.c_float), ("nu", C.c_float), ("eps", C.c_float), ("g", C.c_float * 3),
-                ("pressure_form", C.c_int)]
+                ("pressure_form", C.c_int), ("delta_form", C.c_int), ("renorm_rcond", C.c_float)]
 
 
 class SphError(RuntimeError):
@@ -114,6 +114,8 @@ def make_params(params) -> SphParams:
     for k in range(3):
         p.g[k] = float(params.g[k])
     p.pressure_form = int(params.pressure_form)
+    p.delta_form = int(getattr(params, "delta_form", 0))
+    p.renorm_rcond = float(getattr(params, "renorm_rcond", 1e-4))
     return p
 
 

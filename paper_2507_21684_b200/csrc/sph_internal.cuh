@@ -90,6 +90,8 @@ struct KPar {
     float visc_nu;  // 2(d+2) nu
     float Bp;       // rho0 c0^2 / gamma
     int form;       // pressure form: 0 symmetric Eq.40, 1 (p_i+p_j)/(rho_i rho_j)
+    int delta_form; // 0 Molteni-Colagrossi delta-term, 1 with the renormalised density gradient of [43]
+    float rcond;    // eigenvalue cutoff of the pseudo-inverse L_i (delta_form 1)
     int uniform_h;  // all h equal (then the H-dependent constants below are valid)
     float H, invH, cW, cG, cK, ell, e2, eta, kd;
 };
@@ -161,6 +163,8 @@ struct sph_ctx {
     DevBuf maskbuf, tile_words, tile_mask_base;   // hit masks of the count pass, per-tile mask offsets
     // one-kernel build: cell statistics, look-back states, {ticket, overflow}, tiles in Morton order (cached per grid)
     DevBuf fstats, tstate, fctl;
+    // delta_form 1: current positions {x,y,z,h}, {V,rho}, moments, {g,V}, adjoint records and sorted partial results
+    DevBuf d_pos, d_va, d_mom, d_g4, d_lr, d_dx4, d_gb4, d_rb, d_rc, d_rd, d_re, d_x2, d_vb, d_ab, d_part;
     struct TileOrder {                            // cache slot: the order depends on the grid and on B only
         DevBuf buf;
         bool valid = false;
@@ -343,9 +347,28 @@ int sph_rk_prepare_lists(sph_ctx *ctx, const sph_domain *dom, float skin, const 
                          cudaStream_t st);
 int sph_lists_valid_impl(sph_ctx *ctx, const float *x, const float *h, float skin_needed, int32_t *valid_out,
                          float *max_disp_out, cudaStream_t st);
-int sph_launch_renorm_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *rb, const float4 *rc, const float2 *rd,
-                               const float *re, float *x_bar, float *vol_bar, float *A_bar, cudaStream_t st);
-int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float2 *va_s, float4 *mom, cudaStream_t st);
+int sph_launch_renorm_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float4 *rb, const float4 *rc,
+                               const float2 *rd, const float *re, const uint32_t *perm, float *x_bar, float *vol_bar,
+                               float *A_bar, cudaStream_t st);
+int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float2 *va_s, float4 *mom, cudaStream_t st);
+int sph_launch_delta_term_tile(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float4 *g4, const float2 *lr,
+                               bool adjoint, float *drho_io, float4 *out4_io, float4 *dx4, float4 *gb4, float *partial,
+                               cudaStream_t st);
+// delta_form 1 (sph_delta.cu): the second part of the delta-term of [43] on top of a finished RHS / VJP launch
+int sph_delta_forward(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2, float *drho,
+                      float4 *out4, cudaStream_t st);
+int sph_delta_adjoint(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2, const float4 *cot,
+                      float *xb, float *rb, float4 *xb4, float *params_bar, cudaStream_t st);
+// renormalisation passes on given sorted positions (sph_pairs.cu)
+int sph_renorm_moments_any(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float2 *va_s, float4 *mom, cudaStream_t st);
+int sph_renorm_vjp_pairs_any(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float4 *rb, const float4 *rc,
+                             const float2 *rd, const float *re, const uint32_t *perm, float *x_bar, float *vol_bar,
+                             float *A_bar, cudaStream_t st);
+int sph_delta_term_generic(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float4 *g4, const float2 *lr, bool adjoint,
+                           float *drho_io, float4 *out4_io, float4 *dx4, float4 *gb4, float *partial, int *npartial,
+                           cudaStream_t st);
+int sph_renorm_solve_sorted(sph_ctx *ctx, const KPar &kp, const float4 *mom, const float2 *va_s, const float4 *gbar4,
+                            float4 *g4_out, float4 *rb, float4 *rc, float2 *rd, float *re, cudaStream_t st);
 int sph_launch_grad_sum_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *ga_s, float *x_bar, float *a_bar,
                                  cudaStream_t st);
 int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,

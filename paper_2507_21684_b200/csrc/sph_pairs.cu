@@ -604,7 +604,7 @@ k_renorm_vjp(int64_t n, KPar kp, float margin, const float4 *__restrict__ pos_s,
         vb = group_sum<GS>(vb);
         ab = group_sum<GS>(ab);
         if (gl == 0) {
-            const int64_t i = perm[row];
+            const int64_t i = perm ? (int64_t)perm[row] : row;       // null perm: sorted order
 #pragma unroll
             for (int k = 0; k < DIM; ++k) xb_out[i * DIM + k] = xb[k];
             if (vb_out) vb_out[i] = vb;
@@ -857,6 +857,139 @@ k_vjp(int64_t n, KPar kp, float margin, const float4 *__restrict__ s0, const flo
     }
 }
 
+// ------------------------------------------------------------------------------------------ delta-term of [43], generic lists
+// Same sums as k_delta_term_tile (sph_pairs_tile.cu) on the 32-bit sorted-id lists with global gathers.
+template <int DIM, int GS, bool VARH, bool ADJ>
+__global__ void __launch_bounds__(kBlock)
+k_delta_term(int64_t n, KPar kp, float margin, const float4 *__restrict__ pos4, const float4 *__restrict__ g4,
+             const float2 *__restrict__ lr, const long long *__restrict__ row_ptr, const int32_t *__restrict__ col,
+             const uint32_t *__restrict__ perm, float *__restrict__ drho_io, float4 *__restrict__ out4_io,
+             float4 *__restrict__ dx4, float4 *__restrict__ gb4, float *__restrict__ partial)
+{
+    constexpr int kGroups = kBlock / GS;
+    const int g = threadIdx.x / GS, gl = threadIdx.x % GS;
+    const int64_t row0 = (int64_t)blockIdx.x * kGroups * kRowsPerGroup;
+    const HC hu = hc_uniform<DIM>(kp);
+    float SX = 0.f;
+    for (int rr = 0; rr < kRowsPerGroup; ++rr) {
+        const int64_t row = row0 + (int64_t)rr * kGroups + g;
+        if (row >= n) break;
+        const float4 pi = __ldg(pos4 + row), gi = __ldg(g4 + row);
+        float2 li = make_float2(0.f, 1.f);
+        if (ADJ) li = __ldg(lr + row);
+        const float xi[3] = {pi.x, pi.y, pi.z};
+        const bool seam = row_near_seam(xi, kp, margin);
+        const long long b = row_ptr[row], e = row_ptr[row + 1];
+        float acc = 0.f, xb[3] = {0.f, 0.f, 0.f}, gb[3] = {0.f, 0.f, 0.f}, rb = 0.f;
+        for (long long p = b + gl; p < e; p += GS) {
+            const int32_t j = __ldg(col + p);
+            const float4 pj = __ldg(pos4 + j), gj = __ldg(g4 + j);
+            const float xj[3] = {pj.x, pj.y, pj.z};
+            float d[3], r2;
+            if (seam) rel_pos<DIM, true>(xi, xj, kp, d, r2); else rel_pos<DIM, false>(xi, xj, kp, d, r2);
+            HC hc = hu;
+            if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+            const float rr2 = fast_sqrt(r2);
+            const float t = fmaxf(fmaf(-hc.invH, rr2, 1.0f), 0.f);
+            const float t2 = t * t, t4 = t2 * t2;
+            const float G = hc.cG * fmaf(5.0f * hc.invH, rr2, 1.0f) * (t4 * t);
+            const float gs[3] = {gi.x + gj.x, gi.y + gj.y, DIM == 3 ? gi.z + gj.z : 0.f};
+            const float S = fmaf(gs[2], d[2], fmaf(gs[1], d[1], gs[0] * d[0]));
+            const float cc = VARH ? -0.5f * hc.kd : 1.0f;
+            if (!ADJ) {
+                acc = fmaf(cc * gj.w, S * G, acc);
+            } else {
+                const float2 lj = __ldg(lr + j);
+                const float K = hc.cK * t4;
+                const float w = cc * fmaf(li.x, gj.w, -(lj.x * gi.w));
+                const float SK = S * K;
+#pragma unroll
+                for (int kk = 0; kk < DIM; ++kk) {
+                    xb[kk] = fmaf(w, fmaf(gs[kk], G, SK * d[kk]), xb[kk]);
+                    gb[kk] = fmaf(w * G, d[kk], gb[kk]);
+                }
+                rb = fmaf(cc * lj.x, S * G, rb);
+                SX = fmaf(cc * li.x * gj.w, S * G, SX);
+            }
+        }
+        const float cu = VARH ? 1.0f : -0.5f * hu.kd;
+        if (!ADJ) {
+            acc = group_sum<GS>(acc) * cu;
+            if (gl == 0) {
+                if (out4_io) out4_io[row].w += acc;
+                else drho_io[perm[row]] += acc;
+            }
+        } else {
+#pragma unroll
+            for (int kk = 0; kk < DIM; ++kk) {
+                xb[kk] = group_sum<GS>(xb[kk]) * cu;
+                gb[kk] = group_sum<GS>(gb[kk]) * cu;
+            }
+            rb = group_sum<GS>(rb) * cu * gi.w / li.y;
+            if (gl == 0) {
+                dx4[row] = make_float4(xb[0], xb[1], xb[2], rb);
+                gb4[row] = make_float4(gb[0], gb[1], gb[2], 0.f);
+            }
+        }
+    }
+    if (ADJ) {
+        __shared__ float red[kBlock / 32];
+        if (!VARH) SX *= -0.5f * hu.kd;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) SX += __shfl_xor_sync(0xffffffffu, SX, o);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = SX;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            float v = 0.f;
+            for (int w = 0; w < kBlock / 32; ++w) v += red[w];
+            partial[blockIdx.x] = v;
+        }
+    }
+}
+
+// g = M^+ b in sorted order as {g, V} (gbar4 == nullptr), or the records of the adjoint pair pass for a sorted
+// cotangent gbar4 (see k_renorm_solve_vjp)
+template <int DIM>
+__global__ void k_renorm_solve_sorted(int64_t n, const float4 *__restrict__ mom, const float2 *__restrict__ va_s,
+                                      const float4 *__restrict__ gbar4, float rcond, float4 *__restrict__ g4_out,
+                                      float4 *__restrict__ rb, float4 *__restrict__ rc, float2 *__restrict__ rd,
+                                      float *__restrict__ re)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    float m[6], b[3], L[3][3], P[3][3];
+    renorm_load<DIM>(mom, p, m, b);
+    renorm_pinv<DIM>(m, rcond, L, P);
+    float g[3];
+#pragma unroll
+    for (int r = 0; r < 3; ++r) g[r] = fmaf(L[r][0], b[0], fmaf(L[r][1], b[1], L[r][2] * b[2]));
+    const float2 va = va_s[p];
+    if (!gbar4) {
+        g4_out[p] = make_float4(g[0], g[1], g[2], va.x);
+        return;
+    }
+    const float4 q = gbar4[p];
+    const float gb[3] = {q.x, q.y, DIM == 3 ? q.z : 0.f};
+    float bb[3], c[3], u[3];
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        bb[r] = fmaf(L[r][0], gb[0], fmaf(L[r][1], gb[1], L[r][2] * gb[2]));
+        c[r] = gb[r] - fmaf(P[r][0], gb[0], fmaf(P[r][1], gb[1], P[r][2] * gb[2]));
+    }
+#pragma unroll
+    for (int r = 0; r < 3; ++r) u[r] = fmaf(L[r][0], g[0], fmaf(L[r][1], g[1], L[r][2] * g[2]));
+    auto N = [&](int r, int s) { return -(bb[r] * g[s] + g[r] * bb[s]) + (c[r] * u[s] + u[r] * c[s]); };
+    rb[p] = make_float4(va.x, va.y, bb[0], bb[1]);
+    if (DIM == 3) {
+        rc[p] = make_float4(bb[2], N(0, 0), N(0, 1), N(0, 2));
+        rd[p] = make_float2(N(1, 1), N(1, 2));
+        re[p] = N(2, 2);
+    } else {
+        rd[p] = make_float2(N(0, 0), N(0, 1));
+        re[p] = N(1, 1);
+    }
+}
+
 // B2 stage 2: one block, binary64 accumulation of the per-block partials in index order, then the chain rule
 // from the ten sums to params_bar = d/d{c0, rho0, gamma, delta, alpha, nu, eps, g0, g1, g2}.
 __global__ void k_reduce_params(int64_t nblocks, const float *__restrict__ partials, KPar kp, int accumulate,
@@ -903,10 +1036,14 @@ int sph_kpar_make(const sph_ctx *ctx, const sph_params *par, KPar *kp)
 {
     if (!(par->c0 > 0.f) || !(par->rho0 > 0.f) || !(par->eps > 0.f) || !(par->gamma > 0.f)) return SPH_E_INVALID;
     if (par->pressure_form != 0 && par->pressure_form != 1) return SPH_E_INVALID;
+    if (par->delta_form != 0 && par->delta_form != 1) return SPH_E_INVALID;
+    if (par->delta_form == 1 && !(par->renorm_rcond >= 0.f && par->renorm_rcond < 1.f)) return SPH_E_INVALID;
     const GridGeom &gg = ctx->geom;
     memset(kp, 0, sizeof(*kp));
     kp->dim = gg.dim;
     kp->form = par->pressure_form;
+    kp->delta_form = par->delta_form;
+    kp->rcond = par->renorm_rcond;
     for (int k = 0; k < 3; ++k) {
         kp->periodic[k] = gg.periodic[k];
         kp->L[k] = gg.L[k];
@@ -984,8 +1121,16 @@ int sph_launch_rhs_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
     const int32_t *col = ctx->col.as<int32_t>();
     const uint32_t *perm = ctx->perm.as<uint32_t>();
     const bool sorted = out4 != nullptr;
+    if (ctx->tile_mode) {
+        {
+            KScope ks(ctx, SPH_K_RHS, 1, st);
+            SPH_TRY(sph_launch_rhs_tile(ctx, kp, s0, s1, s2, kind_s, drho, acc, out4, st));
+        }
+        if (kp.delta_form == 1) SPH_TRY(sph_delta_forward(ctx, kp, s0, s1, s2, drho, out4, st));
+        return SPH_OK;
+    }
+    {
     KScope ks(ctx, SPH_K_RHS, 1, st);
-    if (ctx->tile_mode) return sph_launch_rhs_tile(ctx, kp, s0, s1, s2, kind_s, drho, acc, out4, st);
 #define SPH_RHS_LAUNCH(DIM, GS, VARH, SORTED)                                                                     \
     k_rhs<DIM, GS, VARH, SORTED><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, s0, s1, s2, kind_s, rp, col, \
                                                                      perm, drho, acc, out4)
@@ -1006,7 +1151,9 @@ int sph_launch_rhs_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
     }
 #undef SPH_RHS_GS
 #undef SPH_RHS_LAUNCH
+    }
     SPH_CUDA_TRY(cudaGetLastError());
+    if (kp.delta_form == 1) SPH_TRY(sph_delta_forward(ctx, kp, s0, s1, s2, drho, out4, st));
     return SPH_OK;
 }
 
@@ -1053,6 +1200,43 @@ int sph_launch_vjp_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
         KScope ks(ctx, SPH_K_REDUCE, 1, st);
         k_reduce_params<<<1, 128, 0, st>>>((int64_t)grid, part, kp, accumulate_params, params_bar);
     }
+    SPH_CUDA_TRY(cudaGetLastError());
+    if (kp.delta_form == 1) SPH_TRY(sph_delta_adjoint(ctx, kp, s0, s1, s2, cot, xb, rb, xb4, params_bar, st));
+    return SPH_OK;
+}
+
+int sph_delta_term_generic(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float4 *g4, const float2 *lr, bool adjoint,
+                           float *drho_io, float4 *out4_io, float4 *dx4, float4 *gb4, float *partial, int *npartial,
+                           cudaStream_t st)
+{
+    const int64_t n = ctx->n;
+    const float margin = seam_margin(ctx);
+    const int gs = kp.dim == 3 ? 32 : 16;
+    const unsigned grid = pair_grid(n, gs);
+    if (npartial) *npartial = (int)grid;
+#define SPH_DG_LAUNCH(DIM, GS, VARH, ADJ)                                                                          \
+    k_delta_term<DIM, GS, VARH, ADJ><<<grid, kBlock, 0, st>>>(n, kp, margin, pos4, g4, lr, ctx->row_ptr.as<long long>(), \
+                                                             ctx->col.as<int32_t>(), ctx->perm.as<uint32_t>(), drho_io,  \
+                                                             out4_io, dx4, gb4, partial)
+    if (kp.dim == 3) {
+        if (kp.uniform_h) { if (adjoint) SPH_DG_LAUNCH(3, 32, false, true); else SPH_DG_LAUNCH(3, 32, false, false); }
+        else { if (adjoint) SPH_DG_LAUNCH(3, 32, true, true); else SPH_DG_LAUNCH(3, 32, true, false); }
+    } else {
+        if (kp.uniform_h) { if (adjoint) SPH_DG_LAUNCH(2, 16, false, true); else SPH_DG_LAUNCH(2, 16, false, false); }
+        else { if (adjoint) SPH_DG_LAUNCH(2, 16, true, true); else SPH_DG_LAUNCH(2, 16, true, false); }
+    }
+#undef SPH_DG_LAUNCH
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_renorm_solve_sorted(sph_ctx *ctx, const KPar &kp, const float4 *mom, const float2 *va_s, const float4 *gbar4,
+                            float4 *g4_out, float4 *rb, float4 *rc, float2 *rd, float *re, cudaStream_t st)
+{
+    const int64_t n = ctx->n;
+    const unsigned nb1 = (unsigned)((n + 255) / 256);
+    if (kp.dim == 3) k_renorm_solve_sorted<3><<<nb1, 256, 0, st>>>(n, mom, va_s, gbar4, kp.rcond, g4_out, rb, rc, rd, re);
+    else k_renorm_solve_sorted<2><<<nb1, 256, 0, st>>>(n, mom, va_s, gbar4, kp.rcond, g4_out, rb, rc, rd, re);
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
@@ -1179,17 +1363,40 @@ extern "C" int sph_grad_sum_vjp(sph_ctx *ctx, const float *a, const float *g_bar
 }
 
 // moments M_i, b_i of the kernel renormalisation on either list layout (forward, and recomputed by the adjoint)
-static int launch_renorm_moments(sph_ctx *ctx, const KPar &kp, const float2 *va_s, float4 *mom, cudaStream_t st)
+int sph_renorm_moments_any(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float2 *va_s, float4 *mom, cudaStream_t st)
 {
-    if (ctx->tile_mode) return sph_launch_renorm_tile(ctx, kp, va_s, mom, st);
+    if (ctx->tile_mode) return sph_launch_renorm_tile(ctx, kp, pos4, va_s, mom, st);
     const int64_t n = ctx->n;
     const float margin = seam_margin(ctx);
 #define SPH_RN_LAUNCH(DIM, GS, VARH)                                                                             \
-    k_renorm<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), va_s,  \
+    k_renorm<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, pos4, va_s,                      \
                                                                 ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>(), mom)
     if (kp.dim == 3) { if (kp.uniform_h) SPH_RN_LAUNCH(3, 32, false); else SPH_RN_LAUNCH(3, 32, true); }
     else { if (kp.uniform_h) SPH_RN_LAUNCH(2, 16, false); else SPH_RN_LAUNCH(2, 16, true); }
 #undef SPH_RN_LAUNCH
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+static int launch_renorm_moments(sph_ctx *ctx, const KPar &kp, const float2 *va_s, float4 *mom, cudaStream_t st)
+{
+    return sph_renorm_moments_any(ctx, kp, ctx->pos_s.as<float4>(), va_s, mom, st);
+}
+
+// pair pass of the renormalised-gradient adjoint on given positions; perm == nullptr: outputs in sorted order
+int sph_renorm_vjp_pairs_any(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float4 *rb, const float4 *rc,
+                             const float2 *rd, const float *re, const uint32_t *perm, float *x_bar, float *vol_bar,
+                             float *A_bar, cudaStream_t st)
+{
+    if (ctx->tile_mode) return sph_launch_renorm_vjp_tile(ctx, kp, pos4, rb, rc, rd, re, perm, x_bar, vol_bar, A_bar, st);
+    const int64_t n = ctx->n;
+    const float margin = seam_margin(ctx);
+#define SPH_RNV_LAUNCH(DIM, GS, VARH)                                                                                  \
+    k_renorm_vjp<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, pos4, rb, rc, rd,                  \
+                                                                    re, ctx->row_ptr.as<long long>(),                   \
+                                                                    ctx->col.as<int32_t>(), perm, x_bar, vol_bar, A_bar)
+    if (kp.dim == 3) { if (kp.uniform_h) SPH_RNV_LAUNCH(3, 16, false); else SPH_RNV_LAUNCH(3, 16, true); }
+    else { if (kp.uniform_h) SPH_RNV_LAUNCH(2, 16, false); else SPH_RNV_LAUNCH(2, 16, true); }
+#undef SPH_RNV_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
@@ -1247,7 +1454,6 @@ extern "C" int sph_renorm_gradient_vjp(sph_ctx *ctx, const float *vol, const flo
     float *re = ctx->m_s.as<float>();
     KScope ks(ctx, SPH_K_DENSITY, 4, st);
     const unsigned nb1 = (unsigned)((n + 255) / 256);
-    const float margin = seam_margin(ctx);
     // forward moments again (nothing is kept between calls), then the per-particle adjoint of g = M^+ b
     k_gather_f32x2<<<nb1, 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), vol, A, va_s);
     SPH_TRY(launch_renorm_moments(ctx, kp, va_s, mom, st));
@@ -1255,17 +1461,8 @@ extern "C" int sph_renorm_gradient_vjp(sph_ctx *ctx, const float *vol, const flo
         k_renorm_solve_vjp<3><<<nb1, 256, 0, st>>>(n, mom, va_s, ctx->perm.as<uint32_t>(), grad_bar, rcond, rb, rc, rd, re);
     else
         k_renorm_solve_vjp<2><<<nb1, 256, 0, st>>>(n, mom, va_s, ctx->perm.as<uint32_t>(), grad_bar, rcond, rb, rc, rd, re);
-    if (ctx->tile_mode) return sph_launch_renorm_vjp_tile(ctx, kp, rb, rc, rd, re, x_bar, vol_bar, A_bar, st);
-#define SPH_RNV_LAUNCH(DIM, GS, VARH)                                                                                  \
-    k_renorm_vjp<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), rb, rc, rd, \
-                                                                    re, ctx->row_ptr.as<long long>(),                   \
-                                                                    ctx->col.as<int32_t>(), ctx->perm.as<uint32_t>(),   \
-                                                                    x_bar, vol_bar, A_bar)
-    if (kp.dim == 3) { if (kp.uniform_h) SPH_RNV_LAUNCH(3, 16, false); else SPH_RNV_LAUNCH(3, 16, true); }
-    else { if (kp.uniform_h) SPH_RNV_LAUNCH(2, 16, false); else SPH_RNV_LAUNCH(2, 16, true); }
-#undef SPH_RNV_LAUNCH
-    SPH_CUDA_TRY(cudaGetLastError());
-    return SPH_OK;
+    return sph_renorm_vjp_pairs_any(ctx, kp, ctx->pos_s.as<float4>(), rb, rc, rd, re, ctx->perm.as<uint32_t>(), x_bar,
+                                    vol_bar, A_bar, st);
 }
 
 extern "C" int sph_rhs(sph_ctx *ctx, const sph_params *par, const float *x, const float *v, const float *rho,

@@ -467,7 +467,7 @@ k_renorm_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__
             vb = group_sum<GS>(vb);
             ab = group_sum<GS>(ab);
             if (gl == 0 && live) {
-                const int64_t i = perm[row0 + r];
+                const int64_t i = perm ? (int64_t)perm[row0 + r] : (int64_t)(row0 + r);   // null perm: sorted order
 #pragma unroll
                 for (int k = 0; k < DIM; ++k) xb_out[i * DIM + k] = xb[k];
                 if (vb_out) vb_out[i] = vb;
@@ -877,6 +877,125 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
     }
 }
 
+// ------------------------------------------------------------------------------------------ delta-term of [43]
+// Second part of the delta-SPH diffusion with the renormalised density gradient (sph_params.delta_form = 1; PAPER.md:103,
+// 85, 524-530; reading R17):  X_ij = -delta l_ij c0 V_j (g_i + g_j).d G,  g = <grad rho>^L.
+// smem: A = {x,y,z,h} (current positions), B = {g_x,g_y,g_z,V}, ADJ: C = {lambda, rho} (float2).
+//   ADJ = false: drho_i += sum_j X_ij                                   (added to the caller's array or to out4[row].w)
+//   ADJ = true : gather form of the adjoint for the cotangent lambda (both ordered pairs of every neighbour in the
+//                owner's row; w = lambda_i V_j - lambda_j V_i, S = (g_i+g_j).d, Q = (g_i+g_j) G + S K d):
+//                x_bar_i += c w Q,  g_bar_i += c w G d,  rho_bar_i += lambda_j c V_i S G / rho_i,  and per tile
+//                sum lambda_i X_ij (-> delta_bar, c0_bar).  Written in SORTED order: dx4 = {x_bar, rho_bar}, gb4 = {g_bar, 0}.
+constexpr int kDeltaState = 40;
+template <int DIM, int GS, bool VARH, bool ADJ>
+__global__ void __launch_bounds__(kPtMaxWarps * 32)
+k_delta_term_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ pos4, const float4 *__restrict__ g4,
+                  const float2 *__restrict__ lr, const uint32_t *__restrict__ cell_start,
+                  const uint32_t *__restrict__ cell_end, const long long *__restrict__ row_ptr,
+                  const uint16_t *__restrict__ col16, const uint32_t *__restrict__ perm, float *__restrict__ drho_io,
+                  float4 *__restrict__ out4_io, float4 *__restrict__ dx4, float4 *__restrict__ gb4,
+                  float *__restrict__ partial)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    size_t o = 0;
+    float4 *A = reinterpret_cast<float4 *>(smem_raw + o); o += (size_t)ts.mcap * 16;
+    float4 *B = reinterpret_cast<float4 *>(smem_raw + o); o += (size_t)ts.mcap * 16;
+    float2 *C = reinterpret_cast<float2 *>(smem_raw + o); o += (size_t)ts.mcap * 8;
+    uint32_t *rp = reinterpret_cast<uint32_t *>(smem_raw + o); o += (size_t)(ts.tcap + 4) * 4;
+    uint16_t *selfq = reinterpret_cast<uint16_t *>(smem_raw + o); o += (size_t)ts.tcap * 2;
+    o = (o + 15) & ~(size_t)15;
+    uint16_t *ring = reinterpret_cast<uint16_t *>(smem_raw + o);
+    __shared__ TileTab tt;
+    __shared__ float red[kPtMaxWarps];
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (tt.T == 0) {
+        if (ADJ && threadIdx.x == 0) partial[blockIdx.x] = 0.f;
+        return;
+    }
+    stage_halo(tt, pos4, A, g4, B, nullptr, nullptr, ADJ ? lr : nullptr, C, nullptr, nullptr);
+    stage_rows(tt, row_ptr, rp, selfq);
+    cp_async_wait<0>();
+    __syncthreads();
+    stage_shift<DIM>(tt, A);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gl = lane % GS;
+    const HC hu = hc_uniform<DIM>(kp);
+    const uint32_t row0 = tt.row0;
+    float SX = 0.f;                                              // per lane: sum lambda_i V_j S G (c applied below)
+    tile_row_passes<GS>(tt, rp, ring, ts.rb, col16, row_ptr[tt.row0],
+        [&](uint32_t r, bool live, uint32_t b, uint32_t e_in, const uint16_t *idx) {
+            const uint32_t qi = selfq[r];
+            const uint32_t e = live ? e_in : b;
+            const float4 pi = A[qi], gi = B[qi];
+            float2 li = make_float2(0.f, 1.f);
+            if (ADJ) li = C[qi];
+            float acc = 0.f, xb[3] = {0.f, 0.f, 0.f}, gb[3] = {0.f, 0.f, 0.f}, rb = 0.f;
+            for (uint32_t k = b + gl; k < e; k += GS) {
+                const uint32_t j = idx[k];
+                SPH_ASSERT(j < tt.M);
+                const float4 pj = A[j], gj = B[j];
+                const float d[3] = {pi.x - pj.x, pi.y - pj.y, DIM == 3 ? pi.z - pj.z : 0.f};
+                const float r2 = fmaf(d[2], d[2], fmaf(d[1], d[1], d[0] * d[0]));
+                HC hc = hu;
+                if (VARH) hc = hc_make<DIM>(fmaxf(pi.w, pj.w), kp);
+                const float rr = fast_sqrt(r2);
+                const float t = fmaxf(fmaf(-hc.invH, rr, 1.0f), 0.f);
+                const float t2 = t * t, t4 = t2 * t2;
+                const float G = hc.cG * fmaf(5.0f * hc.invH, rr, 1.0f) * (t4 * t);
+                const float gs[3] = {gi.x + gj.x, gi.y + gj.y, DIM == 3 ? gi.z + gj.z : 0.f};
+                const float S = fmaf(gs[2], d[2], fmaf(gs[1], d[1], gs[0] * d[0]));
+                const float cc = VARH ? -0.5f * hc.kd : 1.0f;       // uniform h: the factor -delta l c0 is applied per row
+                if (!ADJ) {
+                    acc = fmaf(cc * gj.w, S * G, acc);
+                } else {
+                    const float2 lj = C[j];
+                    const float K = hc.cK * t4;
+                    const float w = cc * fmaf(li.x, gj.w, -(lj.x * gi.w));      // c (lambda_i V_j - lambda_j V_i)
+                    const float SK = S * K;
+#pragma unroll
+                    for (int kk = 0; kk < DIM; ++kk) {
+                        xb[kk] = fmaf(w, fmaf(gs[kk], G, SK * d[kk]), xb[kk]);
+                        gb[kk] = fmaf(w * G, d[kk], gb[kk]);
+                    }
+                    rb = fmaf(cc * lj.x, S * G, rb);                            // x V_i / rho_i below
+                    SX = fmaf(cc * li.x * gj.w, S * G, SX);
+                }
+            }
+            const float cu = VARH ? 1.0f : -0.5f * hu.kd;
+            if (!ADJ) {
+                acc = group_sum<GS>(acc) * cu;
+                if (gl == 0 && live) {
+                    const uint32_t row = row0 + r;
+                    if (out4_io) out4_io[row].w += acc;
+                    else drho_io[perm[row]] += acc;
+                }
+            } else {
+#pragma unroll
+                for (int kk = 0; kk < DIM; ++kk) {
+                    xb[kk] = group_sum<GS>(xb[kk]) * cu;
+                    gb[kk] = group_sum<GS>(gb[kk]) * cu;
+                }
+                rb = group_sum<GS>(rb) * cu * gi.w / li.y;
+                if (gl == 0 && live) {
+                    const uint32_t row = row0 + r;
+                    dx4[row] = make_float4(xb[0], xb[1], xb[2], rb);
+                    gb4[row] = make_float4(gb[0], gb[1], gb[2], 0.f);
+                }
+            }
+        });
+    if (ADJ) {
+        if (!VARH) SX *= -0.5f * hu.kd;
+#pragma unroll
+        for (int o2 = 16; o2 > 0; o2 >>= 1) SX += __shfl_xor_sync(0xffffffffu, SX, o2);
+        if (lane == 0) red[warp] = SX;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            float v = 0.f;
+            for (int w = 0; w < nwarps; ++w) v += red[w];
+            partial[blockIdx.x] = v;
+        }
+    }
+}
+
 } // namespace
 
 // ==========================================================================================
@@ -995,7 +1114,7 @@ int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s
     return SPH_OK;
 }
 
-int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float2 *va_s, float4 *mom, cudaStream_t st)
+int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float2 *va_s, float4 *mom, cudaStream_t st)
 {
     const TileGeom &tg = ctx->tg;
     const int gs = tile_group(ctx, false);
@@ -1007,7 +1126,7 @@ int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float2 *va_s, flo
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_renorm_tile<DIM, GS, VARH>), smem);                                                     \
         k_renorm_tile<DIM, GS, VARH><<<(unsigned)tg.ntiles, threads, smem, st>>>(                                     \
-            tg, kp, ts, ctx->pos_s.as<float4>(), va_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),  \
+            tg, kp, ts, pos4, va_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),                     \
             ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), mom);                                            \
     } while (0)
 #define SPH_RNT_GS(GS)                                                                                      \
@@ -1026,8 +1145,9 @@ int sph_launch_renorm_tile(sph_ctx *ctx, const KPar &kp, const float2 *va_s, flo
     return SPH_OK;
 }
 
-int sph_launch_renorm_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *rb, const float4 *rc, const float2 *rd,
-                               const float *re, float *x_bar, float *vol_bar, float *A_bar, cudaStream_t st)
+int sph_launch_renorm_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float4 *rb, const float4 *rc,
+                               const float2 *rd, const float *re, const uint32_t *perm, float *x_bar, float *vol_bar,
+                               float *A_bar, cudaStream_t st)
 {
     const TileGeom &tg = ctx->tg;
     const int gs = tile_group(ctx, true);
@@ -1039,9 +1159,9 @@ int sph_launch_renorm_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *rb, c
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_renorm_vjp_tile<DIM, GS, VARH>), smem);                                                 \
         k_renorm_vjp_tile<DIM, GS, VARH><<<(unsigned)tg.ntiles, threads, smem, st>>>(                                 \
-            tg, kp, ts, ctx->pos_s.as<float4>(), rb, rc, rd, re, ctx->cell_start.as<uint32_t>(),                      \
+            tg, kp, ts, pos4, rb, rc, rd, re, ctx->cell_start.as<uint32_t>(),                                         \
             ctx->cell_end.as<uint32_t>(), ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(),                    \
-            ctx->perm.as<uint32_t>(), x_bar, vol_bar, A_bar);                                                         \
+            perm, x_bar, vol_bar, A_bar);                                                         \
     } while (0)
 #define SPH_RNVT_GS(GS)                                                                                       \
     do {                                                                                                      \
@@ -1221,6 +1341,45 @@ int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
 #undef SPH_VT_LAUNCH1
 #undef SPH_VT_LAUNCH2
     }
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
+}
+
+// delta-term of [43] (tile layout); see k_delta_term_tile.  pos4/g4/lr: sorted arrays of the current state.
+int sph_launch_delta_term_tile(sph_ctx *ctx, const KPar &kp, const float4 *pos4, const float4 *g4, const float2 *lr,
+                               bool adjoint, float *drho_io, float4 *out4_io, float4 *dx4, float4 *gb4, float *partial,
+                               cudaStream_t st)
+{
+    const TileGeom &tg = ctx->tg;
+    const int gs = tile_group(ctx, false);
+    int threads;
+    TileSizes ts;
+    size_t smem;
+    tile_launch_cfg(ctx, kDeltaState, gs, sizeof(TileTab) + kPtMaxWarps * 4, kPtMaxWarps, 64, &threads, &ts, &smem);
+#define SPH_DLT_LAUNCH(DIM, GS, VARH, ADJ)                                                                            \
+    do {                                                                                                              \
+        SPH_TILE_SMEM_ATTR((k_delta_term_tile<DIM, GS, VARH, ADJ>), smem);                                            \
+        k_delta_term_tile<DIM, GS, VARH, ADJ><<<(unsigned)tg.ntiles, threads, smem, st>>>(                            \
+            tg, kp, ts, pos4, g4, lr, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),                   \
+            ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), drho_io, out4_io, dx4, \
+            gb4, partial);                                                                                            \
+    } while (0)
+#define SPH_DLT_GS(GS)                                                                                                \
+    do {                                                                                                              \
+        if (kp.dim == 3) {                                                                                            \
+            if (kp.uniform_h) { if (adjoint) SPH_DLT_LAUNCH(3, GS, false, true); else SPH_DLT_LAUNCH(3, GS, false, false); } \
+            else { if (adjoint) SPH_DLT_LAUNCH(3, GS, true, true); else SPH_DLT_LAUNCH(3, GS, true, false); }           \
+        } else {                                                                                                      \
+            if (kp.uniform_h) { if (adjoint) SPH_DLT_LAUNCH(2, GS, false, true); else SPH_DLT_LAUNCH(2, GS, false, false); } \
+            else { if (adjoint) SPH_DLT_LAUNCH(2, GS, true, true); else SPH_DLT_LAUNCH(2, GS, true, false); }           \
+        }                                                                                                             \
+    } while (0)
+    switch (gs) {
+    case 16: SPH_DLT_GS(16); break;
+    default: SPH_DLT_GS(8); break;
+    }
+#undef SPH_DLT_GS
+#undef SPH_DLT_LAUNCH
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

@@ -384,6 +384,54 @@ def test_pressure_form_1_rhs_vjp_and_rk_parity(sph, case):
     assert max_norm_err(_np(rho).astype(np.float64) - wl.rho, ro2 - wl.rho) < TOL_FWD + fl(wl.rho, ro2 - wl.rho)
 
 
+@pytest.mark.parametrize("case", ["C0p", "C1s", "C2p", "C3p", "C4s"])
+def test_delta_form_1_rhs_vjp_and_rk_parity(sph, case):
+    """delta_form = 1: the delta-SPH diffusion of [43] with the renormalised density gradient (PAPER.md:103, 85, 524-530;
+    reading R17).  RHS (two more pair passes and a per-particle pseudo-inverse before the term), its adjoint including the
+    path through L_i, one RK4 step and the step's adjoint, all against the oracle; on every list layout."""
+    wl = CASES[case]()
+    base = wl.params.__dict__
+    par = W.Params(**{**base, "delta_form": 1, "renorm_rcond": 1e-4,
+                      **({} if case.startswith("C2") else {"alpha": 0.02, "g": (0.3, -0.2, 0.1)})})
+    lam, mu = W.random_cotangents(wl)
+    _, dev, _ = build(wl, 1.0, sph)
+    lists = oracle_lists(wl)
+    drho, acc = sph.rhs(par, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+    d_o, a_o, sd, sa = oracle.rhs(wl.domain, par, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *lists, with_scales=True)
+    _check_forward(f"{case} delta_form 1", _np(drho), _np(acc), d_o, a_o, sd, sa, floor_for(case))
+    d0, _ = oracle.rhs(wl.domain, W.Params(**{**par.__dict__, "delta_form": 0}), wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *lists)
+    if not case.startswith("C2"):                # (smooth hydrostatic density: the term is small against the continuity part)
+        assert np.max(np.abs(d0 - d_o)) > 1e-3 * np.max(np.abs(d_o))      # the two forms differ
+    xb, vb, rb, pb = sph.rhs_vjp(par, dev.x, dev.v, dev.rho, dev.m, dev.kind, torch.from_numpy(lam).cuda(),
+                                 torch.from_numpy(mu).cuda())
+    xo, vo, ro, po = oracle.rhs_vjp(wl.domain, par, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *lists, lam, mu)
+    errs = dict(x=max_norm_err(_np(xb), xo), v=max_norm_err(_np(vb), vo), rho=max_norm_err(_np(rb), ro))
+    pe = _params_err(_np(pb), po)
+    print(f"{case} delta_form 1: vjp errs {errs} params {pe:.2e}")
+    assert max(errs.values()) < TOL_VJP and pe < TOL_VJP
+    # one RK4 step and its adjoint (gradient of the kinetic energy after the step)
+    skin = 0.1
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin) * np.float32(1.0001))
+    dt = wl.dt if wl.dt > 0 else 0.1 * float(wl.h.min()) / par.c0
+    x, v, rho = dev.x.clone(), dev.v.clone(), dev.rho.clone()
+    sph.rk_step(wl.domain, par, dt, skin, x, v, rho, dev.m, dev.h, dev.kind)
+    xo2, vo2, ro2 = oracle.rk4_step(wl.domain, par, dt, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, method=1)
+    fl = lambda a, b: 2.0 ** -23 * np.max(np.abs(a)) / max(np.max(np.abs(b)), 1e-300)
+    assert max_norm_err(_np(v).astype(np.float64) - wl.v, vo2 - wl.v) < TOL_FWD + fl(wl.v, vo2 - wl.v)
+    assert max_norm_err(_np(rho).astype(np.float64) - wl.rho, ro2 - wl.rho) < TOL_FWD + fl(wl.rho, ro2 - wl.rho)
+    xb = torch.zeros_like(dev.x)
+    vb = (dev.m[:, None] * v).contiguous()
+    rb = torch.zeros_like(dev.rho)
+    pb = torch.zeros(10, device="cuda")
+    sph.rk_step_vjp(wl.domain, par, dt, skin, dev.x, dev.v, dev.rho, dev.m, dev.h, dev.kind, xb, vb, rb, pb)
+    xo, vo, ro, po = oracle.rk4_step_vjp(wl.domain, par, dt, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, np.zeros_like(vo2),
+                                         wl.m.astype(np.float64)[:, None] * vo2, np.zeros(wl.n), method=1)
+    errs = dict(x=max_norm_err(_np(xb), xo), v=max_norm_err(_np(vb), vo), rho=max_norm_err(_np(rb), ro))
+    pe = _params_err(_np(pb), po)
+    print(f"{case} delta_form 1: rk vjp errs {errs} params {pe:.2e}")
+    assert max(errs.values()) < TOL_VJP and pe < TOL_VJP
+
+
 def test_rhs_independent_of_skin(sph):
     """pairs with r >= H_ij in a skin-enlarged list contribute exactly 0 (kernel clamp)"""
     wl = CASES["C3p"]()
