@@ -184,6 +184,14 @@ int sph_rk_step_vjp(sph_ctx *ctx, const sph_domain *dom, const sph_params *par, 
                     const uint8_t *kind, float *x_bar, float *v_bar, float *rho_bar, float *params_bar,
                     sph_stream_t stream);
 
+/* Particle shifting at the end of a step (the scheme of [41] is not printed: reading R18 of DESIGN.md
+ * takes the Fickian form along the gradient of the particle concentration):
+ *     x_i <- x_i - theta l_i^2 sum_j (m_j/rho_j) grad_i W_ij     for fluid kinds (kind 0),  l_i = h_i / kappa_d,
+ * evaluated at the CURRENT positions x on the lists of the last sph_neighbors / sph_rk_step (they must still be a
+ * superset of the neighbours: e.g. directly after sph_rk_step, whose lists carry the skin).  x: in/out. */
+int sph_shift(sph_ctx *ctx, float theta, float *x, const float *m, const float *rho, const uint8_t *kind,
+              sph_stream_t stream);
+
 /* End-to-end convenience call with HOST buffers (pageable or pinned): copies the inputs to the device, runs
  * sph_build_cells + sph_neighbors(search_scale) + sph_rhs + sph_rhs_vjp, copies the seven outputs back and
  * synchronises.  Output pointers may be NULL (skipped).  params_bar: host float[10]. */

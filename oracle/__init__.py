@@ -135,6 +135,19 @@ def grad_sum(domain, x, h, a, row_ptr, col_idx):
     return g
 
 
+def shift(domain, x, h, m, rho, kind, theta, row_ptr, col_idx):
+    """Particle shifting at the end of a step (reading R18, Fickian form):
+    x_i <- x_i - theta l_i^2 sum_j (m_j/rho_j) grad_i W_ij for fluid kinds, l = h/kappa_d."""
+    dim = int(domain.dim)
+    kap = 2.171239 if dim == 2 else 2.207940
+    g = grad_sum(domain, x, h, _d(m) / _d(rho), row_ptr, col_idx)
+    ell = _d(np.asarray(h, dtype=np.float32)) / kap
+    out = _d(x).copy()
+    fluid = np.asarray(kind) == 0
+    out[fluid] -= theta * (ell[fluid] ** 2)[:, None] * g[fluid]
+    return out
+
+
 def grad_sum_vjp(domain, x, h, a, row_ptr, col_idx, g_bar):
     """(x_bar, a_bar) = J^T g_bar of grad_sum() with the adjacency held fixed"""
     dim, per, lo, hi = _dom(domain)

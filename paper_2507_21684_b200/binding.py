@@ -19,7 +19,7 @@ EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph
            "sph_density_vjp", "sph_lists_valid", "sph_grad_sum", "sph_grad_sum_vjp", "sph_renorm_gradient", "sph_renorm_gradient_vjp",
            "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
            "sph_check", "sph_strerror", "sph_get_info", "sph_get_layout", "sph_profile_enable", "sph_profile_read",
-           "sph_set_option")
+           "sph_set_option", "sph_shift")
 
 # keys of sph_set_option (enum SPH_OPT_* in include/sph.h)
 OPT_PAIR_GROUP, OPT_LIST_MODE, OPT_TILE_EDGE, OPT_PAIR_WARPS, OPT_FILL_MASKS, OPT_RK_EXTRA_SKIN = 1, 2, 3, 4, 5, 6
@@ -72,6 +72,7 @@ def load_library(path: str = LIB_PATH):
     lib.sph_grad_sum_vjp.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.sph_renorm_gradient.argtypes = [vp, vp, vp, C.c_float, vp, vp, vp]
     lib.sph_renorm_gradient_vjp.argtypes = [vp, vp, vp, C.c_float, vp, vp, vp, vp, vp]
+    lib.sph_shift.argtypes = [vp, f32, vp, vp, vp, vp, vp]
     lib.sph_lists_valid.argtypes = [vp, vp, f32, C.POINTER(C.c_int32), C.POINTER(f32), vp]
     lib.sph_rhs.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 7 + [vp]
     lib.sph_rhs_vjp.argtypes = [vp, C.POINTER(SphParams)] + [vp] * 11 + [vp]
@@ -182,6 +183,14 @@ class Sph:
         col = torch.empty(max(self.nnz, 1), dtype=torch.int32, device=f"cuda:{self.device}")
         self._chk(self.lib.sph_neighbors_export(self._ctx, _ptr(row_ptr), _ptr(col), _stream()))
         return row_ptr, col[: self.nnz]
+
+    def shift(self, theta, x, m, rho, kind):
+        """particle shifting at the end of a step: x <- x - theta l^2 sum_j V_j grad_i W_ij for fluid
+        kinds, at the current positions, on the lists of the last build; x in place"""
+        _f32(x, (self.n, self.dim)); _f32(m, (self.n,)); _f32(rho, (self.n,))
+        assert kind.dtype == torch.uint8 and kind.is_cuda and kind.is_contiguous()
+        self._chk(self.lib.sph_shift(self._ctx, float(theta), _ptr(x), _ptr(m), _ptr(rho), _ptr(kind), _stream()))
+        return x
 
     def lists_valid(self, x, skin_needed: float = 0.0):
         """(valid, max displacement since the build): the Verlet-list test of PAPER.md:568"""

@@ -163,6 +163,7 @@ struct sph_ctx {
     DevBuf maskbuf, tile_words, tile_mask_base;   // hit masks of the count pass, per-tile mask offsets
     // one-kernel build: cell statistics, look-back states, {ticket, overflow}, tiles in Morton order (cached per grid)
     DevBuf fstats, tstate, fctl;
+    const float4 *pos_override = nullptr;         // sph_shift: sph_grad_sum's kernels read these positions instead of pos_s
     // delta_form 1: current positions {x,y,z,h}, {V,rho}, moments, {g,V}, adjoint records and sorted partial results
     DevBuf d_pos, d_va, d_mom, d_g4, d_lr, d_dx4, d_gb4, d_rb, d_rc, d_rd, d_re, d_x2, d_vb, d_ab, d_part;
     struct TileOrder {                            // cache slot: the order depends on the grid and on B only

@@ -1328,7 +1328,8 @@ static int grad_sum_common(sph_ctx *ctx, const float *a, const float *g_bar, flo
     if (ctx->tile_mode) return sph_launch_grad_sum_vjp_tile(ctx, kp, ga, v_out, a_out, st);
     const float margin = seam_margin(ctx);
 #define SPH_GS_LAUNCH(DIM, GS, VARH, VJP)                                                                             \
-    k_grad_sum<DIM, GS, VARH, VJP><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(), ga,   \
+    k_grad_sum<DIM, GS, VARH, VJP><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin,                                \
+                                                                       ctx->pos_override ? ctx->pos_override : ctx->pos_s.as<float4>(), ga, \
                                                                        ctx->row_ptr.as<long long>(), ctx->col.as<int32_t>(), \
                                                                        ctx->perm.as<uint32_t>(), v_out, a_out)
 #define SPH_GS_DIM(DIM, GS)                                                                                  \
@@ -1360,6 +1361,86 @@ extern "C" int sph_grad_sum_vjp(sph_ctx *ctx, const float *a, const float *g_bar
     SPH_CUDA_TRY(cudaSetDevice(ctx->device));
     ctx->last_stream = (cudaStream_t)stream;
     return grad_sum_common(ctx, a, g_bar, x_bar, a_bar, true, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------------------------------ particle shifting
+// End-of-step particle shifting ("particle-shifting only at the end of each overall timestep", PAPER.md:680;
+// the scheme of [41] is not printed -- DESIGN.md reading R18: the Fickian form, shift along the gradient of the particle
+// concentration C_i = sum_j V_j W_ij):   x_i <- x_i - theta l_i^2 sum_j V_j grad_i W_ij   for fluid kinds, l = h/kappa_d.
+// The sum is sph_grad_sum with a = m/rho, evaluated at the CURRENT positions on the lists of the last build (valid as
+// long as they are a superset of the neighbours, e.g. right after sph_rk_step with its skin).
+namespace {
+template <int DIM>
+__global__ void k_shift_prep(int64_t n, KPar kp, const uint32_t *__restrict__ perm, const float4 *__restrict__ pos_s,
+                             const float *__restrict__ x, const float *__restrict__ m, const float *__restrict__ rho,
+                             float4 *__restrict__ pos4, float *__restrict__ vol)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const int64_t i = perm[p];
+    const float4 pb = pos_s[p];
+    const float xb[3] = {pb.x, pb.y, pb.z};
+    float xw[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) {
+        float xv = x[i * DIM + k];
+        if (kp.periodic[k]) {                                  // the periodic image next to the build position (k_pack_state)
+            xv = wrap_coord(xv, kp.lo[k], kp.hi[k], kp.L[k]);
+            const float dd = xv - xb[k];
+            xv = dd > kp.halfL[k] ? xv - kp.L[k] : (dd < -kp.halfL[k] ? xv + kp.L[k] : xv);
+        }
+        xw[k] = xv;
+    }
+    pos4[p] = make_float4(xw[0], xw[1], xw[2], pb.w);
+    vol[i] = m[i] / rho[i];                                    // caller order: the weights of sph_grad_sum
+}
+template <int DIM>
+__global__ void k_shift_apply(int64_t n, float theta, float inv_kappa, const uint32_t *__restrict__ inv_perm,
+                              const float4 *__restrict__ pos_s, const uint8_t *__restrict__ kind, const float *__restrict__ g,
+                              float *__restrict__ x)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n || kind[i]) return;
+    const float ell = pos_s[inv_perm[i]].w * inv_kappa;
+    const float c = -theta * ell * ell;
+#pragma unroll
+    for (int k = 0; k < DIM; ++k) x[i * DIM + k] = fmaf(c, g[i * DIM + k], x[i * DIM + k]);
+}
+} // namespace
+
+extern "C" int sph_shift(sph_ctx *ctx, float theta, float *x, const float *m, const float *rho, const uint8_t *kind,
+                         sph_stream_t stream)
+{
+    if (!ctx || !x || !m || !rho || !kind || !isfinite(theta)) return SPH_E_INVALID;
+    if (!ctx->lists_ready) return SPH_E_STATE;
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    const int64_t n = ctx->n;
+    sph_params dummy{};
+    dummy.c0 = 1.f; dummy.rho0 = 1.f; dummy.gamma = 1.f; dummy.eps = 1.f;
+    KPar kp;
+    SPH_TRY(sph_kpar_make(ctx, &dummy, &kp));
+    SPH_TRY(ctx->d_pos.reserve((size_t)n * 16));
+    SPH_TRY(ctx->d_vb.reserve((size_t)n * 4));
+    SPH_TRY(ctx->d_x2.reserve((size_t)n * 12));
+    const unsigned nb1 = (unsigned)((n + 255) / 256);
+    {
+        KScope ks(ctx, SPH_K_PACK, 1, st);
+        if (kp.dim == 3) k_shift_prep<3><<<nb1, 256, 0, st>>>(n, kp, ctx->perm.as<uint32_t>(), ctx->pos_s.as<float4>(), x, m, rho, ctx->d_pos.as<float4>(), ctx->d_vb.as<float>());
+        else k_shift_prep<2><<<nb1, 256, 0, st>>>(n, kp, ctx->perm.as<uint32_t>(), ctx->pos_s.as<float4>(), x, m, rho, ctx->d_pos.as<float4>(), ctx->d_vb.as<float>());
+    }
+    ctx->pos_override = ctx->d_pos.as<float4>();
+    const int rc = grad_sum_common(ctx, ctx->d_vb.as<float>(), nullptr, ctx->d_x2.as<float>(), nullptr, false, st);
+    ctx->pos_override = nullptr;
+    SPH_TRY(rc);
+    {
+        KScope ks(ctx, SPH_K_RK, 1, st);
+        if (kp.dim == 3) k_shift_apply<3><<<nb1, 256, 0, st>>>(n, theta, kp.inv_kappa, ctx->inv_perm.as<uint32_t>(), ctx->pos_s.as<float4>(), kind, ctx->d_x2.as<float>(), x);
+        else k_shift_apply<2><<<nb1, 256, 0, st>>>(n, theta, kp.inv_kappa, ctx->inv_perm.as<uint32_t>(), ctx->pos_s.as<float4>(), kind, ctx->d_x2.as<float>(), x);
+    }
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
 }
 
 // moments M_i, b_i of the kernel renormalisation on either list layout (forward, and recomputed by the adjoint)

@@ -1192,7 +1192,8 @@ static int launch_grad_sum_tile(sph_ctx *ctx, const KPar &kp, const float *a_s, 
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_grad_sum_tile<DIM, GS, VARH, VJP>), smem);                                              \
         k_grad_sum_tile<DIM, GS, VARH, VJP><<<(unsigned)tg.ntiles, threads, smem, st>>>(                              \
-            tg, kp, ts, ctx->pos_s.as<float4>(), a_s, ga_s, ctx->cell_start.as<uint32_t>(),                           \
+            tg, kp, ts, ctx->pos_override ? ctx->pos_override : ctx->pos_s.as<float4>(), a_s, ga_s,                   \
+            ctx->cell_start.as<uint32_t>(),                                                                           \
             ctx->cell_end.as<uint32_t>(), ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(),                    \
             ctx->perm.as<uint32_t>(), v_out, a_out);                                                                  \
     } while (0)

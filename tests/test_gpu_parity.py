@@ -432,6 +432,37 @@ def test_delta_form_1_rhs_vjp_and_rk_parity(sph, case):
     assert max(errs.values()) < TOL_VJP and pe < TOL_VJP
 
 
+@pytest.mark.parametrize("case", ["C0p", "C2p", "C3p", "C4s"])
+def test_shift_parity(sph, case):
+    """sph_shift (reading R18) at positions that moved since the list build, against oracle.shift on the
+    oracle's own lists of the moved positions (the skin list is a superset; the extra pairs contribute exactly 0)"""
+    wl = CASES[case]()
+    skin = 0.1
+    wl.domain.cell_size = float(np.float32(wl.domain.cell_size) * np.float32(1.0 + skin) * np.float32(1.0001))
+    _, dev, _ = build(wl, 1.0 + skin, sph)
+    rng = np.random.default_rng(4)
+    x1 = (wl.x + rng.uniform(-0.02, 0.02, size=wl.x.shape) * float(wl.h.min())).astype(np.float32)
+    if not any(wl.domain.periodic):
+        x1 = np.clip(x1, np.float32(wl.domain.lo[0]) + 1e-6, None)
+        for k in range(wl.dim):
+            x1[:, k] = np.clip(x1[:, k], np.float32(wl.domain.lo[k]) + np.float32(1e-6), np.float32(wl.domain.hi[k]) - np.float32(1e-6))
+    theta = 0.4
+    xg = torch.from_numpy(x1.copy()).cuda()
+    sph.shift(theta, xg, dev.m, dev.rho, dev.kind)
+    import copy
+    wl1 = copy.copy(wl)
+    wl1.x = x1
+    xo = oracle.shift(wl.domain, x1, wl.h, wl.m, wl.rho, wl.kind, theta, *oracle_lists(wl1))
+    dg, do = _np(xg).astype(np.float64) - x1, xo - x1
+    # the shift is a sum that cancels on near-lattices: judged against the size of its terms like drho/dt (R10)
+    kap = 2.171239 if wl.dim == 2 else 2.207940
+    scale = theta * (float(wl.h.max()) / kap) ** 2 * float(np.max(wl.m / wl.rho)) * abs(oracle.gfac(0.5 * float(wl.h.min()), float(wl.h.min()), wl.dim)) * 0.5 * float(wl.h.min()) * 50
+    err = float(np.max(np.abs(dg - do)) / max(np.max(np.abs(do)), 1e-3 * scale))
+    print(f"{case}: shift err {err:.2e} (max shift {np.max(np.abs(do)) / float(wl.h.min()):.2e} h)")
+    assert err < TOL_FWD + 2.0 ** -23 * np.max(np.abs(x1)) / max(np.max(np.abs(do)), 1e-300)
+    assert np.all(_np(xg)[wl.kind == 1] == x1[wl.kind == 1])
+
+
 def test_rhs_independent_of_skin(sph):
     """pairs with r >= H_ij in a skin-enlarged list contribute exactly 0 (kernel clamp)"""
     wl = CASES["C3p"]()

@@ -547,6 +547,31 @@ def test_rhs_boundary_kinds():
     assert acc2[near, 0] > acc1[near, 0]
 
 
+# ------------------------------------------------------------------------------------------ shifting
+def test_shift_restores_a_displaced_particle_and_leaves_a_lattice_alone():
+    """Fickian shifting x <- x - theta l^2 grad C, C = sum_j V_j W_ij (reading R18): nothing moves on a periodic lattice
+    (grad C = 0 by symmetry); a particle displaced from its lattice site is pushed back along the displacement, its
+    neighbours away from it; boundary kinds do not move; the concentration becomes more uniform."""
+    wl = W.make(0, n_axis=16)
+    lists = oracle.neighbors(wl.domain, wl.x, wl.h, method=1)
+    x1 = oracle.shift(wl.domain, wl.x, wl.h, wl.m, wl.rho, wl.kind, 0.5, *lists)
+    assert np.max(np.abs(x1 - wl.x)) < 1e-12
+    x = wl.x.astype(np.float64).copy()
+    i = 16 * 8 + 8
+    disp = np.array([0.3, 0.2]) * wl.dx
+    x[i] += disp
+    lists = oracle.neighbors(wl.domain, x.astype(np.float32), wl.h, method=1)
+    x32 = x.astype(np.float32)
+    kind = wl.kind.copy()
+    kind[i + 1] = 1
+    xs = oracle.shift(wl.domain, x32, wl.h, wl.m, wl.rho, kind, 0.5, *lists)
+    move = xs[i] - x32[i]
+    assert np.dot(move, disp) < 0 and np.linalg.norm(move) < np.linalg.norm(disp)      # back towards the site, no overshoot
+    assert np.all(xs[i + 1] == x32[i + 1])                                              # boundary kind: fixed
+    conc = lambda xx: oracle.density(wl.domain, xx.astype(np.float32), wl.h, wl.m, *lists)
+    assert np.std(conc(xs)) < np.std(conc(x32))
+
+
 # ------------------------------------------------------------------------------------------ delta-term of [43]
 def _open_box_case(dim, n_axis, seed, amp):
     """disordered particles in an open (bounded) box: the outer layers have truncated neighbourhoods (free surface)"""
