@@ -80,8 +80,9 @@ enum {
     SPH_OK = 0,
     SPH_E_INVALID = -1, /* null pointer, n <= 0, dim not 2/3, eps <= 0, c0/rho0 <= 0, unsupported option */
     SPH_E_DOMAIN = -2,  /* cell_size < search radius, < 3 cells on a periodic axis, hi <= lo, too many cells,
-                           non-finite or out-of-box position on a bounded axis (detected on device, reported by
-                           the next synchronising call or sph_check) */
+                           non-finite or out-of-box position on a bounded axis, h or rho not a positive finite
+                           number, non-finite mass (detected on device in a sticky flag that sph_build_cells
+                           clears; reported by sph_neighbors, the *_host calls and sph_check) */
     SPH_E_STATE = -3,   /* call order violated (neighbours before cells, RHS before neighbours, different n) */
     SPH_E_NOMEM = -4,   /* device or host allocation failed */
     SPH_E_CUDA = -5     /* a CUDA runtime call failed */

@@ -139,7 +139,7 @@ extern "C" int sph_forward_backward_host(sph_ctx *ctx, const sph_domain *dom, co
     if (rho_bar) SPH_CUDA_TRY(cudaMemcpyAsync(rho_bar, ctx->ho_rb.p, ns, cudaMemcpyDeviceToHost, st));
     if (params_bar) SPH_CUDA_TRY(cudaMemcpyAsync(params_bar, ctx->ho_pb.p, 40, cudaMemcpyDeviceToHost, st));
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
-    return SPH_OK;
+    return sph_check(ctx);
 }
 
 extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_domain *dom_rk, const sph_params *par,
@@ -183,6 +183,11 @@ extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_doma
     SPH_CUDA_TRY(cudaMemcpyAsync(ctx->hmu.p, acc_bar, nv, cudaMemcpyHostToDevice, cs));
     SPH_CUDA_TRY(cudaEventRecord(ctx->ev_in, cs));
     int64_t nnz0 = 0;
+    // whatever path leaves this function, a later sph_rk_step must not take lists prepared here for its own
+    struct PreparedGuard {
+        sph_ctx *c;
+        ~PreparedGuard() { c->rk_lists_prepared = false; c->rk_final_chunks = 1; }
+    } prepared_guard{ctx};
     SPH_TRY(sph_build_cells(ctx, dom, dx, dh, n, ss));
     SPH_TRY(sph_neighbors(ctx, 1.0f, &nnz0, ss));
     SPH_CUDA_TRY(cudaStreamWaitEvent(st, ctx->ev_in, 0));
@@ -208,8 +213,6 @@ extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_doma
         if (!ctx->ev_final[c]) SPH_CUDA_TRY(cudaEventCreateWithFlags(&ctx->ev_final[c], cudaEventDisableTiming));
     ctx->rk_final_chunks = kFinalChunks;
     const int rc_rk = sph_rk_step(ctx, dom_rk, par, dt, skin, n, dx, dv, dr, dm, dh, dk, ss);
-    ctx->rk_final_chunks = 1;
-    ctx->rk_lists_prepared = false;
     SPH_TRY(rc_rk);
     if (nnz_out) {
         nnz_out[0] = nnz0;
@@ -226,7 +229,7 @@ extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_doma
     }
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
     SPH_CUDA_TRY(cudaStreamSynchronize(cs));
-    return SPH_OK;
+    return sph_check(ctx);
 }
 
 // ------------------------------------------------------------------------------------------ profiling

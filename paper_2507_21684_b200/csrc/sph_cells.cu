@@ -245,6 +245,7 @@ __global__ void k_max_displacement(const float *__restrict__ x, const float *__r
         const float4 b = pos_s[inv_perm[i]];
         const float xb[3] = {b.x, b.y, b.z};
         float r2 = 0.f;
+        bool outside = false;
         for (int k = 0; k < gg.dim; ++k) {
             float xv = x[i * gg.dim + k];
             float d;
@@ -253,10 +254,13 @@ __global__ void k_max_displacement(const float *__restrict__ x, const float *__r
                 d = d > 0.5f * gg.L[k] ? d - gg.L[k] : (d < -0.5f * gg.L[k] ? d + gg.L[k] : d);
             } else {
                 d = xv - xb[k];
+                if (!(xv >= gg.lo[k] && xv <= gg.hi[k])) outside = true;
             }
             r2 = fmaf(d, d, r2);
         }
         r = sqrtf(r2);
+        // left a bounded axis: never valid, so the caller rebuilds and sph_build_cells reports SPH_E_DOMAIN
+        if (outside) r = __uint_as_float(0x7f800000u);
         if (!(r >= 0.f)) r = __uint_as_float(0x7f800000u);        // NaN position: never valid
         if (h && h[i] != b.w) r = __uint_as_float(0x7f800000u);   // the lists were built for another h: never valid
     }

@@ -199,7 +199,17 @@ struct sph_ctx {
 // device flag pair of the uniform-mass fast path: [0] non-zero = all masses of the last pack equal, [1] = that mass
 // (float bits).  Written on the stream by the pack kernels (k_pack_state, k_rk_base), read by the pair kernels: the
 // host never needs to know -- both variants of a pair kernel are launched and the one whose turn it is not returns.
-inline uint32_t *sph_um_flag(const sph_ctx *ctx) { return ctx->stats.as<uint32_t>() + 13; }
+constexpr int kUmSlot = 13;
+inline uint32_t *sph_um_flag(const sph_ctx *ctx) { return ctx->stats.as<uint32_t>() + kUmSlot; }
+#ifdef __CUDACC__
+// Pack kernels: a density that is not a positive finite number, or a mass that is not finite, raises bit 4 of the
+// sticky device error flag (stats[0], the word k_wrap_key uses for positions and h; `um` points kUmSlot words past it).
+// Reported as SPH_E_DOMAIN by the next synchronising call or sph_check.
+__device__ __forceinline__ void sph_flag_bad_state(uint32_t *um, float rho, float m)
+{
+    if (!(rho > 0.f && rho <= 3.402823466e38f) || !(fabsf(m) <= 3.402823466e38f)) atomicOr(um - kUmSlot, 4u);
+}
+#endif
 
 // Counts `nlaunch` kernel launches of class `cls` and, when profiling is on, brackets them with events on `st`.
 struct KScope {

@@ -107,6 +107,7 @@ __global__ void k_pack_state(int64_t n, KPar kp, const uint32_t *__restrict__ pe
     }
     const float r = rho[i], mi = m[i], h = pb.w;
     if (mi != m_first) um[0] = 0u;
+    sph_flag_bad_state(um, r, mi);
     const float u = (r - kp.rho0) / kp.rho0;
     const float lg = log1pf(u);
     const float ugm1 = expm1f(kp.gamma * lg);        // (rho/rho0)^gamma - 1

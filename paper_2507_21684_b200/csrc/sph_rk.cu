@@ -83,6 +83,7 @@ __global__ void k_rk_base(int64_t n, KPar kp, const uint32_t *__restrict__ perm,
     }
     const float r = rho[i], mi = m[i];
     if (mi != m_first) um[0] = 0u;
+    sph_flag_bad_state(um, r, mi);
     b0[p] = make_float4(X[0], X[1], X[2], ps.w);
     b1[p] = make_float4(Vv[0], Vv[1], Vv[2], r);
     m_s[p] = mi;
@@ -287,12 +288,14 @@ extern "C" int sph_rk_step(sph_ctx *ctx, const sph_domain *dom, const sph_params
                            float *x, float *v, float *rho, const float *m, const float *h, const uint8_t *kind,
                            sph_stream_t stream)
 {
-    if (!ctx || !dom || !par || !x || !v || !rho || !m || !h || !kind || !(skin >= 0.f)) return SPH_E_INVALID;
+    if (!ctx) return SPH_E_INVALID;
+    const bool prepared = ctx->rk_lists_prepared;                    // built by sph_rk_prepare_lists for this call
+    ctx->rk_lists_prepared = false;
+    if (!dom || !par || !x || !v || !rho || !m || !h || !kind || !(skin >= 0.f)) return SPH_E_INVALID;
     if (n <= 0) return SPH_E_INVALID;
     SPH_CUDA_TRY(cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
-    if (ctx->rk_lists_prepared) ctx->rk_lists_prepared = false;     // built by sph_rk_prepare_lists for this call
-    else SPH_TRY(rebuild(ctx, dom, skin, x, h, n, st));
+    if (!prepared || !ctx->lists_ready || ctx->n != n) SPH_TRY(rebuild(ctx, dom, skin, x, h, n, st));
     KPar kp;
     SPH_TRY(sph_kpar_make(ctx, par, &kp));
     SPH_TRY(ctx->s0.reserve((size_t)n * 16));

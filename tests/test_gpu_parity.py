@@ -160,6 +160,45 @@ def test_error_codes(sph):
     with pytest.raises(SphError) as e:
         sph.rhs(par, dev.x, dev.v, dev.rho, dev.m, dev.kind)
     assert e.value.code == -1
+    # a density that is not a positive finite number (or a non-finite mass) raises the device flag in the pack kernel
+    for bad_rho in (0.0, -1.0, float("nan"), float("inf")):
+        sph.build_cells(wl.domain, dev.x, dev.h)
+        sph.neighbors(1.0)
+        sph.check()
+        rb = dev.rho.clone()
+        rb[11] = bad_rho
+        sph.rhs(wl.params, dev.x, dev.v, rb, dev.m, dev.kind)
+        with pytest.raises(SphError) as e:
+            sph.check()
+        assert e.value.code == -2
+    # h <= 0 or non-finite
+    for bad_h in (0.0, -0.1, float("nan")):
+        hb = dev.h.clone()
+        hb[3] = bad_h
+        sph.build_cells(wl.domain, dev.x, hb)
+        with pytest.raises(SphError) as e:
+            sph.neighbors(1.0)
+        assert e.value.code == -2
+
+
+def test_verlet_reuse_rejects_positions_outside_a_bounded_axis(sph):
+    """sph_lists_valid never calls lists valid once a particle has left a bounded axis: the RK4 step then rebuilds, and
+    the rebuild reports the position (SPH_E_DOMAIN) instead of integrating on stale lists"""
+    wl = W.make(2, dx=0.05)                      # C2 (2D, bounded in y)
+    dev = Dev(wl)
+    dom = W.rk_domain(wl, 0.2)
+    x, v, rho = dev.x.clone(), dev.v.clone(), dev.rho.clone()
+    sph.rk_step(dom, wl.params, 0.0, 0.2, x, v, rho, dev.m, dev.h, dev.kind)
+    ok, _ = sph.lists_valid(x, 0.2)
+    assert ok
+    bounded = [k for k in range(wl.domain.dim) if not wl.domain.periodic[k]]
+    assert bounded
+    x[5, bounded[0]] = wl.domain.hi[bounded[0]] + 1e-3         # a tiny move, far below the skin, but out of the box
+    ok, D = sph.lists_valid(x, 0.2)
+    assert not ok and D == float("inf")
+    with pytest.raises(SphError) as e:
+        sph.rk_step(dom, wl.params, 0.0, 0.2, x, v, rho, dev.m, dev.h, dev.kind)
+    assert e.value.code == -2
 
 
 # ------------------------------------------------------------------------------------------ density / RHS / VJP
