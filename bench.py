@@ -252,7 +252,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
-                    help="sph_set_option before the run (integer keys of include/sph.h, e.g. 9=0: rows in stored order); "
+                    help="sph_set_option before the run (integer keys of include/sph.h, e.g. 9=1: bulk-copy staging of the halo); "
                          "repeatable.  For A/B measurements: the line records it in config.options")
     ap.add_argument("--ref-rows", type=int, default=100000)
     ap.add_argument("--cpu-budget", type=float, default=12.0)

@@ -214,6 +214,11 @@ int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_domain *dom_rk,
 
 /* Fetch the device-side error flag (synchronises the context's last stream). */
 int sph_check(sph_ctx *ctx);
+/* Debug builds only (python -m paper_2507_21684_b200.build --bounds, -DSPH_BOUNDS: every shared-memory gather index,
+ * ring offset and staging offset of the tile kernels is a checked access).  *count (host) = violations seen since the
+ * library was loaded (the first 16 also print their source line); -1 when the library is not a debug build.
+ * Synchronises the device. */
+int sph_debug_bounds_violations(sph_ctx *ctx, int64_t *count);
 const char *sph_strerror(int code);
 
 /* Introspection for tests / bench (host values of the last build): grid size per axis, nnz, number of kernels
@@ -265,6 +270,9 @@ enum {
                                instead of 40 / 56 bytes per pair, one general -- and a device flag written by this
                                call's own pack kernel decides which of them runs (no host synchronisation);
                                0: only the general variant is launched */
+    SPH_OPT_STAGE_BULK = 9, /* 0 (default): the tile pair kernels stage a halo with one 16-byte cp.async per particle and
+                               array; 1: sph_rhs / sph_rhs_vjp stage their float4 arrays with one cp.async.bulk per halo
+                               cell and array, completing on one mbarrier per CTA (A/B measurement) */
     SPH_OPT_RK_EXTRA_SKIN = 6 /* Verlet lists across steps: value/1000 = extra skin e (in units of h).  With
                                e > 0 sph_rk_step / sph_rk_step_vjp build their lists with search_scale = 1 + skin + e
                                (the domain's cell_size must cover it) and a later call with the same domain, n and h

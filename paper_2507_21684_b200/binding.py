@@ -18,12 +18,12 @@ LIB_PATH = os.path.join(HERE, "libsph_b200.so")
 EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph_neighbors_export", "sph_density",
            "sph_density_vjp", "sph_lists_valid", "sph_grad_sum", "sph_grad_sum_vjp", "sph_renorm_gradient", "sph_renorm_gradient_vjp",
            "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
-           "sph_check", "sph_strerror", "sph_get_info", "sph_get_layout", "sph_profile_enable", "sph_profile_read",
+           "sph_check", "sph_debug_bounds_violations", "sph_strerror", "sph_get_info", "sph_get_layout", "sph_profile_enable", "sph_profile_read",
            "sph_set_option", "sph_shift")
 
 # keys of sph_set_option (enum SPH_OPT_* in include/sph.h)
 OPT_PAIR_GROUP, OPT_LIST_MODE, OPT_TILE_EDGE, OPT_PAIR_WARPS, OPT_FILL_MASKS, OPT_RK_EXTRA_SKIN = 1, 2, 3, 4, 5, 6
-OPT_UNIFORM_MASS_PATH, OPT_BUILD_FUSED = 7, 8
+OPT_UNIFORM_MASS_PATH, OPT_BUILD_FUSED, OPT_STAGE_BULK = 7, 8, 9
 LIST_AUTO, LIST_GENERIC, LIST_TILE = 0, 1, 2
 
 # kernel classes of sph_profile_read (enum SPH_K_* in include/sph.h)
@@ -86,6 +86,7 @@ def load_library(path: str = LIB_PATH):
     lib.sph_set_option.argtypes = [vp, C.c_int, C.c_int]
     lib.sph_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
     lib.sph_check.argtypes = [vp]
+    lib.sph_debug_bounds_violations.argtypes = [vp, C.POINTER(C.c_int64)]
     lib.sph_strerror.argtypes = [C.c_int]
     lib.sph_strerror.restype = C.c_char_p
     lib.sph_get_info.argtypes = [vp, C.POINTER(C.c_int32 * 3), C.POINTER(i64), C.POINTER(i64), C.POINTER(i64)]
@@ -355,6 +356,12 @@ class Sph:
 
     def check(self):
         self._chk(self.lib.sph_check(self._ctx))
+
+    def debug_bounds_violations(self) -> int:
+        """violations counted by a --bounds debug build of the library; -1 for a normal build"""
+        c = C.c_int64(0)
+        self._chk(self.lib.sph_debug_bounds_violations(self._ctx, C.byref(c)))
+        return int(c.value)
 
     def layout(self):
         """layout of the lists of the last neighbors(): mode 1 generic / 2 tile-local, tile edge, largest halo / rows"""

@@ -66,6 +66,24 @@ extern "C" int sph_check(sph_ctx *ctx)
     return flag ? SPH_E_DOMAIN : SPH_OK;
 }
 
+#ifdef SPH_BOUNDS
+unsigned int sph_bounds_read_fused();
+unsigned int sph_bounds_read_pairs_tile();
+#endif
+// violations counted by the checked accesses of a -DSPH_BOUNDS build since the library was loaded; -1 in a normal build
+extern "C" int sph_debug_bounds_violations(sph_ctx *ctx, int64_t *count)
+{
+    if (!ctx || !count) return SPH_E_INVALID;
+#ifdef SPH_BOUNDS
+    SPH_CUDA_TRY(cudaSetDevice(ctx->device));
+    SPH_CUDA_TRY(cudaDeviceSynchronize());
+    *count = (int64_t)sph_bounds_read_fused() + (int64_t)sph_bounds_read_pairs_tile();
+#else
+    *count = -1;
+#endif
+    return SPH_OK;
+}
+
 extern "C" const char *sph_strerror(int code)
 {
     switch (code) {
@@ -293,6 +311,9 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
         return SPH_OK;
     case SPH_OPT_BUILD_FUSED:
         ctx->opt_build_fused = value != 0;
+        return SPH_OK;
+    case SPH_OPT_STAGE_BULK:
+        ctx->opt_stage_bulk = value != 0;
         return SPH_OK;
     case SPH_OPT_UNIFORM_MASS_PATH:
         ctx->opt_no_um = value == 0;

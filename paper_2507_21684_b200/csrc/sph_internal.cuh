@@ -136,6 +136,7 @@ struct sph_ctx {
     int opt_tile_edge = 0;      // 0 auto, else force the tile edge B (1, 2, 4)
     int opt_fused_warps = 0;    // warps per CTA of the one-kernel build (0 = default)
     int opt_build_fused = 1;    // 1: the tile-local lists are built by the one-kernel build (sph_neighbors_fused.cu) when a tile fits it
+    int opt_stage_bulk = 0;     // 1: k_rhs_tile / k_vjp_tile stage their float4 halo arrays with cp.async.bulk + one mbarrier (measured: profiles/r02_f)
     int opt_no_um = 0;          // 1: never launch the uniform-mass variants of the tile pair kernels (A/B measurements, tests)
     bool tile_mode = false;     // lists of the last sph_neighbors are tile-local (col16)
     TileGeom tg{};

@@ -243,6 +243,7 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
             pj.x = rel_coord(pj.x, sh[0], org[0]);
             pj.y = rel_coord(pj.y, sh[1], org[1]);
             if (DIM == 3) pj.z = rel_coord(pj.z, sh[2], org[2]);
+            SPH_ASSERT(q < (uint32_t)fs.mcap);
             sm.cand[q] = pj;
         }
     }
@@ -253,10 +254,12 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
         uint16_t *cm = sm.cmap + (size_t)tc * ncap;
         uint32_t g = 0;
         for_each_run<DIM>(tt, sl, [&](uint32_t q0, uint32_t q1) {
+            SPH_ASSERT(g + (q1 - q0) <= (uint32_t)ncap && q1 <= (uint32_t)fs.mcap);
             for (uint32_t i = lane; i < q1 - q0; i += 32) cm[g + i] = (uint16_t)(q0 + i);
             g += q1 - q0;
         });
         const uint32_t gpad = (g + kCandBlock - 1) / kCandBlock * kCandBlock;
+        SPH_ASSERT(gpad <= (uint32_t)ncap);
         for (uint32_t i = g + lane; i < gpad; i += 32) cm[i] = (uint16_t)kQNone;
         if (lane == 0) c_nc[tc] = g;
     }
@@ -324,7 +327,9 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
                     uint32_t rb[kCPL], rb2[kCPL], qk[kCPL];
 #pragma unroll
                     for (int k = 0; k < kCPL; ++k) {
+                        SPH_ASSERT(cb * kCandBlock + k * 32 + lane < (uint32_t)ncap);
                         qk[k] = cm[cb * kCandBlock + k * 32 + lane];
+                        SPH_ASSERT(qk[k] == kQNone || qk[k] < (uint32_t)fs.mcap);
                         float4 pj = make_float4(1.0e18f, 1.0e18f, DIM == 3 ? 1.0e18f : 0.f, 0.f);   // padding: never a hit
                         if (qk[k] != kQNone) pj = sm.cand[qk[k]];
                         nx[k] = make_float2(-pj.x, -pj.x);
@@ -415,6 +420,7 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
                     for (int k = 0; k < kCPL; ++k) {
                         const uint32_t w = cb * kCPL + k;
                         if (w * 32u >= Nc) continue;                       // uniform: no valid candidate in this word
+                        SPH_ASSERT(w < (uint32_t)(ncap / 32) && row_base + nr <= (uint32_t)tcap);
                         uint32_t *mw = sm.masks + (size_t)w * tcap + row_base;
                         const uint32_t y = warp_transpose32(rb[k]);
                         if (islot >= 0 && (uint32_t)islot < nr1) mw[islot] = y;
@@ -496,6 +502,7 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
     constexpr uint32_t kGR = 32 / kRowLanes;                     // rows of a group
     const uint32_t wcap = (((uint32_t)fs.scap + 8u) / (uint32_t)kFW - 8u) & ~7u;   // entries of a warp's image (+ 8 of slack)
     uint16_t *wst = sm.stage + (size_t)warp * (wcap + 8u);
+    SPH_ASSERT((size_t)kFW * (wcap + 8u) <= (size_t)fs.scap + 8u);
     const uint32_t mstride = (uint32_t)tcap * 4u;
     const uint32_t ngroups = (T + kGR - 1u) / kGR;
     long long base = -1;
@@ -553,6 +560,7 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
                         : "memory");
                 if (__all_sync(0xffffffffu, m == 0u && maddr == mend && pend == 0u)) break;
             }
+            SPH_ASSERT(daddr <= (uint32_t)__cvta_generic_to_shared(wst + 8u + wcap));        // the warp's image was not overrun
         }
         if (base < 0) {                                          // first group of this warp: the base may still be on its way
             while (s_ready == 0u) __nanosleep(200);           // leave the issue slots to the warps that still expand
@@ -603,6 +611,7 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
                 while (m) {
                     const int hb = 31 - __clz(m);
                     m ^= 1u << hb;
+                    SPH_ASSERT(32u * w + 31u - (uint32_t)hb < (uint32_t)ncap);
                     dst[k++] = cm[32u * w + 31u - (uint32_t)hb];
                 }
             }
@@ -808,3 +817,12 @@ int sph_neighbors_fused_run(sph_ctx *ctx, const SearchPar &sp, const TileGeom &t
     if (nnz_out) *nnz_out = nnz;
     return SPH_OK;
 }
+
+#ifdef SPH_BOUNDS
+unsigned int sph_bounds_read_fused()
+{
+    unsigned int v = 0;
+    cudaMemcpyFromSymbol(&v, sph_bounds_count, sizeof(v));
+    return v;
+}
+#endif

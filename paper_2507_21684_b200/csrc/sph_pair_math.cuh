@@ -1,8 +1,30 @@
-// sph_pair_math.cuh -- H-dependent constants of the Wendland C4 pair terms (Eq.25-29), shared by the
+// sph_pair_math.cuh -- particle record and H-dependent constants of the Wendland C4 pair terms (Eq.25-29), shared by the
 // global-gather pair kernels (sph_pairs.cu) and the tile kernels (sph_pairs_tile.cu).
 #pragma once
 
 #include "sph_internal.cuh"
+
+// Sorted state of one particle as the pair loops see it, and the record layout both kernel families read it from:
+// DIM 3: s0 = {x,y,z,rho}  s1 = {vx,vy,vz,P}  s2 (float2) = {V,h};   DIM 2: s0 = {x,y,vx,vy}  s1 = {rho,V,P,h}.
+// In 3D everything a pair needs when mass and h are uniform sits in s0, s1 (the uniform-mass tile kernels leave s2 out
+// and pass V = m0 / rho, h = H instead).
+struct Part {
+    float x[3], v[3], rho, V, P, h;
+};
+template <int DIM>
+static __device__ __forceinline__ Part part_unpack(const float4 &a, const float4 &b, float V3 = 0.f, float h3 = 0.f)
+{
+    Part p;
+    if (DIM == 3) {
+        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.rho = a.w;
+        p.v[0] = b.x; p.v[1] = b.y; p.v[2] = b.z; p.P = b.w;
+        p.V = V3; p.h = h3;
+    } else {
+        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = 0.f; p.v[0] = a.z; p.v[1] = a.w; p.v[2] = 0.f;
+        p.rho = b.x; p.V = b.y; p.P = b.z; p.h = b.w;
+    }
+    return p;
+}
 
 // H-dependent constants of one pair (or of the whole launch when h is uniform)
 struct HC {

@@ -14,29 +14,17 @@ namespace {
 constexpr int kBlock = 256;          // threads per block
 constexpr int kRowsPerGroup = 8;     // rows each lane group walks through
 
-// sorted state of one particle as the pair loops see it
-struct Part {
-    float x[3], v[3], rho, V, P, h;
-};
-
-// layouts: DIM 3: s0 = {x,y,z,rho} s1 = {vx,vy,vz,P} s2(float2) = {V,h};  DIM 2: s0 = {x,y,vx,vy} s1 = {rho,V,P,h}
-// (3D: everything a pair needs when mass and h are uniform sits in s0, s1 -- the tile kernels then leave s2 out)
+// global-memory load of a particle record (layout: sph_pair_math.cuh)
 template <int DIM>
 __device__ __forceinline__ Part load_part(const float4 *__restrict__ s0, const float4 *__restrict__ s1,
                                           const float2 *__restrict__ s2, int64_t j)
 {
-    Part p;
-    float4 a = __ldg(s0 + j), b = __ldg(s1 + j);
+    const float4 a = __ldg(s0 + j), b = __ldg(s1 + j);
     if (DIM == 3) {
-        float2 c = __ldg(s2 + j);
-        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.rho = a.w;
-        p.v[0] = b.x; p.v[1] = b.y; p.v[2] = b.z; p.P = b.w;
-        p.V = c.x; p.h = c.y;
-    } else {
-        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = 0.f; p.v[0] = a.z; p.v[1] = a.w; p.v[2] = 0.f;
-        p.rho = b.x; p.V = b.y; p.P = b.z; p.h = b.w;
+        const float2 c = __ldg(s2 + j);
+        return part_unpack<3>(a, b, c.x, c.y);
     }
-    return p;
+    return part_unpack<DIM>(a, b);
 }
 
 template <int DIM, bool WRAP>

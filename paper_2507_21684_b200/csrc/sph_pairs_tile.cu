@@ -45,15 +45,59 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// Bulk-copy staging (SPH_OPT_STAGE_BULK, include/sph.h): one cp.async.bulk per halo cell and float4 array instead of one
+// 16-byte cp.async per particle, all completing on one mbarrier of the CTA (a tile is staged once, so phase 0 only).
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile("{\n"
+                 ".reg .pred p;\n"
+                 "SPH_MBAR_WAIT:\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                 "@p bra SPH_MBAR_DONE;\n"
+                 "bra SPH_MBAR_WAIT;\n"
+                 "SPH_MBAR_DONE:\n"
+                 "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+                 : "memory");
+}
+
 // Copies the halo of the tile (every halo cell is one contiguous run of the sorted arrays) into shared memory with
 // cp.async: no registers, every copy of the CTA in flight at once.  Null sources are skipped (compile time).
 __device__ __forceinline__ void stage_halo(const TileTab &tt, const float4 *__restrict__ g0, float4 *d0,
                                            const float4 *__restrict__ g1, float4 *d1, const float4 *__restrict__ g2,
                                            float4 *d2, const float2 *__restrict__ gc, float2 *dc,
-                                           const float *__restrict__ gf, float *df)
+                                           const float *__restrict__ gf, float *df, uint64_t *bar = nullptr)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const uint32_t a0 = smem_u32(d0), a1 = smem_u32(d1), a2 = smem_u32(d2), ac = smem_u32(dc), af = smem_u32(df);
+    if (bar) {
+        // the float4 arrays by bulk copies (runs are 16-byte aligned multiples of 16 bytes by construction); the caller has
+        // initialised the barrier (count 1) and synchronised.  The float2 / float arrays below stay per-particle copies.
+        if (threadIdx.x == 0) mbar_expect_tx(bar, (uint32_t)tt.M * 16u * ((g0 ? 1u : 0u) + (g1 ? 1u : 0u) + (g2 ? 1u : 0u)));
+        for (int hc = threadIdx.x; hc < tt.nh; hc += blockDim.x) {
+            const uint32_t o0 = tt.h_off[hc], cnt = tt.h_off[hc + 1] - o0, gs = tt.h_start[hc];
+            if (cnt == 0) continue;
+            if (g0) bulk_g2s(a0 + o0 * 16, g0 + gs, cnt * 16, bar);
+            if (g1) bulk_g2s(a1 + o0 * 16, g1 + gs, cnt * 16, bar);
+            if (g2) bulk_g2s(a2 + o0 * 16, g2 + gs, cnt * 16, bar);
+        }
+        g0 = nullptr; g1 = nullptr; g2 = nullptr;
+        if (!gc && !gf) return;
+    }
     for (int hc = warp; hc < tt.nh; hc += nwarps) {
         const uint32_t o0 = tt.h_off[hc], cnt = tt.h_off[hc + 1] - o0, gs = tt.h_start[hc];
         for (uint32_t l = lane; l < cnt; l += 32) {
@@ -155,40 +199,27 @@ __device__ __forceinline__ void tile_row_passes(const TileTab &tt, const uint32_
     cp_async_wait<0>();
 }
 
-// sorted state of one particle as the pair loops see it
-// layouts: DIM 3: s0 = {x,y,z,rho} s1 = {vx,vy,vz,P} s2(float2) = {V,h};  DIM 2: s0 = {x,y,vx,vy} s1 = {rho,V,P,h}
+// shared-memory load of a particle record (layout: sph_pair_math.cuh)
 // UM (3D, uniform mass m0 and uniform h): s2 is not staged at all -- V = m0/rho costs one MUFU and one multiply against
 // a third gather with its bank conflicts (the shared-memory data pipe is the binding unit, profiles/r01_g)
-struct Part {
-    float x[3], v[3], rho, V, P, h;
-};
 template <int DIM, bool UM = false>
 __device__ __forceinline__ Part load_part(const float4 *s0, const float4 *s1, const float2 *s2, uint32_t j, float m0 = 0.f,
                                           float H = 0.f)
 {
-    Part p;
     const float4 a = s0[j], b = s1[j];
     if (DIM == 3) {
-        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = a.z; p.rho = a.w;
-        p.v[0] = b.x; p.v[1] = b.y; p.v[2] = b.z; p.P = b.w;
-        if (UM) {
-            p.V = m0 * fast_rcp(a.w);
-            p.h = H;
-        } else {
-            const float2 c = s2[j];
-            p.V = c.x; p.h = c.y;
-        }
-    } else {
-        p.x[0] = a.x; p.x[1] = a.y; p.x[2] = 0.f; p.v[0] = a.z; p.v[1] = a.w; p.v[2] = 0.f;
-        p.rho = b.x; p.V = b.y; p.P = b.z; p.h = b.w;
+        if (UM) return part_unpack<3>(a, b, m0 * fast_rcp(a.w), H);
+        const float2 c = s2[j];
+        return part_unpack<3>(a, b, c.x, c.y);
     }
-    return p;
+    return part_unpack<DIM>(a, b);
 }
 
 // shared-memory carve-up: A, B (float4[mcap]), [cot float4[mcap]], C (float2[mcap], 3D only), rp[tcap+1],
 // selfq[tcap], index ring [nwarps][2][rb]
 struct TileSizes {
     int mcap, tcap, rb;
+    int bulk;            // SPH_OPT_STAGE_BULK: k_rhs_tile / k_vjp_tile stage their float4 arrays with cp.async.bulk
 };
 template <int DIM>
 struct SmemMap {
@@ -578,9 +609,16 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
     __shared__ TileTab tt;
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
     if (tt.T == 0) return;
-    stage_halo(tt, s0, sm.A, s1, sm.B, nullptr, nullptr, (DIM == 3 && !UM) ? s2 : nullptr, sm.C, nullptr, nullptr);
+    __shared__ uint64_t mbar;
+    if (ts.bulk) {
+        if (threadIdx.x == 0) mbar_init(&mbar, 1);
+        __syncthreads();
+    }
+    stage_halo(tt, s0, sm.A, s1, sm.B, nullptr, nullptr, (DIM == 3 && !UM) ? s2 : nullptr, sm.C, nullptr, nullptr,
+               ts.bulk ? &mbar : nullptr);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
     cp_async_wait<0>();
+    if (ts.bulk) mbar_wait(&mbar, 0);
     __syncthreads();
     stage_shift<DIM>(tt, sm.A);
     const int gl = (threadIdx.x & 31) % GS;
@@ -698,9 +736,16 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
         if (threadIdx.x < kNPartT) partials[(int64_t)blockIdx.x * kNPartT + threadIdx.x] = 0.f;
         return;
     }
-    stage_halo(tt, s0, sm.A, s1, sm.B, cot, sm.cot, (DIM == 3 && !UM) ? s2 : nullptr, sm.C, nullptr, nullptr);
+    __shared__ uint64_t mbar;
+    if (ts.bulk) {
+        if (threadIdx.x == 0) mbar_init(&mbar, 1);
+        __syncthreads();
+    }
+    stage_halo(tt, s0, sm.A, s1, sm.B, cot, sm.cot, (DIM == 3 && !UM) ? s2 : nullptr, sm.C, nullptr, nullptr,
+               ts.bulk ? &mbar : nullptr);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
     cp_async_wait<0>();
+    if (ts.bulk) mbar_wait(&mbar, 0);
     __syncthreads();
     stage_shift<DIM>(tt, sm.A);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gl = lane % GS;
@@ -1023,6 +1068,7 @@ static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, size_t 
     rb = (rb + 7) & ~7;
     if (rb < 64) rb = 64;
     ts->rb = rb;
+    ts->bulk = ctx->opt_stage_bulk;
     const size_t fixed = (size_t)ts->mcap * state_bytes + (size_t)(ts->tcap + 4) * 4 + (size_t)ts->tcap * 2 + 16;
     const size_t sm_total = 233472, per_cta = 1024 + static_smem, cta_max = 232448 - static_smem;
     auto need = [&](int warps) { return fixed + (size_t)warps * 2 * rb * 2; };
@@ -1384,3 +1430,12 @@ int sph_launch_delta_term_tile(sph_ctx *ctx, const KPar &kp, const float4 *pos4,
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }
+
+#ifdef SPH_BOUNDS
+unsigned int sph_bounds_read_pairs_tile()
+{
+    unsigned int v = 0;
+    cudaMemcpyFromSymbol(&v, sph_bounds_count, sizeof(v));
+    return v;
+}
+#endif

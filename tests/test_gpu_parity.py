@@ -54,7 +54,7 @@ def _np(t):
 
 # every test runs on both list layouts of the library (include/sph.h, SPH_OPT_LIST_MODE): "tile" = automatic choice
 # (tile-local 16-bit lists + shared-memory halo kernels wherever a halo fits), "generic" = 32-bit lists + global
-# gathers, "tile_b1" = tile-local lists on single-cell blocks
+# gathers, "tile_b1" = tile-local lists on single-cell blocks with the round-1 three-kernel build (count / scan / fill)
 @pytest.fixture(scope="module", params=["tile", "generic", "tile_b1"])
 def sph(request):
     s = Sph(0)
@@ -66,7 +66,10 @@ def sph(request):
         s.set_option(OPT_BUILD_FUSED, 0)
         s.set_option(OPT_FILL_MASKS, 0)          # this variant also covers the fill that repeats the distance tests
     yield s
+    # a -DSPH_BOUNDS debug build of the library counts out-of-range shared-memory accesses; a normal build reports -1
+    bad = s.debug_bounds_violations()
     s.close()
+    assert bad <= 0, f"{bad} checked shared-memory accesses were out of range (SPH_BOUNDS build)"
 
 
 def test_layout_is_the_requested_one(sph):
@@ -386,6 +389,28 @@ def test_uniform_mass_variant_and_general_variant_agree(sph):
                 assert _params_err(_np(pb), po) < TOL_VJP
             finally:
                 sph.set_option(OPT_UNIFORM_MASS_PATH, 1)
+
+
+@pytest.mark.parametrize("case", ["C1s", "C2p", "C3p", "C4s"])
+def test_bulk_copy_staging_is_bitwise_the_same(sph, case):
+    """SPH_OPT_STAGE_BULK: the halo of a tile staged with cp.async.bulk + one mbarrier instead of per-particle cp.async
+    (include/sph.h).  The staged bytes are the same, so RHS and VJP must agree bit for bit with the default path."""
+    from paper_2507_21684_b200.binding import OPT_STAGE_BULK
+    wl = CASES[case]()
+    lam, mu = W.random_cotangents(wl)
+    _, dev, _ = build(wl, 1.0, sph)
+    lam_d, mu_d = torch.from_numpy(lam).cuda(), torch.from_numpy(mu).cuda()
+    out = []
+    for bulk in (0, 1):
+        sph.set_option(OPT_STAGE_BULK, bulk)
+        try:
+            drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+            xb, vb, rb, pb = sph.rhs_vjp(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind, lam_d, mu_d)
+            out.append([_np(t).copy() for t in (drho, acc, xb, vb, rb, pb)])
+        finally:
+            sph.set_option(OPT_STAGE_BULK, 0)
+    for a, b in zip(*out):
+        assert np.array_equal(a, b)
 
 
 @pytest.mark.parametrize("case", ["C0p", "C2p", "C3p", "C4s"])
