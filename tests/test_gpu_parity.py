@@ -204,6 +204,38 @@ def test_verlet_reuse_rejects_positions_outside_a_bounded_axis(sph):
     assert e.value.code == -2
 
 
+@pytest.mark.parametrize("case", ["C1s", "C3p", "C4s"])
+def test_slab_decomposition_on_one_rank_matches_the_plain_call(sph, case):
+    """paper_2507_21684_b200.sharded with world size 1: the only neighbour of the slab is the slab itself, so the ghosts
+    are its own periodic images (shifted by -+L) and the local problem is bounded along the cut axis.  Through the CUDA
+    kernels this must reproduce the plain periodic call up to the binary32 rounding of the shifted positions (the
+    2- and 3-rank bookkeeping is covered on CPU, tests/test_multirank_cpu.py)."""
+    from paper_2507_21684_b200.sharded import ShardedSph, CudaSolver
+    wl = CASES[case]()
+    lam, mu = W.random_cotangents(wl)
+    _, dev, _ = build(wl, 1.0, sph)
+    lam_d, mu_d = torch.from_numpy(lam).cuda(), torch.from_numpy(mu).cuda()
+    dens0 = sph.density(dev.m).clone()
+    drho0, acc0 = (t.clone() for t in sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind))
+    xb0, vb0, rb0, pb0 = (t.clone() for t in sph.rhs_vjp(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind, lam_d, mu_d))
+    solver = CudaSolver(0)
+    try:
+        sh = ShardedSph(wl.domain, float(wl.domain.cell_size), solver)
+        assert sh.world == 1 and sum(sh.plan(dev.x)) > 0
+        dens = sh.density(dev.x, dev.m, dev.h)
+        drho, acc = sh.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.h, dev.kind)
+        xb, vb, rb, pb = sh.rhs_vjp(wl.params, lam_d, mu_d)
+        lists = oracle_lists(wl)
+        _, _, sd, sa = oracle.rhs(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *lists, with_scales=True)
+        for got, ref, scale in ((dens, dens0, None), (drho, drho0, float(sd.max())), (acc, acc0, float(sa.max())),
+                                (xb, xb0, None), (vb, vb0, None), (rb, rb0, None)):
+            scale = float(ref.abs().max()) if scale is None else scale
+            assert float((got - ref).abs().max()) / scale < 1e-5
+        assert _params_err(_np(pb), _np(pb0).astype(np.float64)) < 1e-4
+    finally:
+        solver.close()
+
+
 # ------------------------------------------------------------------------------------------ density / RHS / VJP
 @pytest.mark.parametrize("case", list(CASES))
 def test_density_parity(sph, case):
