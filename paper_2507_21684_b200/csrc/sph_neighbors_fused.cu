@@ -38,6 +38,7 @@ struct FusedSizes {
     int mcap;            // halo particles (multiple of 8)
     int tcap;            // rows of a tile
     int ncap;            // candidates of one target cell, multiple of kCandBlock
+    int wcap;            // mask words of a row = ceil(most candidates of a cell / 32) <= ncap / 32
     int pcap;            // row pairs of a tile
     int scap;            // entries of the staging image (multiple of 8)
     int nt_max;          // target cells of a tile
@@ -170,7 +171,7 @@ struct FusedSmem {
         stage = reinterpret_cast<uint16_t *>(base);
         size_t r0 = (size_t)fs.mcap * 16 + (size_t)fs.pcap * 32, r1 = (size_t)(fs.scap + 8) * 2;
         o = ((r0 > r1 ? r0 : r1) + 15) & ~(size_t)15;
-        masks = reinterpret_cast<uint32_t *>(base + o); o += (size_t)(fs.ncap / 32) * fs.tcap * 4;
+        masks = reinterpret_cast<uint32_t *>(base + o); o += (size_t)fs.wcap * fs.tcap * 4;
         cmap = reinterpret_cast<uint16_t *>(base + o); o += (size_t)fs.nt_max * fs.ncap * 2;
         o = (o + 3) & ~(size_t)3;
         off = reinterpret_cast<uint32_t *>(base + o); o += (size_t)(fs.tcap + 1) * 4;
@@ -182,7 +183,7 @@ struct FusedSmem {
 // bytes behind the overlay region, and the whole carve-up (must mirror FusedSmem)
 size_t fused_fixed_bytes(const FusedSizes &fs)
 {
-    size_t o = (size_t)(fs.ncap / 32) * fs.tcap * 4 + (size_t)fs.nt_max * fs.ncap * 2;
+    size_t o = (size_t)fs.wcap * fs.tcap * 4 + (size_t)fs.nt_max * fs.ncap * 2;
     o = (o + 3) & ~(size_t)3;
     o += (size_t)(fs.tcap + 1) * 4 + (size_t)fs.tcap * 6 + (size_t)fs.tcap * 4 + 16;
     return o;
@@ -420,7 +421,7 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
                     for (int k = 0; k < kCPL; ++k) {
                         const uint32_t w = cb * kCPL + k;
                         if (w * 32u >= Nc) continue;                       // uniform: no valid candidate in this word
-                        SPH_ASSERT(w < (uint32_t)(ncap / 32) && row_base + nr <= (uint32_t)tcap);
+                        SPH_ASSERT(w < (uint32_t)fs.wcap && row_base + nr <= (uint32_t)tcap);
                         uint32_t *mw = sm.masks + (size_t)w * tcap + row_base;
                         const uint32_t y = warp_transpose32(rb[k]);
                         if (islot >= 0 && (uint32_t)islot < nr1) mw[islot] = y;
@@ -740,6 +741,8 @@ int sph_neighbors_fused_run(sph_ctx *ctx, const SearchPar &sp, const TileGeom &t
     fs.tcap = (int)((Tmax + 7u) & ~7u);
     fs.ncap = (int)((ncmax + kCandBlock - 1) / kCandBlock * kCandBlock);
     if (fs.ncap < kCandBlock) fs.ncap = kCandBlock;
+    fs.wcap = (int)((ncmax + 31u) / 32u);
+    if (fs.wcap < 1) fs.wcap = 1;
     fs.nt_max = 1;
     for (int k = 0; k < gg.dim; ++k) fs.nt_max *= tg.B;
     fs.pcap = fs.tcap / 2 + fs.nt_max + 1;
@@ -753,7 +756,18 @@ int sph_neighbors_fused_run(sph_ctx *ctx, const SearchPar &sp, const TileGeom &t
     const size_t r0 = (size_t)fs.mcap * 16 + (size_t)fs.pcap * 32;
     fs.scap = 8;
     const size_t fixed = fused_fixed_bytes(fs) + 16;
-    const size_t cta_max = 232448 - 4096, two = (233472 - 2 * 5120) / 2;   // static shared memory + 1 KB per CTA set aside
+    // 227 KB per CTA minus the kernel's static shared memory (asked from the runtime, largest of the four variants)
+    static size_t static_smem = 0;
+    if (!static_smem) {
+        cudaFuncAttributes fa;
+        size_t mx = 0;
+        SPH_CUDA_TRY(cudaFuncGetAttributes(&fa, k_nb_fused<2, false>)); mx = std::max(mx, fa.sharedSizeBytes);
+        SPH_CUDA_TRY(cudaFuncGetAttributes(&fa, k_nb_fused<2, true>)); mx = std::max(mx, fa.sharedSizeBytes);
+        SPH_CUDA_TRY(cudaFuncGetAttributes(&fa, k_nb_fused<3, false>)); mx = std::max(mx, fa.sharedSizeBytes);
+        SPH_CUDA_TRY(cudaFuncGetAttributes(&fa, k_nb_fused<3, true>)); mx = std::max(mx, fa.sharedSizeBytes);
+        static_smem = (mx + 127) & ~(size_t)127;
+    }
+    const size_t cta_max = 232448 - static_smem, two = (233472 - 2 * 5120) / 2;   // two CTAs per SM: 1 KB each set aside
     if (fixed + r0 > cta_max) return 1;
     const size_t budget = fixed + r0 <= two ? two : cta_max;
     {

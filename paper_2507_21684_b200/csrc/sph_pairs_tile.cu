@@ -27,6 +27,22 @@ __device__ __forceinline__ float group_sum(float v)
     return v;
 }
 
+// Sums four per-lane values over the GS lanes of a group with 2 + 1 + log2(GS/4) shuffles instead of 4 log2(GS): the
+// first two butterfly steps halve the number of values a lane carries.  Lane gl ends up with the total of component
+// q = 2 [gl & GS/2] + [gl & GS/4]; the lanes with (gl & (GS/4 - 1)) == 0 are the four writers.  Fixed order: deterministic.
+template <int GS>
+__device__ __forceinline__ float group_sum4(float v0, float v1, float v2, float v3, int gl)
+{
+    static_assert(GS >= 4, "four components need four lanes");
+    const bool hi = (gl & (GS / 2)) != 0, mid = (gl & (GS / 4)) != 0;
+    float a = (hi ? v2 : v0) + __shfl_xor_sync(0xffffffffu, hi ? v0 : v2, GS / 2);
+    float b = (hi ? v3 : v1) + __shfl_xor_sync(0xffffffffu, hi ? v1 : v3, GS / 2);
+    float c = (mid ? b : a) + __shfl_xor_sync(0xffffffffu, mid ? a : b, GS / 4);
+#pragma unroll
+    for (int o = GS / 8; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    return c;
+}
+
 // ------------------------------------------------------------------------------------------ staging
 __device__ __forceinline__ void cp_async16(uint32_t smem_addr, const void *gptr)
 {
@@ -166,35 +182,46 @@ __device__ __forceinline__ void tile_row_passes(const TileTab &tt, const uint32_
     uint16_t *myring = ring + (size_t)warp * 2 * rb;
     const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(myring);
 
-    auto issue = [&](uint32_t r0, int buf) {
+    // 32-bit bookkeeping: entry k of the tile sits at seg[tb7 + k], seg 16-byte aligned (chunks of 8 entries)
+    const uint32_t tb7 = (uint32_t)(tilebase & 7ll);
+    const uint16_t *seg = col16 + (tilebase - (long long)tb7);
+    // copies the segment of the pass that starts at row r0 into half `buf` of the ring; returns its first entry and
+    // whether it fitted (the consumer of the pass needs both, one iteration later)
+    auto issue = [&](uint32_t r0, int buf, uint32_t &s_out, bool &fits) {
+        s_out = 0;
+        fits = false;
         if (r0 < T) {
-            const long long a = tilebase + rp[r0], e = tilebase + rp[min(r0 + RPW, T)];
-            const long long a0 = a & ~7ll;
-            const uint32_t nchunk = (uint32_t)((e - a0 + 7) >> 3);
-            if (nchunk * 8 <= (uint32_t)rb)
-                for (uint32_t c = lane; c < nchunk; c += 32)
-                    cp_async16(ring_s + (uint32_t)(buf * rb + c * 8) * 2, col16 + a0 + c * 8);
+            const uint32_t s = rp[r0], e = rp[min(r0 + RPW, T)];
+            const uint32_t c0 = (tb7 + s) >> 3, nchunk = ((tb7 + e + 7u) >> 3) - c0;
+            s_out = s;
+            fits = nchunk * 8u <= (uint32_t)rb;
+            if (fits) {
+                const uint16_t *src = seg + (size_t)c0 * 8;
+                const uint32_t dst = ring_s + (uint32_t)(buf * rb) * 2u;
+                for (uint32_t c = lane; c < nchunk; c += 32) cp_async16(dst + c * 16u, src + c * 8u);
+            }
         }
         cp_async_commit();
     };
     int buf = 0;
-    issue(warp * RPW, 0);
+    uint32_t s_cur, s_nxt;
+    bool f_cur, f_nxt;
+    issue(warp * RPW, 0, s_cur, f_cur);
     for (uint32_t r0 = warp * RPW; r0 < T; r0 += step, buf ^= 1) {
-        issue(r0 + step, buf ^ 1);
+        issue(r0 + step, buf ^ 1, s_nxt, f_nxt);
         cp_async_wait<1>();
         __syncwarp();
         const uint32_t r = min(r0 + g, T - 1);
         const bool live = r0 + g < T;
         const uint32_t b = rp[r], e = rp[r + 1];
         SPH_ASSERT(r < T && e >= b);
-        const uint32_t s = rp[r0];
-        const long long a = tilebase + s, e_seg = tilebase + rp[min(r0 + RPW, T)];
-        const long long a0 = a & ~7ll;
-        if ((uint32_t)((e_seg - a0 + 7) >> 3) * 8 <= (uint32_t)rb)
-            body(r, live, b, e, (const uint16_t *)(myring + buf * rb + (uint32_t)(a - a0)) - s);
+        if (f_cur)
+            body(r, live, b, e, (const uint16_t *)(myring + buf * rb + ((tb7 + s_cur) & 7u)) - s_cur);
         else
             body(r, live, b, e, col16 + tilebase);
         __syncwarp();
+        s_cur = s_nxt;
+        f_cur = f_nxt;
     }
     cp_async_wait<0>();
 }
@@ -685,24 +712,19 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                 a1 = fmaf(cf, d1, a1);
                 if (DIM == 3) a2 = fmaf(cf, d2, a2);
             }
-            float dr = pi.rho * sA + (VARH ? sD : hu.kd * sD);
-            dr = group_sum<GS>(dr);
-            a0 = group_sum<GS>(a0);
-            a1 = group_sum<GS>(a1);
-            if (DIM == 3) a2 = group_sum<GS>(a2);
-            if (gl == 0 && live) {
+            const float dr = pi.rho * sA + (VARH ? sD : hu.kd * sD);
+            // components {a0, a1, a2, drho} of the row, one per quarter of the lane group
+            float val = group_sum4<GS>(a0, a1, a2, dr, gl);
+            if ((gl & (GS / 4 - 1)) == 0 && live) {
+                const int q = ((gl & (GS / 2)) ? 2 : 0) + ((gl & (GS / 4)) ? 1 : 0);
                 const uint32_t row = row0 + r;
-                a0 = fixed ? 0.f : a0 + kp.g[0];
-                a1 = fixed ? 0.f : a1 + kp.g[1];
-                a2 = fixed ? 0.f : a2 + kp.g[2];
+                if (q < 3) val = fixed ? 0.f : val + kp.g[q];
                 if (OUT_SORTED) {
-                    out4[row] = make_float4(a0, a1, a2, dr);
+                    reinterpret_cast<float *>(out4 + row)[q] = val;
                 } else {
                     const int64_t i = perm[row];
-                    drho_out[i] = dr;
-                    acc_out[i * DIM] = a0;
-                    acc_out[i * DIM + 1] = a1;
-                    if (DIM == 3) acc_out[i * DIM + 2] = a2;
+                    if (q == 3) drho_out[i] = val;
+                    else if (q < DIM) acc_out[i * DIM + q] = val;
                 }
             }
         });
