@@ -85,7 +85,8 @@ enum {
                            clears; reported by sph_neighbors, the *_host calls and sph_check) */
     SPH_E_STATE = -3,   /* call order violated (neighbours before cells, RHS before neighbours, different n) */
     SPH_E_NOMEM = -4,   /* device or host allocation failed */
-    SPH_E_CUDA = -5     /* a CUDA runtime call failed */
+    SPH_E_CUDA = -5,    /* a CUDA runtime call failed */
+    SPH_E_TOO_LARGE = -6 /* size beyond the fixed capacity of an allocation-free entry point (sph_prefix_sum_noalloc) */
 };
 
 /* Create a context on CUDA device `device`.  n_max is a sizing hint (scratch grows on demand). */
@@ -211,6 +212,25 @@ int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_domain *dom_rk,
                   float skin, int64_t n, float *x, float *v, float *rho, const float *m, const float *h,
                   const uint8_t *kind, const float *drho_bar, const float *acc_bar, float *density, float *drho_dt,
                   float *acc, float *x_bar, float *v_bar, float *rho_bar, float *params_bar, int64_t *nnz_out);
+
+/* Allocation-free exclusive prefix sum: step N6 of the neighbour build (per-row counts -> 64-bit CSR offsets,
+ * PAPER.md:557-558 App. B step 2) for callers that cannot call cudaMalloc -- code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid allocation.  It needs no sph_ctx and calls no cudaMalloc / cudaFree / allocating
+ * library routine: the block sums of the scan live in a fixed device array inside the library (128 KiB on every GPU
+ * that loads it, until exit), which limits n to SPH_PREFIX_SUM_NOALLOC_MAX.
+ *   device : CUDA device of the buffers; made current (and left current), as every other call does with its context's
+ *   counts : device uint32[n], read only;   offsets: device int64[n + 1], written: offsets[i] = counts[0] + ... +
+ *            counts[i-1], offsets[n] = the total.  Both stay owned by the caller; they must not overlap.
+ *   n      : 0 <= n <= SPH_PREFIX_SUM_NOALLOC_MAX.  n == 0 does the per-device set-up only (one symbol look-up, no
+ *            launch): call it once per device BEFORE a stream capture starts; later calls only launch three kernels on
+ *            `stream`, asynchronously.
+ * Returns SPH_E_TOO_LARGE for n beyond the maximum (nothing is launched), SPH_E_INVALID for a null pointer, negative n
+ * or a device number outside 0..63, SPH_E_CUDA if the runtime fails.
+ * All calls on a device share the one scratch array.  Its old contents never matter (every word a call reads it has
+ * written first), but two calls whose kernels OVERLAP on the GPU -- different streams without an ordering between
+ * them, or several host threads -- race on it and both results are garbage: order them on one stream or by events. */
+#define SPH_PREFIX_SUM_NOALLOC_MAX (1ll << 26)
+int sph_prefix_sum_noalloc(int device, const uint32_t *counts, int64_t *offsets, int64_t n, sph_stream_t stream);
 
 /* Fetch the device-side error flag (synchronises the context's last stream). */
 int sph_check(sph_ctx *ctx);

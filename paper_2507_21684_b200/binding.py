@@ -19,7 +19,7 @@ EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph
            "sph_density_vjp", "sph_lists_valid", "sph_grad_sum", "sph_grad_sum_vjp", "sph_renorm_gradient", "sph_renorm_gradient_vjp",
            "sph_rhs", "sph_rhs_vjp", "sph_rk_step", "sph_rk_step_vjp", "sph_forward_backward_host", "sph_step_host",
            "sph_check", "sph_debug_bounds_violations", "sph_strerror", "sph_get_info", "sph_get_layout", "sph_profile_enable", "sph_profile_read",
-           "sph_set_option", "sph_shift")
+           "sph_set_option", "sph_shift", "sph_prefix_sum_noalloc")
 
 # keys of sph_set_option (enum SPH_OPT_* in include/sph.h)
 OPT_PAIR_GROUP, OPT_LIST_MODE, OPT_TILE_EDGE, OPT_PAIR_WARPS, OPT_FILL_MASKS, OPT_RK_EXTRA_SKIN = 1, 2, 3, 4, 5, 6
@@ -86,6 +86,7 @@ def load_library(path: str = LIB_PATH):
     lib.sph_set_option.argtypes = [vp, C.c_int, C.c_int]
     lib.sph_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
     lib.sph_check.argtypes = [vp]
+    lib.sph_prefix_sum_noalloc.argtypes = [C.c_int, vp, vp, i64, vp]
     lib.sph_debug_bounds_violations.argtypes = [vp, C.POINTER(C.c_int64)]
     lib.sph_strerror.argtypes = [C.c_int]
     lib.sph_strerror.restype = C.c_char_p
@@ -134,6 +135,23 @@ def _f32(t, shape=None):
     if shape is not None:
         assert tuple(t.shape) == tuple(shape), (tuple(t.shape), shape)
     return t
+
+
+PREFIX_SUM_NOALLOC_MAX = 1 << 26      # SPH_PREFIX_SUM_NOALLOC_MAX of include/sph.h
+
+
+def prefix_sum_noalloc(counts, offsets):
+    """sph_prefix_sum_noalloc: exclusive prefix sum of a uint32 count array (viewed through an int32 / uint32 CUDA tensor
+    of n entries) into the caller's int64 tensor of n + 1 entries, on the current stream.  Allocates nothing -- neither
+    here (both tensors are the caller's) nor in the library; raises SphError(-6) beyond PREFIX_SUM_NOALLOC_MAX."""
+    lib = load_library()
+    assert counts.is_cuda and counts.is_contiguous() and counts.dtype in (torch.int32, torch.uint32)
+    n = int(counts.numel())
+    assert offsets.is_cuda and offsets.is_contiguous() and offsets.dtype == torch.int64 and offsets.numel() == n + 1
+    rc = lib.sph_prefix_sum_noalloc(int(counts.device.index or 0), _ptr(counts), _ptr(offsets), n, _stream())
+    if rc != 0:
+        raise SphError(rc, lib.sph_strerror(rc).decode())
+    return offsets
 
 
 class Sph:

@@ -93,6 +93,7 @@ extern "C" const char *sph_strerror(int code)
     case SPH_E_STATE: return "call order violated";
     case SPH_E_NOMEM: return "out of memory";
     case SPH_E_CUDA: return "CUDA runtime error (or no CUDA device: this library has no CPU fallback)";
+    case SPH_E_TOO_LARGE: return "size beyond the fixed capacity of an allocation-free entry point";
     default: return "unknown error";
     }
 }

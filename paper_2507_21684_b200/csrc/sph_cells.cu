@@ -5,6 +5,8 @@
 
 #include <math.h>
 
+#include <mutex>
+
 namespace {
 
 constexpr int kThreads = 256;
@@ -451,4 +453,51 @@ extern "C" int sph_lists_valid(sph_ctx *ctx, const float *x, float skin_needed, 
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
     return sph_lists_valid_impl(ctx, x, nullptr, skin_needed, valid_out, max_disp_out, st);
+}
+
+// ------------------------------------------------------------------------------------------ allocation-free prefix sum
+// Step N6 (exclusive scan of the per-row counts -> 64-bit CSR offsets, App. B step 2) for callers that
+// must not allocate: CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Same three kernels as
+// sph_scan_u32 above; the block sums, which that path keeps in a context buffer that grows on demand, live here in a
+// file-scope device array of fixed size (16384 x 8 B = 128 KiB, held by every GPU that loads the library until exit).
+//
+// In host code `g_scan_noalloc` is the host-side stand-in of the symbol, NOT a device address: the address the kernels
+// get is looked up once per device, with that device current, by cudaGetSymbolAddress.
+constexpr int64_t kNoAllocMaxCount = (int64_t)SPH_PREFIX_SUM_NOALLOC_MAX;
+constexpr int64_t kNoAllocMaxBlocks = (kNoAllocMaxCount + kScanTile - 1) / kScanTile;
+static __device__ __align__(256) unsigned long long g_scan_noalloc[kNoAllocMaxBlocks];
+
+namespace {
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+unsigned long long *g_noalloc_ptr[kNoAllocMaxDevices] = {};
+}
+
+extern "C" int sph_prefix_sum_noalloc(int device, const uint32_t *counts, int64_t *offsets, int64_t n, sph_stream_t stream)
+{
+    if (device < 0 || device >= kNoAllocMaxDevices || n < 0) return SPH_E_INVALID;
+    if (n > kNoAllocMaxCount) return SPH_E_TOO_LARGE;
+    if (n > 0 && (!counts || !offsets)) return SPH_E_INVALID;
+    SPH_CUDA_TRY(cudaSetDevice(device));
+    unsigned long long *sums = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+        if (!g_noalloc_ptr[device]) {
+            void *p = nullptr;
+            SPH_CUDA_TRY(cudaGetSymbolAddress(&p, g_scan_noalloc));     // this device's copy of the array
+            if (!p) return SPH_E_CUDA;
+            g_noalloc_ptr[device] = static_cast<unsigned long long *>(p);
+        }
+        sums = g_noalloc_ptr[device];
+    }
+    if (n == 0) return SPH_OK;                                          // set-up only
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t nb = (n + kScanTile - 1) / kScanTile;
+    // every entry of sums[0, nb) is overwritten by k_scan_reduce before it is read and nothing beyond nb is read, so
+    // the contents a previous call left behind need no clearing
+    k_scan_reduce<<<(unsigned)nb, kScanThreads, 0, st>>>(counts, n, sums);
+    k_scan_sums<<<1, kScanThreads, 0, st>>>(sums, nb);
+    k_scan_apply<long long><<<(unsigned)nb, kScanThreads, 0, st>>>(counts, reinterpret_cast<long long *>(offsets), n, sums, 1);
+    SPH_CUDA_TRY(cudaGetLastError());
+    return SPH_OK;
 }
