@@ -293,6 +293,10 @@ enum {
     SPH_OPT_STAGE_BULK = 9, /* 0 (default): the tile pair kernels stage a halo with one 16-byte cp.async per particle and
                                array; 1: sph_rhs / sph_rhs_vjp stage their float4 arrays with one cp.async.bulk per halo
                                cell and array, completing on one mbarrier per CTA (A/B measurement) */
+    SPH_OPT_VJP_SPLIT = 10, /* 1 (default): in 3D on 2x2x2-cell tiles the adjoint pair kernel of sph_rhs_vjp gives each CTA HALF
+                               a tile (one z-layer of its cells, staging the three layers of halo cells around it), so
+                               that two CTAs are resident per SM and one stages while the other computes;
+                               0: one CTA per tile (A/B measurement);  2: sph_rhs too (measured slower, A/B only) */
     SPH_OPT_RK_EXTRA_SKIN = 6 /* Verlet lists across steps: value/1000 = extra skin e (in units of h).  With
                                e > 0 sph_rk_step / sph_rk_step_vjp build their lists with search_scale = 1 + skin + e
                                (the domain's cell_size must cover it) and a later call with the same domain, n and h

@@ -316,6 +316,10 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
     case SPH_OPT_STAGE_BULK:
         ctx->opt_stage_bulk = value != 0;
         return SPH_OK;
+    case SPH_OPT_VJP_SPLIT:
+        if (value < 0 || value > 2) return SPH_E_INVALID;
+        ctx->opt_vjp_split = value;
+        return SPH_OK;
     case SPH_OPT_UNIFORM_MASS_PATH:
         ctx->opt_no_um = value == 0;
         return SPH_OK;

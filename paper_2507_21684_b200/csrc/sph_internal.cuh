@@ -137,10 +137,12 @@ struct sph_ctx {
     int opt_fused_warps = 0;    // warps per CTA of the one-kernel build (0 = default)
     int opt_build_fused = 1;    // 1: the tile-local lists are built by the one-kernel build (sph_neighbors_fused.cu) when a tile fits it
     int opt_stage_bulk = 0;     // 1: k_rhs_tile / k_vjp_tile stage their float4 halo arrays with cp.async.bulk + one mbarrier (measured: profiles/r02_f)
+    int opt_vjp_split = 1;      // 1: k_vjp_tile works on half a 2x2x2 tile per CTA (two resident CTAs per SM instead of one)
     int opt_no_um = 0;          // 1: never launch the uniform-mass variants of the tile pair kernels (A/B measurements, tests)
     bool tile_mode = false;     // lists of the last sph_neighbors are tile-local (col16)
     TileGeom tg{};
     uint32_t tile_Mmax = 0, tile_Tmax = 0;   // largest halo / row count of a tile
+    uint32_t tile_Mhalf = 0;                 // largest halo of HALF a tile (3D, 2x2x2 cells: three z-layers); 0 = no halves
     int64_t n_hint = 0;
     int64_t n = 0;
     bool cells_ready = false, lists_ready = false;
@@ -201,6 +203,7 @@ struct sph_ctx {
 // (float bits).  Written on the stream by the pack kernels (k_pack_state, k_rk_base), read by the pair kernels: the
 // host never needs to know -- both variants of a pair kernel are launched and the one whose turn it is not returns.
 constexpr int kUmSlot = 13;
+constexpr int kTileHalfSlot = 15;      // stats word: largest halo of half a 2x2x2 tile (three of its four z-layers of cells)
 inline uint32_t *sph_um_flag(const sph_ctx *ctx) { return ctx->stats.as<uint32_t>() + kUmSlot; }
 #ifdef __CUDACC__
 // Pack kernels: a density that is not a positive finite number, or a mass that is not finite, raises bit 4 of the
@@ -385,6 +388,7 @@ int sph_launch_grad_sum_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *ga_
                                  cudaStream_t st);
 int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
                         const uint8_t *kind_s, float *drho, float *acc, float4 *out4, cudaStream_t st);
+int sph_vjp_tile_split(const sph_ctx *ctx, const KPar &kp);
 int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
                         const float4 *cot, const float4 *eos, float *xb, float *vb, float *rb, float4 *xb4, float4 *vb4,
                         float *partials, cudaStream_t st);

@@ -296,11 +296,11 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
         SPH_CUDA_TRY(cudaMemcpyAsync(ctx->h_pinned + 16, ctx->fstats.p, 16, cudaMemcpyDeviceToHost, st));
     }
     // the statistics of sph_build_cells (error flag, max/min h) are needed on the host to size the search
-    uint32_t hs[11];
+    uint32_t hs[16];
     uint32_t *hpin = reinterpret_cast<uint32_t *>(ctx->h_pinned + 8);
-    SPH_CUDA_TRY(cudaMemcpyAsync(hpin, ctx->stats.p, 44, cudaMemcpyDeviceToHost, st));
+    SPH_CUDA_TRY(cudaMemcpyAsync(hpin, ctx->stats.p, 64, cudaMemcpyDeviceToHost, st));
     SPH_CUDA_TRY(cudaStreamSynchronize(st));
-    memcpy(hs, hpin, 44);
+    memcpy(hs, hpin, 64);
     ctx->f_ncmax = 0;
     ctx->f_pairs = 0;
     if (fused_stats) {
@@ -346,6 +346,7 @@ extern "C" int sph_neighbors(sph_ctx *ctx, float search_scale, int64_t *nnz_out,
         const uint32_t Mmax = hs[4 + 2 * k], Tmax = hs[5 + 2 * k];
         if (!sph_tile_fits(gg.dim, Mmax)) continue;
         SPH_TRY(sph_neighbors_tile_run(ctx, sp, cand[k], Mmax, Tmax, hs[10], st, nnz_out));
+        ctx->tile_Mhalf = (gg.dim == 3 && cand[k] == 2) ? hs[kTileHalfSlot] : 0u;
         ctx->search_scale = search_scale;
         ctx->lists_ready = true;
         return SPH_OK;

@@ -437,10 +437,12 @@ k_nb_expand(TileGeom tg, int wcap, int wbcap, const uint32_t *__restrict__ cell_
 // largest halo population and largest row count over all tiles of a candidate decomposition (one thread per tile)
 template <int DIM>
 __global__ void k_tile_stats(TileGeom tg, const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
-                             uint32_t *__restrict__ out /* [2]: Mmax, Tmax */, uint32_t *__restrict__ occ_out)
+                             uint32_t *__restrict__ out /* [2]: Mmax, Tmax */, uint32_t *__restrict__ occ_out,
+                             uint32_t *__restrict__ half_out /* or NULL: largest halo of HALF a tile (k_vjp_tile) */)
 {
     const int tile = blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t M = 0, T = 0, occ = 0;
+    uint32_t M = 0, T = 0, occ = 0, Mh = 0;
+    uint32_t slab[4] = {0u, 0u, 0u, 0u};                    // halo particles per z-layer of cells (B <= 2 in 3D)
     if (tile < tg.ntiles) {
         int b = tile, bc[3] = {0, 0, 0};
         bc[0] = b % tg.nb[0];
@@ -471,17 +473,30 @@ __global__ void k_tile_stats(TileGeom tg, const uint32_t *__restrict__ cell_star
                     }
                     const uint32_t cc = cell_end[lin] - cell_start[lin];
                     M += cc;
+                    if (DIM == 3 && cz - lo[2] < 4) slab[cz - lo[2]] += cc;
                     if (tgt) T += cc;
                     occ = max(occ, cc);
                 }
+        // a tile of two cell layers in z can be worked on as two halves, each with the three layers around its own
+        if (DIM == 3 && half_out) {
+            if (t1[2] - t0[2] != 1) Mh = M;
+            else
+                for (int s = 0; s < 2; ++s) {
+                    uint32_t m = 0;
+                    for (int cz = max(t0[2] + s - 1, lo[2]); cz <= min(t0[2] + s + 1, hi[2]); ++cz) m += slab[cz - lo[2]];
+                    Mh = max(Mh, m);
+                }
+        }
     }
     M = __reduce_max_sync(0xffffffffu, M);
     T = __reduce_max_sync(0xffffffffu, T);
+    Mh = __reduce_max_sync(0xffffffffu, Mh);
     occ = __reduce_max_sync(0xffffffffu, occ);
     if ((threadIdx.x & 31) == 0) {
         atomicMax(&out[0], M);
         atomicMax(&out[1], T);
         atomicMax(occ_out, occ);                     // largest cell occupancy
+        if (half_out) atomicMax(half_out, Mh);
     }
 }
 
@@ -553,12 +568,15 @@ int sph_tile_stats_launch(sph_ctx *ctx, const int *cand, int ncand, cudaStream_t
 {
     uint32_t *stats = ctx->stats.as<uint32_t>();
     SPH_CUDA_TRY(cudaMemsetAsync(stats + 4, 0, 7 * sizeof(uint32_t), st));
+    SPH_CUDA_TRY(cudaMemsetAsync(stats + kTileHalfSlot, 0, sizeof(uint32_t), st));
     for (int k = 0; k < ncand; ++k) {
         const TileGeom tg = make_tile_geom(ctx->geom, cand[k]);
         KScope ks(ctx, SPH_K_COUNT, 1, st);
         const unsigned nb = (unsigned)((tg.ntiles + 127) / 128);
-        if (tg.dim == 3) k_tile_stats<3><<<nb, 128, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), stats + 4 + 2 * k, stats + 10);
-        else k_tile_stats<2><<<nb, 128, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), stats + 4 + 2 * k, stats + 10);
+        if (tg.dim == 3)
+            k_tile_stats<3><<<nb, 128, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), stats + 4 + 2 * k, stats + 10,
+                                                cand[k] == 2 ? stats + kTileHalfSlot : nullptr);
+        else k_tile_stats<2><<<nb, 128, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), stats + 4 + 2 * k, stats + 10, nullptr);
     }
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;

@@ -981,23 +981,26 @@ __global__ void k_renorm_solve_sorted(int64_t n, const float4 *__restrict__ mom,
 
 // B2 stage 2: one block, binary64 accumulation of the per-block partials in index order, then the chain rule
 // from the ten sums to params_bar = d/d{c0, rho0, gamma, delta, alpha, nu, eps, g0, g1, g2}.
-__global__ void k_reduce_params(int64_t nblocks, const float *__restrict__ partials, KPar kp, int accumulate,
+constexpr int kReduceThreads = 512;
+__global__ void __launch_bounds__(kReduceThreads)
+k_reduce_params(int64_t nblocks, const float *__restrict__ partials, KPar kp, int accumulate,
                                 float *__restrict__ params_bar)
 {
-    __shared__ double sh[10][128];
+    __shared__ double sh[10][kReduceThreads];
+    __shared__ double S[10];
     double acc[10];
     for (int k = 0; k < 10; ++k) acc[k] = 0.0;
     for (int64_t b = threadIdx.x; b < nblocks; b += blockDim.x)
         for (int k = 0; k < 10; ++k) acc[k] += (double)partials[b * kNPart + k];
     for (int k = 0; k < 10; ++k) sh[k][threadIdx.x] = acc[k];
     __syncthreads();
+    if (threadIdx.x < 10) {                                  // thread k: sum k over the threads, in index order
+        double v = 0.0;
+        for (int t = 0; t < (int)blockDim.x; ++t) v += sh[threadIdx.x][t];
+        S[threadIdx.x] = v;
+    }
+    __syncthreads();
     if (threadIdx.x == 0) {
-        double S[10];
-        for (int k = 0; k < 10; ++k) {
-            double v = 0.0;
-            for (int t = 0; t < (int)blockDim.x; ++t) v += sh[k][t];
-            S[k] = v;
-        }
         const double S_D1 = S[0], S_P1 = S[1], S_PL = S[2], S_eps = S[3], T_E = S[4], T_0 = S[5], T_g = S[6];
         const double c0 = kp.c0, rho0 = kp.rho0, visc = kp.visc_nu;
         double out[10];
@@ -1157,7 +1160,7 @@ int sph_launch_vjp_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
     const uint32_t *perm = ctx->perm.as<uint32_t>();
     const bool sorted = xb4 != nullptr;
     const int gs = ctx->opt_group ? ctx->opt_group : (kp.dim == 3 ? 32 : 16);
-    const unsigned grid = ctx->tile_mode ? (unsigned)ctx->tg.ntiles : pair_grid(n, gs);
+    const unsigned grid = ctx->tile_mode ? (unsigned)ctx->tg.ntiles * (unsigned)sph_vjp_tile_split(ctx, kp) : pair_grid(n, gs);
     SPH_TRY(ctx->partials.reserve((size_t)grid * kNPart * 4));
     float *part = ctx->partials.as<float>();
     if (ctx->tile_mode) {
@@ -1187,7 +1190,7 @@ int sph_launch_vjp_sorted(sph_ctx *ctx, const KPar &kp, const float4 *s0, const 
     }
     if (params_bar) {
         KScope ks(ctx, SPH_K_REDUCE, 1, st);
-        k_reduce_params<<<1, 128, 0, st>>>((int64_t)grid, part, kp, accumulate_params, params_bar);
+        k_reduce_params<<<1, kReduceThreads, 0, st>>>((int64_t)grid, part, kp, accumulate_params, params_bar);
     }
     SPH_CUDA_TRY(cudaGetLastError());
     if (kp.delta_form == 1) SPH_TRY(sph_delta_adjoint(ctx, kp, s0, s1, s2, cot, xb, rb, xb4, params_bar, st));

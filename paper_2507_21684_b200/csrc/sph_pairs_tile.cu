@@ -96,10 +96,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 __device__ __forceinline__ void stage_halo(const TileTab &tt, const float4 *__restrict__ g0, float4 *d0,
                                            const float4 *__restrict__ g1, float4 *d1, const float4 *__restrict__ g2,
                                            float4 *d2, const float2 *__restrict__ gc, float2 *dc,
-                                           const float *__restrict__ gf, float *df, uint64_t *bar = nullptr)
+                                           const float *__restrict__ gf, float *df, uint64_t *bar = nullptr,
+                                           int hc_lo = 0, int hc_hi = -1, uint32_t q_lo = 0)
 {
+    // [hc_lo, hc_hi): the halo cells to stage (default: all); the particle with halo-linear index q lands at slot q - q_lo
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    const uint32_t a0 = smem_u32(d0), a1 = smem_u32(d1), a2 = smem_u32(d2), ac = smem_u32(dc), af = smem_u32(df);
+    if (hc_hi < 0) hc_hi = tt.nh;
+    const uint32_t a0 = smem_u32(d0) - q_lo * 16u, a1 = smem_u32(d1) - q_lo * 16u, a2 = smem_u32(d2) - q_lo * 16u,
+                   ac = smem_u32(dc) - q_lo * 8u, af = smem_u32(df) - q_lo * 4u;
     if (bar) {
         // the float4 arrays by bulk copies (runs are 16-byte aligned multiples of 16 bytes by construction); the caller has
         // initialised the barrier (count 1) and synchronised.  The float2 / float arrays below stay per-particle copies.
@@ -114,7 +118,7 @@ __device__ __forceinline__ void stage_halo(const TileTab &tt, const float4 *__re
         g0 = nullptr; g1 = nullptr; g2 = nullptr;
         if (!gc && !gf) return;
     }
-    for (int hc = warp; hc < tt.nh; hc += nwarps) {
+    for (int hc = hc_lo + warp; hc < hc_hi; hc += nwarps) {
         const uint32_t o0 = tt.h_off[hc], cnt = tt.h_off[hc + 1] - o0, gs = tt.h_start[hc];
         for (uint32_t l = lane; l < cnt; l += 32) {
             const uint32_t q = o0 + l;
@@ -131,11 +135,13 @@ __device__ __forceinline__ void stage_halo(const TileTab &tt, const float4 *__re
 // after the copies have landed (wait + __syncthreads): add the periodic shift to the positions of the halo cells
 // that lie across a face.  Contains a __syncthreads on seam tiles (uniform per CTA).
 template <int DIM>
-__device__ __forceinline__ void stage_shift(const TileTab &tt, float4 *d0)
+__device__ __forceinline__ void stage_shift(const TileTab &tt, float4 *d0, int hc_lo = 0, int hc_hi = -1, uint32_t q_lo = 0)
 {
     if (!tt.seam) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    for (int hc = warp; hc < tt.nh; hc += nwarps) {
+    if (hc_hi < 0) hc_hi = tt.nh;
+    d0 -= q_lo;
+    for (int hc = hc_lo + warp; hc < hc_hi; hc += nwarps) {
         const float sx = tt.h_shift[0][hc], sy = tt.h_shift[1][hc], sz = DIM == 3 ? tt.h_shift[2][hc] : 0.f;
         if (sx == 0.f && sy == 0.f && sz == 0.f) continue;
         const uint32_t o0 = tt.h_off[hc], cnt = tt.h_off[hc + 1] - o0;
@@ -164,6 +170,48 @@ __device__ __forceinline__ void stage_rows(const TileTab &tt, const long long *_
     }
 }
 
+// sizes of the shared-memory carve-up of one launch (SmemMap below) and its launch-wide switches
+struct TileSizes {
+    int mcap, tcap, rb;
+    int split;           // k_vjp_tile: 2 = each CTA takes half a tile (one z-layer of a 2x2x2 block), 1 = a whole tile
+    int bulk;            // SPH_OPT_STAGE_BULK: k_rhs_tile / k_vjp_tile stage their float4 arrays with cp.async.bulk
+};
+
+// ts.split == 2 (3D, 2x2x2-cell tiles): two CTAs per tile, each with the rows of one z-layer of target cells and the three
+// z-layers of halo cells around it -- a contiguous range of halo cells, of halo-linear indices and (the sort key is the
+// Morton code, z its top bit inside a block) of rows.  A halo particle q is staged at slot q - q_lo, and the gathers use
+// base pointers moved back by q_lo, so the list entries are used as they are.  Two resident CTAs instead of one (or three
+// instead of two) let one stage its halo while the others compute.
+struct TilePart {
+    uint32_t row_lo, row_hi, q_lo, q_hi;
+    int hc_lo, hc_hi;
+};
+template <int DIM>
+__device__ __forceinline__ int tile_of_block(const TileSizes &ts)
+{
+    return (DIM == 3 && ts.split == 2) ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
+}
+template <int DIM>
+__device__ __forceinline__ TilePart tile_part(const TileTab &tt, const TileSizes &ts)
+{
+    TilePart tp{0u, tt.T, 0u, tt.M, 0, tt.nh};
+    if (DIM == 3 && ts.split == 2) {
+        const int half = (int)(blockIdx.x & 1u), per = tt.tn[0] * tt.tn[1];
+        if (half >= tt.tn[2]) tp.row_hi = 0;                    // a tile with one layer only: its first CTA has it all
+        else if (tt.tn[2] == 2) {
+            tp.row_lo = tt.t_off[half * per];
+            tp.row_hi = tt.t_off[(half + 1) * per];
+            const int zt = tt.tlo[2] + half, slab = tt.ext[0] * tt.ext[1];
+            tp.hc_lo = max(zt - 1, 0) * slab;
+            tp.hc_hi = (min(zt + 1, tt.ext[2] - 1) + 1) * slab;
+            tp.q_lo = tt.h_off[tp.hc_lo];
+            tp.q_hi = tt.h_off[tp.hc_hi];
+        }
+    }
+    SPH_ASSERT(tp.q_hi - tp.q_lo <= (uint32_t)ts.mcap);
+    return tp;
+}
+
 // ------------------------------------------------------------------------------------------ index ring
 // Drives the rows of a tile through `body(r, live, b, e, idx)`: row r of the tile (clamped to T-1; `live` false for
 // the padding groups of the last pass), its tile-relative entry range [b,e), and a pointer such that idx[k] is the
@@ -172,12 +220,14 @@ __device__ __forceinline__ void stage_rows(const TileTab &tt, const long long *_
 // processed.  A segment that does not fit the ring is read from global memory directly (correct, slower).
 template <int GS, class Body>
 __device__ __forceinline__ void tile_row_passes(const TileTab &tt, const uint32_t *rp, uint16_t *ring, int rb,
-                                                const uint16_t *__restrict__ col16, long long tilebase, Body body)
+                                                const uint16_t *__restrict__ col16, long long tilebase, Body body,
+                                                uint32_t row_lo = 0, uint32_t row_hi = 0xffffffffu)
 {
+    // [row_lo, row_hi): the rows of the tile this CTA works on (default: all of them)
     constexpr int RPW = 32 / GS;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int g = lane / GS;
-    const uint32_t T = tt.T;
+    const uint32_t T = min(tt.T, row_hi);
     const uint32_t step = nwarps * RPW;
     uint16_t *myring = ring + (size_t)warp * 2 * rb;
     const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(myring);
@@ -206,8 +256,8 @@ __device__ __forceinline__ void tile_row_passes(const TileTab &tt, const uint32_
     int buf = 0;
     uint32_t s_cur, s_nxt;
     bool f_cur, f_nxt;
-    issue(warp * RPW, 0, s_cur, f_cur);
-    for (uint32_t r0 = warp * RPW; r0 < T; r0 += step, buf ^= 1) {
+    issue(row_lo + warp * RPW, 0, s_cur, f_cur);
+    for (uint32_t r0 = row_lo + warp * RPW; r0 < T; r0 += step, buf ^= 1) {
         issue(r0 + step, buf ^ 1, s_nxt, f_nxt);
         cp_async_wait<1>();
         __syncwarp();
@@ -244,10 +294,6 @@ __device__ __forceinline__ Part load_part(const float4 *s0, const float4 *s1, co
 
 // shared-memory carve-up: A, B (float4[mcap]), [cot float4[mcap]], C (float2[mcap], 3D only), rp[tcap+1],
 // selfq[tcap], index ring [nwarps][2][rb]
-struct TileSizes {
-    int mcap, tcap, rb;
-    int bulk;            // SPH_OPT_STAGE_BULK: k_rhs_tile / k_vjp_tile stage their float4 arrays with cp.async.bulk
-};
 template <int DIM>
 struct SmemMap {
     float4 *A, *B, *cot;
@@ -634,26 +680,28 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const SmemMap<DIM> sm(smem_raw, ts, false, !UM);
     __shared__ TileTab tt;
-    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
-    if (tt.T == 0) return;
+    tile_setup<DIM>(tg, tile_of_block<DIM>(ts), cell_start, cell_end, tt);
+    const TilePart tp = tile_part<DIM>(tt, ts);
+    if (tp.row_hi <= tp.row_lo) return;
     __shared__ uint64_t mbar;
-    if (ts.bulk) {
+    const bool bulk = ts.bulk && ts.split != 2;
+    if (bulk) {
         if (threadIdx.x == 0) mbar_init(&mbar, 1);
         __syncthreads();
     }
     stage_halo(tt, s0, sm.A, s1, sm.B, nullptr, nullptr, (DIM == 3 && !UM) ? s2 : nullptr, sm.C, nullptr, nullptr,
-               ts.bulk ? &mbar : nullptr);
+               bulk ? &mbar : nullptr, tp.hc_lo, tp.hc_hi, tp.q_lo);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
     cp_async_wait<0>();
-    if (ts.bulk) mbar_wait(&mbar, 0);
+    if (bulk) mbar_wait(&mbar, 0);
     __syncthreads();
-    stage_shift<DIM>(tt, sm.A);
+    stage_shift<DIM>(tt, sm.A, tp.hc_lo, tp.hc_hi, tp.q_lo);
     const int gl = (threadIdx.x & 31) % GS;
     const HC hu = hc_uniform<DIM>(kp);
     const float rho0 = kp.rho0;
     const float umG = m0 * hu.cG, umG5 = umG * 5.0f * hu.invH;      // uniform mass: m0 G = (umG + umG5 r) (1-q)^5
-    const float4 *A = sm.A, *B = sm.B;
-    const float2 *C = sm.C;
+    const float4 *A = sm.A - tp.q_lo, *B = sm.B - tp.q_lo;
+    const float2 *C = sm.C - tp.q_lo;
     const uint16_t *selfq = sm.selfq;
     const uint32_t row0 = tt.row0;
     tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
@@ -668,7 +716,7 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
 #pragma unroll 2
             for (uint32_t k = b + gl; k < e; k += GS) {
                 const uint32_t j = idx[k];
-                SPH_ASSERT(j < tt.M);
+                SPH_ASSERT(j >= tp.q_lo && j < tp.q_hi);
                 const Part pj = load_part<DIM, UM>(A, B, C, j, m0, kp.H);
                 const float d0 = pi.x[0] - pj.x[0], d1 = pi.x[1] - pj.x[1], d2 = DIM == 3 ? pi.x[2] - pj.x[2] : 0.f;
                 const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
@@ -727,7 +775,7 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                     else if (q < DIM) acc_out[i * DIM + q] = val;
                 }
             }
-        });
+        }, tp.row_lo, tp.row_hi);
 }
 
 // ------------------------------------------------------------------------------------------ B1: VJP
@@ -753,30 +801,36 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
     const SmemMap<DIM> sm(smem_raw, ts, true, !UM);
     __shared__ TileTab tt;
     __shared__ float red[kVjpMaxWarps][kNPartT];
-    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
-    if (tt.T == 0) {
+    tile_setup<DIM>(tg, tile_of_block<DIM>(ts), cell_start, cell_end, tt);
+    const TilePart tp = tile_part<DIM>(tt, ts);
+    const uint32_t row_lo = tp.row_lo, row_hi = tp.row_hi, q_lo = tp.q_lo;
+    const int hc_lo = tp.hc_lo, hc_hi = tp.hc_hi;
+    if (row_hi <= row_lo) {
         if (threadIdx.x < kNPartT) partials[(int64_t)blockIdx.x * kNPartT + threadIdx.x] = 0.f;
         return;
     }
     __shared__ uint64_t mbar;
-    if (ts.bulk) {
+    const bool bulk = ts.bulk && ts.split != 2;
+    if (bulk) {
         if (threadIdx.x == 0) mbar_init(&mbar, 1);
         __syncthreads();
     }
     stage_halo(tt, s0, sm.A, s1, sm.B, cot, sm.cot, (DIM == 3 && !UM) ? s2 : nullptr, sm.C, nullptr, nullptr,
-               ts.bulk ? &mbar : nullptr);
+               bulk ? &mbar : nullptr, hc_lo, hc_hi, q_lo);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
     cp_async_wait<0>();
-    if (ts.bulk) mbar_wait(&mbar, 0);
+    if (bulk) mbar_wait(&mbar, 0);
     __syncthreads();
-    stage_shift<DIM>(tt, sm.A);
+    stage_shift<DIM>(tt, sm.A, hc_lo, hc_hi, q_lo);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gl = lane % GS;
     const HC hu = hc_uniform<DIM>(kp);
     const float rho0 = kp.rho0;
-    const float4 *A = sm.A, *B = sm.B, *Ct = sm.cot;
-    const float2 *C = sm.C;
+    const float4 *A = sm.A - q_lo, *B = sm.B - q_lo, *Ct = sm.cot - q_lo;
+    const float2 *C = sm.C - q_lo;
     const uint16_t *selfq = sm.selfq;
     const uint32_t row0 = tt.row0;
+    const uint32_t q_hi = tp.q_hi;
+    (void)q_hi;
     float S_D1 = 0.f, S_P1 = 0.f, S_PL = 0.f, S_eps = 0.f;                 // per lane, over all its pairs
     float T_E = 0.f, T_0 = 0.f, T_g = 0.f, G0 = 0.f, G1 = 0.f, G2 = 0.f;   // lane 0 of each group, per row
     tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
@@ -792,7 +846,7 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
             float xb[3] = {0.f, 0.f, 0.f}, vb[3] = {0.f, 0.f, 0.f}, rb = 0.f, Z = 0.f, Zr = 0.f;
             for (uint32_t k = b + gl; k < e; k += GS) {
                 const uint32_t j = idx[k];
-                SPH_ASSERT(j < tt.M);
+                SPH_ASSERT(j >= q_lo && j < q_hi);
                 Part pj = load_part<DIM, UM>(A, B, C, j, m0, kp.H);
                 const float4 cj = Ct[j];
                 const float lam_j = cj.x, mu_j[3] = {cj.y, cj.z, cj.w};
@@ -917,7 +971,7 @@ k_vjp_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                     rb_out[i] = rb;
                 }
             }
-        });
+        }, row_lo, row_hi);
     // S_D1 = sum lam_i D_ij/(delta c0), S_PL = sum ell xphi1, S_eps = d/d eps: factors left out of the loop
     if (!VARH) {
         S_D1 *= 2.0f * hu.ell;
@@ -1081,9 +1135,10 @@ static int tile_group(const sph_ctx *ctx, bool vjp)
 // the register file (64 K per SM, allocated per warp in units of 256) admit; ties go to more CTAs (measured on C3,
 // profiles/r01_c: two co-resident CTAs beat one of twice the size -- their staging and epilogue phases overlap).
 static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, size_t static_smem, int max_warps, int regs,
-                            int *threads, TileSizes *ts, size_t *smem)
+                            int *threads, TileSizes *ts, size_t *smem, uint32_t halo_max = 0)
 {
-    ts->mcap = (int)((ctx->tile_Mmax + 7u) & ~7u);
+    // halo_max: the most halo particles a CTA stages (default: those of a whole tile)
+    ts->mcap = (int)(((halo_max ? halo_max : ctx->tile_Mmax) + 7u) & ~7u);
     ts->tcap = (int)((ctx->tile_Tmax + 7u) & ~7u);
     const double mean = ctx->n > 0 ? (double)ctx->nnz / (double)ctx->n : 1.0;
     int rb = (int)((32 / gs) * mean * 1.25) + 24;
@@ -1091,6 +1146,7 @@ static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, size_t 
     if (rb < 64) rb = 64;
     ts->rb = rb;
     ts->bulk = ctx->opt_stage_bulk;
+    ts->split = 1;
     const size_t fixed = (size_t)ts->mcap * state_bytes + (size_t)(ts->tcap + 4) * 4 + (size_t)ts->tcap * 2 + 16;
     const size_t sm_total = 233472, per_cta = 1024 + static_smem, cta_max = 232448 - static_smem;
     auto need = [&](int warps) { return fixed + (size_t)warps * 2 * rb * 2; };
@@ -1314,12 +1370,16 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
         int threads;
         TileSizes ts;
         size_t smem;
-        tile_launch_cfg(ctx, kp.dim == 3 ? (UMv ? 32 : 40) : 32, gs, sizeof(TileTab), kPtMaxWarps, 64, &threads, &ts, &smem);
+        const int split = ctx->opt_vjp_split >= 2 ? sph_vjp_tile_split(ctx, kp) : 1;
+        const unsigned grid = (unsigned)tg.ntiles * (unsigned)split;
+        tile_launch_cfg(ctx, kp.dim == 3 ? (UMv ? 32 : 40) : 32, gs, sizeof(TileTab), kPtMaxWarps, 64, &threads, &ts, &smem,
+                        split == 2 ? ctx->tile_Mhalf : 0u);
+        ts.split = split;
         if (pass == 1) ctx->launches += 1;                     // the second variant is a launch too
 #define SPH_RT_LAUNCH2(DIM, GS, VARH, SORTED, F1, UM)                                                                \
     do {                                                                                                             \
         SPH_TILE_SMEM_ATTR((k_rhs_tile<DIM, GS, VARH, SORTED, F1, UM>), smem);                                       \
-        k_rhs_tile<DIM, GS, VARH, SORTED, F1, UM><<<(unsigned)tg.ntiles, threads, smem, st>>>(                       \
+        k_rhs_tile<DIM, GS, VARH, SORTED, F1, UM><<<grid, threads, smem, st>>>(                                      \
             tg, kp, ts, s0, s1, s2, kind_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),            \
             ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), drho, acc, out4, um); \
     } while (0)
@@ -1356,6 +1416,12 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
     return SPH_OK;
 }
 
+// CTAs per tile of k_vjp_tile: 2 in 3D on 2x2x2-cell tiles (each CTA takes one z-layer of the block)
+int sph_vjp_tile_split(const sph_ctx *ctx, const KPar &kp)
+{
+    return (ctx->opt_vjp_split && kp.dim == 3 && ctx->tg.B == 2 && ctx->tile_Mhalf > 0) ? 2 : 1;
+}
+
 int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const float4 *s1, const float2 *s2,
                         const float4 *cot, const float4 *eos, float *xb, float *vb, float *rb, float4 *xb4, float4 *vb4,
                         float *partials, cudaStream_t st)
@@ -1365,18 +1431,21 @@ int sph_launch_vjp_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
     const bool sorted = xb4 != nullptr;
     const bool dual = kp.dim == 3 && kp.uniform_h && !ctx->opt_no_um;
     const uint32_t *um = dual ? sph_um_flag(ctx) : nullptr;
+    const int split = sph_vjp_tile_split(ctx, kp);
+    const unsigned grid = (unsigned)tg.ntiles * (unsigned)split;
     for (int pass = 0; pass < (dual ? 2 : 1); ++pass) {
         const bool UMv = dual && pass == 0;
         int threads;
         TileSizes ts;
         size_t smem;
         tile_launch_cfg(ctx, kp.dim == 3 ? (UMv ? 48 : 56) : 48, gs, sizeof(TileTab) + kVjpMaxWarps * kNPartT * 4, kVjpMaxWarps, 80, &threads,
-                        &ts, &smem);
+                        &ts, &smem, split == 2 ? ctx->tile_Mhalf : 0u);
+        ts.split = split;
         if (pass == 1) ctx->launches += 1;
 #define SPH_VT_LAUNCH2(DIM, GS, VARH, SORTED, F1, UM)                                                                 \
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_vjp_tile<DIM, GS, VARH, SORTED, F1, UM>), smem);                                        \
-        k_vjp_tile<DIM, GS, VARH, SORTED, F1, UM><<<(unsigned)tg.ntiles, threads, smem, st>>>(                        \
+        k_vjp_tile<DIM, GS, VARH, SORTED, F1, UM><<<grid, threads, smem, st>>>(                                       \
             tg, kp, ts, s0, s1, s2, cot, eos, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),           \
             ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), xb, vb, rb, xb4, vb4,  \
             partials, um);                                                                                            \

@@ -423,6 +423,35 @@ def test_uniform_mass_variant_and_general_variant_agree(sph):
                 sph.set_option(OPT_UNIFORM_MASS_PATH, 1)
 
 
+@pytest.mark.parametrize("case", ["C3p", "C3s", "fuzz3d"])
+def test_vjp_on_half_tiles_agrees_with_whole_tiles(sph, case):
+    """SPH_OPT_VJP_SPLIT (include/sph.h): in 3D on 2x2x2-cell tiles the adjoint kernel gives each CTA one z-layer of a tile
+    with the three layers of halo cells around it.  Every row still sums its own list in the same order, so x_bar, v_bar,
+    rho_bar are bit-identical to the one-CTA-per-tile launch; params_bar is reduced over twice as many partial records
+    (same terms, other grouping) and is held to the adjoint tolerance.  fuzz3d: bounded / odd cell counts, where a tile
+    may have a single layer."""
+    from paper_2507_21684_b200.binding import OPT_VJP_SPLIT
+    if case == "fuzz3d":
+        wl = next(w for w in (fuzz_workload(s, scale=1.0)[0] for s in range(40)) if w.dim == 3 and w.n > 1500)
+    else:
+        wl = CASES[case]()
+    lam, mu = W.random_cotangents(wl)
+    _, dev, _ = build(wl, 1.0, sph)
+    lam_d, mu_d = torch.from_numpy(lam).cuda(), torch.from_numpy(mu).cuda()
+    out = []
+    for split in (0, 1):
+        sph.set_option(OPT_VJP_SPLIT, split)
+        try:
+            out.append([_np(t).copy() for t in sph.rhs_vjp(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind, lam_d, mu_d)])
+        finally:
+            sph.set_option(OPT_VJP_SPLIT, 1)
+    for a, b in zip(out[0][:3], out[1][:3]):
+        assert np.array_equal(a, b)
+    assert _params_err(out[1][3], out[0][3].astype(np.float64)) < TOL_VJP
+    xo, vo, ro, po = oracle.rhs_vjp(wl.domain, wl.params, wl.x, wl.v, wl.rho, wl.m, wl.h, wl.kind, *oracle_lists(wl), lam, mu)
+    assert _params_err(out[1][3], po) < TOL_VJP
+
+
 @pytest.mark.parametrize("case", ["C1s", "C2p", "C3p", "C4s"])
 def test_bulk_copy_staging_is_bitwise_the_same(sph, case):
     """SPH_OPT_STAGE_BULK: the halo of a tile staged with cp.async.bulk + one mbarrier instead of per-particle cp.async
