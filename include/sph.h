@@ -297,6 +297,9 @@ enum {
                                a tile (one z-layer of its cells, staging the three layers of halo cells around it), so
                                that two CTAs are resident per SM and one stages while the other computes;
                                0: one CTA per tile (A/B measurement);  2: sph_rhs too (measured slower, A/B only) */
+    SPH_OPT_TILE_TABLES = 11, /* 1 (default): the per-tile tables (halo cell offsets, row ranges, periodic shifts) are computed
+                               once per neighbour build and loaded by every tile kernel;  0: every CTA derives them from
+                               the cell table again (A/B measurement) */
     SPH_OPT_RK_EXTRA_SKIN = 6 /* Verlet lists across steps: value/1000 = extra skin e (in units of h).  With
                                e > 0 sph_rk_step / sph_rk_step_vjp build their lists with search_scale = 1 + skin + e
                                (the domain's cell_size must cover it) and a later call with the same domain, n and h

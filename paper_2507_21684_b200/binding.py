@@ -23,7 +23,7 @@ EXPORTS = ("sph_create", "sph_destroy", "sph_build_cells", "sph_neighbors", "sph
 
 # keys of sph_set_option (enum SPH_OPT_* in include/sph.h)
 OPT_PAIR_GROUP, OPT_LIST_MODE, OPT_TILE_EDGE, OPT_PAIR_WARPS, OPT_FILL_MASKS, OPT_RK_EXTRA_SKIN = 1, 2, 3, 4, 5, 6
-OPT_UNIFORM_MASS_PATH, OPT_BUILD_FUSED, OPT_STAGE_BULK, OPT_VJP_SPLIT = 7, 8, 9, 10
+OPT_UNIFORM_MASS_PATH, OPT_BUILD_FUSED, OPT_STAGE_BULK, OPT_VJP_SPLIT, OPT_TILE_TABLES = 7, 8, 9, 10, 11
 LIST_AUTO, LIST_GENERIC, LIST_TILE = 0, 1, 2
 
 # kernel classes of sph_profile_read (enum SPH_K_* in include/sph.h)

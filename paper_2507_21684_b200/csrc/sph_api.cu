@@ -33,7 +33,7 @@ extern "C" int sph_destroy(sph_ctx *ctx)
     cudaDeviceSynchronize();
     DevBuf *bufs[] = {&ctx->key_a, &ctx->key_b, &ctx->idx_a, &ctx->idx_b, &ctx->hist, &ctx->perm, &ctx->inv_perm,
                       &ctx->key_sorted, &ctx->pos_s, &ctx->cell_start, &ctx->cell_end, &ctx->stats, &ctx->cnt,
-                      &ctx->row_ptr, &ctx->col, &ctx->col16, &ctx->scan_tmp, &ctx->maskbuf, &ctx->tile_words, &ctx->tile_mask_base, &ctx->fstats, &ctx->tstate, &ctx->fctl, &ctx->d_pos, &ctx->d_va, &ctx->d_mom, &ctx->d_g4, &ctx->d_lr, &ctx->d_dx4, &ctx->d_gb4, &ctx->d_rb, &ctx->d_rc, &ctx->d_rd, &ctx->d_re, &ctx->d_x2, &ctx->d_vb, &ctx->d_ab, &ctx->d_part, &ctx->tile_orders[0].buf, &ctx->tile_orders[1].buf, &ctx->tile_orders[2].buf, &ctx->tile_orders[3].buf, &ctx->s0, &ctx->s1, &ctx->s2, &ctx->s3, &ctx->c0buf,
+                      &ctx->row_ptr, &ctx->col, &ctx->col16, &ctx->scan_tmp, &ctx->maskbuf, &ctx->tile_words, &ctx->tile_mask_base, &ctx->fstats, &ctx->tstate, &ctx->fctl, &ctx->tile_tabs, &ctx->d_pos, &ctx->d_va, &ctx->d_mom, &ctx->d_g4, &ctx->d_lr, &ctx->d_dx4, &ctx->d_gb4, &ctx->d_rb, &ctx->d_rc, &ctx->d_rd, &ctx->d_re, &ctx->d_x2, &ctx->d_vb, &ctx->d_ab, &ctx->d_part, &ctx->tile_orders[0].buf, &ctx->tile_orders[1].buf, &ctx->tile_orders[2].buf, &ctx->tile_orders[3].buf, &ctx->s0, &ctx->s1, &ctx->s2, &ctx->s3, &ctx->c0buf,
                       &ctx->out4, &ctx->m_s, &ctx->kind_s, &ctx->partials, &ctx->eos, &ctx->hx, &ctx->hv, &ctx->hrho,
                       &ctx->hm, &ctx->hh, &ctx->hkind, &ctx->hlam, &ctx->hmu, &ctx->ho_drho, &ctx->ho_acc, &ctx->ho_xb,
                       &ctx->ho_vb, &ctx->ho_rb, &ctx->ho_pb, &ctx->ho_dens};
@@ -315,6 +315,9 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
         return SPH_OK;
     case SPH_OPT_STAGE_BULK:
         ctx->opt_stage_bulk = value != 0;
+        return SPH_OK;
+    case SPH_OPT_TILE_TABLES:
+        ctx->opt_tile_tables = value != 0;
         return SPH_OK;
     case SPH_OPT_VJP_SPLIT:
         if (value < 0 || value > 2) return SPH_E_INVALID;

@@ -76,6 +76,7 @@ struct TileGeom {
     int ncell[3];
     int periodic[3];
     float L[3];
+    const void *tabs;  // device TileTab[ntiles] written once per build (k_tile_tables), or NULL: every CTA derives its own
 };
 
 // Per-launch physical constants (derived once on the host from sph_params).
@@ -137,6 +138,7 @@ struct sph_ctx {
     int opt_fused_warps = 0;    // warps per CTA of the one-kernel build (0 = default)
     int opt_build_fused = 1;    // 1: the tile-local lists are built by the one-kernel build (sph_neighbors_fused.cu) when a tile fits it
     int opt_stage_bulk = 0;     // 1: k_rhs_tile / k_vjp_tile stage their float4 halo arrays with cp.async.bulk + one mbarrier (measured: profiles/r02_f)
+    int opt_tile_tables = 1;    // 1: the tables of a tile are computed once per build and loaded by the tile kernels
     int opt_vjp_split = 1;      // 1: k_vjp_tile works on half a 2x2x2 tile per CTA (two resident CTAs per SM instead of one)
     int opt_no_um = 0;          // 1: never launch the uniform-mass variants of the tile pair kernels (A/B measurements, tests)
     bool tile_mode = false;     // lists of the last sph_neighbors are tile-local (col16)
@@ -166,6 +168,7 @@ struct sph_ctx {
     DevBuf maskbuf, tile_words, tile_mask_base;   // hit masks of the count pass, per-tile mask offsets
     // one-kernel build: cell statistics, look-back states, {ticket, overflow}, tiles in Morton order (cached per grid)
     DevBuf fstats, tstate, fctl;
+    DevBuf tile_tabs;           // TileTab of every tile of the last build (sph_tiles.cuh)
     const float4 *pos_override = nullptr;         // sph_shift: sph_grad_sum's kernels read these positions instead of pos_s
     // delta_form 1: current positions {x,y,z,h}, {V,rho}, moments, {g,V}, adjoint records and sorted partial results
     DevBuf d_pos, d_va, d_mom, d_g4, d_lr, d_dx4, d_gb4, d_rb, d_rc, d_rd, d_re, d_x2, d_vb, d_ab, d_part;

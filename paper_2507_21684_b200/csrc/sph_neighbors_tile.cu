@@ -500,6 +500,18 @@ __global__ void k_tile_stats(TileGeom tg, const uint32_t *__restrict__ cell_star
     }
 }
 
+// tables of every tile, once per build: the tile kernels then load theirs instead of deriving it (sph_tiles.cuh)
+template <int DIM>
+__global__ void __launch_bounds__(64)
+k_tile_tables(TileGeom tg, const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end, TileTab *__restrict__ out)
+{
+    __shared__ TileTab tt;
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);          // tg.tabs is NULL here
+    const uint32_t *src = reinterpret_cast<const uint32_t *>(&tt);
+    uint32_t *dst = reinterpret_cast<uint32_t *>(out + blockIdx.x);
+    for (int i = threadIdx.x; i < (int)(sizeof(TileTab) / 4); i += blockDim.x) dst[i] = src[i];
+}
+
 // ---------------------------------------------------------------------------------------- col16 -> sorted ids
 // (export and the generic pair kernels only) one CTA per tile; rows of a tile are contiguous
 template <int DIM>
@@ -604,7 +616,16 @@ int sph_neighbors_tile_run(sph_ctx *ctx, const SearchPar &sp, int B, uint32_t Mm
 {
     const int64_t n = ctx->n;
     const GridGeom &gg = ctx->geom;
-    const TileGeom tg = make_tile_geom(gg, B);
+    TileGeom tg = make_tile_geom(gg, B);
+    if (ctx->opt_tile_tables) {
+        SPH_TRY(ctx->tile_tabs.reserve((size_t)tg.ntiles * sizeof(TileTab)));
+        KScope ks(ctx, SPH_K_COUNT, 1, st);
+        if (gg.dim == 3)
+            k_tile_tables<3><<<(unsigned)tg.ntiles, 64, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), ctx->tile_tabs.as<TileTab>());
+        else
+            k_tile_tables<2><<<(unsigned)tg.ntiles, 64, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(), ctx->tile_tabs.as<TileTab>());
+        tg.tabs = ctx->tile_tabs.p;
+    }
     if (ctx->opt_build_fused && ctx->f_ncmax) {
         // the one-kernel build (sph_neighbors_fused.cu); 1 = a tile does not fit its shared-memory carve-up
         const int rc = sph_neighbors_fused_run(ctx, sp, tg, Mmax, Tmax, ctx->f_ncmax, ctx->f_pairs, st, nnz_out);

@@ -37,6 +37,16 @@ __device__ __forceinline__ void tile_setup(const TileGeom &tg, int tile, const u
                                            const uint32_t *__restrict__ cell_end, TileTab &tt)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (tg.tabs) {
+        // the tables of this tile were written at build time (k_tile_tables): one coalesced read instead of the cell-table
+        // look-ups, two scans and three barriers below
+        static_assert(sizeof(TileTab) % 4 == 0, "TileTab is copied word by word");
+        const uint32_t *src = reinterpret_cast<const uint32_t *>(static_cast<const TileTab *>(tg.tabs) + tile);
+        uint32_t *dst = reinterpret_cast<uint32_t *>(&tt);
+        for (int i = threadIdx.x; i < (int)(sizeof(TileTab) / 4); i += blockDim.x) dst[i] = __ldg(src + i);
+        __syncthreads();
+        return;
+    }
     if (threadIdx.x == 0) {
         int b = tile, bc[3] = {0, 0, 0};
         bc[0] = b % tg.nb[0];
