@@ -62,43 +62,48 @@ __global__ void k_wrap_key(const float *__restrict__ x, const float *__restrict_
 }
 
 // ------------------------------------------------------------------------------------------ N2
-// Stable LSD radix sort, 8-bit digits.  Each warp owns a contiguous chunk of kChunk keys and ranks them
+// Stable LSD radix sort, digits of up to kRsMaxBits bits (the host picks the fewest passes that cover the key, then the
+// narrowest digit for that many passes).  Each warp owns a contiguous chunk of kChunk keys and ranks them
 // round by round (32 keys per round) with __match_any_sync, so equal keys keep their input order.
 constexpr int kRsWarps = 8;
 constexpr int kRsItems = 16;
 constexpr int kChunk = 32 * kRsItems;
+constexpr int kRsMaxBits = 9;
+constexpr int kRsMaxBins = 1 << kRsMaxBits;
 
 __global__ void __launch_bounds__(kRsWarps * 32)
-k_radix_hist(const uint32_t *__restrict__ key, int64_t n, int shift, int64_t nchunks, uint32_t *__restrict__ hist)
+k_radix_hist(const uint32_t *__restrict__ key, int64_t n, int shift, int bits, int64_t nchunks, uint32_t *__restrict__ hist)
 {
-    __shared__ uint32_t cnt[kRsWarps][256];
+    __shared__ uint32_t cnt[kRsWarps][kRsMaxBins];
+    const uint32_t bins = 1u << bits, mask = bins - 1u;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t chunk = (int64_t)blockIdx.x * kRsWarps + warp;
-    for (int d = lane; d < 256; d += 32) cnt[warp][d] = 0;
+    for (uint32_t d = lane; d < bins; d += 32) cnt[warp][d] = 0;
     __syncwarp();
     if (chunk < nchunks) {
         const int64_t base = chunk * kChunk;
         for (int r = 0; r < kRsItems; ++r) {
             int64_t i = base + r * 32 + lane;
-            uint32_t d = i < n ? ((key[i] >> shift) & 255u) : 256u;
+            uint32_t d = i < n ? ((key[i] >> shift) & mask) : bins;
             uint32_t peers = __match_any_sync(0xffffffffu, d);
-            if (d < 256u && (peers & ((1u << lane) - 1u)) == 0u) cnt[warp][d] += __popc(peers);
+            if (d < bins && (peers & ((1u << lane) - 1u)) == 0u) cnt[warp][d] += __popc(peers);
             __syncwarp();
         }
-        for (int d = lane; d < 256; d += 32) hist[(int64_t)d * nchunks + chunk] = cnt[warp][d];
+        for (uint32_t d = lane; d < bins; d += 32) hist[(int64_t)d * nchunks + chunk] = cnt[warp][d];
     }
 }
 
 __global__ void __launch_bounds__(kRsWarps * 32)
 k_radix_scatter(const uint32_t *__restrict__ key_in, const uint32_t *__restrict__ val_in,
-                uint32_t *__restrict__ key_out, uint32_t *__restrict__ val_out, int64_t n, int shift,
+                uint32_t *__restrict__ key_out, uint32_t *__restrict__ val_out, int64_t n, int shift, int bits,
                 int64_t nchunks, const uint32_t *__restrict__ hist_scanned)
 {
-    __shared__ uint32_t off[kRsWarps][256];
+    __shared__ uint32_t off[kRsWarps][kRsMaxBins];
+    const uint32_t bins = 1u << bits, mask = bins - 1u;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t chunk = (int64_t)blockIdx.x * kRsWarps + warp;
     if (chunk >= nchunks) return;
-    for (int d = lane; d < 256; d += 32) off[warp][d] = hist_scanned[(int64_t)d * nchunks + chunk];
+    for (uint32_t d = lane; d < bins; d += 32) off[warp][d] = hist_scanned[(int64_t)d * nchunks + chunk];
     __syncwarp();
     const int64_t base = chunk * kChunk;
     for (int r = 0; r < kRsItems; ++r) {
@@ -106,7 +111,7 @@ k_radix_scatter(const uint32_t *__restrict__ key_in, const uint32_t *__restrict_
         bool live = i < n;
         uint32_t k = live ? key_in[i] : 0u;
         uint32_t v = live ? (val_in ? val_in[i] : (uint32_t)i) : 0u;
-        uint32_t d = live ? ((k >> shift) & 255u) : 256u;
+        uint32_t d = live ? ((k >> shift) & mask) : bins;
         uint32_t peers = __match_any_sync(0xffffffffu, d);
         uint32_t lower = peers & ((1u << lane) - 1u);
         uint32_t pos = 0;
@@ -366,7 +371,7 @@ extern "C" int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float 
     SPH_TRY(ctx->key_b.reserve((size_t)n * 4));
     SPH_TRY(ctx->idx_a.reserve((size_t)n * 4));
     SPH_TRY(ctx->idx_b.reserve((size_t)n * 4));
-    SPH_TRY(ctx->hist.reserve((size_t)nchunks * 256 * 4));
+    SPH_TRY(ctx->hist.reserve((size_t)nchunks * kRsMaxBins * 4));
     SPH_TRY(ctx->perm.reserve((size_t)n * 4));
     SPH_TRY(ctx->inv_perm.reserve((size_t)n * 4));
     SPH_TRY(ctx->pos_s.reserve((size_t)n * 16));
@@ -387,16 +392,17 @@ extern "C" int sph_build_cells(sph_ctx *ctx, const sph_domain *dom, const float 
 
     // LSD radix passes over the used key bits
     const int keybits = gg.bits * gg.dim;
-    const int passes = (keybits + 7) / 8;
+    const int passes = (keybits + kRsMaxBits - 1) / kRsMaxBits;
+    const int dbits = (keybits + passes - 1) / passes;           // <= kRsMaxBits
     uint32_t *kin = ctx->key_a.as<uint32_t>(), *kout = ctx->key_b.as<uint32_t>();
     uint32_t *vin = nullptr, *vout = ctx->idx_b.as<uint32_t>();
     uint32_t *vother = ctx->idx_a.as<uint32_t>();
     const unsigned rblk = (unsigned)((nchunks + kRsWarps - 1) / kRsWarps);
     for (int p = 0; p < passes; ++p) {
         KScope ks(ctx, SPH_K_SORT, 5, st);
-        k_radix_hist<<<rblk, kRsWarps * 32, 0, st>>>(kin, n, 8 * p, nchunks, ctx->hist.as<uint32_t>());
-        SPH_TRY(sph_scan_u32(ctx, ctx->hist.as<uint32_t>(), ctx->hist.p, false, nchunks * 256, st));
-        k_radix_scatter<<<rblk, kRsWarps * 32, 0, st>>>(kin, vin, kout, vout, n, 8 * p, nchunks, ctx->hist.as<uint32_t>());
+        k_radix_hist<<<rblk, kRsWarps * 32, 0, st>>>(kin, n, dbits * p, dbits, nchunks, ctx->hist.as<uint32_t>());
+        SPH_TRY(sph_scan_u32(ctx, ctx->hist.as<uint32_t>(), ctx->hist.p, false, nchunks << dbits, st));
+        k_radix_scatter<<<rblk, kRsWarps * 32, 0, st>>>(kin, vin, kout, vout, n, dbits * p, dbits, nchunks, ctx->hist.as<uint32_t>());
         uint32_t *t = kin;
         kin = kout;
         kout = t;
