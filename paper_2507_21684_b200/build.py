@@ -3,7 +3,7 @@
     python -m paper_2507_21684_b200.build [--force] [--verbose] [--bounds]
 
 --bounds: debug build with -DSPH_BOUNDS (checked shared-memory indices in the tile kernels, sph_internal.cuh); it
-replaces the library in place, so rebuild with --force afterwards.
+replaces the library in place; the next plain build (or __graft_entry__.build()) notices and rebuilds the normal one.
 
 nvcc cross-compiles without a GPU.  No --use_fast_math: the neighbour predicate and the position wrap
 are fixed sequences of IEEE operations (readings R3/R4); fast approximations are used
@@ -18,6 +18,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsph_b200.so")
+STAMP = os.path.join(HERE, "_obj", "flavour.txt")     # "normal" or "bounds": what the library in place was built as
 
 
 def sources():
@@ -26,6 +27,11 @@ def sources():
 
 def _stale():
     if not os.path.exists(LIB):
+        return True
+    try:
+        if open(STAMP).read().strip() != "normal":        # a --bounds debug library was left in place
+            return True
+    except OSError:
         return True
     t = os.path.getmtime(LIB)
     deps = sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(HERE, "..", "include", "sph.h")]
@@ -60,6 +66,9 @@ def build(force: bool = False, verbose: bool = False, bounds: bool = False) -> s
         if r.returncode != 0:
             raise subprocess.CalledProcessError(r.returncode, r.args)
     subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs, check=True)
+    os.makedirs(os.path.dirname(STAMP), exist_ok=True)
+    with open(STAMP, "w") as f:
+        f.write("bounds\n" if bounds else "normal\n")
     return LIB
 
 
