@@ -28,7 +28,7 @@
 
 namespace {
 
-constexpr int kFWmax = 12;             // warps per CTA (launch bound)
+constexpr int kFWmax = 16;             // warps per CTA (launch bound)
 constexpr int kRowLanes = 4;           // lanes that share a row in the expansion (phase 3)
 constexpr int kCPL = 4;                // candidates per lane in the test loop
 constexpr int kCandBlock = 32 * kCPL;  // candidates per work unit
@@ -197,7 +197,7 @@ size_t fused_smem_bytes(const FusedSizes &fs)
 // ---------------------------------------------------------------------------------------------------- the kernel
 // ctl[0] = ticket counter, ctl[1] = overflow flag (col16 too small: lists not written, counts still exact)
 template <int DIM, bool VARH>
-__global__ void __launch_bounds__(kFWmax * 32)
+__global__ void __launch_bounds__(kFWmax * 32, 2)
 k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, const float4 *__restrict__ pos_s,
            const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
            const uint32_t *__restrict__ tile_order, uint32_t *__restrict__ ctl, unsigned long long *__restrict__ tstate,
