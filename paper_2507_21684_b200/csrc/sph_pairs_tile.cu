@@ -300,11 +300,12 @@ struct SmemMap {
     float2 *C;
     uint32_t *rp;
     uint16_t *selfq, *ring;
-    __device__ SmemMap(unsigned char *base, const TileSizes &ts, bool with_cot, bool with_C = true)
+    // b_bytes: bytes per halo particle of the B slot (16; 4 when a kernel keeps one float there, as the density does)
+    __device__ SmemMap(unsigned char *base, const TileSizes &ts, bool with_cot, bool with_C = true, int b_bytes = 16)
     {
         size_t o = 0;
         A = reinterpret_cast<float4 *>(base + o); o += (size_t)ts.mcap * 16;
-        B = reinterpret_cast<float4 *>(base + o); o += (size_t)ts.mcap * 16;
+        B = reinterpret_cast<float4 *>(base + o); o += (size_t)ts.mcap * b_bytes;
         cot = reinterpret_cast<float4 *>(base + o); if (with_cot) o += (size_t)ts.mcap * 16;
         C = reinterpret_cast<float2 *>(base + o); if (DIM == 3 && with_C) o += (size_t)ts.mcap * 8;
         rp = reinterpret_cast<uint32_t *>(base + o); o += (size_t)(ts.tcap + 4) * 4;
@@ -324,7 +325,7 @@ k_density_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ po
                const uint32_t *__restrict__ perm, float *__restrict__ rho_out)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const SmemMap<DIM> sm(smem_raw, ts, false);
+    const SmemMap<DIM> sm(smem_raw, ts, false, false, 4);     // 20 bytes per halo particle: three CTAs per SM at C3
     float *Ms = reinterpret_cast<float *>(sm.B);
     __shared__ TileTab tt;
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
@@ -1182,7 +1183,7 @@ int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, floa
     int threads;
     TileSizes ts;
     size_t smem;
-    tile_launch_cfg(ctx, kp.dim == 3 ? 40 : 32, gs, sizeof(TileTab), kPtMaxWarps, 64, &threads, &ts, &smem);   // same carve-up as the RHS kernel (SmemMap)
+    tile_launch_cfg(ctx, 20, gs, sizeof(TileTab), kPtMaxWarps, 40, &threads, &ts, &smem);   // {x,y,z,h} + m per halo particle; every variant compiles to <= 40 registers
 #define SPH_DT_LAUNCH(DIM, GS, VARH)                                                                                  \
     do {                                                                                                              \
         SPH_TILE_SMEM_ATTR((k_density_tile<DIM, GS, VARH>), smem);                                                    \
