@@ -248,7 +248,12 @@ __device__ __forceinline__ void tile_row_passes(const TileTab &tt, const uint32_
             if (fits) {
                 const uint16_t *src = seg + (size_t)c0 * 8;
                 const uint32_t dst = ring_s + (uint32_t)(buf * rb) * 2u;
-                for (uint32_t c = lane; c < nchunk; c += 32) cp_async16(dst + c * 16u, src + c * 8u);
+                // a segment is rarely longer than 64 chunks: two copies per lane at fixed offsets from one address pair
+                const uint16_t *src_l = src + (size_t)lane * 8;
+                const uint32_t dst_l = dst + (uint32_t)lane * 16u;
+                if ((uint32_t)lane < nchunk) cp_async16(dst_l, src_l);
+                if ((uint32_t)lane + 32u < nchunk) cp_async16(dst_l + 512u, src_l + 256);
+                for (uint32_t c = lane + 64; c < nchunk; c += 32) cp_async16(dst + c * 16u, src + c * 8u);
             }
         }
         cp_async_commit();
