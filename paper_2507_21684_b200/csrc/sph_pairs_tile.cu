@@ -120,15 +120,19 @@ __device__ __forceinline__ void stage_halo(const TileTab &tt, const float4 *__re
     }
     for (int hc = hc_lo + warp; hc < hc_hi; hc += nwarps) {
         const uint32_t o0 = tt.h_off[hc], cnt = tt.h_off[hc + 1] - o0, gs = tt.h_start[hc];
-        for (uint32_t l = lane; l < cnt; l += 32) {
-            const uint32_t q = o0 + l;
-            const size_t g = (size_t)gs + l;
+        auto copy = [&](uint32_t q, size_t g) {
             if (g0) cp_async16(a0 + q * 16, g0 + g);
             if (g1) cp_async16(a1 + q * 16, g1 + g);
             if (g2) cp_async16(a2 + q * 16, g2 + g);
             if (gc) cp_async8(ac + q * 8, gc + g);
             if (gf) cp_async4(af + q * 4, gf + g);
-        }
+        };
+        // a cell rarely holds more than 64 particles: two rounds at fixed offsets from one set of addresses, then the rest
+        const uint32_t q = o0 + lane;
+        const size_t g = (size_t)gs + lane;
+        if ((uint32_t)lane < cnt) copy(q, g);
+        if ((uint32_t)lane + 32u < cnt) copy(q + 32u, g + 32);
+        for (uint32_t l = lane + 64; l < cnt; l += 32) copy(o0 + l, (size_t)gs + l);
     }
     cp_async_commit();
 }
