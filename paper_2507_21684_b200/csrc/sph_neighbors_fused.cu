@@ -209,14 +209,17 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
     // per target cell: candidates, first row pair, first row (relative to the tile's first SORTED row: the rows of a tile
     // follow the Morton order of its cells, not the raster order of the target-cell table)
     __shared__ uint32_t c_nc[kTileMaxTgt], c_pb[kTileMaxTgt + 1], c_rb[kTileMaxTgt], c_ub[kTileMaxTgt + 1];
-    __shared__ uint32_t s_ticket, s_tot, s_grp;
+    __shared__ uint32_t s_ticket, s_tot, s_grp, s_hits;
     __shared__ volatile uint32_t s_ready;                    // set once the look-back has produced s_base
+    __shared__ volatile uint32_t s_off_ready;                // set once off[] (the row offsets of the tile) is complete
     __shared__ long long s_base;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, kFW = blockDim.x >> 5;
     if (threadIdx.x == 0) {
         s_ticket = atomicAdd(&ctl[0], 1u);
         s_grp = 0;
         s_ready = 0;
+        s_off_ready = 0;
+        s_hits = 0;
     }
     __syncthreads();
     const uint32_t ticket = s_ticket;
@@ -309,6 +312,7 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
         // units are dealt round-robin; inside a cell the candidate block runs fastest, so the (smaller) units of a
         // cell's last row chunk spread over the warps like the full ones
         int tc = 0;
+        uint32_t my_hits = 0;                               // hits of the lane's candidates: the tile's total is known after phase 1
         for (uint32_t unit = warp; unit < c_ub[tt.nt]; unit += kFW) {
                 {
                     while (unit >= c_ub[tc + 1]) ++tc;
@@ -423,6 +427,8 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
                         if (w * 32u >= Nc) continue;                       // uniform: no valid candidate in this word
                         SPH_ASSERT(w < (uint32_t)fs.wcap && row_base + nr <= (uint32_t)tcap);
                         uint32_t *mw = sm.masks + (size_t)w * tcap + row_base;
+                        // rows i < nr1 sit at bits 2 np1 - 1 - i (the duplicate of an odd last row below them is not a row)
+                        my_hits += (uint32_t)__popc(rb[k] >> (2u * np1 - nr1)) + (nr2 ? (uint32_t)__popc(rb2[k] >> (2u * np2 - nr2)) : 0u);
                         const uint32_t y = warp_transpose32(rb[k]);
                         if (islot >= 0 && (uint32_t)islot < nr1) mw[islot] = y;
                         if (nr2 > 8u) {
@@ -437,11 +443,25 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
                     }
                 }
         }
+        my_hits = __reduce_add_sync(0xffffffffu, my_hits);
+        if (lane == 0 && my_hits) atomicAdd(&s_hits, my_hits);
     }
-    __syncthreads();
+    __syncthreads();                                          // masks complete, s_hits = entries of the tile
 
-    // ---- phase 2: counts, offsets; the tile's base comes from the look-back, which only warp 0 waits for
-    for (uint32_t r = threadIdx.x; r < T; r += blockDim.x) {
+    // ---- phase 2: warp 0 looks back for the tile's base (its total is known already) WHILE the other warps count the
+    // rows, split them for phase 3 and scan the counts; they meet at a barrier of their own, warp 0 joins phase 3 when the
+    // base is there.
+    const uint32_t tot = s_hits;
+    if (warp == 0) {
+        const long long b = tile_lookback(tstate, ticket, tot);
+        if (lane == 0) {
+            s_base = b;
+            __threadfence_block();
+            s_ready = 1u;
+        }
+    } else {
+    const uint32_t nthr2 = blockDim.x - 32u;
+    for (uint32_t r = threadIdx.x - 32u; r < T; r += nthr2) {
         // the row's mask words are split among its four lanes of phase 3 at word boundaries, by HITS (the words of the
         // middle plane of the neighbourhood hold twice the hits of the outer ones): lane q starts at the first word at
         // which the running count reaches q/4 of the total
@@ -465,8 +485,8 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
         }
         sm.off[r] = c;
     }
-    __syncthreads();
-    if (warp == 0) {
+    asm volatile("bar.sync 1, %0;" ::"r"(nthr2) : "memory");    // warps 1 .. kFW-1: counts complete
+    if (warp == 1) {
         uint32_t carry = 0;
         for (uint32_t r0 = 0; r0 < T; r0 += 32) {
             const uint32_t r = r0 + lane;
@@ -484,16 +504,18 @@ k_nb_fused(TileGeom tg, GridGeom gg, SearchPar sp, FusedSizes fs, long long n, c
             sm.off[T] = carry;
             s_tot = carry;
         }
-    }
-    __syncthreads();                                          // off[] complete: the last block-wide barrier
-    const uint32_t tot = s_tot;
-    if (warp == 0) {
-        const long long b = tile_lookback(tstate, ticket, tot);
+        __syncwarp();
         if (lane == 0) {
-            s_base = b;
+            SPH_ASSERT(s_tot == tot);
             __threadfence_block();
-            s_ready = 1u;
+            s_off_ready = 1u;
         }
+    }
+    asm volatile("bar.sync 1, %0;" ::"r"(nthr2) : "memory");    // off[] complete for the warps that wrote it
+    }
+    if (warp == 0) {
+        while (s_off_ready == 0u) __nanosleep(100);
+        __threadfence_block();
     }
 
     // ---- phase 3: masks -> halo indices.  Groups of 8 consecutive rows, handed out to the warps by a shared counter; a
