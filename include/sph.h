@@ -296,7 +296,8 @@ enum {
     SPH_OPT_VJP_SPLIT = 10, /* 1 (default): in 3D on 2x2x2-cell tiles the adjoint pair kernel of sph_rhs_vjp gives each CTA HALF
                                a tile (one z-layer of its cells, staging the three layers of halo cells around it), so
                                that two CTAs are resident per SM and one stages while the other computes;
-                               0: one CTA per tile (A/B measurement);  2: sph_rhs too (measured slower, A/B only) */
+                               0: one CTA per tile (A/B measurement).  (The same split of the forward kernel was
+                               measured slower and is not built in: profiles/r02_h.) */
     SPH_OPT_TILE_TABLES = 11, /* 1 (default): the per-tile tables (halo cell offsets, row ranges, periodic shifts) are computed
                                once per neighbour build and loaded by every tile kernel;  0: every CTA derives them from
                                the cell table again (A/B measurement) */

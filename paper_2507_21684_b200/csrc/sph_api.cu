@@ -320,8 +320,7 @@ extern "C" int sph_set_option(sph_ctx *ctx, int key, int value)
         ctx->opt_tile_tables = value != 0;
         return SPH_OK;
     case SPH_OPT_VJP_SPLIT:
-        if (value < 0 || value > 2) return SPH_E_INVALID;
-        ctx->opt_vjp_split = value;
+        ctx->opt_vjp_split = value != 0;
         return SPH_OK;
     case SPH_OPT_UNIFORM_MASS_PATH:
         ctx->opt_no_um = value == 0;

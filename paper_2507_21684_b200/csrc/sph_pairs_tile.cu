@@ -690,28 +690,29 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const SmemMap<DIM> sm(smem_raw, ts, false, !UM);
     __shared__ TileTab tt;
-    tile_setup<DIM>(tg, tile_of_block<DIM>(ts), cell_start, cell_end, tt);
-    const TilePart tp = tile_part<DIM>(tt, ts);
-    if (tp.row_hi <= tp.row_lo) return;
+    // whole tiles: half tiles (k_vjp_tile) were measured for this kernel twice and cost more staging than the third
+    // resident CTA hides (profiles/r02_h, r02_i); without them the gathers need no index offset
+    tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
+    if (tt.T == 0) return;
     __shared__ uint64_t mbar;
-    const bool bulk = ts.bulk && ts.split != 2;
+    const bool bulk = ts.bulk != 0;
     if (bulk) {
         if (threadIdx.x == 0) mbar_init(&mbar, 1);
         __syncthreads();
     }
     stage_halo(tt, s0, sm.A, s1, sm.B, nullptr, nullptr, (DIM == 3 && !UM) ? s2 : nullptr, sm.C, nullptr, nullptr,
-               bulk ? &mbar : nullptr, tp.hc_lo, tp.hc_hi, tp.q_lo);
+               bulk ? &mbar : nullptr);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
     cp_async_wait<0>();
     if (bulk) mbar_wait(&mbar, 0);
     __syncthreads();
-    stage_shift<DIM>(tt, sm.A, tp.hc_lo, tp.hc_hi, tp.q_lo);
+    stage_shift<DIM>(tt, sm.A);
     const int gl = (threadIdx.x & 31) % GS;
     const HC hu = hc_uniform<DIM>(kp);
     const float rho0 = kp.rho0;
     const float umG = m0 * hu.cG, umG5 = umG * 5.0f * hu.invH;      // uniform mass: m0 G = (umG + umG5 r) (1-q)^5
-    const float4 *A = sm.A - tp.q_lo, *B = sm.B - tp.q_lo;
-    const float2 *C = sm.C - tp.q_lo;
+    const float4 *A = sm.A, *B = sm.B;
+    const float2 *C = sm.C;
     const uint16_t *selfq = sm.selfq;
     const uint32_t row0 = tt.row0;
     tile_row_passes<GS>(tt, sm.rp, sm.ring, ts.rb, col16, row_ptr[tt.row0],
@@ -726,7 +727,7 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
 #pragma unroll 2
             for (uint32_t k = b + gl; k < e; k += GS) {
                 const uint32_t j = idx[k];
-                SPH_ASSERT(j >= tp.q_lo && j < tp.q_hi);
+                SPH_ASSERT(j < tt.M);
                 const Part pj = load_part<DIM, UM>(A, B, C, j, m0, kp.H);
                 const float d0 = pi.x[0] - pj.x[0], d1 = pi.x[1] - pj.x[1], d2 = DIM == 3 ? pi.x[2] - pj.x[2] : 0.f;
                 const float r2 = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
@@ -785,7 +786,7 @@ k_rhs_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ s0, co
                     else if (q < DIM) acc_out[i * DIM + q] = val;
                 }
             }
-        }, tp.row_lo, tp.row_hi);
+        });
 }
 
 // ------------------------------------------------------------------------------------------ B1: VJP
@@ -1380,11 +1381,8 @@ int sph_launch_rhs_tile(sph_ctx *ctx, const KPar &kp, const float4 *s0, const fl
         int threads;
         TileSizes ts;
         size_t smem;
-        const int split = ctx->opt_vjp_split >= 2 ? sph_vjp_tile_split(ctx, kp) : 1;
-        const unsigned grid = (unsigned)tg.ntiles * (unsigned)split;
-        tile_launch_cfg(ctx, kp.dim == 3 ? (UMv ? 32 : 40) : 32, gs, sizeof(TileTab), kPtMaxWarps, 64, &threads, &ts, &smem,
-                        split == 2 ? ctx->tile_Mhalf : 0u);
-        ts.split = split;
+        const unsigned grid = (unsigned)tg.ntiles;
+        tile_launch_cfg(ctx, kp.dim == 3 ? (UMv ? 32 : 40) : 32, gs, sizeof(TileTab), kPtMaxWarps, 64, &threads, &ts, &smem);
         if (pass == 1) ctx->launches += 1;                     // the second variant is a launch too
 #define SPH_RT_LAUNCH2(DIM, GS, VARH, SORTED, F1, UM)                                                                \
     do {                                                                                                             \
