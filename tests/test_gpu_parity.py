@@ -453,6 +453,32 @@ def test_vjp_on_half_tiles_agrees_with_whole_tiles(sph, case):
 
 
 @pytest.mark.parametrize("case", ["C1s", "C2p", "C3p", "C4s"])
+def test_tile_tables_loaded_or_derived_give_the_same_results(sph, case):
+    """SPH_OPT_TILE_TABLES (include/sph.h): the tables of a tile are written once per build and loaded by the tile kernels
+    (default), or derived by every CTA from the cell table.  Same tables either way: lists, density, RHS and VJP must
+    agree bit for bit."""
+    from paper_2507_21684_b200.binding import OPT_TILE_TABLES
+    wl = CASES[case]()
+    lam, mu = W.random_cotangents(wl)
+    lam_d, mu_d = torch.from_numpy(lam).cuda(), torch.from_numpy(mu).cuda()
+    out = []
+    for tables in (1, 0):
+        sph.set_option(OPT_TILE_TABLES, tables)
+        try:
+            _, dev, nnz = build(wl, 1.0, sph)
+            rp, ci = sph.neighbors_export()
+            dens = sph.density(dev.m)
+            drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind)
+            xb, vb, rb, pb = sph.rhs_vjp(wl.params, dev.x, dev.v, dev.rho, dev.m, dev.kind, lam_d, mu_d)
+            out.append([nnz] + [_np(t).copy() for t in (rp, ci, dens, drho, acc, xb, vb, rb, pb)])
+        finally:
+            sph.set_option(OPT_TILE_TABLES, 1)
+    assert out[0][0] == out[1][0]
+    for a, b in zip(out[0][1:], out[1][1:]):
+        assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("case", ["C1s", "C2p", "C3p", "C4s"])
 def test_bulk_copy_staging_is_bitwise_the_same(sph, case):
     """SPH_OPT_STAGE_BULK: the halo of a tile staged with cp.async.bulk + one mbarrier instead of per-particle cp.async
     (include/sph.h).  The staged bytes are the same, so RHS and VJP must agree bit for bit with the default path."""
