@@ -289,7 +289,9 @@ enum {
                                enqueued in two variants -- one that assumes all masses equal and gathers 32 / 48
                                instead of 40 / 56 bytes per pair, one general -- and a device flag written by this
                                call's own pack kernel decides which of them runs (no host synchronisation);
-                               0: only the general variant is launched */
+                               sph_density does the same with a flag of its own (written by its mass gather): the
+                               uniform-mass variant neither stages nor gathers the masses.
+                               0: only the general variants are launched */
     SPH_OPT_STAGE_BULK = 9, /* 0 (default): the tile pair kernels stage a halo with one 16-byte cp.async per particle and
                                array; 1: sph_rhs / sph_rhs_vjp stage their float4 arrays with one cp.async.bulk per halo
                                cell and array, completing on one mbarrier per CTA (A/B measurement) */

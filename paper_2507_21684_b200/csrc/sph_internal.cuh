@@ -206,6 +206,7 @@ struct sph_ctx {
 // (float bits).  Written on the stream by the pack kernels (k_pack_state, k_rk_base), read by the pair kernels: the
 // host never needs to know -- both variants of a pair kernel are launched and the one whose turn it is not returns.
 constexpr int kUmSlot = 13;
+constexpr int kDensUmSlot = 3;        // stats word: all masses of the last sph_density call are equal (its own gather kernel writes it)
 constexpr int kTileHalfSlot = 15;      // stats word: largest halo of half a 2x2x2 tile (three of its four z-layers of cells)
 inline uint32_t *sph_um_flag(const sph_ctx *ctx) { return ctx->stats.as<uint32_t>() + kUmSlot; }
 #ifdef __CUDACC__
@@ -355,7 +356,8 @@ __device__ __forceinline__ int cell_coord_raw(double x, double lo, double edge)
 
 // host-side launch helpers implemented in the .cu files
 int sph_tile_expand_col(sph_ctx *ctx, cudaStream_t st);   // tile-local lists -> 32-bit sorted ids in ctx->col
-int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, float *rho_out, cudaStream_t st);
+int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, float *rho_out, const uint32_t *um,
+                            const float *m_caller, cudaStream_t st);
 int sph_launch_density_vjp_tile(sph_ctx *ctx, const KPar &kp, const float2 *mr_s, float *x_bar, float *m_bar,
                                 cudaStream_t st);
 int sph_launch_grad_sum_tile(sph_ctx *ctx, const KPar &kp, const float *a_s, float *g_out, cudaStream_t st);

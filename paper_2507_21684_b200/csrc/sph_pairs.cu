@@ -139,6 +139,16 @@ __global__ void k_gather_f32(int64_t n, const uint32_t *__restrict__ perm, const
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p < n) out[p] = in[perm[p]];
 }
+// the same, and clears *um (preset to non-zero) when the values are not all equal to in[0]
+__global__ void k_gather_f32_um(int64_t n, const uint32_t *__restrict__ perm, const float *__restrict__ in,
+                                float *__restrict__ out, uint32_t *__restrict__ um)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const float first = __ldg(in), v = in[perm[p]];
+    out[p] = v;
+    if (v != first) *um = 0u;
+}
 __global__ void k_gather_f32_w(int64_t n, const uint32_t *__restrict__ perm, const float *__restrict__ in,
                                float4 *__restrict__ out)
 {
@@ -1247,8 +1257,18 @@ extern "C" int sph_density(sph_ctx *ctx, const float *m, float *rho_out, sph_str
     SPH_TRY(sph_kpar_make(ctx, &dummy, &kp));
     SPH_TRY(ctx->m_s.reserve((size_t)n * 4));
     KScope ks(ctx, SPH_K_DENSITY, 2, st);
+    if (ctx->tile_mode) {
+        // uniform-mass fast path (SPH_OPT_UNIFORM_MASS_PATH): the gather kernel leaves "all masses equal" in a device flag
+        uint32_t *um = ctx->opt_no_um ? nullptr : ctx->stats.as<uint32_t>() + kDensUmSlot;
+        if (um) {
+            SPH_CUDA_TRY(cudaMemsetAsync(um, 1, 4, st));
+            k_gather_f32_um<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), m, ctx->m_s.as<float>(), um);
+        } else {
+            k_gather_f32<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), m, ctx->m_s.as<float>());
+        }
+        return sph_launch_density_tile(ctx, kp, ctx->m_s.as<float>(), rho_out, um, m, st);
+    }
     k_gather_f32<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, ctx->perm.as<uint32_t>(), m, ctx->m_s.as<float>());
-    if (ctx->tile_mode) return sph_launch_density_tile(ctx, kp, ctx->m_s.as<float>(), rho_out, st);
     const float margin = seam_margin(ctx);
 #define SPH_DENS_LAUNCH(DIM, GS, VARH)                                                                               \
     k_density<DIM, GS, VARH><<<pair_grid(n, GS), kBlock, 0, st>>>(n, kp, margin, ctx->pos_s.as<float4>(),           \

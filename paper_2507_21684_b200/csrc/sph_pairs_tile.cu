@@ -326,20 +326,25 @@ struct SmemMap {
 
 // ------------------------------------------------------------------------------------------ D: density
 // smem: A = {x,y,z,h}[mcap], Ms = m[mcap] (in the B slot), rp, selfq, ring
-template <int DIM, int GS, bool VARH>
+// UM: all masses equal (device flag `um`, written by sph_density's own gather kernel: the launch whose turn it is not
+// returns at once, as in k_rhs_tile): the masses are neither staged nor gathered, rho_i = m_0 sum_j W_ij with m_0 = m[0]
+template <int DIM, int GS, bool VARH, bool UM>
 __global__ void __launch_bounds__(kPtMaxWarps * 32)
 k_density_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ pos_s, const float *__restrict__ m_s,
                const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
                const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16,
-               const uint32_t *__restrict__ perm, float *__restrict__ rho_out)
+               const uint32_t *__restrict__ perm, float *__restrict__ rho_out, const uint32_t *__restrict__ um,
+               const float *__restrict__ m_caller)
 {
+    if (um && (um[0] != 0u) != UM) return;
+    const float m0 = UM ? __ldg(m_caller) : 0.f;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const SmemMap<DIM> sm(smem_raw, ts, false, false, 4);     // 20 bytes per halo particle: three CTAs per SM at C3
+    const SmemMap<DIM> sm(smem_raw, ts, false, false, UM ? 0 : 4);     // 20 (16) bytes per halo particle: three CTAs per SM at C3
     float *Ms = reinterpret_cast<float *>(sm.B);
     __shared__ TileTab tt;
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
     if (tt.T == 0) return;
-    stage_halo(tt, pos_s, sm.A, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, m_s, Ms);
+    stage_halo(tt, pos_s, sm.A, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, UM ? nullptr : m_s, Ms);
     stage_rows(tt, row_ptr, sm.rp, sm.selfq);
     cp_async_wait<0>();
     __syncthreads();
@@ -366,10 +371,10 @@ k_density_tile(TileGeom tg, KPar kp, TileSizes ts, const float4 *__restrict__ po
                 const float t = fmaxf(1.0f - q, 0.f);
                 const float t2 = t * t, t6 = t2 * t2 * t2;
                 const float w = hc.cW * t6 * fmaf(q, fmaf(q, 35.0f / 3.0f, 6.0f), 1.0f);   // Eq.25/27
-                acc = fmaf(Ms[j], w, acc);
+                acc = UM ? acc + w : fmaf(Ms[j], w, acc);
             }
             acc = group_sum<GS>(acc);
-            if (gl == 0 && live) rho_out[perm[row0 + r]] = acc;
+            if (gl == 0 && live) rho_out[perm[row0 + r]] = UM ? m0 * acc : acc;
         });
 }
 
@@ -1186,33 +1191,46 @@ static void tile_launch_cfg(const sph_ctx *ctx, int state_bytes, int gs, size_t 
 #define SPH_TILE_SMEM_ATTR(KERNEL, SMEM) \
     SPH_CUDA_TRY(cudaFuncSetAttribute(KERNEL, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM)))
 
-int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, float *rho_out, cudaStream_t st)
+int sph_launch_density_tile(sph_ctx *ctx, const KPar &kp, const float *m_s, float *rho_out, const uint32_t *um,
+                            const float *m_caller, cudaStream_t st)
 {
+    // um: device flag "all masses equal" of this call (or NULL: general variant only); both variants are enqueued and the
+    // one whose turn it is not returns at once
     const TileGeom &tg = ctx->tg;
     const int gs = tile_group(ctx, false);
-    int threads;
-    TileSizes ts;
-    size_t smem;
-    tile_launch_cfg(ctx, 20, gs, sizeof(TileTab), kPtMaxWarps, 40, &threads, &ts, &smem);   // {x,y,z,h} + m per halo particle; every variant compiles to <= 40 registers
+    for (int pass = 0; pass < (um ? 2 : 1); ++pass) {
+        const bool UMv = um && pass == 0;
+        int threads;
+        TileSizes ts;
+        size_t smem;
+        // {x,y,z,h} (+ m) per halo particle; every variant compiles to <= 40 registers
+        tile_launch_cfg(ctx, UMv ? 16 : 20, gs, sizeof(TileTab), kPtMaxWarps, 40, &threads, &ts, &smem);
+        if (pass == 1) ctx->launches += 1;
+#define SPH_DT_LAUNCH2(DIM, GS, VARH, UM)                                                                             \
+    do {                                                                                                              \
+        SPH_TILE_SMEM_ATTR((k_density_tile<DIM, GS, VARH, UM>), smem);                                                \
+        k_density_tile<DIM, GS, VARH, UM><<<(unsigned)tg.ntiles, threads, smem, st>>>(                                \
+            tg, kp, ts, ctx->pos_s.as<float4>(), m_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),   \
+            ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), rho_out, um, m_caller); \
+    } while (0)
 #define SPH_DT_LAUNCH(DIM, GS, VARH)                                                                                  \
     do {                                                                                                              \
-        SPH_TILE_SMEM_ATTR((k_density_tile<DIM, GS, VARH>), smem);                                                    \
-        k_density_tile<DIM, GS, VARH><<<(unsigned)tg.ntiles, threads, smem, st>>>(                                    \
-            tg, kp, ts, ctx->pos_s.as<float4>(), m_s, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),   \
-            ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->perm.as<uint32_t>(), rho_out);              \
+        if (UMv) SPH_DT_LAUNCH2(DIM, GS, VARH, true); else SPH_DT_LAUNCH2(DIM, GS, VARH, false);                      \
     } while (0)
 #define SPH_DT_GS(GS)                                                                                     \
     do {                                                                                                  \
         if (kp.dim == 3) { if (kp.uniform_h) SPH_DT_LAUNCH(3, GS, false); else SPH_DT_LAUNCH(3, GS, true); } \
         else { if (kp.uniform_h) SPH_DT_LAUNCH(2, GS, false); else SPH_DT_LAUNCH(2, GS, true); }             \
     } while (0)
-    switch (gs) {
-    case 16: SPH_DT_GS(16); break;
-    case 32: SPH_DT_GS(32); break;
-    default: SPH_DT_GS(8); break;
-    }
+        switch (gs) {
+        case 16: SPH_DT_GS(16); break;
+        case 32: SPH_DT_GS(32); break;
+        default: SPH_DT_GS(8); break;
+        }
 #undef SPH_DT_GS
 #undef SPH_DT_LAUNCH
+#undef SPH_DT_LAUNCH2
+    }
     SPH_CUDA_TRY(cudaGetLastError());
     return SPH_OK;
 }

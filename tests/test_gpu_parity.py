@@ -413,6 +413,9 @@ def test_uniform_mass_variant_and_general_variant_agree(sph):
             try:
                 _, dev, _ = build(wl, 1.0, sph)
                 m_dev = torch.from_numpy(m).cuda()
+                # sph_density has its own flag (written by its gather kernel) and its own pair of variants
+                dens = sph.density(m_dev)
+                assert max_norm_err(_np(dens), oracle.density(wl.domain, wl.x, wl.h, m, *lists)) < TOL_FWD
                 drho, acc = sph.rhs(wl.params, dev.x, dev.v, dev.rho, m_dev, dev.kind)
                 _check_forward(f"C3p masses {variant}, uniform-mass path {um_path}", _np(drho), _np(acc), d_o, a_o, sd, sa, FLOOR)
                 xb, vb, rb, pb = sph.rhs_vjp(wl.params, dev.x, dev.v, dev.rho, m_dev, dev.kind, torch.from_numpy(lam).cuda(),
