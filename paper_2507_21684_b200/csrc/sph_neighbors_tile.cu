@@ -517,13 +517,26 @@ k_tile_tables(TileGeom tg, const uint32_t *__restrict__ cell_start, const uint32
 template <int DIM>
 __global__ void __launch_bounds__(256)
 k_expand_col16(TileGeom tg, const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ cell_end,
-               const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16, int32_t *__restrict__ col)
+               const long long *__restrict__ row_ptr, const uint16_t *__restrict__ col16, int32_t *__restrict__ col,
+               uint32_t mapcap)
 {
+    extern __shared__ uint32_t qmap[];                    // [mapcap] halo-linear index -> sorted index, when the halo fits
     __shared__ TileTab tt;
     tile_setup<DIM>(tg, blockIdx.x, cell_start, cell_end, tt);
     if (tt.T == 0) return;
     const long long b = row_ptr[tt.row0], e = row_ptr[tt.row0 + tt.T];
-    for (long long p = b + threadIdx.x; p < e; p += blockDim.x) col[p] = (int32_t)tile_q_to_sorted(tt, col16[p]);
+    if (tt.M <= mapcap) {
+        // one table look-up per entry instead of a binary search over the halo cells
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+        for (int hc = warp; hc < tt.nh; hc += nwarps) {
+            const uint32_t o0 = tt.h_off[hc], cnt = tt.h_off[hc + 1] - o0, gs = tt.h_start[hc];
+            for (uint32_t l = lane; l < cnt; l += 32) qmap[o0 + l] = gs + l;
+        }
+        __syncthreads();
+        for (long long p = b + threadIdx.x; p < e; p += blockDim.x) col[p] = (int32_t)qmap[col16[p]];
+    } else {
+        for (long long p = b + threadIdx.x; p < e; p += blockDim.x) col[p] = (int32_t)tile_q_to_sorted(tt, col16[p]);
+    }
 }
 
 } // namespace
@@ -752,12 +765,14 @@ int sph_tile_expand_col(sph_ctx *ctx, cudaStream_t st)
     SPH_TRY(ctx->col.reserve((size_t)(ctx->nnz > 0 ? ctx->nnz : 1) * 4));
     KScope ks(ctx, SPH_K_EXPORT, 1, st);
     const TileGeom &tg = ctx->tg;
+    const uint32_t mapcap = ctx->tile_Mmax <= 11000u ? ctx->tile_Mmax : 0u;     // 44 KB of dynamic shared memory at most
+    const size_t smem = (size_t)mapcap * 4;
     if (tg.dim == 3)
-        k_expand_col16<3><<<(unsigned)tg.ntiles, 256, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),
-                                                              ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->col.as<int32_t>());
+        k_expand_col16<3><<<(unsigned)tg.ntiles, 256, smem, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),
+                                                                 ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->col.as<int32_t>(), mapcap);
     else
-        k_expand_col16<2><<<(unsigned)tg.ntiles, 256, 0, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),
-                                                              ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->col.as<int32_t>());
+        k_expand_col16<2><<<(unsigned)tg.ntiles, 256, smem, st>>>(tg, ctx->cell_start.as<uint32_t>(), ctx->cell_end.as<uint32_t>(),
+                                                                 ctx->row_ptr.as<long long>(), ctx->col16.as<uint16_t>(), ctx->col.as<int32_t>(), mapcap);
     SPH_CUDA_TRY(cudaGetLastError());
     ctx->col_valid = true;
     return SPH_OK;
