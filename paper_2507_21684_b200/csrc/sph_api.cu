@@ -45,6 +45,7 @@ extern "C" int sph_destroy(sph_ctx *ctx)
     if (ctx->ev_out) cudaEventDestroy(ctx->ev_out);
     for (int c = 0; c < 4; ++c)
         if (ctx->ev_final[c]) cudaEventDestroy(ctx->ev_final[c]);
+    if (ctx->ev_final_x) cudaEventDestroy(ctx->ev_final_x);
     for (const ProfRec &r : ctx->prof.live) {
         cudaEventDestroy(r.a);
         cudaEventDestroy(r.b);
@@ -230,6 +231,7 @@ extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_doma
     constexpr int kFinalChunks = 4;
     for (int c = 0; c < kFinalChunks; ++c)
         if (!ctx->ev_final[c]) SPH_CUDA_TRY(cudaEventCreateWithFlags(&ctx->ev_final[c], cudaEventDisableTiming));
+    if (!ctx->ev_final_x) SPH_CUDA_TRY(cudaEventCreateWithFlags(&ctx->ev_final_x, cudaEventDisableTiming));
     ctx->rk_final_chunks = kFinalChunks;
     const int rc_rk = sph_rk_step(ctx, dom_rk, par, dt, skin, n, dx, dv, dr, dm, dh, dk, ss);
     SPH_TRY(rc_rk);
@@ -237,12 +239,14 @@ extern "C" int sph_step_host(sph_ctx *ctx, const sph_domain *dom, const sph_doma
         nnz_out[0] = nnz0;
         nnz_out[1] = ctx->nnz;
     }
+    // the new positions were complete before the last right-hand side started: they leave while it runs
+    SPH_CUDA_TRY(cudaStreamWaitEvent(cs, ctx->ev_final_x, 0));
+    SPH_CUDA_TRY(cudaMemcpyAsync(x, dx, nv, cudaMemcpyDeviceToHost, cs));
     for (int c = 0; c < kFinalChunks; ++c) {
         const int64_t i0 = n * c / kFinalChunks, i1 = n * (c + 1) / kFinalChunks;
         SPH_CUDA_TRY(cudaStreamWaitEvent(cs, ctx->ev_final[c], 0));
         if (i1 <= i0) continue;
         const size_t ov = (size_t)i0 * dom->dim, cv = (size_t)(i1 - i0) * dom->dim * 4, cs1 = (size_t)(i1 - i0) * 4;
-        SPH_CUDA_TRY(cudaMemcpyAsync(x + ov, dx + ov, cv, cudaMemcpyDeviceToHost, cs));
         SPH_CUDA_TRY(cudaMemcpyAsync(v + ov, dv + ov, cv, cudaMemcpyDeviceToHost, cs));
         SPH_CUDA_TRY(cudaMemcpyAsync(rho + i0, dr + i0, cs1, cudaMemcpyDeviceToHost, cs));
     }

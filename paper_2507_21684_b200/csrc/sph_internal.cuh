@@ -198,6 +198,7 @@ struct sph_ctx {
     int rk_final_chunks = 1;
     bool rk_lists_prepared = false;  // sph_step_host has already run sph_rk_prepare_lists for the coming sph_rk_step
     cudaEvent_t ev_final[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev_final_x = nullptr;     // sph_step_host: the advanced positions are complete (before the last RHS)
     // host staging for *_host call
     DevBuf hx, hv, hrho, hm, hh, hkind, hlam, hmu, ho_drho, ho_acc, ho_xb, ho_vb, ho_rb, ho_pb, ho_dens;
 };

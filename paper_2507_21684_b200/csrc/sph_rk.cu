@@ -147,8 +147,11 @@ __global__ void k_rk_final(int64_t n, float dt, float blast, const uint32_t *__r
     rho[i] = fmaf(dt, fmaf(blast, k.w, ax.w), rho[i]);
 }
 
-// the same update for the caller indices [i0, i1) (one thread per caller index, gathers through inv_perm)
-template <int DIM>
+// the same update for the caller indices [i0, i1) (one thread per caller index, gathers through inv_perm).
+// WHAT: 1 = positions only, 2 = velocities and densities only, 3 = all.  The new positions need the velocities of the
+// LAST stage state, not the last right-hand side, so sph_step_host has them computed (and copied out) while the fourth
+// right-hand side still runs.
+template <int DIM, int WHAT>
 __global__ void k_rk_final_range(int64_t i0, int64_t i1, float dt, float blast, const uint32_t *__restrict__ inv_perm,
                                  const uint8_t *__restrict__ kind_s, const float4 *__restrict__ k4, StageBufs last,
                                  const float4 *__restrict__ accx, const float4 *__restrict__ accv, float *__restrict__ x,
@@ -157,20 +160,24 @@ __global__ void k_rk_final_range(int64_t i0, int64_t i1, float dt, float blast, 
     const int64_t i = i0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= i1) return;
     const int64_t p = inv_perm[i];
-    const float4 k = k4[p];
-    float vp[3];
-    if (DIM == 3) { const float4 t = last.s1[p]; vp[0] = t.x; vp[1] = t.y; vp[2] = t.z; }
-    else { const float4 t = last.s0[p]; vp[0] = t.z; vp[1] = t.w; vp[2] = 0.f; }
-    if (kind_s[p]) vp[0] = vp[1] = vp[2] = 0.f;
-    const float4 ax = accx[p], av = accv[p];
-    const float dx[3] = {fmaf(blast, vp[0], ax.x), fmaf(blast, vp[1], ax.y), fmaf(blast, vp[2], ax.z)};
-    const float dv[3] = {fmaf(blast, k.x, av.x), fmaf(blast, k.y, av.y), fmaf(blast, k.z, av.z)};
+    const float4 ax = accx[p];
+    if (WHAT & 1) {
+        float vp[3];
+        if (DIM == 3) { const float4 t = last.s1[p]; vp[0] = t.x; vp[1] = t.y; vp[2] = t.z; }
+        else { const float4 t = last.s0[p]; vp[0] = t.z; vp[1] = t.w; vp[2] = 0.f; }
+        if (kind_s[p]) vp[0] = vp[1] = vp[2] = 0.f;
+        const float dx[3] = {fmaf(blast, vp[0], ax.x), fmaf(blast, vp[1], ax.y), fmaf(blast, vp[2], ax.z)};
 #pragma unroll
-    for (int kk = 0; kk < DIM; ++kk) {
-        x[i * DIM + kk] = fmaf(dt, dx[kk], x[i * DIM + kk]);
-        v[i * DIM + kk] = fmaf(dt, dv[kk], v[i * DIM + kk]);
+        for (int kk = 0; kk < DIM; ++kk) x[i * DIM + kk] = fmaf(dt, dx[kk], x[i * DIM + kk]);
     }
-    rho[i] = fmaf(dt, fmaf(blast, k.w, ax.w), rho[i]);
+    if (WHAT & 2) {
+        const float4 k = k4[p];
+        const float4 av = accv[p];
+        const float dv[3] = {fmaf(blast, k.x, av.x), fmaf(blast, k.y, av.y), fmaf(blast, k.z, av.z)};
+#pragma unroll
+        for (int kk = 0; kk < DIM; ++kk) v[i * DIM + kk] = fmaf(dt, dv[kk], v[i * DIM + kk]);
+        rho[i] = fmaf(dt, fmaf(blast, k.w, ax.w), rho[i]);
+    }
 }
 
 // ---- adjoint helpers ---------------------------------------------------------------------------------
@@ -331,6 +338,17 @@ extern "C" int sph_rk_step(sph_ctx *ctx, const sph_domain *dom, const sph_params
             else
                 k_rk_stage<2><<<nb(n), 256, 0, st>>>(n, kp, c[s] * dt, b[s - 1], s == 1, b0, b1, m_s, kind_s, k4, sb, sb, accx, accv);
         }
+        if (s == 3 && ctx->rk_final_chunks > 1) {
+            // sph_step_host: the new positions are complete before the last right-hand side (they need v of this stage
+            // state only); the caller copies them out while it runs
+            KScope ks(ctx, SPH_K_RK, 1, st);
+            const uint32_t *inv_perm = ctx->inv_perm.as<uint32_t>();
+            if (kp.dim == 3)
+                k_rk_final_range<3, 1><<<nb(n), 256, 0, st>>>(0, n, dt, b[3], inv_perm, kind_s, k4, sb, accx, accv, x, v, rho);
+            else
+                k_rk_final_range<2, 1><<<nb(n), 256, 0, st>>>(0, n, dt, b[3], inv_perm, kind_s, k4, sb, accx, accv, x, v, rho);
+            SPH_CUDA_TRY(cudaEventRecord(ctx->ev_final_x, st));
+        }
         SPH_TRY(sph_launch_rhs_sorted(ctx, kp, sb.s0, sb.s1, sb.s2, kind_s, nullptr, nullptr, k4, st));
     }
     if (ctx->rk_final_chunks > 1) {
@@ -342,9 +360,9 @@ extern "C" int sph_rk_step(sph_ctx *ctx, const sph_domain *dom, const sph_params
             if (i1 > i0) {
                 KScope ks(ctx, SPH_K_RK, 1, st);
                 if (kp.dim == 3)
-                    k_rk_final_range<3><<<nb(i1 - i0), 256, 0, st>>>(i0, i1, dt, b[3], inv_perm, kind_s, k4, sb, accx, accv, x, v, rho);
+                    k_rk_final_range<3, 2><<<nb(i1 - i0), 256, 0, st>>>(i0, i1, dt, b[3], inv_perm, kind_s, k4, sb, accx, accv, x, v, rho);
                 else
-                    k_rk_final_range<2><<<nb(i1 - i0), 256, 0, st>>>(i0, i1, dt, b[3], inv_perm, kind_s, k4, sb, accx, accv, x, v, rho);
+                    k_rk_final_range<2, 2><<<nb(i1 - i0), 256, 0, st>>>(i0, i1, dt, b[3], inv_perm, kind_s, k4, sb, accx, accv, x, v, rho);
             }
             SPH_CUDA_TRY(cudaEventRecord(ctx->ev_final[cI], st));
         }
